@@ -1,0 +1,245 @@
+"""Seeded synthetic workloads (inputs only) for the hydrostatic free-surface time step.
+
+This module is the ONE piece shared by the CUDA path and the CPU oracle: it draws the
+seeded inputs (grids, bathymetry, initial fields, wind stress) for the five configurations
+of BASELINE.json and holds none of the method's arithmetic (no stencils, no scans, no
+solves, no masks).  It imports numpy only.
+
+The shapes stand in for the paper's workloads (§6: near-global
+75S-75N latitude-longitude domains, periodic in longitude, 48-100 stretched levels,
+realistic bathymetry) whose data (ECCO2 forcing, real bathymetry) are not
+available here.  Recipes follow SURVEY.md §8(d) and are restated in DESIGN.md §4.
+
+Every workload is a plain dict:
+
+    grid   : dict(kind, nx, ny, nz, periodic_x, periodic_y, x0, dx, y0, dy, radius,
+                  rotation_rate, f0, beta)
+    z_faces: float64[nz+1], increasing, z_faces[nz] == 0
+    depth  : float64[ny, nx]  bottom depth in metres (>= 0, 0 = land)
+    params : dict(precision, dt, substeps, chi, g, alpha, beta_s, T0, S0, rho0,
+                  nu_h, kappa_h, nu_z, kappa_z)
+    fields : dict(u, v, T, S [nz,ny,nx]; eta, tau_x, tau_y [ny,nx])  float64, already
+             rounded to the run precision (the fp64 oracle receives the rounded values)
+    steps  : number of baroclinic steps the configuration asks for
+    name   : label
+"""
+from __future__ import annotations
+
+import numpy as np
+
+SEED_BASE = 6662
+
+EARTH_RADIUS = 6371000.0
+EARTH_ROTATION = 7.292115e-5
+GRAVITY = 9.80665
+
+
+def _params(precision, dt, substeps, nu_h, kappa_h, beta_s=8e-4):
+    return dict(precision=int(precision), dt=float(dt), substeps=int(substeps), chi=0.1,
+                g=GRAVITY, alpha=2e-4, beta_s=float(beta_s), T0=10.0, S0=35.0, rho0=1025.0,
+                nu_h=float(nu_h), kappa_h=float(kappa_h), nu_z=1e-4, kappa_z=1e-5)
+
+
+def _round_to(precision, a):
+    a = np.asarray(a, dtype=np.float64)
+    if precision == 32:
+        return a.astype(np.float32).astype(np.float64)
+    return a
+
+
+def geometric_z_faces(nz, top_dz, total_depth):
+    """nz layers whose thickness grows geometrically downward from top_dz at the surface and
+    sums to total_depth (the ratio is solved for, so the sum is exact)."""
+    if abs(nz * top_dz - total_depth) < 1e-9 * total_depth:
+        dz = np.full(nz, top_dz)
+    else:
+        lo, hi = 1.0 + 1e-12, 4.0
+        for _ in range(200):
+            r = 0.5 * (lo + hi)
+            s = top_dz * (r ** nz - 1.0) / (r - 1.0)
+            if s < total_depth:
+                lo = r
+            else:
+                hi = r
+        r = 0.5 * (lo + hi)
+        dz = top_dz * r ** np.arange(nz)          # index 0 = surface layer
+    zf = np.zeros(nz + 1)
+    zf[:nz] = -np.cumsum(dz)[::-1]                # zf[0] = -total, zf[nz] = 0
+    zf[0] = -float(total_depth)
+    zf[nz] = 0.0
+    return zf
+
+
+def _z_centres(zf):
+    return 0.5 * (zf[:-1] + zf[1:])
+
+
+def _low_mode_field(rng, ny, nx, nmodes, periodic=True):
+    """Smooth random 2-D field: sum over wavenumbers 1..nmodes per axis of cosines with seeded
+    amplitude and phase.  Returns values on cell centres, normalised to max |.| = 1."""
+    y = (np.arange(ny) + 0.5) / ny
+    x = (np.arange(nx) + 0.5) / nx
+    f = np.zeros((ny, nx))
+    for ky in range(1, nmodes + 1):
+        for kx in range(1, nmodes + 1):
+            a = rng.standard_normal()
+            px, py = rng.uniform(0, 2 * np.pi, size=2)
+            f += a * np.cos(2 * np.pi * kx * x[None, :] + px) * np.cos(2 * np.pi * ky * y[:, None] + py)
+    return f / np.max(np.abs(f))
+
+
+def fractal_field(rng, ny, nx, slope=-2.0):
+    """Seeded Gaussian noise filtered in Fourier space to a power spectrum ~ K^slope
+    (K = horizontal wavenumber magnitude in index space; doubly periodic FFT)."""
+    noise = rng.standard_normal((ny, nx))
+    fk = np.fft.rfft2(noise)
+    ky = np.fft.fftfreq(ny)[:, None] * ny
+    kx = np.fft.rfftfreq(nx)[None, :] * nx
+    K = np.sqrt(kx * kx + ky * ky)
+    K[0, 0] = 1.0
+    fk *= K ** (0.5 * slope)
+    fk[0, 0] = 0.0
+    out = np.fft.irfft2(fk, s=(ny, nx))
+    return out / out.std()
+
+
+# ------------------------------------------------------------------------------------------
+# config 0: doubly periodic f-plane box
+# ------------------------------------------------------------------------------------------
+def config0(nx=32, ny=32, nz=8, steps=10, seed=SEED_BASE + 0):
+    rng = np.random.default_rng(np.random.PCG64(seed))
+    Hd = 400.0
+    zf = geometric_z_faces(nz, Hd / nz, Hd)
+    zc = _z_centres(zf)
+    grid = dict(kind=0, nx=nx, ny=ny, nz=nz, periodic_x=1, periodic_y=1, x0=0.0, dx=1000.0,
+                y0=0.0, dy=1000.0, radius=EARTH_RADIUS, rotation_rate=EARTH_ROTATION,
+                f0=1e-4, beta=0.0)
+    depth = np.full((ny, nx), Hd)
+    T = 10.0 + 0.02 * (zc[:, None, None] + Hd) + 0.01 * rng.standard_normal((nz, ny, nx))
+    S = np.full((nz, ny, nx), 35.0)
+    prof = 0.5 * (1.0 + np.cos(np.pi * zc / Hd))
+    u2 = _low_mode_field(rng, ny, nx, 4)
+    v2 = _low_mode_field(rng, ny, nx, 4)
+    u = 0.1 * u2[None] * prof[:, None, None]
+    v = 0.1 * v2[None] * prof[:, None, None]
+    z2 = np.zeros((ny, nx))
+    fields = dict(u=u, v=v, T=T, S=S, eta=z2.copy(), tau_x=z2.copy(), tau_y=z2.copy())
+    params = _params(64, 60.0, 20, 10.0, 1.0, beta_s=0.0)
+    return dict(name="cfg0_fplane_box", grid=grid, z_faces=zf, depth=depth, params=params,
+                fields={k: _round_to(64, a) for k, a in fields.items()}, steps=steps)
+
+
+# ------------------------------------------------------------------------------------------
+# config 1: closed beta-plane basin with smooth bathymetry and zonal wind
+# ------------------------------------------------------------------------------------------
+def config1(nx=256, ny=256, nz=32, steps=100, seed=SEED_BASE + 1):
+    rng = np.random.default_rng(np.random.PCG64(seed))
+    Hd = 4000.0
+    zf = geometric_z_faces(nz, 10.0, Hd)
+    zc = _z_centres(zf)
+    dx = 5000.0 * 256.0 / nx
+    grid = dict(kind=0, nx=nx, ny=ny, nz=nz, periodic_x=0, periodic_y=0, x0=0.0, dx=dx,
+                y0=0.0, dy=dx, radius=EARTH_RADIUS, rotation_rate=EARTH_ROTATION,
+                f0=1e-4, beta=2e-11)
+    bump = _low_mode_field(rng, ny, nx, 2)                    # 4 low seeded modes
+    depth = 3000.0 + 1000.0 * bump                            # 2-4 km
+    depth[0, :] = depth[-1, :] = 0.0                          # outer ring of land cells
+    depth[:, 0] = depth[:, -1] = 0.0
+    T = np.broadcast_to((2.0 + 18.0 * np.exp(zc / 800.0))[:, None, None], (nz, ny, nx)).copy()
+    S = np.broadcast_to((35.0 - np.exp(zc / 500.0))[:, None, None], (nz, ny, nx)).copy()
+    yc = (np.arange(ny) + 0.5) / ny
+    tau_x = np.broadcast_to((0.1 * np.cos(np.pi * yc))[:, None], (ny, nx)).copy()
+    z3 = np.zeros((nz, ny, nx))
+    z2 = np.zeros((ny, nx))
+    fields = dict(u=z3.copy(), v=z3.copy(), T=T, S=S, eta=z2.copy(), tau_x=tau_x, tau_y=z2.copy())
+    params = _params(64, 300.0, 30, 100.0, 10.0)
+    return dict(name="cfg1_double_gyre", grid=grid, z_faces=zf, depth=depth, params=params,
+                fields={k: _round_to(64, a) for k, a in fields.items()}, steps=steps)
+
+
+# ------------------------------------------------------------------------------------------
+# configs 2-4: near-global latitude-longitude grids with fractal immersed bathymetry
+# ------------------------------------------------------------------------------------------
+def latlon_bathymetry(rng, ny, nx, max_depth=6000.0, land_fraction=0.30):
+    F = fractal_field(rng, ny, nx, slope=-2.0)
+    q_land = np.quantile(F, land_fraction)
+    q_hi = np.quantile(F, 0.99)
+    depth = np.clip(max_depth * (F - q_land) / (q_hi - q_land), 50.0, max_depth)
+    depth[F < q_land] = 0.0
+    return depth
+
+
+def latlon(nx, ny, nz, *, dt, substeps, steps, nu_h, kappa_h, precision, seed, name,
+           noise=True, lat0=-75.0, lat1=75.0, window=None):
+    """Near-global lat-lon workload.  `window=(j0, j1, i0, i1)` cuts a sub-window out of the
+    full-size fields (identical values) and turns it into a closed box: not periodic, and the
+    bathymetry is used as is (the library treats non-periodic edges as land)."""
+    rng = np.random.default_rng(np.random.PCG64(seed))
+    dlat = (lat1 - lat0) / ny
+    dlon = 360.0 / nx
+    zf = geometric_z_faces(nz, 10.0, 6000.0)
+    zc = _z_centres(zf)
+    depth = latlon_bathymetry(rng, ny, nx)
+    latc = np.deg2rad(lat0 + (np.arange(ny) + 0.5) * dlat)
+    # wind stress: zonal 0.1*cos(3*lat) plus seeded low modes (periodic in longitude)
+    tx_modes = _low_mode_field(rng, ny, nx, 3)
+    ty_modes = _low_mode_field(rng, ny, nx, 3)
+    tau_x = 0.1 * np.cos(3.0 * latc)[:, None] + 0.02 * tx_modes
+    tau_y = 0.02 * ty_modes
+
+    if window is None:
+        j0, j1, i0, i1 = 0, ny, 0, nx
+    else:
+        j0, j1, i0, i1 = window
+    wny, wnx = j1 - j0, i1 - i0
+    cos2 = (np.cos(latc[j0:j1]) ** 2)[:, None]
+    cos2lat = np.cos(2.0 * latc[j0:j1])[:, None]
+    T = np.empty((nz, wny, wnx))
+    S = np.empty((nz, wny, wnx))
+    for k in range(nz):                       # level by level: full-size noise, keep the window
+        Tk = 2.0 + 25.0 * cos2 * np.exp(zc[k] / 800.0)
+        Sk = 35.0 - cos2lat * np.exp(zc[k] / 500.0)
+        if noise:
+            nT = rng.standard_normal((ny, nx), dtype=np.float32)[j0:j1, i0:i1]
+            nS = rng.standard_normal((ny, nx), dtype=np.float32)[j0:j1, i0:i1]
+            T[k] = Tk + 0.01 * nT
+            S[k] = Sk + 0.001 * nS
+        else:
+            T[k] = Tk
+            S[k] = Sk
+    grid = dict(kind=1, nx=wnx, ny=wny, nz=nz, periodic_x=1 if window is None else 0,
+                periodic_y=0, x0=i0 * dlon, dx=dlon, y0=lat0 + j0 * dlat, dy=dlat,
+                radius=EARTH_RADIUS, rotation_rate=EARTH_ROTATION, f0=0.0, beta=0.0)
+    z3 = np.zeros((nz, wny, wnx))
+    fields = dict(u=z3, v=z3.copy(), T=T, S=S, eta=np.zeros((wny, wnx)),
+                  tau_x=tau_x[j0:j1, i0:i1].copy(), tau_y=tau_y[j0:j1, i0:i1].copy())
+    params = _params(precision, dt, substeps, nu_h, kappa_h)
+    return dict(name=name, grid=grid, z_faces=zf, depth=depth[j0:j1, i0:i1].copy(), params=params,
+                fields={k: _round_to(precision, a) for k, a in fields.items()}, steps=steps)
+
+
+def config2(nx=1440, ny=600, nz=50, steps=50, precision=64, seed=SEED_BASE + 2, window=None):
+    scale = 1440.0 / nx       # reduced-resolution analogues: dt ~ resolution, capped at 1200 s (f dt < 0.2)
+    return latlon(nx, ny, nz, dt=min(540.0 * scale, 1200.0), substeps=30, steps=steps, nu_h=1000.0 * scale,
+                  kappa_h=100.0 * scale, precision=precision, seed=seed,
+                  name="cfg2_latlon_quarter_deg" if precision == 64 else "cfg3_latlon_quarter_deg_fp32",
+                  window=window)
+
+
+def config3(nx=1440, ny=600, nz=50, steps=50, window=None):
+    # "same grid and seeded fields as config 2" -> config 2's seed, values rounded to fp32
+    return config2(nx, ny, nz, steps, precision=32, seed=SEED_BASE + 2, window=window)
+
+
+def config4(nx=2880, ny=1200, nz=100, steps=20, seed=SEED_BASE + 4, window=None, precision=32):
+    scale = 2880.0 / nx
+    return latlon(nx, ny, nz, dt=min(270.0 * scale, 1200.0), substeps=40, steps=steps, nu_h=500.0 * scale,
+                  kappa_h=50.0 * scale, precision=precision, seed=seed,
+                  name="cfg4_latlon_eighth_deg_fp32", window=window)
+
+
+CONFIGS = {0: config0, 1: config1, 2: config2, 3: config3, 4: config4}
+
+
+def make(config, **kw):
+    return CONFIGS[int(config)](**kw)
