@@ -1,0 +1,114 @@
+/* ocn.h — C ABI of libocn: the B200-native (sm_100a) hydrostatic free-surface time step.
+ *
+ * One call of ocn_time_step(model, n) advances the hydrostatic Boussinesq equations on a
+ * staggered C-grid (§5.2) by n baroclinic steps: fused WENO-upwind tendency
+ * kernels, quasi-AB2 + backward-Euler vertical diffusion by a tridiagonal
+ * solve, the split-explicit barotropic sub-cycle, the barotropic
+ * correction and the column diagnostics.  Every step of that path runs in CUDA kernels of this
+ * library; there is no CPU fallback.  The discrete equations are fixed in DESIGN.md §3.
+ *
+ * Conventions
+ *   - Field buffers crossing the ABI are `precision`-bit floats (32 or 64), INTERIOR cells only,
+ *     layout [k][j][i] with i (longitude / x) fastest and k = 0 the bottom layer.  u is stored on
+ *     the west face of cell i, v on the south face of cell j, w on the bottom face of cell k
+ *     (nz+1 levels).  eta, tau_x (at u points), tau_y (at v points) are [j][i].
+ *   - Handles and all device memory are owned by the library.  I/O buffers are owned by the
+ *     caller and never retained.  A grid must outlive the models created from it.
+ *   - Every call returns ocn_status and never throws; ocn_last_error() gives the message of the
+ *     last non-OK status on the calling thread.  Asynchronous CUDA faults surface at the next
+ *     ocn_get_fields / ocn_synchronize.
+ */
+#ifndef OCN_H
+#define OCN_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ocn_grid ocn_grid;
+typedef struct ocn_model ocn_model;
+
+typedef enum {
+    OCN_OK = 0, OCN_EINVAL = 1, OCN_ENOMEM = 2, OCN_ECUDA = 3, OCN_ESTATE = 4, OCN_EUNSUPPORTED = 5
+} ocn_status;
+
+/* Horizontal grid (lat-lon domain of PAPER.md:102). */
+typedef struct {
+    int kind;                       /* 0 cartesian (f/beta-plane), 1 latitude-longitude */
+    int nx, ny, nz;                 /* nx, ny >= 3; 2 <= nz <= 250 */
+    int periodic_x, periodic_y;     /* non-periodic edges are solid walls (land halo) */
+    double x0, dx;                  /* metres, or degrees longitude (uniform) */
+    double y0, dy;                  /* metres, or degrees latitude  (uniform) */
+    double radius, rotation_rate;   /* lat-lon: sphere radius [m], Omega [1/s] */
+    double f0, beta;                /* cartesian: f = f0 + beta (y - y_mid) */
+} ocn_grid_desc;
+
+/* z_faces: HOST, nz+1 doubles, increasing, z_faces[nz] = 0 (surface).
+ * bottom_depth: HOST, ny*nx doubles, metres >= 0, 0 = land.  Immersed boundary = full cells,
+ * cell wet iff its centre lies above the bottom; columns with < 2 wet cells are land
+ * (DESIGN.md §3.3).  Host-only: allocates nothing on the device. */
+ocn_status ocn_grid_create(const ocn_grid_desc* desc, const double* z_faces, const double* bottom_depth,
+                           ocn_grid** out);
+ocn_status ocn_grid_destroy(ocn_grid* grid);
+
+/* Model parameters. */
+typedef struct {
+    int precision;                  /* 32 or 64: dtype of every field buffer crossing the ABI and
+                                       of all device fields, tendencies and metrics */
+    double dt;                      /* baroclinic time step [s] */
+    int substeps;                   /* barotropic sub-steps M per baroclinic step */
+    double chi;                     /* quasi-AB2 offset (0.1) */
+    double g, alpha, beta_s, T0, S0, rho0;      /* linear equation of state, reference density */
+    double nu_h, kappa_h, nu_z, kappa_z;        /* constant viscosities / diffusivities [m^2/s] */
+    const double* filter_weights;   /* HOST, `substeps` doubles a_1..a_M, or NULL = power-law
+                                       default of DESIGN.md §3.9; copied at creation */
+    int device;                     /* CUDA device ordinal */
+    void* stream;                   /* cudaStream_t of the caller (e.g. torch's), NULL = default */
+} ocn_model_desc;
+
+/* Allocates all device state (13 3-D arrays + 2-D arrays + tables) on `device`. */
+ocn_status ocn_model_create(const ocn_grid* grid, const ocn_model_desc* desc, ocn_model** out);
+ocn_status ocn_model_destroy(ocn_model* model);
+
+/* Field set.  NULL member = skip.  on_device = 0: HOST pointers; 1: DEVICE pointers on the
+ * model's device (contiguous, same layout). */
+typedef struct {
+    void *u, *v, *T, *S;            /* nz*ny*nx */
+    void *w;                        /* (nz+1)*ny*nx, get only */
+    void *eta;                      /* ny*nx */
+    void *tau_x, *tau_y;            /* ny*nx, N/m^2, set only */
+    int on_device;
+} ocn_fields;
+
+/* Copies fields in (masking closed faces / land), on the model's stream.  If any of u, v, T, S,
+ * eta is given: re-derives U, V = sum(u dz), w, and resets the AB2 history (the next step is an
+ * Euler step).  Setting only tau_x / tau_y keeps the history (per-step forcing update). */
+ocn_status ocn_set_fields(ocn_model* model, const ocn_fields* fields);
+/* Enqueues n baroclinic steps on the stream; no host synchronisation. */
+ocn_status ocn_time_step(ocn_model* model, int n);
+/* Copies fields out (land / closed faces = 0) and synchronises the stream. */
+ocn_status ocn_get_fields(ocn_model* model, ocn_fields* fields);
+ocn_status ocn_synchronize(ocn_model* model);
+
+/* Expanded 3-D integer masks for the bit-exact test (HOST buffers, NULL = skip): wet, order_x,
+ * order_y, order_zeta_u, order_zeta_v: nz*ny*nx; order_z: (nz+1)*ny*nx.  Expanded on the host
+ * from the same compact 2-D threshold maps the kernels read. */
+ocn_status ocn_get_masks(const ocn_grid* grid, unsigned char* wet, unsigned char* order_x,
+                         unsigned char* order_y, unsigned char* order_z,
+                         unsigned char* order_zeta_u, unsigned char* order_zeta_v);
+
+/* Number of kernel launches enqueued by one baroclinic step, and device bytes held by the model. */
+ocn_status ocn_model_info(const ocn_model* model, int* launches_per_step, unsigned long long* device_bytes);
+
+/* Debug / parity hooks (HOST double buffers, NULL = skip): the AB2 history G^{n-1} of each
+ * prognostic field (nz*ny*nx each) and the barotropic transports U, V (ny*nx). */
+ocn_status ocn_get_debug(ocn_model* model, double* Gu, double* Gv, double* GT, double* GS,
+                         double* U, double* V);
+
+const char* ocn_last_error(void);
+const char* ocn_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,115 @@
+// common.cuh — device-side parameter block, memory layout and small device helpers of libocn.
+//
+// Layout: every 3-D field is [k][j][i] with i fastest, a physical halo of 3
+// cells in i and j, row pitch sx = roundup(nx + 6, 32) elements, and the base pointer shifted so
+// that element (k, j, i = 0) of every row starts a 128-byte line.  2-D fields use the same
+// plane layout (one level).  Halos of periodic directions mirror the interior (written by the
+// producing kernel through store_halo); halos of bounded directions are zero forever (solid wall).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define OCN_HALO 3
+
+namespace ocn {
+
+template <class T>
+struct DevP {
+    int nx, ny, nz;
+    int sx, sy;            // plane pitch / rows (with halo)
+    long long sz;          // level stride = sx * sy
+    int px, py;            // periodic flags
+    // prognostic state (time level n), w diagnostic, forward-eliminated right-hand sides, AB2 history
+    T *u, *v, *t, *s, *w;
+    T *du, *dv, *dt_, *ds;
+    T *Gu, *Gv, *Gt, *Gs;
+    // 2-D (plane layout with halo)
+    T *eta[2], *U[2], *V[2];       // barotropic state, double buffered inside the sub-cycle
+    T *etab, *Ub, *Vb;             // weighted running averages
+    T *GU, *GV;                    // barotropic forcing
+    T *SU, *SV;                    // sum_k dz u*, sum_k dz v*
+    T *Hu, *Hv, *rHu, *rHv;        // depth at u / v points and reciprocals (0 on closed columns)
+    T *taux, *tauy;
+    // compact masks (plane layout with halo): thresholds in level index
+    const uint2* m8;               // bytes: kb, tx1, tx2, tx3 | ty1, ty2, ty3, 0
+    const uchar4* mz;              // zu2, zu3, zv2, zv3
+    // horizontal metrics per row, index j + OCN_HALO, rows -3 .. ny+3
+    const T *dxC, *dxF, *AzC, *AzF, *fF, *rdxC, *rdxF, *rAzC, *rAzF;
+    T dy, rdy;
+    // vertical grid
+    const T *dz, *rdz, *dzc;       // dzc[k] = zc[k] - zc[k-1] (k >= 1)
+    T hz_top;                      // zf[nz] - zc[nz-1]
+    // top-down Thomas tables: momentum (nu_z) and tracers (kappa_z)
+    const T *sp_m, *e_m, *im_m, *imb_m;
+    const T *sp_t, *e_t, *im_t, *imb_t;
+    // physics
+    T dt, g, alpha, beta_s, T0, S0, rrho0, nu_h, kappa_h;
+    T dtau;
+};
+
+template <class T>
+__device__ __forceinline__ T ldg(const T* p) { return __ldg(p); }
+
+// store a value and its periodic halo images (up to 3 extra copies)
+template <class T>
+__device__ __forceinline__ void store_halo(T* __restrict__ plane, int sx, int nx, int ny, int px, int py,
+                                           int j, int i, T val) {
+    T* p = plane + (long long)(j + OCN_HALO) * sx + i;
+    *p = val;
+    int di = 0, dj = 0;
+    if (px) { if (i < OCN_HALO) di = nx; else if (i >= nx - OCN_HALO) di = -nx; }
+    if (py) { if (j < OCN_HALO) dj = ny; else if (j >= ny - OCN_HALO) dj = -ny; }
+    if (di) p[di] = val;
+    if (dj) p[(long long)dj * sx] = val;
+    if (di && dj) p[(long long)dj * sx + di] = val;
+    // very small periodic domains (n < 6): a cell can be the image of both halos
+    if (px && nx < 2 * OCN_HALO) {
+        if (i < OCN_HALO && i >= nx - OCN_HALO) { p[-nx] = val; if (dj) p[(long long)dj * sx - nx] = val; }
+    }
+    if (py && ny < 2 * OCN_HALO) {
+        if (j < OCN_HALO && j >= ny - OCN_HALO) {
+            p[-(long long)ny * sx] = val;
+            if (di) p[-(long long)ny * sx + di] = val;
+            if (px && nx < 2 * OCN_HALO && i < OCN_HALO && i >= nx - OCN_HALO) p[-(long long)ny * sx - nx] = val;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// WENO face value (Shu 1997 as cited at PAPER.md:244).  Cells n-3..n+2 are
+// (a, b, c, d, e, f); the face lies between c and d; q0 is the upwind cell.
+// Division-free nonlinear weights: alpha_s ~ d_s * prod_{t != s} (eps + beta_t)^2, one division.
+// ---------------------------------------------------------------------------------------------
+template <class T>
+__device__ __forceinline__ T weno_face(T a, T b, T c, T d, T e, T f, T vel, int order) {
+    const bool pos = vel > T(0);
+    const T qm2 = pos ? a : f, qm1 = pos ? b : e, q0 = pos ? c : d, q1 = pos ? d : c, q2 = pos ? e : b;
+    const T eps = T(1e-6);
+    if (order >= 3) {
+        const T p0 = (T(2) * qm2 - T(7) * qm1 + T(11) * q0) * T(1.0 / 6.0);
+        const T p1 = (-qm1 + T(5) * q0 + T(2) * q1) * T(1.0 / 6.0);
+        const T p2 = (T(2) * q0 + T(5) * q1 - q2) * T(1.0 / 6.0);
+        const T s0 = qm2 - T(2) * qm1 + q0, t0 = qm2 - T(4) * qm1 + T(3) * q0;
+        const T s1 = qm1 - T(2) * q0 + q1, t1 = qm1 - q1;
+        const T s2 = q0 - T(2) * q1 + q2, t2 = T(3) * q0 - T(4) * q1 + q2;
+        const T b0 = eps + T(13.0 / 12.0) * s0 * s0 + T(0.25) * t0 * t0;
+        const T b1 = eps + T(13.0 / 12.0) * s1 * s1 + T(0.25) * t1 * t1;
+        const T b2 = eps + T(13.0 / 12.0) * s2 * s2 + T(0.25) * t2 * t2;
+        const T b01 = b0 * b1, b02 = b0 * b2, b12 = b1 * b2;
+        const T a0 = T(0.1) * b12 * b12, a1 = T(0.6) * b02 * b02, a2 = T(0.3) * b01 * b01;
+        return (a0 * p0 + a1 * p1 + a2 * p2) / (a0 + a1 + a2);
+    }
+    if (order == 2) {
+        const T p0 = T(0.5) * (T(3) * q0 - qm1), p1 = T(0.5) * (q0 + q1);
+        const T b0 = eps + (q0 - qm1) * (q0 - qm1), b1 = eps + (q1 - q0) * (q1 - q0);
+        const T a0 = T(1.0 / 3.0) * b1 * b1, a1 = T(2.0 / 3.0) * b0 * b0;
+        return (a0 * p0 + a1 * p1) / (a0 + a1);
+    }
+    return order == 1 ? q0 : T(0);
+}
+
+__device__ __forceinline__ int order3(int k, int t1, int t2, int t3) {
+    return (k >= t1) + (k >= t2) + (k >= t3);
+}
+
+}  // namespace ocn

@@ -1,0 +1,178 @@
+// kernels_column.cuh — column and 2-D kernels: barotropic sub-step (S6), back-substitution +
+// barotropic correction (second half of S4, S7), vertical velocity scan (S8), halo-aware
+// scatter / gather for ocn_set_fields / ocn_get_fields (S10 is folded into store_halo).
+#pragma once
+#include "common.cuh"
+
+namespace ocn {
+
+// ---------------------------------------------------------------------------------------------
+// S6: one forward-backward barotropic sub-step (DESIGN.md §3.8 step 6): eta first, then U, V
+// with the new eta.  eta is recomputed redundantly for the west and south neighbours so that
+// one launch advances the whole sub-step.  Reads buffer `cur`, writes buffer `cur ^ 1`.
+// ---------------------------------------------------------------------------------------------
+template <class T>
+__global__ void __launch_bounds__(256) k_barotropic(const DevP<T> P, const int cur, const T am, const int first) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    if (i >= P.nx || j >= P.ny) return;
+    const int sx = P.sx, nz = P.nz, r = j + OCN_HALO;
+    const long long c = (long long)r * sx + i;
+    const T* __restrict__ e0 = P.eta[cur];
+    const T* __restrict__ U0 = P.U[cur];
+    const T* __restrict__ V0 = P.V[cur];
+    const uint2 m = P.m8[c];
+    const bool wet_c = (m.x & 255) < nz, wet_w = (P.m8[c - 1].x & 255) < nz, wet_s = (P.m8[c - sx].x & 255) < nz;
+    const bool mu = ((m.x >> 8) & 255) < nz, mv = (m.y & 255) < nz;
+    const T dy = P.dy, dtau = P.dtau;
+    const T dF0 = P.dxF[r], dF1 = P.dxF[r + 1], dFm = P.dxF[r - 1];
+    const T Uc = U0[c], Vc = V0[c];
+    T ec = e0[c], ew = e0[c - 1], es = e0[c - sx];
+    if (wet_c) ec -= dtau * (dy * (U0[c + 1] - Uc) + dF1 * V0[c + sx] - dF0 * Vc) * P.rAzC[r];
+    if (wet_w) ew -= dtau * (dy * (Uc - U0[c - 1]) + dF1 * V0[c + sx - 1] - dF0 * V0[c - 1]) * P.rAzC[r];
+    if (wet_s) es -= dtau * (dy * (U0[c - sx + 1] - U0[c - sx]) + dF0 * Vc - dFm * V0[c - sx]) * P.rAzC[r - 1];
+    const T Un = mu ? Uc + dtau * (-P.g * P.Hu[c] * (ec - ew) * P.rdxC[r] + P.GU[c]) : T(0);
+    const T Vn = mv ? Vc + dtau * (-P.g * P.Hv[c] * (ec - es) * P.rdy + P.GV[c]) : T(0);
+    store_halo(P.eta[cur ^ 1], sx, P.nx, P.ny, P.px, P.py, j, i, ec);
+    store_halo(P.U[cur ^ 1], sx, P.nx, P.ny, P.px, P.py, j, i, Un);
+    store_halo(P.V[cur ^ 1], sx, P.nx, P.ny, P.px, P.py, j, i, Vn);
+    if (first) { P.etab[c] = am * ec; P.Ub[c] = am * Un; P.Vb[c] = am * Vn; }
+    else       { P.etab[c] += am * ec; P.Ub[c] += am * Un; P.Vb[c] += am * Vn; }
+}
+
+// step 7: the filtered values become the barotropic state (buffer 0, with halos)
+template <class T>
+__global__ void __launch_bounds__(256) k_barotropic_finish(const DevP<T> P) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    if (i >= P.nx || j >= P.ny) return;
+    const long long c = (long long)(j + OCN_HALO) * P.sx + i;
+    store_halo(P.eta[0], P.sx, P.nx, P.ny, P.px, P.py, j, i, P.etab[c]);
+    store_halo(P.U[0], P.sx, P.nx, P.ny, P.px, P.py, j, i, P.Ub[c]);
+    store_halo(P.V[0], P.sx, P.nx, P.ny, P.px, P.py, j, i, P.Vb[c]);
+}
+
+// ---------------------------------------------------------------------------------------------
+// S4 (back-substitution, bottom-up) + S7 (barotropic correction).  The implicit operator
+// conserves the column integral, so sum_k dz u** = sum_k dz u* (SU from K1) and the correction
+// (Ubar - SU) / Hu is known before the sweep.
+// ---------------------------------------------------------------------------------------------
+template <class T>
+__global__ void __launch_bounds__(128) k_backsub_correct(const DevP<T> P) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    if (i >= P.nx || j >= P.ny) return;
+    const int sx = P.sx, nz = P.nz;
+    const long long sz = P.sz, c = (long long)(j + OCN_HALO) * sx + i;
+    const uint2 m = P.m8[c];
+    const int kb = m.x & 255, tx1 = (m.x >> 8) & 255, ty1 = m.y & 255;
+    if (tx1 < nz) {
+        const T cu = (P.Ub[c] - P.SU[c]) * P.rHu[c];
+        T prev = 0;
+        for (int k = tx1; k < nz; ++k) {
+            const T x = P.du[k * sz + c] + (k > tx1 ? P.e_m[k] * prev : T(0));
+            prev = x;
+            store_halo(P.u + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, x + cu);
+        }
+    }
+    if (ty1 < nz) {
+        const T cv = (P.Vb[c] - P.SV[c]) * P.rHv[c];
+        T prev = 0;
+        for (int k = ty1; k < nz; ++k) {
+            const T x = P.dv[k * sz + c] + (k > ty1 ? P.e_m[k] * prev : T(0));
+            prev = x;
+            store_halo(P.v + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, x + cv);
+        }
+    }
+    if (kb < nz) {
+        T pt = 0, ps = 0;
+        for (int k = kb; k < nz; ++k) {
+            const T e = k > kb ? P.e_t[k] : T(0);
+            pt = P.dt_[k * sz + c] + e * pt;
+            ps = P.ds[k * sz + c] + e * ps;
+            store_halo(P.t + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, pt);
+            store_halo(P.s + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, ps);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// S8: w from continuity, bottom-up scan; runs through land where D = 0.
+// ---------------------------------------------------------------------------------------------
+template <class T>
+__global__ void __launch_bounds__(128) k_vertical_velocity(const DevP<T> P) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    if (i >= P.nx || j >= P.ny) return;
+    const int sx = P.sx, nz = P.nz, r = j + OCN_HALO;
+    const long long sz = P.sz, c = (long long)r * sx + i;
+    const T dy = P.dy, dF0 = P.dxF[r], dF1 = P.dxF[r + 1], rA = P.rAzC[r];
+    double w = 0.0;
+    for (int k = 0; k < nz; ++k) {
+        const T* __restrict__ pu = P.u + k * sz + c;
+        const T* __restrict__ pv = P.v + k * sz + c;
+        const T D = (dy * (pu[1] - pu[0]) + dF1 * pv[sx] - dF0 * pv[0]) * rA;
+        w -= (double)P.dz[k] * (double)D;
+        store_halo(P.w + (k + 1) * sz, sx, P.nx, P.ny, P.px, P.py, j, i, (T)w);
+    }
+}
+
+// U, V = sum_k dz u, v of the current state into buffer 0 (ocn_set_fields)
+template <class T>
+__global__ void __launch_bounds__(128) k_init_transport(const DevP<T> P) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    if (i >= P.nx || j >= P.ny) return;
+    const long long sz = P.sz, c = (long long)(j + OCN_HALO) * P.sx + i;
+    double su = 0, sv = 0;
+    for (int k = 0; k < P.nz; ++k) { su += (double)P.dz[k] * (double)P.u[k * sz + c]; sv += (double)P.dz[k] * (double)P.v[k * sz + c]; }
+    store_halo(P.U[0], P.sx, P.nx, P.ny, P.px, P.py, j, i, (T)su);
+    store_halo(P.V[0], P.sx, P.nx, P.ny, P.px, P.py, j, i, (T)sv);
+}
+
+// ---------------------------------------------------------------------------------------------
+// scatter (contiguous interior -> halo'd plane layout, masked) and gather (back, land = 0)
+// kind: 0 u, 1 v, 2 T (offset T0), 3 S (offset S0), 4 eta, 5 plain 2-D, 6 w (nz+1 levels, gather only)
+// ---------------------------------------------------------------------------------------------
+template <class T>
+__device__ __forceinline__ bool cell_open(const DevP<T>& P, long long c, int k, int kind) {
+    const uint2 m = P.m8[c];
+    const int kb = m.x & 255, tx1 = (m.x >> 8) & 255, ty1 = m.y & 255;
+    switch (kind) {
+        case 0: return k >= tx1;
+        case 1: return k >= ty1;
+        case 2: case 3: return k >= kb;
+        case 4: return kb < P.nz;
+        default: return true;
+    }
+}
+
+template <class T>
+__global__ void __launch_bounds__(256) k_scatter(const DevP<T> P, T* __restrict__ dst, const T* __restrict__ src,
+                                                 const int nl, const int kind) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    if (i >= P.nx || j >= P.ny) return;
+    const long long c = (long long)(j + OCN_HALO) * P.sx + i;
+    const T off = kind == 2 ? P.T0 : kind == 3 ? P.S0 : T(0);
+    for (int k = blockIdx.z; k < nl; k += gridDim.z) {
+        const T v = cell_open(P, c, k, kind) ? src[((long long)k * P.ny + j) * P.nx + i] - off : T(0);
+        store_halo(dst + k * P.sz, P.sx, P.nx, P.ny, P.px, P.py, j, i, v);
+    }
+}
+
+template <class T, class O>
+__global__ void __launch_bounds__(256) k_gather(const DevP<T> P, O* __restrict__ dst, const T* __restrict__ src,
+                                                const int nl, const int kind) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    if (i >= P.nx || j >= P.ny) return;
+    const long long c = (long long)(j + OCN_HALO) * P.sx + i;
+    const T off = kind == 2 ? P.T0 : kind == 3 ? P.S0 : T(0);
+    for (int k = blockIdx.z; k < nl; k += gridDim.z) {
+        const T v = cell_open(P, c, k, kind) ? src[k * P.sz + c] + off : T(0);
+        dst[((long long)k * P.ny + j) * P.nx + i] = (O)v;
+    }
+}
+
+}  // namespace ocn

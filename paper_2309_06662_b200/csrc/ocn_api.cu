@@ -1,0 +1,447 @@
+// ocn_api.cu — the C ABI of libocn (include/ocn.h): host-side scheduling only.  Every step of the
+// hot path runs in the kernels of kernels_tend.cuh / kernels_column.cuh.
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "grid_host.h"
+#include "kernels_column.cuh"
+#include "kernels_tend.cuh"
+
+namespace {
+
+thread_local std::string g_err;
+ocn_status fail(ocn_status s, const std::string& m) { g_err = m; return s; }
+
+#define CK(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess)                                                                     \
+            return fail(e_ == cudaErrorMemoryAllocation ? OCN_ENOMEM : OCN_ECUDA,                  \
+                        std::string(#call) + ": " + cudaGetErrorString(e_));                       \
+    } while (0)
+
+constexpr int LEAD = 32;   // elements before the first row so that i = 0 starts a 128-byte line
+
+}  // namespace
+
+struct ocn_model {
+    const ocn_grid* g = nullptr;
+    ocn_model_desc d{};
+    int prec = 64;
+    cudaStream_t stream = nullptr;
+    bool own_stream = false;
+    std::vector<double> a_w;
+    double dtau = 0;
+    bool have_history = false;
+    std::vector<void*> allocs;
+    unsigned long long bytes = 0;
+    ocn::DevP<float> pf{};
+    ocn::DevP<double> pd{};
+    void* stage = nullptr;              // contiguous staging buffer, (nz+1)*ny*nx doubles
+    cudaGraphExec_t graph = nullptr;    // one steady-state (AB2) step
+    int launches_per_step = 0;
+};
+
+namespace {
+
+template <class T>
+ocn_status dev_alloc(ocn_model* M, size_t n, T** out, bool lead) {
+    void* p = nullptr;
+    const size_t total = (n + (lead ? 2 * LEAD : 0)) * sizeof(T);
+    CK(cudaMalloc(&p, total));
+    CK(cudaMemsetAsync(p, 0, total, M->stream));
+    M->allocs.push_back(p);
+    M->bytes += total;
+    *out = reinterpret_cast<T*>(p) + (lead ? LEAD : 0);
+    return OCN_OK;
+}
+
+template <class T>
+ocn_status upload(ocn_model* M, const std::vector<double>& src, const T** out) {
+    std::vector<T> tmp(src.begin(), src.end());
+    T* p = nullptr;
+    ocn_status s = dev_alloc(M, tmp.size(), &p, false);
+    if (s != OCN_OK) return s;
+    CK(cudaMemcpyAsync(p, tmp.data(), tmp.size() * sizeof(T), cudaMemcpyHostToDevice, M->stream));
+    CK(cudaStreamSynchronize(M->stream));
+    *out = p;
+    return OCN_OK;
+}
+
+template <class T>
+ocn::DevP<T>& params(ocn_model* M);
+template <> ocn::DevP<float>& params<float>(ocn_model* M) { return M->pf; }
+template <> ocn::DevP<double>& params<double>(ocn_model* M) { return M->pd; }
+
+dim3 grid2(const ocn_grid* g, dim3 b, int z = 1) { return dim3((g->nx + b.x - 1) / b.x, (g->ny + b.y - 1) / b.y, z); }
+
+template <class T>
+ocn_status build_model(ocn_model* M) {
+    const ocn_grid* g = M->g;
+    ocn::DevP<T>& P = params<T>(M);
+    const int nz = g->nz;
+    P.nx = g->nx; P.ny = g->ny; P.nz = nz; P.sx = g->sx; P.sy = g->sy; P.sz = (long long)g->sx * g->sy;
+    P.px = g->d.periodic_x != 0; P.py = g->d.periodic_y != 0;
+    const size_t n3 = (size_t)P.sz * nz, n2 = (size_t)P.sz;
+    ocn_status s;
+    // plane-layout arrays: allocation starts LEAD elements before row -3; cell (j, i) is at
+    // base[(j+3)*sx + i] and i = 0 is 128-byte aligned (sx is a multiple of 32 elements)
+    auto plane = [&](size_t n, T** out) -> ocn_status {
+        return dev_alloc(M, n, out, true);
+    };
+    T** f3[] = {&P.u, &P.v, &P.t, &P.s, &P.du, &P.dv, &P.dt_, &P.ds, &P.Gu, &P.Gv, &P.Gt, &P.Gs};
+    for (T** f : f3) if ((s = plane(n3, f)) != OCN_OK) return s;
+    if ((s = plane(n3 + n2, &P.w)) != OCN_OK) return s;
+    T** f2[] = {&P.eta[0], &P.eta[1], &P.U[0], &P.U[1], &P.V[0], &P.V[1], &P.etab, &P.Ub, &P.Vb, &P.GU, &P.GV,
+                &P.SU, &P.SV, &P.Hu, &P.Hv, &P.rHu, &P.rHv, &P.taux, &P.tauy};
+    for (T** f : f2) if ((s = plane(n2, f)) != OCN_OK) return s;
+    // masks
+    {
+        uint2* p8 = nullptr; uchar4* pz = nullptr;
+        if ((s = dev_alloc(M, g->m8.size(), &p8, false)) != OCN_OK) return s;
+        if ((s = dev_alloc(M, g->mz.size(), &pz, false)) != OCN_OK) return s;
+        CK(cudaMemcpyAsync(p8, g->m8.data(), g->m8.size() * 8, cudaMemcpyHostToDevice, M->stream));
+        CK(cudaMemcpyAsync(pz, g->mz.data(), g->mz.size() * 4, cudaMemcpyHostToDevice, M->stream));
+        P.m8 = p8 + LEAD; P.mz = pz + LEAD;          // host planes were built with the same lead
+    }
+    // metrics (+ reciprocals), vertical grid
+    auto recip = [](const std::vector<double>& a) { std::vector<double> r(a.size()); for (size_t q = 0; q < a.size(); ++q) r[q] = 1.0 / a[q]; return r; };
+    if ((s = upload(M, g->dxC, &P.dxC)) != OCN_OK || (s = upload(M, g->dxF, &P.dxF)) != OCN_OK ||
+        (s = upload(M, g->AzC, &P.AzC)) != OCN_OK || (s = upload(M, g->AzF, &P.AzF)) != OCN_OK ||
+        (s = upload(M, g->fF, &P.fF)) != OCN_OK || (s = upload(M, recip(g->dxC), &P.rdxC)) != OCN_OK ||
+        (s = upload(M, recip(g->dxF), &P.rdxF)) != OCN_OK || (s = upload(M, recip(g->AzC), &P.rAzC)) != OCN_OK ||
+        (s = upload(M, recip(g->AzF), &P.rAzF)) != OCN_OK || (s = upload(M, g->dz, &P.dz)) != OCN_OK ||
+        (s = upload(M, recip(g->dz), &P.rdz)) != OCN_OK || (s = upload(M, g->dzc, &P.dzc)) != OCN_OK)
+        return s;
+    P.dy = (T)g->dy; P.rdy = (T)(1.0 / g->dy);
+    P.hz_top = (T)(g->zf[nz] - g->zc[nz - 1]);
+    // top-down Thomas tables
+    for (int pass = 0; pass < 2; ++pass) {
+        const double dtk = M->d.dt * (pass == 0 ? M->d.nu_z : M->d.kappa_z);
+        std::vector<double> sp(nz, 0.0), e(nz, 0.0), im(nz, 1.0), imb(nz, 1.0);
+        double e_above = 0.0;
+        for (int k = nz - 1; k >= 0; --k) {
+            const double s_up = (k <= nz - 2) ? dtk / (g->dz[k] * g->dzc[k + 1]) : 0.0;
+            const double s_dn = (k >= 1) ? dtk / (g->dz[k] * g->dzc[k]) : 0.0;
+            const double m = 1.0 + s_up + s_dn - s_up * e_above;
+            const double mb = 1.0 + s_up - s_up * e_above;
+            sp[k] = s_up; im[k] = 1.0 / m; imb[k] = 1.0 / mb; e[k] = s_dn / m;
+            e_above = e[k];
+        }
+        if (pass == 0) {
+            if ((s = upload(M, sp, &P.sp_m)) != OCN_OK || (s = upload(M, e, &P.e_m)) != OCN_OK ||
+                (s = upload(M, im, &P.im_m)) != OCN_OK || (s = upload(M, imb, &P.imb_m)) != OCN_OK) return s;
+        } else {
+            if ((s = upload(M, sp, &P.sp_t)) != OCN_OK || (s = upload(M, e, &P.e_t)) != OCN_OK ||
+                (s = upload(M, im, &P.im_t)) != OCN_OK || (s = upload(M, imb, &P.imb_t)) != OCN_OK) return s;
+        }
+    }
+    P.dt = (T)M->d.dt; P.g = (T)M->d.g; P.alpha = (T)M->d.alpha; P.beta_s = (T)M->d.beta_s;
+    P.T0 = (T)M->d.T0; P.S0 = (T)M->d.S0; P.rrho0 = (T)(1.0 / M->d.rho0);
+    P.nu_h = (T)M->d.nu_h; P.kappa_h = (T)M->d.kappa_h; P.dtau = (T)M->dtau;
+    // Hu, Hv = sum_k dz over open faces, and reciprocals
+    {
+        std::vector<T> hu(n2 + 2 * LEAD, T(0)), hv(hu), rhu(hu), rhv(hu);
+        for (int j = 0; j < g->ny; ++j)
+            for (int i = 0; i < g->nx; ++i) {
+                const uint64_t w = g->m8[g->pidx(j, i)];
+                const int tx1 = (w >> 8) & 255, ty1 = (w >> 32) & 255;
+                double a = 0, b = 0;
+                for (int k = 0; k < nz; ++k) { if (k >= tx1) a += g->dz[k]; if (k >= ty1) b += g->dz[k]; }
+                const size_t q = g->pidx(j, i);
+                hu[q] = (T)a; hv[q] = (T)b; rhu[q] = a > 0 ? (T)(1.0 / a) : T(0); rhv[q] = b > 0 ? (T)(1.0 / b) : T(0);
+            }
+        const size_t nb = hu.size() * sizeof(T);
+        CK(cudaMemcpyAsync(P.Hu - LEAD, hu.data(), nb, cudaMemcpyHostToDevice, M->stream));
+        CK(cudaMemcpyAsync(P.Hv - LEAD, hv.data(), nb, cudaMemcpyHostToDevice, M->stream));
+        CK(cudaMemcpyAsync(P.rHu - LEAD, rhu.data(), nb, cudaMemcpyHostToDevice, M->stream));
+        CK(cudaMemcpyAsync(P.rHv - LEAD, rhv.data(), nb, cudaMemcpyHostToDevice, M->stream));
+        CK(cudaStreamSynchronize(M->stream));
+    }
+    CK(cudaMalloc(&M->stage, (size_t)(nz + 1) * g->ny * g->nx * sizeof(double)));
+    M->bytes += (size_t)(nz + 1) * g->ny * g->nx * sizeof(double);
+    M->launches_per_step = M->d.substeps + 4;
+    return OCN_OK;
+}
+
+}  // namespace
+
+// =================================================================================================
+// step scheduling
+// =================================================================================================
+namespace {
+
+template <class T>
+ocn_status launch_step(ocn_model* M, bool euler) {
+    const ocn_grid* g = M->g;
+    const ocn::DevP<T>& P = params<T>(M);
+    const T c0 = euler ? T(1) : (T)(1.5 + M->d.chi), c1 = euler ? T(0) : (T)(0.5 + M->d.chi);
+    const dim3 bc(32, 4), b2(32, 8);
+    ocn::k_tendency<T><<<grid2(g, bc), bc, 0, M->stream>>>(P, c0, c1);
+    int cur = 0;
+    for (int m = 1; m <= M->d.substeps; ++m) {
+        ocn::k_barotropic<T><<<grid2(g, b2), b2, 0, M->stream>>>(P, cur, (T)M->a_w[m - 1], m == 1 ? 1 : 0);
+        cur ^= 1;
+    }
+    ocn::k_barotropic_finish<T><<<grid2(g, b2), b2, 0, M->stream>>>(P);
+    ocn::k_backsub_correct<T><<<grid2(g, bc), bc, 0, M->stream>>>(P);
+    ocn::k_vertical_velocity<T><<<grid2(g, bc), bc, 0, M->stream>>>(P);
+    CK(cudaGetLastError());
+    return OCN_OK;
+}
+
+template <class T>
+ocn_status run_steps(ocn_model* M, int n) {
+    ocn_status s;
+    while (n > 0 && !M->have_history) {          // Euler start after ocn_set_fields
+        if ((s = launch_step<T>(M, true)) != OCN_OK) return s;
+        M->have_history = true; --n;
+    }
+    if (n <= 0) return OCN_OK;
+    if (!M->graph) {                              // capture one steady-state step once
+        cudaGraph_t gr = nullptr;
+        CK(cudaStreamBeginCapture(M->stream, cudaStreamCaptureModeThreadLocal));
+        s = launch_step<T>(M, false);
+        cudaError_t e = cudaStreamEndCapture(M->stream, &gr);
+        if (s != OCN_OK) { if (gr) cudaGraphDestroy(gr); return s; }
+        CK(e);
+        CK(cudaGraphInstantiate(&M->graph, gr, 0));
+        CK(cudaGraphDestroy(gr));
+    }
+    for (int q = 0; q < n; ++q) CK(cudaGraphLaunch(M->graph, M->stream));
+    return OCN_OK;
+}
+
+template <class T>
+ocn_status set_one(ocn_model* M, const void* src, T* dst, int nl, int kind, bool on_device) {
+    const ocn_grid* g = M->g;
+    const size_t n = (size_t)nl * g->ny * g->nx;
+    const T* dsrc = static_cast<const T*>(src);
+    if (!on_device) {
+        CK(cudaMemcpyAsync(M->stage, src, n * sizeof(T), cudaMemcpyHostToDevice, M->stream));
+        dsrc = static_cast<const T*>(M->stage);
+    }
+    const dim3 b(32, 8);
+    ocn::k_scatter<T><<<grid2(g, b, nl < 64 ? nl : 64), b, 0, M->stream>>>(params<T>(M), dst, dsrc, nl, kind);
+    CK(cudaGetLastError());
+    if (!on_device) CK(cudaStreamSynchronize(M->stream));   // staging buffer is reused by the next field
+    return OCN_OK;
+}
+
+template <class T>
+ocn_status set_fields_t(ocn_model* M, const ocn_fields* f) {
+    ocn::DevP<T>& P = params<T>(M);
+    const int nz = M->g->nz;
+    const bool dev = f->on_device != 0;
+    ocn_status s;
+    if (f->u && (s = set_one<T>(M, f->u, P.u, nz, 0, dev)) != OCN_OK) return s;
+    if (f->v && (s = set_one<T>(M, f->v, P.v, nz, 1, dev)) != OCN_OK) return s;
+    if (f->T && (s = set_one<T>(M, f->T, P.t, nz, 2, dev)) != OCN_OK) return s;
+    if (f->S && (s = set_one<T>(M, f->S, P.s, nz, 3, dev)) != OCN_OK) return s;
+    if (f->eta && (s = set_one<T>(M, f->eta, P.eta[0], 1, 4, dev)) != OCN_OK) return s;
+    if (f->tau_x && (s = set_one<T>(M, f->tau_x, P.taux, 1, 5, dev)) != OCN_OK) return s;
+    if (f->tau_y && (s = set_one<T>(M, f->tau_y, P.tauy, 1, 5, dev)) != OCN_OK) return s;
+    if (f->u || f->v || f->T || f->S || f->eta) {
+        const dim3 bc(32, 4);
+        ocn::k_init_transport<T><<<grid2(M->g, bc), bc, 0, M->stream>>>(P);
+        ocn::k_vertical_velocity<T><<<grid2(M->g, bc), bc, 0, M->stream>>>(P);
+        CK(cudaGetLastError());
+        M->have_history = false;
+    }
+    return OCN_OK;
+}
+
+template <class T, class O>
+ocn_status get_one(ocn_model* M, void* dst, const T* src, int nl, int kind, bool on_device) {
+    const ocn_grid* g = M->g;
+    const size_t n = (size_t)nl * g->ny * g->nx;
+    O* ddst = on_device ? static_cast<O*>(dst) : static_cast<O*>(M->stage);
+    const dim3 b(32, 8);
+    ocn::k_gather<T, O><<<grid2(g, b, nl < 64 ? nl : 64), b, 0, M->stream>>>(params<T>(M), ddst, src, nl, kind);
+    CK(cudaGetLastError());
+    if (!on_device) {
+        CK(cudaMemcpyAsync(dst, M->stage, n * sizeof(O), cudaMemcpyDeviceToHost, M->stream));
+        CK(cudaStreamSynchronize(M->stream));
+    }
+    return OCN_OK;
+}
+
+template <class T>
+ocn_status get_fields_t(ocn_model* M, ocn_fields* f) {
+    ocn::DevP<T>& P = params<T>(M);
+    const int nz = M->g->nz;
+    const bool dev = f->on_device != 0;
+    ocn_status s;
+    if (f->u && (s = get_one<T, T>(M, f->u, P.u, nz, 0, dev)) != OCN_OK) return s;
+    if (f->v && (s = get_one<T, T>(M, f->v, P.v, nz, 1, dev)) != OCN_OK) return s;
+    if (f->T && (s = get_one<T, T>(M, f->T, P.t, nz, 2, dev)) != OCN_OK) return s;
+    if (f->S && (s = get_one<T, T>(M, f->S, P.s, nz, 3, dev)) != OCN_OK) return s;
+    if (f->w && (s = get_one<T, T>(M, f->w, P.w, nz + 1, 6, dev)) != OCN_OK) return s;
+    if (f->eta && (s = get_one<T, T>(M, f->eta, P.eta[0], 1, 4, dev)) != OCN_OK) return s;
+    if (f->tau_x && (s = get_one<T, T>(M, f->tau_x, P.taux, 1, 5, dev)) != OCN_OK) return s;
+    if (f->tau_y && (s = get_one<T, T>(M, f->tau_y, P.tauy, 1, 5, dev)) != OCN_OK) return s;
+    CK(cudaStreamSynchronize(M->stream));
+    return OCN_OK;
+}
+
+template <class T>
+ocn_status get_debug_t(ocn_model* M, double* Gu, double* Gv, double* GT, double* GS, double* U, double* V) {
+    ocn::DevP<T>& P = params<T>(M);
+    const int nz = M->g->nz;
+    ocn_status s;
+    if (Gu && (s = get_one<T, double>(M, Gu, P.Gu, nz, 5, false)) != OCN_OK) return s;
+    if (Gv && (s = get_one<T, double>(M, Gv, P.Gv, nz, 5, false)) != OCN_OK) return s;
+    if (GT && (s = get_one<T, double>(M, GT, P.Gt, nz, 5, false)) != OCN_OK) return s;
+    if (GS && (s = get_one<T, double>(M, GS, P.Gs, nz, 5, false)) != OCN_OK) return s;
+    if (U && (s = get_one<T, double>(M, U, P.U[0], 1, 5, false)) != OCN_OK) return s;
+    if (V && (s = get_one<T, double>(M, V, P.V[0], 1, 5, false)) != OCN_OK) return s;
+    return OCN_OK;
+}
+
+}  // namespace
+
+// =================================================================================================
+// C ABI
+// =================================================================================================
+extern "C" {
+
+const char* ocn_last_error(void) { return g_err.c_str(); }
+const char* ocn_version(void) { return "libocn 0.1 (sm_100a)"; }
+
+ocn_status ocn_grid_create(const ocn_grid_desc* d, const double* z_faces, const double* depth, ocn_grid** out) {
+    if (!d || !z_faces || !depth || !out) return fail(OCN_EINVAL, "null argument");
+    if (d->nx < OCN_HALO || d->ny < OCN_HALO || d->nz < 2) return fail(OCN_EINVAL, "grid too small (nx, ny >= 3, nz >= 2)");
+    if (d->nz > 250) return fail(OCN_EUNSUPPORTED, "nz > 250 (level thresholds are stored in 8 bits)");
+    if (d->kind != 0 && d->kind != 1) return fail(OCN_EINVAL, "kind must be 0 (cartesian) or 1 (lat-lon)");
+    if (d->kind == 1 && d->periodic_y) return fail(OCN_EINVAL, "a lat-lon grid cannot be periodic in latitude");
+    if (!(d->dx > 0) || !(d->dy > 0)) return fail(OCN_EINVAL, "dx, dy must be positive");
+    ocn_grid* g = new (std::nothrow) ocn_grid();
+    if (!g) return fail(OCN_ENOMEM, "host allocation failed");
+    try {
+        const std::string e = ocn_host::build_grid(*g, *d, z_faces, depth);
+        if (!e.empty()) { delete g; return fail(OCN_EINVAL, e); }
+    } catch (const std::exception& ex) { delete g; return fail(OCN_ENOMEM, ex.what()); }
+    *out = g;
+    return OCN_OK;
+}
+
+ocn_status ocn_grid_destroy(ocn_grid* g) { delete g; return OCN_OK; }
+
+ocn_status ocn_get_masks(const ocn_grid* g, unsigned char* wet, unsigned char* ox, unsigned char* oy,
+                         unsigned char* oz, unsigned char* ozu, unsigned char* ozv) {
+    if (!g) return fail(OCN_EINVAL, "null grid");
+    const int nx = g->nx, ny = g->ny, nz = g->nz;
+    for (int k = 0; k <= nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                const uint64_t m = g->m8[g->pidx(j, i)];
+                const uint32_t z = g->mz[g->pidx(j, i)];
+                const int kb = m & 255, tx1 = (m >> 8) & 255, tx2 = (m >> 16) & 255, tx3 = (m >> 24) & 255;
+                const int ty1 = (m >> 32) & 255, ty2 = (m >> 40) & 255, ty3 = (m >> 48) & 255;
+                const size_t n = ((size_t)k * ny + j) * nx + i;
+                if (oz) oz[n] = (unsigned char)((k >= 1 && k < nz) ? std::max(0, std::min(3, std::min(k - kb, nz - k))) : 0);
+                if (k == nz) continue;
+                if (wet) wet[n] = k >= kb;
+                if (ox) ox[n] = (unsigned char)((k >= tx1) + (k >= tx2) + (k >= tx3));
+                if (oy) oy[n] = (unsigned char)((k >= ty1) + (k >= ty2) + (k >= ty3));
+                if (ozu) ozu[n] = (unsigned char)(k >= tx1 ? 1 + (k >= (int)(z & 255)) + (k >= (int)((z >> 8) & 255)) : 0);
+                if (ozv) ozv[n] = (unsigned char)(k >= ty1 ? 1 + (k >= (int)((z >> 16) & 255)) + (k >= (int)(z >> 24)) : 0);
+            }
+    return OCN_OK;
+}
+
+ocn_status ocn_model_create(const ocn_grid* g, const ocn_model_desc* d, ocn_model** out) {
+    if (!g || !d || !out) return fail(OCN_EINVAL, "null argument");
+    if (d->precision != 32 && d->precision != 64) return fail(OCN_EINVAL, "precision must be 32 or 64");
+    if (!(d->dt > 0) || d->substeps < 1) return fail(OCN_EINVAL, "dt must be > 0 and substeps >= 1");
+    if (!(d->rho0 > 0)) return fail(OCN_EINVAL, "rho0 must be > 0");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+        return fail(OCN_ECUDA, "no CUDA device: libocn has no CPU fallback");
+    if (d->device < 0 || d->device >= ndev) return fail(OCN_EINVAL, "bad device ordinal");
+    CK(cudaSetDevice(d->device));
+    ocn_model* M = new (std::nothrow) ocn_model();
+    if (!M) return fail(OCN_ENOMEM, "host allocation failed");
+    M->g = g; M->d = *d; M->prec = d->precision;
+    // filter weights: power law p = 2, q = 4 unless given; dtau centres the average on t^{n+1}
+    const int Ms = d->substeps;
+    M->a_w.resize(Ms);
+    if (d->filter_weights) {
+        for (int m = 0; m < Ms; ++m) M->a_w[m] = d->filter_weights[m];
+    } else {
+        double sum = 0;
+        for (int m = 1; m <= Ms; ++m) { const double s = (double)m / (Ms + 1); const double s2 = s * s; M->a_w[m - 1] = s2 * (1.0 - s2 * s2); sum += M->a_w[m - 1]; }
+        for (int m = 0; m < Ms; ++m) M->a_w[m] /= sum;
+    }
+    double first = 0;
+    for (int m = 1; m <= Ms; ++m) first += m * M->a_w[m - 1];
+    if (!(first > 0)) { delete M; return fail(OCN_EINVAL, "filter weights have no positive first moment"); }
+    M->dtau = d->dt / first;
+    M->d.filter_weights = nullptr;
+    if (d->stream) M->stream = static_cast<cudaStream_t>(d->stream);
+    else {
+        cudaError_t e = cudaStreamCreateWithFlags(&M->stream, cudaStreamNonBlocking);
+        if (e != cudaSuccess) { delete M; return fail(OCN_ECUDA, cudaGetErrorString(e)); }
+        M->own_stream = true;
+    }
+    const ocn_status s = d->precision == 32 ? build_model<float>(M) : build_model<double>(M);
+    if (s != OCN_OK) { const std::string keep = g_err; ocn_model_destroy(M); g_err = keep; return s; }
+    *out = M;
+    return OCN_OK;
+}
+
+ocn_status ocn_model_destroy(ocn_model* M) {
+    if (!M) return OCN_OK;
+    cudaSetDevice(M->d.device);
+    if (M->stream) cudaStreamSynchronize(M->stream);
+    if (M->graph) cudaGraphExecDestroy(M->graph);
+    for (void* p : M->allocs) cudaFree(p);
+    if (M->stage) cudaFree(M->stage);
+    if (M->own_stream && M->stream) cudaStreamDestroy(M->stream);
+    delete M;
+    return OCN_OK;
+}
+
+ocn_status ocn_set_fields(ocn_model* M, const ocn_fields* f) {
+    if (!M || !f) return fail(OCN_EINVAL, "null argument");
+    if (f->w) return fail(OCN_EINVAL, "w is diagnostic (get only)");
+    CK(cudaSetDevice(M->d.device));
+    return M->prec == 32 ? set_fields_t<float>(M, f) : set_fields_t<double>(M, f);
+}
+
+ocn_status ocn_time_step(ocn_model* M, int n) {
+    if (!M || n < 0) return fail(OCN_EINVAL, "bad argument");
+    CK(cudaSetDevice(M->d.device));
+    return M->prec == 32 ? run_steps<float>(M, n) : run_steps<double>(M, n);
+}
+
+ocn_status ocn_get_fields(ocn_model* M, ocn_fields* f) {
+    if (!M || !f) return fail(OCN_EINVAL, "null argument");
+    CK(cudaSetDevice(M->d.device));
+    return M->prec == 32 ? get_fields_t<float>(M, f) : get_fields_t<double>(M, f);
+}
+
+ocn_status ocn_synchronize(ocn_model* M) {
+    if (!M) return fail(OCN_EINVAL, "null model");
+    CK(cudaStreamSynchronize(M->stream));
+    return OCN_OK;
+}
+
+ocn_status ocn_model_info(const ocn_model* M, int* launches, unsigned long long* bytes) {
+    if (!M) return fail(OCN_EINVAL, "null model");
+    if (launches) *launches = M->launches_per_step;
+    if (bytes) *bytes = M->bytes;
+    return OCN_OK;
+}
+
+ocn_status ocn_get_debug(ocn_model* M, double* Gu, double* Gv, double* GT, double* GS, double* U, double* V) {
+    if (!M) return fail(OCN_EINVAL, "null model");
+    CK(cudaSetDevice(M->d.device));
+    return M->prec == 32 ? get_debug_t<float>(M, Gu, Gv, GT, GS, U, V) : get_debug_t<double>(M, Gu, Gv, GT, GS, U, V);
+}
+
+}  // extern "C"

@@ -1,0 +1,178 @@
+"""Thin ctypes binding over the C ABI of libocn.so (include/ocn.h): argument marshalling only.
+
+Function names mirror the C entry points (ocn_grid_create, ocn_model_create, ocn_set_fields,
+ocn_time_step, ocn_get_fields, ocn_get_masks, ...); `Model` is a convenience wrapper that owns the
+handles.  torch is used only for pinned host buffers / streams by callers; this module needs
+numpy + ctypes.  There is no CPU fallback: a missing library or GPU raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libocn.so")
+_lib = None
+
+OCN_OK = 0
+
+
+class ocn_grid_desc(C.Structure):
+    _fields_ = [("kind", C.c_int), ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
+                ("periodic_x", C.c_int), ("periodic_y", C.c_int),
+                ("x0", C.c_double), ("dx", C.c_double), ("y0", C.c_double), ("dy", C.c_double),
+                ("radius", C.c_double), ("rotation_rate", C.c_double), ("f0", C.c_double), ("beta", C.c_double)]
+
+
+class ocn_model_desc(C.Structure):
+    _fields_ = [("precision", C.c_int), ("dt", C.c_double), ("substeps", C.c_int), ("chi", C.c_double),
+                ("g", C.c_double), ("alpha", C.c_double), ("beta_s", C.c_double), ("T0", C.c_double),
+                ("S0", C.c_double), ("rho0", C.c_double), ("nu_h", C.c_double), ("kappa_h", C.c_double),
+                ("nu_z", C.c_double), ("kappa_z", C.c_double), ("filter_weights", C.POINTER(C.c_double)),
+                ("device", C.c_int), ("stream", C.c_void_p)]
+
+
+class ocn_fields(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("u", "v", "T", "S", "w", "eta", "tau_x", "tau_y")] + [("on_device", C.c_int)]
+
+
+EXPORTS = ["ocn_grid_create", "ocn_grid_destroy", "ocn_model_create", "ocn_model_destroy", "ocn_set_fields",
+           "ocn_time_step", "ocn_get_fields", "ocn_synchronize", "ocn_get_masks", "ocn_model_info",
+           "ocn_get_debug", "ocn_last_error", "ocn_version"]
+
+
+def lib():
+    """Loads libocn.so (built in-tree by paper_2309_06662_b200.build); fails loudly if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_SO):
+            raise RuntimeError(f"{_SO} is missing: run `python -m paper_2309_06662_b200.build` (no CPU fallback)")
+        L = C.CDLL(_SO)
+        L.ocn_last_error.restype = C.c_char_p
+        L.ocn_version.restype = C.c_char_p
+        vp = C.c_void_p
+        L.ocn_grid_create.argtypes = [C.POINTER(ocn_grid_desc), vp, vp, C.POINTER(vp)]
+        L.ocn_grid_destroy.argtypes = [vp]
+        L.ocn_model_create.argtypes = [vp, C.POINTER(ocn_model_desc), C.POINTER(vp)]
+        L.ocn_model_destroy.argtypes = [vp]
+        L.ocn_set_fields.argtypes = [vp, C.POINTER(ocn_fields)]
+        L.ocn_time_step.argtypes = [vp, C.c_int]
+        L.ocn_get_fields.argtypes = [vp, C.POINTER(ocn_fields)]
+        L.ocn_synchronize.argtypes = [vp]
+        L.ocn_get_masks.argtypes = [vp] + [vp] * 6
+        L.ocn_model_info.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_ulonglong)]
+        L.ocn_get_debug.argtypes = [vp] + [vp] * 6
+        _lib = L
+    return _lib
+
+
+def _check(rc):
+    if rc != OCN_OK:
+        raise RuntimeError(f"libocn status {rc}: {lib().ocn_last_error().decode()}")
+
+
+def _ptr(a):
+    return None if a is None else C.c_void_p(a.ctypes.data)
+
+
+class Grid:
+    def __init__(self, grid, z_faces, depth):
+        self.desc = ocn_grid_desc(**{k: grid[k] for k, _ in ocn_grid_desc._fields_})
+        self.nx, self.ny, self.nz = int(grid["nx"]), int(grid["ny"]), int(grid["nz"])
+        zf = np.ascontiguousarray(z_faces, dtype=np.float64)
+        h = np.ascontiguousarray(depth, dtype=np.float64)
+        if zf.size != self.nz + 1 or h.shape != (self.ny, self.nx):
+            raise ValueError("z_faces / depth shape mismatch")
+        self.h = C.c_void_p()
+        _check(lib().ocn_grid_create(C.byref(self.desc), _ptr(zf), _ptr(h), C.byref(self.h)))
+
+    def masks(self):
+        nz, ny, nx = self.nz, self.ny, self.nx
+        names = ("wet", "order_x", "order_y", "order_z", "order_zeta_u", "order_zeta_v")
+        out = {n: np.zeros((nz + 1 if n == "order_z" else nz, ny, nx), np.uint8) for n in names}
+        _check(lib().ocn_get_masks(self.h, *[_ptr(out[n]) for n in names]))
+        return out
+
+    def close(self):
+        if getattr(self, "h", None):
+            lib().ocn_grid_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class Model:
+    """ocn_model_create + ocn_set_fields on a workload dict (paper_2309_06662_b200.workloads)."""
+
+    def __init__(self, workload, device=0, stream=None, filter_weights=None, set_fields=True):
+        self.grid = Grid(workload["grid"], workload["z_faces"], workload["depth"])
+        p = dict(workload["params"])
+        self.precision = int(p["precision"])
+        self.dtype = np.float32 if self.precision == 32 else np.float64
+        self._fw = None if filter_weights is None else np.ascontiguousarray(filter_weights, dtype=np.float64)
+        fw = self._fw.ctypes.data_as(C.POINTER(C.c_double)) if self._fw is not None else None
+        self.desc = ocn_model_desc(filter_weights=fw, device=int(device), stream=stream, **p)
+        self.nx, self.ny, self.nz = self.grid.nx, self.grid.ny, self.grid.nz
+        self.h = C.c_void_p()
+        _check(lib().ocn_model_create(self.grid.h, C.byref(self.desc), C.byref(self.h)))
+        if set_fields and "fields" in workload:
+            self.set_fields(**workload["fields"])
+
+    # -- host numpy arrays ---------------------------------------------------------------
+    def set_fields(self, **kw):
+        keep = {k: np.ascontiguousarray(v, dtype=self.dtype) for k, v in kw.items() if v is not None}
+        f = ocn_fields(on_device=0, **{k: v.ctypes.data for k, v in keep.items()})
+        _check(lib().ocn_set_fields(self.h, C.byref(f)))
+
+    def get_fields(self, names=("u", "v", "T", "S", "w", "eta")):
+        nz, ny, nx = self.nz, self.ny, self.nx
+        shp = {"w": (nz + 1, ny, nx), "eta": (ny, nx), "tau_x": (ny, nx), "tau_y": (ny, nx)}
+        out = {k: np.zeros(shp.get(k, (nz, ny, nx)), self.dtype) for k in names}
+        f = ocn_fields(on_device=0, **{k: v.ctypes.data for k, v in out.items()})
+        _check(lib().ocn_get_fields(self.h, C.byref(f)))
+        return out
+
+    # -- raw pointers (pinned host or device memory owned by the caller, e.g. torch tensors) ----
+    def set_fields_ptr(self, on_device=False, **ptrs):
+        f = ocn_fields(on_device=int(on_device), **{k: int(v) for k, v in ptrs.items()})
+        _check(lib().ocn_set_fields(self.h, C.byref(f)))
+
+    def get_fields_ptr(self, on_device=False, **ptrs):
+        f = ocn_fields(on_device=int(on_device), **{k: int(v) for k, v in ptrs.items()})
+        _check(lib().ocn_get_fields(self.h, C.byref(f)))
+
+    def time_step(self, n=1):
+        _check(lib().ocn_time_step(self.h, int(n)))
+
+    def synchronize(self):
+        _check(lib().ocn_synchronize(self.h))
+
+    def info(self):
+        n, b = C.c_int(), C.c_ulonglong()
+        _check(lib().ocn_model_info(self.h, C.byref(n), C.byref(b)))
+        return dict(launches_per_step=n.value, device_bytes=b.value)
+
+    def debug(self):
+        nz, ny, nx = self.nz, self.ny, self.nx
+        d = {k: np.zeros((nz, ny, nx)) for k in ("Gu", "Gv", "GT", "GS")}
+        d["U"] = np.zeros((ny, nx)); d["V"] = np.zeros((ny, nx))
+        _check(lib().ocn_get_debug(self.h, *[_ptr(d[k]) for k in ("Gu", "Gv", "GT", "GS", "U", "V")]))
+        return d
+
+    def close(self):
+        if getattr(self, "h", None):
+            lib().ocn_model_destroy(self.h)
+            self.h = None
+        self.grid.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
