@@ -66,7 +66,7 @@ typedef struct {
     void* stream;                   /* cudaStream_t of the caller (e.g. torch's), NULL = default */
 } ocn_model_desc;
 
-/* Allocates all device state (13 3-D arrays + 2-D arrays + tables) on `device`. */
+/* Allocates all device state (14 3-D arrays + 2-D arrays + tables) on `device`. */
 ocn_status ocn_model_create(const ocn_grid* grid, const ocn_model_desc* desc, ocn_model** out);
 ocn_status ocn_model_destroy(ocn_model* model);
 

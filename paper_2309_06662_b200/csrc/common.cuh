@@ -20,7 +20,7 @@ struct DevP {
     long long sz;          // level stride = sx * sy
     int px, py;            // periodic flags
     // prognostic state (time level n), w diagnostic, forward-eliminated right-hand sides, AB2 history
-    T *u, *v, *t, *s, *w;
+    T *u, *v, *t, *s, *w, *p;
     T *du, *dv, *dt_, *ds;
     T *Gu, *Gv, *Gt, *Gs;
     // 2-D (plane layout with halo)
@@ -39,16 +39,38 @@ struct DevP {
     // vertical grid
     const T *dz, *rdz, *dzc;       // dzc[k] = zc[k] - zc[k-1] (k >= 1)
     T hz_top;                      // zf[nz] - zc[nz-1]
-    // top-down Thomas tables: momentum (nu_z) and tracers (kappa_z)
-    const T *sp_m, *e_m, *im_m, *imb_m;
-    const T *sp_t, *e_t, *im_t, *imb_t;
+    // Thomas tables, bottom-up elimination in the oracle's order.  Momentum (nu_z)
+    // and tracers (kappa_z).  sm[k]: sub-diagonal s^-_k (open face below); cp/m/rm are indexed
+    // [kf * nz + k] by the column's first open level kf: cp = modified super-diagonal, m = pivot,
+    // rm = 1 / m.
+    const T *sm_m, *cp_m, *m_m, *rm_m;
+    const T *sm_t, *cp_t, *m_t, *rm_t;
     // physics
-    T dt, g, alpha, beta_s, T0, S0, rrho0, nu_h, kappa_h;
+    T dt, g, alpha, beta_s, rrho0, nu_h, kappa_h;
+    T Toff, Soff;          // storage offsets of the tracers: (T0, S0) in fp32, 0 in fp64
+    T dT0, dS0;            // T0 - Toff, S0 - Soff: what is left to subtract in the buoyancy
     T dtau;
 };
 
 template <class T>
 __device__ __forceinline__ T ldg(const T* p) { return __ldg(p); }
+
+// Arithmetic whose rounding order is fixed (no FMA contraction) in fp64, so that the tracer /
+// pressure column passes reproduce the rounding sequence of the discrete equations as written
+// (DESIGN.md §6.5); fp32 lets the compiler contract and divides by multiplying with rm.
+template <class T> struct Ex;
+template <> struct Ex<double> {
+    static __device__ __forceinline__ double mul(double a, double b) { return __dmul_rn(a, b); }
+    static __device__ __forceinline__ double add(double a, double b) { return __dadd_rn(a, b); }
+    static __device__ __forceinline__ double sub(double a, double b) { return __dsub_rn(a, b); }
+    static __device__ __forceinline__ double div(double a, double m, double) { return __ddiv_rn(a, m); }
+};
+template <> struct Ex<float> {
+    static __device__ __forceinline__ float mul(float a, float b) { return a * b; }
+    static __device__ __forceinline__ float add(float a, float b) { return a + b; }
+    static __device__ __forceinline__ float sub(float a, float b) { return a - b; }
+    static __device__ __forceinline__ float div(float a, float, float rm) { return a * rm; }
+};
 
 // store a value and its periodic halo images (up to 3 extra copies)
 template <class T>

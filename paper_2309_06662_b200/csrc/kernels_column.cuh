@@ -6,6 +6,13 @@
 
 namespace ocn {
 
+// linear equation of state; t, s are the stored (offset) tracers
+template <class T>
+__device__ __forceinline__ T buoyancy(const DevP<T>& P, T t, T s) {
+    typedef Ex<T> E;
+    return E::mul(P.g, E::sub(E::mul(P.alpha, E::sub(t, P.dT0)), E::mul(P.beta_s, E::sub(s, P.dS0))));
+}
+
 // ---------------------------------------------------------------------------------------------
 // S6: one forward-backward barotropic sub-step (DESIGN.md §3.8 step 6): eta first, then U, V
 // with the new eta.  eta is recomputed redundantly for the west and south neighbours so that
@@ -53,12 +60,14 @@ __global__ void __launch_bounds__(256) k_barotropic_finish(const DevP<T> P) {
 }
 
 // ---------------------------------------------------------------------------------------------
-// S4 (back-substitution, bottom-up) + S7 (barotropic correction).  The implicit operator
-// conserves the column integral, so sum_k dz u** = sum_k dz u* (SU from K1) and the correction
-// (Ubar - SU) / Hu is known before the sweep.
+// S4 (back-substitution, top-down) + S7 (barotropic correction) + S9 (hydrostatic pressure of
+// the new T, S, integrated downward from the surface in the same sweep).
+// The implicit operator conserves the column integral, so sum_k dz u** = sum_k dz u* (SU from
+// K1) and the correction (Ubar - SU) / Hu is known before the sweep.
 // ---------------------------------------------------------------------------------------------
 template <class T>
 __global__ void __launch_bounds__(128) k_backsub_correct(const DevP<T> P) {
+    typedef Ex<T> E;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
     if (i >= P.nx || j >= P.ny) return;
@@ -68,31 +77,57 @@ __global__ void __launch_bounds__(128) k_backsub_correct(const DevP<T> P) {
     const int kb = m.x & 255, tx1 = (m.x >> 8) & 255, ty1 = m.y & 255;
     if (tx1 < nz) {
         const T cu = (P.Ub[c] - P.SU[c]) * P.rHu[c];
-        T prev = 0;
-        for (int k = tx1; k < nz; ++k) {
-            const T x = P.du[k * sz + c] + (k > tx1 ? P.e_m[k] * prev : T(0));
-            prev = x;
+        const T* __restrict__ cp = P.cp_m + tx1 * nz;
+        T x = 0;
+        for (int k = nz - 1; k >= tx1; --k) {
+            x = E::sub(P.du[k * sz + c], E::mul(cp[k], x));          // cp[nz-1] = 0
             store_halo(P.u + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, x + cu);
         }
     }
     if (ty1 < nz) {
         const T cv = (P.Vb[c] - P.SV[c]) * P.rHv[c];
-        T prev = 0;
-        for (int k = ty1; k < nz; ++k) {
-            const T x = P.dv[k * sz + c] + (k > ty1 ? P.e_m[k] * prev : T(0));
-            prev = x;
+        const T* __restrict__ cp = P.cp_m + ty1 * nz;
+        T x = 0;
+        for (int k = nz - 1; k >= ty1; --k) {
+            x = E::sub(P.dv[k * sz + c], E::mul(cp[k], x));
             store_halo(P.v + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, x + cv);
         }
     }
     if (kb < nz) {
-        T pt = 0, ps = 0;
-        for (int k = kb; k < nz; ++k) {
-            const T e = k > kb ? P.e_t[k] : T(0);
-            pt = P.dt_[k * sz + c] + e * pt;
-            ps = P.ds[k * sz + c] + e * ps;
-            store_halo(P.t + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, pt);
-            store_halo(P.s + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, ps);
+        const T* __restrict__ cp = P.cp_t + kb * nz;
+        T xt = 0, xs = 0, b1 = 0, pk = 0;
+        for (int k = nz - 1; k >= kb; --k) {
+            const T ck = cp[k];
+            xt = E::sub(P.dt_[k * sz + c], E::mul(ck, xt));
+            xs = E::sub(P.ds[k * sz + c], E::mul(ck, xs));
+            store_halo(P.t + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, xt);
+            store_halo(P.s + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, xs);
+            const T b0 = buoyancy(P, xt, xs);
+            pk = k == nz - 1 ? -E::mul(b0, P.hz_top)
+                             : E::sub(pk, E::mul(E::mul(T(0.5), E::add(b1, b0)), P.dzc[k + 1]));
+            b1 = b0;
+            store_halo(P.p + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, pk);
         }
+    }
+}
+
+// S9 alone (ocn_set_fields): hydrostatic pressure of the current T, S
+template <class T>
+__global__ void __launch_bounds__(128) k_pressure(const DevP<T> P) {
+    typedef Ex<T> E;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    if (i >= P.nx || j >= P.ny) return;
+    const int sx = P.sx, nz = P.nz;
+    const long long sz = P.sz, c = (long long)(j + OCN_HALO) * sx + i;
+    const int kb = P.m8[c].x & 255;
+    T b1 = 0, pk = 0;
+    for (int k = nz - 1; k >= kb; --k) {
+        const T b0 = buoyancy(P, P.t[k * sz + c], P.s[k * sz + c]);
+        pk = k == nz - 1 ? -E::mul(b0, P.hz_top)
+                         : E::sub(pk, E::mul(E::mul(T(0.5), E::add(b1, b0)), P.dzc[k + 1]));
+        b1 = b0;
+        store_halo(P.p + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, pk);
     }
 }
 
@@ -132,7 +167,7 @@ __global__ void __launch_bounds__(128) k_init_transport(const DevP<T> P) {
 
 // ---------------------------------------------------------------------------------------------
 // scatter (contiguous interior -> halo'd plane layout, masked) and gather (back, land = 0)
-// kind: 0 u, 1 v, 2 T (offset T0), 3 S (offset S0), 4 eta, 5 plain 2-D, 6 w (nz+1 levels, gather only)
+// kind: 0 u, 1 v, 2 T (offset Toff), 3 S (offset Soff), 4 eta, 5 plain 2-D, 6 w (nz+1 levels, gather only)
 // ---------------------------------------------------------------------------------------------
 template <class T>
 __device__ __forceinline__ bool cell_open(const DevP<T>& P, long long c, int k, int kind) {
@@ -154,7 +189,7 @@ __global__ void __launch_bounds__(256) k_scatter(const DevP<T> P, T* __restrict_
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
     if (i >= P.nx || j >= P.ny) return;
     const long long c = (long long)(j + OCN_HALO) * P.sx + i;
-    const T off = kind == 2 ? P.T0 : kind == 3 ? P.S0 : T(0);
+    const T off = kind == 2 ? P.Toff : kind == 3 ? P.Soff : T(0);
     for (int k = blockIdx.z; k < nl; k += gridDim.z) {
         const T v = cell_open(P, c, k, kind) ? src[((long long)k * P.ny + j) * P.nx + i] - off : T(0);
         store_halo(dst + k * P.sz, P.sx, P.nx, P.ny, P.px, P.py, j, i, v);
@@ -168,7 +203,7 @@ __global__ void __launch_bounds__(256) k_gather(const DevP<T> P, O* __restrict__
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
     if (i >= P.nx || j >= P.ny) return;
     const long long c = (long long)(j + OCN_HALO) * P.sx + i;
-    const T off = kind == 2 ? P.T0 : kind == 3 ? P.S0 : T(0);
+    const T off = kind == 2 ? P.Toff : kind == 3 ? P.Soff : T(0);
     for (int k = blockIdx.z; k < nl; k += gridDim.z) {
         const T v = cell_open(P, c, k, kind) ? src[k * P.sz + c] + off : T(0);
         dst[((long long)k * P.ny + j) * P.nx + i] = (O)v;

@@ -93,7 +93,7 @@ ocn_status build_model(ocn_model* M) {
     auto plane = [&](size_t n, T** out) -> ocn_status {
         return dev_alloc(M, n, out, true);
     };
-    T** f3[] = {&P.u, &P.v, &P.t, &P.s, &P.du, &P.dv, &P.dt_, &P.ds, &P.Gu, &P.Gv, &P.Gt, &P.Gs};
+    T** f3[] = {&P.u, &P.v, &P.t, &P.s, &P.p, &P.du, &P.dv, &P.dt_, &P.ds, &P.Gu, &P.Gv, &P.Gt, &P.Gs};
     for (T** f : f3) if ((s = plane(n3, f)) != OCN_OK) return s;
     if ((s = plane(n3 + n2, &P.w)) != OCN_OK) return s;
     T** f2[] = {&P.eta[0], &P.eta[1], &P.U[0], &P.U[1], &P.V[0], &P.V[1], &P.etab, &P.Ub, &P.Vb, &P.GU, &P.GV,
@@ -119,29 +119,37 @@ ocn_status build_model(ocn_model* M) {
         return s;
     P.dy = (T)g->dy; P.rdy = (T)(1.0 / g->dy);
     P.hz_top = (T)(g->zf[nz] - g->zc[nz - 1]);
-    // top-down Thomas tables
+    // Thomas tables: bottom-up elimination started at the column's first open
+    // level kf; sub-diagonal sm[k], and per (kf, k) the pivot m, its reciprocal and the modified
+    // super-diagonal cp, computed in fp64 exactly as the equations of DESIGN.md §3.8 step 4 are written
     for (int pass = 0; pass < 2; ++pass) {
         const double dtk = M->d.dt * (pass == 0 ? M->d.nu_z : M->d.kappa_z);
-        std::vector<double> sp(nz, 0.0), e(nz, 0.0), im(nz, 1.0), imb(nz, 1.0);
-        double e_above = 0.0;
-        for (int k = nz - 1; k >= 0; --k) {
-            const double s_up = (k <= nz - 2) ? dtk / (g->dz[k] * g->dzc[k + 1]) : 0.0;
-            const double s_dn = (k >= 1) ? dtk / (g->dz[k] * g->dzc[k]) : 0.0;
-            const double m = 1.0 + s_up + s_dn - s_up * e_above;
-            const double mb = 1.0 + s_up - s_up * e_above;
-            sp[k] = s_up; im[k] = 1.0 / m; imb[k] = 1.0 / mb; e[k] = s_dn / m;
-            e_above = e[k];
+        std::vector<double> sm(nz, 0.0), cp((size_t)nz * nz, 0.0), mm((size_t)nz * nz, 1.0), rm((size_t)nz * nz, 1.0);
+        for (int k = 1; k < nz; ++k) sm[k] = dtk / (g->dz[k] * g->dzc[k]);
+        for (int kf = 0; kf < nz; ++kf) {
+            double cprev = 0.0;
+            for (int k = kf; k < nz; ++k) {
+                const double sp = (k + 1 <= nz - 1) ? dtk / (g->dz[k] * g->dzc[k + 1]) : 0.0;
+                const double smk = (k > kf) ? sm[k] : 0.0;
+                const double b = 1.0 + sp + smk;
+                const double lo = -smk, up = -sp;
+                const double m = (k == kf) ? b : b - lo * cprev;
+                cprev = up / m;
+                cp[(size_t)kf * nz + k] = cprev; mm[(size_t)kf * nz + k] = m; rm[(size_t)kf * nz + k] = 1.0 / m;
+            }
         }
         if (pass == 0) {
-            if ((s = upload(M, sp, &P.sp_m)) != OCN_OK || (s = upload(M, e, &P.e_m)) != OCN_OK ||
-                (s = upload(M, im, &P.im_m)) != OCN_OK || (s = upload(M, imb, &P.imb_m)) != OCN_OK) return s;
+            if ((s = upload(M, sm, &P.sm_m)) != OCN_OK || (s = upload(M, cp, &P.cp_m)) != OCN_OK ||
+                (s = upload(M, mm, &P.m_m)) != OCN_OK || (s = upload(M, rm, &P.rm_m)) != OCN_OK) return s;
         } else {
-            if ((s = upload(M, sp, &P.sp_t)) != OCN_OK || (s = upload(M, e, &P.e_t)) != OCN_OK ||
-                (s = upload(M, im, &P.im_t)) != OCN_OK || (s = upload(M, imb, &P.imb_t)) != OCN_OK) return s;
+            if ((s = upload(M, sm, &P.sm_t)) != OCN_OK || (s = upload(M, cp, &P.cp_t)) != OCN_OK ||
+                (s = upload(M, mm, &P.m_t)) != OCN_OK || (s = upload(M, rm, &P.rm_t)) != OCN_OK) return s;
         }
     }
     P.dt = (T)M->d.dt; P.g = (T)M->d.g; P.alpha = (T)M->d.alpha; P.beta_s = (T)M->d.beta_s;
-    P.T0 = (T)M->d.T0; P.S0 = (T)M->d.S0; P.rrho0 = (T)(1.0 / M->d.rho0);
+    P.Toff = sizeof(T) == 4 ? (T)M->d.T0 : T(0); P.Soff = sizeof(T) == 4 ? (T)M->d.S0 : T(0);
+    P.dT0 = (T)(M->d.T0 - (double)P.Toff); P.dS0 = (T)(M->d.S0 - (double)P.Soff);
+    P.rrho0 = (T)(1.0 / M->d.rho0);
     P.nu_h = (T)M->d.nu_h; P.kappa_h = (T)M->d.kappa_h; P.dtau = (T)M->dtau;
     // Hu, Hv = sum_k dz over open faces, and reciprocals
     {
@@ -249,6 +257,7 @@ ocn_status set_fields_t(ocn_model* M, const ocn_fields* f) {
         const dim3 bc(32, 4);
         ocn::k_init_transport<T><<<grid2(M->g, bc), bc, 0, M->stream>>>(P);
         ocn::k_vertical_velocity<T><<<grid2(M->g, bc), bc, 0, M->stream>>>(P);
+        ocn::k_pressure<T><<<grid2(M->g, bc), bc, 0, M->stream>>>(P);
         CK(cudaGetLastError());
         M->have_history = false;
     }

@@ -59,15 +59,10 @@ def test_first_step_tendencies_match():
     G = ref.tendencies()
     gpu.time_step(1)
     d = gpu.debug()                                          # G^{n-1} after one step = G of the initial state
-    # tracers are carried as offsets from (T0, S0): G differs by the exact top-cell source
-    w_top = ref.get_fields()["w"][-1]
-    dz_top = np.diff(wl["z_faces"])[-1]
-    G["GT"][-1] -= 0.0                                       # oracle G_T is for the full tracer
     for n in ("Gu", "Gv"):
         assert rel_linf(d[n], G[n]) < 1e-12, n
-    gt = d["GT"].copy(); gt[-1] -= wl["params"]["T0"] * w_top / dz_top
-    gs = d["GS"].copy(); gs[-1] -= wl["params"]["S0"] * w_top / dz_top
-    assert rel_linf(gt, G["GT"]) < 1e-10 and rel_linf(gs, G["GS"]) < 1e-10
+    # fp64 carries the full tracers (offsets are an fp32-only storage transform)
+    assert rel_linf(d["GT"], G["GT"]) < 1e-12 and rel_linf(d["GS"], G["GS"]) < 1e-12
 
 
 def test_config0_fp64_10_steps():
