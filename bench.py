@@ -1,0 +1,361 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the hydrostatic free-surface time step (libocn) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
+
+One "step" is one baroclinic time step = the whole hot path over the
+seeded synthetic workload of BASELINE.json config C (default 4: 2880x1200x100 near-global
+lat-lon grid, fp32, 40 barotropic sub-steps — the configuration the metric is quoted on).
+Prints ONE JSON line (rank 0): cell-updates/s (all grid cells, land included — the paper's
+"grid size" convention), SYPD-equivalent, per-stage device times, the HBM
+roofline of the dominant kernel, the end-to-end number through the C ABI with host buffers,
+and the CPU oracle timed on this box's host cores as a reported baseline.
+
+N > 1 (torchrun): the path does not shard in this round ("replicas only"): every
+rank steps an independent replica of the same workload on its own GPU, no data-path collective;
+time = max over ranks, value = N x cells x K / time, scaling "weak".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "cell_updates_per_s"
+UNIT = "cell-updates/s"
+# algorithmic HBM words per wet cell-update of each stage: compulsory reads + writes
+STAGE_WORDS = {"tendency": 18, "backsub_correct_pressure": 9, "vertical_velocity": 3}
+# window of config 4 the oracle is timed on: (j0, j1, i0, i1)
+CPU_WINDOW = (500, 700, 1300, 1700)
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-e2e", action="store_true", help="skip the end-to-end (host buffer) leg")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    return ap.parse_args()
+
+
+def workload_name(wl):
+    g = wl["grid"]
+    return "%s %dx%dx%d fp%d M=%d dt=%gs" % (wl["name"], g["nx"], g["ny"], g["nz"], wl["params"]["precision"],
+                                             wl["params"]["substeps"], wl["params"]["dt"])
+
+
+def sypd(dt, sec_per_step):
+    return dt / (365.0 * sec_per_step)          # the paper's year is 365 d
+
+
+# ---------------------------------------------------------------------------------------------
+# CPU oracle leg (cpu_baseline and --impl reference)
+# ---------------------------------------------------------------------------------------------
+def oracle_sample(config):
+    from paper_2309_06662_b200 import workloads as W
+    if config == 4:
+        wl = W.config4(window=CPU_WINDOW, steps=1)
+        what = "config 4 window j=%d:%d i=%d:%d (closed box, identical physics)" % CPU_WINDOW
+    elif config in (2, 3):
+        wl = W.make(config, window=(200, 400, 500, 900), steps=1)
+        what = "config %d window j=200:400 i=500:900 (closed box)" % config
+    else:
+        wl = W.make(config)
+        what = "config %d full size" % config
+    return wl, what
+
+
+def time_oracle(config, steps, warmup):
+    import oracle
+    oracle.build()
+    wl, what = oracle_sample(config)
+    g = wl["grid"]
+    cells = g["nx"] * g["ny"] * g["nz"]
+    ref = oracle.RefModel(wl)
+    ref.step(max(1, warmup))                     # Euler start + AB2 warm-up
+    t0 = time.perf_counter()
+    ref.step(steps)
+    dt = time.perf_counter() - t0
+    return dict(value=cells * steps / dt, sec_per_step=dt / steps, cores=oracle.num_threads(), cells=cells,
+                sample="%s: %dx%dx%d cells, %d steps after %d warm-up" % (what, g["nx"], g["ny"], g["nz"], steps,
+                                                                         max(1, warmup)),
+                dt_model=wl["params"]["dt"], name=workload_name(wl))
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    steps = min(args.steps, 3) if args.config >= 2 else args.steps
+    r = time_oracle(args.config, steps, min(args.warmup, 2))
+    line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": steps, "warmup": min(args.warmup, 2), "ms_per_step": 1e3 * r["sec_per_step"],
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": r["name"], "sample": r["sample"]},
+            "sypd_equivalent_of_sample": sypd(r["dt_model"], r["sec_per_step"]),
+            "cpu_baseline": {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle",
+                             "sample": r["sample"]},
+            "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ---------------------------------------------------------------------------------------------
+# clocks during the timed region (B200_PROFILING.md recipe)
+# ---------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, device):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(device), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except OSError:
+            pass
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for ln in self.f.read().splitlines():
+            c = [x.strip() for x in ln.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1])); mx.append(float(c[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, c[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        self.f.close()
+        os.unlink(self.f.name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def measured_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, torch copy_)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(workload, kernel):
+    """DRAM bytes per launch of `kernel` from the committed ncu --set full capture, if it was taken
+    on this workload (profiles/traffic.json, written by hand from the capture's raw page)."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            t = json.load(f)
+        e = t.get(kernel)
+        if e and e.get("workload") == workload:
+            return float(e["dram_bytes_per_launch"])
+    except Exception:
+        pass
+    return None
+
+
+# ---------------------------------------------------------------------------------------------
+# the CUDA arm
+# ---------------------------------------------------------------------------------------------
+def wet_cells(model):
+    import ctypes as C
+    from paper_2309_06662_b200 import ocn
+    wet = np.zeros((model.nz, model.ny, model.nx), np.uint8)
+    rc = ocn.lib().ocn_get_masks(model.grid.h, C.c_void_p(wet.ctypes.data), None, None, None, None, None)
+    assert rc == 0
+    return int(wet.sum(dtype=np.int64))
+
+
+def run_ours(args):
+    import torch
+    from paper_2309_06662_b200 import build as ocn_build
+    from paper_2309_06662_b200 import ocn, workloads as W
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (libocn has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        ocn_build.build()
+    if dist is not None:
+        dist.barrier()
+
+    K, Wm = args.steps, max(args.warmup, 3)
+    wl = W.make(args.config)
+    g, prm = wl["grid"], wl["params"]
+    nx, ny, nz = g["nx"], g["ny"], g["nz"]
+    cells = nx * ny * nz
+    np_dtype = np.float32 if prm["precision"] == 32 else np.float64
+    t_dtype = torch.float32 if prm["precision"] == 32 else torch.float64
+    stream = torch.cuda.Stream(device=local)
+    model = ocn.Model(wl, device=local, stream=stream.cuda_stream)
+    nwet = wet_cells(model)
+    info = model.info()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    def max_over_ranks(x):
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    # ---- device-resident timing: K steps of the production path (one CUDA graph launch per step) ----
+    model.time_step(Wm)
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    clocks = ClockSampler(local)
+    barrier()
+    e0.record(stream)
+    model.time_step(K)
+    e1.record(stream)
+    barrier()
+    ms_total = max_over_ranks(e0.elapsed_time(e1))
+    # ---- same K steps again with an event between stages: per-kernel durations for the roofline ----
+    model.profile_enable(True)
+    model.time_step(1)
+    model.profile_read(reset=True)
+    model.time_step(K)
+    stages = model.profile_read(reset=True)
+    model.profile_enable(False)
+    clk = clocks.stop()
+    sec_per_step = ms_total * 1e-3 / K
+    value = world * cells * K / (ms_total * 1e-3)
+
+    # finite check of the state the timed steps produced (d2h of eta only)
+    eta = model.get_fields(names=("eta",))["eta"]
+    assert np.isfinite(eta).all(), "non-finite eta after the timed steps"
+
+    # ---- roofline of the dominant kernel ----
+    peak, peak_src = measured_peak()
+    word = 4 if prm["precision"] == 32 else 8
+    dom = max(stages, key=lambda s: stages[s]["ms"])
+    words = STAGE_WORDS.get(dom)
+    roof = None
+    stage_out = {}
+    for s, v in stages.items():
+        stage_out[s] = {"ms_per_step": v["ms"] / K, "launches_per_step": v["launches"] / K}
+        if s in STAGE_WORDS:
+            stage_out[s]["algorithmic_gbs"] = STAGE_WORDS[s] * word * nwet / (v["ms"] / K * 1e-3) / 1e9
+    if words is not None:
+        alg_bytes = words * word * nwet
+        ach = alg_bytes / (stages[dom]["ms"] / K * 1e-3) / 1e9
+        roof = {"kernel": dom, "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
+                "bytes_per_wet_cell": words * word, "traffic": ncu_traffic(workload_name(wl), dom)}
+    else:                       # the 2-D sub-cycle dominates (tiny 3-D grids): 16 words per column per sub-step
+        ncol = nx * ny
+        alg_bytes = 16 * word * ncol * prm["substeps"]
+        ach = alg_bytes / (stages[dom]["ms"] / K * 1e-3) / 1e9
+        roof = {"kernel": dom, "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes, "traffic": None}
+
+    # ---- end to end through the C ABI with HOST (pinned) buffers ----
+    e2e = None
+    if not args.no_e2e:
+        f = wl["fields"]
+        pin = {k: torch.from_numpy(np.ascontiguousarray(f[k], dtype=np_dtype)).pin_memory()
+               for k in ("u", "v", "T", "S", "eta", "tau_x", "tau_y")}
+        out = {k: torch.empty(pin[k].shape, dtype=t_dtype).pin_memory() for k in ("u", "v", "T", "S", "eta")}
+        out["w"] = torch.empty((nz + 1, ny, nx), dtype=t_dtype).pin_memory()
+        eta_step = torch.empty((ny, nx), dtype=t_dtype).pin_memory()
+        Ke = K
+        def e2e_job():
+            model.set_fields_ptr(**{k: pin[k].data_ptr() for k in ("u", "v", "T", "S", "eta", "tau_x", "tau_y")})
+            for _ in range(Ke):
+                model.set_fields_ptr(tau_x=pin["tau_x"].data_ptr(), tau_y=pin["tau_y"].data_ptr())   # per-step forcing
+                model.time_step(1)
+                model.get_fields_ptr(eta=eta_step.data_ptr())                                        # per-step result
+            model.get_fields_ptr(**{k: out[k].data_ptr() for k in out})
+        e2e_job()                                   # warm-up (also re-creates the AB2 start)
+        barrier()
+        t0 = time.perf_counter()
+        e0.record(stream)
+        e2e_job()
+        e1.record(stream)
+        barrier()
+        wall = time.perf_counter() - t0
+        ms_e = max_over_ranks(max(e0.elapsed_time(e1), wall * 1e3))
+        b2 = ny * nx * word
+        h2d = (4 * cells * word + 3 * b2) / Ke + 2 * b2
+        d2h = (4 * cells * word + (nz + 1) * b2 + b2) / Ke + b2
+        e2e = {"value": world * cells * Ke / (ms_e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": d2h, "steps": Ke,
+               "what": "ocn_set_fields(full state, pinned host) + per step [ocn_set_fields(tau) + ocn_time_step(1) "
+                       "+ ocn_get_fields(eta)] + ocn_get_fields(full state + w); state transfers amortised over the steps"}
+        del pin, out
+    model.close()
+
+    # ---- CPU oracle on this box's host cores (rank 0, N = 1 only) ----
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        r = time_oracle(args.config, 3 if args.config >= 2 else 5, 1)
+        cpu = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"]}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+                "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f32" if prm["precision"] == 32 else "f64", "data": "synthetic",
+                "config": {"workload": workload_name(wl), "cells": cells, "wet_cells": nwet,
+                           "l2": "working set %.1f GB >> 126 MB L2 (no flush needed)" % (info["device_bytes"] / 1e9)
+                                 if info["device_bytes"] > 1e9 else "working set fits L2 (launch/latency bound; roofline n/a)",
+                           "parallelism": "replicas x%d" % world},
+                "sypd_equivalent": sypd(prm["dt"], sec_per_step),
+                "wet_cell_updates_per_s": world * nwet * K / (ms_total * 1e-3),
+                "stages": stage_out, "roofline": roof, "e2e": e2e, "cpu_baseline": cpu,
+                "gpu_launches": info["launches_per_step"] * K, "clocks": clk,
+                "device_bytes": info["device_bytes"]}
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -44,6 +44,12 @@ struct ocn_model {
     void* stage = nullptr;              // contiguous staging buffer, (nz+1)*ny*nx doubles
     cudaGraphExec_t graph = nullptr;    // one steady-state (AB2) step
     int launches_per_step = 0;
+    // per-stage timing (ocn_profile_*)
+    bool profiling = false;
+    std::vector<cudaEvent_t> ev_pool;   // OCN_NSTAGES + 1 events per profiled step
+    size_t ev_used = 0;
+    double prof_ms[OCN_NSTAGES] = {0, 0, 0, 0};
+    long long prof_launches[OCN_NSTAGES] = {0, 0, 0, 0};
 };
 
 namespace {
@@ -183,21 +189,58 @@ ocn_status build_model(ocn_model* M) {
 // =================================================================================================
 namespace {
 
+ocn_status prof_flush(ocn_model* M) {           // fold recorded events into the per-stage totals
+    if (M->ev_used == 0) return OCN_OK;
+    CK(cudaStreamSynchronize(M->stream));
+    for (size_t q = 0; q + OCN_NSTAGES < M->ev_used + 1 && q < M->ev_used; q += OCN_NSTAGES + 1)
+        for (int s = 0; s < OCN_NSTAGES; ++s) {
+            float ms = 0.f;
+            CK(cudaEventElapsedTime(&ms, M->ev_pool[q + s], M->ev_pool[q + s + 1]));
+            M->prof_ms[s] += ms;
+        }
+    M->ev_used = 0;
+    return OCN_OK;
+}
+
+ocn_status prof_mark(ocn_model* M) {
+    if (!M->profiling) return OCN_OK;
+    if (M->ev_used == M->ev_pool.size()) {
+        cudaEvent_t e;
+        CK(cudaEventCreate(&e));
+        M->ev_pool.push_back(e);
+    }
+    CK(cudaEventRecord(M->ev_pool[M->ev_used++], M->stream));
+    return OCN_OK;
+}
+
 template <class T>
 ocn_status launch_step(ocn_model* M, bool euler) {
     const ocn_grid* g = M->g;
+    ocn_status ps;
+    if (M->profiling && M->ev_used + OCN_NSTAGES + 1 > 4096 && (ps = prof_flush(M)) != OCN_OK) return ps;
+#define MARK(stage, n)                                                   \
+    do {                                                                 \
+        if ((ps = prof_mark(M)) != OCN_OK) return ps;                    \
+        if (M->profiling && (stage) >= 0) M->prof_launches[stage] += (n); \
+    } while (0)
     const ocn::DevP<T>& P = params<T>(M);
     const T c0 = euler ? T(1) : (T)(1.5 + M->d.chi), c1 = euler ? T(0) : (T)(0.5 + M->d.chi);
     const dim3 bc(32, 4), b2(32, 8);
+    MARK(-1, 0);
     ocn::k_tendency<T><<<grid2(g, bc), bc, 0, M->stream>>>(P, c0, c1);
+    MARK(0, 1);
     int cur = 0;
     for (int m = 1; m <= M->d.substeps; ++m) {
         ocn::k_barotropic<T><<<grid2(g, b2), b2, 0, M->stream>>>(P, cur, (T)M->a_w[m - 1], m == 1 ? 1 : 0);
         cur ^= 1;
     }
     ocn::k_barotropic_finish<T><<<grid2(g, b2), b2, 0, M->stream>>>(P);
+    MARK(1, M->d.substeps + 1);
     ocn::k_backsub_correct<T><<<grid2(g, bc), bc, 0, M->stream>>>(P);
+    MARK(2, 1);
     ocn::k_vertical_velocity<T><<<grid2(g, bc), bc, 0, M->stream>>>(P);
+    MARK(3, 1);
+#undef MARK
     CK(cudaGetLastError());
     return OCN_OK;
 }
@@ -210,6 +253,10 @@ ocn_status run_steps(ocn_model* M, int n) {
         M->have_history = true; --n;
     }
     if (n <= 0) return OCN_OK;
+    if (M->profiling) {                           // direct launches with stage events
+        for (int q = 0; q < n; ++q) if ((s = launch_step<T>(M, false)) != OCN_OK) return s;
+        return OCN_OK;
+    }
     if (!M->graph) {                              // capture one steady-state step once
         cudaGraph_t gr = nullptr;
         CK(cudaStreamBeginCapture(M->stream, cudaStreamCaptureModeThreadLocal));
@@ -408,6 +455,7 @@ ocn_status ocn_model_destroy(ocn_model* M) {
     cudaSetDevice(M->d.device);
     if (M->stream) cudaStreamSynchronize(M->stream);
     if (M->graph) cudaGraphExecDestroy(M->graph);
+    for (cudaEvent_t e : M->ev_pool) cudaEventDestroy(e);
     for (void* p : M->allocs) cudaFree(p);
     if (M->stage) cudaFree(M->stage);
     if (M->own_stream && M->stream) cudaStreamDestroy(M->stream);
@@ -445,6 +493,32 @@ ocn_status ocn_model_info(const ocn_model* M, int* launches, unsigned long long*
     if (launches) *launches = M->launches_per_step;
     if (bytes) *bytes = M->bytes;
     return OCN_OK;
+}
+
+ocn_status ocn_profile_enable(ocn_model* M, int on) {
+    if (!M) return fail(OCN_EINVAL, "null model");
+    CK(cudaSetDevice(M->d.device));
+    if (!on) { const ocn_status s = prof_flush(M); if (s != OCN_OK) return s; }
+    M->profiling = on != 0;
+    return OCN_OK;
+}
+
+ocn_status ocn_profile_read(ocn_model* M, double* ms, long long* launches, int reset) {
+    if (!M) return fail(OCN_EINVAL, "null model");
+    CK(cudaSetDevice(M->d.device));
+    const ocn_status s = prof_flush(M);
+    if (s != OCN_OK) return s;
+    for (int q = 0; q < OCN_NSTAGES; ++q) {
+        if (ms) ms[q] = M->prof_ms[q];
+        if (launches) launches[q] = M->prof_launches[q];
+        if (reset) { M->prof_ms[q] = 0; M->prof_launches[q] = 0; }
+    }
+    return OCN_OK;
+}
+
+const char* ocn_stage_name(int stage) {
+    static const char* names[OCN_NSTAGES] = {"tendency", "barotropic", "backsub_correct_pressure", "vertical_velocity"};
+    return (stage >= 0 && stage < OCN_NSTAGES) ? names[stage] : "";
 }
 
 ocn_status ocn_get_debug(ocn_model* M, double* Gu, double* Gv, double* GT, double* GS, double* U, double* V) {

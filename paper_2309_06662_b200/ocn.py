@@ -40,7 +40,9 @@ class ocn_fields(C.Structure):
 
 EXPORTS = ["ocn_grid_create", "ocn_grid_destroy", "ocn_model_create", "ocn_model_destroy", "ocn_set_fields",
            "ocn_time_step", "ocn_get_fields", "ocn_synchronize", "ocn_get_masks", "ocn_model_info",
-           "ocn_get_debug", "ocn_last_error", "ocn_version"]
+           "ocn_get_debug", "ocn_last_error", "ocn_version", "ocn_profile_enable", "ocn_profile_read",
+           "ocn_stage_name"]
+NSTAGES = 4
 
 
 def lib():
@@ -64,6 +66,10 @@ def lib():
         L.ocn_get_masks.argtypes = [vp] + [vp] * 6
         L.ocn_model_info.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_ulonglong)]
         L.ocn_get_debug.argtypes = [vp] + [vp] * 6
+        L.ocn_profile_enable.argtypes = [vp, C.c_int]
+        L.ocn_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong), C.c_int]
+        L.ocn_stage_name.restype = C.c_char_p
+        L.ocn_stage_name.argtypes = [C.c_int]
         _lib = L
     return _lib
 
@@ -157,6 +163,15 @@ class Model:
         n, b = C.c_int(), C.c_ulonglong()
         _check(lib().ocn_model_info(self.h, C.byref(n), C.byref(b)))
         return dict(launches_per_step=n.value, device_bytes=b.value)
+
+    def profile_enable(self, on=True):
+        _check(lib().ocn_profile_enable(self.h, int(bool(on))))
+
+    def profile_read(self, reset=True):
+        ms = (C.c_double * NSTAGES)()
+        n = (C.c_longlong * NSTAGES)()
+        _check(lib().ocn_profile_read(self.h, ms, n, int(bool(reset))))
+        return {lib().ocn_stage_name(q).decode(): dict(ms=ms[q], launches=n[q]) for q in range(NSTAGES)}
 
     def debug(self):
         nz, ny, nx = self.nz, self.ny, self.nx
