@@ -34,7 +34,7 @@ if ROOT not in sys.path:
 METRIC = "cell_updates_per_s"
 UNIT = "cell-updates/s"
 # algorithmic HBM words per wet cell-update of each stage: compulsory reads + writes
-STAGE_WORDS = {"tendency": 18, "backsub_correct_pressure": 9, "vertical_velocity": 3}
+STAGE_WORDS = {"tendency": 17, "backsub_correct_pressure": 9}
 # window of config 4 the oracle is timed on: (j0, j1, i0, i1)
 CPU_WINDOW = (500, 700, 1300, 1700)
 

@@ -2,9 +2,12 @@
 //
 // Layout: every 3-D field is [k][j][i] with i fastest, a physical halo of 3
 // cells in i and j, row pitch sx = roundup(nx + 6, 32) elements, and the base pointer shifted so
-// that element (k, j, i = 0) of every row starts a 128-byte line.  2-D fields use the same
-// plane layout (one level).  Halos of periodic directions mirror the interior (written by the
-// producing kernel through store_halo); halos of bounded directions are zero forever (solid wall).
+// that element (k, j, i = 0) of every row starts a 128-byte line.  The prognostic groups are
+// stored interleaved, one element = a pair: uv = (u, v), ts = (T, S), and likewise their AB2
+// history G and eliminated right-hand sides d, so that one 8/16-byte access moves both members
+// and the tracer pair shares one set of WENO weights' worth of index arithmetic.  2-D fields use
+// the same plane layout (one level).  Halos of periodic directions mirror the interior (written
+// by the producing kernel through store_halo); halos of bounded directions are zero forever.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -13,16 +16,24 @@
 
 namespace ocn {
 
+template <class T> struct Pair;
+template <> struct Pair<float> { typedef float2 type; };
+template <> struct Pair<double> { typedef double2 type; };
+template <class T> __device__ __forceinline__ typename Pair<T>::type mk2(T a, T b) { typename Pair<T>::type r; r.x = a; r.y = b; return r; }
+
 template <class T>
 struct DevP {
+    typedef typename Pair<T>::type T2;
     int nx, ny, nz;
     int sx, sy;            // plane pitch / rows (with halo)
     long long sz;          // level stride = sx * sy
     int px, py;            // periodic flags
-    // prognostic state (time level n), w diagnostic, forward-eliminated right-hand sides, AB2 history
-    T *u, *v, *t, *s, *w, *p;
-    T *du, *dv, *dt_, *ds;
-    T *Gu, *Gv, *Gt, *Gs;
+    // prognostic state (time level n) as pairs, stored pressure, w (filled on demand for
+    // ocn_get_fields), eliminated right-hand sides, AB2 history
+    T2 *uv, *ts;
+    T *p, *w;
+    T2 *duv, *dts;
+    T2 *Guv, *Gts;
     // 2-D (plane layout with halo)
     T *eta[2], *U[2], *V[2];       // barotropic state, double buffered inside the sub-cycle
     T *etab, *Ub, *Vb;             // weighted running averages
@@ -72,27 +83,29 @@ template <> struct Ex<float> {
     static __device__ __forceinline__ float div(float a, float, float rm) { return a * rm; }
 };
 
-// store a value and its periodic halo images (up to 3 extra copies)
+// store a value and its periodic halo images (up to 3 extra copies); T may be a pair type
 template <class T>
 __device__ __forceinline__ void store_halo(T* __restrict__ plane, int sx, int nx, int ny, int px, int py,
-                                           int j, int i, T val) {
-    T* p = plane + (long long)(j + OCN_HALO) * sx + i;
+                                           int j, int i, T val, int st = 1) {
+    // st: element stride of the plane (2 when addressing one member of a pair array as scalars)
+    T* p = plane + ((long long)(j + OCN_HALO) * sx + i) * st;
     *p = val;
+    const long long row = (long long)sx * st;
     int di = 0, dj = 0;
     if (px) { if (i < OCN_HALO) di = nx; else if (i >= nx - OCN_HALO) di = -nx; }
     if (py) { if (j < OCN_HALO) dj = ny; else if (j >= ny - OCN_HALO) dj = -ny; }
-    if (di) p[di] = val;
-    if (dj) p[(long long)dj * sx] = val;
-    if (di && dj) p[(long long)dj * sx + di] = val;
+    if (di) p[di * st] = val;
+    if (dj) p[dj * row] = val;
+    if (di && dj) p[dj * row + di * st] = val;
     // very small periodic domains (n < 6): a cell can be the image of both halos
     if (px && nx < 2 * OCN_HALO) {
-        if (i < OCN_HALO && i >= nx - OCN_HALO) { p[-nx] = val; if (dj) p[(long long)dj * sx - nx] = val; }
+        if (i < OCN_HALO && i >= nx - OCN_HALO) { p[-nx * st] = val; if (dj) p[dj * row - nx * st] = val; }
     }
     if (py && ny < 2 * OCN_HALO) {
         if (j < OCN_HALO && j >= ny - OCN_HALO) {
-            p[-(long long)ny * sx] = val;
-            if (di) p[-(long long)ny * sx + di] = val;
-            if (px && nx < 2 * OCN_HALO && i < OCN_HALO && i >= nx - OCN_HALO) p[-(long long)ny * sx - nx] = val;
+            p[-ny * row] = val;
+            if (di) p[-ny * row + di * st] = val;
+            if (px && nx < 2 * OCN_HALO && i < OCN_HALO && i >= nx - OCN_HALO) p[-ny * row - nx * st] = val;
         }
     }
 }

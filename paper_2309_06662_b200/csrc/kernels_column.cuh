@@ -68,6 +68,7 @@ __global__ void __launch_bounds__(256) k_barotropic_finish(const DevP<T> P) {
 template <class T>
 __global__ void __launch_bounds__(128) k_backsub_correct(const DevP<T> P) {
     typedef Ex<T> E;
+    typedef typename Pair<T>::type T2;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
     if (i >= P.nx || j >= P.ny) return;
@@ -75,38 +76,32 @@ __global__ void __launch_bounds__(128) k_backsub_correct(const DevP<T> P) {
     const long long sz = P.sz, c = (long long)(j + OCN_HALO) * sx + i;
     const uint2 m = P.m8[c];
     const int kb = m.x & 255, tx1 = (m.x >> 8) & 255, ty1 = m.y & 255;
-    if (tx1 < nz) {
-        const T cu = (P.Ub[c] - P.SU[c]) * P.rHu[c];
-        const T* __restrict__ cp = P.cp_m + tx1 * nz;
-        T x = 0;
-        for (int k = nz - 1; k >= tx1; --k) {
-            x = E::sub(P.du[k * sz + c], E::mul(cp[k], x));          // cp[nz-1] = 0
-            store_halo(P.u + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, x + cu);
-        }
-    }
-    if (ty1 < nz) {
-        const T cv = (P.Vb[c] - P.SV[c]) * P.rHv[c];
-        const T* __restrict__ cp = P.cp_m + ty1 * nz;
-        T x = 0;
-        for (int k = nz - 1; k >= ty1; --k) {
-            x = E::sub(P.dv[k * sz + c], E::mul(cp[k], x));
-            store_halo(P.v + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, x + cv);
-        }
-    }
-    if (kb < nz) {
-        const T* __restrict__ cp = P.cp_t + kb * nz;
-        T xt = 0, xs = 0, b1 = 0, pk = 0;
-        for (int k = nz - 1; k >= kb; --k) {
-            const T ck = cp[k];
-            xt = E::sub(P.dt_[k * sz + c], E::mul(ck, xt));
-            xs = E::sub(P.ds[k * sz + c], E::mul(ck, xs));
-            store_halo(P.t + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, xt);
-            store_halo(P.s + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, xs);
-            const T b0 = buoyancy(P, xt, xs);
-            pk = k == nz - 1 ? -E::mul(b0, P.hz_top)
-                             : E::sub(pk, E::mul(E::mul(T(0.5), E::add(b1, b0)), P.dzc[k + 1]));
-            b1 = b0;
-            store_halo(P.p + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, pk);
+    if (kb >= nz) return;
+    const T cu = tx1 < nz ? (P.Ub[c] - P.SU[c]) * P.rHu[c] : T(0);
+    const T cv = ty1 < nz ? (P.Vb[c] - P.SV[c]) * P.rHv[c] : T(0);
+    const T* __restrict__ cpu = P.cp_m + min(tx1, nz - 1) * nz;
+    const T* __restrict__ cpv = P.cp_m + min(ty1, nz - 1) * nz;
+    const T* __restrict__ cpt = P.cp_t + kb * nz;
+    T xu = 0, xv = 0, xt = 0, xs = 0, b1 = 0, pk = 0;
+    for (int k = nz - 1; k >= kb; --k) {
+        const long long o = k * sz + c;
+        const T2 d_ts = P.dts[o];
+        const T ck = cpt[k];
+        xt = E::sub(d_ts.x, E::mul(ck, xt));                         // cp[nz-1] = 0
+        xs = E::sub(d_ts.y, E::mul(ck, xs));
+        store_halo(P.ts + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, mk2(xt, xs));
+        const T b0 = buoyancy(P, xt, xs);
+        pk = k == nz - 1 ? -E::mul(b0, P.hz_top)
+                         : E::sub(pk, E::mul(E::mul(T(0.5), E::add(b1, b0)), P.dzc[k + 1]));
+        b1 = b0;
+        store_halo(P.p + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, pk);
+        const bool mu = k >= tx1, mv = k >= ty1;
+        if (mu | mv) {
+            const T2 d_uv = P.duv[o];
+            T un = 0, vn = 0;
+            if (mu) { xu = E::sub(d_uv.x, E::mul(cpu[k], xu)); un = xu + cu; }
+            if (mv) { xv = E::sub(d_uv.y, E::mul(cpv[k], xv)); vn = xv + cv; }
+            store_halo(P.uv + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, mk2(un, vn));
         }
     }
 }
@@ -123,7 +118,8 @@ __global__ void __launch_bounds__(128) k_pressure(const DevP<T> P) {
     const int kb = P.m8[c].x & 255;
     T b1 = 0, pk = 0;
     for (int k = nz - 1; k >= kb; --k) {
-        const T b0 = buoyancy(P, P.t[k * sz + c], P.s[k * sz + c]);
+        const typename Pair<T>::type q = P.ts[k * sz + c];
+        const T b0 = buoyancy(P, q.x, q.y);
         pk = k == nz - 1 ? -E::mul(b0, P.hz_top)
                          : E::sub(pk, E::mul(E::mul(T(0.5), E::add(b1, b0)), P.dzc[k + 1]));
         b1 = b0;
@@ -144,9 +140,8 @@ __global__ void __launch_bounds__(128) k_vertical_velocity(const DevP<T> P) {
     const T dy = P.dy, dF0 = P.dxF[r], dF1 = P.dxF[r + 1], rA = P.rAzC[r];
     double w = 0.0;
     for (int k = 0; k < nz; ++k) {
-        const T* __restrict__ pu = P.u + k * sz + c;
-        const T* __restrict__ pv = P.v + k * sz + c;
-        const T D = (dy * (pu[1] - pu[0]) + dF1 * pv[sx] - dF0 * pv[0]) * rA;
+        const typename Pair<T>::type* __restrict__ q = P.uv + k * sz + c;
+        const T D = (dy * (q[1].x - q[0].x) + dF1 * q[sx].y - dF0 * q[0].y) * rA;
         w -= (double)P.dz[k] * (double)D;
         store_halo(P.w + (k + 1) * sz, sx, P.nx, P.ny, P.px, P.py, j, i, (T)w);
     }
@@ -160,13 +155,14 @@ __global__ void __launch_bounds__(128) k_init_transport(const DevP<T> P) {
     if (i >= P.nx || j >= P.ny) return;
     const long long sz = P.sz, c = (long long)(j + OCN_HALO) * P.sx + i;
     double su = 0, sv = 0;
-    for (int k = 0; k < P.nz; ++k) { su += (double)P.dz[k] * (double)P.u[k * sz + c]; sv += (double)P.dz[k] * (double)P.v[k * sz + c]; }
+    for (int k = 0; k < P.nz; ++k) { const typename Pair<T>::type q = P.uv[k * sz + c]; su += (double)P.dz[k] * (double)q.x; sv += (double)P.dz[k] * (double)q.y; }
     store_halo(P.U[0], P.sx, P.nx, P.ny, P.px, P.py, j, i, (T)su);
     store_halo(P.V[0], P.sx, P.nx, P.ny, P.px, P.py, j, i, (T)sv);
 }
 
 // ---------------------------------------------------------------------------------------------
 // scatter (contiguous interior -> halo'd plane layout, masked) and gather (back, land = 0)
+// st = element stride of the device array (2 = one member of a pair array, base already offset)
 // kind: 0 u, 1 v, 2 T (offset Toff), 3 S (offset Soff), 4 eta, 5 plain 2-D, 6 w (nz+1 levels, gather only)
 // ---------------------------------------------------------------------------------------------
 template <class T>
@@ -184,7 +180,7 @@ __device__ __forceinline__ bool cell_open(const DevP<T>& P, long long c, int k, 
 
 template <class T>
 __global__ void __launch_bounds__(256) k_scatter(const DevP<T> P, T* __restrict__ dst, const T* __restrict__ src,
-                                                 const int nl, const int kind) {
+                                                 const int nl, const int kind, const int st) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
     if (i >= P.nx || j >= P.ny) return;
@@ -192,20 +188,20 @@ __global__ void __launch_bounds__(256) k_scatter(const DevP<T> P, T* __restrict_
     const T off = kind == 2 ? P.Toff : kind == 3 ? P.Soff : T(0);
     for (int k = blockIdx.z; k < nl; k += gridDim.z) {
         const T v = cell_open(P, c, k, kind) ? src[((long long)k * P.ny + j) * P.nx + i] - off : T(0);
-        store_halo(dst + k * P.sz, P.sx, P.nx, P.ny, P.px, P.py, j, i, v);
+        store_halo(dst + k * P.sz * st, P.sx, P.nx, P.ny, P.px, P.py, j, i, v, st);
     }
 }
 
 template <class T, class O>
 __global__ void __launch_bounds__(256) k_gather(const DevP<T> P, O* __restrict__ dst, const T* __restrict__ src,
-                                                const int nl, const int kind) {
+                                                const int nl, const int kind, const int st) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
     if (i >= P.nx || j >= P.ny) return;
     const long long c = (long long)(j + OCN_HALO) * P.sx + i;
     const T off = kind == 2 ? P.Toff : kind == 3 ? P.Soff : T(0);
     for (int k = blockIdx.z; k < nl; k += gridDim.z) {
-        const T v = cell_open(P, c, k, kind) ? src[k * P.sz + c] + off : T(0);
+        const T v = cell_open(P, c, k, kind) ? src[(k * P.sz + c) * st] + off : T(0);
         dst[((long long)k * P.ny + j) * P.nx + i] = (O)v;
     }
 }

@@ -1,0 +1,401 @@
+// kernels_tile.cuh — K1: the fused tendency kernel (S1 + S2 + S3 + elimination half of S4 + S5 +
+// S8 on the fly), one CTA per (TX x TY) tile of columns, marching k from the bottom up.
+//
+// Data movement: the halo'd k-planes of the tile are brought into shared memory
+// by TMA (cp.async.bulk.tensor.3d) DP levels ahead of use, into small rings:
+//     ts = (T, S) pairs : planes k-2 .. k+3 live (horizontal and vertical WENO stencils)
+//     uv = (u, v) pairs : planes k, k+1
+//     p                 : plane k
+// one mbarrier per in-flight level.  Nothing on the compute path waits on a global load except
+// the AB2 history read (own point, issued two phases ahead).  Per level:
+//   phase 1  zeta on the halo'd tile; K, D on the tile + west/south ring; w[k+1] = w[k] - dz D
+//            (S8 fused: the column accumulators live in registers of the thread that owns the point)
+//   phase 2  every west / south face of the tile (+ the east / north edge) is reconstructed ONCE:
+//            WENO face value of the (T, S) pair -> advective + diffusive flux, to shared memory;
+//            the owning thread does the vertical face
+//   phase 3  per cell: G_T, G_S from the flux planes; G_u, G_v from zeta, K, D, p, w; quasi-AB2,
+//            predictor, elimination sweep of the implicit solve, barotropic forcing sums; stores.
+#pragma once
+#include <cuda.h>
+
+#include "common.cuh"
+
+namespace ocn {
+
+// ---- mbarrier / TMA (PTX; SASS: SYNCS.*, UTMALDG) ------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    const uint32_t a = smem_u32(bar);
+    uint32_t ok;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void tma_load_plane(void* dst, const CUtensorMap* map, uint64_t* bar, int x, int y, int z) {
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+                 ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(x), "r"(y), "r"(z) : "memory");
+}
+
+// WENO face value of a pair with one advecting velocity and one order code
+template <class T2, class T>
+__device__ __forceinline__ T2 weno_face2(T2 a, T2 b, T2 c, T2 d, T2 e, T2 f, T vel, int order) {
+    T2 r;
+    r.x = weno_face(a.x, b.x, c.x, d.x, e.x, f.x, vel, order);
+    r.y = weno_face(a.y, b.y, c.y, d.y, e.y, f.y, vel, order);
+    return r;
+}
+
+__host__ __device__ constexpr int rup128(int b) { return (b + 127) / 128 * 128; }
+
+template <class T, int TX_, int TY_>
+struct Tile {
+    typedef typename Pair<T>::type T2;
+    static constexpr int TX = TX_, TY = TY_, NT = TX * TY;
+    static constexpr int BX = TX + 8, BY = TY + 6;       // TMA box: origin (i0 - 4, j0 - 3)
+    static constexpr int OX = 4, OY = 3;                 // box coordinates of tile cell (0, 0)
+    static constexpr int DP = 2;                         // prefetch distance in levels
+    static constexpr int R_TS = DP + 5, R_UV = DP + 1, R_P = DP, NB = DP;
+    static constexpr int RX = TX + 1, RY = TY + 1;       // tile + west/south ring (K, D, w) or + east/north edge (faces, masks)
+    static constexpr int PL2 = rup128(BX * BY * (int)sizeof(T2)), PL1 = rup128(BX * BY * (int)sizeof(T));
+    static constexpr int BYTES2 = BX * BY * (int)sizeof(T2), BYTES1 = BX * BY * (int)sizeof(T);
+    // shared-memory map (byte offsets from a 128-byte aligned base)
+    static constexpr int O_TS = 0;
+    static constexpr int O_UV = O_TS + R_TS * PL2;
+    static constexpr int O_P = O_UV + R_UV * PL2;
+    static constexpr int O_ZETA = O_P + R_P * PL1;
+    static constexpr int O_KD = O_ZETA + PL1;                                   // T2 (K, D) on RX x RY
+    static constexpr int O_W = O_KD + rup128(RX * RY * (int)sizeof(T2));        // 2 buffers of T on RX x RY
+    static constexpr int O_FX = O_W + 2 * rup128(RX * RY * (int)sizeof(T));     // T2 on RX x TY
+    static constexpr int O_FY = O_FX + rup128(RX * TY * (int)sizeof(T2));       // T2 on TX x RY
+    static constexpr int O_M8 = O_FY + rup128(TX * RY * (int)sizeof(T2));       // uint2 on RX x RY
+    static constexpr int O_MET = O_M8 + rup128(RX * RY * 8);                    // 6 row-metric arrays of BY + 1
+    static constexpr int O_BAR = O_MET + rup128(6 * (BY + 1) * (int)sizeof(T));
+    static constexpr int SMEM = O_BAR + 128 + 128;                              // + alignment slack
+};
+
+
+template <class T, int TX, int TY>
+__global__ void __launch_bounds__(TX * TY, (sizeof(T) == 4 ? 2 : 1))
+k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__ CUtensorMap m_ts,
+                const __grid_constant__ CUtensorMap m_uv, const __grid_constant__ CUtensorMap m_p) {
+    typedef Tile<T, TX, TY> C;
+    typedef typename C::T2 T2;
+    typedef Ex<T> E;
+    constexpr int BX = C::BX, BY = C::BY, RX = C::RX, RY = C::RY, NT = C::NT, OX = C::OX, OY = C::OY;
+    extern __shared__ unsigned char smem_raw[];
+    unsigned char* sm = (unsigned char*)(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
+    T* const s_zeta = (T*)(sm + C::O_ZETA);
+    T2* const s_kd = (T2*)(sm + C::O_KD);
+    T2* const s_fx = (T2*)(sm + C::O_FX);
+    T2* const s_fy = (T2*)(sm + C::O_FY);
+    uint2* const s_m8 = (uint2*)(sm + C::O_M8);
+    T* const s_dxC = (T*)(sm + C::O_MET);
+    T* const s_dxF = s_dxC + (BY + 1);
+    T* const s_rAzC = s_dxF + (BY + 1);
+    T* const s_rAzF = s_rAzC + (BY + 1);
+    T* const s_rdxC = s_rAzF + (BY + 1);
+    uint64_t* const bars = (uint64_t*)(sm + C::O_BAR);
+    __shared__ int s_kmin;
+
+    const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * TX + tx;
+    const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;
+    const int i = i0 + tx, j = j0 + ty;
+    const int nz = P.nz, sx = P.sx;
+    const long long sz = P.sz;
+
+    // ---- masks of the tile (+ east / north edge) and the first level with any open cell -----
+    if (tid == 0) s_kmin = nz;
+    __syncthreads();
+    {
+        const uint32_t nzb = (uint32_t)nz;
+        const uint2 land = make_uint2(nzb * 0x01010101u, nzb * 0x00010101u);
+        int kloc = nz;
+        for (int q = tid; q < (TX + 2) * (TY + 2); q += NT) {
+            const int qx = q % (TX + 2) - 1, qy = q / (TX + 2) - 1;
+            const int ii = i0 + qx, jj = j0 + qy;
+            uint2 m = land;
+            if (ii < P.nx + OCN_HALO && jj < P.ny + OCN_HALO) m = P.m8[(long long)(jj + OCN_HALO) * sx + ii];
+            kloc = min(kloc, (int)(m.x & 255u));
+            if (qx >= 0 && qy >= 0) s_m8[qy * RX + qx] = m;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) kloc = min(kloc, __shfl_xor_sync(0xffffffffu, kloc, o));
+        if ((tid & 31) == 0) atomicMin(&s_kmin, kloc);
+    }
+    __syncthreads();
+    const int kmin = s_kmin;
+    if (kmin >= nz) return;                              // all land: forcing sums stay zero
+
+    // ---- one-time shared-memory setup --------------------------------------------------------
+    for (int q = tid; q < C::O_M8 / 16; q += NT) ((uint4*)sm)[q] = make_uint4(0u, 0u, 0u, 0u);
+    {
+        const int nr = P.ny + 2 * OCN_HALO + 1;
+        for (int q = tid; q <= BY; q += NT) {
+            const int r = min(j0 + q, nr - 1);
+            s_dxC[q] = P.dxC[r]; s_dxF[q] = P.dxF[r]; s_rAzC[q] = P.rAzC[r]; s_rAzF[q] = P.rAzF[r]; s_rdxC[q] = P.rdxC[r];
+        }
+    }
+    if (tid == 0) {
+#pragma unroll
+        for (int b = 0; b < C::NB; ++b) mbar_init(&bars[b], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // zero fill (generic) before TMA writes (async)
+    __syncthreads();
+
+    // group(m) = the planes level m needs beyond those of level m - 1: ts(m + 3), uv(m + 1), p(m)
+    auto issue_group = [&](int m, bool first) {
+        uint64_t* bar = &bars[(m - kmin) % C::NB];
+        uint32_t bytes = C::BYTES1;
+        const int tlo = first ? max(m - 2, 0) : m + 3, thi = min(m + 3, nz - 1);
+        const int ulo = first ? m : m + 1, uhi = min(m + 1, nz - 1);
+        if (thi >= tlo) bytes += (uint32_t)(thi - tlo + 1) * C::BYTES2;
+        if (uhi >= ulo) bytes += (uint32_t)(uhi - ulo + 1) * C::BYTES2;
+        mbar_expect_tx(bar, bytes);
+        for (int q = tlo; q <= thi; ++q) tma_load_plane(sm + C::O_TS + (q % C::R_TS) * C::PL2, &m_ts, bar, 2 * i0, j0, q);
+        for (int q = ulo; q <= uhi; ++q) tma_load_plane(sm + C::O_UV + (q % C::R_UV) * C::PL2, &m_uv, bar, 2 * i0, j0, q);
+        tma_load_plane(sm + C::O_P + (m % C::R_P) * C::PL1, &m_p, bar, i0, j0, m);
+    };
+    if (tid == 0) {
+        issue_group(kmin, true);
+#pragma unroll
+        for (int d = 1; d < C::DP; ++d) if (kmin + d < nz) issue_group(kmin + d, false);
+    }
+
+    // ---- per-thread column state ------------------------------------------------------------
+    const bool incol = i < P.nx && j < P.ny;
+    const long long c = (long long)(j + OCN_HALO) * sx + i;
+    const uint2 m_own = s_m8[ty * RX + tx];
+    const int kb = incol ? (int)(m_own.x & 255u) : nz;
+    const int tx1 = incol ? (int)((m_own.x >> 8) & 255u) : nz, ty1 = incol ? (int)(m_own.y & 255u) : nz;
+    uchar4 mzt = make_uchar4(255, 255, 255, 255);
+    if (kb < nz) mzt = P.mz[c];
+    const int r = j + OCN_HALO;                          // row-metric index of this thread's row
+    const int rc = min(r, P.ny + 2 * OCN_HALO - 1);
+    const T dy = P.dy, rdy = P.rdy;
+    const T dxFj = P.dxF[rc], dxFn = P.dxF[rc + 1], rdxCj = P.rdxC[rc], rdxFj = P.rdxF[rc];
+    const T AzCj = P.AzC[rc], AzCs = P.AzC[rc - 1], rAzCj = P.rAzC[rc], rAzFj = P.rAzF[rc];
+    const T fFj = P.fF[rc], fFn = P.fF[rc + 1];
+    const int bx = tx + OX, by = ty + OY;                // this cell in box coordinates
+    const int bo = by * BX + bx;
+
+    double wacc0 = 0.0, wacc1 = 0.0;                     // w accumulators of this thread's ring points
+    T2 fz_bot = mk2(T(0), T(0));                         // vertical tracer flux through the face below
+    T u_dn = 0, v_dn = 0;
+    T2 dduv = mk2(T(0), T(0)), ddts = mk2(T(0), T(0));   // eliminated right-hand sides of the level below
+    double aGU = 0, aGV = 0, aSU = 0, aSV = 0;
+    const T* __restrict__ mt = P.m_t + min(kb, nz - 1) * nz;
+    const T* __restrict__ rmt = P.rm_t + min(kb, nz - 1) * nz;
+    const T* __restrict__ mmu = P.m_m + min(tx1, nz - 1) * nz;
+    const T* __restrict__ rmu = P.rm_m + min(tx1, nz - 1) * nz;
+    const T* __restrict__ mmv = P.m_m + min(ty1, nz - 1) * nz;
+    const T* __restrict__ rmv = P.rm_m + min(ty1, nz - 1) * nz;
+
+    for (int k = kmin; k < nz; ++k) {
+        const bool wetc = k >= kb;
+        const long long o = k * sz + c;
+        // AB2 history and pivots of this level: issued now, consumed in phase 3
+        T2 gm_uv = mk2(T(0), T(0)), gm_ts = mk2(T(0), T(0));
+        T piv_t = 1, piv_u = 1, piv_v = 1;
+        if (wetc) {
+            gm_uv = P.Guv[o]; gm_ts = P.Gts[o];
+            if (sizeof(T) == 8) { piv_t = mt[k]; piv_u = mmu[k]; piv_v = mmv[k]; }
+            else                { piv_t = rmt[k]; piv_u = rmu[k]; piv_v = rmv[k]; }
+        }
+        const T dzk = P.dz[k], rdzk = P.rdz[k];
+        mbar_wait(&bars[(k - kmin) % C::NB], (uint32_t)(((k - kmin) / C::NB) & 1));
+        const T2* __restrict__ s_uv = (const T2*)(sm + C::O_UV + (k % C::R_UV) * C::PL2);
+        const T2* __restrict__ s_uv1 = (const T2*)(sm + C::O_UV + ((k + 1) % C::R_UV) * C::PL2);
+        const T* __restrict__ s_p = (const T*)(sm + C::O_P + (k % C::R_P) * C::PL1);
+        const T* __restrict__ s_w0 = (const T*)(sm + C::O_W + (k & 1) * rup128(RX * RY * (int)sizeof(T)));
+        T* __restrict__ s_w1 = (T*)(sm + C::O_W + ((k + 1) & 1) * rup128(RX * RY * (int)sizeof(T)));
+
+        // ================= phase 1: zeta, K, D, w[k+1] =================
+#pragma unroll
+        for (int h = 0; h < (BX - 1) * (BY - 1); h += NT) {
+            const int q = h + tid;
+            if (q < (BX - 1) * (BY - 1)) {
+                const int px = 1 + q % (BX - 1), py = 1 + q / (BX - 1);
+                const T2 a = s_uv[py * BX + px], as = s_uv[(py - 1) * BX + px], aw = s_uv[py * BX + px - 1];
+                s_zeta[py * BX + px] = (dy * (a.y - aw.y) - (s_dxC[py] * a.x - s_dxC[py - 1] * as.x)) * s_rAzF[py];
+            }
+        }
+#pragma unroll
+        for (int h = 0, n = 0; h < RX * RY; h += NT, ++n) {
+            const int q = h + tid;
+            if (q < RX * RY) {
+                const int qx = q % RX, qy = q / RX;
+                const int px = qx + OX - 1, py = qy + OY - 1;          // cells i0 - 1 + qx, j0 - 1 + qy
+                const T2 a = s_uv[py * BX + px], ae = s_uv[py * BX + px + 1], an = s_uv[(py + 1) * BX + px];
+                const T Kc = T(0.25) * (a.x * a.x + ae.x * ae.x) + T(0.25) * (a.y * a.y + an.y * an.y);
+                const T Dc = (dy * (ae.x - a.x) + s_dxF[py + 1] * an.y - s_dxF[py] * a.y) * s_rAzC[py];
+                s_kd[q] = mk2(Kc, Dc);
+                double& wa = n == 0 ? wacc0 : wacc1;
+                wa -= (double)dzk * (double)Dc;
+                s_w1[q] = (T)wa;
+            }
+        }
+        __syncthreads();
+
+        // ================= phase 2: tracer face fluxes, each face once =================
+        {
+            const T2* __restrict__ s_ts = (const T2*)(sm + C::O_TS + (k % C::R_TS) * C::PL2);
+            constexpr int NFX = RX * TY, NFY = TX * RY;
+#pragma unroll
+            for (int h = 0; h < NFX + NFY; h += NT) {
+                const int f = h + tid;
+                if (f < NFX) {                                           // west face of cell (fx, fy)
+                    const int fx = f % RX, fy = f / RX;
+                    const uint32_t mx = s_m8[fy * RX + fx].x;
+                    const int t1 = (mx >> 8) & 255u, t2 = (mx >> 16) & 255u, t3 = mx >> 24;
+                    const int ord = order3(k, t1, t2, t3);
+                    T2 flux = mk2(T(0), T(0));
+                    if (ord > 0) {
+                        const int b = (fy + OY) * BX + fx + OX;
+                        const T u = s_uv[b].x;
+                        const T ax = dy * dzk;
+                        const T2 cw = s_ts[b - 1], cc = s_ts[b];
+                        const T2 fv = weno_face2<T2, T>(s_ts[b - 3], s_ts[b - 2], cw, cc, s_ts[b + 1], s_ts[b + 2], u, ord);
+                        const T kd = P.kappa_h * ax * s_rdxC[fy + OY];
+                        flux.x = u * ax * fv.x - kd * (cc.x - cw.x);
+                        flux.y = u * ax * fv.y - kd * (cc.y - cw.y);
+                    }
+                    s_fx[f] = flux;
+                } else if (f < NFX + NFY) {                              // south face of cell (gx, gy)
+                    const int g = f - NFX;
+                    const int gx = g % TX, gy = g / TX;
+                    const uint32_t my = s_m8[gy * RX + gx].y;
+                    const int t1 = my & 255u, t2 = (my >> 8) & 255u, t3 = (my >> 16) & 255u;
+                    const int ord = order3(k, t1, t2, t3);
+                    T2 flux = mk2(T(0), T(0));
+                    if (ord > 0) {
+                        const int b = (gy + OY) * BX + gx + OX;
+                        const T v = s_uv[b].y;
+                        const T ay = s_dxF[gy + OY] * dzk;
+                        const T2 cs = s_ts[b - BX], cc = s_ts[b];
+                        const T2 fv = weno_face2<T2, T>(s_ts[b - 3 * BX], s_ts[b - 2 * BX], cs, cc, s_ts[b + BX], s_ts[b + 2 * BX], v, ord);
+                        const T kd = P.kappa_h * ay * rdy;
+                        flux.x = v * ay * fv.x - kd * (cc.x - cs.x);
+                        flux.y = v * ay * fv.y - kd * (cc.y - cs.y);
+                    }
+                    s_fy[g] = flux;
+                }
+            }
+        }
+        // vertical face above cell k (own column)
+        const int qo = (ty + 1) * RX + tx + 1;                           // this column in the ring arrays
+        const T w_c1 = s_w1[qo], w_c0 = s_w0[qo];
+        T2 fz_top = mk2(T(0), T(0));
+        if (wetc) {
+            const int ozt = (k + 1 < nz) ? min(3, min(k + 1 - kb, nz - k - 1)) : 0;
+            if (ozt > 0) {
+                auto tsz = [&](int kk) -> T2 { return ((const T2*)(sm + C::O_TS + ((kk + C::R_TS) % C::R_TS) * C::PL2))[bo]; };
+                const T2 fv = weno_face2<T2, T>(tsz(k - 2), tsz(k - 1), tsz(k), tsz(k + 1), tsz(k + 2), tsz(k + 3), w_c1, ozt);
+                fz_top.x = w_c1 * AzCj * fv.x;
+                fz_top.y = w_c1 * AzCj * fv.y;
+            }
+        }
+        __syncthreads();
+
+        // ================= phase 3: tendencies of this cell, AB2, elimination =================
+        if (wetc) {
+            const bool mu = k >= tx1, mv = k >= ty1;
+            // ---- tracers ----
+            const T2 fw = s_fx[ty * RX + tx], fe = s_fx[ty * RX + tx + 1];
+            const T2 fs = s_fy[ty * TX + tx], fn = s_fy[(ty + 1) * TX + tx];
+            const T2 tsc = ((const T2*)(sm + C::O_TS + (k % C::R_TS) * C::PL2))[bo];
+            T GT = -((fe.x - fw.x) + (fn.x - fs.x) + (fz_top.x - fz_bot.x)) * rAzCj * rdzk;
+            T GS = -((fe.y - fw.y) + (fn.y - fs.y) + (fz_top.y - fz_bot.y)) * rAzCj * rdzk;
+            if (k == nz - 1) {                 // tracers are stored as offsets from (Toff, Soff): exact source
+                const T src = w_c1 * rdzk;     // of the constant under the zero-top-flux linear free surface
+                GT += P.Toff * src; GS += P.Soff * src;
+            }
+            // ---- momentum ----
+            const T2 uvc = s_uv[bo];
+            const T u_c = uvc.x, v_c = uvc.y;
+            T Gu = 0, Gv = 0;
+            if (mu | mv) {
+                const T2 uv_w = s_uv[bo - 1], uv_n = s_uv[bo + BX], uv_nw = s_uv[bo + BX - 1];
+                const T2 uv_s = s_uv[bo - BX], uv_e = s_uv[bo + 1], uv_se = s_uv[bo - BX + 1];
+                const T2 uv_up = (k + 1 < nz) ? s_uv1[bo] : mk2(T(0), T(0));
+                const T z00 = s_zeta[bo];
+                const T2 kdc = s_kd[qo];
+                const T pc = s_p[bo];
+                if (mu) {
+                    const T vsum_s = uv_w.y + v_c, vsum_n = uv_nw.y + uv_n.y;
+                    const T vhat = T(0.25) * (dxFj * vsum_s + dxFn * vsum_n) * rdxCj;
+                    const int ozu = 1 + (k >= mzt.x) + (k >= mzt.y);
+                    const T z01 = s_zeta[bo + BX];
+                    const T zt = ozu == 1 ? (vhat > T(0) ? z00 : z01)
+                                          : weno_face(s_zeta[bo - 2 * BX], s_zeta[bo - BX], z00, z01, s_zeta[bo + 2 * BX],
+                                                      s_zeta[bo + 3 * BX], vhat, ozu);
+                    const T Cu = T(0.5) * (fFj * T(0.5) * dxFj * vsum_s + fFn * T(0.5) * dxFn * vsum_n) * rdxCj;
+                    const T2 kdw = s_kd[qo - 1];
+                    const T dK = (kdc.x - kdw.x) * rdxCj;
+                    const T dP = (pc - s_p[bo - 1]) * rdxCj;
+                    const T dlo = (k >= 1 && k - 1 >= tx1) ? u_c - u_dn : T(0);
+                    const T dhi = (k + 1 <= nz - 1) ? uv_up.x - u_c : T(0);
+                    const T Au = T(0.5) * (T(0.5) * (s_w1[qo - 1] + w_c1) * dhi + T(0.5) * (s_w0[qo - 1] + w_c0) * dlo) * rdzk;
+                    const T Vu = P.nu_h * ((kdc.y - kdw.y) * rdxCj - (z01 - z00) * rdy);
+                    const T tau = (k == nz - 1) ? P.taux[c] * P.rrho0 * rdzk : T(0);
+                    Gu = zt * vhat + Cu - dK - dP - Au + Vu + tau;
+                }
+                if (mv) {
+                    const T uhat = T(0.25) * (uv_s.x + u_c + uv_se.x + uv_e.x);
+                    const int ozv = 1 + (k >= mzt.z) + (k >= mzt.w);
+                    const T z10 = s_zeta[bo + 1];
+                    const T zt = ozv == 1 ? (uhat > T(0) ? z00 : z10)
+                                          : weno_face(s_zeta[bo - 2], s_zeta[bo - 1], z00, z10, s_zeta[bo + 2], s_zeta[bo + 3], uhat, ozv);
+                    const T Cv = fFj * uhat;
+                    const T2 kds = s_kd[qo - RX];
+                    const T dK = (kdc.x - kds.x) * rdy;
+                    const T dP = (pc - s_p[bo - BX]) * rdy;
+                    const T dlo = (k >= 1 && k - 1 >= ty1) ? v_c - v_dn : T(0);
+                    const T dhi = (k + 1 <= nz - 1) ? uv_up.y - v_c : T(0);
+                    const T Av = T(0.5) * (T(0.5) * (AzCs * s_w1[qo - RX] + AzCj * w_c1) * dhi
+                                         + T(0.5) * (AzCs * s_w0[qo - RX] + AzCj * w_c0) * dlo) * rAzFj * rdzk;
+                    const T Vv = P.nu_h * ((kdc.y - kds.y) * rdy + (z10 - z00) * rdxFj);
+                    const T tau = (k == nz - 1) ? P.tauy[c] * P.rrho0 * rdzk : T(0);
+                    Gv = -zt * uhat - Cv - dK - dP - Av + Vv + tau;
+                }
+            }
+            // ---- quasi-AB2, predictor, elimination sweep (S3, S4, S5) ----
+            const T Ghu = c0 * Gu - c1 * gm_uv.x, Ghv = c0 * Gv - c1 * gm_uv.y;
+            const T Ght = c0 * GT - c1 * gm_ts.x, Ghs = c0 * GS - c1 * gm_ts.y;
+            P.Guv[o] = mk2(Gu, Gv);
+            P.Gts[o] = mk2(GT, GS);
+            if (mu) {
+                const T us = E::add(u_c, E::mul(P.dt, Ghu));
+                aGU += (double)dzk * (double)Ghu; aSU += (double)dzk * (double)us;
+                const T smk = k > tx1 ? P.sm_m[k] : T(0);
+                dduv.x = E::div(E::add(us, E::mul(smk, dduv.x)), piv_u, piv_u);
+            }
+            if (mv) {
+                const T vs2 = E::add(v_c, E::mul(P.dt, Ghv));
+                aGV += (double)dzk * (double)Ghv; aSV += (double)dzk * (double)vs2;
+                const T smk = k > ty1 ? P.sm_m[k] : T(0);
+                dduv.y = E::div(E::add(vs2, E::mul(smk, dduv.y)), piv_v, piv_v);
+            }
+            {
+                const T smk = k > kb ? P.sm_t[k] : T(0);
+                ddts.x = E::div(E::add(E::add(tsc.x, E::mul(P.dt, Ght)), E::mul(smk, ddts.x)), piv_t, piv_t);
+                ddts.y = E::div(E::add(E::add(tsc.y, E::mul(P.dt, Ghs)), E::mul(smk, ddts.y)), piv_t, piv_t);
+            }
+            P.duv[o] = dduv;
+            P.dts[o] = ddts;
+            u_dn = u_c; v_dn = v_c;
+        }
+        fz_bot = fz_top;
+        __syncthreads();                       // every plane of level k is dead: refill the ring
+        if (tid == 0 && k + C::DP < nz) issue_group(k + C::DP, false);
+    }
+    if (incol && kb < nz) { P.GU[c] = (T)aGU; P.GV[c] = (T)aGV; P.SU[c] = (T)aSU; P.SV[c] = (T)aSV; }
+}
+}  // namespace ocn

@@ -1,5 +1,6 @@
 // ocn_api.cu — the C ABI of libocn (include/ocn.h): host-side scheduling only.  Every step of the
 // hot path runs in the kernels of kernels_tend.cuh / kernels_column.cuh.
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include <cstdio>
@@ -9,7 +10,7 @@
 
 #include "grid_host.h"
 #include "kernels_column.cuh"
-#include "kernels_tend.cuh"
+#include "kernels_tile.cuh"
 
 namespace {
 
@@ -43,13 +44,14 @@ struct ocn_model {
     ocn::DevP<double> pd{};
     void* stage = nullptr;              // contiguous staging buffer, (nz+1)*ny*nx doubles
     cudaGraphExec_t graph = nullptr;    // one steady-state (AB2) step
+    CUtensorMap tm_ts{}, tm_uv{}, tm_p{};   // TMA descriptors of the halo'd (T,S), (u,v) and p arrays
     int launches_per_step = 0;
     // per-stage timing (ocn_profile_*)
     bool profiling = false;
     std::vector<cudaEvent_t> ev_pool;   // OCN_NSTAGES + 1 events per profiled step
     size_t ev_used = 0;
-    double prof_ms[OCN_NSTAGES] = {0, 0, 0, 0};
-    long long prof_launches[OCN_NSTAGES] = {0, 0, 0, 0};
+    double prof_ms[OCN_NSTAGES] = {0, 0, 0};
+    long long prof_launches[OCN_NSTAGES] = {0, 0, 0};
 };
 
 namespace {
@@ -83,6 +85,34 @@ ocn::DevP<T>& params(ocn_model* M);
 template <> ocn::DevP<float>& params<float>(ocn_model* M) { return M->pf; }
 template <> ocn::DevP<double>& params<double>(ocn_model* M) { return M->pd; }
 
+constexpr int TILE_X = 32, TILE_Y = 8;    // K1 tile (kernels_tile.cuh)
+
+// TMA descriptor of a halo'd 3-D array seen as [levels][rows][inner] scalars
+ocn_status make_tmap(CUtensorMap* tm, bool f64, void* base, unsigned long long inner, unsigned long long rows,
+                     unsigned long long levels, unsigned box_inner, unsigned box_rows) {
+    typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static encode_fn encode = nullptr;
+    if (!encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        CK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr));
+        if (!fn || qr != cudaDriverEntryPointSuccess) return fail(OCN_ECUDA, "cuTensorMapEncodeTiled not available");
+        encode = reinterpret_cast<encode_fn>(fn);
+    }
+    const unsigned long long es = f64 ? 8 : 4;
+    const cuuint64_t dims[3] = {inner, rows, levels};
+    const cuuint64_t strides[2] = {inner * es, inner * rows * es};
+    const cuuint32_t box[3] = {box_inner, box_rows, 1};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    const CUresult r = encode(tm, f64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, base, dims,
+                              strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                              CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(OCN_ECUDA, "cuTensorMapEncodeTiled failed (code " + std::to_string((int)r) + ")");
+    return OCN_OK;
+}
+
 dim3 grid2(const ocn_grid* g, dim3 b, int z = 1) { return dim3((g->nx + b.x - 1) / b.x, (g->ny + b.y - 1) / b.y, z); }
 
 template <class T>
@@ -99,8 +129,10 @@ ocn_status build_model(ocn_model* M) {
     auto plane = [&](size_t n, T** out) -> ocn_status {
         return dev_alloc(M, n, out, true);
     };
-    T** f3[] = {&P.u, &P.v, &P.t, &P.s, &P.p, &P.du, &P.dv, &P.dt_, &P.ds, &P.Gu, &P.Gv, &P.Gt, &P.Gs};
-    for (T** f : f3) if ((s = plane(n3, f)) != OCN_OK) return s;
+    typedef typename ocn::Pair<T>::type T2;
+    T2** f3[] = {&P.uv, &P.ts, &P.duv, &P.dts, &P.Guv, &P.Gts};
+    for (T2** f : f3) if ((s = dev_alloc(M, n3, f, true)) != OCN_OK) return s;
+    if ((s = plane(n3, &P.p)) != OCN_OK) return s;
     if ((s = plane(n3 + n2, &P.w)) != OCN_OK) return s;
     T** f2[] = {&P.eta[0], &P.eta[1], &P.U[0], &P.U[1], &P.V[0], &P.V[1], &P.etab, &P.Ub, &P.Vb, &P.GU, &P.GV,
                 &P.SU, &P.SV, &P.Hu, &P.Hv, &P.rHu, &P.rHv, &P.taux, &P.tauy};
@@ -178,7 +210,18 @@ ocn_status build_model(ocn_model* M) {
     }
     CK(cudaMalloc(&M->stage, (size_t)(nz + 1) * g->ny * g->nx * sizeof(double)));
     M->bytes += (size_t)(nz + 1) * g->ny * g->nx * sizeof(double);
-    M->launches_per_step = M->d.substeps + 4;
+    M->launches_per_step = M->d.substeps + 3;
+    // TMA descriptors: box origin (i0 - 4, j0 - 3), so the map starts 4 elements before (row -3, i = 0)
+    {
+        typedef ocn::Tile<T, TILE_X, TILE_Y> C;
+        const bool f64 = sizeof(T) == 8;
+        const unsigned long long sxu = (unsigned long long)g->sx, syu = (unsigned long long)g->sy;
+        if ((s = make_tmap(&M->tm_ts, f64, (T*)P.ts - 2 * C::OX, 2 * sxu, syu, nz, 2 * C::BX, C::BY)) != OCN_OK ||
+            (s = make_tmap(&M->tm_uv, f64, (T*)P.uv - 2 * C::OX, 2 * sxu, syu, nz, 2 * C::BX, C::BY)) != OCN_OK ||
+            (s = make_tmap(&M->tm_p, f64, P.p - C::OX, sxu, syu, nz, C::BX, C::BY)) != OCN_OK)
+            return s;
+        CK(cudaFuncSetAttribute(ocn::k_tendency_tile<T, TILE_X, TILE_Y>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
+    }
     return OCN_OK;
 }
 
@@ -227,7 +270,11 @@ ocn_status launch_step(ocn_model* M, bool euler) {
     const T c0 = euler ? T(1) : (T)(1.5 + M->d.chi), c1 = euler ? T(0) : (T)(0.5 + M->d.chi);
     const dim3 bc(32, 4), b2(32, 8);
     MARK(-1, 0);
-    ocn::k_tendency<T><<<grid2(g, bc), bc, 0, M->stream>>>(P, c0, c1);
+    {
+        typedef ocn::Tile<T, TILE_X, TILE_Y> C;
+        const dim3 bt(TILE_X, TILE_Y);
+        ocn::k_tendency_tile<T, TILE_X, TILE_Y><<<grid2(g, bt), bt, C::SMEM, M->stream>>>(P, c0, c1, M->tm_ts, M->tm_uv, M->tm_p);
+    }
     MARK(0, 1);
     int cur = 0;
     for (int m = 1; m <= M->d.substeps; ++m) {
@@ -238,8 +285,6 @@ ocn_status launch_step(ocn_model* M, bool euler) {
     MARK(1, M->d.substeps + 1);
     ocn::k_backsub_correct<T><<<grid2(g, bc), bc, 0, M->stream>>>(P);
     MARK(2, 1);
-    ocn::k_vertical_velocity<T><<<grid2(g, bc), bc, 0, M->stream>>>(P);
-    MARK(3, 1);
 #undef MARK
     CK(cudaGetLastError());
     return OCN_OK;
@@ -272,7 +317,7 @@ ocn_status run_steps(ocn_model* M, int n) {
 }
 
 template <class T>
-ocn_status set_one(ocn_model* M, const void* src, T* dst, int nl, int kind, bool on_device) {
+ocn_status set_one(ocn_model* M, const void* src, T* dst, int nl, int kind, bool on_device, int st = 1) {
     const ocn_grid* g = M->g;
     const size_t n = (size_t)nl * g->ny * g->nx;
     const T* dsrc = static_cast<const T*>(src);
@@ -281,7 +326,7 @@ ocn_status set_one(ocn_model* M, const void* src, T* dst, int nl, int kind, bool
         dsrc = static_cast<const T*>(M->stage);
     }
     const dim3 b(32, 8);
-    ocn::k_scatter<T><<<grid2(g, b, nl < 64 ? nl : 64), b, 0, M->stream>>>(params<T>(M), dst, dsrc, nl, kind);
+    ocn::k_scatter<T><<<grid2(g, b, nl < 64 ? nl : 64), b, 0, M->stream>>>(params<T>(M), dst, dsrc, nl, kind, st);
     CK(cudaGetLastError());
     if (!on_device) CK(cudaStreamSynchronize(M->stream));   // staging buffer is reused by the next field
     return OCN_OK;
@@ -293,17 +338,16 @@ ocn_status set_fields_t(ocn_model* M, const ocn_fields* f) {
     const int nz = M->g->nz;
     const bool dev = f->on_device != 0;
     ocn_status s;
-    if (f->u && (s = set_one<T>(M, f->u, P.u, nz, 0, dev)) != OCN_OK) return s;
-    if (f->v && (s = set_one<T>(M, f->v, P.v, nz, 1, dev)) != OCN_OK) return s;
-    if (f->T && (s = set_one<T>(M, f->T, P.t, nz, 2, dev)) != OCN_OK) return s;
-    if (f->S && (s = set_one<T>(M, f->S, P.s, nz, 3, dev)) != OCN_OK) return s;
+    if (f->u && (s = set_one<T>(M, f->u, (T*)P.uv, nz, 0, dev, 2)) != OCN_OK) return s;
+    if (f->v && (s = set_one<T>(M, f->v, (T*)P.uv + 1, nz, 1, dev, 2)) != OCN_OK) return s;
+    if (f->T && (s = set_one<T>(M, f->T, (T*)P.ts, nz, 2, dev, 2)) != OCN_OK) return s;
+    if (f->S && (s = set_one<T>(M, f->S, (T*)P.ts + 1, nz, 3, dev, 2)) != OCN_OK) return s;
     if (f->eta && (s = set_one<T>(M, f->eta, P.eta[0], 1, 4, dev)) != OCN_OK) return s;
     if (f->tau_x && (s = set_one<T>(M, f->tau_x, P.taux, 1, 5, dev)) != OCN_OK) return s;
     if (f->tau_y && (s = set_one<T>(M, f->tau_y, P.tauy, 1, 5, dev)) != OCN_OK) return s;
     if (f->u || f->v || f->T || f->S || f->eta) {
         const dim3 bc(32, 4);
         ocn::k_init_transport<T><<<grid2(M->g, bc), bc, 0, M->stream>>>(P);
-        ocn::k_vertical_velocity<T><<<grid2(M->g, bc), bc, 0, M->stream>>>(P);
         ocn::k_pressure<T><<<grid2(M->g, bc), bc, 0, M->stream>>>(P);
         CK(cudaGetLastError());
         M->have_history = false;
@@ -312,12 +356,12 @@ ocn_status set_fields_t(ocn_model* M, const ocn_fields* f) {
 }
 
 template <class T, class O>
-ocn_status get_one(ocn_model* M, void* dst, const T* src, int nl, int kind, bool on_device) {
+ocn_status get_one(ocn_model* M, void* dst, const T* src, int nl, int kind, bool on_device, int st = 1) {
     const ocn_grid* g = M->g;
     const size_t n = (size_t)nl * g->ny * g->nx;
     O* ddst = on_device ? static_cast<O*>(dst) : static_cast<O*>(M->stage);
     const dim3 b(32, 8);
-    ocn::k_gather<T, O><<<grid2(g, b, nl < 64 ? nl : 64), b, 0, M->stream>>>(params<T>(M), ddst, src, nl, kind);
+    ocn::k_gather<T, O><<<grid2(g, b, nl < 64 ? nl : 64), b, 0, M->stream>>>(params<T>(M), ddst, src, nl, kind, st);
     CK(cudaGetLastError());
     if (!on_device) {
         CK(cudaMemcpyAsync(dst, M->stage, n * sizeof(O), cudaMemcpyDeviceToHost, M->stream));
@@ -332,10 +376,15 @@ ocn_status get_fields_t(ocn_model* M, ocn_fields* f) {
     const int nz = M->g->nz;
     const bool dev = f->on_device != 0;
     ocn_status s;
-    if (f->u && (s = get_one<T, T>(M, f->u, P.u, nz, 0, dev)) != OCN_OK) return s;
-    if (f->v && (s = get_one<T, T>(M, f->v, P.v, nz, 1, dev)) != OCN_OK) return s;
-    if (f->T && (s = get_one<T, T>(M, f->T, P.t, nz, 2, dev)) != OCN_OK) return s;
-    if (f->S && (s = get_one<T, T>(M, f->S, P.s, nz, 3, dev)) != OCN_OK) return s;
+    if (f->u && (s = get_one<T, T>(M, f->u, (T*)P.uv, nz, 0, dev, 2)) != OCN_OK) return s;
+    if (f->v && (s = get_one<T, T>(M, f->v, (T*)P.uv + 1, nz, 1, dev, 2)) != OCN_OK) return s;
+    if (f->T && (s = get_one<T, T>(M, f->T, (T*)P.ts, nz, 2, dev, 2)) != OCN_OK) return s;
+    if (f->S && (s = get_one<T, T>(M, f->S, (T*)P.ts + 1, nz, 3, dev, 2)) != OCN_OK) return s;
+    if (f->w) {                                   // w is diagnosed on demand (K1 recomputes it on the fly)
+        const dim3 bc(32, 4);
+        ocn::k_vertical_velocity<T><<<grid2(M->g, bc), bc, 0, M->stream>>>(P);
+        CK(cudaGetLastError());
+    }
     if (f->w && (s = get_one<T, T>(M, f->w, P.w, nz + 1, 6, dev)) != OCN_OK) return s;
     if (f->eta && (s = get_one<T, T>(M, f->eta, P.eta[0], 1, 4, dev)) != OCN_OK) return s;
     if (f->tau_x && (s = get_one<T, T>(M, f->tau_x, P.taux, 1, 5, dev)) != OCN_OK) return s;
@@ -349,10 +398,10 @@ ocn_status get_debug_t(ocn_model* M, double* Gu, double* Gv, double* GT, double*
     ocn::DevP<T>& P = params<T>(M);
     const int nz = M->g->nz;
     ocn_status s;
-    if (Gu && (s = get_one<T, double>(M, Gu, P.Gu, nz, 5, false)) != OCN_OK) return s;
-    if (Gv && (s = get_one<T, double>(M, Gv, P.Gv, nz, 5, false)) != OCN_OK) return s;
-    if (GT && (s = get_one<T, double>(M, GT, P.Gt, nz, 5, false)) != OCN_OK) return s;
-    if (GS && (s = get_one<T, double>(M, GS, P.Gs, nz, 5, false)) != OCN_OK) return s;
+    if (Gu && (s = get_one<T, double>(M, Gu, (T*)P.Guv, nz, 5, false, 2)) != OCN_OK) return s;
+    if (Gv && (s = get_one<T, double>(M, Gv, (T*)P.Guv + 1, nz, 5, false, 2)) != OCN_OK) return s;
+    if (GT && (s = get_one<T, double>(M, GT, (T*)P.Gts, nz, 5, false, 2)) != OCN_OK) return s;
+    if (GS && (s = get_one<T, double>(M, GS, (T*)P.Gts + 1, nz, 5, false, 2)) != OCN_OK) return s;
     if (U && (s = get_one<T, double>(M, U, P.U[0], 1, 5, false)) != OCN_OK) return s;
     if (V && (s = get_one<T, double>(M, V, P.V[0], 1, 5, false)) != OCN_OK) return s;
     return OCN_OK;
@@ -517,7 +566,7 @@ ocn_status ocn_profile_read(ocn_model* M, double* ms, long long* launches, int r
 }
 
 const char* ocn_stage_name(int stage) {
-    static const char* names[OCN_NSTAGES] = {"tendency", "barotropic", "backsub_correct_pressure", "vertical_velocity"};
+    static const char* names[OCN_NSTAGES] = {"tendency", "barotropic", "backsub_correct_pressure"};
     return (stage >= 0 && stage < OCN_NSTAGES) ? names[stage] : "";
 }
 
