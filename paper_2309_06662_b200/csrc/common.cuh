@@ -143,6 +143,61 @@ __device__ __forceinline__ T weno_face(T a, T b, T c, T d, T e, T f, T vel, int 
     return order == 1 ? q0 : T(0);
 }
 
+// ---------------------------------------------------------------------------------------------
+// fp32 pair arithmetic (Blackwell packed fp32: add/mul/fma.rn.f32x2 -> SASS FADD2 / FMUL2 / FFMA2).
+// The (T, S) pair shares velocity, order and stencil geometry, and the two vorticity
+// reconstructions of a cell share the arithmetic, so one packed instruction serves both members.
+// The weights are the same division-free form as weno_face; the final quotient uses the
+// hardware reciprocal (2 ulp), well inside the fp32 tolerance.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ float2 f2(float a) { return make_float2(a, a); }
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ float2 mul2(float2 a, float2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
+
+// fifth-order face value from the upwind-ordered stencil (q0 = upwind cell)
+__device__ __forceinline__ float2 weno5_pair(float2 qm2, float2 qm1, float2 q0, float2 q1, float2 q2) {
+    const float2 p0 = fma2(f2(11.f / 6.f), q0, fma2(f2(-7.f / 6.f), qm1, mul2(f2(2.f / 6.f), qm2)));
+    const float2 p1 = fma2(f2(2.f / 6.f), q1, fma2(f2(5.f / 6.f), q0, mul2(f2(-1.f / 6.f), qm1)));
+    const float2 p2 = fma2(f2(-1.f / 6.f), q2, fma2(f2(5.f / 6.f), q1, mul2(f2(2.f / 6.f), q0)));
+    const float2 s0 = fma2(f2(-2.f), qm1, add2(qm2, q0)), t0 = fma2(f2(3.f), q0, fma2(f2(-4.f), qm1, qm2));
+    const float2 s1 = fma2(f2(-2.f), q0, add2(qm1, q1)), t1 = fma2(f2(-1.f), q1, qm1);
+    const float2 s2 = fma2(f2(-2.f), q1, add2(q0, q2)), t2 = fma2(f2(3.f), q0, fma2(f2(-4.f), q1, q2));
+    const float2 eps = f2(1e-6f), c13 = f2(13.f / 12.f), c4 = f2(0.25f);
+    const float2 b0 = fma2(mul2(c13, s0), s0, fma2(mul2(c4, t0), t0, eps));
+    const float2 b1 = fma2(mul2(c13, s1), s1, fma2(mul2(c4, t1), t1, eps));
+    const float2 b2 = fma2(mul2(c13, s2), s2, fma2(mul2(c4, t2), t2, eps));
+    const float2 b01 = mul2(b0, b1), b02 = mul2(b0, b2), b12 = mul2(b1, b2);
+    const float2 a0 = mul2(mul2(f2(0.1f), b12), b12), a1 = mul2(mul2(f2(0.6f), b02), b02), a2 = mul2(mul2(f2(0.3f), b01), b01);
+    const float2 num = fma2(a2, p2, fma2(a1, p1, mul2(a0, p0))), den = add2(add2(a0, a1), a2);
+    return make_float2(__fdividef(num.x, den.x), __fdividef(num.y, den.y));
+}
+__device__ __forceinline__ float2 weno3_pair(float2 qm1, float2 q0, float2 q1) {
+    const float2 p0 = fma2(f2(1.5f), q0, mul2(f2(-0.5f), qm1)), p1 = mul2(f2(0.5f), add2(q0, q1));
+    const float2 d0 = fma2(f2(-1.f), qm1, q0), d1 = fma2(f2(-1.f), q0, q1);
+    const float2 eps = f2(1e-6f);
+    const float2 b0 = fma2(d0, d0, eps), b1 = fma2(d1, d1, eps);
+    const float2 a0 = mul2(mul2(f2(1.f / 3.f), b1), b1), a1 = mul2(mul2(f2(2.f / 3.f), b0), b0);
+    const float2 num = fma2(a1, p1, mul2(a0, p0)), den = add2(a0, a1);
+    return make_float2(__fdividef(num.x, den.x), __fdividef(num.y, den.y));
+}
+
+// face value of a pair with one advecting velocity and one order code
+template <class T2, class T>
+__device__ __forceinline__ T2 weno_face2(T2 a, T2 b, T2 c, T2 d, T2 e, T2 f, T vel, int order) {
+    T2 r;
+    r.x = weno_face(a.x, b.x, c.x, d.x, e.x, f.x, vel, order);
+    r.y = weno_face(a.y, b.y, c.y, d.y, e.y, f.y, vel, order);
+    return r;
+}
+__device__ __forceinline__ float2 weno_face2(float2 a, float2 b, float2 c, float2 d, float2 e, float2 f, float vel, int order) {
+    const bool pos = vel > 0.f;
+    const float2 qm1 = pos ? b : e, q0 = pos ? c : d, q1 = pos ? d : c;
+    if (order >= 3) return weno5_pair(pos ? a : f, qm1, q0, q1, pos ? e : b);
+    if (order == 2) return weno3_pair(qm1, q0, q1);
+    return order == 1 ? q0 : make_float2(0.f, 0.f);
+}
+
 __device__ __forceinline__ int order3(int k, int t1, int t2, int t3) {
     return (k >= t1) + (k >= t2) + (k >= t3);
 }

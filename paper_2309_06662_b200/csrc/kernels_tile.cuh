@@ -43,15 +43,6 @@ __device__ __forceinline__ void tma_load_plane(void* dst, const CUtensorMap* map
                  ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(x), "r"(y), "r"(z) : "memory");
 }
 
-// WENO face value of a pair with one advecting velocity and one order code
-template <class T2, class T>
-__device__ __forceinline__ T2 weno_face2(T2 a, T2 b, T2 c, T2 d, T2 e, T2 f, T vel, int order) {
-    T2 r;
-    r.x = weno_face(a.x, b.x, c.x, d.x, e.x, f.x, vel, order);
-    r.y = weno_face(a.y, b.y, c.y, d.y, e.y, f.y, vel, order);
-    return r;
-}
-
 __host__ __device__ constexpr int rup128(int b) { return (b + 127) / 128 * 128; }
 
 template <class T, int TX_, int TY_>
@@ -89,8 +80,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     typedef typename C::T2 T2;
     typedef Ex<T> E;
     constexpr int BX = C::BX, BY = C::BY, RX = C::RX, RY = C::RY, NT = C::NT, OX = C::OX, OY = C::OY;
-    extern __shared__ unsigned char smem_raw[];
-    unsigned char* sm = (unsigned char*)(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
+    extern __shared__ __align__(1024) unsigned char sm[];     // dynamic only: starts the CTA's window, 1 KB aligned
     T* const s_zeta = (T*)(sm + C::O_ZETA);
     T2* const s_kd = (T2*)(sm + C::O_KD);
     T2* const s_fx = (T2*)(sm + C::O_FX);
@@ -102,7 +92,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     T* const s_rAzF = s_rAzC + (BY + 1);
     T* const s_rdxC = s_rAzF + (BY + 1);
     uint64_t* const bars = (uint64_t*)(sm + C::O_BAR);
-    __shared__ int s_kmin;
+    int& s_kmin = *(int*)(sm + C::O_BAR + 64);
 
     const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * TX + tx;
     const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;
@@ -262,7 +252,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                         const T u = s_uv[b].x;
                         const T ax = dy * dzk;
                         const T2 cw = s_ts[b - 1], cc = s_ts[b];
-                        const T2 fv = weno_face2<T2, T>(s_ts[b - 3], s_ts[b - 2], cw, cc, s_ts[b + 1], s_ts[b + 2], u, ord);
+                        const T2 fv = weno_face2(s_ts[b - 3], s_ts[b - 2], cw, cc, s_ts[b + 1], s_ts[b + 2], u, ord);
                         const T kd = P.kappa_h * ax * s_rdxC[fy + OY];
                         flux.x = u * ax * fv.x - kd * (cc.x - cw.x);
                         flux.y = u * ax * fv.y - kd * (cc.y - cw.y);
@@ -280,7 +270,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                         const T v = s_uv[b].y;
                         const T ay = s_dxF[gy + OY] * dzk;
                         const T2 cs = s_ts[b - BX], cc = s_ts[b];
-                        const T2 fv = weno_face2<T2, T>(s_ts[b - 3 * BX], s_ts[b - 2 * BX], cs, cc, s_ts[b + BX], s_ts[b + 2 * BX], v, ord);
+                        const T2 fv = weno_face2(s_ts[b - 3 * BX], s_ts[b - 2 * BX], cs, cc, s_ts[b + BX], s_ts[b + 2 * BX], v, ord);
                         const T kd = P.kappa_h * ay * rdy;
                         flux.x = v * ay * fv.x - kd * (cc.x - cs.x);
                         flux.y = v * ay * fv.y - kd * (cc.y - cs.y);
@@ -297,7 +287,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             const int ozt = (k + 1 < nz) ? min(3, min(k + 1 - kb, nz - k - 1)) : 0;
             if (ozt > 0) {
                 auto tsz = [&](int kk) -> T2 { return ((const T2*)(sm + C::O_TS + ((kk + C::R_TS) % C::R_TS) * C::PL2))[bo]; };
-                const T2 fv = weno_face2<T2, T>(tsz(k - 2), tsz(k - 1), tsz(k), tsz(k + 1), tsz(k + 2), tsz(k + 3), w_c1, ozt);
+                const T2 fv = weno_face2(tsz(k - 2), tsz(k - 1), tsz(k), tsz(k + 1), tsz(k + 2), tsz(k + 3), w_c1, ozt);
                 fz_top.x = w_c1 * AzCj * fv.x;
                 fz_top.y = w_c1 * AzCj * fv.y;
             }
