@@ -61,13 +61,21 @@ struct Tile {
     static constexpr int O_UV = O_TS + R_TS * PL2;
     static constexpr int O_P = O_UV + R_UV * PL2;
     static constexpr int O_ZETA = O_P + R_P * PL1;
-    static constexpr int O_KD = O_ZETA + PL1;                                   // T2 (K, D) on RX x RY
-    static constexpr int O_W = O_KD + rup128(RX * RY * (int)sizeof(T2));        // 2 buffers of T on RX x RY
-    static constexpr int O_FX = O_W + 2 * rup128(RX * RY * (int)sizeof(T));     // T2 on RX x TY
-    static constexpr int O_FY = O_FX + rup128(RX * TY * (int)sizeof(T2));       // T2 on TX x RY
-    static constexpr int O_M8 = O_FY + rup128(TX * RY * (int)sizeof(T2));       // uint2 on RX x RY
+    static constexpr int O_KD = O_ZETA + 2 * PL1;                               // 2 x T2 (K, D) on RX x RY
+    static constexpr int KDB = rup128(RX * RY * (int)sizeof(T2)), WB = rup128(RX * RY * (int)sizeof(T));
+    static constexpr int O_W = O_KD + 2 * KDB;                                  // 3 buffers of T on RX x RY
+    static constexpr int NFX = RX * TY, NFY = TX * RY, NF = NFX + NFY;        // west faces, then south faces
+    static constexpr int FLB = rup128(NF * (int)sizeof(T2));
+    static constexpr int O_FLUX = O_W + 3 * WB;                                 // 2 x T2 per face
+    static constexpr int O_M8 = O_FLUX + 2 * FLB;                               // uint2 on RX x RY (not zero-filled from here on)
     static constexpr int O_MET = O_M8 + rup128(RX * RY * 8);                    // 6 row-metric arrays of BY + 1
-    static constexpr int O_BAR = O_MET + rup128(6 * (BY + 1) * (int)sizeof(T));
+    static constexpr int O_CELL = O_MET + rup128(6 * (BY + 1) * (int)sizeof(T)); // uint16: cells sorted by first wet level
+    static constexpr int O_FS = O_CELL + rup128(NT * 2);                        // uint2: face descriptors sorted by first open level
+    static constexpr int O_NC = O_FS + rup128(NF * 8);                          // uint16[256]: active cells at level k
+    static constexpr int O_NF = O_NC + 512;                                     // uint16[256]: active faces at level k
+    static constexpr int O_BAR = O_NF + 512;
+    static constexpr int SORT_N = 1024;                                         // bitonic scratch (in the ts ring, before TMA starts)
+    static_assert(NF <= SORT_N && NT <= SORT_N && SORT_N * 4 <= R_TS * PL2, "sort scratch");
     static constexpr int SMEM = O_BAR + 128 + 128;                              // + alignment slack
 };
 
@@ -81,10 +89,10 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     typedef Ex<T> E;
     constexpr int BX = C::BX, BY = C::BY, RX = C::RX, RY = C::RY, NT = C::NT, OX = C::OX, OY = C::OY;
     extern __shared__ __align__(1024) unsigned char sm[];     // dynamic only: starts the CTA's window, 1 KB aligned
-    T* const s_zeta = (T*)(sm + C::O_ZETA);
-    T2* const s_kd = (T2*)(sm + C::O_KD);
-    T2* const s_fx = (T2*)(sm + C::O_FX);
-    T2* const s_fy = (T2*)(sm + C::O_FY);
+    unsigned short* const s_cell = (unsigned short*)(sm + C::O_CELL);
+    uint2* const s_fs = (uint2*)(sm + C::O_FS);
+    unsigned short* const s_nc = (unsigned short*)(sm + C::O_NC);
+    unsigned short* const s_nf = (unsigned short*)(sm + C::O_NF);
     uint2* const s_m8 = (uint2*)(sm + C::O_M8);
     T* const s_dxC = (T*)(sm + C::O_MET);
     T* const s_dxF = s_dxC + (BY + 1);
@@ -96,7 +104,6 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
 
     const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * TX + tx;
     const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;
-    const int i = i0 + tx, j = j0 + ty;
     const int nz = P.nz, sx = P.sx;
     const long long sz = P.sz;
 
@@ -123,6 +130,69 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     const int kmin = s_kmin;
     if (kmin >= nz) return;                              // all land: forcing sums stay zero
 
+    // ---- compaction lists: cells sorted by their first wet level, faces by their
+    // first open level, so that at level k the active work is a dense prefix of each list ----------
+    {
+        uint32_t* const key = (uint32_t*)sm;                              // scratch in the (still unused) ts ring
+        auto bitonic = [&](int n) {                                       // ascending sort of key[0 .. n), n a power of two
+            for (int k2 = 2; k2 <= n; k2 <<= 1)
+                for (int j2 = k2 >> 1; j2 > 0; j2 >>= 1) {
+                    for (int q = tid; q < n; q += NT) {
+                        const int x = q ^ j2;
+                        if (x > q) {
+                            const uint32_t a = key[q], b = key[x];
+                            if ((a > b) == ((q & k2) == 0)) { key[q] = b; key[x] = a; }
+                        }
+                    }
+                    __syncthreads();
+                }
+        };
+        auto count_le = [&](int n, int lev) {                             // number of keys with threshold <= lev
+            int lo = 0, hi = n;
+            while (lo < hi) { const int mid = (lo + hi) >> 1; if ((int)(key[mid] >> 16) <= lev) lo = mid + 1; else hi = mid; }
+            return lo;
+        };
+        // cells
+        {
+            const int gx = tid % TX, gy = tid / TX;
+            const bool in = i0 + gx < P.nx && j0 + gy < P.ny;
+            const uint32_t kbg = in ? (s_m8[gy * RX + gx].x & 255u) : (uint32_t)nz;
+            key[tid] = (kbg << 16) | (uint32_t)tid;
+        }
+        __syncthreads();
+        bitonic(NT);
+        s_cell[tid] = (unsigned short)(key[tid] & 0xffffu);
+        if (tid < 256) s_nc[tid] = (unsigned short)count_le(NT, tid);
+        __syncthreads();
+        // faces: fid < NFX = west face of cell (fid % RX, fid / RX); else south face of cell (g % TX, g / TX), g = fid - NFX
+        for (int q = tid; q < C::SORT_N; q += NT) {
+            uint32_t kq = 0xffffffffu;
+            if (q < C::NF) {
+                const bool isy = q >= C::NFX;
+                const int g = isy ? q - C::NFX : q;
+                const int fx = isy ? g % TX : g % RX, fy = isy ? g / TX : g / RX;
+                const uint2 m = s_m8[fy * RX + fx];
+                const uint32_t t1 = isy ? (m.y & 255u) : ((m.x >> 8) & 255u);
+                kq = (t1 << 16) | (uint32_t)q;
+            }
+            key[q] = kq;
+        }
+        __syncthreads();
+        bitonic(C::SORT_N);
+        for (int q = tid; q < C::NF; q += NT) {
+            const int fid = (int)(key[q] & 0xffffu);
+            const bool isy = fid >= C::NFX;
+            const int g = isy ? fid - C::NFX : fid;
+            const int fx = isy ? g % TX : g % RX, fy = isy ? g / TX : g / RX;
+            const uint2 m = s_m8[fy * RX + fx];
+            const uint32_t thr = isy ? (m.y & 0xffffffu) : (m.x >> 8);
+            const uint32_t b = (uint32_t)((fy + OY) * BX + fx + OX);
+            s_fs[q] = make_uint2(b | ((uint32_t)(fy + OY) << 10) | ((isy ? 1u : 0u) << 14) | ((uint32_t)fid << 16), thr);
+        }
+        if (tid < 256) s_nf[tid] = (unsigned short)min(count_le(C::SORT_N, tid), (int)C::NF);
+        __syncthreads();
+    }
+
     // ---- one-time shared-memory setup --------------------------------------------------------
     for (int q = tid; q < C::O_M8 / 16; q += NT) ((uint4*)sm)[q] = make_uint4(0u, 0u, 0u, 0u);
     {
@@ -140,29 +210,34 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // zero fill (generic) before TMA writes (async)
     __syncthreads();
 
-    // group(m) = the planes level m needs beyond those of level m - 1: ts(m + 3), uv(m + 1), p(m)
+    // Iteration m of the march does parts A(m) = phases 1 + 2 of level m and B(m - 1) = phase 3 of level
+    // m - 1, then ONE block barrier.  group(m) = the planes iteration m needs beyond those of iteration
+    // m - 1: ts(m + 2) (vertical stencil of B(m - 1)), uv(m), p(m - 1).
     auto issue_group = [&](int m, bool first) {
         uint64_t* bar = &bars[(m - kmin) % C::NB];
-        uint32_t bytes = C::BYTES1;
-        const int tlo = first ? max(m - 2, 0) : m + 3, thi = min(m + 3, nz - 1);
-        const int ulo = first ? m : m + 1, uhi = min(m + 1, nz - 1);
+        uint32_t bytes = 0;
+        const int tlo = first ? max(m - 3, 0) : m + 2, thi = min(m + 2, nz - 1);
         if (thi >= tlo) bytes += (uint32_t)(thi - tlo + 1) * C::BYTES2;
-        if (uhi >= ulo) bytes += (uint32_t)(uhi - ulo + 1) * C::BYTES2;
+        if (m < nz) bytes += C::BYTES2;
+        if (m - 1 >= kmin) bytes += C::BYTES1;
         mbar_expect_tx(bar, bytes);
         for (int q = tlo; q <= thi; ++q) tma_load_plane(sm + C::O_TS + (q % C::R_TS) * C::PL2, &m_ts, bar, 2 * i0, j0, q);
-        for (int q = ulo; q <= uhi; ++q) tma_load_plane(sm + C::O_UV + (q % C::R_UV) * C::PL2, &m_uv, bar, 2 * i0, j0, q);
-        tma_load_plane(sm + C::O_P + (m % C::R_P) * C::PL1, &m_p, bar, i0, j0, m);
+        if (m < nz) tma_load_plane(sm + C::O_UV + (m % C::R_UV) * C::PL2, &m_uv, bar, 2 * i0, j0, m);
+        if (m - 1 >= kmin) tma_load_plane(sm + C::O_P + ((m - 1) % C::R_P) * C::PL1, &m_p, bar, i0, j0, m - 1);
     };
     if (tid == 0) {
         issue_group(kmin, true);
 #pragma unroll
-        for (int d = 1; d < C::DP; ++d) if (kmin + d < nz) issue_group(kmin + d, false);
+        for (int d = 1; d < C::DP; ++d) if (kmin + d <= nz) issue_group(kmin + d, false);
     }
 
     // ---- per-thread column state ------------------------------------------------------------
+    const int g_own = s_cell[tid];                       // the cell this thread owns for the whole march
+    const int cx = g_own % TX, cy = g_own / TX;
+    const int i = i0 + cx, j = j0 + cy;
     const bool incol = i < P.nx && j < P.ny;
     const long long c = (long long)(j + OCN_HALO) * sx + i;
-    const uint2 m_own = s_m8[ty * RX + tx];
+    const uint2 m_own = s_m8[cy * RX + cx];
     const int kb = incol ? (int)(m_own.x & 255u) : nz;
     const int tx1 = incol ? (int)((m_own.x >> 8) & 255u) : nz, ty1 = incol ? (int)(m_own.y & 255u) : nz;
     uchar4 mzt = make_uchar4(255, 255, 255, 255);
@@ -173,7 +248,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     const T dxFj = P.dxF[rc], dxFn = P.dxF[rc + 1], rdxCj = P.rdxC[rc], rdxFj = P.rdxF[rc];
     const T AzCj = P.AzC[rc], AzCs = P.AzC[rc - 1], rAzCj = P.rAzC[rc], rAzFj = P.rAzF[rc];
     const T fFj = P.fF[rc], fFn = P.fF[rc + 1];
-    const int bx = tx + OX, by = ty + OY;                // this cell in box coordinates
+    const int bx = cx + OX, by = cy + OY;                // this cell in box coordinates
     const int bo = by * BX + bx;
 
     double wacc0 = 0.0, wacc1 = 0.0;                     // w accumulators of this thread's ring points
@@ -188,203 +263,192 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     const T* __restrict__ mmv = P.m_m + min(ty1, nz - 1) * nz;
     const T* __restrict__ rmv = P.rm_m + min(ty1, nz - 1) * nz;
 
-    for (int k = kmin; k < nz; ++k) {
-        const bool wetc = k >= kb;
-        const long long o = k * sz + c;
-        // AB2 history and pivots of this level: issued now, consumed in phase 3
+    for (int m = kmin; m <= nz; ++m) {
+        const int kB = m - 1;                                 // level of part B (phase 3) in this iteration
+        const bool doB = kB >= kmin, wetc = doB && kB >= kb;
+        const long long o = (long long)kB * sz + c;
+        // AB2 history and pivots of level kB: issued now, consumed after part A
         T2 gm_uv = mk2(T(0), T(0)), gm_ts = mk2(T(0), T(0));
         T piv_t = 1, piv_u = 1, piv_v = 1;
         if (wetc) {
             gm_uv = P.Guv[o]; gm_ts = P.Gts[o];
-            if (sizeof(T) == 8) { piv_t = mt[k]; piv_u = mmu[k]; piv_v = mmv[k]; }
-            else                { piv_t = rmt[k]; piv_u = rmu[k]; piv_v = rmv[k]; }
+            if (sizeof(T) == 8) { piv_t = mt[kB]; piv_u = mmu[kB]; piv_v = mmv[kB]; }
+            else                { piv_t = rmt[kB]; piv_u = rmu[kB]; piv_v = rmv[kB]; }
         }
-        const T dzk = P.dz[k], rdzk = P.rdz[k];
-        mbar_wait(&bars[(k - kmin) % C::NB], (uint32_t)(((k - kmin) / C::NB) & 1));
-        const T2* __restrict__ s_uv = (const T2*)(sm + C::O_UV + (k % C::R_UV) * C::PL2);
-        const T2* __restrict__ s_uv1 = (const T2*)(sm + C::O_UV + ((k + 1) % C::R_UV) * C::PL2);
-        const T* __restrict__ s_p = (const T*)(sm + C::O_P + (k % C::R_P) * C::PL1);
-        const T* __restrict__ s_w0 = (const T*)(sm + C::O_W + (k & 1) * rup128(RX * RY * (int)sizeof(T)));
-        T* __restrict__ s_w1 = (T*)(sm + C::O_W + ((k + 1) & 1) * rup128(RX * RY * (int)sizeof(T)));
+        mbar_wait(&bars[(m - kmin) % C::NB], (uint32_t)(((m - kmin) / C::NB) & 1));
 
-        // ================= phase 1: zeta, K, D, w[k+1] =================
-#pragma unroll
-        for (int h = 0; h < (BX - 1) * (BY - 1); h += NT) {
-            const int q = h + tid;
-            if (q < (BX - 1) * (BY - 1)) {
-                const int px = 1 + q % (BX - 1), py = 1 + q / (BX - 1);
-                const T2 a = s_uv[py * BX + px], as = s_uv[(py - 1) * BX + px], aw = s_uv[py * BX + px - 1];
-                s_zeta[py * BX + px] = (dy * (a.y - aw.y) - (s_dxC[py] * a.x - s_dxC[py - 1] * as.x)) * s_rAzF[py];
+        if (m < nz) {                                         // ---------------- part A: level k = m ----------------
+            const int k = m;
+            const T dzk = P.dz[k];
+            const T2* __restrict__ s_uv = (const T2*)(sm + C::O_UV + (k % C::R_UV) * C::PL2);
+            T* __restrict__ s_zeta = (T*)(sm + C::O_ZETA + (k & 1) * C::PL1);
+            T2* __restrict__ s_kd = (T2*)(sm + C::O_KD + (k & 1) * C::KDB);
+            T* __restrict__ s_w1 = (T*)(sm + C::O_W + ((k + 1) % 3) * C::WB);
+            T2* __restrict__ s_flux = (T2*)(sm + C::O_FLUX + (k & 1) * C::FLB);
+            // ================= phase 1: zeta, K, D, w[k+1] =================
+    #pragma unroll
+            for (int h = 0; h < (BX - 1) * (BY - 1); h += NT) {
+                const int q = h + tid;
+                if (q < (BX - 1) * (BY - 1)) {
+                    const int px = 1 + q % (BX - 1), py = 1 + q / (BX - 1);
+                    const T2 a = s_uv[py * BX + px], as = s_uv[(py - 1) * BX + px], aw = s_uv[py * BX + px - 1];
+                    s_zeta[py * BX + px] = (dy * (a.y - aw.y) - (s_dxC[py] * a.x - s_dxC[py - 1] * as.x)) * s_rAzF[py];
+                }
             }
-        }
-#pragma unroll
-        for (int h = 0, n = 0; h < RX * RY; h += NT, ++n) {
-            const int q = h + tid;
-            if (q < RX * RY) {
-                const int qx = q % RX, qy = q / RX;
-                const int px = qx + OX - 1, py = qy + OY - 1;          // cells i0 - 1 + qx, j0 - 1 + qy
-                const T2 a = s_uv[py * BX + px], ae = s_uv[py * BX + px + 1], an = s_uv[(py + 1) * BX + px];
-                const T Kc = T(0.25) * (a.x * a.x + ae.x * ae.x) + T(0.25) * (a.y * a.y + an.y * an.y);
-                const T Dc = (dy * (ae.x - a.x) + s_dxF[py + 1] * an.y - s_dxF[py] * a.y) * s_rAzC[py];
-                s_kd[q] = mk2(Kc, Dc);
-                double& wa = n == 0 ? wacc0 : wacc1;
-                wa -= (double)dzk * (double)Dc;
-                s_w1[q] = (T)wa;
+    #pragma unroll
+            for (int h = 0, n = 0; h < RX * RY; h += NT, ++n) {
+                const int q = h + tid;
+                if (q < RX * RY) {
+                    const int qx = q % RX, qy = q / RX;
+                    const int px = qx + OX - 1, py = qy + OY - 1;          // cells i0 - 1 + qx, j0 - 1 + qy
+                    const T2 a = s_uv[py * BX + px], ae = s_uv[py * BX + px + 1], an = s_uv[(py + 1) * BX + px];
+                    const T Kc = T(0.25) * (a.x * a.x + ae.x * ae.x) + T(0.25) * (a.y * a.y + an.y * an.y);
+                    const T Dc = (dy * (ae.x - a.x) + s_dxF[py + 1] * an.y - s_dxF[py] * a.y) * s_rAzC[py];
+                    s_kd[q] = mk2(Kc, Dc);
+                    double& wa = n == 0 ? wacc0 : wacc1;
+                    wa -= (double)dzk * (double)Dc;
+                    s_w1[q] = (T)wa;
+                }
             }
-        }
-        __syncthreads();
-
-        // ================= phase 2: tracer face fluxes, each face once =================
-        {
-            const T2* __restrict__ s_ts = (const T2*)(sm + C::O_TS + (k % C::R_TS) * C::PL2);
-            constexpr int NFX = RX * TY, NFY = TX * RY;
-#pragma unroll
-            for (int h = 0; h < NFX + NFY; h += NT) {
-                const int f = h + tid;
-                if (f < NFX) {                                           // west face of cell (fx, fy)
-                    const int fx = f % RX, fy = f / RX;
-                    const uint32_t mx = s_m8[fy * RX + fx].x;
-                    const int t1 = (mx >> 8) & 255u, t2 = (mx >> 16) & 255u, t3 = mx >> 24;
-                    const int ord = order3(k, t1, t2, t3);
-                    T2 flux = mk2(T(0), T(0));
-                    if (ord > 0) {
-                        const int b = (fy + OY) * BX + fx + OX;
-                        const T u = s_uv[b].x;
-                        const T ax = dy * dzk;
-                        const T2 cw = s_ts[b - 1], cc = s_ts[b];
-                        const T2 fv = weno_face2(s_ts[b - 3], s_ts[b - 2], cw, cc, s_ts[b + 1], s_ts[b + 2], u, ord);
-                        const T kd = P.kappa_h * ax * s_rdxC[fy + OY];
-                        flux.x = u * ax * fv.x - kd * (cc.x - cw.x);
-                        flux.y = u * ax * fv.y - kd * (cc.y - cw.y);
-                    }
-                    s_fx[f] = flux;
-                } else if (f < NFX + NFY) {                              // south face of cell (gx, gy)
-                    const int g = f - NFX;
-                    const int gx = g % TX, gy = g / TX;
-                    const uint32_t my = s_m8[gy * RX + gx].y;
-                    const int t1 = my & 255u, t2 = (my >> 8) & 255u, t3 = (my >> 16) & 255u;
-                    const int ord = order3(k, t1, t2, t3);
-                    T2 flux = mk2(T(0), T(0));
-                    if (ord > 0) {
-                        const int b = (gy + OY) * BX + gx + OX;
-                        const T v = s_uv[b].y;
-                        const T ay = s_dxF[gy + OY] * dzk;
-                        const T2 cs = s_ts[b - BX], cc = s_ts[b];
-                        const T2 fv = weno_face2(s_ts[b - 3 * BX], s_ts[b - 2 * BX], cs, cc, s_ts[b + BX], s_ts[b + 2 * BX], v, ord);
-                        const T kd = P.kappa_h * ay * rdy;
-                        flux.x = v * ay * fv.x - kd * (cc.x - cs.x);
-                        flux.y = v * ay * fv.y - kd * (cc.y - cs.y);
-                    }
-                    s_fy[g] = flux;
+            // ================= phase 2: tracer face fluxes, each open face once =================
+            {
+                const T2* __restrict__ s_ts = (const T2*)(sm + C::O_TS + (k % C::R_TS) * C::PL2);
+                const int nface = s_nf[k];
+                for (int f = tid; f < nface; f += NT) {
+                    const uint2 d = s_fs[f];
+                    const int b = d.x & 1023u, row = (d.x >> 10) & 15u, fid = d.x >> 16;
+                    const bool isy = (d.x >> 14) & 1u;
+                    const int st = isy ? BX : 1;
+                    const int ord = order3(k, d.y & 255u, (d.y >> 8) & 255u, (d.y >> 16) & 255u);   // >= 1 here
+                    const T2 uvf = s_uv[b];
+                    const T vel = isy ? uvf.y : uvf.x;
+                    const T area = (isy ? s_dxF[row] : dy) * dzk;
+                    const T kd = P.kappa_h * area * (isy ? rdy : s_rdxC[row]);
+                    const T2 cm = s_ts[b - st], cc = s_ts[b];
+                    const T2 fv = weno_face2(s_ts[b - 3 * st], s_ts[b - 2 * st], cm, cc, s_ts[b + st], s_ts[b + 2 * st], vel, ord);
+                    T2 flux;
+                    flux.x = vel * area * fv.x - kd * (cc.x - cm.x);
+                    flux.y = vel * area * fv.y - kd * (cc.y - cm.y);
+                    s_flux[fid] = flux;
                 }
             }
         }
-        // vertical face above cell k (own column)
-        const int qo = (ty + 1) * RX + tx + 1;                           // this column in the ring arrays
-        const T w_c1 = s_w1[qo], w_c0 = s_w0[qo];
-        T2 fz_top = mk2(T(0), T(0));
-        if (wetc) {
-            const int ozt = (k + 1 < nz) ? min(3, min(k + 1 - kb, nz - k - 1)) : 0;
-            if (ozt > 0) {
-                auto tsz = [&](int kk) -> T2 { return ((const T2*)(sm + C::O_TS + ((kk + C::R_TS) % C::R_TS) * C::PL2))[bo]; };
-                const T2 fv = weno_face2(tsz(k - 2), tsz(k - 1), tsz(k), tsz(k + 1), tsz(k + 2), tsz(k + 3), w_c1, ozt);
-                fz_top.x = w_c1 * AzCj * fv.x;
-                fz_top.y = w_c1 * AzCj * fv.y;
+        if (doB) {                                            // ---------------- part B: level k = m - 1 ----------------
+            const int k = kB;
+            const T dzk = P.dz[k], rdzk = P.rdz[k];
+            const T2* __restrict__ s_uv = (const T2*)(sm + C::O_UV + (k % C::R_UV) * C::PL2);
+            const T2* __restrict__ s_uv1 = (const T2*)(sm + C::O_UV + ((k + 1) % C::R_UV) * C::PL2);
+            const T* __restrict__ s_p = (const T*)(sm + C::O_P + (k % C::R_P) * C::PL1);
+            const T* __restrict__ s_w0 = (const T*)(sm + C::O_W + (k % 3) * C::WB);
+            const T* __restrict__ s_w1 = (const T*)(sm + C::O_W + ((k + 1) % 3) * C::WB);
+            const T* __restrict__ s_zeta = (const T*)(sm + C::O_ZETA + (k & 1) * C::PL1);
+            const T2* __restrict__ s_kd = (const T2*)(sm + C::O_KD + (k & 1) * C::KDB);
+            const T2* __restrict__ s_flux = (const T2*)(sm + C::O_FLUX + (k & 1) * C::FLB);
+            // vertical face above cell k (own column)
+            const int qo = (cy + 1) * RX + cx + 1;                           // this column in the ring arrays
+            const T w_c1 = s_w1[qo], w_c0 = s_w0[qo];
+            T2 fz_top = mk2(T(0), T(0));
+            if (wetc) {
+                const int ozt = (k + 1 < nz) ? min(3, min(k + 1 - kb, nz - k - 1)) : 0;
+                if (ozt > 0) {
+                    auto tsz = [&](int kk) -> T2 { return ((const T2*)(sm + C::O_TS + ((kk + C::R_TS) % C::R_TS) * C::PL2))[bo]; };
+                    const T2 fv = weno_face2(tsz(k - 2), tsz(k - 1), tsz(k), tsz(k + 1), tsz(k + 2), tsz(k + 3), w_c1, ozt);
+                    fz_top.x = w_c1 * AzCj * fv.x;
+                    fz_top.y = w_c1 * AzCj * fv.y;
+                }
             }
-        }
-        __syncthreads();
-
-        // ================= phase 3: tendencies of this cell, AB2, elimination =================
-        if (wetc) {
-            const bool mu = k >= tx1, mv = k >= ty1;
-            // ---- tracers ----
-            const T2 fw = s_fx[ty * RX + tx], fe = s_fx[ty * RX + tx + 1];
-            const T2 fs = s_fy[ty * TX + tx], fn = s_fy[(ty + 1) * TX + tx];
-            const T2 tsc = ((const T2*)(sm + C::O_TS + (k % C::R_TS) * C::PL2))[bo];
-            T GT = -((fe.x - fw.x) + (fn.x - fs.x) + (fz_top.x - fz_bot.x)) * rAzCj * rdzk;
-            T GS = -((fe.y - fw.y) + (fn.y - fs.y) + (fz_top.y - fz_bot.y)) * rAzCj * rdzk;
-            if (k == nz - 1) {                 // tracers are stored as offsets from (Toff, Soff): exact source
-                const T src = w_c1 * rdzk;     // of the constant under the zero-top-flux linear free surface
-                GT += P.Toff * src; GS += P.Soff * src;
-            }
-            // ---- momentum ----
-            const T2 uvc = s_uv[bo];
-            const T u_c = uvc.x, v_c = uvc.y;
-            T Gu = 0, Gv = 0;
-            if (mu | mv) {
-                const T2 uv_w = s_uv[bo - 1], uv_n = s_uv[bo + BX], uv_nw = s_uv[bo + BX - 1];
-                const T2 uv_s = s_uv[bo - BX], uv_e = s_uv[bo + 1], uv_se = s_uv[bo - BX + 1];
-                const T2 uv_up = (k + 1 < nz) ? s_uv1[bo] : mk2(T(0), T(0));
-                const T z00 = s_zeta[bo];
-                const T2 kdc = s_kd[qo];
-                const T pc = s_p[bo];
+            // ================= phase 3: tendencies of this cell, AB2, elimination =================
+            if (wetc) {
+                const bool mu = k >= tx1, mv = k >= ty1;
+                // ---- tracers ----
+                const T2 fw = s_flux[cy * RX + cx], fe = s_flux[cy * RX + cx + 1];
+                const T2 fs = s_flux[C::NFX + cy * TX + cx], fn = s_flux[C::NFX + (cy + 1) * TX + cx];
+                const T2 tsc = ((const T2*)(sm + C::O_TS + (k % C::R_TS) * C::PL2))[bo];
+                T GT = -((fe.x - fw.x) + (fn.x - fs.x) + (fz_top.x - fz_bot.x)) * rAzCj * rdzk;
+                T GS = -((fe.y - fw.y) + (fn.y - fs.y) + (fz_top.y - fz_bot.y)) * rAzCj * rdzk;
+                if (k == nz - 1) {                 // tracers are stored as offsets from (Toff, Soff): exact source
+                    const T src = w_c1 * rdzk;     // of the constant under the zero-top-flux linear free surface
+                    GT += P.Toff * src; GS += P.Soff * src;
+                }
+                // ---- momentum ----
+                const T2 uvc = s_uv[bo];
+                const T u_c = uvc.x, v_c = uvc.y;
+                T Gu = 0, Gv = 0;
+                if (mu | mv) {
+                    const T2 uv_w = s_uv[bo - 1], uv_n = s_uv[bo + BX], uv_nw = s_uv[bo + BX - 1];
+                    const T2 uv_s = s_uv[bo - BX], uv_e = s_uv[bo + 1], uv_se = s_uv[bo - BX + 1];
+                    const T2 uv_up = (k + 1 < nz) ? s_uv1[bo] : mk2(T(0), T(0));
+                    const T z00 = s_zeta[bo];
+                    const T2 kdc = s_kd[qo];
+                    const T pc = s_p[bo];
+                    if (mu) {
+                        const T vsum_s = uv_w.y + v_c, vsum_n = uv_nw.y + uv_n.y;
+                        const T vhat = T(0.25) * (dxFj * vsum_s + dxFn * vsum_n) * rdxCj;
+                        const int ozu = 1 + (k >= mzt.x) + (k >= mzt.y);
+                        const T z01 = s_zeta[bo + BX];
+                        const T zt = ozu == 1 ? (vhat > T(0) ? z00 : z01)
+                                              : weno_face(s_zeta[bo - 2 * BX], s_zeta[bo - BX], z00, z01, s_zeta[bo + 2 * BX],
+                                                          s_zeta[bo + 3 * BX], vhat, ozu);
+                        const T Cu = T(0.5) * (fFj * T(0.5) * dxFj * vsum_s + fFn * T(0.5) * dxFn * vsum_n) * rdxCj;
+                        const T2 kdw = s_kd[qo - 1];
+                        const T dK = (kdc.x - kdw.x) * rdxCj;
+                        const T dP = (pc - s_p[bo - 1]) * rdxCj;
+                        const T dlo = (k >= 1 && k - 1 >= tx1) ? u_c - u_dn : T(0);
+                        const T dhi = (k + 1 <= nz - 1) ? uv_up.x - u_c : T(0);
+                        const T Au = T(0.5) * (T(0.5) * (s_w1[qo - 1] + w_c1) * dhi + T(0.5) * (s_w0[qo - 1] + w_c0) * dlo) * rdzk;
+                        const T Vu = P.nu_h * ((kdc.y - kdw.y) * rdxCj - (z01 - z00) * rdy);
+                        const T tau = (k == nz - 1) ? P.taux[c] * P.rrho0 * rdzk : T(0);
+                        Gu = zt * vhat + Cu - dK - dP - Au + Vu + tau;
+                    }
+                    if (mv) {
+                        const T uhat = T(0.25) * (uv_s.x + u_c + uv_se.x + uv_e.x);
+                        const int ozv = 1 + (k >= mzt.z) + (k >= mzt.w);
+                        const T z10 = s_zeta[bo + 1];
+                        const T zt = ozv == 1 ? (uhat > T(0) ? z00 : z10)
+                                              : weno_face(s_zeta[bo - 2], s_zeta[bo - 1], z00, z10, s_zeta[bo + 2], s_zeta[bo + 3], uhat, ozv);
+                        const T Cv = fFj * uhat;
+                        const T2 kds = s_kd[qo - RX];
+                        const T dK = (kdc.x - kds.x) * rdy;
+                        const T dP = (pc - s_p[bo - BX]) * rdy;
+                        const T dlo = (k >= 1 && k - 1 >= ty1) ? v_c - v_dn : T(0);
+                        const T dhi = (k + 1 <= nz - 1) ? uv_up.y - v_c : T(0);
+                        const T Av = T(0.5) * (T(0.5) * (AzCs * s_w1[qo - RX] + AzCj * w_c1) * dhi
+                                             + T(0.5) * (AzCs * s_w0[qo - RX] + AzCj * w_c0) * dlo) * rAzFj * rdzk;
+                        const T Vv = P.nu_h * ((kdc.y - kds.y) * rdy + (z10 - z00) * rdxFj);
+                        const T tau = (k == nz - 1) ? P.tauy[c] * P.rrho0 * rdzk : T(0);
+                        Gv = -zt * uhat - Cv - dK - dP - Av + Vv + tau;
+                    }
+                }
+                // ---- quasi-AB2, predictor, elimination sweep (S3, S4, S5) ----
+                const T Ghu = c0 * Gu - c1 * gm_uv.x, Ghv = c0 * Gv - c1 * gm_uv.y;
+                const T Ght = c0 * GT - c1 * gm_ts.x, Ghs = c0 * GS - c1 * gm_ts.y;
+                P.Guv[o] = mk2(Gu, Gv);
+                P.Gts[o] = mk2(GT, GS);
                 if (mu) {
-                    const T vsum_s = uv_w.y + v_c, vsum_n = uv_nw.y + uv_n.y;
-                    const T vhat = T(0.25) * (dxFj * vsum_s + dxFn * vsum_n) * rdxCj;
-                    const int ozu = 1 + (k >= mzt.x) + (k >= mzt.y);
-                    const T z01 = s_zeta[bo + BX];
-                    const T zt = ozu == 1 ? (vhat > T(0) ? z00 : z01)
-                                          : weno_face(s_zeta[bo - 2 * BX], s_zeta[bo - BX], z00, z01, s_zeta[bo + 2 * BX],
-                                                      s_zeta[bo + 3 * BX], vhat, ozu);
-                    const T Cu = T(0.5) * (fFj * T(0.5) * dxFj * vsum_s + fFn * T(0.5) * dxFn * vsum_n) * rdxCj;
-                    const T2 kdw = s_kd[qo - 1];
-                    const T dK = (kdc.x - kdw.x) * rdxCj;
-                    const T dP = (pc - s_p[bo - 1]) * rdxCj;
-                    const T dlo = (k >= 1 && k - 1 >= tx1) ? u_c - u_dn : T(0);
-                    const T dhi = (k + 1 <= nz - 1) ? uv_up.x - u_c : T(0);
-                    const T Au = T(0.5) * (T(0.5) * (s_w1[qo - 1] + w_c1) * dhi + T(0.5) * (s_w0[qo - 1] + w_c0) * dlo) * rdzk;
-                    const T Vu = P.nu_h * ((kdc.y - kdw.y) * rdxCj - (z01 - z00) * rdy);
-                    const T tau = (k == nz - 1) ? P.taux[c] * P.rrho0 * rdzk : T(0);
-                    Gu = zt * vhat + Cu - dK - dP - Au + Vu + tau;
+                    const T us = E::add(u_c, E::mul(P.dt, Ghu));
+                    aGU += (double)dzk * (double)Ghu; aSU += (double)dzk * (double)us;
+                    const T smk = k > tx1 ? P.sm_m[k] : T(0);
+                    dduv.x = E::div(E::add(us, E::mul(smk, dduv.x)), piv_u, piv_u);
                 }
                 if (mv) {
-                    const T uhat = T(0.25) * (uv_s.x + u_c + uv_se.x + uv_e.x);
-                    const int ozv = 1 + (k >= mzt.z) + (k >= mzt.w);
-                    const T z10 = s_zeta[bo + 1];
-                    const T zt = ozv == 1 ? (uhat > T(0) ? z00 : z10)
-                                          : weno_face(s_zeta[bo - 2], s_zeta[bo - 1], z00, z10, s_zeta[bo + 2], s_zeta[bo + 3], uhat, ozv);
-                    const T Cv = fFj * uhat;
-                    const T2 kds = s_kd[qo - RX];
-                    const T dK = (kdc.x - kds.x) * rdy;
-                    const T dP = (pc - s_p[bo - BX]) * rdy;
-                    const T dlo = (k >= 1 && k - 1 >= ty1) ? v_c - v_dn : T(0);
-                    const T dhi = (k + 1 <= nz - 1) ? uv_up.y - v_c : T(0);
-                    const T Av = T(0.5) * (T(0.5) * (AzCs * s_w1[qo - RX] + AzCj * w_c1) * dhi
-                                         + T(0.5) * (AzCs * s_w0[qo - RX] + AzCj * w_c0) * dlo) * rAzFj * rdzk;
-                    const T Vv = P.nu_h * ((kdc.y - kds.y) * rdy + (z10 - z00) * rdxFj);
-                    const T tau = (k == nz - 1) ? P.tauy[c] * P.rrho0 * rdzk : T(0);
-                    Gv = -zt * uhat - Cv - dK - dP - Av + Vv + tau;
+                    const T vs2 = E::add(v_c, E::mul(P.dt, Ghv));
+                    aGV += (double)dzk * (double)Ghv; aSV += (double)dzk * (double)vs2;
+                    const T smk = k > ty1 ? P.sm_m[k] : T(0);
+                    dduv.y = E::div(E::add(vs2, E::mul(smk, dduv.y)), piv_v, piv_v);
                 }
+                {
+                    const T smk = k > kb ? P.sm_t[k] : T(0);
+                    ddts.x = E::div(E::add(E::add(tsc.x, E::mul(P.dt, Ght)), E::mul(smk, ddts.x)), piv_t, piv_t);
+                    ddts.y = E::div(E::add(E::add(tsc.y, E::mul(P.dt, Ghs)), E::mul(smk, ddts.y)), piv_t, piv_t);
+                }
+                P.duv[o] = dduv;
+                P.dts[o] = ddts;
+                u_dn = u_c; v_dn = v_c;
             }
-            // ---- quasi-AB2, predictor, elimination sweep (S3, S4, S5) ----
-            const T Ghu = c0 * Gu - c1 * gm_uv.x, Ghv = c0 * Gv - c1 * gm_uv.y;
-            const T Ght = c0 * GT - c1 * gm_ts.x, Ghs = c0 * GS - c1 * gm_ts.y;
-            P.Guv[o] = mk2(Gu, Gv);
-            P.Gts[o] = mk2(GT, GS);
-            if (mu) {
-                const T us = E::add(u_c, E::mul(P.dt, Ghu));
-                aGU += (double)dzk * (double)Ghu; aSU += (double)dzk * (double)us;
-                const T smk = k > tx1 ? P.sm_m[k] : T(0);
-                dduv.x = E::div(E::add(us, E::mul(smk, dduv.x)), piv_u, piv_u);
-            }
-            if (mv) {
-                const T vs2 = E::add(v_c, E::mul(P.dt, Ghv));
-                aGV += (double)dzk * (double)Ghv; aSV += (double)dzk * (double)vs2;
-                const T smk = k > ty1 ? P.sm_m[k] : T(0);
-                dduv.y = E::div(E::add(vs2, E::mul(smk, dduv.y)), piv_v, piv_v);
-            }
-            {
-                const T smk = k > kb ? P.sm_t[k] : T(0);
-                ddts.x = E::div(E::add(E::add(tsc.x, E::mul(P.dt, Ght)), E::mul(smk, ddts.x)), piv_t, piv_t);
-                ddts.y = E::div(E::add(E::add(tsc.y, E::mul(P.dt, Ghs)), E::mul(smk, ddts.y)), piv_t, piv_t);
-            }
-            P.duv[o] = dduv;
-            P.dts[o] = ddts;
-            u_dn = u_c; v_dn = v_c;
+            fz_bot = fz_top;
         }
-        fz_bot = fz_top;
-        __syncthreads();                       // every plane of level k is dead: refill the ring
-        if (tid == 0 && k + C::DP < nz) issue_group(k + C::DP, false);
+        __syncthreads();                       // planes of level m - 1 are dead: refill the ring
+        if (tid == 0 && m + C::DP <= nz) issue_group(m + C::DP, false);
     }
     if (incol && kb < nz) { P.GU[c] = (T)aGU; P.GV[c] = (T)aGV; P.SU[c] = (T)aSU; P.SV[c] = (T)aSV; }
 }
