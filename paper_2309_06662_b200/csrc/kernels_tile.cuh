@@ -74,8 +74,6 @@ struct Tile {
     static constexpr int O_NC = O_FS + rup128(NF * 8);                          // uint16[256]: active cells at level k
     static constexpr int O_NF = O_NC + 512;                                     // uint16[256]: active faces at level k
     static constexpr int O_BAR = O_NF + 512;
-    static constexpr int SORT_N = 1024;                                         // bitonic scratch (in the ts ring, before TMA starts)
-    static_assert(NF <= SORT_N && NT <= SORT_N && SORT_N * 4 <= R_TS * PL2, "sort scratch");
     static constexpr int SMEM = O_BAR + 128 + 128;                              // + alignment slack
 };
 
@@ -131,66 +129,80 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     if (kmin >= nz) return;                              // all land: forcing sums stay zero
 
     // ---- compaction lists: cells sorted by their first wet level, faces by their
-    // first open level, so that at level k the active work is a dense prefix of each list ----------
+    // first open level (stable counting sort on the 8-bit level), so that at level k the active work
+    // is a dense prefix of each list and keeps the geometric order (coalescing) within a level ------
     {
-        uint32_t* const key = (uint32_t*)sm;                              // scratch in the (still unused) ts ring
-        auto bitonic = [&](int n) {                                       // ascending sort of key[0 .. n), n a power of two
-            for (int k2 = 2; k2 <= n; k2 <<= 1)
-                for (int j2 = k2 >> 1; j2 > 0; j2 >>= 1) {
-                    for (int q = tid; q < n; q += NT) {
-                        const int x = q ^ j2;
-                        if (x > q) {
-                            const uint32_t a = key[q], b = key[x];
-                            if ((a > b) == ((q & k2) == 0)) { key[q] = b; key[x] = a; }
-                        }
-                    }
-                    __syncthreads();
+        constexpr int MAXR = (C::NF + NT - 1) / NT;                      // rounds of NT items
+        unsigned short* const cnt = (unsigned short*)sm;                  // [virtual warp][key], scratch in the unused ts ring
+        int* const base = (int*)(sm + MAXR * (NT / 32) * 256 * 2);        // [key] exclusive prefix, then [256 + w] warp sums
+        static_assert(MAXR * (NT / 32) * 512 + 2048 <= C::R_TS * C::PL2, "sort scratch");
+        const int lane = tid & 31, wrp = tid >> 5;
+        // sorts items 0 .. n-1 by keyf(q) in [0, 255]; emit(q, rank); nle[k] = number of items with key <= k
+        auto csort = [&](const int n, auto keyf, auto emit, unsigned short* nle) {
+            const int nr = (n + NT - 1) / NT;
+            for (int q = tid; q < nr * (NT / 32) * 256; q += NT) cnt[q] = 0;
+            __syncthreads();
+            int kq[MAXR], lr[MAXR];
+#pragma unroll
+            for (int r = 0; r < MAXR; ++r) {
+                const int q = r * NT + tid;
+                const bool on = r < nr && q < n;
+                const unsigned act = __ballot_sync(0xffffffffu, on);
+                kq[r] = 0; lr[r] = 0;
+                if (on) {
+                    kq[r] = keyf(q);
+                    const unsigned peers = __match_any_sync(act, kq[r]);
+                    lr[r] = __popc(peers & ((1u << lane) - 1u));
+                    if (lr[r] == 0) cnt[(r * (NT / 32) + wrp) * 256 + kq[r]] = (unsigned short)__popc(peers);
                 }
-        };
-        auto count_le = [&](int n, int lev) {                             // number of keys with threshold <= lev
-            int lo = 0, hi = n;
-            while (lo < hi) { const int mid = (lo + hi) >> 1; if ((int)(key[mid] >> 16) <= lev) lo = mid + 1; else hi = mid; }
-            return lo;
-        };
-        // cells
-        {
-            const int gx = tid % TX, gy = tid / TX;
-            const bool in = i0 + gx < P.nx && j0 + gy < P.ny;
-            const uint32_t kbg = in ? (s_m8[gy * RX + gx].x & 255u) : (uint32_t)nz;
-            key[tid] = (kbg << 16) | (uint32_t)tid;
-        }
-        __syncthreads();
-        bitonic(NT);
-        s_cell[tid] = (unsigned short)(key[tid] & 0xffffu);
-        if (tid < 256) s_nc[tid] = (unsigned short)count_le(NT, tid);
-        __syncthreads();
-        // faces: fid < NFX = west face of cell (fid % RX, fid / RX); else south face of cell (g % TX, g / TX), g = fid - NFX
-        for (int q = tid; q < C::SORT_N; q += NT) {
-            uint32_t kq = 0xffffffffu;
-            if (q < C::NF) {
-                const bool isy = q >= C::NFX;
-                const int g = isy ? q - C::NFX : q;
-                const int fx = isy ? g % TX : g % RX, fy = isy ? g / TX : g / RX;
-                const uint2 m = s_m8[fy * RX + fx];
-                const uint32_t t1 = isy ? (m.y & 255u) : ((m.x >> 8) & 255u);
-                kq = (t1 << 16) | (uint32_t)q;
             }
-            key[q] = kq;
-        }
-        __syncthreads();
-        bitonic(C::SORT_N);
-        for (int q = tid; q < C::NF; q += NT) {
-            const int fid = (int)(key[q] & 0xffffu);
-            const bool isy = fid >= C::NFX;
+            __syncthreads();
+            {                                                             // thread t owns key t
+                int run = 0;
+                for (int vw = 0; vw < nr * (NT / 32); ++vw) {
+                    const int cc = cnt[vw * 256 + tid];
+                    cnt[vw * 256 + tid] = (unsigned short)run;
+                    run += cc;
+                }
+                int inc = run;                                            // block-wide inclusive scan of the key totals
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
+                if (lane == 31) base[256 + wrp] = inc;
+                __syncthreads();
+                int off = 0;
+                for (int w = 0; w < wrp; ++w) off += base[256 + w];
+                base[tid] = off + inc - run;
+                nle[tid] = (unsigned short)(off + inc);
+            }
+            __syncthreads();
+#pragma unroll
+            for (int r = 0; r < MAXR; ++r) {
+                const int q = r * NT + tid;
+                if (r < nr && q < n) emit(q, base[kq[r]] + (int)cnt[(r * (NT / 32) + wrp) * 256 + kq[r]] + lr[r]);
+            }
+            __syncthreads();
+        };
+        static_assert(NT == 256, "one thread per key");
+        csort(NT,
+              [&](int q) { const int gx = q % TX, gy = q / TX;
+                           return (i0 + gx < P.nx && j0 + gy < P.ny) ? (int)(s_m8[gy * RX + gx].x & 255u) : nz; },
+              [&](int q, int rank) { s_cell[rank] = (unsigned short)q; }, s_nc);
+        // faces: fid < NFX = west face of cell (fid % RX, fid / RX); else south face of cell (g % TX, g / TX), g = fid - NFX
+        auto face_cell = [&](int fid, bool& isy, int& fx, int& fy) {
+            isy = fid >= C::NFX;
             const int g = isy ? fid - C::NFX : fid;
-            const int fx = isy ? g % TX : g % RX, fy = isy ? g / TX : g / RX;
-            const uint2 m = s_m8[fy * RX + fx];
-            const uint32_t thr = isy ? (m.y & 0xffffffu) : (m.x >> 8);
-            const uint32_t b = (uint32_t)((fy + OY) * BX + fx + OX);
-            s_fs[q] = make_uint2(b | ((uint32_t)(fy + OY) << 10) | ((isy ? 1u : 0u) << 14) | ((uint32_t)fid << 16), thr);
-        }
-        if (tid < 256) s_nf[tid] = (unsigned short)min(count_le(C::SORT_N, tid), (int)C::NF);
-        __syncthreads();
+            fx = isy ? g % TX : g % RX; fy = isy ? g / TX : g / RX;
+        };
+        csort(C::NF,
+              [&](int q) { bool isy; int fx, fy; face_cell(q, isy, fx, fy);
+                           const uint2 m = s_m8[fy * RX + fx];
+                           return (int)(isy ? (m.y & 255u) : ((m.x >> 8) & 255u)); },
+              [&](int fid, int rank) { bool isy; int fx, fy; face_cell(fid, isy, fx, fy);
+                           const uint2 m = s_m8[fy * RX + fx];
+                           const uint32_t thr = isy ? (m.y & 0xffffffu) : (m.x >> 8);
+                           const uint32_t bb = (uint32_t)((fy + OY) * BX + fx + OX);
+                           s_fs[rank] = make_uint2(bb | ((uint32_t)(fy + OY) << 10) | ((isy ? 1u : 0u) << 14) | ((uint32_t)fid << 16), thr); },
+              s_nf);
     }
 
     // ---- one-time shared-memory setup --------------------------------------------------------
