@@ -52,7 +52,7 @@ struct DevP {
     T hz_top;                      // zf[nz] - zc[nz-1]
     // Thomas tables, bottom-up elimination in the oracle's order.  Momentum (nu_z)
     // and tracers (kappa_z).  sm[k]: sub-diagonal s^-_k (open face below); cp/m/rm are indexed
-    // [kf * nz + k] by the column's first open level kf: cp = modified super-diagonal, m = pivot,
+    // [k * nz + kf] by the column's first open level kf: cp = modified super-diagonal, m = pivot,
     // rm = 1 / m.
     const T *sm_m, *cp_m, *m_m, *rm_m;
     const T *sm_t, *cp_t, *m_t, *rm_t;

@@ -79,29 +79,43 @@ __global__ void __launch_bounds__(128) k_backsub_correct(const DevP<T> P) {
     if (kb >= nz) return;
     const T cu = tx1 < nz ? (P.Ub[c] - P.SU[c]) * P.rHu[c] : T(0);
     const T cv = ty1 < nz ? (P.Vb[c] - P.SV[c]) * P.rHv[c] : T(0);
-    const T* __restrict__ cpu = P.cp_m + min(tx1, nz - 1) * nz;
-    const T* __restrict__ cpv = P.cp_m + min(ty1, nz - 1) * nz;
-    const T* __restrict__ cpt = P.cp_t + kb * nz;
+    const T* __restrict__ cpu = P.cp_m + min(tx1, nz - 1);
+    const T* __restrict__ cpv = P.cp_m + min(ty1, nz - 1);
+    const T* __restrict__ cpt = P.cp_t + kb;
     T xu = 0, xv = 0, xt = 0, xs = 0, b1 = 0, pk = 0;
-    for (int k = nz - 1; k >= kb; --k) {
-        const long long o = k * sz + c;
-        const T2 d_ts = P.dts[o];
-        const T ck = cpt[k];
-        xt = E::sub(d_ts.x, E::mul(ck, xt));                         // cp[nz-1] = 0
-        xs = E::sub(d_ts.y, E::mul(ck, xs));
-        store_halo(P.ts + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, mk2(xt, xs));
-        const T b0 = buoyancy(P, xt, xs);
-        pk = k == nz - 1 ? -E::mul(b0, P.hz_top)
-                         : E::sub(pk, E::mul(E::mul(T(0.5), E::add(b1, b0)), P.dzc[k + 1]));
-        b1 = b0;
-        store_halo(P.p + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, pk);
-        const bool mu = k >= tx1, mv = k >= ty1;
-        if (mu | mv) {
-            const T2 d_uv = P.duv[o];
-            T un = 0, vn = 0;
-            if (mu) { xu = E::sub(d_uv.x, E::mul(cpu[k], xu)); un = xu + cu; }
-            if (mv) { xv = E::sub(d_uv.y, E::mul(cpv[k], xv)); vn = xv + cv; }
-            store_halo(P.uv + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, mk2(un, vn));
+    const int kuv = min(tx1, ty1);
+    constexpr int NB = 4;                                  // levels whose loads are in flight together
+    for (int k0 = nz - 1; k0 >= kb; k0 -= NB) {
+        T2 d_ts[NB], d_uv[NB];
+#pragma unroll
+        for (int q = 0; q < NB; ++q) {
+            const int k = k0 - q;
+            d_ts[q] = mk2(T(0), T(0)); d_uv[q] = mk2(T(0), T(0));
+            if (k >= kb) {
+                d_ts[q] = P.dts[k * sz + c];
+                if (k >= kuv) d_uv[q] = P.duv[k * sz + c];
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < NB; ++q) {
+            const int k = k0 - q;
+            if (k < kb) break;
+            const T ck = cpt[k * nz];
+            xt = E::sub(d_ts[q].x, E::mul(ck, xt));                      // cp[nz-1] = 0
+            xs = E::sub(d_ts[q].y, E::mul(ck, xs));
+            store_halo(P.ts + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, mk2(xt, xs));
+            const T b0 = buoyancy(P, xt, xs);
+            pk = k == nz - 1 ? -E::mul(b0, P.hz_top)
+                             : E::sub(pk, E::mul(E::mul(T(0.5), E::add(b1, b0)), P.dzc[k + 1]));
+            b1 = b0;
+            store_halo(P.p + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, pk);
+            const bool mu = k >= tx1, mv = k >= ty1;
+            if (mu | mv) {
+                T un = 0, vn = 0;
+                if (mu) { xu = E::sub(d_uv[q].x, E::mul(cpu[k * nz], xu)); un = xu + cu; }
+                if (mv) { xv = E::sub(d_uv[q].y, E::mul(cpv[k * nz], xv)); vn = xv + cv; }
+                store_halo(P.uv + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, mk2(un, vn));
+            }
         }
     }
 }

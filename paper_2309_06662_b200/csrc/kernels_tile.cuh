@@ -268,12 +268,12 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     T u_dn = 0, v_dn = 0;
     T2 dduv = mk2(T(0), T(0)), ddts = mk2(T(0), T(0));   // eliminated right-hand sides of the level below
     double aGU = 0, aGV = 0, aSU = 0, aSV = 0;
-    const T* __restrict__ mt = P.m_t + min(kb, nz - 1) * nz;
-    const T* __restrict__ rmt = P.rm_t + min(kb, nz - 1) * nz;
-    const T* __restrict__ mmu = P.m_m + min(tx1, nz - 1) * nz;
-    const T* __restrict__ rmu = P.rm_m + min(tx1, nz - 1) * nz;
-    const T* __restrict__ mmv = P.m_m + min(ty1, nz - 1) * nz;
-    const T* __restrict__ rmv = P.rm_m + min(ty1, nz - 1) * nz;
+    const T* __restrict__ mt = P.m_t + min(kb, nz - 1);
+    const T* __restrict__ rmt = P.rm_t + min(kb, nz - 1);
+    const T* __restrict__ mmu = P.m_m + min(tx1, nz - 1);
+    const T* __restrict__ rmu = P.rm_m + min(tx1, nz - 1);
+    const T* __restrict__ mmv = P.m_m + min(ty1, nz - 1);
+    const T* __restrict__ rmv = P.rm_m + min(ty1, nz - 1);
 
     for (int m = kmin; m <= nz; ++m) {
         const int kB = m - 1;                                 // level of part B (phase 3) in this iteration
@@ -284,8 +284,8 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
         T piv_t = 1, piv_u = 1, piv_v = 1;
         if (wetc) {
             gm_uv = P.Guv[o]; gm_ts = P.Gts[o];
-            if (sizeof(T) == 8) { piv_t = mt[kB]; piv_u = mmu[kB]; piv_v = mmv[kB]; }
-            else                { piv_t = rmt[kB]; piv_u = rmu[kB]; piv_v = rmv[kB]; }
+            if (sizeof(T) == 8) { piv_t = mt[kB * nz]; piv_u = mmu[kB * nz]; piv_v = mmv[kB * nz]; }
+            else                { piv_t = rmt[kB * nz]; piv_u = rmu[kB * nz]; piv_v = rmv[kB * nz]; }
         }
         mbar_wait(&bars[(m - kmin) % C::NB], (uint32_t)(((m - kmin) / C::NB) & 1));
 

@@ -158,7 +158,7 @@ ocn_status build_model(ocn_model* M) {
     P.dy = (T)g->dy; P.rdy = (T)(1.0 / g->dy);
     P.hz_top = (T)(g->zf[nz] - g->zc[nz - 1]);
     // Thomas tables: bottom-up elimination started at the column's first open
-    // level kf; sub-diagonal sm[k], and per (kf, k) the pivot m, its reciprocal and the modified
+    // level kf; sub-diagonal sm[k], and per (k, kf) the pivot m, its reciprocal and the modified
     // super-diagonal cp, computed in fp64 exactly as the equations of DESIGN.md §3.8 step 4 are written
     for (int pass = 0; pass < 2; ++pass) {
         const double dtk = M->d.dt * (pass == 0 ? M->d.nu_z : M->d.kappa_z);
@@ -173,7 +173,7 @@ ocn_status build_model(ocn_model* M) {
                 const double lo = -smk, up = -sp;
                 const double m = (k == kf) ? b : b - lo * cprev;
                 cprev = up / m;
-                cp[(size_t)kf * nz + k] = cprev; mm[(size_t)kf * nz + k] = m; rm[(size_t)kf * nz + k] = 1.0 / m;
+                cp[(size_t)k * nz + kf] = cprev; mm[(size_t)k * nz + kf] = m; rm[(size_t)k * nz + kf] = 1.0 / m;   // [k][kf]: a warp works at one k
             }
         }
         if (pass == 0) {
