@@ -68,8 +68,8 @@ struct Tile {
     static constexpr int FLB = rup128(NF * (int)sizeof(T2));
     static constexpr int O_FLUX = O_W + 3 * WB;                                 // 2 x T2 per face
     static constexpr int O_M8 = O_FLUX + 2 * FLB;                               // uint2 on RX x RY (not zero-filled from here on)
-    static constexpr int O_MET = O_M8 + rup128(RX * RY * 8);                    // 6 row-metric arrays of BY + 1
-    static constexpr int O_CELL = O_MET + rup128(6 * (BY + 1) * (int)sizeof(T)); // uint16: cells sorted by first wet level
+    static constexpr int O_MET = O_M8 + rup128(RX * RY * 8);                    // 8 row-metric arrays of BY + 1
+    static constexpr int O_CELL = O_MET + rup128(8 * (BY + 1) * (int)sizeof(T)); // uint16: cells sorted by first wet level
     static constexpr int O_FS = O_CELL + rup128(NT * 2);                        // uint2: face descriptors sorted by first open level
     static constexpr int O_NC = O_FS + rup128(NF * 8);                          // uint16[256]: active cells at level k
     static constexpr int O_NF = O_NC + 512;                                     // uint16[256]: active faces at level k
@@ -97,6 +97,9 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     T* const s_rAzC = s_dxF + (BY + 1);
     T* const s_rAzF = s_rAzC + (BY + 1);
     T* const s_rdxC = s_rAzF + (BY + 1);
+    T* const s_AzC = s_rdxC + (BY + 1);
+    T* const s_fF = s_AzC + (BY + 1);
+    T* const s_rdxF = s_fF + (BY + 1);
     uint64_t* const bars = (uint64_t*)(sm + C::O_BAR);
     int& s_kmin = *(int*)(sm + C::O_BAR + 64);
 
@@ -212,6 +215,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
         for (int q = tid; q <= BY; q += NT) {
             const int r = min(j0 + q, nr - 1);
             s_dxC[q] = P.dxC[r]; s_dxF[q] = P.dxF[r]; s_rAzC[q] = P.rAzC[r]; s_rAzF[q] = P.rAzF[r]; s_rdxC[q] = P.rdxC[r];
+            s_AzC[q] = P.AzC[r]; s_fF[q] = P.fF[r]; s_rdxF[q] = P.rdxF[r];
         }
     }
     if (tid == 0) {
@@ -254,12 +258,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     const int tx1 = incol ? (int)((m_own.x >> 8) & 255u) : nz, ty1 = incol ? (int)(m_own.y & 255u) : nz;
     uchar4 mzt = make_uchar4(255, 255, 255, 255);
     if (kb < nz) mzt = P.mz[c];
-    const int r = j + OCN_HALO;                          // row-metric index of this thread's row
-    const int rc = min(r, P.ny + 2 * OCN_HALO - 1);
     const T dy = P.dy, rdy = P.rdy;
-    const T dxFj = P.dxF[rc], dxFn = P.dxF[rc + 1], rdxCj = P.rdxC[rc], rdxFj = P.rdxF[rc];
-    const T AzCj = P.AzC[rc], AzCs = P.AzC[rc - 1], rAzCj = P.rAzC[rc], rAzFj = P.rAzF[rc];
-    const T fFj = P.fF[rc], fFn = P.fF[rc + 1];
     const int bx = cx + OX, by = cy + OY;                // this cell in box coordinates
     const int bo = by * BX + bx;
 
@@ -268,12 +267,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     T u_dn = 0, v_dn = 0;
     T2 dduv = mk2(T(0), T(0)), ddts = mk2(T(0), T(0));   // eliminated right-hand sides of the level below
     double aGU = 0, aGV = 0, aSU = 0, aSV = 0;
-    const T* __restrict__ mt = P.m_t + min(kb, nz - 1);
-    const T* __restrict__ rmt = P.rm_t + min(kb, nz - 1);
-    const T* __restrict__ mmu = P.m_m + min(tx1, nz - 1);
-    const T* __restrict__ rmu = P.rm_m + min(tx1, nz - 1);
-    const T* __restrict__ mmv = P.m_m + min(ty1, nz - 1);
-    const T* __restrict__ rmv = P.rm_m + min(ty1, nz - 1);
+    const int kbc = min(kb, nz - 1), txc = min(tx1, nz - 1), tyc = min(ty1, nz - 1);   // pivot-table columns
 
     for (int m = kmin; m <= nz; ++m) {
         const int kB = m - 1;                                 // level of part B (phase 3) in this iteration
@@ -284,8 +278,8 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
         T piv_t = 1, piv_u = 1, piv_v = 1;
         if (wetc) {
             gm_uv = P.Guv[o]; gm_ts = P.Gts[o];
-            if (sizeof(T) == 8) { piv_t = mt[kB * nz]; piv_u = mmu[kB * nz]; piv_v = mmv[kB * nz]; }
-            else                { piv_t = rmt[kB * nz]; piv_u = rmu[kB * nz]; piv_v = rmv[kB * nz]; }
+            if (sizeof(T) == 8) { piv_t = P.m_t[kB * nz + kbc]; piv_u = P.m_m[kB * nz + txc]; piv_v = P.m_m[kB * nz + tyc]; }
+            else                { piv_t = P.rm_t[kB * nz + kbc]; piv_u = P.rm_m[kB * nz + txc]; piv_v = P.rm_m[kB * nz + tyc]; }
         }
         mbar_wait(&bars[(m - kmin) % C::NB], (uint32_t)(((m - kmin) / C::NB) & 1));
 
@@ -300,7 +294,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             // ================= phase 1: zeta, K, D, w[k+1] =================
     #pragma unroll
             for (int h = 0; h < (BX - 1) * (BY - 1); h += NT) {
-                const int q = h + tid;
+                const int q = h + (NT - 1 - tid);
                 if (q < (BX - 1) * (BY - 1)) {
                     const int px = 1 + q % (BX - 1), py = 1 + q / (BX - 1);
                     const T2 a = s_uv[py * BX + px], as = s_uv[(py - 1) * BX + px], aw = s_uv[py * BX + px - 1];
@@ -309,7 +303,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             }
     #pragma unroll
             for (int h = 0, n = 0; h < RX * RY; h += NT, ++n) {
-                const int q = h + tid;
+                const int q = h + (NT - 1 - tid);
                 if (q < RX * RY) {
                     const int qx = q % RX, qy = q / RX;
                     const int px = qx + OX - 1, py = qy + OY - 1;          // cells i0 - 1 + qx, j0 - 1 + qy
@@ -326,7 +320,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             {
                 const T2* __restrict__ s_ts = (const T2*)(sm + C::O_TS + (k % C::R_TS) * C::PL2);
                 const int nface = s_nf[k];
-                for (int f = tid; f < nface; f += NT) {
+                for (int f = NT - 1 - tid; f < nface; f += NT) {
                     const uint2 d = s_fs[f];
                     const int b = d.x & 1023u, row = (d.x >> 10) & 15u, fid = d.x >> 16;
                     const bool isy = (d.x >> 14) & 1u;
@@ -351,6 +345,9 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             const T2* __restrict__ s_uv = (const T2*)(sm + C::O_UV + (k % C::R_UV) * C::PL2);
             const T2* __restrict__ s_uv1 = (const T2*)(sm + C::O_UV + ((k + 1) % C::R_UV) * C::PL2);
             const T* __restrict__ s_p = (const T*)(sm + C::O_P + (k % C::R_P) * C::PL1);
+            const T dxFj = s_dxF[by], dxFn = s_dxF[by + 1], rdxCj = s_rdxC[by], rdxFj = s_rdxF[by];
+            const T AzCj = s_AzC[by], AzCs = s_AzC[by - 1], rAzCj = s_rAzC[by], rAzFj = s_rAzF[by];
+            const T fFj = s_fF[by], fFn = s_fF[by + 1];
             const T* __restrict__ s_w0 = (const T*)(sm + C::O_W + (k % 3) * C::WB);
             const T* __restrict__ s_w1 = (const T*)(sm + C::O_W + ((k + 1) % 3) * C::WB);
             const T* __restrict__ s_zeta = (const T*)(sm + C::O_ZETA + (k & 1) * C::PL1);
