@@ -102,7 +102,7 @@ ocn_status ocn_model_info(const ocn_model* model, int* launches_per_step, unsign
 
 /* Per-stage device timing (used by bench.py for the roofline of the dominant kernel).
  * Stages: 0 = K1 fused tendency / AB2 / elimination, 1 = barotropic sub-cycle (all M sub-steps +
- * finish), 2 = K3 back-substitution / correction / pressure.  (w is recomputed on the fly inside
+ * finish; the sub-cycle runs BT_HALO sub-steps per launch on shared-memory tiles), 2 = K3 back-substitution / correction / pressure.  (w is recomputed on the fly inside
  * K1 and written out only when ocn_get_fields asks for it.)
  * While enabled, ocn_time_step launches the kernels of a step directly (no CUDA graph) and
  * records a CUDA event on the model's stream between stages.  ocn_profile_read synchronises

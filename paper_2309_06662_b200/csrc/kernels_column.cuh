@@ -14,37 +14,125 @@ __device__ __forceinline__ T buoyancy(const DevP<T>& P, T t, T s) {
 }
 
 // ---------------------------------------------------------------------------------------------
-// S6: one forward-backward barotropic sub-step (DESIGN.md §3.8 step 6): eta first, then U, V
-// with the new eta.  eta is recomputed redundantly for the west and south neighbours so that
-// one launch advances the whole sub-step.  Reads buffer `cur`, writes buffer `cur ^ 1`.
+// S6, resident form: one launch advances `ns` (<= BT_HALO) forward-backward
+// sub-steps of a (BTX x BTY) tile held in shared memory together with a halo of BT_HALO columns
+// that is recomputed redundantly and shrinks by one ring per sub-step — the paper's wide-halo
+// idea for the barotropic mode applied to the on-chip tile, so eta, U, V make one
+// HBM round trip per `ns` sub-steps instead of one per sub-step.  Periodic directions are wrapped
+// when the tile is loaded (no physical halo is needed), bounded ones read land.
+// Reads buffer `cur`, writes buffer `cur ^ 1`; the filter sums live in registers during the launch.
 // ---------------------------------------------------------------------------------------------
-template <class T>
-__global__ void __launch_bounds__(256) k_barotropic(const DevP<T> P, const int cur, const T am, const int first) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const int j = blockIdx.y * blockDim.y + threadIdx.y;
-    if (i >= P.nx || j >= P.ny) return;
-    const int sx = P.sx, nz = P.nz, r = j + OCN_HALO;
-    const long long c = (long long)r * sx + i;
+#define BT_HALO 6
+
+template <class T, int BTX, int BTY>
+struct BtTile {
+    static constexpr int EX = BTX + 2 * BT_HALO, EY = BTY + 2 * BT_HALO, NE = EX * EY;
+    static constexpr int NT = 512, PER = (BTX * BTY + NT - 1) / NT;
+    static constexpr int SMEM = NE * (7 * (int)sizeof(T) + 1) + 4 * (EY + 1) * (int)sizeof(T) + 64 + BT_HALO * (int)sizeof(T);
+};
+
+template <class T, int BTX, int BTY>
+__global__ void __launch_bounds__(512) k_barotropic_tile(const DevP<T> P, const int cur, const int ns, const int first,
+                                                         const T a0, const T a1, const T a2, const T a3, const T a4, const T a5) {
+    typedef BtTile<T, BTX, BTY> C;
+    constexpr int EX = C::EX, EY = C::EY, NE = C::NE, NT = C::NT, H = BT_HALO;
+    extern __shared__ __align__(16) unsigned char smb[];
+    T* const se = (T*)smb;                 // eta
+    T* const sU = se + NE;
+    T* const sV = sU + NE;
+    T* const sGU = sV + NE;
+    T* const sGV = sGU + NE;
+    T* const sHu = sGV + NE;
+    T* const sHv = sHu + NE;
+    T* const rAz = sHv + NE;               // per extended row: 1 / AzC, 1 / dxC, dxF (row), dxF (row + 1)
+    T* const rdx = rAz + (EY + 1);
+    T* const dF = rdx + (EY + 1);          // EY + 1 entries
+    T* const saw = dF + (EY + 1);          // filter weights of this launch
+    unsigned char* const smk = (unsigned char*)(saw + BT_HALO);   // bit 0 wet, bit 1 open u face, bit 2 open v face
+    const int tid = threadIdx.x;
+    const int i0 = blockIdx.x * BTX, j0 = blockIdx.y * BTY;
+    const int nx = P.nx, ny = P.ny, nz = P.nz, sx = P.sx;
+    if (tid == 0) { saw[0] = a0; saw[1] = a1; saw[2] = a2; saw[3] = a3; saw[4] = a4; saw[5] = a5; }
+
+    // ---- load the extended tile (wrap / land) ----
+    for (int q = tid; q <= EY; q += NT) {
+        int jj = j0 - H + q;
+        if (P.py) jj = ((jj % ny) + ny) % ny;
+        const int r = min(max(jj, -OCN_HALO), ny + OCN_HALO) + OCN_HALO;      // metric rows exist for -3 .. ny + 3
+        if (q < EY) { rAz[q] = P.rAzC[r]; rdx[q] = P.rdxC[r]; }
+        dF[q] = P.dxF[r];
+    }
     const T* __restrict__ e0 = P.eta[cur];
     const T* __restrict__ U0 = P.U[cur];
     const T* __restrict__ V0 = P.V[cur];
-    const uint2 m = P.m8[c];
-    const bool wet_c = (m.x & 255) < nz, wet_w = (P.m8[c - 1].x & 255) < nz, wet_s = (P.m8[c - sx].x & 255) < nz;
-    const bool mu = ((m.x >> 8) & 255) < nz, mv = (m.y & 255) < nz;
-    const T dy = P.dy, dtau = P.dtau;
-    const T dF0 = P.dxF[r], dF1 = P.dxF[r + 1], dFm = P.dxF[r - 1];
-    const T Uc = U0[c], Vc = V0[c];
-    T ec = e0[c], ew = e0[c - 1], es = e0[c - sx];
-    if (wet_c) ec -= dtau * (dy * (U0[c + 1] - Uc) + dF1 * V0[c + sx] - dF0 * Vc) * P.rAzC[r];
-    if (wet_w) ew -= dtau * (dy * (Uc - U0[c - 1]) + dF1 * V0[c + sx - 1] - dF0 * V0[c - 1]) * P.rAzC[r];
-    if (wet_s) es -= dtau * (dy * (U0[c - sx + 1] - U0[c - sx]) + dF0 * Vc - dFm * V0[c - sx]) * P.rAzC[r - 1];
-    const T Un = mu ? Uc + dtau * (-P.g * P.Hu[c] * (ec - ew) * P.rdxC[r] + P.GU[c]) : T(0);
-    const T Vn = mv ? Vc + dtau * (-P.g * P.Hv[c] * (ec - es) * P.rdy + P.GV[c]) : T(0);
-    store_halo(P.eta[cur ^ 1], sx, P.nx, P.ny, P.px, P.py, j, i, ec);
-    store_halo(P.U[cur ^ 1], sx, P.nx, P.ny, P.px, P.py, j, i, Un);
-    store_halo(P.V[cur ^ 1], sx, P.nx, P.ny, P.px, P.py, j, i, Vn);
-    if (first) { P.etab[c] = am * ec; P.Ub[c] = am * Un; P.Vb[c] = am * Vn; }
-    else       { P.etab[c] += am * ec; P.Ub[c] += am * Un; P.Vb[c] += am * Vn; }
+    for (int q = tid; q < NE; q += NT) {
+        const int x = q % EX, y = q / EX;
+        int ii = i0 - H + x, jj = j0 - H + y;
+        bool in = true;
+        if (P.px) ii = ((ii % nx) + nx) % nx; else in = in && ii >= 0 && ii < nx;
+        if (P.py) jj = ((jj % ny) + ny) % ny; else in = in && jj >= 0 && jj < ny;
+        T e = 0, u = 0, v = 0, gu = 0, gv = 0, hu = 0, hv = 0;
+        unsigned char mk = 0;
+        if (in) {
+            const long long c = (long long)(jj + OCN_HALO) * sx + ii;
+            const uint2 m = P.m8[c];
+            mk = (unsigned char)(((m.x & 255u) < (unsigned)nz ? 1 : 0) | ((((m.x >> 8) & 255u) < (unsigned)nz) ? 2 : 0) |
+                                 (((m.y & 255u) < (unsigned)nz) ? 4 : 0));
+            if (mk) { e = e0[c]; u = U0[c]; v = V0[c]; gu = P.GU[c]; gv = P.GV[c]; hu = P.Hu[c]; hv = P.Hv[c]; }
+        }
+        se[q] = e; sU[q] = u; sV[q] = v; smk[q] = mk;
+        sGU[q] = gu; sGV[q] = gv; sHu[q] = hu; sHv[q] = hv;
+    }
+    __syncthreads();
+
+    // ---- the interior points this thread owns, and their filter sums ----
+    T be[C::PER], bU[C::PER], bV[C::PER];
+#pragma unroll
+    for (int n = 0; n < C::PER; ++n) { be[n] = 0; bU[n] = 0; bV[n] = 0; }
+    const T dy = P.dy, dtau = P.dtau, g = P.g, rdy = P.rdy;
+
+    for (int s = 0; s < ns; ++s) {
+        // eta: valid on [s, EX - 1 - s) x [s, EY - 1 - s) given U, V valid on [s, EX - s) x [s, EY - s)
+        for (int q = tid; q < NE; q += NT) {
+            const int x = q % EX, y = q / EX;
+            if (x < EX - 1 && y < EY - 1 && (smk[q] & 1))
+                se[q] -= dtau * (dy * (sU[q + 1] - sU[q]) + dF[y + 1] * sV[q + EX] - dF[y] * sV[q]) * rAz[y];
+        }
+        __syncthreads();
+        for (int q = tid; q < NE; q += NT) {
+            const int x = q % EX, y = q / EX;
+            const unsigned char mk = smk[q];
+            const T ec = se[q];
+            if (x > 0) sU[q] = (mk & 2) ? sU[q] + dtau * (-g * sHu[q] * (ec - se[q - 1]) * rdx[y] + sGU[q]) : T(0);
+            if (y > 0) sV[q] = (mk & 4) ? sV[q] + dtau * (-g * sHv[q] * (ec - se[q - EX]) * rdy + sGV[q]) : T(0);
+        }
+        __syncthreads();
+        const T am = saw[s];
+#pragma unroll
+        for (int n = 0; n < C::PER; ++n) {
+            const int t = n * NT + tid;
+            if (t < BTX * BTY) {
+                const int q = (t / BTX + H) * EX + (t % BTX) + H;
+                be[n] += am * se[q]; bU[n] += am * sU[q]; bV[n] += am * sV[q];
+            }
+        }
+    }
+    // ---- write back the interior ----
+#pragma unroll
+    for (int n = 0; n < C::PER; ++n) {
+        const int t = n * NT + tid;
+        if (t < BTX * BTY) {
+            const int tx = t % BTX, ty = t / BTX;
+            const int i = i0 + tx, j = j0 + ty;
+            if (i < nx && j < ny) {
+                const int q = (ty + H) * EX + tx + H;
+                const long long c = (long long)(j + OCN_HALO) * sx + i;
+                P.eta[cur ^ 1][c] = se[q]; P.U[cur ^ 1][c] = sU[q]; P.V[cur ^ 1][c] = sV[q];
+                if (first) { P.etab[c] = be[n]; P.Ub[c] = bU[n]; P.Vb[c] = bV[n]; }
+                else       { P.etab[c] += be[n]; P.Ub[c] += bU[n]; P.Vb[c] += bV[n]; }
+            }
+        }
+    }
 }
 
 // step 7: the filtered values become the barotropic state (buffer 0, with halos)

@@ -3,6 +3,7 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cstdio>
 #include <cstring>
 #include <string>
@@ -86,6 +87,7 @@ template <> ocn::DevP<float>& params<float>(ocn_model* M) { return M->pf; }
 template <> ocn::DevP<double>& params<double>(ocn_model* M) { return M->pd; }
 
 constexpr int TILE_X = 32, TILE_Y = 8;    // K1 tile (kernels_tile.cuh)
+constexpr int BT_X = 64, BT_Y = 32;       // barotropic tile (kernels_column.cuh)
 
 // TMA descriptor of a halo'd 3-D array seen as [levels][rows][inner] scalars
 ocn_status make_tmap(CUtensorMap* tm, bool f64, void* base, unsigned long long inner, unsigned long long rows,
@@ -210,7 +212,7 @@ ocn_status build_model(ocn_model* M) {
     }
     CK(cudaMalloc(&M->stage, (size_t)(nz + 1) * g->ny * g->nx * sizeof(double)));
     M->bytes += (size_t)(nz + 1) * g->ny * g->nx * sizeof(double);
-    M->launches_per_step = M->d.substeps + 3;
+    M->launches_per_step = (M->d.substeps + BT_HALO - 1) / BT_HALO + 3;
     // TMA descriptors: box origin (i0 - 4, j0 - 3), so the map starts 4 elements before (row -3, i = 0)
     {
         typedef ocn::Tile<T, TILE_X, TILE_Y> C;
@@ -221,6 +223,8 @@ ocn_status build_model(ocn_model* M) {
             (s = make_tmap(&M->tm_p, f64, P.p - C::OX, sxu, syu, nz, C::BX, C::BY)) != OCN_OK)
             return s;
         CK(cudaFuncSetAttribute(ocn::k_tendency_tile<T, TILE_X, TILE_Y>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
+        CK(cudaFuncSetAttribute(ocn::k_barotropic_tile<T, BT_X, BT_Y>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                ocn::BtTile<T, BT_X, BT_Y>::SMEM));
     }
     return OCN_OK;
 }
@@ -276,13 +280,21 @@ ocn_status launch_step(ocn_model* M, bool euler) {
         ocn::k_tendency_tile<T, TILE_X, TILE_Y><<<grid2(g, bt), bt, C::SMEM, M->stream>>>(P, c0, c1, M->tm_ts, M->tm_uv, M->tm_p);
     }
     MARK(0, 1);
-    int cur = 0;
-    for (int m = 1; m <= M->d.substeps; ++m) {
-        ocn::k_barotropic<T><<<grid2(g, b2), b2, 0, M->stream>>>(P, cur, (T)M->a_w[m - 1], m == 1 ? 1 : 0);
-        cur ^= 1;
+    {
+        typedef ocn::BtTile<T, BT_X, BT_Y> B;
+        const dim3 gb((g->nx + BT_X - 1) / BT_X, (g->ny + BT_Y - 1) / BT_Y);
+        int cur = 0;
+        for (int m0 = 0; m0 < M->d.substeps; m0 += BT_HALO) {
+            const int ns = std::min(BT_HALO, M->d.substeps - m0);
+            T a[BT_HALO];
+            for (int q = 0; q < BT_HALO; ++q) a[q] = q < ns ? (T)M->a_w[m0 + q] : T(0);
+            ocn::k_barotropic_tile<T, BT_X, BT_Y><<<gb, B::NT, B::SMEM, M->stream>>>(P, cur, ns, m0 == 0 ? 1 : 0, a[0], a[1], a[2],
+                                                                                 a[3], a[4], a[5]);
+            cur ^= 1;
+        }
     }
     ocn::k_barotropic_finish<T><<<grid2(g, b2), b2, 0, M->stream>>>(P);
-    MARK(1, M->d.substeps + 1);
+    MARK(1, (M->d.substeps + BT_HALO - 1) / BT_HALO + 1);
     ocn::k_backsub_correct<T><<<grid2(g, bc), bc, 0, M->stream>>>(P);
     MARK(2, 1);
 #undef MARK
