@@ -27,12 +27,12 @@ __device__ __forceinline__ T buoyancy(const DevP<T>& P, T t, T s) {
 template <class T, int BTX, int BTY>
 struct BtTile {
     static constexpr int EX = BTX + 2 * BT_HALO, EY = BTY + 2 * BT_HALO, NE = EX * EY;
-    static constexpr int NT = 512, PER = (BTX * BTY + NT - 1) / NT;
+    static constexpr int NT = 1024, PER = (BTX * BTY + NT - 1) / NT;
     static constexpr int SMEM = NE * (7 * (int)sizeof(T) + 1) + 4 * (EY + 1) * (int)sizeof(T) + 64 + BT_HALO * (int)sizeof(T);
 };
 
 template <class T, int BTX, int BTY>
-__global__ void __launch_bounds__(512) k_barotropic_tile(const DevP<T> P, const int cur, const int ns, const int first,
+__global__ void __launch_bounds__(1024) k_barotropic_tile(const DevP<T> P, const int cur, const int ns, const int first,
                                                          const T a0, const T a1, const T a2, const T a3, const T a4, const T a5) {
     typedef BtTile<T, BTX, BTY> C;
     constexpr int EX = C::EX, EY = C::EY, NE = C::NE, NT = C::NT, H = BT_HALO;
