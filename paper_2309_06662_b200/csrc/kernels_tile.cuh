@@ -104,7 +104,13 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     int& s_kmin = *(int*)(sm + C::O_BAR + 64);
 
     const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * TX + tx;
-    const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;
+    // rasterisation: tiles are taken in bands of RB tile-rows, y fastest inside a band, so that the
+    // tiles resident together form a compact patch and their halo planes are shared through L2
+    constexpr int RB = 4;
+    const int bid = blockIdx.x + gridDim.x * blockIdx.y;
+    const int band = bid / (RB * (int)gridDim.x), inb = bid - band * RB * (int)gridDim.x;
+    const int rows = min(RB, (int)gridDim.y - band * RB);
+    const int i0 = (inb / rows) * TX, j0 = (band * RB + inb % rows) * TY;
     const int nz = P.nz, sx = P.sx;
     const long long sz = P.sz;
 
