@@ -197,7 +197,7 @@ def wet_cells(model):
 def run_ours(args):
     import torch
     from paper_2309_06662_b200 import build as ocn_build
-    from paper_2309_06662_b200 import ocn, workloads as W
+    from paper_2309_06662_b200 import ocn, replicas, workloads as W
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -227,17 +227,10 @@ def run_ours(args):
     info = model.info()
 
     def barrier():
-        torch.cuda.synchronize()
-        if dist is not None:
-            dist.barrier()
-            torch.cuda.synchronize()
+        replicas.barrier(dist, torch.cuda.synchronize)
 
     def max_over_ranks(x):
-        if dist is None:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return replicas.max_over_ranks(x, dist, device="cuda")
 
     # ---- device-resident timing: K steps of the production path (one CUDA graph launch per step) ----
     model.time_step(Wm)
@@ -259,7 +252,7 @@ def run_ours(args):
     model.profile_enable(False)
     clk = clocks.stop()
     sec_per_step = ms_total * 1e-3 / K
-    value = world * cells * K / (ms_total * 1e-3)
+    value = replicas.aggregate_throughput(cells, K, ms_total, world)
 
     # finite check of the state the timed steps produced (d2h of eta only)
     eta = model.get_fields(names=("eta",))["eta"]

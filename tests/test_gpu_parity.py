@@ -122,3 +122,63 @@ def test_tau_only_update_keeps_history():
     a, b = gpu.get_fields(), ref.get_fields()
     for n in FIELDS:
         assert rel_linf(a[n], b[n]) <= 1e-11, n
+
+
+# ---------------------------------------------------------------------------------------------
+# full sizes, in the launch configuration bench.py times
+# ---------------------------------------------------------------------------------------------
+def test_config4_full_size_matches_oracle_inside_a_window():
+    """The full 2880x1200x100 fp32 grid is stepped twice on the GPU; the oracle steps a 300x220x100 window cut from
+    the same seeded fields as a closed box.  One step has a finite domain of dependence (3 cells of stencil + one cell
+    per barotropic sub-step = 43 cells), so after 2 steps every point further than 86 cells from the window's walls
+    must agree with the full-size run: those are outputs the oracle can compute, compared element by element."""
+    j0, j1, i0, i1 = 450, 670, 1250, 1550
+    steps, margin = 2, 2 * (40 + 3) + 2
+    full = W.config4()
+    gpu = ocn.Model(full)
+    gpu.time_step(steps)
+    a = gpu.get_fields()
+    dbg_ok = all(np.isfinite(a[n]).all() for n in FIELDS)
+    gpu.close()
+    assert dbg_ok
+    del full
+    win = W.config4(window=(j0, j1, i0, i1))
+    ref = oracle.RefModel(win)
+    ref.step(steps)
+    b = ref.get_fields()
+    js, je, is_, ie = margin, (j1 - j0) - margin, margin, (i1 - i0) - margin
+    assert je - js >= 40 and ie - is_ >= 100
+    for n in FIELDS:
+        fa = a[n][..., j0 + js:j0 + je, i0 + is_:i0 + ie].astype(np.float64)
+        fb = b[n][..., js:je, is_:ie]
+        err = np.abs(fa - fb).max() / max(np.abs(b[n]).max(), 1e-300)
+        assert err <= TOL[32], (n, err)
+
+
+def test_config3_full_size_invariants():
+    """Properties that hold at any size, on the full 1440x600x50 fp32 grid: land stays exactly zero, the fields stay
+    finite, the tracer integrals are conserved to fp32 round-off, and the depth integral of u equals the filtered
+    barotropic transport after the correction step."""
+    wl = W.config3()
+    gpu = ocn.Model(wl)
+    m = gpu.grid.masks()
+    wet = m["wet"].astype(bool)
+    mu = m["order_zeta_u"] > 0
+    dz = np.diff(wl["z_faces"])
+    g = wl["grid"]
+    lat = np.deg2rad(g["y0"] + (np.arange(g["ny"]) + 0.5) * g["dy"])
+    vol = (dz[:, None, None] * np.cos(lat)[None, :, None]) * wet            # cell volume up to a constant factor
+    f0 = gpu.get_fields(names=("T", "S"))
+    I0 = {n: float((f0[n].astype(np.float64) * vol).sum()) for n in ("T", "S")}
+    gpu.time_step(5)
+    f = gpu.get_fields()
+    for n in FIELDS:
+        assert np.isfinite(f[n]).all(), n
+    assert np.all(f["T"][~wet] == 0) and np.all(f["S"][~wet] == 0) and np.all(f["u"][~mu] == 0)
+    for n in ("T", "S"):
+        I1 = float((f[n].astype(np.float64) * vol).sum())
+        assert abs(I1 - I0[n]) <= 2e-6 * abs(I0[n]), (n, I0[n], I1)
+    U = gpu.debug()["U"]
+    su = (f["u"].astype(np.float64) * dz[:, None, None]).sum(axis=0)
+    assert np.abs(su - U).max() <= 2e-4 * max(np.abs(U).max(), 1e-30)
+    gpu.close()
