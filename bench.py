@@ -233,10 +233,10 @@ def run_ours(args):
         return replicas.max_over_ranks(x, dist, device="cuda")
 
     # ---- device-resident timing: K steps of the production path (one CUDA graph launch per step) ----
+    clocks = ClockSampler(local)                 # samples from the warm-up on: nvidia-smi needs ~0.2 s to start
     model.time_step(Wm)
     barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    clocks = ClockSampler(local)
     barrier()
     e0.record(stream)
     model.time_step(K)
