@@ -48,7 +48,7 @@ __host__ __device__ constexpr int rup128(int b) { return (b + 127) / 128 * 128; 
 template <class T, int TX_, int TY_>
 struct Tile {
     typedef typename Pair<T>::type T2;
-    static constexpr int TX = TX_, TY = TY_, NT = TX * TY;
+    static constexpr int TX = TX_, TY = TY_, NC = TX * TY, NT = NC;   // cells = threads; a thread owns the tracers of one cell and the momentum of another
     static constexpr int BX = TX + 8, BY = TY + 6;       // TMA box: origin (i0 - 4, j0 - 3)
     static constexpr int OX = 4, OY = 3;                 // box coordinates of tile cell (0, 0)
     static constexpr int DP = 2;                         // prefetch distance in levels
@@ -70,7 +70,7 @@ struct Tile {
     static constexpr int O_M8 = O_FLUX + 2 * FLB;                               // uint2 on RX x RY (not zero-filled from here on)
     static constexpr int O_MET = O_M8 + rup128(RX * RY * 8);                    // 8 row-metric arrays of BY + 1
     static constexpr int O_CELL = O_MET + rup128(8 * (BY + 1) * (int)sizeof(T)); // uint16: cells sorted by first wet level
-    static constexpr int O_FS = O_CELL + rup128(NT * 2);                        // uint2: face descriptors sorted by first open level
+    static constexpr int O_FS = O_CELL + rup128(NC * 2);                        // uint2: face descriptors sorted by first open level
     static constexpr int O_NC = O_FS + rup128(NF * 8);                          // uint16[256]: active cells at level k
     static constexpr int O_NF = O_NC + 512;                                     // uint16[256]: active faces at level k
     static constexpr int O_BAR = O_NF + 512;
@@ -85,7 +85,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     typedef Tile<T, TX, TY> C;
     typedef typename C::T2 T2;
     typedef Ex<T> E;
-    constexpr int BX = C::BX, BY = C::BY, RX = C::RX, RY = C::RY, NT = C::NT, OX = C::OX, OY = C::OY;
+    constexpr int BX = C::BX, BY = C::BY, RX = C::RX, RY = C::RY, NT = C::NT, NC = C::NC, OX = C::OX, OY = C::OY;
     extern __shared__ __align__(1024) unsigned char sm[];     // dynamic only: starts the CTA's window, 1 KB aligned
     unsigned short* const s_cell = (unsigned short*)(sm + C::O_CELL);
     uint2* const s_fs = (uint2*)(sm + C::O_FS);
@@ -166,22 +166,26 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 }
             }
             __syncthreads();
-            {                                                             // thread t owns key t
+            {                                                             // thread t < 256 owns key t
+                const int kt = tid & 255;
                 int run = 0;
-                for (int vw = 0; vw < nr * (NT / 32); ++vw) {
-                    const int cc = cnt[vw * 256 + tid];
-                    cnt[vw * 256 + tid] = (unsigned short)run;
-                    run += cc;
-                }
+                if (tid < 256)
+                    for (int vw = 0; vw < nr * (NT / 32); ++vw) {
+                        const int cc = cnt[vw * 256 + kt];
+                        cnt[vw * 256 + kt] = (unsigned short)run;
+                        run += cc;
+                    }
                 int inc = run;                                            // block-wide inclusive scan of the key totals
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
-                if (lane == 31) base[256 + wrp] = inc;
+                if (lane == 31 && tid < 256) base[256 + wrp] = inc;
                 __syncthreads();
-                int off = 0;
-                for (int w = 0; w < wrp; ++w) off += base[256 + w];
-                base[tid] = off + inc - run;
-                nle[tid] = (unsigned short)(off + inc);
+                if (tid < 256) {
+                    int off = 0;
+                    for (int w = 0; w < wrp; ++w) off += base[256 + w];
+                    base[kt] = off + inc - run;
+                    nle[kt] = (unsigned short)(off + inc);
+                }
             }
             __syncthreads();
 #pragma unroll
@@ -191,8 +195,8 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             }
             __syncthreads();
         };
-        static_assert(NT == 256, "one thread per key");
-        csort(NT,
+        static_assert(NC == 256, "one thread per key");
+        csort(NC,
               [&](int q) { const int gx = q % TX, gy = q / TX;
                            return (i0 + gx < P.nx && j0 + gy < P.ny) ? (int)(s_m8[gy * RX + gx].x & 255u) : nz; },
               [&](int q, int rank) { s_cell[rank] = (unsigned short)q; }, s_nc);
@@ -254,38 +258,50 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     }
 
     // ---- per-thread column state ------------------------------------------------------------
-    const int g_own = s_cell[tid];                       // the cell this thread owns for the whole march
-    const int cx = g_own % TX, cy = g_own / TX;
-    const int i = i0 + cx, j = j0 + cy;
-    const bool incol = i < P.nx && j < P.ny;
-    const long long c = (long long)(j + OCN_HALO) * sx + i;
-    const uint2 m_own = s_m8[cy * RX + cx];
-    const int kb = incol ? (int)(m_own.x & 255u) : nz;
-    const int tx1 = incol ? (int)((m_own.x >> 8) & 255u) : nz, ty1 = incol ? (int)(m_own.y & 255u) : nz;
-    uchar4 mzt = make_uchar4(255, 255, 255, 255);
-    if (kb < nz) mzt = P.mz[c];
+    // A thread owns the TRACERS of the cell of rank tid and the MOMENTUM of the cell of rank NC-1-tid in the
+    // sorted list: early (deep) cells are paired with late (shallow) ones, so when only part of the tile is
+    // wet at a level the two halves of part B run on different warps instead of one after the other.
+    struct Cell { int cx, cy, kb, tx1, ty1, bo, by; long long c; bool incol; uchar4 mzt; };
+    auto make_cell = [&](int rank) {
+        Cell X;
+        const int g = s_cell[rank];
+        X.cx = g % TX; X.cy = g / TX;
+        const int i = i0 + X.cx, j = j0 + X.cy;
+        X.incol = i < P.nx && j < P.ny;
+        X.c = (long long)(j + OCN_HALO) * sx + i;
+        const uint2 mo = s_m8[X.cy * RX + X.cx];
+        X.kb = X.incol ? (int)(mo.x & 255u) : nz;
+        X.tx1 = X.incol ? (int)((mo.x >> 8) & 255u) : nz; X.ty1 = X.incol ? (int)(mo.y & 255u) : nz;
+        X.mzt = make_uchar4(255, 255, 255, 255);
+        if (X.kb < nz) X.mzt = P.mz[X.c];
+        X.by = X.cy + OY; X.bo = X.by * BX + X.cx + OX;
+        return X;
+    };
+    const Cell cT = make_cell(tid), cM = make_cell(NC - 1 - tid);
     const T dy = P.dy, rdy = P.rdy;
-    const int bx = cx + OX, by = cy + OY;                // this cell in box coordinates
-    const int bo = by * BX + bx;
 
     double wacc0 = 0.0, wacc1 = 0.0;                     // w accumulators of this thread's ring points
     T2 fz_bot = mk2(T(0), T(0));                         // vertical tracer flux through the face below
     T u_dn = 0, v_dn = 0;
     T2 dduv = mk2(T(0), T(0)), ddts = mk2(T(0), T(0));   // eliminated right-hand sides of the level below
     double aGU = 0, aGV = 0, aSU = 0, aSV = 0;
-    const int kbc = min(kb, nz - 1), txc = min(tx1, nz - 1), tyc = min(ty1, nz - 1);   // pivot-table columns
 
     for (int m = kmin; m <= nz; ++m) {
         const int kB = m - 1;                                 // level of part B (phase 3) in this iteration
-        const bool doB = kB >= kmin, wetc = doB && kB >= kb;
-        const long long o = (long long)kB * sz + c;
+        const bool doB = kB >= kmin, wetT = doB && kB >= cT.kb, wetM = doB && kB >= cM.kb;
+        const long long oT = (long long)kB * sz + cT.c, oM = (long long)kB * sz + cM.c;
         // AB2 history and pivots of level kB: issued now, consumed after part A
         T2 gm_uv = mk2(T(0), T(0)), gm_ts = mk2(T(0), T(0));
         T piv_t = 1, piv_u = 1, piv_v = 1;
-        if (wetc) {
-            gm_uv = P.Guv[o]; gm_ts = P.Gts[o];
-            if (sizeof(T) == 8) { piv_t = P.m_t[kB * nz + kbc]; piv_u = P.m_m[kB * nz + txc]; piv_v = P.m_m[kB * nz + tyc]; }
-            else                { piv_t = P.rm_t[kB * nz + kbc]; piv_u = P.rm_m[kB * nz + txc]; piv_v = P.rm_m[kB * nz + tyc]; }
+        if (wetT) {
+            gm_ts = P.Gts[oT];
+            piv_t = sizeof(T) == 8 ? P.m_t[kB * nz + min(cT.kb, nz - 1)] : P.rm_t[kB * nz + min(cT.kb, nz - 1)];
+        }
+        if (wetM) {
+            gm_uv = P.Guv[oM];
+            const int txc = min(cM.tx1, nz - 1), tyc = min(cM.ty1, nz - 1);
+            if (sizeof(T) == 8) { piv_u = P.m_m[kB * nz + txc]; piv_v = P.m_m[kB * nz + tyc]; }
+            else                { piv_u = P.rm_m[kB * nz + txc]; piv_v = P.rm_m[kB * nz + tyc]; }
         }
         mbar_wait(&bars[(m - kmin) % C::NB], (uint32_t)(((m - kmin) / C::NB) & 1));
 
@@ -351,19 +367,20 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             const T2* __restrict__ s_uv = (const T2*)(sm + C::O_UV + (k % C::R_UV) * C::PL2);
             const T2* __restrict__ s_uv1 = (const T2*)(sm + C::O_UV + ((k + 1) % C::R_UV) * C::PL2);
             const T* __restrict__ s_p = (const T*)(sm + C::O_P + (k % C::R_P) * C::PL1);
-            const T dxFj = s_dxF[by], dxFn = s_dxF[by + 1], rdxCj = s_rdxC[by], rdxFj = s_rdxF[by];
-            const T AzCj = s_AzC[by], AzCs = s_AzC[by - 1], rAzCj = s_rAzC[by], rAzFj = s_rAzF[by];
-            const T fFj = s_fF[by], fFn = s_fF[by + 1];
             const T* __restrict__ s_w0 = (const T*)(sm + C::O_W + (k % 3) * C::WB);
             const T* __restrict__ s_w1 = (const T*)(sm + C::O_W + ((k + 1) % 3) * C::WB);
             const T* __restrict__ s_zeta = (const T*)(sm + C::O_ZETA + (k & 1) * C::PL1);
             const T2* __restrict__ s_kd = (const T2*)(sm + C::O_KD + (k & 1) * C::KDB);
             const T2* __restrict__ s_flux = (const T2*)(sm + C::O_FLUX + (k & 1) * C::FLB);
-            // vertical face above cell k (own column)
-            const int qo = (cy + 1) * RX + cx + 1;                           // this column in the ring arrays
-            const T w_c1 = s_w1[qo], w_c0 = s_w0[qo];
+            // ---------- tracer half: the cell of rank tid ----------
             T2 fz_top = mk2(T(0), T(0));
-            if (wetc) {
+            if (wetT) {
+                const int cx = cT.cx, cy = cT.cy, kb = cT.kb, bo = cT.bo, by = cT.by;
+                const long long o = oT;
+                const T AzCj = s_AzC[by], rAzCj = s_rAzC[by];
+                const T w_c1 = s_w1[(cy + 1) * RX + cx + 1];
+                // vertical face above cell k (own column)
+                {
                 const int ozt = (k + 1 < nz) ? min(3, min(k + 1 - kb, nz - k - 1)) : 0;
                 if (ozt > 0) {
                     auto tsz = [&](int kk) -> T2 { return ((const T2*)(sm + C::O_TS + ((kk + C::R_TS) % C::R_TS) * C::PL2))[bo]; };
@@ -372,9 +389,6 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                     fz_top.y = w_c1 * AzCj * fv.y;
                 }
             }
-            // ================= phase 3: tendencies of this cell, AB2, elimination =================
-            if (wetc) {
-                const bool mu = k >= tx1, mv = k >= ty1;
                 // ---- tracers ----
                 const T2 fw = s_flux[cy * RX + cx], fe = s_flux[cy * RX + cx + 1];
                 const T2 fs = s_flux[C::NFX + cy * TX + cx], fn = s_flux[C::NFX + (cy + 1) * TX + cx];
@@ -385,6 +399,25 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                     const T src = w_c1 * rdzk;     // of the constant under the zero-top-flux linear free surface
                     GT += P.Toff * src; GS += P.Soff * src;
                 }
+                // ---- quasi-AB2, predictor, elimination sweep (S3, S4) ----
+                const T Ght = c0 * GT - c1 * gm_ts.x, Ghs = c0 * GS - c1 * gm_ts.y;
+                P.Gts[o] = mk2(GT, GS);
+                const T smk = k > kb ? P.sm_t[k] : T(0);
+                ddts.x = E::div(E::add(E::add(tsc.x, E::mul(P.dt, Ght)), E::mul(smk, ddts.x)), piv_t, piv_t);
+                ddts.y = E::div(E::add(E::add(tsc.y, E::mul(P.dt, Ghs)), E::mul(smk, ddts.y)), piv_t, piv_t);
+                P.dts[o] = ddts;
+            }
+            // ---------- momentum half: the cell of rank NC - 1 - tid ----------
+            if (wetM) {
+                const int cx = cM.cx, cy = cM.cy, tx1 = cM.tx1, ty1 = cM.ty1, bo = cM.bo, by = cM.by;
+                const long long o = oM, c = cM.c;
+                const uchar4 mzt = cM.mzt;
+                const int qo = (cy + 1) * RX + cx + 1;                       // this column in the ring arrays
+                const T w_c1 = s_w1[qo], w_c0 = s_w0[qo];
+                const T dxFj = s_dxF[by], dxFn = s_dxF[by + 1], rdxCj = s_rdxC[by], rdxFj = s_rdxF[by];
+                const T AzCj = s_AzC[by], AzCs = s_AzC[by - 1], rAzFj = s_rAzF[by];
+                const T fFj = s_fF[by], fFn = s_fF[by + 1];
+                const bool mu = k >= tx1, mv = k >= ty1;
                 // ---- momentum ----
                 const T2 uvc = s_uv[bo];
                 const T u_c = uvc.x, v_c = uvc.y;
@@ -436,9 +469,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 }
                 // ---- quasi-AB2, predictor, elimination sweep (S3, S4, S5) ----
                 const T Ghu = c0 * Gu - c1 * gm_uv.x, Ghv = c0 * Gv - c1 * gm_uv.y;
-                const T Ght = c0 * GT - c1 * gm_ts.x, Ghs = c0 * GS - c1 * gm_ts.y;
                 P.Guv[o] = mk2(Gu, Gv);
-                P.Gts[o] = mk2(GT, GS);
                 if (mu) {
                     const T us = E::add(u_c, E::mul(P.dt, Ghu));
                     aGU += (double)dzk * (double)Ghu; aSU += (double)dzk * (double)us;
@@ -451,13 +482,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                     const T smk = k > ty1 ? P.sm_m[k] : T(0);
                     dduv.y = E::div(E::add(vs2, E::mul(smk, dduv.y)), piv_v, piv_v);
                 }
-                {
-                    const T smk = k > kb ? P.sm_t[k] : T(0);
-                    ddts.x = E::div(E::add(E::add(tsc.x, E::mul(P.dt, Ght)), E::mul(smk, ddts.x)), piv_t, piv_t);
-                    ddts.y = E::div(E::add(E::add(tsc.y, E::mul(P.dt, Ghs)), E::mul(smk, ddts.y)), piv_t, piv_t);
-                }
                 P.duv[o] = dduv;
-                P.dts[o] = ddts;
                 u_dn = u_c; v_dn = v_c;
             }
             fz_bot = fz_top;
@@ -465,6 +490,6 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
         __syncthreads();                       // planes of level m - 1 are dead: refill the ring
         if (tid == 0 && m + C::DP <= nz) issue_group(m + C::DP, false);
     }
-    if (incol && kb < nz) { P.GU[c] = (T)aGU; P.GV[c] = (T)aGV; P.SU[c] = (T)aSU; P.SV[c] = (T)aSV; }
+    if (cM.incol && cM.kb < nz) { P.GU[cM.c] = (T)aGU; P.GV[cM.c] = (T)aGV; P.SU[cM.c] = (T)aSU; P.SV[cM.c] = (T)aSV; }
 }
 }  // namespace ocn

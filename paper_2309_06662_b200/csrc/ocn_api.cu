@@ -277,7 +277,7 @@ ocn_status launch_step(ocn_model* M, bool euler) {
     {
         typedef ocn::Tile<T, TILE_X, TILE_Y> C;
         const dim3 bt(TILE_X, TILE_Y);
-        ocn::k_tendency_tile<T, TILE_X, TILE_Y><<<grid2(g, bt), bt, C::SMEM, M->stream>>>(P, c0, c1, M->tm_ts, M->tm_uv, M->tm_p);
+        ocn::k_tendency_tile<T, TILE_X, TILE_Y><<<grid2(g, dim3(TILE_X, TILE_Y)), bt, C::SMEM, M->stream>>>(P, c0, c1, M->tm_ts, M->tm_uv, M->tm_p);
     }
     MARK(0, 1);
     {
