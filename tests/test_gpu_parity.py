@@ -182,3 +182,59 @@ def test_config3_full_size_invariants():
     su = (f["u"].astype(np.float64) * dz[:, None, None]).sum(axis=0)
     assert np.abs(su - U).max() <= 2e-4 * max(np.abs(U).max(), 1e-30)
     gpu.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# degenerate and extreme shapes
+# ---------------------------------------------------------------------------------------------
+def test_all_land_domain_is_a_no_op():
+    wl = box(nx=40, ny=20, nz=6, depth=600.0, periodic=(1, 0))
+    wl["depth"][:] = 0.0
+    gpu = ocn.Model(wl)
+    gpu.time_step(3)
+    f = gpu.get_fields()
+    for n in FIELDS:
+        assert np.all(f[n] == 0.0), n
+    gpu.close()
+
+
+def test_smallest_grids_and_two_levels():
+    for nx, ny, nz, per in ((3, 3, 2, (1, 1)), (5, 4, 3, (0, 0)), (33, 9, 2, (1, 0))):
+        wl = W.config0(nx=max(nx, 3), ny=max(ny, 3), nz=nz)
+        wl["grid"]["periodic_x"], wl["grid"]["periodic_y"] = per
+        run_both(wl, 4, check_every=[1, 4])
+
+
+def test_isolated_columns_and_one_cell_channels():
+    # a checkerboard-ish bathymetry: isolated wet columns (no open faces) and one-cell-wide channels, ragged depths
+    rng = np.random.default_rng(11)
+    wl = W.config1(nx=70, ny=21, nz=9, steps=6)
+    d = wl["depth"]
+    d[::2, ::2] = 0.0                                   # isolated columns on odd rows / columns
+    d[10, :] = 3500.0                                   # one zonal channel
+    d[:, 35] = rng.uniform(200.0, 4000.0, size=d.shape[0])
+    d[0, :] = d[-1, :] = 0.0; d[:, 0] = d[:, -1] = 0.0
+    wl["fields"]["u"] = 0.05 * rng.standard_normal(wl["fields"]["u"].shape)
+    wl["fields"]["v"] = 0.05 * rng.standard_normal(wl["fields"]["v"].shape)
+    run_both(wl, 6, check_every=[1, 6])
+
+
+def test_deep_column_count_nz_200_fp64():
+    # many levels (the plane rings wrap many times), closed box with bathymetry; fp64 so that the tolerance tests
+    # the logic and not the conditioning of a tiny box
+    wl = W.config4(nx=2880, ny=1200, nz=100, window=(600, 640, 2000, 2070), steps=3, precision=64)
+    zf = W.geometric_z_faces(200, 5.0, 6000.0)
+    nz = 200
+    f = wl["fields"]
+    zc_old = 0.5 * (wl["z_faces"][:-1] + wl["z_faces"][1:]); zc = 0.5 * (zf[:-1] + zf[1:])
+    def regrid(a):
+        out = np.empty((nz,) + a.shape[1:])
+        for j in range(a.shape[1]):
+            for i in range(a.shape[2]):
+                out[:, j, i] = np.interp(zc, zc_old, a[:, j, i])
+        return out
+    for n in ("u", "v", "T", "S"):
+        f[n] = regrid(f[n])
+    wl["z_faces"] = zf
+    wl["grid"]["nz"] = nz
+    run_both(wl, 3, check_every=[1, 3])
