@@ -193,17 +193,20 @@ def latlon(nx, ny, nz, *, dt, substeps, steps, nu_h, kappa_h, precision, seed, n
         j0, j1, i0, i1 = window
     wny, wnx = j1 - j0, i1 - i0
     cos2 = (np.cos(latc[j0:j1]) ** 2)[:, None]
-    cos2lat = np.cos(2.0 * latc[j0:j1])[:, None]
     T = np.empty((nz, wny, wnx))
     S = np.empty((nz, wny, wnx))
     for k in range(nz):                       # level by level: full-size noise, keep the window
-        Tk = 2.0 + 25.0 * cos2 * np.exp(zc[k] / 800.0)
-        Sk = 35.0 - cos2lat * np.exp(zc[k] / 500.0)
+        # statically stable everywhere: warm and fresh at the surface (dT/dz > 0, dS/dz < 0 at every
+        # latitude), 5 K of stratification left at the poleward walls; the noise decays with depth so
+        # that it never overturns the weak abyssal stratification
+        Tk = 2.0 + (5.0 + 20.0 * cos2) * np.exp(zc[k] / 800.0)
+        Sk = 35.0 - cos2 * np.exp(zc[k] / 500.0)
+        damp = np.exp(zc[k] / 2000.0)
         if noise:
             nT = rng.standard_normal((ny, nx), dtype=np.float32)[j0:j1, i0:i1]
             nS = rng.standard_normal((ny, nx), dtype=np.float32)[j0:j1, i0:i1]
-            T[k] = Tk + 0.01 * nT
-            S[k] = Sk + 0.001 * nS
+            T[k] = Tk + 0.01 * damp * nT
+            S[k] = Sk + 0.001 * damp * nS
         else:
             T[k] = Tk
             S[k] = Sk
