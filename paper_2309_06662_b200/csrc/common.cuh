@@ -31,7 +31,8 @@ struct DevP {
     // prognostic state (time level n) as pairs, stored pressure, w (filled on demand for
     // ocn_get_fields), eliminated right-hand sides, AB2 history
     T2 *uv, *ts;
-    T *p, *w;
+    double* p;             // hydrostatic pressure, fp64 in both precisions
+    T* w;
     T2 *duv, *dts;
     T2 *Guv, *Gts;
     // 2-D (plane layout with halo)
@@ -62,6 +63,8 @@ struct DevP {
     T dt, g, alpha, beta_s, rrho0, nu_h, kappa_h;
     T Toff, Soff;          // storage offsets of the tracers: (T0, S0) in fp32, 0 in fp64
     T dT0, dS0;            // T0 - Toff, S0 - Soff: what is left to subtract in the buoyancy
+    double g_d, alpha_d, beta_d, dT0_d, dS0_d, hz_top_d;   // fp64 copies for the pressure integral
+    const double* dzc_d;
     T dtau;
 };
 

@@ -6,11 +6,19 @@
 
 namespace ocn {
 
-// linear equation of state; t, s are the stored (offset) tracers
+// linear equation of state and one level of the downward pressure integral, in fp64 with the
+// rounding order of the equations as written; t, s are the stored (offset) tracers.  In fp32 runs this keeps
+// the rounding of p ~ 1e2 m^2/s^2 (whose horizontal differences drive the flow) out of the momentum equation.
 template <class T>
-__device__ __forceinline__ T buoyancy(const DevP<T>& P, T t, T s) {
-    typedef Ex<T> E;
-    return E::mul(P.g, E::sub(E::mul(P.alpha, E::sub(t, P.dT0)), E::mul(P.beta_s, E::sub(s, P.dS0))));
+__device__ __forceinline__ double buoyancy(const DevP<T>& P, T t, T s) {
+    typedef Ex<double> E;
+    return E::mul(P.g_d, E::sub(E::mul(P.alpha_d, E::sub((double)t, P.dT0_d)), E::mul(P.beta_d, E::sub((double)s, P.dS0_d))));
+}
+template <class T>
+__device__ __forceinline__ double pressure_level(const DevP<T>& P, int k, double b0, double b1, double p_above) {
+    typedef Ex<double> E;
+    return k == P.nz - 1 ? -E::mul(b0, P.hz_top_d)
+                         : E::sub(p_above, E::mul(E::mul(0.5, E::add(b1, b0)), P.dzc_d[k + 1]));
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -173,7 +181,8 @@ __global__ void __launch_bounds__(128) k_backsub_correct(const DevP<T> P) {
     const T* __restrict__ cpu = P.cp_m + min(tx1, nz - 1);
     const T* __restrict__ cpv = P.cp_m + min(ty1, nz - 1);
     const T* __restrict__ cpt = P.cp_t + kb;
-    T xu = 0, xv = 0, xt = 0, xs = 0, b1 = 0, pk = 0;
+    T xu = 0, xv = 0, xt = 0, xs = 0;
+    double b1 = 0, pk = 0;
     const int kuv = min(tx1, ty1);
     constexpr int NB = 4;                                  // levels whose loads are in flight together
     for (int k0 = nz - 1; k0 >= kb; k0 -= NB) {
@@ -195,9 +204,8 @@ __global__ void __launch_bounds__(128) k_backsub_correct(const DevP<T> P) {
             xt = E::sub(d_ts[q].x, E::mul(ck, xt));                      // cp[nz-1] = 0
             xs = E::sub(d_ts[q].y, E::mul(ck, xs));
             store_halo(P.ts + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, mk2(xt, xs));
-            const T b0 = buoyancy(P, xt, xs);
-            pk = k == nz - 1 ? -E::mul(b0, P.hz_top)
-                             : E::sub(pk, E::mul(E::mul(T(0.5), E::add(b1, b0)), P.dzc[k + 1]));
+            const double b0 = buoyancy(P, xt, xs);
+            pk = pressure_level(P, k, b0, b1, pk);
             b1 = b0;
             store_halo(P.p + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, pk);
             const bool mu = k >= tx1, mv = k >= ty1;
@@ -221,12 +229,11 @@ __global__ void __launch_bounds__(128) k_pressure(const DevP<T> P) {
     const int sx = P.sx, nz = P.nz;
     const long long sz = P.sz, c = (long long)(j + OCN_HALO) * sx + i;
     const int kb = P.m8[c].x & 255;
-    T b1 = 0, pk = 0;
+    double b1 = 0, pk = 0;
     for (int k = nz - 1; k >= kb; --k) {
         const typename Pair<T>::type q = P.ts[k * sz + c];
-        const T b0 = buoyancy(P, q.x, q.y);
-        pk = k == nz - 1 ? -E::mul(b0, P.hz_top)
-                         : E::sub(pk, E::mul(E::mul(T(0.5), E::add(b1, b0)), P.dzc[k + 1]));
+        const double b0 = buoyancy(P, q.x, q.y);
+        pk = pressure_level(P, k, b0, b1, pk);
         b1 = b0;
         store_halo(P.p + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, pk);
     }

@@ -54,13 +54,14 @@ struct Tile {
     static constexpr int DP = 2;                         // prefetch distance in levels
     static constexpr int R_TS = DP + 5, R_UV = DP + 1, R_P = DP, NB = DP;
     static constexpr int RX = TX + 1, RY = TY + 1;       // tile + west/south ring (K, D, w) or + east/north edge (faces, masks)
-    static constexpr int PL2 = rup128(BX * BY * (int)sizeof(T2)), PL1 = rup128(BX * BY * (int)sizeof(T));
-    static constexpr int BYTES2 = BX * BY * (int)sizeof(T2), BYTES1 = BX * BY * (int)sizeof(T);
+    static constexpr int PL2 = rup128(BX * BY * (int)sizeof(T2)), PL1 = rup128(BX * BY * (int)sizeof(T)),
+                         PLP = rup128(BX * BY * 8);          // pressure planes are fp64
+    static constexpr int BYTES2 = BX * BY * (int)sizeof(T2), BYTESP = BX * BY * 8;
     // shared-memory map (byte offsets from a 128-byte aligned base)
     static constexpr int O_TS = 0;
     static constexpr int O_UV = O_TS + R_TS * PL2;
     static constexpr int O_P = O_UV + R_UV * PL2;
-    static constexpr int O_ZETA = O_P + R_P * PL1;
+    static constexpr int O_ZETA = O_P + R_P * PLP;
     static constexpr int O_KD = O_ZETA + 2 * PL1;                               // 2 x T2 (K, D) on RX x RY
     static constexpr int KDB = rup128(RX * RY * (int)sizeof(T2)), WB = rup128(RX * RY * (int)sizeof(T));
     static constexpr int O_W = O_KD + 2 * KDB;                                  // 3 buffers of T on RX x RY
@@ -245,11 +246,11 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
         const int tlo = first ? max(m - 3, 0) : m + 2, thi = min(m + 2, nz - 1);
         if (thi >= tlo) bytes += (uint32_t)(thi - tlo + 1) * C::BYTES2;
         if (m < nz) bytes += C::BYTES2;
-        if (m - 1 >= kmin) bytes += C::BYTES1;
+        if (m - 1 >= kmin) bytes += C::BYTESP;
         mbar_expect_tx(bar, bytes);
         for (int q = tlo; q <= thi; ++q) tma_load_plane(sm + C::O_TS + (q % C::R_TS) * C::PL2, &m_ts, bar, 2 * i0, j0, q);
         if (m < nz) tma_load_plane(sm + C::O_UV + (m % C::R_UV) * C::PL2, &m_uv, bar, 2 * i0, j0, m);
-        if (m - 1 >= kmin) tma_load_plane(sm + C::O_P + ((m - 1) % C::R_P) * C::PL1, &m_p, bar, i0, j0, m - 1);
+        if (m - 1 >= kmin) tma_load_plane(sm + C::O_P + ((m - 1) % C::R_P) * C::PLP, &m_p, bar, i0, j0, m - 1);
     };
     if (tid == 0) {
         issue_group(kmin, true);
@@ -366,7 +367,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             const T dzk = P.dz[k], rdzk = P.rdz[k];
             const T2* __restrict__ s_uv = (const T2*)(sm + C::O_UV + (k % C::R_UV) * C::PL2);
             const T2* __restrict__ s_uv1 = (const T2*)(sm + C::O_UV + ((k + 1) % C::R_UV) * C::PL2);
-            const T* __restrict__ s_p = (const T*)(sm + C::O_P + (k % C::R_P) * C::PL1);
+            const double* __restrict__ s_p = (const double*)(sm + C::O_P + (k % C::R_P) * C::PLP);
             const T* __restrict__ s_w0 = (const T*)(sm + C::O_W + (k % 3) * C::WB);
             const T* __restrict__ s_w1 = (const T*)(sm + C::O_W + ((k + 1) % 3) * C::WB);
             const T* __restrict__ s_zeta = (const T*)(sm + C::O_ZETA + (k & 1) * C::PL1);
@@ -428,7 +429,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                     const T2 uv_up = (k + 1 < nz) ? s_uv1[bo] : mk2(T(0), T(0));
                     const T z00 = s_zeta[bo];
                     const T2 kdc = s_kd[qo];
-                    const T pc = s_p[bo];
+                    const double pc = s_p[bo];
                     if (mu) {
                         const T vsum_s = uv_w.y + v_c, vsum_n = uv_nw.y + uv_n.y;
                         const T vhat = T(0.25) * (dxFj * vsum_s + dxFn * vsum_n) * rdxCj;
@@ -440,7 +441,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                         const T Cu = T(0.5) * (fFj * T(0.5) * dxFj * vsum_s + fFn * T(0.5) * dxFn * vsum_n) * rdxCj;
                         const T2 kdw = s_kd[qo - 1];
                         const T dK = (kdc.x - kdw.x) * rdxCj;
-                        const T dP = (pc - s_p[bo - 1]) * rdxCj;
+                        const T dP = (T)(pc - s_p[bo - 1]) * rdxCj;
                         const T dlo = (k >= 1 && k - 1 >= tx1) ? u_c - u_dn : T(0);
                         const T dhi = (k + 1 <= nz - 1) ? uv_up.x - u_c : T(0);
                         const T Au = T(0.5) * (T(0.5) * (s_w1[qo - 1] + w_c1) * dhi + T(0.5) * (s_w0[qo - 1] + w_c0) * dlo) * rdzk;
@@ -457,7 +458,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                         const T Cv = fFj * uhat;
                         const T2 kds = s_kd[qo - RX];
                         const T dK = (kdc.x - kds.x) * rdy;
-                        const T dP = (pc - s_p[bo - BX]) * rdy;
+                        const T dP = (T)(pc - s_p[bo - BX]) * rdy;
                         const T dlo = (k >= 1 && k - 1 >= ty1) ? v_c - v_dn : T(0);
                         const T dhi = (k + 1 <= nz - 1) ? uv_up.y - v_c : T(0);
                         const T Av = T(0.5) * (T(0.5) * (AzCs * s_w1[qo - RX] + AzCj * w_c1) * dhi

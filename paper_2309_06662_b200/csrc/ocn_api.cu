@@ -134,7 +134,7 @@ ocn_status build_model(ocn_model* M) {
     typedef typename ocn::Pair<T>::type T2;
     T2** f3[] = {&P.uv, &P.ts, &P.duv, &P.dts, &P.Guv, &P.Gts};
     for (T2** f : f3) if ((s = dev_alloc(M, n3, f, true)) != OCN_OK) return s;
-    if ((s = plane(n3, &P.p)) != OCN_OK) return s;
+    if ((s = dev_alloc(M, n3, &P.p, true)) != OCN_OK) return s;
     if ((s = plane(n3 + n2, &P.w)) != OCN_OK) return s;
     double** fb[] = {&P.eta[0], &P.eta[1], &P.U[0], &P.U[1], &P.V[0], &P.V[1], &P.etab, &P.Ub, &P.Vb, &P.GU, &P.GV, &P.SU, &P.SV};
     for (double** f : fb) if ((s = dev_alloc(M, n2, f, true)) != OCN_OK) return s;
@@ -158,6 +158,11 @@ ocn_status build_model(ocn_model* M) {
         (s = upload(M, recip(g->AzF), &P.rAzF)) != OCN_OK || (s = upload(M, g->dz, &P.dz)) != OCN_OK ||
         (s = upload(M, recip(g->dz), &P.rdz)) != OCN_OK || (s = upload(M, g->dzc, &P.dzc)) != OCN_OK)
         return s;
+    {
+        const double* dzc_d = nullptr;
+        if ((s = upload<double>(M, g->dzc, &dzc_d)) != OCN_OK) return s;
+        P.dzc_d = dzc_d;
+    }
     P.dy = (T)g->dy; P.rdy = (T)(1.0 / g->dy);
     P.hz_top = (T)(g->zf[nz] - g->zc[nz - 1]);
     // Thomas tables: bottom-up elimination started at the column's first open
@@ -191,6 +196,8 @@ ocn_status build_model(ocn_model* M) {
     P.Toff = sizeof(T) == 4 ? (T)M->d.T0 : T(0); P.Soff = sizeof(T) == 4 ? (T)M->d.S0 : T(0);
     P.dT0 = (T)(M->d.T0 - (double)P.Toff); P.dS0 = (T)(M->d.S0 - (double)P.Soff);
     P.rrho0 = (T)(1.0 / M->d.rho0);
+    P.g_d = M->d.g; P.alpha_d = M->d.alpha; P.beta_d = M->d.beta_s; P.hz_top_d = g->zf[nz] - g->zc[nz - 1];
+    P.dT0_d = M->d.T0 - (double)P.Toff; P.dS0_d = M->d.S0 - (double)P.Soff;
     P.nu_h = (T)M->d.nu_h; P.kappa_h = (T)M->d.kappa_h; P.dtau = (T)M->dtau;
     // Hu, Hv = sum_k dz over open faces, and reciprocals
     {
@@ -221,7 +228,7 @@ ocn_status build_model(ocn_model* M) {
         const unsigned long long sxu = (unsigned long long)g->sx, syu = (unsigned long long)g->sy;
         if ((s = make_tmap(&M->tm_ts, f64, (T*)P.ts - 2 * C::OX, 2 * sxu, syu, nz, 2 * C::BX, C::BY)) != OCN_OK ||
             (s = make_tmap(&M->tm_uv, f64, (T*)P.uv - 2 * C::OX, 2 * sxu, syu, nz, 2 * C::BX, C::BY)) != OCN_OK ||
-            (s = make_tmap(&M->tm_p, f64, P.p - C::OX, sxu, syu, nz, C::BX, C::BY)) != OCN_OK)
+            (s = make_tmap(&M->tm_p, true, P.p - C::OX, sxu, syu, nz, C::BX, C::BY)) != OCN_OK)
             return s;
         CK(cudaFuncSetAttribute(ocn::k_tendency_tile<T, TILE_X, TILE_Y>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
         CK(cudaFuncSetAttribute(ocn::k_barotropic_tile<T, BT_X, BT_Y>, cudaFuncAttributeMaxDynamicSharedMemorySize,
