@@ -36,12 +36,10 @@ struct DevP {
     T2 *duv, *dts;
     T2 *Guv, *Gts;
     // 2-D (plane layout with halo)
-    // The barotropic mode is carried in fp64 in both precisions: U = u H ~ 1e3 m^2/s makes
-    // fp32 rounding of the sub-cycled transports the dominant error of w otherwise; these are 2-D arrays.
-    double *eta[2], *U[2], *V[2];  // barotropic state, double buffered inside the sub-cycle
-    double *etab, *Ub, *Vb;        // weighted running averages
-    double *GU, *GV;               // barotropic forcing
-    double *SU, *SV;               // sum_k dz u*, sum_k dz v*
+    T *eta[2], *U[2], *V[2];       // barotropic state, double buffered inside the sub-cycle
+    T *etab, *Ub, *Vb;             // weighted running averages
+    T *GU, *GV;                    // barotropic forcing
+    T *SU, *SV;                    // sum_k dz u*, sum_k dz v*
     T *Hu, *Hv, *rHu, *rHv;        // depth at u / v points and reciprocals (0 on closed columns)
     T *taux, *tauy;
     // compact masks (plane layout with halo): thresholds in level index

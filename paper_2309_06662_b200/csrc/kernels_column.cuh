@@ -36,29 +36,27 @@ template <class T, int BTX, int BTY>
 struct BtTile {
     static constexpr int EX = BTX + 2 * BT_HALO, EY = BTY + 2 * BT_HALO, NE = EX * EY;
     static constexpr int NT = 1024, PER = (BTX * BTY + NT - 1) / NT;
-    static constexpr int SMEM = NE * (5 * 8 + 2 * (int)sizeof(T) + 1) + 4 * (EY + 1) * 8 + 64 + BT_HALO * 8;
+    static constexpr int SMEM = NE * (7 * (int)sizeof(T) + 1) + 4 * (EY + 1) * (int)sizeof(T) + 64 + BT_HALO * (int)sizeof(T);
 };
 
 template <class T, int BTX, int BTY>
 __global__ void __launch_bounds__(1024) k_barotropic_tile(const DevP<T> P, const int cur, const int ns, const int first,
-                                                         const double a0, const double a1, const double a2, const double a3, const double a4,
-                                                         const double a5) {
+                                                         const T a0, const T a1, const T a2, const T a3, const T a4, const T a5) {
     typedef BtTile<T, BTX, BTY> C;
     constexpr int EX = C::EX, EY = C::EY, NE = C::NE, NT = C::NT, H = BT_HALO;
     extern __shared__ __align__(16) unsigned char smb[];
-    typedef double B;                       // the barotropic state and its arithmetic are fp64 in both precisions
-    B* const se = (B*)smb;                  // eta
-    B* const sU = se + NE;
-    B* const sV = sU + NE;
-    B* const sGU = sV + NE;
-    B* const sGV = sGU + NE;
-    B* const rAz = sGV + NE;                // per extended row: 1 / AzC, 1 / dxC, dxF (row), dxF (row + 1)
-    B* const rdx = rAz + (EY + 1);
-    B* const dF = rdx + (EY + 1);           // EY + 1 entries
-    B* const saw = dF + (EY + 1);           // filter weights of this launch
-    T* const sHu = (T*)(saw + BT_HALO);
+    T* const se = (T*)smb;                 // eta
+    T* const sU = se + NE;
+    T* const sV = sU + NE;
+    T* const sGU = sV + NE;
+    T* const sGV = sGU + NE;
+    T* const sHu = sGV + NE;
     T* const sHv = sHu + NE;
-    unsigned char* const smk = (unsigned char*)(sHv + NE);   // bit 0 wet, bit 1 open u face, bit 2 open v face
+    T* const rAz = sHv + NE;               // per extended row: 1 / AzC, 1 / dxC, dxF (row), dxF (row + 1)
+    T* const rdx = rAz + (EY + 1);
+    T* const dF = rdx + (EY + 1);          // EY + 1 entries
+    T* const saw = dF + (EY + 1);          // filter weights of this launch
+    unsigned char* const smk = (unsigned char*)(saw + BT_HALO);   // bit 0 wet, bit 1 open u face, bit 2 open v face
     const int tid = threadIdx.x;
     const int i0 = blockIdx.x * BTX, j0 = blockIdx.y * BTY;
     const int nx = P.nx, ny = P.ny, nz = P.nz, sx = P.sx;
@@ -72,17 +70,16 @@ __global__ void __launch_bounds__(1024) k_barotropic_tile(const DevP<T> P, const
         if (q < EY) { rAz[q] = P.rAzC[r]; rdx[q] = P.rdxC[r]; }
         dF[q] = P.dxF[r];
     }
-    const double* __restrict__ e0 = P.eta[cur];
-    const double* __restrict__ U0 = P.U[cur];
-    const double* __restrict__ V0 = P.V[cur];
+    const T* __restrict__ e0 = P.eta[cur];
+    const T* __restrict__ U0 = P.U[cur];
+    const T* __restrict__ V0 = P.V[cur];
     for (int q = tid; q < NE; q += NT) {
         const int x = q % EX, y = q / EX;
         int ii = i0 - H + x, jj = j0 - H + y;
         bool in = true;
         if (P.px) ii = ((ii % nx) + nx) % nx; else in = in && ii >= 0 && ii < nx;
         if (P.py) jj = ((jj % ny) + ny) % ny; else in = in && jj >= 0 && jj < ny;
-        B e = 0, u = 0, v = 0, gu = 0, gv = 0;
-        T hu = 0, hv = 0;
+        T e = 0, u = 0, v = 0, gu = 0, gv = 0, hu = 0, hv = 0;
         unsigned char mk = 0;
         if (in) {
             const long long c = (long long)(jj + OCN_HALO) * sx + ii;
@@ -97,10 +94,10 @@ __global__ void __launch_bounds__(1024) k_barotropic_tile(const DevP<T> P, const
     __syncthreads();
 
     // ---- the interior points this thread owns, and their filter sums ----
-    B be[C::PER], bU[C::PER], bV[C::PER];
+    T be[C::PER], bU[C::PER], bV[C::PER];
 #pragma unroll
     for (int n = 0; n < C::PER; ++n) { be[n] = 0; bU[n] = 0; bV[n] = 0; }
-    const B dy = P.dy, dtau = P.dtau, g = P.g, rdy = P.rdy;
+    const T dy = P.dy, dtau = P.dtau, g = P.g, rdy = P.rdy;
 
     for (int s = 0; s < ns; ++s) {
         // eta: valid on [s, EX - 1 - s) x [s, EY - 1 - s) given U, V valid on [s, EX - s) x [s, EY - s)
@@ -113,12 +110,12 @@ __global__ void __launch_bounds__(1024) k_barotropic_tile(const DevP<T> P, const
         for (int q = tid; q < NE; q += NT) {
             const int x = q % EX, y = q / EX;
             const unsigned char mk = smk[q];
-            const B ec = se[q];
-            if (x > 0) sU[q] = (mk & 2) ? sU[q] + dtau * (-g * (B)sHu[q] * (ec - se[q - 1]) * rdx[y] + sGU[q]) : B(0);
-            if (y > 0) sV[q] = (mk & 4) ? sV[q] + dtau * (-g * (B)sHv[q] * (ec - se[q - EX]) * rdy + sGV[q]) : B(0);
+            const T ec = se[q];
+            if (x > 0) sU[q] = (mk & 2) ? sU[q] + dtau * (-g * sHu[q] * (ec - se[q - 1]) * rdx[y] + sGU[q]) : T(0);
+            if (y > 0) sV[q] = (mk & 4) ? sV[q] + dtau * (-g * sHv[q] * (ec - se[q - EX]) * rdy + sGV[q]) : T(0);
         }
         __syncthreads();
-        const B am = saw[s];
+        const T am = saw[s];
 #pragma unroll
         for (int n = 0; n < C::PER; ++n) {
             const int t = n * NT + tid;
@@ -176,8 +173,8 @@ __global__ void __launch_bounds__(128) k_backsub_correct(const DevP<T> P) {
     const uint2 m = P.m8[c];
     const int kb = m.x & 255, tx1 = (m.x >> 8) & 255, ty1 = m.y & 255;
     if (kb >= nz) return;
-    const T cu = tx1 < nz ? (T)((P.Ub[c] - P.SU[c]) * (double)P.rHu[c]) : T(0);
-    const T cv = ty1 < nz ? (T)((P.Vb[c] - P.SV[c]) * (double)P.rHv[c]) : T(0);
+    const T cu = tx1 < nz ? (P.Ub[c] - P.SU[c]) * P.rHu[c] : T(0);
+    const T cv = ty1 < nz ? (P.Vb[c] - P.SV[c]) * P.rHv[c] : T(0);
     const T* __restrict__ cpu = P.cp_m + min(tx1, nz - 1);
     const T* __restrict__ cpv = P.cp_m + min(ty1, nz - 1);
     const T* __restrict__ cpt = P.cp_t + kb;
@@ -268,8 +265,8 @@ __global__ void __launch_bounds__(128) k_init_transport(const DevP<T> P) {
     const long long sz = P.sz, c = (long long)(j + OCN_HALO) * P.sx + i;
     double su = 0, sv = 0;
     for (int k = 0; k < P.nz; ++k) { const typename Pair<T>::type q = P.uv[k * sz + c]; su += (double)P.dz[k] * (double)q.x; sv += (double)P.dz[k] * (double)q.y; }
-    store_halo(P.U[0], P.sx, P.nx, P.ny, P.px, P.py, j, i, su);
-    store_halo(P.V[0], P.sx, P.nx, P.ny, P.px, P.py, j, i, sv);
+    store_halo(P.U[0], P.sx, P.nx, P.ny, P.px, P.py, j, i, (T)su);
+    store_halo(P.V[0], P.sx, P.nx, P.ny, P.px, P.py, j, i, (T)sv);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -290,8 +287,8 @@ __device__ __forceinline__ bool cell_open(const DevP<T>& P, long long c, int k, 
     }
 }
 
-template <class T, class D>
-__global__ void __launch_bounds__(256) k_scatter(const DevP<T> P, D* __restrict__ dst, const T* __restrict__ src,
+template <class T>
+__global__ void __launch_bounds__(256) k_scatter(const DevP<T> P, T* __restrict__ dst, const T* __restrict__ src,
                                                  const int nl, const int kind, const int st) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
@@ -300,12 +297,12 @@ __global__ void __launch_bounds__(256) k_scatter(const DevP<T> P, D* __restrict_
     const T off = kind == 2 ? P.Toff : kind == 3 ? P.Soff : T(0);
     for (int k = blockIdx.z; k < nl; k += gridDim.z) {
         const T v = cell_open(P, c, k, kind) ? src[((long long)k * P.ny + j) * P.nx + i] - off : T(0);
-        store_halo(dst + k * P.sz * st, P.sx, P.nx, P.ny, P.px, P.py, j, i, (D)v, st);
+        store_halo(dst + k * P.sz * st, P.sx, P.nx, P.ny, P.px, P.py, j, i, v, st);
     }
 }
 
-template <class T, class S, class O>
-__global__ void __launch_bounds__(256) k_gather(const DevP<T> P, O* __restrict__ dst, const S* __restrict__ src,
+template <class T, class O>
+__global__ void __launch_bounds__(256) k_gather(const DevP<T> P, O* __restrict__ dst, const T* __restrict__ src,
                                                 const int nl, const int kind, const int st) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
@@ -313,7 +310,7 @@ __global__ void __launch_bounds__(256) k_gather(const DevP<T> P, O* __restrict__
     const long long c = (long long)(j + OCN_HALO) * P.sx + i;
     const T off = kind == 2 ? P.Toff : kind == 3 ? P.Soff : T(0);
     for (int k = blockIdx.z; k < nl; k += gridDim.z) {
-        const S v = cell_open(P, c, k, kind) ? src[(k * P.sz + c) * st] + (S)off : S(0);
+        const T v = cell_open(P, c, k, kind) ? src[(k * P.sz + c) * st] + off : T(0);
         dst[((long long)k * P.ny + j) * P.nx + i] = (O)v;
     }
 }

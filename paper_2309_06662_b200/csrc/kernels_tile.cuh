@@ -491,6 +491,6 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
         __syncthreads();                       // planes of level m - 1 are dead: refill the ring
         if (tid == 0 && m + C::DP <= nz) issue_group(m + C::DP, false);
     }
-    if (cM.incol && cM.kb < nz) { P.GU[cM.c] = aGU; P.GV[cM.c] = aGV; P.SU[cM.c] = aSU; P.SV[cM.c] = aSV; }
+    if (cM.incol && cM.kb < nz) { P.GU[cM.c] = (T)aGU; P.GV[cM.c] = (T)aGV; P.SU[cM.c] = (T)aSU; P.SV[cM.c] = (T)aSV; }
 }
 }  // namespace ocn

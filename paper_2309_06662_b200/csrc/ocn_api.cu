@@ -136,9 +136,8 @@ ocn_status build_model(ocn_model* M) {
     for (T2** f : f3) if ((s = dev_alloc(M, n3, f, true)) != OCN_OK) return s;
     if ((s = dev_alloc(M, n3, &P.p, true)) != OCN_OK) return s;
     if ((s = plane(n3 + n2, &P.w)) != OCN_OK) return s;
-    double** fb[] = {&P.eta[0], &P.eta[1], &P.U[0], &P.U[1], &P.V[0], &P.V[1], &P.etab, &P.Ub, &P.Vb, &P.GU, &P.GV, &P.SU, &P.SV};
-    for (double** f : fb) if ((s = dev_alloc(M, n2, f, true)) != OCN_OK) return s;
-    T** f2[] = {&P.Hu, &P.Hv, &P.rHu, &P.rHv, &P.taux, &P.tauy};
+    T** f2[] = {&P.eta[0], &P.eta[1], &P.U[0], &P.U[1], &P.V[0], &P.V[1], &P.etab, &P.Ub, &P.Vb, &P.GU, &P.GV,
+                &P.SU, &P.SV, &P.Hu, &P.Hv, &P.rHu, &P.rHv, &P.taux, &P.tauy};
     for (T** f : f2) if ((s = plane(n2, f)) != OCN_OK) return s;
     // masks
     {
@@ -294,8 +293,8 @@ ocn_status launch_step(ocn_model* M, bool euler) {
         int cur = 0;
         for (int m0 = 0; m0 < M->d.substeps; m0 += BT_HALO) {
             const int ns = std::min(BT_HALO, M->d.substeps - m0);
-            double a[BT_HALO];
-            for (int q = 0; q < BT_HALO; ++q) a[q] = q < ns ? M->a_w[m0 + q] : 0.0;
+            T a[BT_HALO];
+            for (int q = 0; q < BT_HALO; ++q) a[q] = q < ns ? (T)M->a_w[m0 + q] : T(0);
             ocn::k_barotropic_tile<T, BT_X, BT_Y><<<gb, B::NT, B::SMEM, M->stream>>>(P, cur, ns, m0 == 0 ? 1 : 0, a[0], a[1], a[2],
                                                                                  a[3], a[4], a[5]);
             cur ^= 1;
@@ -336,8 +335,8 @@ ocn_status run_steps(ocn_model* M, int n) {
     return OCN_OK;
 }
 
-template <class T, class D>
-ocn_status set_one(ocn_model* M, const void* src, D* dst, int nl, int kind, bool on_device, int st = 1) {
+template <class T>
+ocn_status set_one(ocn_model* M, const void* src, T* dst, int nl, int kind, bool on_device, int st = 1) {
     const ocn_grid* g = M->g;
     const size_t n = (size_t)nl * g->ny * g->nx;
     const T* dsrc = static_cast<const T*>(src);
@@ -346,7 +345,7 @@ ocn_status set_one(ocn_model* M, const void* src, D* dst, int nl, int kind, bool
         dsrc = static_cast<const T*>(M->stage);
     }
     const dim3 b(32, 8);
-    ocn::k_scatter<T, D><<<grid2(g, b, nl < 64 ? nl : 64), b, 0, M->stream>>>(params<T>(M), dst, dsrc, nl, kind, st);
+    ocn::k_scatter<T><<<grid2(g, b, nl < 64 ? nl : 64), b, 0, M->stream>>>(params<T>(M), dst, dsrc, nl, kind, st);
     CK(cudaGetLastError());
     if (!on_device) CK(cudaStreamSynchronize(M->stream));   // staging buffer is reused by the next field
     return OCN_OK;
@@ -375,13 +374,13 @@ ocn_status set_fields_t(ocn_model* M, const ocn_fields* f) {
     return OCN_OK;
 }
 
-template <class T, class O, class S>
-ocn_status get_one(ocn_model* M, void* dst, const S* src, int nl, int kind, bool on_device, int st = 1) {
+template <class T, class O>
+ocn_status get_one(ocn_model* M, void* dst, const T* src, int nl, int kind, bool on_device, int st = 1) {
     const ocn_grid* g = M->g;
     const size_t n = (size_t)nl * g->ny * g->nx;
     O* ddst = on_device ? static_cast<O*>(dst) : static_cast<O*>(M->stage);
     const dim3 b(32, 8);
-    ocn::k_gather<T, S, O><<<grid2(g, b, nl < 64 ? nl : 64), b, 0, M->stream>>>(params<T>(M), ddst, src, nl, kind, st);
+    ocn::k_gather<T, O><<<grid2(g, b, nl < 64 ? nl : 64), b, 0, M->stream>>>(params<T>(M), ddst, src, nl, kind, st);
     CK(cudaGetLastError());
     if (!on_device) {
         CK(cudaMemcpyAsync(dst, M->stage, n * sizeof(O), cudaMemcpyDeviceToHost, M->stream));
