@@ -33,8 +33,10 @@ if ROOT not in sys.path:
 
 METRIC = "cell_updates_per_s"
 UNIT = "cell-updates/s"
-# algorithmic HBM words per wet cell-update of each stage: compulsory reads + writes
-STAGE_WORDS = {"tendency": 17, "backsub_correct_pressure": 9}
+# algorithmic HBM bytes per wet cell-update of each stage: compulsory reads + writes; every array is
+# `word` bytes per value except the hydrostatic pressure, which is stored in fp64 in both precisions
+def stage_bytes(stage, word):
+    return {"tendency": 16 * word + 8, "backsub_correct_pressure": 8 * word + 8}.get(stage)
 # window of config 4 the oracle is timed on: (j0, j1, i0, i1)
 CPU_WINDOW = (500, 700, 1300, 1700)
 
@@ -262,19 +264,19 @@ def run_ours(args):
     peak, peak_src = measured_peak()
     word = 4 if prm["precision"] == 32 else 8
     dom = max(stages, key=lambda s: stages[s]["ms"])
-    words = STAGE_WORDS.get(dom)
+    dom_bytes = stage_bytes(dom, word)
     roof = None
     stage_out = {}
     for s, v in stages.items():
         stage_out[s] = {"ms_per_step": v["ms"] / K, "launches_per_step": v["launches"] / K}
-        if s in STAGE_WORDS:
-            stage_out[s]["algorithmic_gbs"] = STAGE_WORDS[s] * word * nwet / (v["ms"] / K * 1e-3) / 1e9
-    if words is not None:
-        alg_bytes = words * word * nwet
+        if stage_bytes(s, word):
+            stage_out[s]["algorithmic_gbs"] = stage_bytes(s, word) * nwet / (v["ms"] / K * 1e-3) / 1e9
+    if dom_bytes is not None:
+        alg_bytes = dom_bytes * nwet
         ach = alg_bytes / (stages[dom]["ms"] / K * 1e-3) / 1e9
         roof = {"kernel": dom, "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
-                "bytes_per_wet_cell": words * word, "traffic": ncu_traffic(workload_name(wl), dom)}
+                "bytes_per_wet_cell": dom_bytes, "traffic": ncu_traffic(workload_name(wl), dom)}
     else:                       # the 2-D sub-cycle dominates (tiny 3-D grids): 16 words per column per sub-step
         ncol = nx * ny
         alg_bytes = 16 * word * ncol * prm["substeps"]
