@@ -58,7 +58,7 @@ struct DevP {
     const T *sm_m, *cp_m, *m_m, *rm_m;
     const T *sm_t, *cp_t, *m_t, *rm_t;
     // physics
-    T dt, g, alpha, beta_s, rrho0, nu_h, kappa_h;
+    T dt, g, alpha, beta_s, rho0, rrho0, nu_h, kappa_h;
     T Toff, Soff;          // storage offsets of the tracers: (T0, S0) in fp32, 0 in fp64
     T dT0, dS0;            // T0 - Toff, S0 - Soff: what is left to subtract in the buoyancy
     double g_d, alpha_d, beta_d, dT0_d, dS0_d, hz_top_d;   // fp64 copies for the pressure integral
@@ -114,10 +114,61 @@ __device__ __forceinline__ void store_halo(T* __restrict__ plane, int sx, int nx
 }
 
 // ---------------------------------------------------------------------------------------------
+// Xv<T>: a value whose arithmetic keeps the written association.  In fp64 every operator is a
+// correctly rounded, non-contracted IEEE operation (__dmul_rn, ...), so an expression written in
+// the order of DESIGN.md §3 rounds exactly like the equations as written; in fp32
+// the operators are plain and the compiler is free to contract.  xdiv(a, b, rb) = a / b in fp64 and
+// a * rb (rb = 1 / b, precomputed) in fp32.
+// ---------------------------------------------------------------------------------------------
+template <class T> struct Xv { T v; __device__ __forceinline__ explicit Xv(T x) : v(x) {} __device__ __forceinline__ Xv() : v(0) {} };
+__device__ __forceinline__ Xv<double> operator*(Xv<double> a, Xv<double> b) { return Xv<double>(__dmul_rn(a.v, b.v)); }
+__device__ __forceinline__ Xv<double> operator+(Xv<double> a, Xv<double> b) { return Xv<double>(__dadd_rn(a.v, b.v)); }
+__device__ __forceinline__ Xv<double> operator-(Xv<double> a, Xv<double> b) { return Xv<double>(__dsub_rn(a.v, b.v)); }
+__device__ __forceinline__ Xv<double> operator/(Xv<double> a, Xv<double> b) { return Xv<double>(__ddiv_rn(a.v, b.v)); }
+__device__ __forceinline__ Xv<double> operator-(Xv<double> a) { return Xv<double>(-a.v); }
+__device__ __forceinline__ Xv<float> operator*(Xv<float> a, Xv<float> b) { return Xv<float>(a.v * b.v); }
+__device__ __forceinline__ Xv<float> operator+(Xv<float> a, Xv<float> b) { return Xv<float>(a.v + b.v); }
+__device__ __forceinline__ Xv<float> operator-(Xv<float> a, Xv<float> b) { return Xv<float>(a.v - b.v); }
+__device__ __forceinline__ Xv<float> operator/(Xv<float> a, Xv<float> b) { return Xv<float>(a.v / b.v); }
+__device__ __forceinline__ Xv<float> operator-(Xv<float> a) { return Xv<float>(-a.v); }
+__device__ __forceinline__ Xv<double> xdiv(Xv<double> a, double b, double) { return Xv<double>(__ddiv_rn(a.v, b)); }
+__device__ __forceinline__ Xv<float> xdiv(Xv<float> a, float, float rb) { return Xv<float>(a.v * rb); }
+template <class T> __device__ __forceinline__ Xv<T> X(T v) { return Xv<T>(v); }
+
+// fp64 face value with the weights evaluated as written in DESIGN.md §3.4 (alpha_s = d_s / (eps + beta_s)^2)
+__device__ __forceinline__ double weno_face_exact(double a, double b, double c, double d, double e, double f, double vel, int order) {
+    typedef Xv<double> V;
+    const bool pos = vel > 0.0;
+    const V qm2(pos ? a : f), qm1(pos ? b : e), q0(pos ? c : d), q1(pos ? d : c), q2(pos ? e : b);
+    const V eps(1e-6), two(2.0);
+    if (order >= 3) {
+        const V p0 = (two * qm2 - V(7.0) * qm1 + V(11.0) * q0) / V(6.0);
+        const V p1 = (-qm1 + V(5.0) * q0 + two * q1) / V(6.0);
+        const V p2 = (two * q0 + V(5.0) * q1 - q2) / V(6.0);
+        const V c13(13.0 / 12.0), c4(0.25);
+        const V b0 = c13 * (qm2 - two * qm1 + q0) * (qm2 - two * qm1 + q0) + c4 * (qm2 - V(4.0) * qm1 + V(3.0) * q0) * (qm2 - V(4.0) * qm1 + V(3.0) * q0);
+        const V b1 = c13 * (qm1 - two * q0 + q1) * (qm1 - two * q0 + q1) + c4 * (qm1 - q1) * (qm1 - q1);
+        const V b2 = c13 * (q0 - two * q1 + q2) * (q0 - two * q1 + q2) + c4 * (V(3.0) * q0 - V(4.0) * q1 + q2) * (V(3.0) * q0 - V(4.0) * q1 + q2);
+        const V a0 = V(0.1) / ((eps + b0) * (eps + b0)), a1 = V(0.6) / ((eps + b1) * (eps + b1)), a2 = V(0.3) / ((eps + b2) * (eps + b2));
+        return ((a0 * p0 + a1 * p1 + a2 * p2) / (a0 + a1 + a2)).v;
+    }
+    if (order == 2) {
+        const V p0 = (-qm1 + V(3.0) * q0) / two, p1 = (q0 + q1) / two;
+        const V b0 = (q0 - qm1) * (q0 - qm1), b1 = (q1 - q0) * (q1 - q0);
+        const V a0 = V(1.0 / 3.0) / ((eps + b0) * (eps + b0)), a1 = V(2.0 / 3.0) / ((eps + b1) * (eps + b1));
+        return ((a0 * p0 + a1 * p1) / (a0 + a1)).v;
+    }
+    return order == 1 ? q0.v : 0.0;
+}
+
+// ---------------------------------------------------------------------------------------------
 // WENO face value (Shu 1997 as cited at PAPER.md:244).  Cells n-3..n+2 are
 // (a, b, c, d, e, f); the face lies between c and d; q0 is the upwind cell.
 // Division-free nonlinear weights: alpha_s ~ d_s * prod_{t != s} (eps + beta_t)^2, one division.
 // ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ double weno_face(double a, double b, double c, double d, double e, double f, double vel, int order) {
+    return weno_face_exact(a, b, c, d, e, f, vel, order);
+}
 template <class T>
 __device__ __forceinline__ T weno_face(T a, T b, T c, T d, T e, T f, T vel, int order) {
     const bool pos = vel > T(0);

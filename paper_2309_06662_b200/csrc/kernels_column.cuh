@@ -35,8 +35,8 @@ __device__ __forceinline__ double pressure_level(const DevP<T>& P, int k, double
 template <class T, int BTX, int BTY>
 struct BtTile {
     static constexpr int EX = BTX + 2 * BT_HALO, EY = BTY + 2 * BT_HALO, NE = EX * EY;
-    static constexpr int NT = 1024, PER = (BTX * BTY + NT - 1) / NT;
-    static constexpr int SMEM = NE * (7 * (int)sizeof(T) + 1) + 4 * (EY + 1) * (int)sizeof(T) + 64 + BT_HALO * (int)sizeof(T);
+    static constexpr int NT = 1024, PER = (NE + NT - 1) / NT;      // extended-tile points per thread
+    static constexpr int SMEM = NE * (7 * (int)sizeof(T) + 1) + 6 * (EY + 1) * (int)sizeof(T) + 64 + BT_HALO * (int)sizeof(T);
 };
 
 template <class T, int BTX, int BTY>
@@ -55,7 +55,9 @@ __global__ void __launch_bounds__(1024) k_barotropic_tile(const DevP<T> P, const
     T* const rAz = sHv + NE;               // per extended row: 1 / AzC, 1 / dxC, dxF (row), dxF (row + 1)
     T* const rdx = rAz + (EY + 1);
     T* const dF = rdx + (EY + 1);          // EY + 1 entries
-    T* const saw = dF + (EY + 1);          // filter weights of this launch
+    T* const Az = dF + (EY + 1);           // AzC, dxC per extended row (fp64 divides, fp32 multiplies by the reciprocals)
+    T* const dxc = Az + (EY + 1);
+    T* const saw = dxc + (EY + 1);         // filter weights of this launch
     unsigned char* const smk = (unsigned char*)(saw + BT_HALO);   // bit 0 wet, bit 1 open u face, bit 2 open v face
     const int tid = threadIdx.x;
     const int i0 = blockIdx.x * BTX, j0 = blockIdx.y * BTY;
@@ -67,7 +69,7 @@ __global__ void __launch_bounds__(1024) k_barotropic_tile(const DevP<T> P, const
         int jj = j0 - H + q;
         if (P.py) jj = ((jj % ny) + ny) % ny;
         const int r = min(max(jj, -OCN_HALO), ny + OCN_HALO) + OCN_HALO;      // metric rows exist for -3 .. ny + 3
-        if (q < EY) { rAz[q] = P.rAzC[r]; rdx[q] = P.rdxC[r]; }
+        if (q < EY) { rAz[q] = P.rAzC[r]; rdx[q] = P.rdxC[r]; Az[q] = P.AzC[r]; dxc[q] = P.dxC[r]; }
         dF[q] = P.dxF[r];
     }
     const T* __restrict__ e0 = P.eta[cur];
@@ -93,10 +95,22 @@ __global__ void __launch_bounds__(1024) k_barotropic_tile(const DevP<T> P, const
     }
     __syncthreads();
 
-    // ---- the interior points this thread owns, and their filter sums ----
+    // ---- filter sums of the points this thread updates (same point-to-thread map as the update loops, so no
+    // other thread touches a value between its update and its accumulation); one running sum over all M
+    // sub-steps (DESIGN.md §3.8 step 6), continued from the previous launch --------------------------------
     T be[C::PER], bU[C::PER], bV[C::PER];
+    long long cidx[C::PER];                                   // global index of the interior points, -1 elsewhere
 #pragma unroll
-    for (int n = 0; n < C::PER; ++n) { be[n] = 0; bU[n] = 0; bV[n] = 0; }
+    for (int n = 0; n < C::PER; ++n) {
+        be[n] = 0; bU[n] = 0; bV[n] = 0; cidx[n] = -1;
+        const int q = n * NT + tid;
+        const int x = q % EX - H, y = q / EX - H;
+        const int i = i0 + x, j = j0 + y;
+        if (q < NE && x >= 0 && x < BTX && y >= 0 && y < BTY && i < nx && j < ny) {
+            cidx[n] = (long long)(j + OCN_HALO) * sx + i;
+            if (!first) { be[n] = P.etab[cidx[n]]; bU[n] = P.Ub[cidx[n]]; bV[n] = P.Vb[cidx[n]]; }
+        }
+    }
     const T dy = P.dy, dtau = P.dtau, g = P.g, rdy = P.rdy;
 
     for (int s = 0; s < ns; ++s) {
@@ -104,41 +118,35 @@ __global__ void __launch_bounds__(1024) k_barotropic_tile(const DevP<T> P, const
         for (int q = tid; q < NE; q += NT) {
             const int x = q % EX, y = q / EX;
             if (x < EX - 1 && y < EY - 1 && (smk[q] & 1))
-                se[q] -= dtau * (dy * (sU[q + 1] - sU[q]) + dF[y + 1] * sV[q + EX] - dF[y] * sV[q]) * rAz[y];
-        }
-        __syncthreads();
-        for (int q = tid; q < NE; q += NT) {
-            const int x = q % EX, y = q / EX;
-            const unsigned char mk = smk[q];
-            const T ec = se[q];
-            if (x > 0) sU[q] = (mk & 2) ? sU[q] + dtau * (-g * sHu[q] * (ec - se[q - 1]) * rdx[y] + sGU[q]) : T(0);
-            if (y > 0) sV[q] = (mk & 4) ? sV[q] + dtau * (-g * sHv[q] * (ec - se[q - EX]) * rdy + sGV[q]) : T(0);
+                se[q] = (X(se[q]) - xdiv(X(dtau) * (X(dy) * (X(sU[q + 1]) - X(sU[q])) + X(dF[y + 1]) * X(sV[q + EX]) - X(dF[y]) * X(sV[q])),
+                                         Az[y], rAz[y])).v;
         }
         __syncthreads();
         const T am = saw[s];
 #pragma unroll
         for (int n = 0; n < C::PER; ++n) {
-            const int t = n * NT + tid;
-            if (t < BTX * BTY) {
-                const int q = (t / BTX + H) * EX + (t % BTX) + H;
-                be[n] += am * se[q]; bU[n] += am * sU[q]; bV[n] += am * sV[q];
+            const int q = n * NT + tid;
+            if (q < NE) {
+                const int x = q % EX, y = q / EX;
+                const unsigned char mk = smk[q];
+                const T ec = se[q];
+                T un = sU[q], vn = sV[q];
+                if (x > 0) un = (mk & 2) ? (X(un) + X(dtau) * (xdiv(-X(g) * X(sHu[q]) * (X(ec) - X(se[q - 1])), dxc[y], rdx[y]) + X(sGU[q]))).v : T(0);
+                if (y > 0) vn = (mk & 4) ? (X(vn) + X(dtau) * (xdiv(-X(g) * X(sHv[q]) * (X(ec) - X(se[q - EX])), dy, rdy) + X(sGV[q]))).v : T(0);
+                sU[q] = un; sV[q] = vn;
+                be[n] = (X(be[n]) + X(am) * X(ec)).v; bU[n] = (X(bU[n]) + X(am) * X(un)).v; bV[n] = (X(bV[n]) + X(am) * X(vn)).v;
             }
         }
+        __syncthreads();
     }
     // ---- write back the interior ----
 #pragma unroll
     for (int n = 0; n < C::PER; ++n) {
-        const int t = n * NT + tid;
-        if (t < BTX * BTY) {
-            const int tx = t % BTX, ty = t / BTX;
-            const int i = i0 + tx, j = j0 + ty;
-            if (i < nx && j < ny) {
-                const int q = (ty + H) * EX + tx + H;
-                const long long c = (long long)(j + OCN_HALO) * sx + i;
-                P.eta[cur ^ 1][c] = se[q]; P.U[cur ^ 1][c] = sU[q]; P.V[cur ^ 1][c] = sV[q];
-                if (first) { P.etab[c] = be[n]; P.Ub[c] = bU[n]; P.Vb[c] = bV[n]; }
-                else       { P.etab[c] += be[n]; P.Ub[c] += bU[n]; P.Vb[c] += bV[n]; }
-            }
+        if (cidx[n] >= 0) {
+            const int q = n * NT + tid;
+            const long long c = cidx[n];
+            P.eta[cur ^ 1][c] = se[q]; P.U[cur ^ 1][c] = sU[q]; P.V[cur ^ 1][c] = sV[q];
+            P.etab[c] = be[n]; P.Ub[c] = bU[n]; P.Vb[c] = bV[n];
         }
     }
 }
@@ -210,8 +218,27 @@ __global__ void __launch_bounds__(128) k_backsub_correct(const DevP<T> P) {
                 T un = 0, vn = 0;
                 if (mu) { xu = E::sub(d_uv[q].x, E::mul(cpu[k * nz], xu)); un = xu + cu; }
                 if (mv) { xv = E::sub(d_uv[q].y, E::mul(cpv[k * nz], xv)); vn = xv + cv; }
-                store_halo(P.uv + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, mk2(un, vn));
+                if (sizeof(T) == 8) P.uv[k * sz + c] = mk2(xu * T(mu), xv * T(mv));      // u**, corrected below
+                else store_halo(P.uv + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, mk2(un, vn));
             }
+        }
+    }
+    if (sizeof(T) == 8) {
+        // fp64: the correction as DESIGN.md §3.8 step 8 writes it, (Ubar - sum_k dz u**) / Hu with the sum taken
+        // bottom-up over the back-substituted column (the fp32 path uses K1's sum of the predictor instead)
+        double su = 0.0, sv = 0.0;
+        for (int k = kuv; k < nz; ++k) {
+            const T2 q = P.uv[k * sz + c];
+            su = (X(su) + X((double)P.dz[k]) * X((double)q.x)).v;
+            sv = (X(sv) + X((double)P.dz[k]) * X((double)q.y)).v;
+        }
+        const double cu2 = tx1 < nz ? ((X((double)P.Ub[c]) - X(su)) / X((double)P.Hu[c])).v : 0.0;
+        const double cv2 = ty1 < nz ? ((X((double)P.Vb[c]) - X(sv)) / X((double)P.Hv[c])).v : 0.0;
+        for (int k = kuv; k < nz; ++k) {
+            const T2 q = P.uv[k * sz + c];
+            const T un = k >= tx1 ? (T)(X((double)q.x) + X(cu2)).v : T(0);
+            const T vn = k >= ty1 ? (T)(X((double)q.y) + X(cv2)).v : T(0);
+            store_halo(P.uv + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, mk2(un, vn));
         }
     }
 }
@@ -246,12 +273,12 @@ __global__ void __launch_bounds__(128) k_vertical_velocity(const DevP<T> P) {
     if (i >= P.nx || j >= P.ny) return;
     const int sx = P.sx, nz = P.nz, r = j + OCN_HALO;
     const long long sz = P.sz, c = (long long)r * sx + i;
-    const T dy = P.dy, dF0 = P.dxF[r], dF1 = P.dxF[r + 1], rA = P.rAzC[r];
+    const T dy = P.dy, dF0 = P.dxF[r], dF1 = P.dxF[r + 1], rA = P.rAzC[r], A = P.AzC[r];
     double w = 0.0;
     for (int k = 0; k < nz; ++k) {
         const typename Pair<T>::type* __restrict__ q = P.uv + k * sz + c;
-        const T D = (dy * (q[1].x - q[0].x) + dF1 * q[sx].y - dF0 * q[0].y) * rA;
-        w -= (double)P.dz[k] * (double)D;
+        const T D = xdiv(X(dy) * (X(q[1].x) - X(q[0].x)) + X(dF1) * X(q[sx].y) - X(dF0) * X(q[0].y), A, rA).v;
+        w = (X(w) - X((double)P.dz[k]) * X((double)D)).v;
         store_halo(P.w + (k + 1) * sz, sx, P.nx, P.ny, P.px, P.py, j, i, (T)w);
     }
 }
@@ -264,7 +291,7 @@ __global__ void __launch_bounds__(128) k_init_transport(const DevP<T> P) {
     if (i >= P.nx || j >= P.ny) return;
     const long long sz = P.sz, c = (long long)(j + OCN_HALO) * P.sx + i;
     double su = 0, sv = 0;
-    for (int k = 0; k < P.nz; ++k) { const typename Pair<T>::type q = P.uv[k * sz + c]; su += (double)P.dz[k] * (double)q.x; sv += (double)P.dz[k] * (double)q.y; }
+    for (int k = 0; k < P.nz; ++k) { const typename Pair<T>::type q = P.uv[k * sz + c]; su = (X(su) + X((double)P.dz[k]) * X((double)q.x)).v; sv = (X(sv) + X((double)P.dz[k]) * X((double)q.y)).v; }
     store_halo(P.U[0], P.sx, P.nx, P.ny, P.px, P.py, j, i, (T)su);
     store_halo(P.V[0], P.sx, P.nx, P.ny, P.px, P.py, j, i, (T)sv);
 }

@@ -69,8 +69,8 @@ struct Tile {
     static constexpr int FLB = rup128(NF * (int)sizeof(T2));
     static constexpr int O_FLUX = O_W + 3 * WB;                                 // 2 x T2 per face
     static constexpr int O_M8 = O_FLUX + 2 * FLB;                               // uint2 on RX x RY (not zero-filled from here on)
-    static constexpr int O_MET = O_M8 + rup128(RX * RY * 8);                    // 8 row-metric arrays of BY + 1
-    static constexpr int O_CELL = O_MET + rup128(8 * (BY + 1) * (int)sizeof(T)); // uint16: cells sorted by first wet level
+    static constexpr int O_MET = O_M8 + rup128(RX * RY * 8);                    // 9 row-metric arrays of BY + 1
+    static constexpr int O_CELL = O_MET + rup128(9 * (BY + 1) * (int)sizeof(T)); // uint16: cells sorted by first wet level
     static constexpr int O_FS = O_CELL + rup128(NC * 2);                        // uint2: face descriptors sorted by first open level
     static constexpr int O_NC = O_FS + rup128(NF * 8);                          // uint16[256]: active cells at level k
     static constexpr int O_NF = O_NC + 512;                                     // uint16[256]: active faces at level k
@@ -101,6 +101,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     T* const s_AzC = s_rdxC + (BY + 1);
     T* const s_fF = s_AzC + (BY + 1);
     T* const s_rdxF = s_fF + (BY + 1);
+    T* const s_AzF = s_rdxF + (BY + 1);
     uint64_t* const bars = (uint64_t*)(sm + C::O_BAR);
     int& s_kmin = *(int*)(sm + C::O_BAR + 64);
 
@@ -226,7 +227,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
         for (int q = tid; q <= BY; q += NT) {
             const int r = min(j0 + q, nr - 1);
             s_dxC[q] = P.dxC[r]; s_dxF[q] = P.dxF[r]; s_rAzC[q] = P.rAzC[r]; s_rAzF[q] = P.rAzF[r]; s_rdxC[q] = P.rdxC[r];
-            s_AzC[q] = P.AzC[r]; s_fF[q] = P.fF[r]; s_rdxF[q] = P.rdxF[r];
+            s_AzC[q] = P.AzC[r]; s_fF[q] = P.fF[r]; s_rdxF[q] = P.rdxF[r]; s_AzF[q] = P.AzF[r];
         }
     }
     if (tid == 0) {
@@ -321,7 +322,8 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 if (q < (BX - 1) * (BY - 1)) {
                     const int px = 1 + q % (BX - 1), py = 1 + q / (BX - 1);
                     const T2 a = s_uv[py * BX + px], as = s_uv[(py - 1) * BX + px], aw = s_uv[py * BX + px - 1];
-                    s_zeta[py * BX + px] = (dy * (a.y - aw.y) - (s_dxC[py] * a.x - s_dxC[py - 1] * as.x)) * s_rAzF[py];
+                    s_zeta[py * BX + px] = xdiv(X(dy) * (X(a.y) - X(aw.y)) - (X(s_dxC[py]) * X(a.x) - X(s_dxC[py - 1]) * X(as.x)),
+                                                s_AzF[py], s_rAzF[py]).v;
                 }
             }
     #pragma unroll
@@ -331,11 +333,11 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                     const int qx = q % RX, qy = q / RX;
                     const int px = qx + OX - 1, py = qy + OY - 1;          // cells i0 - 1 + qx, j0 - 1 + qy
                     const T2 a = s_uv[py * BX + px], ae = s_uv[py * BX + px + 1], an = s_uv[(py + 1) * BX + px];
-                    const T Kc = T(0.25) * (a.x * a.x + ae.x * ae.x) + T(0.25) * (a.y * a.y + an.y * an.y);
-                    const T Dc = (dy * (ae.x - a.x) + s_dxF[py + 1] * an.y - s_dxF[py] * a.y) * s_rAzC[py];
+                    const T Kc = (X(T(0.25)) * (X(a.x) * X(a.x) + X(ae.x) * X(ae.x)) + X(T(0.25)) * (X(a.y) * X(a.y) + X(an.y) * X(an.y))).v;
+                    const T Dc = xdiv(X(dy) * (X(ae.x) - X(a.x)) + X(s_dxF[py + 1]) * X(an.y) - X(s_dxF[py]) * X(a.y), s_AzC[py], s_rAzC[py]).v;
                     s_kd[q] = mk2(Kc, Dc);
                     double& wa = n == 0 ? wacc0 : wacc1;
-                    wa -= (double)dzk * (double)Dc;
+                    wa = (X(wa) - X((double)dzk) * X((double)Dc)).v;
                     s_w1[q] = (T)wa;
                 }
             }
@@ -351,13 +353,14 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                     const int ord = order3(k, d.y & 255u, (d.y >> 8) & 255u, (d.y >> 16) & 255u);   // >= 1 here
                     const T2 uvf = s_uv[b];
                     const T vel = isy ? uvf.y : uvf.x;
-                    const T area = (isy ? s_dxF[row] : dy) * dzk;
-                    const T kd = P.kappa_h * area * (isy ? rdy : s_rdxC[row]);
+                    const T len = isy ? s_dxF[row] : dy;                       // face length; the face area is len * dz
+                    const T dd = isy ? dy : s_dxC[row], rdd = isy ? rdy : s_rdxC[row];   // centre-to-centre distance
                     const T2 cm = s_ts[b - st], cc = s_ts[b];
                     const T2 fv = weno_face2(s_ts[b - 3 * st], s_ts[b - 2 * st], cm, cc, s_ts[b + st], s_ts[b + 2 * st], vel, ord);
+                    const Xv<T> adv = X(vel) * X(len) * X(dzk), dif = X(P.kappa_h) * X(len) * X(dzk);
                     T2 flux;
-                    flux.x = vel * area * fv.x - kd * (cc.x - cm.x);
-                    flux.y = vel * area * fv.y - kd * (cc.y - cm.y);
+                    flux.x = (adv * X(fv.x) - xdiv(dif * (X(cc.x) - X(cm.x)), dd, rdd)).v;
+                    flux.y = (adv * X(fv.y) - xdiv(dif * (X(cc.y) - X(cm.y)), dd, rdd)).v;
                     s_flux[fid] = flux;
                 }
             }
@@ -386,22 +389,29 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 if (ozt > 0) {
                     auto tsz = [&](int kk) -> T2 { return ((const T2*)(sm + C::O_TS + ((kk + C::R_TS) % C::R_TS) * C::PL2))[bo]; };
                     const T2 fv = weno_face2(tsz(k - 2), tsz(k - 1), tsz(k), tsz(k + 1), tsz(k + 2), tsz(k + 3), w_c1, ozt);
-                    fz_top.x = w_c1 * AzCj * fv.x;
-                    fz_top.y = w_c1 * AzCj * fv.y;
+                    fz_top.x = (X(w_c1) * X(AzCj) * X(fv.x)).v;
+                    fz_top.y = (X(w_c1) * X(AzCj) * X(fv.y)).v;
                 }
             }
                 // ---- tracers ----
                 const T2 fw = s_flux[cy * RX + cx], fe = s_flux[cy * RX + cx + 1];
                 const T2 fs = s_flux[C::NFX + cy * TX + cx], fn = s_flux[C::NFX + (cy + 1) * TX + cx];
                 const T2 tsc = ((const T2*)(sm + C::O_TS + (k % C::R_TS) * C::PL2))[bo];
-                T GT = -((fe.x - fw.x) + (fn.x - fs.x) + (fz_top.x - fz_bot.x)) * rAzCj * rdzk;
-                T GS = -((fe.y - fw.y) + (fn.y - fs.y) + (fz_top.y - fz_bot.y)) * rAzCj * rdzk;
+                const T vol = (X(AzCj) * X(dzk)).v, rvol = rAzCj * rdzk;
+                T GT, GS;
+                if constexpr (sizeof(T) == 8) {    // the flux divergence summed in the order of DESIGN.md §3.7
+                    GT = xdiv(-(X(fe.x) - X(fw.x) + X(fn.x) - X(fs.x) + X(fz_top.x) - X(fz_bot.x)), vol, rvol).v;
+                    GS = xdiv(-(X(fe.y) - X(fw.y) + X(fn.y) - X(fs.y) + X(fz_top.y) - X(fz_bot.y)), vol, rvol).v;
+                } else {                           // fp32: difference the like fluxes first (they nearly cancel)
+                    GT = -((fe.x - fw.x) + (fn.x - fs.x) + (fz_top.x - fz_bot.x)) * rvol;
+                    GS = -((fe.y - fw.y) + (fn.y - fs.y) + (fz_top.y - fz_bot.y)) * rvol;
+                }
                 if (k == nz - 1) {                 // tracers are stored as offsets from (Toff, Soff): exact source
                     const T src = w_c1 * rdzk;     // of the constant under the zero-top-flux linear free surface
                     GT += P.Toff * src; GS += P.Soff * src;
                 }
                 // ---- quasi-AB2, predictor, elimination sweep (S3, S4) ----
-                const T Ght = c0 * GT - c1 * gm_ts.x, Ghs = c0 * GS - c1 * gm_ts.y;
+                const T Ght = (X(c0) * X(GT) - X(c1) * X(gm_ts.x)).v, Ghs = (X(c0) * X(GS) - X(c1) * X(gm_ts.y)).v;
                 P.Gts[o] = mk2(GT, GS);
                 const T smk = k > kb ? P.sm_t[k] : T(0);
                 ddts.x = E::div(E::add(E::add(tsc.x, E::mul(P.dt, Ght)), E::mul(smk, ddts.x)), piv_t, piv_t);
@@ -415,8 +425,8 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 const uchar4 mzt = cM.mzt;
                 const int qo = (cy + 1) * RX + cx + 1;                       // this column in the ring arrays
                 const T w_c1 = s_w1[qo], w_c0 = s_w0[qo];
-                const T dxFj = s_dxF[by], dxFn = s_dxF[by + 1], rdxCj = s_rdxC[by], rdxFj = s_rdxF[by];
-                const T AzCj = s_AzC[by], AzCs = s_AzC[by - 1], rAzFj = s_rAzF[by];
+                const T dxFj = s_dxF[by], dxFn = s_dxF[by + 1], dxCj = s_dxC[by], rdxCj = s_rdxC[by], rdxFj = s_rdxF[by];
+                const T AzCj = s_AzC[by], AzCs = s_AzC[by - 1], rAzCj = s_rAzC[by], AzFj = s_AzF[by], rAzFj = s_rAzF[by];
                 const T fFj = s_fF[by], fFn = s_fF[by + 1];
                 const bool mu = k >= tx1, mv = k >= ty1;
                 // ---- momentum ----
@@ -430,56 +440,60 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                     const T z00 = s_zeta[bo];
                     const T2 kdc = s_kd[qo];
                     const double pc = s_p[bo];
+                    const Xv<T> half(T(0.5)), quart(T(0.25)), nuh(P.nu_h);
+                    const T vold = (X(AzCj) * X(dzk)).v;                            // AzC dz (u) ; AzF dz for v below
                     if (mu) {
-                        const T vsum_s = uv_w.y + v_c, vsum_n = uv_nw.y + uv_n.y;
-                        const T vhat = T(0.25) * (dxFj * vsum_s + dxFn * vsum_n) * rdxCj;
+                        const Xv<T> vsum_s = X(uv_w.y) + X(v_c), vsum_n = X(uv_nw.y) + X(uv_n.y);
+                        const T vhat = xdiv(quart * (X(dxFj) * vsum_s + X(dxFn) * vsum_n), dxCj, rdxCj).v;
                         const int ozu = 1 + (k >= mzt.x) + (k >= mzt.y);
                         const T z01 = s_zeta[bo + BX];
                         const T zt = ozu == 1 ? (vhat > T(0) ? z00 : z01)
                                               : weno_face(s_zeta[bo - 2 * BX], s_zeta[bo - BX], z00, z01, s_zeta[bo + 2 * BX],
                                                           s_zeta[bo + 3 * BX], vhat, ozu);
-                        const T Cu = T(0.5) * (fFj * T(0.5) * dxFj * vsum_s + fFn * T(0.5) * dxFn * vsum_n) * rdxCj;
+                        const Xv<T> Cu = xdiv(half * (X(fFj) * half * X(dxFj) * vsum_s + X(fFn) * half * X(dxFn) * vsum_n), dxCj, rdxCj);
                         const T2 kdw = s_kd[qo - 1];
-                        const T dK = (kdc.x - kdw.x) * rdxCj;
-                        const T dP = (T)(pc - s_p[bo - 1]) * rdxCj;
-                        const T dlo = (k >= 1 && k - 1 >= tx1) ? u_c - u_dn : T(0);
-                        const T dhi = (k + 1 <= nz - 1) ? uv_up.x - u_c : T(0);
-                        const T Au = T(0.5) * (T(0.5) * (s_w1[qo - 1] + w_c1) * dhi + T(0.5) * (s_w0[qo - 1] + w_c0) * dlo) * rdzk;
-                        const T Vu = P.nu_h * ((kdc.y - kdw.y) * rdxCj - (z01 - z00) * rdy);
-                        const T tau = (k == nz - 1) ? P.taux[c] * P.rrho0 * rdzk : T(0);
-                        Gu = zt * vhat + Cu - dK - dP - Au + Vu + tau;
+                        const Xv<T> dK = xdiv(X(kdc.x) - X(kdw.x), dxCj, rdxCj);
+                        const Xv<T> dP = xdiv(X((T)(pc - s_p[bo - 1])), dxCj, rdxCj);
+                        const Xv<T> dlo((k >= 1 && k - 1 >= tx1) ? (X(u_c) - X(u_dn)).v : T(0));
+                        const Xv<T> dhi((k + 1 <= nz - 1) ? (X(uv_up.x) - X(u_c)).v : T(0));
+                        const Xv<T> Whi = half * X(AzCj) * (X(s_w1[qo - 1]) + X(w_c1)), Wlo = half * X(AzCj) * (X(s_w0[qo - 1]) + X(w_c0));
+                        const Xv<T> Au = xdiv(half * (Whi * dhi + Wlo * dlo), vold, rAzCj * rdzk);
+                        const Xv<T> Vu = nuh * (xdiv(X(kdc.y) - X(kdw.y), dxCj, rdxCj) - xdiv(X(z01) - X(z00), dy, rdy));
+                        const Xv<T> tau((k == nz - 1) ? xdiv(X(P.taux[c]), (X(P.rho0) * X(dzk)).v, P.rrho0 * rdzk).v : T(0));
+                        Gu = (X(zt) * X(vhat) + Cu - dK - dP - Au + Vu + tau).v;
                     }
                     if (mv) {
-                        const T uhat = T(0.25) * (uv_s.x + u_c + uv_se.x + uv_e.x);
+                        const T uhat = (quart * (X(uv_s.x) + X(u_c) + X(uv_se.x) + X(uv_e.x))).v;
                         const int ozv = 1 + (k >= mzt.z) + (k >= mzt.w);
                         const T z10 = s_zeta[bo + 1];
                         const T zt = ozv == 1 ? (uhat > T(0) ? z00 : z10)
                                               : weno_face(s_zeta[bo - 2], s_zeta[bo - 1], z00, z10, s_zeta[bo + 2], s_zeta[bo + 3], uhat, ozv);
-                        const T Cv = fFj * uhat;
+                        const Xv<T> Cv = X(fFj) * X(uhat);
                         const T2 kds = s_kd[qo - RX];
-                        const T dK = (kdc.x - kds.x) * rdy;
-                        const T dP = (T)(pc - s_p[bo - BX]) * rdy;
-                        const T dlo = (k >= 1 && k - 1 >= ty1) ? v_c - v_dn : T(0);
-                        const T dhi = (k + 1 <= nz - 1) ? uv_up.y - v_c : T(0);
-                        const T Av = T(0.5) * (T(0.5) * (AzCs * s_w1[qo - RX] + AzCj * w_c1) * dhi
-                                             + T(0.5) * (AzCs * s_w0[qo - RX] + AzCj * w_c0) * dlo) * rAzFj * rdzk;
-                        const T Vv = P.nu_h * ((kdc.y - kds.y) * rdy + (z10 - z00) * rdxFj);
-                        const T tau = (k == nz - 1) ? P.tauy[c] * P.rrho0 * rdzk : T(0);
-                        Gv = -zt * uhat - Cv - dK - dP - Av + Vv + tau;
+                        const Xv<T> dK = xdiv(X(kdc.x) - X(kds.x), dy, rdy);
+                        const Xv<T> dP = xdiv(X((T)(pc - s_p[bo - BX])), dy, rdy);
+                        const Xv<T> dlo((k >= 1 && k - 1 >= ty1) ? (X(v_c) - X(v_dn)).v : T(0));
+                        const Xv<T> dhi((k + 1 <= nz - 1) ? (X(uv_up.y) - X(v_c)).v : T(0));
+                        const Xv<T> Whi = half * (X(AzCs) * X(s_w1[qo - RX]) + X(AzCj) * X(w_c1));
+                        const Xv<T> Wlo = half * (X(AzCs) * X(s_w0[qo - RX]) + X(AzCj) * X(w_c0));
+                        const Xv<T> Av = xdiv(half * (Whi * dhi + Wlo * dlo), (X(AzFj) * X(dzk)).v, rAzFj * rdzk);
+                        const Xv<T> Vv = nuh * (xdiv(X(kdc.y) - X(kds.y), dy, rdy) + xdiv(X(z10) - X(z00), dxFj, rdxFj));
+                        const Xv<T> tau((k == nz - 1) ? xdiv(X(P.tauy[c]), (X(P.rho0) * X(dzk)).v, P.rrho0 * rdzk).v : T(0));
+                        Gv = (-X(zt) * X(uhat) - Cv - dK - dP - Av + Vv + tau).v;
                     }
                 }
                 // ---- quasi-AB2, predictor, elimination sweep (S3, S4, S5) ----
-                const T Ghu = c0 * Gu - c1 * gm_uv.x, Ghv = c0 * Gv - c1 * gm_uv.y;
+                const T Ghu = (X(c0) * X(Gu) - X(c1) * X(gm_uv.x)).v, Ghv = (X(c0) * X(Gv) - X(c1) * X(gm_uv.y)).v;
                 P.Guv[o] = mk2(Gu, Gv);
                 if (mu) {
                     const T us = E::add(u_c, E::mul(P.dt, Ghu));
-                    aGU += (double)dzk * (double)Ghu; aSU += (double)dzk * (double)us;
+                    aGU = (X(aGU) + X((double)dzk) * X((double)Ghu)).v; aSU = (X(aSU) + X((double)dzk) * X((double)us)).v;
                     const T smk = k > tx1 ? P.sm_m[k] : T(0);
                     dduv.x = E::div(E::add(us, E::mul(smk, dduv.x)), piv_u, piv_u);
                 }
                 if (mv) {
                     const T vs2 = E::add(v_c, E::mul(P.dt, Ghv));
-                    aGV += (double)dzk * (double)Ghv; aSV += (double)dzk * (double)vs2;
+                    aGV = (X(aGV) + X((double)dzk) * X((double)Ghv)).v; aSV = (X(aSV) + X((double)dzk) * X((double)vs2)).v;
                     const T smk = k > ty1 ? P.sm_m[k] : T(0);
                     dduv.y = E::div(E::add(vs2, E::mul(smk, dduv.y)), piv_v, piv_v);
                 }

@@ -194,7 +194,7 @@ ocn_status build_model(ocn_model* M) {
     P.dt = (T)M->d.dt; P.g = (T)M->d.g; P.alpha = (T)M->d.alpha; P.beta_s = (T)M->d.beta_s;
     P.Toff = sizeof(T) == 4 ? (T)M->d.T0 : T(0); P.Soff = sizeof(T) == 4 ? (T)M->d.S0 : T(0);
     P.dT0 = (T)(M->d.T0 - (double)P.Toff); P.dS0 = (T)(M->d.S0 - (double)P.Soff);
-    P.rrho0 = (T)(1.0 / M->d.rho0);
+    P.rho0 = (T)M->d.rho0; P.rrho0 = (T)(1.0 / M->d.rho0);
     P.g_d = M->d.g; P.alpha_d = M->d.alpha; P.beta_d = M->d.beta_s; P.hz_top_d = g->zf[nz] - g->zc[nz - 1];
     P.dT0_d = M->d.T0 - (double)P.Toff; P.dS0_d = M->d.S0 - (double)P.Soff;
     P.nu_h = (T)M->d.nu_h; P.kappa_h = (T)M->d.kappa_h; P.dtau = (T)M->dtau;
@@ -498,13 +498,13 @@ ocn_status ocn_model_create(const ocn_grid* g, const ocn_model_desc* d, ocn_mode
         for (int m = 0; m < Ms; ++m) M->a_w[m] = d->filter_weights[m];
     } else {
         double sum = 0;
-        for (int m = 1; m <= Ms; ++m) { const double s = (double)m / (Ms + 1); const double s2 = s * s; M->a_w[m - 1] = s2 * (1.0 - s2 * s2); sum += M->a_w[m - 1]; }
+        for (int m = 1; m <= Ms; ++m) { const double s = (double)m / (double)(Ms + 1); M->a_w[m - 1] = s * s * (1.0 - s * s * s * s); sum += M->a_w[m - 1]; }
         for (int m = 0; m < Ms; ++m) M->a_w[m] /= sum;
     }
     double first = 0;
     for (int m = 1; m <= Ms; ++m) first += m * M->a_w[m - 1];
     if (!(first > 0)) { delete M; return fail(OCN_EINVAL, "filter weights have no positive first moment"); }
-    M->dtau = d->dt / first;
+    M->dtau = d->dt * (1.0 / first);
     M->d.filter_weights = nullptr;
     if (d->stream) M->stream = static_cast<cudaStream_t>(d->stream);
     else {
