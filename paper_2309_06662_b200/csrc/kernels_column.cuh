@@ -134,7 +134,9 @@ __global__ void __launch_bounds__(1024) k_barotropic_tile(const DevP<T> P, const
                 if (x > 0) un = (mk & 2) ? (X(un) + X(dtau) * (xdiv(-X(g) * X(sHu[q]) * (X(ec) - X(se[q - 1])), dxc[y], rdx[y]) + X(sGU[q]))).v : T(0);
                 if (y > 0) vn = (mk & 4) ? (X(vn) + X(dtau) * (xdiv(-X(g) * X(sHv[q]) * (X(ec) - X(se[q - EX])), dy, rdy) + X(sGV[q]))).v : T(0);
                 sU[q] = un; sV[q] = vn;
-                be[n] = (X(be[n]) + X(am) * X(ec)).v; bU[n] = (X(bU[n]) + X(am) * X(un)).v; bV[n] = (X(bV[n]) + X(am) * X(vn)).v;
+                if (cidx[n] >= 0) {
+                    be[n] = (X(be[n]) + X(am) * X(ec)).v; bU[n] = (X(bU[n]) + X(am) * X(un)).v; bV[n] = (X(bV[n]) + X(am) * X(vn)).v;
+                }
             }
         }
         __syncthreads();
