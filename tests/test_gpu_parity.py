@@ -243,11 +243,11 @@ def test_deep_column_count_nz_200_fp64():
 def test_runs_are_bitwise_reproducible():
     """Two runs of the same model give identical bits (no data race, no order-dependent atomics); a race between
     the filter accumulation and the next barotropic sub-step was found this way on the full config 3."""
-    wl = W.config3(nx=720, ny=300, nz=20, steps=6)
+    wl = W.config3()                                     # full size: the race only showed there
     res = []
     for _ in range(2):
         gpu = ocn.Model(wl)
-        gpu.time_step(6)
+        gpu.time_step(5)
         res.append(gpu.get_fields())
         gpu.close()
     for n in FIELDS:
