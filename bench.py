@@ -170,6 +170,15 @@ def measured_peak():
         return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def ncu_entry(workload, kernel):
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            e = json.load(f).get(kernel)
+        return e if e and e.get("workload") == workload else None
+    except Exception:
+        return None
+
+
 def ncu_traffic(workload, kernel):
     """DRAM bytes per launch of `kernel` from the committed ncu --set full capture, if it was taken
     on this workload (profiles/traffic.json, written by hand from the capture's raw page)."""
@@ -284,6 +293,18 @@ def run_ours(args):
         roof = {"kernel": dom, "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes, "traffic": None}
 
+    # K1 is issue bound rather than HBM bound: second view against the fp32 lane-op ceiling
+    # 148 SMs x 128 lanes x SM clock, with the executed thread instructions of the committed ncu capture
+    roof_alu = None
+    ent = ncu_entry(workload_name(wl), dom)
+    if ent and "thread_instructions_per_launch" in ent:
+        mhz = clk.get("sm_mhz") or 1965.0
+        peak_ops = 148 * 128 * mhz * 1e6
+        ach_ops = ent["thread_instructions_per_launch"] / (stages[dom]["ms"] / K * 1e-3)
+        roof_alu = {"kernel": dom, "bound": "alu", "achieved": ach_ops / 1e12, "peak": peak_ops / 1e12,
+                    "unit": "T thread-instr/s", "frac": ach_ops / peak_ops,
+                    "peak_source": "148 SMs x 128 fp32 lanes x sampled SM clock; instructions from profiles/traffic.json (ncu)"}
+
     # ---- end to end through the C ABI with HOST (pinned) buffers ----
     e2e = None
     if not args.no_e2e:
@@ -336,7 +357,7 @@ def run_ours(args):
                            "parallelism": "replicas x%d" % world},
                 "sypd_equivalent": sypd(prm["dt"], sec_per_step),
                 "wet_cell_updates_per_s": world * nwet * K / (ms_total * 1e-3),
-                "stages": stage_out, "roofline": roof, "e2e": e2e, "cpu_baseline": cpu,
+                "stages": stage_out, "roofline": roof, "roofline_alu": roof_alu, "e2e": e2e, "cpu_baseline": cpu,
                 "gpu_launches": info["launches_per_step"] * K, "clocks": clk,
                 "device_bytes": info["device_bytes"]}
         print(json.dumps(line))
