@@ -30,6 +30,9 @@ __device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
 __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive_plain(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     const uint32_t a = smem_u32(bar);
     uint32_t ok;
@@ -45,8 +48,13 @@ __device__ __forceinline__ void tma_load_plane(void* dst, const CUtensorMap* map
 
 __host__ __device__ constexpr int rup128(int b) { return (b + 127) / 128 * 128; }
 
-template <class T, int TX_, int TY_>
+// MODE 0: all four prognostic fields in one kernel; 1: the momentum group (u, v) only; 2: the tracer group (T, S) only.
+// The two group kernels read the same state, write disjoint outputs and run concurrently (ocn_api.cu); each has a
+// smaller register / shared-memory footprint than the fused one, so more CTAs are resident per SM.
+template <class T, int TX_, int TY_, int MODE_ = 0>
 struct Tile {
+    static constexpr int MODE = MODE_;
+    static constexpr bool DO_T = MODE_ != 1, DO_M = MODE_ != 2;
     typedef typename Pair<T>::type T2;
     static constexpr int TX = TX_, TY = TY_, NC = TX * TY, NT = NC;   // cells = threads; a thread owns the tracers of one cell and the momentum of another
     static constexpr int BX = TX + 8, BY = TY + 6;       // TMA box: origin (i0 - 4, j0 - 3)
@@ -59,33 +67,34 @@ struct Tile {
     static constexpr int BYTES2 = BX * BY * (int)sizeof(T2), BYTESP = BX * BY * 8;
     // shared-memory map (byte offsets from a 128-byte aligned base)
     static constexpr int O_TS = 0;
-    static constexpr int O_UV = O_TS + R_TS * PL2;
+    static constexpr int O_UV = O_TS + (DO_T ? R_TS : 0) * PL2;
     static constexpr int O_P = O_UV + R_UV * PL2;
-    static constexpr int O_ZETA = O_P + R_P * PLP;
-    static constexpr int O_KD = O_ZETA + 2 * PL1;                               // 2 x T2 (K, D) on RX x RY
+    static constexpr int O_ZETA = O_P + (DO_M ? R_P : 0) * PLP;
+    static constexpr int O_KD = O_ZETA + (DO_M ? 2 : 0) * PL1;                               // 2 x T2 (K, D) on RX x RY
     static constexpr int KDB = rup128(RX * RY * (int)sizeof(T2)), WB = rup128(RX * RY * (int)sizeof(T));
     static constexpr int O_W = O_KD + 2 * KDB;                                  // 3 buffers of T on RX x RY
     static constexpr int NFX = RX * TY, NFY = TX * RY, NF = NFX + NFY;        // west faces, then south faces
     static constexpr int FLB = rup128(NF * (int)sizeof(T2));
     static constexpr int O_FLUX = O_W + 3 * WB;                                 // 2 x T2 per face
-    static constexpr int O_M8 = O_FLUX + 2 * FLB;                               // uint2 on RX x RY (not zero-filled from here on)
+    static constexpr int O_M8 = O_FLUX + (DO_T ? 2 : 0) * FLB;                               // uint2 on RX x RY (not zero-filled from here on)
     static constexpr int O_MET = O_M8 + rup128(RX * RY * 8);                    // 9 row-metric arrays of BY + 1
     static constexpr int O_CELL = O_MET + rup128(9 * (BY + 1) * (int)sizeof(T)); // uint16: cells sorted by first wet level
     static constexpr int O_FS = O_CELL + rup128(NC * 2);                        // uint2: face descriptors sorted by first open level
-    static constexpr int O_NC = O_FS + rup128(NF * 8);                          // uint16[256]: active cells at level k
+    static constexpr int O_NC = O_FS + (DO_T ? rup128(NF * 8) : 0);                          // uint16[256]: active cells at level k
     static constexpr int O_NF = O_NC + 512;                                     // uint16[256]: active faces at level k
     static constexpr int O_BAR = O_NF + 512;
     static constexpr int SMEM = O_BAR + 128 + 128;                              // + alignment slack
 };
 
 
-template <class T, int TX, int TY>
-__global__ void __launch_bounds__(TX * TY, (sizeof(T) == 4 ? 2 : 1))
+template <class T, int TX, int TY, int MODE, int MINB>
+__global__ void __launch_bounds__(TX * TY, MINB)
 k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__ CUtensorMap m_ts,
                 const __grid_constant__ CUtensorMap m_uv, const __grid_constant__ CUtensorMap m_p) {
-    typedef Tile<T, TX, TY> C;
+    typedef Tile<T, TX, TY, MODE> C;
     typedef typename C::T2 T2;
     typedef Ex<T> E;
+    constexpr bool DO_T = C::DO_T, DO_M = C::DO_M;
     constexpr int BX = C::BX, BY = C::BY, RX = C::RX, RY = C::RY, NT = C::NT, NC = C::NC, OX = C::OX, OY = C::OY;
     extern __shared__ __align__(1024) unsigned char sm[];     // dynamic only: starts the CTA's window, 1 KB aligned
     unsigned short* const s_cell = (unsigned short*)(sm + C::O_CELL);
@@ -143,10 +152,10 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     // first open level (stable counting sort on the 8-bit level), so that at level k the active work
     // is a dense prefix of each list and keeps the geometric order (coalescing) within a level ------
     {
-        constexpr int MAXR = (C::NF + NT - 1) / NT;                      // rounds of NT items
+        constexpr int MAXR = DO_T ? (C::NF + NT - 1) / NT : 1;           // rounds of NT items
         unsigned short* const cnt = (unsigned short*)sm;                  // [virtual warp][key], scratch in the unused ts ring
         int* const base = (int*)(sm + MAXR * (NT / 32) * 256 * 2);        // [key] exclusive prefix, then [256 + w] warp sums
-        static_assert(MAXR * (NT / 32) * 512 + 2048 <= C::R_TS * C::PL2, "sort scratch");
+        static_assert(MAXR * (NT / 32) * 512 + 2048 <= C::O_M8, "sort scratch");
         const int lane = tid & 31, wrp = tid >> 5;
         // sorts items 0 .. n-1 by keyf(q) in [0, 255]; emit(q, rank); nle[k] = number of items with key <= k
         auto csort = [&](const int n, auto keyf, auto emit, unsigned short* nle) {
@@ -202,22 +211,24 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
               [&](int q) { const int gx = q % TX, gy = q / TX;
                            return (i0 + gx < P.nx && j0 + gy < P.ny) ? (int)(s_m8[gy * RX + gx].x & 255u) : nz; },
               [&](int q, int rank) { s_cell[rank] = (unsigned short)q; }, s_nc);
-        // faces: fid < NFX = west face of cell (fid % RX, fid / RX); else south face of cell (g % TX, g / TX), g = fid - NFX
-        auto face_cell = [&](int fid, bool& isy, int& fx, int& fy) {
-            isy = fid >= C::NFX;
-            const int g = isy ? fid - C::NFX : fid;
-            fx = isy ? g % TX : g % RX; fy = isy ? g / TX : g / RX;
-        };
-        csort(C::NF,
-              [&](int q) { bool isy; int fx, fy; face_cell(q, isy, fx, fy);
-                           const uint2 m = s_m8[fy * RX + fx];
-                           return (int)(isy ? (m.y & 255u) : ((m.x >> 8) & 255u)); },
-              [&](int fid, int rank) { bool isy; int fx, fy; face_cell(fid, isy, fx, fy);
-                           const uint2 m = s_m8[fy * RX + fx];
-                           const uint32_t thr = isy ? (m.y & 0xffffffu) : (m.x >> 8);
-                           const uint32_t bb = (uint32_t)((fy + OY) * BX + fx + OX);
-                           s_fs[rank] = make_uint2(bb | ((uint32_t)(fy + OY) << 10) | ((isy ? 1u : 0u) << 14) | ((uint32_t)fid << 16), thr); },
-              s_nf);
+        if constexpr (DO_T) {
+            // faces: fid < NFX = west face of cell (fid % RX, fid / RX); else south face of cell (g % TX, g / TX), g = fid - NFX
+            auto face_cell = [&](int fid, bool& isy, int& fx, int& fy) {
+                isy = fid >= C::NFX;
+                const int g = isy ? fid - C::NFX : fid;
+                fx = isy ? g % TX : g % RX; fy = isy ? g / TX : g / RX;
+            };
+            csort(C::NF,
+                  [&](int q) { bool isy; int fx, fy; face_cell(q, isy, fx, fy);
+                               const uint2 m = s_m8[fy * RX + fx];
+                               return (int)(isy ? (m.y & 255u) : ((m.x >> 8) & 255u)); },
+                  [&](int fid, int rank) { bool isy; int fx, fy; face_cell(fid, isy, fx, fy);
+                               const uint2 m = s_m8[fy * RX + fx];
+                               const uint32_t thr = isy ? (m.y & 0xffffffu) : (m.x >> 8);
+                               const uint32_t bb = (uint32_t)((fy + OY) * BX + fx + OX);
+                               s_fs[rank] = make_uint2(bb | ((uint32_t)(fy + OY) << 10) | ((isy ? 1u : 0u) << 14) | ((uint32_t)fid << 16), thr); },
+                  s_nf);
+        }
     }
 
     // ---- one-time shared-memory setup --------------------------------------------------------
@@ -244,14 +255,15 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     auto issue_group = [&](int m, bool first) {
         uint64_t* bar = &bars[(m - kmin) % C::NB];
         uint32_t bytes = 0;
-        const int tlo = first ? max(m - 3, 0) : m + 2, thi = min(m + 2, nz - 1);
+        const int tlo = first ? max(m - 3, 0) : m + 2, thi = DO_T ? min(m + 2, nz - 1) : -1;
         if (thi >= tlo) bytes += (uint32_t)(thi - tlo + 1) * C::BYTES2;
         if (m < nz) bytes += C::BYTES2;
-        if (m - 1 >= kmin) bytes += C::BYTESP;
+        if (DO_M && m - 1 >= kmin) bytes += C::BYTESP;
+        if (bytes == 0) { mbar_arrive_plain(bar); return; }          // nothing to load for this iteration (tracer mode, m = nz)
         mbar_expect_tx(bar, bytes);
         for (int q = tlo; q <= thi; ++q) tma_load_plane(sm + C::O_TS + (q % C::R_TS) * C::PL2, &m_ts, bar, 2 * i0, j0, q);
         if (m < nz) tma_load_plane(sm + C::O_UV + (m % C::R_UV) * C::PL2, &m_uv, bar, 2 * i0, j0, m);
-        if (m - 1 >= kmin) tma_load_plane(sm + C::O_P + ((m - 1) % C::R_P) * C::PLP, &m_p, bar, i0, j0, m - 1);
+        if (DO_M && m - 1 >= kmin) tma_load_plane(sm + C::O_P + ((m - 1) % C::R_P) * C::PLP, &m_p, bar, i0, j0, m - 1);
     };
     if (tid == 0) {
         issue_group(kmin, true);
@@ -290,7 +302,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
 
     for (int m = kmin; m <= nz; ++m) {
         const int kB = m - 1;                                 // level of part B (phase 3) in this iteration
-        const bool doB = kB >= kmin, wetT = doB && kB >= cT.kb, wetM = doB && kB >= cM.kb;
+        const bool doB = kB >= kmin, wetT = DO_T && doB && kB >= cT.kb, wetM = DO_M && doB && kB >= cM.kb;
         const long long oT = (long long)kB * sz + cT.c, oM = (long long)kB * sz + cM.c;
         // AB2 history and pivots of level kB: issued now, consumed after part A
         T2 gm_uv = mk2(T(0), T(0)), gm_ts = mk2(T(0), T(0));
@@ -316,14 +328,16 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             T* __restrict__ s_w1 = (T*)(sm + C::O_W + ((k + 1) % 3) * C::WB);
             T2* __restrict__ s_flux = (T2*)(sm + C::O_FLUX + (k & 1) * C::FLB);
             // ================= phase 1: zeta, K, D, w[k+1] =================
-    #pragma unroll
-            for (int h = 0; h < (BX - 1) * (BY - 1); h += NT) {
-                const int q = h + (NT - 1 - tid);
-                if (q < (BX - 1) * (BY - 1)) {
-                    const int px = 1 + q % (BX - 1), py = 1 + q / (BX - 1);
-                    const T2 a = s_uv[py * BX + px], as = s_uv[(py - 1) * BX + px], aw = s_uv[py * BX + px - 1];
-                    s_zeta[py * BX + px] = xdiv(X(dy) * (X(a.y) - X(aw.y)) - (X(s_dxC[py]) * X(a.x) - X(s_dxC[py - 1]) * X(as.x)),
-                                                s_AzF[py], s_rAzF[py]).v;
+            if constexpr (DO_M) {
+        #pragma unroll
+                for (int h = 0; h < (BX - 1) * (BY - 1); h += NT) {
+                    const int q = h + (NT - 1 - tid);
+                    if (q < (BX - 1) * (BY - 1)) {
+                        const int px = 1 + q % (BX - 1), py = 1 + q / (BX - 1);
+                        const T2 a = s_uv[py * BX + px], as = s_uv[(py - 1) * BX + px], aw = s_uv[py * BX + px - 1];
+                        s_zeta[py * BX + px] = xdiv(X(dy) * (X(a.y) - X(aw.y)) - (X(s_dxC[py]) * X(a.x) - X(s_dxC[py - 1]) * X(as.x)),
+                                                    s_AzF[py], s_rAzF[py]).v;
+                    }
                 }
             }
     #pragma unroll
@@ -342,7 +356,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 }
             }
             // ================= phase 2: tracer face fluxes, each open face once =================
-            {
+            if constexpr (DO_T) {
                 const T2* __restrict__ s_ts = (const T2*)(sm + C::O_TS + (k % C::R_TS) * C::PL2);
                 const int nface = s_nf[k];
                 for (int f = NT - 1 - tid; f < nface; f += NT) {
@@ -378,7 +392,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             const T2* __restrict__ s_flux = (const T2*)(sm + C::O_FLUX + (k & 1) * C::FLB);
             // ---------- tracer half: the cell of rank tid ----------
             T2 fz_top = mk2(T(0), T(0));
-            if (wetT) {
+            if constexpr (DO_T) if (wetT) {
                 const int cx = cT.cx, cy = cT.cy, kb = cT.kb, bo = cT.bo, by = cT.by;
                 const long long o = oT;
                 const T AzCj = s_AzC[by], rAzCj = s_rAzC[by];
@@ -419,7 +433,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 P.dts[o] = ddts;
             }
             // ---------- momentum half: the cell of rank NC - 1 - tid ----------
-            if (wetM) {
+            if constexpr (DO_M) if (wetM) {
                 const int cx = cM.cx, cy = cM.cy, tx1 = cM.tx1, ty1 = cM.ty1, bo = cM.bo, by = cM.by;
                 const long long o = oM, c = cM.c;
                 const uchar4 mzt = cM.mzt;
@@ -505,6 +519,6 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
         __syncthreads();                       // planes of level m - 1 are dead: refill the ring
         if (tid == 0 && m + C::DP <= nz) issue_group(m + C::DP, false);
     }
-    if (cM.incol && cM.kb < nz) { P.GU[cM.c] = (T)aGU; P.GV[cM.c] = (T)aGV; P.SU[cM.c] = (T)aSU; P.SV[cM.c] = (T)aSV; }
+    if (DO_M && cM.incol && cM.kb < nz) { P.GU[cM.c] = (T)aGU; P.GV[cM.c] = (T)aGV; P.SU[cM.c] = (T)aSU; P.SV[cM.c] = (T)aSV; }
 }
 }  // namespace ocn

@@ -5,6 +5,7 @@
 
 #include <algorithm>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -46,6 +47,9 @@ struct ocn_model {
     void* stage = nullptr;              // contiguous staging buffer, (nz+1)*ny*nx doubles
     cudaGraphExec_t graph = nullptr;    // one steady-state (AB2) step
     CUtensorMap tm_ts{}, tm_uv{}, tm_p{};   // TMA descriptors of the halo'd (T,S), (u,v) and p arrays
+    bool split_k1 = false;              // K1 as two concurrent prognostic-group kernels (OCN_K1_SPLIT=1) or fused
+    cudaStream_t stream2 = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     int launches_per_step = 0;
     // per-stage timing (ocn_profile_*)
     bool profiling = false;
@@ -114,6 +118,13 @@ ocn_status make_tmap(CUtensorMap* tm, bool f64, void* base, unsigned long long i
     if (r != CUDA_SUCCESS) return fail(OCN_ECUDA, "cuTensorMapEncodeTiled failed (code " + std::to_string((int)r) + ")");
     return OCN_OK;
 }
+
+// K1 variants: fused (all four fields), or the two prognostic-group kernels that run concurrently.  MINB = CTAs per SM
+// the register allocation is bounded for.
+template <class T> using k1_fn = void (*)(const ocn::DevP<T>, const T, const T, const CUtensorMap, const CUtensorMap, const CUtensorMap);
+template <class T> k1_fn<T> k1_fused() { return ocn::k_tendency_tile<T, TILE_X, TILE_Y, 0, (sizeof(T) == 4 ? 2 : 1)>; }
+template <class T> k1_fn<T> k1_momentum() { return ocn::k_tendency_tile<T, TILE_X, TILE_Y, 1, (sizeof(T) == 4 ? 3 : 1)>; }
+template <class T> k1_fn<T> k1_tracers() { return ocn::k_tendency_tile<T, TILE_X, TILE_Y, 2, (sizeof(T) == 4 ? 3 : 1)>; }
 
 dim3 grid2(const ocn_grid* g, dim3 b, int z = 1) { return dim3((g->nx + b.x - 1) / b.x, (g->ny + b.y - 1) / b.y, z); }
 
@@ -222,14 +233,16 @@ ocn_status build_model(ocn_model* M) {
     M->launches_per_step = (M->d.substeps + BT_HALO - 1) / BT_HALO + 3;
     // TMA descriptors: box origin (i0 - 4, j0 - 3), so the map starts 4 elements before (row -3, i = 0)
     {
-        typedef ocn::Tile<T, TILE_X, TILE_Y> C;
+        typedef ocn::Tile<T, TILE_X, TILE_Y, 0> C;
         const bool f64 = sizeof(T) == 8;
         const unsigned long long sxu = (unsigned long long)g->sx, syu = (unsigned long long)g->sy;
         if ((s = make_tmap(&M->tm_ts, f64, (T*)P.ts - 2 * C::OX, 2 * sxu, syu, nz, 2 * C::BX, C::BY)) != OCN_OK ||
             (s = make_tmap(&M->tm_uv, f64, (T*)P.uv - 2 * C::OX, 2 * sxu, syu, nz, 2 * C::BX, C::BY)) != OCN_OK ||
             (s = make_tmap(&M->tm_p, true, P.p - C::OX, sxu, syu, nz, C::BX, C::BY)) != OCN_OK)
             return s;
-        CK(cudaFuncSetAttribute(ocn::k_tendency_tile<T, TILE_X, TILE_Y>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
+        CK(cudaFuncSetAttribute(k1_fused<T>(), cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
+        CK(cudaFuncSetAttribute(k1_momentum<T>(), cudaFuncAttributeMaxDynamicSharedMemorySize, (ocn::Tile<T, TILE_X, TILE_Y, 1>::SMEM)));
+        CK(cudaFuncSetAttribute(k1_tracers<T>(), cudaFuncAttributeMaxDynamicSharedMemorySize, (ocn::Tile<T, TILE_X, TILE_Y, 2>::SMEM)));
         CK(cudaFuncSetAttribute(ocn::k_barotropic_tile<T, BT_X, BT_Y>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 ocn::BtTile<T, BT_X, BT_Y>::SMEM));
     }
@@ -282,9 +295,17 @@ ocn_status launch_step(ocn_model* M, bool euler) {
     const dim3 bc(32, 4), b2(32, 8);
     MARK(-1, 0);
     {
-        typedef ocn::Tile<T, TILE_X, TILE_Y> C;
-        const dim3 bt(TILE_X, TILE_Y);
-        ocn::k_tendency_tile<T, TILE_X, TILE_Y><<<grid2(g, dim3(TILE_X, TILE_Y)), bt, C::SMEM, M->stream>>>(P, c0, c1, M->tm_ts, M->tm_uv, M->tm_p);
+        const dim3 bt(TILE_X, TILE_Y), gt = grid2(g, bt);
+        if (!M->split_k1) {
+            k1_fused<T>()<<<gt, bt, ocn::Tile<T, TILE_X, TILE_Y, 0>::SMEM, M->stream>>>(P, c0, c1, M->tm_ts, M->tm_uv, M->tm_p);
+        } else {                                   // the two group kernels side by side (fork / join on a second stream)
+            CK(cudaEventRecord(M->ev_fork, M->stream));
+            CK(cudaStreamWaitEvent(M->stream2, M->ev_fork, 0));
+            k1_momentum<T>()<<<gt, bt, ocn::Tile<T, TILE_X, TILE_Y, 1>::SMEM, M->stream2>>>(P, c0, c1, M->tm_ts, M->tm_uv, M->tm_p);
+            CK(cudaEventRecord(M->ev_join, M->stream2));
+            k1_tracers<T>()<<<gt, bt, ocn::Tile<T, TILE_X, TILE_Y, 2>::SMEM, M->stream>>>(P, c0, c1, M->tm_ts, M->tm_uv, M->tm_p);
+            CK(cudaStreamWaitEvent(M->stream, M->ev_join, 0));
+        }
     }
     MARK(0, 1);
     {
@@ -512,6 +533,16 @@ ocn_status ocn_model_create(const ocn_grid* g, const ocn_model_desc* d, ocn_mode
         if (e != cudaSuccess) { delete M; return fail(OCN_ECUDA, cudaGetErrorString(e)); }
         M->own_stream = true;
     }
+    {
+        const char* e = getenv("OCN_K1_SPLIT");
+        M->split_k1 = e && e[0] == '1';
+        if (cudaStreamCreateWithFlags(&M->stream2, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&M->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&M->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+            ocn_model_destroy(M);
+            return fail(OCN_ECUDA, "stream / event creation failed");
+        }
+    }
     const ocn_status s = d->precision == 32 ? build_model<float>(M) : build_model<double>(M);
     if (s != OCN_OK) { const std::string keep = g_err; ocn_model_destroy(M); g_err = keep; return s; }
     *out = M;
@@ -524,6 +555,9 @@ ocn_status ocn_model_destroy(ocn_model* M) {
     if (M->stream) cudaStreamSynchronize(M->stream);
     if (M->graph) cudaGraphExecDestroy(M->graph);
     for (cudaEvent_t e : M->ev_pool) cudaEventDestroy(e);
+    if (M->ev_fork) cudaEventDestroy(M->ev_fork);
+    if (M->ev_join) cudaEventDestroy(M->ev_join);
+    if (M->stream2) cudaStreamDestroy(M->stream2);
     for (void* p : M->allocs) cudaFree(p);
     if (M->stage) cudaFree(M->stage);
     if (M->own_stream && M->stream) cudaStreamDestroy(M->stream);
