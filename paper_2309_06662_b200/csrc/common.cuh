@@ -169,6 +169,9 @@ __device__ __forceinline__ double weno_face_exact(double a, double b, double c, 
 __device__ __forceinline__ double weno_face(double a, double b, double c, double d, double e, double f, double vel, int order) {
     return weno_face_exact(a, b, c, d, e, f, vel, order);
 }
+// quotient of the weighted sum: reciprocal-based in fp32 (2 ulp), exact in fp64
+__device__ __forceinline__ float fquot(float a, float b) { return __fdividef(a, b); }
+__device__ __forceinline__ double fquot(double a, double b) { return a / b; }
 template <class T>
 __device__ __forceinline__ T weno_face(T a, T b, T c, T d, T e, T f, T vel, int order) {
     const bool pos = vel > T(0);
@@ -186,13 +189,13 @@ __device__ __forceinline__ T weno_face(T a, T b, T c, T d, T e, T f, T vel, int 
         const T b2 = eps + T(13.0 / 12.0) * s2 * s2 + T(0.25) * t2 * t2;
         const T b01 = b0 * b1, b02 = b0 * b2, b12 = b1 * b2;
         const T a0 = T(0.1) * b12 * b12, a1 = T(0.6) * b02 * b02, a2 = T(0.3) * b01 * b01;
-        return (a0 * p0 + a1 * p1 + a2 * p2) / (a0 + a1 + a2);
+        return fquot(a0 * p0 + a1 * p1 + a2 * p2, a0 + a1 + a2);
     }
     if (order == 2) {
         const T p0 = T(0.5) * (T(3) * q0 - qm1), p1 = T(0.5) * (q0 + q1);
         const T b0 = eps + (q0 - qm1) * (q0 - qm1), b1 = eps + (q1 - q0) * (q1 - q0);
         const T a0 = T(1.0 / 3.0) * b1 * b1, a1 = T(2.0 / 3.0) * b0 * b0;
-        return (a0 * p0 + a1 * p1) / (a0 + a1);
+        return fquot(a0 * p0 + a1 * p1, a0 + a1);
     }
     return order == 1 ? q0 : T(0);
 }

@@ -300,7 +300,10 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     T2 dduv = mk2(T(0), T(0)), ddts = mk2(T(0), T(0));   // eliminated right-hand sides of the level below
     double aGU = 0, aGV = 0, aSU = 0, aSV = 0;
 
-    for (int m = kmin; m <= nz; ++m) {
+    // ring slots of level m, carried along the march (no integer division in the loop)
+    auto wrap = [](int x, int r) { return x >= r ? x - r : x; };
+    int rts = kmin % C::R_TS, ruv = kmin % C::R_UV, rp = kmin % C::R_P, r3 = kmin % 3;
+    for (int m = kmin; m <= nz; ++m, rts = wrap(rts + 1, C::R_TS), ruv = wrap(ruv + 1, C::R_UV), rp = wrap(rp + 1, C::R_P), r3 = wrap(r3 + 1, 3)) {
         const int kB = m - 1;                                 // level of part B (phase 3) in this iteration
         const bool doB = kB >= kmin, wetT = DO_T && doB && kB >= cT.kb, wetM = DO_M && doB && kB >= cM.kb;
         const long long oT = (long long)kB * sz + cT.c, oM = (long long)kB * sz + cM.c;
@@ -322,10 +325,10 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
         if (m < nz) {                                         // ---------------- part A: level k = m ----------------
             const int k = m;
             const T dzk = P.dz[k];
-            const T2* __restrict__ s_uv = (const T2*)(sm + C::O_UV + (k % C::R_UV) * C::PL2);
+            const T2* __restrict__ s_uv = (const T2*)(sm + C::O_UV + ruv * C::PL2);
             T* __restrict__ s_zeta = (T*)(sm + C::O_ZETA + (k & 1) * C::PL1);
             T2* __restrict__ s_kd = (T2*)(sm + C::O_KD + (k & 1) * C::KDB);
-            T* __restrict__ s_w1 = (T*)(sm + C::O_W + ((k + 1) % 3) * C::WB);
+            T* __restrict__ s_w1 = (T*)(sm + C::O_W + wrap(r3 + 1, 3) * C::WB);
             T2* __restrict__ s_flux = (T2*)(sm + C::O_FLUX + (k & 1) * C::FLB);
             // ================= phase 1: zeta, K, D, w[k+1] =================
             if constexpr (DO_M) {
@@ -357,7 +360,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             }
             // ================= phase 2: tracer face fluxes, each open face once =================
             if constexpr (DO_T) {
-                const T2* __restrict__ s_ts = (const T2*)(sm + C::O_TS + (k % C::R_TS) * C::PL2);
+                const T2* __restrict__ s_ts = (const T2*)(sm + C::O_TS + rts * C::PL2);
                 const int nface = s_nf[k];
                 for (int f = NT - 1 - tid; f < nface; f += NT) {
                     const uint2 d = s_fs[f];
@@ -382,11 +385,11 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
         if (doB) {                                            // ---------------- part B: level k = m - 1 ----------------
             const int k = kB;
             const T dzk = P.dz[k], rdzk = P.rdz[k];
-            const T2* __restrict__ s_uv = (const T2*)(sm + C::O_UV + (k % C::R_UV) * C::PL2);
-            const T2* __restrict__ s_uv1 = (const T2*)(sm + C::O_UV + ((k + 1) % C::R_UV) * C::PL2);
-            const double* __restrict__ s_p = (const double*)(sm + C::O_P + (k % C::R_P) * C::PLP);
-            const T* __restrict__ s_w0 = (const T*)(sm + C::O_W + (k % 3) * C::WB);
-            const T* __restrict__ s_w1 = (const T*)(sm + C::O_W + ((k + 1) % 3) * C::WB);
+            const T2* __restrict__ s_uv = (const T2*)(sm + C::O_UV + wrap(ruv + C::R_UV - 1, C::R_UV) * C::PL2);
+            const T2* __restrict__ s_uv1 = (const T2*)(sm + C::O_UV + ruv * C::PL2);
+            const double* __restrict__ s_p = (const double*)(sm + C::O_P + wrap(rp + C::R_P - 1, C::R_P) * C::PLP);
+            const T* __restrict__ s_w0 = (const T*)(sm + C::O_W + wrap(r3 + 2, 3) * C::WB);
+            const T* __restrict__ s_w1 = (const T*)(sm + C::O_W + r3 * C::WB);
             const T* __restrict__ s_zeta = (const T*)(sm + C::O_ZETA + (k & 1) * C::PL1);
             const T2* __restrict__ s_kd = (const T2*)(sm + C::O_KD + (k & 1) * C::KDB);
             const T2* __restrict__ s_flux = (const T2*)(sm + C::O_FLUX + (k & 1) * C::FLB);
@@ -401,8 +404,11 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 {
                 const int ozt = (k + 1 < nz) ? min(3, min(k + 1 - kb, nz - k - 1)) : 0;
                 if (ozt > 0) {
-                    auto tsz = [&](int kk) -> T2 { return ((const T2*)(sm + C::O_TS + ((kk + C::R_TS) % C::R_TS) * C::PL2))[bo]; };
-                    const T2 fv = weno_face2(tsz(k - 2), tsz(k - 1), tsz(k), tsz(k + 1), tsz(k + 2), tsz(k + 3), w_c1, ozt);
+                    const int rlo = wrap(rts + C::R_TS - 3, C::R_TS);      // slot of level k - 2 = m - 3
+                    auto tsz = [&](int dk) -> T2 {           // plane of level k + dk, dk = -2 .. 3
+                        return ((const T2*)(sm + C::O_TS + wrap(rlo + dk + 2, C::R_TS) * C::PL2))[bo];
+                    };
+                    const T2 fv = weno_face2(tsz(-2), tsz(-1), tsz(0), tsz(1), tsz(2), tsz(3), w_c1, ozt);
                     fz_top.x = (X(w_c1) * X(AzCj) * X(fv.x)).v;
                     fz_top.y = (X(w_c1) * X(AzCj) * X(fv.y)).v;
                 }
@@ -410,7 +416,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 // ---- tracers ----
                 const T2 fw = s_flux[cy * RX + cx], fe = s_flux[cy * RX + cx + 1];
                 const T2 fs = s_flux[C::NFX + cy * TX + cx], fn = s_flux[C::NFX + (cy + 1) * TX + cx];
-                const T2 tsc = ((const T2*)(sm + C::O_TS + (k % C::R_TS) * C::PL2))[bo];
+                const T2 tsc = ((const T2*)(sm + C::O_TS + wrap(rts + C::R_TS - 1, C::R_TS) * C::PL2))[bo];
                 const T vol = (X(AzCj) * X(dzk)).v, rvol = rAzCj * rdzk;
                 T GT, GS;
                 if constexpr (sizeof(T) == 8) {    // the flux divergence summed in the order of DESIGN.md §3.7
