@@ -265,3 +265,57 @@ def test_fp64_is_bit_identical_to_the_oracle():
         for n in FIELDS:
             assert np.array_equal(a[n], b[n]), (wl["name"], n, rel_linf(a[n], b[n]))
         gpu.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# the rest of the boundary: device buffers, caller's stream, per-step forcing, errors, profiling
+# ---------------------------------------------------------------------------------------------
+def test_device_buffers_and_callers_stream_match_host_path():
+    import torch
+    wl = W.config3(nx=96, ny=40, nz=12, steps=3)
+    host = ocn.Model(wl)
+    host.time_step(3)
+    ref = host.get_fields()
+    host.close()
+    stream = torch.cuda.Stream()
+    dev = ocn.Model(wl, stream=stream.cuda_stream, set_fields=False)
+    keep = {k: torch.from_numpy(np.ascontiguousarray(v, dtype=np.float32)).cuda() for k, v in wl["fields"].items()}
+    torch.cuda.synchronize()
+    dev.set_fields_ptr(on_device=True, **{k: t.data_ptr() for k, t in keep.items()})
+    dev.time_step(3)
+    nz, ny, nx = dev.nz, dev.ny, dev.nx
+    out = {k: torch.empty((nz + 1 if k == "w" else nz, ny, nx) if k != "eta" else (ny, nx), dtype=torch.float32, device="cuda")
+           for k in FIELDS}
+    dev.get_fields_ptr(on_device=True, **{k: t.data_ptr() for k, t in out.items()})     # synchronises the stream
+    for n in FIELDS:
+        assert np.array_equal(out[n].cpu().numpy(), ref[n]), n
+    dev.close()
+
+
+def test_profiling_path_gives_the_same_bits_and_sane_times():
+    wl = W.config3(nx=96, ny=40, nz=12, steps=4)
+    a = ocn.Model(wl); a.time_step(4); fa = a.get_fields(); a.close()
+    b = ocn.Model(wl); b.profile_enable(True); b.time_step(4)
+    prof = b.profile_read()
+    fb = b.get_fields(); b.close()
+    for n in FIELDS:
+        assert np.array_equal(fa[n], fb[n]), n                    # graph replay and direct launches agree bit for bit
+    assert set(prof) == {"tendency", "barotropic", "backsub_correct_pressure"}
+    assert prof["tendency"]["launches"] == 4 and prof["barotropic"]["launches"] == 4 * (30 // 6 + 1)
+    assert all(v["ms"] > 0 for v in prof.values())
+
+
+def test_bad_arguments_on_the_gpu_side():
+    wl = W.config0()
+    m = ocn.Model(wl)
+    with pytest.raises(RuntimeError, match="get only"):
+        m.set_fields_ptr(w=1)
+    with pytest.raises(RuntimeError, match="bad argument"):
+        m.time_step(-1)
+    m.close()
+    bad = dict(wl); bad["params"] = dict(wl["params"], precision=16)
+    with pytest.raises(RuntimeError, match="precision"):
+        ocn.Model(bad)
+    bad["params"] = dict(wl["params"], substeps=0)
+    with pytest.raises(RuntimeError, match="substeps"):
+        ocn.Model(bad)
