@@ -71,6 +71,9 @@ def oracle_sample(config):
     if config == 4:
         wl = W.config4(window=CPU_WINDOW, steps=1)
         what = "config 4 window j=%d:%d i=%d:%d (closed box, identical physics)" % CPU_WINDOW
+    elif config == 5:
+        wl = W.aquaplanet(window=(300, 500, 900, 1300), steps=1)
+        what = "aqua-planet window j=300:500 i=900:1300 (closed box)"
     elif config in (2, 3):
         wl = W.make(config, window=(200, 400, 500, 900), steps=1)
         what = "config %d window j=200:400 i=500:900 (closed box)" % config

@@ -169,8 +169,19 @@ def latlon_bathymetry(rng, ny, nx, max_depth=6000.0, land_fraction=0.30):
     return depth
 
 
+def aquaplanet_bathymetry(ny, nx, max_depth=6000.0, ridge_height=4000.0, ridge_width_deg=8.0):
+    """Idealised bathymetry of the paper's aqua-planet suite: a flat 6 km floor with two
+    meridional (pole-to-pole) Gaussian ridges, 180 degrees apart; no land."""
+    lon = (np.arange(nx) + 0.5) * 360.0 / nx
+    def ridge(l0):
+        d = np.minimum(np.abs(lon - l0), 360.0 - np.abs(lon - l0))
+        return np.exp(-0.5 * (d / ridge_width_deg) ** 2)
+    h = max_depth - ridge_height * np.maximum(ridge(90.0), ridge(270.0))
+    return np.broadcast_to(h[None, :], (ny, nx)).copy()
+
+
 def latlon(nx, ny, nz, *, dt, substeps, steps, nu_h, kappa_h, precision, seed, name,
-           noise=True, lat0=-75.0, lat1=75.0, window=None):
+           noise=True, lat0=-75.0, lat1=75.0, window=None, bathymetry="fractal"):
     """Near-global lat-lon workload.  `window=(j0, j1, i0, i1)` cuts a sub-window out of the
     full-size fields (identical values) and turns it into a closed box: not periodic, and the
     bathymetry is used as is (the library treats non-periodic edges as land)."""
@@ -179,7 +190,7 @@ def latlon(nx, ny, nz, *, dt, substeps, steps, nu_h, kappa_h, precision, seed, n
     dlon = 360.0 / nx
     zf = geometric_z_faces(nz, 10.0, 6000.0)
     zc = _z_centres(zf)
-    depth = latlon_bathymetry(rng, ny, nx)
+    depth = latlon_bathymetry(rng, ny, nx) if bathymetry == "fractal" else aquaplanet_bathymetry(ny, nx)
     latc = np.deg2rad(lat0 + (np.arange(ny) + 0.5) * dlat)
     # wind stress: zonal 0.1*cos(3*lat) plus seeded low modes (periodic in longitude)
     tx_modes = _low_mode_field(rng, ny, nx, 3)
@@ -241,7 +252,18 @@ def config4(nx=2880, ny=1200, nz=100, steps=20, seed=SEED_BASE + 4, window=None,
                   name="cfg4_latlon_eighth_deg_fp32", window=window)
 
 
-CONFIGS = {0: config0, 1: config1, 2: config2, 3: config3, 4: config4}
+def aquaplanet(nx=2160, ny=900, nz=100, steps=20, precision=32, seed=SEED_BASE + 5, window=None):
+    """the aqua-planet workload of the paper's weak-scaling suite at
+    its per-GPU resolution of 1/6 degree x 100 levels: two meridional ridges, no land, the same seeded T/S profiles
+    and wind stress as the realistic-shape configurations.  Not a BASELINE.json config; used as a second bench workload
+    (every cell is wet) and a parity case."""
+    scale = 2160.0 / nx
+    return latlon(nx, ny, nz, dt=min(360.0 * scale, 1200.0), substeps=40, steps=steps, nu_h=700.0 * scale,
+                  kappa_h=70.0 * scale, precision=precision, seed=seed, name="ap_aquaplanet_sixth_deg",
+                  window=window, bathymetry="aquaplanet")
+
+
+CONFIGS = {0: config0, 1: config1, 2: config2, 3: config3, 4: config4, 5: aquaplanet}
 
 
 def make(config, **kw):

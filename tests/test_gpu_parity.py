@@ -319,3 +319,15 @@ def test_bad_arguments_on_the_gpu_side():
     bad["params"] = dict(wl["params"], substeps=0)
     with pytest.raises(RuntimeError, match="substeps"):
         ocn.Model(bad)
+
+
+def test_aquaplanet_reduced_fp32_and_fp64():
+    # two meridional ridges, no land (every tile full): fp32 within 2e-4, fp64 bit-identical
+    run_both(W.aquaplanet(nx=360, ny=150, nz=40, steps=10), 10, check_every=[1, 10])
+    wl = W.aquaplanet(nx=180, ny=75, nz=20, steps=6, precision=64)
+    ref, gpu = oracle.RefModel(wl), ocn.Model(wl)
+    ref.step(6); gpu.time_step(6)
+    a, b = gpu.get_fields(), ref.get_fields()
+    for n in FIELDS:
+        assert np.array_equal(a[n], b[n]), n
+    gpu.close()
