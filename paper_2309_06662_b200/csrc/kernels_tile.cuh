@@ -63,8 +63,8 @@ struct Tile {
     static constexpr int R_TS = DP + 5, R_UV = DP + 1, R_P = DP, NB = DP;
     static constexpr int RX = TX + 1, RY = TY + 1;       // tile + west/south ring (K, D, w) or + east/north edge (faces, masks)
     static constexpr int PL2 = rup128(BX * BY * (int)sizeof(T2)), PL1 = rup128(BX * BY * (int)sizeof(T)),
-                         PLP = rup128(BX * BY * 8);          // pressure planes are fp64
-    static constexpr int BYTES2 = BX * BY * (int)sizeof(T2), BYTESP = BX * BY * 8;
+                         PLP = rup128((TX + 4) * (TY + 1) * 8);   // pressure planes: fp64, box (TX + 4) x (TY + 1), origin (i0 - 4, j0 - 1)
+    static constexpr int BYTES2 = BX * BY * (int)sizeof(T2), BYTESP = (TX + 4) * (TY + 1) * 8, PBX = TX + 4;
     // shared-memory map (byte offsets from a 128-byte aligned base)
     static constexpr int O_TS = 0;
     static constexpr int O_UV = O_TS + (DO_T ? R_TS : 0) * PL2;
@@ -177,26 +177,27 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 }
             }
             __syncthreads();
-            {                                                             // thread t < 256 owns key t
-                const int kt = tid & 255;
+            // per key: offsets of the virtual warps within the key, and the key total (into base[])
+            for (int kt = tid; kt < 256; kt += NT) {
                 int run = 0;
-                if (tid < 256)
-                    for (int vw = 0; vw < nr * (NT / 32); ++vw) {
-                        const int cc = cnt[vw * 256 + kt];
-                        cnt[vw * 256 + kt] = (unsigned short)run;
-                        run += cc;
-                    }
-                int inc = run;                                            // block-wide inclusive scan of the key totals
+                for (int vw = 0; vw < nr * (NT / 32); ++vw) {
+                    const int cc = cnt[vw * 256 + kt];
+                    cnt[vw * 256 + kt] = (unsigned short)run;
+                    run += cc;
+                }
+                base[kt] = run;
+            }
+            __syncthreads();
+            if (wrp == 0) {                                               // exclusive scan of the 256 key totals by one warp
+                int tot[8], sum = 0;
+#pragma unroll
+                for (int e = 0; e < 8; ++e) { tot[e] = base[lane * 8 + e]; sum += tot[e]; }
+                int inc = sum;
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
-                if (lane == 31 && tid < 256) base[256 + wrp] = inc;
-                __syncthreads();
-                if (tid < 256) {
-                    int off = 0;
-                    for (int w = 0; w < wrp; ++w) off += base[256 + w];
-                    base[kt] = off + inc - run;
-                    nle[kt] = (unsigned short)(off + inc);
-                }
+                int off = inc - sum;
+#pragma unroll
+                for (int e = 0; e < 8; ++e) { base[lane * 8 + e] = off; off += tot[e]; nle[lane * 8 + e] = (unsigned short)off; }
             }
             __syncthreads();
 #pragma unroll
@@ -206,7 +207,6 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             }
             __syncthreads();
         };
-        static_assert(NC == 256, "one thread per key");
         csort(NC,
               [&](int q) { const int gx = q % TX, gy = q / TX;
                            return (i0 + gx < P.nx && j0 + gy < P.ny) ? (int)(s_m8[gy * RX + gx].x & 255u) : nz; },
@@ -263,7 +263,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
         mbar_expect_tx(bar, bytes);
         for (int q = tlo; q <= thi; ++q) tma_load_plane(sm + C::O_TS + (q % C::R_TS) * C::PL2, &m_ts, bar, 2 * i0, j0, q);
         if (m < nz) tma_load_plane(sm + C::O_UV + (m % C::R_UV) * C::PL2, &m_uv, bar, 2 * i0, j0, m);
-        if (DO_M && m - 1 >= kmin) tma_load_plane(sm + C::O_P + ((m - 1) % C::R_P) * C::PLP, &m_p, bar, i0, j0, m - 1);
+        if (DO_M && m - 1 >= kmin) tma_load_plane(sm + C::O_P + ((m - 1) % C::R_P) * C::PLP, &m_p, bar, i0, j0 + 2, m - 1);
     };
     if (tid == 0) {
         issue_group(kmin, true);
@@ -459,7 +459,8 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                     const T2 uv_up = (k + 1 < nz) ? s_uv1[bo] : mk2(T(0), T(0));
                     const T z00 = s_zeta[bo];
                     const T2 kdc = s_kd[qo];
-                    const double pc = s_p[bo];
+                    const int pbo = (cy + 1) * C::PBX + cx + 4;
+                    const double pc = s_p[pbo];
                     const Xv<T> half(T(0.5)), quart(T(0.25)), nuh(P.nu_h);
                     const T vold = (X(AzCj) * X(dzk)).v;                            // AzC dz (u) ; AzF dz for v below
                     if (mu) {
@@ -473,7 +474,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                         const Xv<T> Cu = xdiv(half * (X(fFj) * half * X(dxFj) * vsum_s + X(fFn) * half * X(dxFn) * vsum_n), dxCj, rdxCj);
                         const T2 kdw = s_kd[qo - 1];
                         const Xv<T> dK = xdiv(X(kdc.x) - X(kdw.x), dxCj, rdxCj);
-                        const Xv<T> dP = xdiv(X((T)(pc - s_p[bo - 1])), dxCj, rdxCj);
+                        const Xv<T> dP = xdiv(X((T)(pc - s_p[pbo - 1])), dxCj, rdxCj);
                         const Xv<T> dlo((k >= 1 && k - 1 >= tx1) ? (X(u_c) - X(u_dn)).v : T(0));
                         const Xv<T> dhi((k + 1 <= nz - 1) ? (X(uv_up.x) - X(u_c)).v : T(0));
                         const Xv<T> Whi = half * X(AzCj) * (X(s_w1[qo - 1]) + X(w_c1)), Wlo = half * X(AzCj) * (X(s_w0[qo - 1]) + X(w_c0));
@@ -491,7 +492,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                         const Xv<T> Cv = X(fFj) * X(uhat);
                         const T2 kds = s_kd[qo - RX];
                         const Xv<T> dK = xdiv(X(kdc.x) - X(kds.x), dy, rdy);
-                        const Xv<T> dP = xdiv(X((T)(pc - s_p[bo - BX])), dy, rdy);
+                        const Xv<T> dP = xdiv(X((T)(pc - s_p[pbo - C::PBX])), dy, rdy);
                         const Xv<T> dlo((k >= 1 && k - 1 >= ty1) ? (X(v_c) - X(v_dn)).v : T(0));
                         const Xv<T> dhi((k + 1 <= nz - 1) ? (X(uv_up.y) - X(v_c)).v : T(0));
                         const Xv<T> Whi = half * (X(AzCs) * X(s_w1[qo - RX]) + X(AzCj) * X(w_c1));

@@ -238,7 +238,7 @@ ocn_status build_model(ocn_model* M) {
         const unsigned long long sxu = (unsigned long long)g->sx, syu = (unsigned long long)g->sy;
         if ((s = make_tmap(&M->tm_ts, f64, (T*)P.ts - 2 * C::OX, 2 * sxu, syu, nz, 2 * C::BX, C::BY)) != OCN_OK ||
             (s = make_tmap(&M->tm_uv, f64, (T*)P.uv - 2 * C::OX, 2 * sxu, syu, nz, 2 * C::BX, C::BY)) != OCN_OK ||
-            (s = make_tmap(&M->tm_p, true, P.p - C::OX, sxu, syu, nz, C::BX, C::BY)) != OCN_OK)
+            (s = make_tmap(&M->tm_p, true, P.p - C::OX, sxu, syu, nz, C::PBX, TILE_Y + 1)) != OCN_OK)
             return s;
         CK(cudaFuncSetAttribute(k1_fused<T>(), cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
         CK(cudaFuncSetAttribute(k1_momentum<T>(), cudaFuncAttributeMaxDynamicSharedMemorySize, (ocn::Tile<T, TILE_X, TILE_Y, 1>::SMEM)));
