@@ -172,27 +172,35 @@ __global__ void __launch_bounds__(256) k_barotropic_finish(const DevP<T> P) {
 // K1) and the correction (Ubar - SU) / Hu is known before the sweep.
 // ---------------------------------------------------------------------------------------------
 template <class T>
-__global__ void __launch_bounds__(128) k_backsub_correct(const DevP<T> P) {
+__global__ void __launch_bounds__(128, sizeof(T) == 8 ? 4 : 8) k_backsub_correct(const DevP<T> P) {
     typedef Ex<T> E;
     typedef typename Pair<T>::type T2;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
-    if (i >= P.nx || j >= P.ny) return;
+    if (j >= P.ny) return;                                  // uniform over the warp (blockDim.x is a multiple of 32)
+    const bool incol = i < P.nx;
     const int sx = P.sx, nz = P.nz;
-    const long long sz = P.sz, c = (long long)(j + OCN_HALO) * sx + i;
+    const long long sz = P.sz, c = (long long)(j + OCN_HALO) * sx + min(i, P.nx - 1);
     const uint2 m = P.m8[c];
-    const int kb = m.x & 255, tx1 = (m.x >> 8) & 255, ty1 = m.y & 255;
-    if (kb >= nz) return;
+    const int kb = incol ? (int)(m.x & 255) : nz, tx1 = incol ? (int)((m.x >> 8) & 255) : nz, ty1 = incol ? (int)(m.y & 255) : nz;
+    const int kuv = min(tx1, ty1);
+    // Sector-complete stores: the four columns that share a 32-byte sector of a pair / fp64 plane start at the
+    // shallowest of their first levels and the dry ones store the zeros that are there already, so that L2 never has
+    // to fetch a partly written sector from HBM.
+    int kg = min(kb, __shfl_xor_sync(0xffffffffu, kb, 1));
+    kg = min(kg, __shfl_xor_sync(0xffffffffu, kg, 2));
+    int kguv = min(kuv, __shfl_xor_sync(0xffffffffu, kuv, 1));
+    kguv = min(kguv, __shfl_xor_sync(0xffffffffu, kguv, 2));
+    if (kg >= nz || !incol) return;
     const T cu = tx1 < nz ? (P.Ub[c] - P.SU[c]) * P.rHu[c] : T(0);
     const T cv = ty1 < nz ? (P.Vb[c] - P.SV[c]) * P.rHv[c] : T(0);
     const T* __restrict__ cpu = P.cp_m + min(tx1, nz - 1);
     const T* __restrict__ cpv = P.cp_m + min(ty1, nz - 1);
-    const T* __restrict__ cpt = P.cp_t + kb;
+    const T* __restrict__ cpt = P.cp_t + min(kb, nz - 1);
     T xu = 0, xv = 0, xt = 0, xs = 0;
     double b1 = 0, pk = 0;
-    const int kuv = min(tx1, ty1);
-    constexpr int NB = 4;                                  // levels whose loads are in flight together
-    for (int k0 = nz - 1; k0 >= kb; k0 -= NB) {
+    constexpr int NB = 3;                                  // levels whose loads are in flight together (measured best with 8 CTAs / SM)
+    for (int k0 = nz - 1; k0 >= kg; k0 -= NB) {
         T2 d_ts[NB], d_uv[NB];
 #pragma unroll
         for (int q = 0; q < NB; ++q) {
@@ -206,25 +214,31 @@ __global__ void __launch_bounds__(128) k_backsub_correct(const DevP<T> P) {
 #pragma unroll
         for (int q = 0; q < NB; ++q) {
             const int k = k0 - q;
-            if (k < kb) break;
-            const T ck = cpt[k * nz];
-            xt = E::sub(d_ts[q].x, E::mul(ck, xt));                      // cp[nz-1] = 0
-            xs = E::sub(d_ts[q].y, E::mul(ck, xs));
-            store_halo(P.ts + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, mk2(xt, xs));
-            const double b0 = buoyancy(P, xt, xs);
-            pk = pressure_level(P, k, b0, b1, pk);
-            b1 = b0;
-            store_halo(P.p + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, pk);
-            const bool mu = k >= tx1, mv = k >= ty1;
-            if (mu | mv) {
+            if (k < kg) break;
+            T2 ots = mk2(T(0), T(0));
+            double op = 0.0;
+            if (k >= kb) {
+                const T ck = cpt[k * nz];
+                xt = E::sub(d_ts[q].x, E::mul(ck, xt));                      // cp[nz-1] = 0
+                xs = E::sub(d_ts[q].y, E::mul(ck, xs));
+                const double b0 = buoyancy(P, xt, xs);
+                pk = pressure_level(P, k, b0, b1, pk);
+                b1 = b0;
+                ots = mk2(xt, xs); op = pk;
+            }
+            store_halo(P.ts + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, ots);
+            store_halo(P.p + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, op);
+            if (k >= kguv) {
+                const bool mu = k >= tx1, mv = k >= ty1;
                 T un = 0, vn = 0;
                 if (mu) { xu = E::sub(d_uv[q].x, E::mul(cpu[k * nz], xu)); un = xu + cu; }
                 if (mv) { xv = E::sub(d_uv[q].y, E::mul(cpv[k * nz], xv)); vn = xv + cv; }
-                if (sizeof(T) == 8) P.uv[k * sz + c] = mk2(xu * T(mu), xv * T(mv));      // u**, corrected below
+                if (sizeof(T) == 8) { if (mu | mv) P.uv[k * sz + c] = mk2(xu * T(mu), xv * T(mv)); }    // u**, corrected below
                 else store_halo(P.uv + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, mk2(un, vn));
             }
         }
     }
+    if (kuv >= nz) return;
     if (sizeof(T) == 8) {
         // fp64: the correction as DESIGN.md §3.8 step 8 writes it, (Ubar - sum_k dz u**) / Hu with the sum taken
         // bottom-up over the back-substituted column (the fp32 path uses K1's sum of the predictor instead)
