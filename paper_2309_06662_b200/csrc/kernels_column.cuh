@@ -35,12 +35,12 @@ __device__ __forceinline__ double pressure_level(const DevP<T>& P, int k, double
 template <class T, int BTX, int BTY>
 struct BtTile {
     static constexpr int EX = BTX + 2 * BT_HALO, EY = BTY + 2 * BT_HALO, NE = EX * EY;
-    static constexpr int NT = 1024, PER = (NE + NT - 1) / NT;      // extended-tile points per thread
+    static constexpr int NT = BTX * BTY >= 2048 ? 1024 : 512, PER = (NE + NT - 1) / NT;      // extended-tile points per thread
     static constexpr int SMEM = NE * (7 * (int)sizeof(T) + 1) + 6 * (EY + 1) * (int)sizeof(T) + 64 + BT_HALO * (int)sizeof(T);
 };
 
 template <class T, int BTX, int BTY>
-__global__ void __launch_bounds__(1024) k_barotropic_tile(const DevP<T> P, const int cur, const int ns, const int first,
+__global__ void __launch_bounds__((BtTile<T, BTX, BTY>::NT)) k_barotropic_tile(const DevP<T> P, const int cur, const int ns, const int first,
                                                          const T a0, const T a1, const T a2, const T a3, const T a4, const T a5) {
     typedef BtTile<T, BTX, BTY> C;
     constexpr int EX = C::EX, EY = C::EY, NE = C::NE, NT = C::NT, H = BT_HALO;
@@ -67,7 +67,7 @@ __global__ void __launch_bounds__(1024) k_barotropic_tile(const DevP<T> P, const
     // ---- load the extended tile (wrap / land) ----
     for (int q = tid; q <= EY; q += NT) {
         int jj = j0 - H + q;
-        if (P.py) jj = ((jj % ny) + ny) % ny;
+        if (P.py) { while (jj < 0) jj += ny; while (jj >= ny) jj -= ny; }
         const int r = min(max(jj, -OCN_HALO), ny + OCN_HALO) + OCN_HALO;      // metric rows exist for -3 .. ny + 3
         if (q < EY) { rAz[q] = P.rAzC[r]; rdx[q] = P.rdxC[r]; Az[q] = P.AzC[r]; dxc[q] = P.dxC[r]; }
         dF[q] = P.dxF[r];
@@ -75,23 +75,35 @@ __global__ void __launch_bounds__(1024) k_barotropic_tile(const DevP<T> P, const
     const T* __restrict__ e0 = P.eta[cur];
     const T* __restrict__ U0 = P.U[cur];
     const T* __restrict__ V0 = P.V[cur];
-    for (int q = tid; q < NE; q += NT) {
-        const int x = q % EX, y = q / EX;
-        int ii = i0 - H + x, jj = j0 - H + y;
-        bool in = true;
-        if (P.px) ii = ((ii % nx) + nx) % nx; else in = in && ii >= 0 && ii < nx;
-        if (P.py) jj = ((jj % ny) + ny) % ny; else in = in && jj >= 0 && jj < ny;
-        T e = 0, u = 0, v = 0, gu = 0, gv = 0, hu = 0, hv = 0;
-        unsigned char mk = 0;
-        if (in) {
-            const long long c = (long long)(jj + OCN_HALO) * sx + ii;
-            const uint2 m = P.m8[c];
-            mk = (unsigned char)(((m.x & 255u) < (unsigned)nz ? 1 : 0) | ((((m.x >> 8) & 255u) < (unsigned)nz) ? 2 : 0) |
-                                 (((m.y & 255u) < (unsigned)nz) ? 4 : 0));
-            if (mk) { e = e0[c]; u = U0[c]; v = V0[c]; gu = P.GU[c]; gv = P.GV[c]; hu = P.Hu[c]; hv = P.Hv[c]; }
+    {
+        int cs[C::PER];                                        // source plane index of each point, -1 outside a bounded domain
+        uint2 ms[C::PER];
+#pragma unroll
+        for (int n = 0; n < C::PER; ++n) {                     // wrap by steps: the tile reaches at most H + BTX past an edge
+            const int q = n * NT + tid;
+            const int x = q % EX, y = q / EX;
+            int ii = i0 - H + x, jj = j0 - H + y;
+            bool in = q < NE;
+            if (P.px) { while (ii < 0) ii += nx; while (ii >= nx) ii -= nx; } else in = in && ii >= 0 && ii < nx;
+            if (P.py) { while (jj < 0) jj += ny; while (jj >= ny) jj -= ny; } else in = in && jj >= 0 && jj < ny;
+            cs[n] = in ? (jj + OCN_HALO) * sx + ii : -1;
+            ms[n] = make_uint2(nz, nz);
+            if (in) ms[n] = P.m8[cs[n]];
         }
-        se[q] = e; sU[q] = u; sV[q] = v; smk[q] = mk;
-        sGU[q] = gu; sGV[q] = gv; sHu[q] = hu; sHv[q] = hv;
+#pragma unroll
+        for (int n = 0; n < C::PER; ++n) {
+            const int q = n * NT + tid;
+            if (q < NE) {
+                const uint2 m = ms[n];
+                const int c = cs[n];
+                T e = 0, u = 0, v = 0, gu = 0, gv = 0, hu = 0, hv = 0;
+                const unsigned char mk = c < 0 ? 0 : (unsigned char)(((m.x & 255u) < (unsigned)nz ? 1 : 0) | ((((m.x >> 8) & 255u) < (unsigned)nz) ? 2 : 0) |
+                                                                      (((m.y & 255u) < (unsigned)nz) ? 4 : 0));
+                if (mk) { e = e0[c]; u = U0[c]; v = V0[c]; gu = P.GU[c]; gv = P.GV[c]; hu = P.Hu[c]; hv = P.Hv[c]; }
+                se[q] = e; sU[q] = u; sV[q] = v; smk[q] = mk;
+                sGU[q] = gu; sGV[q] = gv; sHu[q] = hu; sHv[q] = hv;
+            }
+        }
     }
     __syncthreads();
 
@@ -99,7 +111,7 @@ __global__ void __launch_bounds__(1024) k_barotropic_tile(const DevP<T> P, const
     // other thread touches a value between its update and its accumulation); one running sum over all M
     // sub-steps (DESIGN.md §3.8 step 6), continued from the previous launch --------------------------------
     T be[C::PER], bU[C::PER], bV[C::PER];
-    long long cidx[C::PER];                                   // global index of the interior points, -1 elsewhere
+    int cidx[C::PER];                                         // plane index of the interior points, -1 elsewhere
 #pragma unroll
     for (int n = 0; n < C::PER; ++n) {
         be[n] = 0; bU[n] = 0; bV[n] = 0; cidx[n] = -1;
@@ -107,12 +119,59 @@ __global__ void __launch_bounds__(1024) k_barotropic_tile(const DevP<T> P, const
         const int x = q % EX - H, y = q / EX - H;
         const int i = i0 + x, j = j0 + y;
         if (q < NE && x >= 0 && x < BTX && y >= 0 && y < BTY && i < nx && j < ny) {
-            cidx[n] = (long long)(j + OCN_HALO) * sx + i;
+            cidx[n] = (j + OCN_HALO) * sx + i;
             if (!first) { be[n] = P.etab[cidx[n]]; bU[n] = P.Ub[cidx[n]]; bV[n] = P.Vb[cidx[n]]; }
         }
     }
     const T dy = P.dy, dtau = P.dtau, g = P.g, rdy = P.rdy;
 
+    if constexpr (sizeof(T) == 4) {
+        // fp32: everything that is constant over the sub-steps (mask, depth, metric, forcing, dtau) is folded into five
+        // per-point coefficients held in registers, zero where the point is closed or on the rim of the extended tile:
+        //   eta -= ce (dy (U_e - U) + dxF_n V_n - dxF V),  U += cu (eta_w - eta) + gu,  V += cv (eta_s - eta) + gv
+        T ce[C::PER], cu[C::PER], cv[C::PER], gu[C::PER], gv[C::PER];
+        uint32_t ypk = 0;                                      // the extended row of each point, one byte each
+        static_assert(C::PER <= 4 && EY < 256, "row bytes");
+#pragma unroll
+        for (int n = 0; n < C::PER; ++n) {
+            ce[n] = cu[n] = cv[n] = gu[n] = gv[n] = 0;
+            const int q = n * NT + tid;
+            if (q < NE) {
+                const int x = q % EX, y = q / EX;
+                const unsigned char mk = smk[q];
+                ypk |= (uint32_t)y << (8 * n);
+                if (x < EX - 1 && y < EY - 1 && (mk & 1)) ce[n] = dtau * rAz[y];
+                if (x > 0 && (mk & 2)) { cu[n] = dtau * g * sHu[q] * rdx[y]; gu[n] = dtau * sGU[q]; }
+                if (y > 0 && (mk & 4)) { cv[n] = dtau * g * sHv[q] * rdy; gv[n] = dtau * sGV[q]; }
+            }
+        }
+        for (int s = 0; s < ns; ++s) {
+#pragma unroll
+            for (int n = 0; n < C::PER; ++n) {
+                const int q = n * NT + tid;
+                if (q < NE) {
+                    const int y = (ypk >> (8 * n)) & 255u;
+                    const int qe = min(q + 1, NE - 1), qn = min(q + EX, NE - 1);      // rim points: ce = 0
+                    const T uc = sU[q], vc = sV[q];
+                    se[q] = se[q] - ce[n] * (dy * (sU[qe] - uc) + dF[y + 1] * sV[qn] - dF[y] * vc);
+                }
+            }
+            __syncthreads();
+            const T am = saw[s];
+#pragma unroll
+            for (int n = 0; n < C::PER; ++n) {
+                const int q = n * NT + tid;
+                if (q < NE) {
+                    const T ec = se[q], ew = se[max(q - 1, 0)], es = se[max(q - EX, 0)];     // rim points: cu = cv = 0
+                    const T un = sU[q] + (cu[n] * (ew - ec) + gu[n]);
+                    const T vn = sV[q] + (cv[n] * (es - ec) + gv[n]);
+                    sU[q] = un; sV[q] = vn;
+                    if (cidx[n] >= 0) { be[n] += am * ec; bU[n] += am * un; bV[n] += am * vn; }
+                }
+            }
+            __syncthreads();
+        }
+    } else {
     for (int s = 0; s < ns; ++s) {
         // eta: valid on [s, EX - 1 - s) x [s, EY - 1 - s) given U, V valid on [s, EX - s) x [s, EY - s)
         for (int q = tid; q < NE; q += NT) {
@@ -141,12 +200,13 @@ __global__ void __launch_bounds__(1024) k_barotropic_tile(const DevP<T> P, const
         }
         __syncthreads();
     }
+    }
     // ---- write back the interior ----
 #pragma unroll
     for (int n = 0; n < C::PER; ++n) {
         if (cidx[n] >= 0) {
             const int q = n * NT + tid;
-            const long long c = cidx[n];
+            const int c = cidx[n];
             P.eta[cur ^ 1][c] = se[q]; P.U[cur ^ 1][c] = sU[q]; P.V[cur ^ 1][c] = sV[q];
             P.etab[c] = be[n]; P.Ub[c] = bU[n]; P.Vb[c] = bV[n];
         }

@@ -91,7 +91,7 @@ template <> ocn::DevP<float>& params<float>(ocn_model* M) { return M->pf; }
 template <> ocn::DevP<double>& params<double>(ocn_model* M) { return M->pd; }
 
 constexpr int TILE_X = 32, TILE_Y = 8;    // K1 tile (kernels_tile.cuh)
-constexpr int BT_X = 64, BT_Y = 32;       // barotropic tile (kernels_column.cuh)
+constexpr int BT_X = 32, BT_Y = 32;       // barotropic tile (kernels_column.cuh)
 
 // TMA descriptor of a halo'd 3-D array seen as [levels][rows][inner] scalars
 ocn_status make_tmap(CUtensorMap* tm, bool f64, void* base, unsigned long long inner, unsigned long long rows,
