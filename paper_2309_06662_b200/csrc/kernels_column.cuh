@@ -30,7 +30,9 @@ __device__ __forceinline__ double pressure_level(const DevP<T>& P, int k, double
 // when the tile is loaded (no physical halo is needed), bounded ones read land.
 // Reads buffer `cur`, writes buffer `cur ^ 1`; the filter sums live in registers during the launch.
 // ---------------------------------------------------------------------------------------------
-#define BT_HALO 6
+#ifndef BT_HALO
+#define BT_HALO 6                  // sub-steps per launch = halo rings of the resident tile (<= 6: the launch carries six weights)
+#endif
 
 template <class T, int BTX, int BTY>
 struct BtTile {
@@ -62,7 +64,11 @@ __global__ void __launch_bounds__((BtTile<T, BTX, BTY>::NT)) k_barotropic_tile(c
     const int tid = threadIdx.x;
     const int i0 = blockIdx.x * BTX, j0 = blockIdx.y * BTY;
     const int nx = P.nx, ny = P.ny, nz = P.nz, sx = P.sx;
-    if (tid == 0) { saw[0] = a0; saw[1] = a1; saw[2] = a2; saw[3] = a3; saw[4] = a4; saw[5] = a5; }
+    if (tid == 0) {
+        const T aw[6] = {a0, a1, a2, a3, a4, a5};
+#pragma unroll
+        for (int q = 0; q < BT_HALO; ++q) saw[q] = aw[q];
+    }
 
     // ---- load the extended tile (wrap / land) ----
     for (int q = tid; q <= EY; q += NT) {

@@ -314,8 +314,8 @@ ocn_status launch_step(ocn_model* M, bool euler) {
         int cur = 0;
         for (int m0 = 0; m0 < M->d.substeps; m0 += BT_HALO) {
             const int ns = std::min(BT_HALO, M->d.substeps - m0);
-            T a[BT_HALO];
-            for (int q = 0; q < BT_HALO; ++q) a[q] = q < ns ? (T)M->a_w[m0 + q] : T(0);
+            T a[6];
+            for (int q = 0; q < 6; ++q) a[q] = q < ns ? (T)M->a_w[m0 + q] : T(0);
             ocn::k_barotropic_tile<T, BT_X, BT_Y><<<gb, B::NT, B::SMEM, M->stream>>>(P, cur, ns, m0 == 0 ? 1 : 0, a[0], a[1], a[2],
                                                                                  a[3], a[4], a[5]);
             cur ^= 1;
