@@ -265,6 +265,12 @@ __global__ void __launch_bounds__(128, sizeof(T) == 8 ? 4 : 8) k_backsub_correct
     const T* __restrict__ cpt = P.cp_t + min(kb, nz - 1);
     T xu = 0, xv = 0, xt = 0, xs = 0;
     double b1 = 0, pk = 0;
+    // columns next to a periodic edge also write their halo images; all others store straight
+    const bool edge = (P.px && (i < OCN_HALO || i >= P.nx - OCN_HALO)) || (P.py && (j < OCN_HALO || j >= P.ny - OCN_HALO));
+    auto put = [&](auto* plane, long long o, auto val) {
+        if (edge) store_halo(plane + (o - c), sx, P.nx, P.ny, P.px, P.py, j, i, val);
+        else plane[o] = val;
+    };
     constexpr int NB = 3;                                  // levels whose loads are in flight together (measured best with 8 CTAs / SM)
     for (int k0 = nz - 1; k0 >= kg; k0 -= NB) {
         T2 d_ts[NB], d_uv[NB];
@@ -292,15 +298,16 @@ __global__ void __launch_bounds__(128, sizeof(T) == 8 ? 4 : 8) k_backsub_correct
                 b1 = b0;
                 ots = mk2(xt, xs); op = pk;
             }
-            store_halo(P.ts + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, ots);
-            store_halo(P.p + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, op);
+            const long long o = k * sz + c;
+            put(P.ts, o, ots);
+            put(P.p, o, op);
             if (k >= kguv) {
                 const bool mu = k >= tx1, mv = k >= ty1;
                 T un = 0, vn = 0;
                 if (mu) { xu = E::sub(d_uv[q].x, E::mul(cpu[k * nz], xu)); un = xu + cu; }
                 if (mv) { xv = E::sub(d_uv[q].y, E::mul(cpv[k * nz], xv)); vn = xv + cv; }
-                if (sizeof(T) == 8) { if (mu | mv) P.uv[k * sz + c] = mk2(xu * T(mu), xv * T(mv)); }    // u**, corrected below
-                else store_halo(P.uv + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, mk2(un, vn));
+                if (sizeof(T) == 8) { if (mu | mv) P.uv[o] = mk2(xu * T(mu), xv * T(mv)); }    // u**, corrected below
+                else put(P.uv, o, mk2(un, vn));
             }
         }
     }
