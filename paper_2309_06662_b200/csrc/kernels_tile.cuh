@@ -148,6 +148,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     const int kmin = s_kmin;
     if (kmin >= nz) return;                              // all land: forcing sums stay zero
 
+    int gT = 0, gU = 0, gV = 0;                          // this thread's cell in the tracer, u and v orders
     // ---- compaction lists: cells sorted by their first wet level, faces by their
     // first open level (stable counting sort on the 8-bit level), so that at level k the active work
     // is a dense prefix of each list and keeps the geometric order (coalescing) within a level ------
@@ -207,10 +208,24 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             }
             __syncthreads();
         };
-        csort(NC,
-              [&](int q) { const int gx = q % TX, gy = q / TX;
-                           return (i0 + gx < P.nx && j0 + gy < P.ny) ? (int)(s_m8[gy * RX + gx].x & 255u) : nz; },
-              [&](int q, int rank) { s_cell[rank] = (unsigned short)q; }, s_nc);
+        // three orders of the tile's cells: by first wet level (tracers), by first open west face (u), by first
+        // open south face (v); the thread keeps its entry of each, so one shared list serves all three
+        auto cell_key = [&](int q, int which) {
+            const int gx = q % TX, gy = q / TX;
+            if (!(i0 + gx < P.nx && j0 + gy < P.ny)) return nz;
+            const uint2 m = s_m8[gy * RX + gx];
+            return (int)(which == 0 ? (m.x & 255u) : which == 1 ? ((m.x >> 8) & 255u) : (m.y & 255u));
+        };
+        auto cell_emit = [&](int q, int rank) { s_cell[rank] = (unsigned short)q; };
+        csort(NC, [&](int q) { return cell_key(q, 0); }, cell_emit, s_nc);
+        gT = s_cell[tid];
+        constexpr int VOFF = (NC / 3) & ~31;                          // v ranks start a third of the way into the CTA
+        if constexpr (DO_M) {
+            csort(NC, [&](int q) { return cell_key(q, 1); }, cell_emit, s_nc);
+            gU = s_cell[NC - 1 - tid];
+            csort(NC, [&](int q) { return cell_key(q, 2); }, cell_emit, s_nc);
+            gV = s_cell[(tid + NC - VOFF) % NC];
+        }
         if constexpr (DO_T) {
             // faces: fid < NFX = west face of cell (fid % RX, fid / RX); else south face of cell (g % TX, g / TX), g = fid - NFX
             auto face_cell = [&](int fid, bool& isy, int& fx, int& fy) {
@@ -272,32 +287,33 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     }
 
     // ---- per-thread column state ------------------------------------------------------------
-    // A thread owns the TRACERS of the cell of rank tid and the MOMENTUM of the cell of rank NC-1-tid in the
-    // sorted list: early (deep) cells are paired with late (shallow) ones, so when only part of the tile is
-    // wet at a level the two halves of part B run on different warps instead of one after the other.
-    struct Cell { int cx, cy, kb, tx1, ty1, bo, by; long long c; bool incol; uchar4 mzt; };
-    auto make_cell = [&](int rank) {
+    // A thread owns the TRACERS of the cell of rank t in the order by first wet level, the U of the cell of rank
+    // N-1-t in the order by first open west face and the V of the cell of rank t - N/3 (mod N) in the order by first
+    // open south face: every block of part B runs on a dense run of threads, and on sparse levels the three runs
+    // (from thread 0 up, from N/3 up, from N-1 down) land on different warps instead of one after the other.
+    struct Cell { int cx, cy, t1, bo, by; long long c; bool incol; unsigned char z2, z3; };
+    auto make_cell = [&](int g, int which) {
         Cell X;
-        const int g = s_cell[rank];
         X.cx = g % TX; X.cy = g / TX;
         const int i = i0 + X.cx, j = j0 + X.cy;
         X.incol = i < P.nx && j < P.ny;
         X.c = (long long)(j + OCN_HALO) * sx + i;
         const uint2 mo = s_m8[X.cy * RX + X.cx];
-        X.kb = X.incol ? (int)(mo.x & 255u) : nz;
-        X.tx1 = X.incol ? (int)((mo.x >> 8) & 255u) : nz; X.ty1 = X.incol ? (int)(mo.y & 255u) : nz;
-        X.mzt = make_uchar4(255, 255, 255, 255);
-        if (X.kb < nz) X.mzt = P.mz[X.c];
+        const int kb = X.incol ? (int)(mo.x & 255u) : nz;
+        X.t1 = !X.incol ? nz : which == 0 ? kb : which == 1 ? (int)((mo.x >> 8) & 255u) : (int)(mo.y & 255u);
+        X.z2 = X.z3 = 255;
+        if (which != 0 && kb < nz) { const uchar4 mz = P.mz[X.c]; X.z2 = which == 1 ? mz.x : mz.z; X.z3 = which == 1 ? mz.y : mz.w; }
         X.by = X.cy + OY; X.bo = X.by * BX + X.cx + OX;
         return X;
     };
-    const Cell cT = make_cell(tid), cM = make_cell(NC - 1 - tid);
+    const Cell cT = make_cell(gT, 0), cU = make_cell(gU, 1), cV = make_cell(gV, 2);
     const T dy = P.dy, rdy = P.rdy;
 
     double wacc0 = 0.0, wacc1 = 0.0;                     // w accumulators of this thread's ring points
     T2 fz_bot = mk2(T(0), T(0));                         // vertical tracer flux through the face below
     T u_dn = 0, v_dn = 0;
-    T2 dduv = mk2(T(0), T(0)), ddts = mk2(T(0), T(0));   // eliminated right-hand sides of the level below
+    T ddu = 0, ddv = 0;
+    T2 ddts = mk2(T(0), T(0));                           // eliminated right-hand sides of the level below
     double aGU = 0, aGV = 0, aSU = 0, aSV = 0;
 
     // ring slots of level m, carried along the march (no integer division in the loop)
@@ -305,20 +321,23 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     int rts = kmin % C::R_TS, ruv = kmin % C::R_UV, rp = kmin % C::R_P, r3 = kmin % 3;
     for (int m = kmin; m <= nz; ++m, rts = wrap(rts + 1, C::R_TS), ruv = wrap(ruv + 1, C::R_UV), rp = wrap(rp + 1, C::R_P), r3 = wrap(r3 + 1, 3)) {
         const int kB = m - 1;                                 // level of part B (phase 3) in this iteration
-        const bool doB = kB >= kmin, wetT = DO_T && doB && kB >= cT.kb, wetM = DO_M && doB && kB >= cM.kb;
-        const long long oT = (long long)kB * sz + cT.c, oM = (long long)kB * sz + cM.c;
+        const bool doB = kB >= kmin, wetT = DO_T && doB && kB >= cT.t1, wetU = DO_M && doB && kB >= cU.t1, wetV = DO_M && doB && kB >= cV.t1;
+        const long long oT = (long long)kB * sz + cT.c, oU = (long long)kB * sz + cU.c, oV = (long long)kB * sz + cV.c;
         // AB2 history and pivots of level kB: issued now, consumed after part A
-        T2 gm_uv = mk2(T(0), T(0)), gm_ts = mk2(T(0), T(0));
+        T2 gm_ts = mk2(T(0), T(0));
+        T gm_u = 0, gm_v = 0;
         T piv_t = 1, piv_u = 1, piv_v = 1;
         if (wetT) {
             gm_ts = P.Gts[oT];
-            piv_t = sizeof(T) == 8 ? P.m_t[kB * nz + min(cT.kb, nz - 1)] : P.rm_t[kB * nz + min(cT.kb, nz - 1)];
+            piv_t = sizeof(T) == 8 ? P.m_t[kB * nz + min(cT.t1, nz - 1)] : P.rm_t[kB * nz + min(cT.t1, nz - 1)];
         }
-        if (wetM) {
-            gm_uv = P.Guv[oM];
-            const int txc = min(cM.tx1, nz - 1), tyc = min(cM.ty1, nz - 1);
-            if (sizeof(T) == 8) { piv_u = P.m_m[kB * nz + txc]; piv_v = P.m_m[kB * nz + tyc]; }
-            else                { piv_u = P.rm_m[kB * nz + txc]; piv_v = P.rm_m[kB * nz + tyc]; }
+        if (wetU) {
+            gm_u = ((const T*)(P.Guv + oU))[0];
+            piv_u = sizeof(T) == 8 ? P.m_m[kB * nz + cU.t1] : P.rm_m[kB * nz + cU.t1];
+        }
+        if (wetV) {
+            gm_v = ((const T*)(P.Guv + oV))[1];
+            piv_v = sizeof(T) == 8 ? P.m_m[kB * nz + cV.t1] : P.rm_m[kB * nz + cV.t1];
         }
         mbar_wait(&bars[(m - kmin) % C::NB], (uint32_t)(((m - kmin) / C::NB) & 1));
 
@@ -396,7 +415,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             // ---------- tracer half: the cell of rank tid ----------
             T2 fz_top = mk2(T(0), T(0));
             if constexpr (DO_T) if (wetT) {
-                const int cx = cT.cx, cy = cT.cy, kb = cT.kb, bo = cT.bo, by = cT.by;
+                const int cx = cT.cx, cy = cT.cy, kb = cT.t1, bo = cT.bo, by = cT.by;
                 const long long o = oT;
                 const T AzCj = s_AzC[by], rAzCj = s_rAzC[by];
                 const T w_c1 = s_w1[(cy + 1) * RX + cx + 1];
@@ -438,94 +457,98 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 ddts.y = E::div(E::add(E::add(tsc.y, E::mul(P.dt, Ghs)), E::mul(smk, ddts.y)), piv_t, piv_t);
                 P.dts[o] = ddts;
             }
-            // ---------- momentum half: the cell of rank NC - 1 - tid ----------
-            if constexpr (DO_M) if (wetM) {
-                const int cx = cM.cx, cy = cM.cy, tx1 = cM.tx1, ty1 = cM.ty1, bo = cM.bo, by = cM.by;
-                const long long o = oM, c = cM.c;
-                const uchar4 mzt = cM.mzt;
+            // ---------- momentum: the u face and the v face this thread owns ----------
+            if constexpr (DO_M) if (wetU) {
+                const int cx = cU.cx, cy = cU.cy, tx1 = cU.t1, bo = cU.bo, by = cU.by;
                 const int qo = (cy + 1) * RX + cx + 1;                       // this column in the ring arrays
                 const T w_c1 = s_w1[qo], w_c0 = s_w0[qo];
-                const T dxFj = s_dxF[by], dxFn = s_dxF[by + 1], dxCj = s_dxC[by], rdxCj = s_rdxC[by], rdxFj = s_rdxF[by];
-                const T AzCj = s_AzC[by], AzCs = s_AzC[by - 1], rAzCj = s_rAzC[by], AzFj = s_AzF[by], rAzFj = s_rAzF[by];
+                const T dxFj = s_dxF[by], dxFn = s_dxF[by + 1], dxCj = s_dxC[by], rdxCj = s_rdxC[by];
+                const T AzCj = s_AzC[by], rAzCj = s_rAzC[by];
                 const T fFj = s_fF[by], fFn = s_fF[by + 1];
-                const bool mu = k >= tx1, mv = k >= ty1;
-                // ---- momentum ----
                 const T2 uvc = s_uv[bo];
                 const T u_c = uvc.x, v_c = uvc.y;
-                T Gu = 0, Gv = 0;
-                if (mu | mv) {
-                    const T2 uv_w = s_uv[bo - 1], uv_n = s_uv[bo + BX], uv_nw = s_uv[bo + BX - 1];
-                    const T2 uv_s = s_uv[bo - BX], uv_e = s_uv[bo + 1], uv_se = s_uv[bo - BX + 1];
-                    const T2 uv_up = (k + 1 < nz) ? s_uv1[bo] : mk2(T(0), T(0));
-                    const T z00 = s_zeta[bo];
-                    const T2 kdc = s_kd[qo];
-                    const int pbo = (cy + 1) * C::PBX + cx + 4;
-                    const double pc = s_p[pbo];
-                    const Xv<T> half(T(0.5)), quart(T(0.25)), nuh(P.nu_h);
-                    const T vold = (X(AzCj) * X(dzk)).v;                            // AzC dz (u) ; AzF dz for v below
-                    if (mu) {
-                        const Xv<T> vsum_s = X(uv_w.y) + X(v_c), vsum_n = X(uv_nw.y) + X(uv_n.y);
-                        const T vhat = xdiv(quart * (X(dxFj) * vsum_s + X(dxFn) * vsum_n), dxCj, rdxCj).v;
-                        const int ozu = 1 + (k >= mzt.x) + (k >= mzt.y);
-                        const T z01 = s_zeta[bo + BX];
-                        const T zt = ozu == 1 ? (vhat > T(0) ? z00 : z01)
-                                              : weno_face(s_zeta[bo - 2 * BX], s_zeta[bo - BX], z00, z01, s_zeta[bo + 2 * BX],
-                                                          s_zeta[bo + 3 * BX], vhat, ozu);
-                        const Xv<T> Cu = xdiv(half * (X(fFj) * half * X(dxFj) * vsum_s + X(fFn) * half * X(dxFn) * vsum_n), dxCj, rdxCj);
-                        const T2 kdw = s_kd[qo - 1];
-                        const Xv<T> dK = xdiv(X(kdc.x) - X(kdw.x), dxCj, rdxCj);
-                        const Xv<T> dP = xdiv(X((T)(pc - s_p[pbo - 1])), dxCj, rdxCj);
-                        const Xv<T> dlo((k >= 1 && k - 1 >= tx1) ? (X(u_c) - X(u_dn)).v : T(0));
-                        const Xv<T> dhi((k + 1 <= nz - 1) ? (X(uv_up.x) - X(u_c)).v : T(0));
-                        const Xv<T> Whi = half * X(AzCj) * (X(s_w1[qo - 1]) + X(w_c1)), Wlo = half * X(AzCj) * (X(s_w0[qo - 1]) + X(w_c0));
-                        const Xv<T> Au = xdiv(half * (Whi * dhi + Wlo * dlo), vold, rAzCj * rdzk);
-                        const Xv<T> Vu = nuh * (xdiv(X(kdc.y) - X(kdw.y), dxCj, rdxCj) - xdiv(X(z01) - X(z00), dy, rdy));
-                        const Xv<T> tau((k == nz - 1) ? xdiv(X(P.taux[c]), (X(P.rho0) * X(dzk)).v, P.rrho0 * rdzk).v : T(0));
-                        Gu = (X(zt) * X(vhat) + Cu - dK - dP - Au + Vu + tau).v;
-                    }
-                    if (mv) {
-                        const T uhat = (quart * (X(uv_s.x) + X(u_c) + X(uv_se.x) + X(uv_e.x))).v;
-                        const int ozv = 1 + (k >= mzt.z) + (k >= mzt.w);
-                        const T z10 = s_zeta[bo + 1];
-                        const T zt = ozv == 1 ? (uhat > T(0) ? z00 : z10)
-                                              : weno_face(s_zeta[bo - 2], s_zeta[bo - 1], z00, z10, s_zeta[bo + 2], s_zeta[bo + 3], uhat, ozv);
-                        const Xv<T> Cv = X(fFj) * X(uhat);
-                        const T2 kds = s_kd[qo - RX];
-                        const Xv<T> dK = xdiv(X(kdc.x) - X(kds.x), dy, rdy);
-                        const Xv<T> dP = xdiv(X((T)(pc - s_p[pbo - C::PBX])), dy, rdy);
-                        const Xv<T> dlo((k >= 1 && k - 1 >= ty1) ? (X(v_c) - X(v_dn)).v : T(0));
-                        const Xv<T> dhi((k + 1 <= nz - 1) ? (X(uv_up.y) - X(v_c)).v : T(0));
-                        const Xv<T> Whi = half * (X(AzCs) * X(s_w1[qo - RX]) + X(AzCj) * X(w_c1));
-                        const Xv<T> Wlo = half * (X(AzCs) * X(s_w0[qo - RX]) + X(AzCj) * X(w_c0));
-                        const Xv<T> Av = xdiv(half * (Whi * dhi + Wlo * dlo), (X(AzFj) * X(dzk)).v, rAzFj * rdzk);
-                        const Xv<T> Vv = nuh * (xdiv(X(kdc.y) - X(kds.y), dy, rdy) + xdiv(X(z10) - X(z00), dxFj, rdxFj));
-                        const Xv<T> tau((k == nz - 1) ? xdiv(X(P.tauy[c]), (X(P.rho0) * X(dzk)).v, P.rrho0 * rdzk).v : T(0));
-                        Gv = (-X(zt) * X(uhat) - Cv - dK - dP - Av + Vv + tau).v;
-                    }
-                }
+                const T2 uv_w = s_uv[bo - 1], uv_n = s_uv[bo + BX], uv_nw = s_uv[bo + BX - 1];
+                const T u_up = (k + 1 < nz) ? s_uv1[bo].x : T(0);
+                const T z00 = s_zeta[bo];
+                const T2 kdc = s_kd[qo];
+                const int pbo = (cy + 1) * C::PBX + cx + 4;
+                const Xv<T> half(T(0.5)), quart(T(0.25)), nuh(P.nu_h);
+                const T vold = (X(AzCj) * X(dzk)).v;
+                const Xv<T> vsum_s = X(uv_w.y) + X(v_c), vsum_n = X(uv_nw.y) + X(uv_n.y);
+                const T vhat = xdiv(quart * (X(dxFj) * vsum_s + X(dxFn) * vsum_n), dxCj, rdxCj).v;
+                const int ozu = 1 + (k >= cU.z2) + (k >= cU.z3);
+                const T z01 = s_zeta[bo + BX];
+                const T zt = ozu == 1 ? (vhat > T(0) ? z00 : z01)
+                                      : weno_face(s_zeta[bo - 2 * BX], s_zeta[bo - BX], z00, z01, s_zeta[bo + 2 * BX],
+                                                  s_zeta[bo + 3 * BX], vhat, ozu);
+                const Xv<T> Cu = xdiv(half * (X(fFj) * half * X(dxFj) * vsum_s + X(fFn) * half * X(dxFn) * vsum_n), dxCj, rdxCj);
+                const T2 kdw = s_kd[qo - 1];
+                const Xv<T> dK = xdiv(X(kdc.x) - X(kdw.x), dxCj, rdxCj);
+                const Xv<T> dP = xdiv(X((T)(s_p[pbo] - s_p[pbo - 1])), dxCj, rdxCj);
+                const Xv<T> dlo((k >= 1 && k - 1 >= tx1) ? (X(u_c) - X(u_dn)).v : T(0));
+                const Xv<T> dhi((k + 1 <= nz - 1) ? (X(u_up) - X(u_c)).v : T(0));
+                const Xv<T> Whi = half * X(AzCj) * (X(s_w1[qo - 1]) + X(w_c1)), Wlo = half * X(AzCj) * (X(s_w0[qo - 1]) + X(w_c0));
+                const Xv<T> Au = xdiv(half * (Whi * dhi + Wlo * dlo), vold, rAzCj * rdzk);
+                const Xv<T> Vu = nuh * (xdiv(X(kdc.y) - X(kdw.y), dxCj, rdxCj) - xdiv(X(z01) - X(z00), dy, rdy));
+                const Xv<T> tau((k == nz - 1) ? xdiv(X(P.taux[cU.c]), (X(P.rho0) * X(dzk)).v, P.rrho0 * rdzk).v : T(0));
+                const T Gu = (X(zt) * X(vhat) + Cu - dK - dP - Au + Vu + tau).v;
                 // ---- quasi-AB2, predictor, elimination sweep (S3, S4, S5) ----
-                const T Ghu = (X(c0) * X(Gu) - X(c1) * X(gm_uv.x)).v, Ghv = (X(c0) * X(Gv) - X(c1) * X(gm_uv.y)).v;
-                P.Guv[o] = mk2(Gu, Gv);
-                if (mu) {
-                    const T us = E::add(u_c, E::mul(P.dt, Ghu));
-                    aGU = (X(aGU) + X((double)dzk) * X((double)Ghu)).v; aSU = (X(aSU) + X((double)dzk) * X((double)us)).v;
-                    const T smk = k > tx1 ? P.sm_m[k] : T(0);
-                    dduv.x = E::div(E::add(us, E::mul(smk, dduv.x)), piv_u, piv_u);
-                }
-                if (mv) {
-                    const T vs2 = E::add(v_c, E::mul(P.dt, Ghv));
-                    aGV = (X(aGV) + X((double)dzk) * X((double)Ghv)).v; aSV = (X(aSV) + X((double)dzk) * X((double)vs2)).v;
-                    const T smk = k > ty1 ? P.sm_m[k] : T(0);
-                    dduv.y = E::div(E::add(vs2, E::mul(smk, dduv.y)), piv_v, piv_v);
-                }
-                P.duv[o] = dduv;
-                u_dn = u_c; v_dn = v_c;
+                const T Ghu = (X(c0) * X(Gu) - X(c1) * X(gm_u)).v;
+                ((T*)(P.Guv + oU))[0] = Gu;
+                const T us = E::add(u_c, E::mul(P.dt, Ghu));
+                aGU = (X(aGU) + X((double)dzk) * X((double)Ghu)).v; aSU = (X(aSU) + X((double)dzk) * X((double)us)).v;
+                const T smk = k > tx1 ? P.sm_m[k] : T(0);
+                ddu = E::div(E::add(us, E::mul(smk, ddu)), piv_u, piv_u);
+                ((T*)(P.duv + oU))[0] = ddu;
+                u_dn = u_c;
+            }
+            if constexpr (DO_M) if (wetV) {
+                const int cx = cV.cx, cy = cV.cy, ty1 = cV.t1, bo = cV.bo, by = cV.by;
+                const int qo = (cy + 1) * RX + cx + 1;
+                const T w_c1 = s_w1[qo], w_c0 = s_w0[qo];
+                const T dxFj = s_dxF[by], rdxFj = s_rdxF[by];
+                const T AzCj = s_AzC[by], AzCs = s_AzC[by - 1], AzFj = s_AzF[by], rAzFj = s_rAzF[by];
+                const T fFj = s_fF[by];
+                const T2 uvc = s_uv[bo];
+                const T u_c = uvc.x, v_c = uvc.y;
+                const T2 uv_s = s_uv[bo - BX], uv_e = s_uv[bo + 1], uv_se = s_uv[bo - BX + 1];
+                const T v_up = (k + 1 < nz) ? s_uv1[bo].y : T(0);
+                const T z00 = s_zeta[bo];
+                const T2 kdc = s_kd[qo];
+                const int pbo = (cy + 1) * C::PBX + cx + 4;
+                const Xv<T> half(T(0.5)), quart(T(0.25)), nuh(P.nu_h);
+                const T uhat = (quart * (X(uv_s.x) + X(u_c) + X(uv_se.x) + X(uv_e.x))).v;
+                const int ozv = 1 + (k >= cV.z2) + (k >= cV.z3);
+                const T z10 = s_zeta[bo + 1];
+                const T zt = ozv == 1 ? (uhat > T(0) ? z00 : z10)
+                                      : weno_face(s_zeta[bo - 2], s_zeta[bo - 1], z00, z10, s_zeta[bo + 2], s_zeta[bo + 3], uhat, ozv);
+                const Xv<T> Cv = X(fFj) * X(uhat);
+                const T2 kds = s_kd[qo - RX];
+                const Xv<T> dK = xdiv(X(kdc.x) - X(kds.x), dy, rdy);
+                const Xv<T> dP = xdiv(X((T)(s_p[pbo] - s_p[pbo - C::PBX])), dy, rdy);
+                const Xv<T> dlo((k >= 1 && k - 1 >= ty1) ? (X(v_c) - X(v_dn)).v : T(0));
+                const Xv<T> dhi((k + 1 <= nz - 1) ? (X(v_up) - X(v_c)).v : T(0));
+                const Xv<T> Whi = half * (X(AzCs) * X(s_w1[qo - RX]) + X(AzCj) * X(w_c1));
+                const Xv<T> Wlo = half * (X(AzCs) * X(s_w0[qo - RX]) + X(AzCj) * X(w_c0));
+                const Xv<T> Av = xdiv(half * (Whi * dhi + Wlo * dlo), (X(AzFj) * X(dzk)).v, rAzFj * rdzk);
+                const Xv<T> Vv = nuh * (xdiv(X(kdc.y) - X(kds.y), dy, rdy) + xdiv(X(z10) - X(z00), dxFj, rdxFj));
+                const Xv<T> tau((k == nz - 1) ? xdiv(X(P.tauy[cV.c]), (X(P.rho0) * X(dzk)).v, P.rrho0 * rdzk).v : T(0));
+                const T Gv = (-X(zt) * X(uhat) - Cv - dK - dP - Av + Vv + tau).v;
+                const T Ghv = (X(c0) * X(Gv) - X(c1) * X(gm_v)).v;
+                ((T*)(P.Guv + oV))[1] = Gv;
+                const T vs2 = E::add(v_c, E::mul(P.dt, Ghv));
+                aGV = (X(aGV) + X((double)dzk) * X((double)Ghv)).v; aSV = (X(aSV) + X((double)dzk) * X((double)vs2)).v;
+                const T smk = k > ty1 ? P.sm_m[k] : T(0);
+                ddv = E::div(E::add(vs2, E::mul(smk, ddv)), piv_v, piv_v);
+                ((T*)(P.duv + oV))[1] = ddv;
+                v_dn = v_c;
             }
             fz_bot = fz_top;
         }
         __syncthreads();                       // planes of level m - 1 are dead: refill the ring
         if (tid == 0 && m + C::DP <= nz) issue_group(m + C::DP, false);
     }
-    if (DO_M && cM.incol && cM.kb < nz) { P.GU[cM.c] = (T)aGU; P.GV[cM.c] = (T)aGV; P.SU[cM.c] = (T)aSU; P.SV[cM.c] = (T)aSV; }
+    if (DO_M && cU.incol && cU.t1 < nz) { P.GU[cU.c] = (T)aGU; P.SU[cU.c] = (T)aSU; }     // never-open faces keep their zeros
+    if (DO_M && cV.incol && cV.t1 < nz) { P.GV[cV.c] = (T)aGV; P.SV[cV.c] = (T)aSV; }
 }
 }  // namespace ocn
