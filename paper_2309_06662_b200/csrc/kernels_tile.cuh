@@ -218,8 +218,8 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
         };
         auto cell_emit = [&](int q, int rank) { s_cell[rank] = (unsigned short)q; };
         csort(NC, [&](int q) { return cell_key(q, 0); }, cell_emit, s_nc);
-        gT = s_cell[tid];
-        constexpr int VOFF = (NC / 3) & ~31;                          // v ranks start a third of the way into the CTA
+        constexpr int TOFF = NC / 2, VOFF = 3 * NC / 4;                   // faces run from thread 0 up, tracers from N/2, v from 3N/4, u from N-1 down
+        gT = s_cell[(tid + NC - TOFF) % NC];
         if constexpr (DO_M) {
             csort(NC, [&](int q) { return cell_key(q, 1); }, cell_emit, s_nc);
             gU = s_cell[NC - 1 - tid];
@@ -381,7 +381,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             if constexpr (DO_T) {
                 const T2* __restrict__ s_ts = (const T2*)(sm + C::O_TS + rts * C::PL2);
                 const int nface = s_nf[k];
-                for (int f = NT - 1 - tid; f < nface; f += NT) {
+                for (int f = tid; f < nface; f += NT) {
                     const uint2 d = s_fs[f];
                     const int b = d.x & 1023u, row = (d.x >> 10) & 15u, fid = d.x >> 16;
                     const bool isy = (d.x >> 14) & 1u;
