@@ -60,7 +60,9 @@ struct Tile {
     static constexpr int BX = TX + 8, BY = TY + 6;       // TMA box: origin (i0 - 4, j0 - 3)
     static constexpr int OX = 4, OY = 3;                 // box coordinates of tile cell (0, 0)
     static constexpr int DP = 2;                         // prefetch distance in levels
-    static constexpr int R_TS = DP + 5, R_UV = DP + 1, R_P = DP, NB = DP;
+    // ring lengths are powers of two (slot of level q = q & (R - 1): no loop-carried slot state); needed: DP + 5, DP + 1, DP, 3
+    static constexpr int R_TS = 8, R_UV = 4, R_P = 2, R_W = 4, NB = DP;
+    static_assert(DP + 5 <= R_TS && DP + 1 <= R_UV && DP <= R_P, "rings");
     static constexpr int RX = TX + 1, RY = TY + 1;       // tile + west/south ring (K, D, w) or + east/north edge (faces, masks)
     static constexpr int PL2 = rup128(BX * BY * (int)sizeof(T2)), PL1 = rup128(BX * BY * (int)sizeof(T)),
                          PLP = rup128((TX + 4) * (TY + 1) * 8);   // pressure planes: fp64, box (TX + 4) x (TY + 1), origin (i0 - 4, j0 - 1)
@@ -72,17 +74,18 @@ struct Tile {
     static constexpr int O_ZETA = O_P + (DO_M ? R_P : 0) * PLP;
     static constexpr int O_KD = O_ZETA + (DO_M ? 2 : 0) * PL1;                               // 2 x T2 (K, D) on RX x RY
     static constexpr int KDB = rup128(RX * RY * (int)sizeof(T2)), WB = rup128(RX * RY * (int)sizeof(T));
-    static constexpr int O_W = O_KD + 2 * KDB;                                  // 3 buffers of T on RX x RY
+    static constexpr int O_W = O_KD + 2 * KDB;                                  // R_W buffers of T on RX x RY (w at face f in slot f & 3)
     static constexpr int NFX = RX * TY, NFY = TX * RY, NF = NFX + NFY;        // west faces, then south faces
     static constexpr int FLB = rup128(NF * (int)sizeof(T2));
-    static constexpr int O_FLUX = O_W + 3 * WB;                                 // 2 x T2 per face
+    static constexpr int O_FLUX = O_W + R_W * WB;                                 // 2 x T2 per face
     static constexpr int O_M8 = O_FLUX + (DO_T ? 2 : 0) * FLB;                               // uint2 on RX x RY (not zero-filled from here on)
     static constexpr int O_MET = O_M8 + rup128(RX * RY * 8);                    // 9 row-metric arrays of BY + 1
     static constexpr int O_CELL = O_MET + rup128(9 * (BY + 1) * (int)sizeof(T)); // uint16: cells sorted by first wet level
     static constexpr int O_FS = O_CELL + rup128(NC * 2);                        // uint2: face descriptors sorted by first open level
     static constexpr int O_NC = O_FS + (DO_T ? rup128(NF * 8) : 0);                          // uint16[256]: active cells at level k
     static constexpr int O_NF = O_NC + 512;                                     // uint16[256]: active faces at level k
-    static constexpr int O_BAR = O_NF + 512;
+    static constexpr int O_DZ = O_NF + 512;                                     // T[256] dz, T[256] 1 / dz
+    static constexpr int O_BAR = O_DZ + 2 * 256 * (int)sizeof(T);
     static constexpr int SMEM = O_BAR + 128 + 128;                              // + alignment slack
 };
 
@@ -111,6 +114,8 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     T* const s_fF = s_AzC + (BY + 1);
     T* const s_rdxF = s_fF + (BY + 1);
     T* const s_AzF = s_rdxF + (BY + 1);
+    T* const s_dz = (T*)(sm + C::O_DZ);
+    T* const s_rdz = s_dz + 256;
     uint64_t* const bars = (uint64_t*)(sm + C::O_BAR);
     int& s_kmin = *(int*)(sm + C::O_BAR + 64);
 
@@ -256,6 +261,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             s_AzC[q] = P.AzC[r]; s_fF[q] = P.fF[r]; s_rdxF[q] = P.rdxF[r]; s_AzF[q] = P.AzF[r];
         }
     }
+    for (int q = tid; q < nz; q += NT) { s_dz[q] = P.dz[q]; s_rdz[q] = P.rdz[q]; }
     if (tid == 0) {
 #pragma unroll
         for (int b = 0; b < C::NB; ++b) mbar_init(&bars[b], 1);
@@ -280,7 +286,10 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
         if (m < nz) tma_load_plane(sm + C::O_UV + (m % C::R_UV) * C::PL2, &m_uv, bar, 2 * i0, j0, m);
         if (DO_M && m - 1 >= kmin) tma_load_plane(sm + C::O_P + ((m - 1) % C::R_P) * C::PLP, &m_p, bar, i0, j0 + 2, m - 1);
     };
-    if (tid == 0) {
+    // the TMA producer is a thread of the warp with the least part-A / part-B work on sparse levels (faces run from
+    // thread 0, tracers from N/2, v from 3N/4, u from N-1 down): its issue latency stays off the critical path
+    constexpr int PROD = (3 * NT / 8) & ~31;
+    if (tid == PROD) {
         issue_group(kmin, true);
 #pragma unroll
         for (int d = 1; d < C::DP; ++d) if (kmin + d <= nz) issue_group(kmin + d, false);
@@ -316,38 +325,43 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     T2 ddts = mk2(T(0), T(0));                           // eliminated right-hand sides of the level below
     double aGU = 0, aGV = 0, aSU = 0, aSV = 0;
 
-    // ring slots of level m, carried along the march (no integer division in the loop)
-    auto wrap = [](int x, int r) { return x >= r ? x - r : x; };
-    int rts = kmin % C::R_TS, ruv = kmin % C::R_UV, rp = kmin % C::R_P, r3 = kmin % 3;
-    for (int m = kmin; m <= nz; ++m, rts = wrap(rts + 1, C::R_TS), ruv = wrap(ruv + 1, C::R_UV), rp = wrap(rp + 1, C::R_P), r3 = wrap(r3 + 1, 3)) {
+    for (int m = kmin; m <= nz; ++m) {
         const int kB = m - 1;                                 // level of part B (phase 3) in this iteration
         const bool doB = kB >= kmin, wetT = DO_T && doB && kB >= cT.t1, wetU = DO_M && doB && kB >= cU.t1, wetV = DO_M && doB && kB >= cV.t1;
-        const long long oT = (long long)kB * sz + cT.c, oU = (long long)kB * sz + cU.c, oV = (long long)kB * sz + cV.c;
-        // AB2 history and pivots of level kB: issued now, consumed after part A
+        // AB2 history and pivots of level kB: issued now, consumed after part A.  A warp without an active cell or
+        // face at this level (most warps on sparsely wet levels) skips this and all of part B.
+        const bool anyB = __any_sync(0xffffffffu, wetT | wetU | wetV);
+        long long oT = 0, oU = 0, oV = 0;
         T2 gm_ts = mk2(T(0), T(0));
         T gm_u = 0, gm_v = 0;
         T piv_t = 1, piv_u = 1, piv_v = 1;
-        if (wetT) {
-            gm_ts = P.Gts[oT];
-            piv_t = sizeof(T) == 8 ? P.m_t[kB * nz + min(cT.t1, nz - 1)] : P.rm_t[kB * nz + min(cT.t1, nz - 1)];
-        }
-        if (wetU) {
-            gm_u = ((const T*)(P.Guv + oU))[0];
-            piv_u = sizeof(T) == 8 ? P.m_m[kB * nz + cU.t1] : P.rm_m[kB * nz + cU.t1];
-        }
-        if (wetV) {
-            gm_v = ((const T*)(P.Guv + oV))[1];
-            piv_v = sizeof(T) == 8 ? P.m_m[kB * nz + cV.t1] : P.rm_m[kB * nz + cV.t1];
+        if (anyB) {
+            const long long okB = (long long)kB * sz;
+            if (wetT) {
+                oT = okB + cT.c;
+                gm_ts = P.Gts[oT];
+                piv_t = sizeof(T) == 8 ? P.m_t[kB * nz + cT.t1] : P.rm_t[kB * nz + cT.t1];
+            }
+            if (wetU) {
+                oU = okB + cU.c;
+                gm_u = ((const T*)(P.Guv + oU))[0];
+                piv_u = sizeof(T) == 8 ? P.m_m[kB * nz + cU.t1] : P.rm_m[kB * nz + cU.t1];
+            }
+            if (wetV) {
+                oV = okB + cV.c;
+                gm_v = ((const T*)(P.Guv + oV))[1];
+                piv_v = sizeof(T) == 8 ? P.m_m[kB * nz + cV.t1] : P.rm_m[kB * nz + cV.t1];
+            }
         }
         mbar_wait(&bars[(m - kmin) % C::NB], (uint32_t)(((m - kmin) / C::NB) & 1));
 
         if (m < nz) {                                         // ---------------- part A: level k = m ----------------
             const int k = m;
-            const T dzk = P.dz[k];
-            const T2* __restrict__ s_uv = (const T2*)(sm + C::O_UV + ruv * C::PL2);
+            const T dzk = s_dz[k];
+            const T2* __restrict__ s_uv = (const T2*)(sm + C::O_UV + (k & (C::R_UV - 1)) * C::PL2);
             T* __restrict__ s_zeta = (T*)(sm + C::O_ZETA + (k & 1) * C::PL1);
             T2* __restrict__ s_kd = (T2*)(sm + C::O_KD + (k & 1) * C::KDB);
-            T* __restrict__ s_w1 = (T*)(sm + C::O_W + wrap(r3 + 1, 3) * C::WB);
+            T* __restrict__ s_w1 = (T*)(sm + C::O_W + ((k + 1) & (C::R_W - 1)) * C::WB);
             T2* __restrict__ s_flux = (T2*)(sm + C::O_FLUX + (k & 1) * C::FLB);
             // ================= phase 1: zeta, K, D, w[k+1] =================
             if constexpr (DO_M) {
@@ -379,7 +393,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             }
             // ================= phase 2: tracer face fluxes, each open face once =================
             if constexpr (DO_T) {
-                const T2* __restrict__ s_ts = (const T2*)(sm + C::O_TS + rts * C::PL2);
+                const T2* __restrict__ s_ts = (const T2*)(sm + C::O_TS + (k & (C::R_TS - 1)) * C::PL2);
                 const int nface = s_nf[k];
                 for (int f = tid; f < nface; f += NT) {
                     const uint2 d = s_fs[f];
@@ -401,14 +415,14 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 }
             }
         }
-        if (doB) {                                            // ---------------- part B: level k = m - 1 ----------------
+        if (anyB) {                                           // ---------------- part B: level k = m - 1 ----------------
             const int k = kB;
-            const T dzk = P.dz[k], rdzk = P.rdz[k];
-            const T2* __restrict__ s_uv = (const T2*)(sm + C::O_UV + wrap(ruv + C::R_UV - 1, C::R_UV) * C::PL2);
-            const T2* __restrict__ s_uv1 = (const T2*)(sm + C::O_UV + ruv * C::PL2);
-            const double* __restrict__ s_p = (const double*)(sm + C::O_P + wrap(rp + C::R_P - 1, C::R_P) * C::PLP);
-            const T* __restrict__ s_w0 = (const T*)(sm + C::O_W + wrap(r3 + 2, 3) * C::WB);
-            const T* __restrict__ s_w1 = (const T*)(sm + C::O_W + r3 * C::WB);
+            const T dzk = s_dz[k], rdzk = s_rdz[k];
+            const T2* __restrict__ s_uv = (const T2*)(sm + C::O_UV + (k & (C::R_UV - 1)) * C::PL2);
+            const T2* __restrict__ s_uv1 = (const T2*)(sm + C::O_UV + ((k + 1) & (C::R_UV - 1)) * C::PL2);
+            const double* __restrict__ s_p = (const double*)(sm + C::O_P + (k & (C::R_P - 1)) * C::PLP);
+            const T* __restrict__ s_w0 = (const T*)(sm + C::O_W + (k & (C::R_W - 1)) * C::WB);
+            const T* __restrict__ s_w1 = (const T*)(sm + C::O_W + ((k + 1) & (C::R_W - 1)) * C::WB);
             const T* __restrict__ s_zeta = (const T*)(sm + C::O_ZETA + (k & 1) * C::PL1);
             const T2* __restrict__ s_kd = (const T2*)(sm + C::O_KD + (k & 1) * C::KDB);
             const T2* __restrict__ s_flux = (const T2*)(sm + C::O_FLUX + (k & 1) * C::FLB);
@@ -423,9 +437,8 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 {
                 const int ozt = (k + 1 < nz) ? min(3, min(k + 1 - kb, nz - k - 1)) : 0;
                 if (ozt > 0) {
-                    const int rlo = wrap(rts + C::R_TS - 3, C::R_TS);      // slot of level k - 2 = m - 3
                     auto tsz = [&](int dk) -> T2 {           // plane of level k + dk, dk = -2 .. 3
-                        return ((const T2*)(sm + C::O_TS + wrap(rlo + dk + 2, C::R_TS) * C::PL2))[bo];
+                        return ((const T2*)(sm + C::O_TS + ((k + dk) & (C::R_TS - 1)) * C::PL2))[bo];
                     };
                     const T2 fv = weno_face2(tsz(-2), tsz(-1), tsz(0), tsz(1), tsz(2), tsz(3), w_c1, ozt);
                     fz_top.x = (X(w_c1) * X(AzCj) * X(fv.x)).v;
@@ -435,7 +448,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 // ---- tracers ----
                 const T2 fw = s_flux[cy * RX + cx], fe = s_flux[cy * RX + cx + 1];
                 const T2 fs = s_flux[C::NFX + cy * TX + cx], fn = s_flux[C::NFX + (cy + 1) * TX + cx];
-                const T2 tsc = ((const T2*)(sm + C::O_TS + wrap(rts + C::R_TS - 1, C::R_TS) * C::PL2))[bo];
+                const T2 tsc = ((const T2*)(sm + C::O_TS + (k & (C::R_TS - 1)) * C::PL2))[bo];
                 const T vol = (X(AzCj) * X(dzk)).v, rvol = rAzCj * rdzk;
                 T GT, GS;
                 if constexpr (sizeof(T) == 8) {    // the flux divergence summed in the order of DESIGN.md §3.7
@@ -546,7 +559,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             fz_bot = fz_top;
         }
         __syncthreads();                       // planes of level m - 1 are dead: refill the ring
-        if (tid == 0 && m + C::DP <= nz) issue_group(m + C::DP, false);
+        if (tid == PROD && m + C::DP <= nz) issue_group(m + C::DP, false);
     }
     if (DO_M && cU.incol && cU.t1 < nz) { P.GU[cU.c] = (T)aGU; P.SU[cU.c] = (T)aSU; }     // never-open faces keep their zeros
     if (DO_M && cV.incol && cV.t1 < nz) { P.GV[cV.c] = (T)aGV; P.SV[cV.c] = (T)aSV; }
