@@ -41,7 +41,9 @@ class ModelDesc(C.Structure):
                 ("g", C.c_double), ("alpha", C.c_double), ("beta_s", C.c_double),
                 ("T0", C.c_double), ("S0", C.c_double), ("rho0", C.c_double),
                 ("nu_h", C.c_double), ("kappa_h", C.c_double), ("nu_z", C.c_double),
-                ("kappa_z", C.c_double), ("filter_weights", C.POINTER(C.c_double))]
+                ("kappa_z", C.c_double), ("filter_weights", C.POINTER(C.c_double)),
+                ("closure", C.c_int), ("ri_nu0", C.c_double), ("ri_c", C.c_double), ("ri_kconv", C.c_double),
+                ("ri_n2c", C.c_double), ("ri_s2min", C.c_double)]
 
 
 class Fields(C.Structure):
@@ -59,6 +61,8 @@ def lib():
         _lib.ocn_ref_barotropic_raw.argtypes = [C.c_void_p, C.c_int, C.c_double]
         _lib.ocn_ref_implicit_column.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_ubyte),
                                                  C.c_double, C.POINTER(C.c_double)]
+        _lib.ocn_ref_implicit_column_var.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_ubyte),
+                                                     C.POINTER(C.c_double), C.POINTER(C.c_double)]
     return _lib
 
 
@@ -94,6 +98,16 @@ def implicit_column(z_faces, open_faces, dt_kappa, phi):
     op = np.ascontiguousarray(open_faces, dtype=np.uint8)
     x = np.array(phi, dtype=np.float64)
     _check(lib().ocn_ref_implicit_column(len(x), _dp(zf), _bp(op), float(dt_kappa), _dp(x)))
+    return x
+
+
+def implicit_column_var(z_faces, open_faces, dt_kappa_faces, phi):
+    zf = np.ascontiguousarray(z_faces, dtype=np.float64)
+    op = np.ascontiguousarray(open_faces, dtype=np.uint8)
+    dk = np.ascontiguousarray(dt_kappa_faces, dtype=np.float64)
+    x = np.array(phi, dtype=np.float64)
+    assert op.size == len(x) + 1 and dk.size == len(x) + 1
+    _check(lib().ocn_ref_implicit_column_var(len(x), _dp(zf), _bp(op), _dp(dk), _dp(x)))
     return x
 
 
@@ -179,6 +193,12 @@ class RefModel:
         nz, ny, nx = self.nz, self.ny, self.nx
         d = dict(p=np.zeros((nz, ny, nx)), U=np.zeros((ny, nx)), V=np.zeros((ny, nx)))
         _check(lib().ocn_ref_get_diagnostics(self.h, _dp(d["p"]), _dp(d["U"]), _dp(d["V"])))
+        return d
+
+    def mixing(self):
+        nz, ny, nx = self.nz, self.ny, self.nx
+        d = dict(nu=np.zeros((nz, ny, nx)), kappa=np.zeros((nz, ny, nx)))
+        _check(lib().ocn_ref_get_mixing(self.h, _dp(d["nu"]), _dp(d["kappa"])))
         return d
 
     def barotropic_raw(self, m, dtau):

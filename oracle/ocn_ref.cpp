@@ -150,6 +150,7 @@ struct ocn_ref_model {
     A3 Gu, Gv, GT, GS;              // G^n
     A3 Gu1, Gv1, GT1, GS1;          // G^{n-1}
     A3 eta, U, V, taux, tauy, Hu, Hv;   // 2-D (nl = 1)
+    A3 nuc, kapc;                   // closure = 1: nu, kappa at the bottom face of tracer cell (k, j, i)
     bool have_history = false;
 };
 
@@ -196,11 +197,13 @@ double weno(const double c[6], int order, double vel) {
 // DESIGN.md §3.8 step 4 — backward-Euler vertical diffusion of one column (Thomas, bottom-up)
 //   (1 + s+_k + s-_k) phi_k - s+_k phi_{k+1} - s-_k phi_{k-1} = phi*_k
 // ---------------------------------------------------------------------------------------------
+//   dtk[k], k = 0..nz: dt * kappa at the face below cell k (a constant array for closure 0,
+//   DESIGN.md §3.12 for closure 1); closed faces are not read
 void implicit_column(int nz, const double* dz, const double* dzc, const unsigned char* open,
-                     double dtk, double* phi, double* cp, double* dp) {
+                     const double* dtk, double* phi, double* cp, double* dp) {
     for (int k = 0; k < nz; ++k) {
-        const double sp = (k + 1 <= nz - 1 && open[k + 1]) ? dtk / (dz[k] * dzc[k + 1]) : 0.0;
-        const double sm = (k >= 1 && open[k]) ? dtk / (dz[k] * dzc[k]) : 0.0;
+        const double sp = (k + 1 <= nz - 1 && open[k + 1]) ? dtk[k + 1] / (dz[k] * dzc[k + 1]) : 0.0;
+        const double sm = (k >= 1 && open[k]) ? dtk[k] / (dz[k] * dzc[k]) : 0.0;
         const double b = 1.0 + sp + sm;
         const double lo = -sm, up = -sp;
         if (k == 0) {
@@ -266,6 +269,40 @@ void compute_p(ocn_ref_model& M) {
                              - 0.5 * (buoyancy(M, k + 1, j, i) + buoyancy(M, k, j, i)) * g.dzc[k + 1];
         }
     fill_halo(M.p, g.px, g.py);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Richardson-number-based vertical mixing with convective adjustment
+// (PAPER.md:114 names it, PAPER.md:78 stores it; the formula is a reading).  At the face below
+// tracer cell (k, j, i), k = 1..nz-1, open iff mw:
+//   N2 = (b_k - b_{k-1}) / dzc_k
+//   S2 = [ (du_w^2 + du_e^2)/2 + (dv_s^2 + dv_n^2)/2 ] / dzc_k^2,   du = u_k - u_{k-1} on the four faces of the column
+//   Ri = max(N2, 0) / (S2 + S2min),  f = 1 / (1 + c Ri)
+//   conv = kconv * min(1, max(-N2, 0) / N2c)          (continuous ramp instead of a switch)
+//   nu = nu_z + nu0 f^2 + conv,   kappa = kappa_z + nu0 f^3 + conv
+// Needs the halos of u, v of the current state.
+// ---------------------------------------------------------------------------------------------
+void compute_mixing(ocn_ref_model& M) {
+    const ocn_ref_grid& g = *M.g;
+    const ocn_ref_model_desc& d = M.d;
+#pragma omp parallel for schedule(static)
+    for (int j = 0; j < g.ny; ++j)
+        for (int i = 0; i < g.nx; ++i) {
+            M.nuc(0, j, i) = 0.0; M.kapc(0, j, i) = 0.0;
+            for (int k = 1; k < g.nz; ++k) {
+                if (!g.mw(k, j, i)) { M.nuc(k, j, i) = 0.0; M.kapc(k, j, i) = 0.0; continue; }
+                const double N2 = (buoyancy(M, k, j, i) - buoyancy(M, k - 1, j, i)) / g.dzc[k];
+                const double duw = M.u(k, j, i) - M.u(k - 1, j, i), due = M.u(k, j, i + 1) - M.u(k - 1, j, i + 1);
+                const double dvs = M.v(k, j, i) - M.v(k - 1, j, i), dvn = M.v(k, j + 1, i) - M.v(k - 1, j + 1, i);
+                const double S2 = (0.5 * (duw * duw + due * due) + 0.5 * (dvs * dvs + dvn * dvn)) / (g.dzc[k] * g.dzc[k]);
+                const double Ri = std::max(N2, 0.0) / (S2 + d.ri_s2min);
+                const double f = 1.0 / (1.0 + d.ri_c * Ri);
+                const double conv = d.ri_kconv * std::min(1.0, std::max(-N2, 0.0) / d.ri_n2c);
+                M.nuc(k, j, i) = d.nu_z + d.ri_nu0 * f * f + conv;
+                M.kapc(k, j, i) = d.kappa_z + d.ri_nu0 * f * f * f + conv;
+            }
+        }
+    fill_halo(M.nuc, g.px, g.py); fill_halo(M.kapc, g.px, g.py);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -439,6 +476,8 @@ void time_step(ocn_ref_model& M) {
     const ocn_ref_grid& g = *M.g;
     const int nx = g.nx, ny = g.ny, nz = g.nz;
     const double dt = M.d.dt;
+    // 0. vertical mixing coefficients of state n (closure 1)
+    if (M.d.closure == 1) compute_mixing(M);
     // 1. G^n from state n
     compute_tendencies(M, M.Gu, M.Gv, M.GT, M.GS);
     // 2. AB2 combination (Euler on the first step after set_fields)
@@ -452,7 +491,7 @@ void time_step(ocn_ref_model& M) {
     for (int f = 0; f < 4; ++f) {
 #pragma omp parallel for schedule(static)
         for (int j = 0; j < ny; ++j) {
-            std::vector<double> col(nz), cp(nz), dp(nz);
+            std::vector<double> col(nz), cp(nz), dp(nz), dtk(nz + 1);
             std::vector<unsigned char> open(nz + 1);
             for (int i = 0; i < nx; ++i) {
                 for (int k = 0; k < nz; ++k) {
@@ -469,9 +508,16 @@ void time_step(ocn_ref_model& M) {
                             : f == 1 ? (g.mv(k, j, i) && g.mv(k - 1, j, i))
                                      : g.mw(k, j, i);
                 }
-                // 4. implicit corrector
-                implicit_column(nz, g.dz.data(), g.dzc.data(), open.data(),
-                                dt * (f < 2 ? M.d.nu_z : M.d.kappa_z), col.data(), cp.data(), dp.data());
+                // 4. implicit corrector; dt * kappa per face: constant, or the closure's value at the
+                //    field's own vertical face (nu averaged from the two tracer columns that share the u / v face)
+                for (int k = 0; k <= nz; ++k) {
+                    if (M.d.closure != 1) { dtk[k] = dt * (f < 2 ? M.d.nu_z : M.d.kappa_z); continue; }
+                    if (!open[k]) { dtk[k] = 0.0; continue; }
+                    dtk[k] = f == 0 ? dt * (0.5 * (M.nuc(k, j, i - 1) + M.nuc(k, j, i)))
+                           : f == 1 ? dt * (0.5 * (M.nuc(k, j - 1, i) + M.nuc(k, j, i)))
+                                    : dt * M.kapc(k, j, i);
+                }
+                implicit_column(nz, g.dz.data(), g.dzc.data(), open.data(), dtk.data(), col.data(), cp.data(), dp.data());
                 for (int k = 0; k < nz; ++k) (*fld[f])(k, j, i) = col[k];
             }
         }
@@ -620,6 +666,9 @@ int ocn_ref_grid_destroy(ocn_ref_grid* g) { delete g; return 0; }
 int ocn_ref_model_create(const ocn_ref_grid* g, const ocn_ref_model_desc* d, ocn_ref_model** out) {
     if (!g || !d || !out) return fail("null argument");
     if (d->substeps < 1 || !(d->dt > 0)) return fail("bad dt / substeps");
+    if (d->closure != 0 && d->closure != 1) return fail("closure must be 0 or 1");
+    if (d->closure == 1 && !(d->ri_n2c > 0 && d->ri_s2min > 0 && d->ri_c >= 0 && d->ri_nu0 >= 0 && d->ri_kconv >= 0))
+        return fail("bad Ri closure parameters");
     ocn_ref_model* M = new ocn_ref_model();
     M->g = g; M->d = *d; M->d.filter_weights = nullptr;
     double ratio;
@@ -636,6 +685,7 @@ int ocn_ref_model_create(const ocn_ref_grid* g, const ocn_ref_model_desc* d, ocn
     for (A3* f : {&M->u, &M->v, &M->T, &M->S, &M->p, &M->Gu, &M->Gv, &M->GT, &M->GS,
                   &M->Gu1, &M->Gv1, &M->GT1, &M->GS1}) f->init(nx, ny, nz);
     M->w.init(nx, ny, nz + 1);
+    if (d->closure == 1) { M->nuc.init(nx, ny, nz); M->kapc.init(nx, ny, nz); }
     for (A3* f : {&M->eta, &M->U, &M->V, &M->taux, &M->tauy, &M->Hu, &M->Hv}) f->init(nx, ny, 1);
     for (int j = 0; j < ny; ++j)
         for (int i = 0; i < nx; ++i) {
@@ -741,7 +791,26 @@ int ocn_ref_implicit_column(int nz, const double* z_faces, const unsigned char* 
     std::vector<double> dz(nz), zc(nz), dzc(nz, 0.0), cp(nz), dp(nz);
     for (int k = 0; k < nz; ++k) { dz[k] = z_faces[k + 1] - z_faces[k]; zc[k] = 0.5 * (z_faces[k] + z_faces[k + 1]); }
     for (int k = 1; k < nz; ++k) dzc[k] = zc[k] - zc[k - 1];
+    const std::vector<double> dtkv(nz + 1, dtk);
+    implicit_column(nz, dz.data(), dzc.data(), open, dtkv.data(), phi, cp.data(), dp.data());
+    return 0;
+}
+
+int ocn_ref_implicit_column_var(int nz, const double* z_faces, const unsigned char* open, const double* dtk, double* phi) {
+    if (nz < 2 || !z_faces || !open || !dtk || !phi) return fail("bad argument");
+    std::vector<double> dz(nz), zc(nz), dzc(nz, 0.0), cp(nz), dp(nz);
+    for (int k = 0; k < nz; ++k) { dz[k] = z_faces[k + 1] - z_faces[k]; zc[k] = 0.5 * (z_faces[k] + z_faces[k + 1]); }
+    for (int k = 1; k < nz; ++k) dzc[k] = zc[k] - zc[k - 1];
     implicit_column(nz, dz.data(), dzc.data(), open, dtk, phi, cp.data(), dp.data());
+    return 0;
+}
+
+int ocn_ref_get_mixing(ocn_ref_model* M, double* nu, double* kappa) {
+    if (!M) return fail("null argument");
+    if (M->d.closure != 1) return fail("model has no Ri closure (closure = 0)");
+    compute_mixing(*M);
+    if (nu) copy_out(M->nuc, nu, M->g->nz);
+    if (kappa) copy_out(M->kapc, kappa, M->g->nz);
     return 0;
 }
 

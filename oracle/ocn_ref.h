@@ -39,6 +39,10 @@ typedef struct {
     double g, alpha, beta_s, T0, S0, rho0;
     double nu_h, kappa_h, nu_z, kappa_z;
     const double* filter_weights;   /* host, `substeps` entries, or NULL = DESIGN.md §3.9 default */
+    /* vertical mixing closure: 0 = constant nu_z / kappa_z,
+     * 1 = Richardson-number based with convective adjustment, nu_z / kappa_z as background */
+    int closure;
+    double ri_nu0, ri_c, ri_kconv, ri_n2c, ri_s2min;
 } ocn_ref_model_desc;
 
 typedef struct {
@@ -77,6 +81,14 @@ double ocn_ref_weno(const double c[6], int order, double vel);
  * open[k], k = 0..nz: 1 if the face below cell k is open (open[0], open[nz] ignored = closed). */
 int ocn_ref_implicit_column(int nz, const double* z_faces, const unsigned char* open,
                             double dt_kappa, double* phi);
+/* the same solve with a diffusivity per face: dt_kappa[k], k = 0..nz, is dt * kappa at the face
+ * below cell k (entries of closed faces are ignored) — DESIGN.md §3.12. */
+int ocn_ref_implicit_column_var(int nz, const double* z_faces, const unsigned char* open,
+                                const double* dt_kappa, double* phi);
+/* Ri-based closure of the CURRENT state: viscosity nu and diffusivity kappa at
+ * the bottom face of tracer cell (k, j, i), each nz*ny*nx (level 0 and closed faces hold 0);
+ * error if the model was created with closure = 0.  NULL = skip. */
+int ocn_ref_get_mixing(ocn_ref_model*, double* nu, double* kappa);
 /* default filter weights a_m (m = 1..M) and dtau/dt */
 int ocn_ref_filter_weights(int M, double* a, double* dtau_over_dt);
 /* tendencies G^n of the CURRENT state (recomputed, no side effects); each nz*ny*nx or NULL */

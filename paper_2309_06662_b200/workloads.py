@@ -17,7 +17,7 @@ Every workload is a plain dict:
     z_faces: float64[nz+1], increasing, z_faces[nz] == 0
     depth  : float64[ny, nx]  bottom depth in metres (>= 0, 0 = land)
     params : dict(precision, dt, substeps, chi, g, alpha, beta_s, T0, S0, rho0,
-                  nu_h, kappa_h, nu_z, kappa_z)
+                  nu_h, kappa_h, nu_z, kappa_z [, closure, ri_nu0, ri_c, ri_kconv, ri_n2c, ri_s2min])
     fields : dict(u, v, T, S [nz,ny,nx]; eta, tau_x, tau_y [ny,nx])  float64, already
              rounded to the run precision (the fp64 oracle receives the rounded values)
     steps  : number of baroclinic steps the configuration asks for
@@ -38,6 +38,16 @@ def _params(precision, dt, substeps, nu_h, kappa_h, beta_s=8e-4):
     return dict(precision=int(precision), dt=float(dt), substeps=int(substeps), chi=0.1,
                 g=GRAVITY, alpha=2e-4, beta_s=float(beta_s), T0=10.0, S0=35.0, rho0=1025.0,
                 nu_h=float(nu_h), kappa_h=float(kappa_h), nu_z=1e-4, kappa_z=1e-5)
+
+
+def with_ri_closure(wl, nu0=5e-3, c=5.0, kconv=0.1, n2c=1e-6, s2min=1e-10):
+    """Switches a workload to the Richardson-number-based vertical mixing closure (the one used in
+    all of the paper's runs; parameters of the reading in DESIGN.md §3.12): only the
+    parameter dict changes, nu_z / kappa_z become the background values."""
+    wl["params"].update(closure=1, ri_nu0=float(nu0), ri_c=float(c), ri_kconv=float(kconv), ri_n2c=float(n2c),
+                        ri_s2min=float(s2min))
+    wl["name"] = wl.get("name", "") + "+ri"
+    return wl
 
 
 def _round_to(precision, a):
