@@ -35,8 +35,13 @@ METRIC = "cell_updates_per_s"
 UNIT = "cell-updates/s"
 # algorithmic HBM bytes per wet cell-update of each stage: compulsory reads + writes; every array is
 # `word` bytes per value except the hydrostatic pressure, which is stored in fp64 in both precisions
-def stage_bytes(stage, word):
-    return {"tendency": 16 * word + 8, "backsub_correct_pressure": 8 * word + 8}.get(stage)
+# With the Ri closure (--closure ri): K4 reads uv, ts and writes (nu, kappa) = 6 words; K5 reads phi* (4) and
+# (nu, kappa) (2), writes d (4) and the super-diagonals (3) = 13 words; K3 reads the 3 super-diagonals on top.
+def stage_bytes(stage, word, closure=0):
+    b = {"tendency": 16 * word + 8, "backsub_correct_pressure": (8 + (3 if closure else 0)) * word + 8}
+    if closure:
+        b["vertical_mixing"] = 19 * word
+    return b.get(stage)
 # window of config 4 the oracle is timed on: (j0, j1, i0, i1)
 CPU_WINDOW = (500, 700, 1300, 1700)
 
@@ -48,6 +53,9 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--closure", default="const", choices=["const", "ri"],
+                    help="vertical mixing: constant coefficients (default, the north_star path) or the Ri-based closure "
+                         "of PAPER.md:114 (SURVEY 8f-1; DESIGN.md §3.12)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the end-to-end (host buffer) leg")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     return ap.parse_args()
@@ -66,7 +74,16 @@ def sypd(dt, sec_per_step):
 # ---------------------------------------------------------------------------------------------
 # CPU oracle leg (cpu_baseline and --impl reference)
 # ---------------------------------------------------------------------------------------------
-def oracle_sample(config):
+def oracle_sample(config, closure="const"):
+    from paper_2309_06662_b200 import workloads as W
+    wl, what = _oracle_sample(config)
+    if closure == "ri":
+        W.with_ri_closure(wl)
+        what += ", Ri closure"
+    return wl, what
+
+
+def _oracle_sample(config):
     from paper_2309_06662_b200 import workloads as W
     if config == 4:
         wl = W.config4(window=CPU_WINDOW, steps=1)
@@ -83,10 +100,10 @@ def oracle_sample(config):
     return wl, what
 
 
-def time_oracle(config, steps, warmup):
+def time_oracle(config, steps, warmup, closure="const"):
     import oracle
     oracle.build()
-    wl, what = oracle_sample(config)
+    wl, what = oracle_sample(config, closure)
     g = wl["grid"]
     cells = g["nx"] * g["ny"] * g["nz"]
     ref = oracle.RefModel(wl)
@@ -105,7 +122,7 @@ def run_reference(args):
     if rank != 0:
         return
     steps = min(args.steps, 3) if args.config >= 2 else args.steps
-    r = time_oracle(args.config, steps, min(args.warmup, 2))
+    r = time_oracle(args.config, steps, min(args.warmup, 2), args.closure)
     line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
             "steps": steps, "warmup": min(args.warmup, 2), "ms_per_step": 1e3 * r["sec_per_step"],
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -230,6 +247,9 @@ def run_ours(args):
 
     K, Wm = args.steps, max(args.warmup, 3)
     wl = W.make(args.config)
+    if args.closure == "ri":
+        W.with_ri_closure(wl)
+    ri = 1 if args.closure == "ri" else 0
     g, prm = wl["grid"], wl["params"]
     nx, ny, nz = g["nx"], g["ny"], g["nz"]
     cells = nx * ny * nz
@@ -276,13 +296,13 @@ def run_ours(args):
     peak, peak_src = measured_peak()
     word = 4 if prm["precision"] == 32 else 8
     dom = max(stages, key=lambda s: stages[s]["ms"])
-    dom_bytes = stage_bytes(dom, word)
+    dom_bytes = stage_bytes(dom, word, ri)
     roof = None
     stage_out = {}
     for s, v in stages.items():
         stage_out[s] = {"ms_per_step": v["ms"] / K, "launches_per_step": v["launches"] / K}
-        if stage_bytes(s, word):
-            stage_out[s]["algorithmic_gbs"] = stage_bytes(s, word) * nwet / (v["ms"] / K * 1e-3) / 1e9
+        if stage_bytes(s, word, ri) and v["launches"]:
+            stage_out[s]["algorithmic_gbs"] = stage_bytes(s, word, ri) * nwet / (v["ms"] / K * 1e-3) / 1e9
     if dom_bytes is not None:
         alg_bytes = dom_bytes * nwet
         ach = alg_bytes / (stages[dom]["ms"] / K * 1e-3) / 1e9
@@ -347,7 +367,7 @@ def run_ours(args):
     # ---- CPU oracle on this box's host cores (rank 0, N = 1 only) ----
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
-        r = time_oracle(args.config, 3 if args.config >= 2 else 5, 1)
+        r = time_oracle(args.config, 3 if args.config >= 2 else 5, 1, args.closure)
         cpu = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"]}
 
     if rank == 0:

@@ -64,6 +64,15 @@ typedef struct {
                                        default of DESIGN.md §3.9; copied at creation */
     int device;                     /* CUDA device ordinal */
     void* stream;                   /* cudaStream_t of the caller (e.g. torch's), NULL = default */
+    /* Vertical mixing closure ("Richardson-number-based parameterization for vertical
+     * mixing due to unresolved shear and convective turbulence"; its coefficient is the second stored
+     * diagnostic of PAPER.md:78; formulas: DESIGN.md §3.12).  closure = 0: constant nu_z / kappa_z.
+     * closure = 1: at every open vertical face of a tracer column
+     *   nu = nu_z + ri_nu0 f^2 + conv,  kappa = kappa_z + ri_nu0 f^3 + conv,  f = 1 / (1 + ri_c Ri),
+     *   Ri = max(N2, 0) / (S2 + ri_s2min),  conv = ri_kconv min(1, max(-N2, 0) / ri_n2c),
+     * evaluated from state n; ri_n2c, ri_s2min > 0, the others >= 0.  Costs three more 3-D arrays. */
+    int closure;
+    double ri_nu0, ri_c, ri_kconv, ri_n2c, ri_s2min;
 } ocn_model_desc;
 
 /* Allocates all device state (14 3-D arrays + 2-D arrays + tables) on `device`. */
@@ -102,13 +111,15 @@ ocn_status ocn_model_info(const ocn_model* model, int* launches_per_step, unsign
 
 /* Per-stage device timing (used by bench.py for the roofline of the dominant kernel).
  * Stages: 0 = K1 fused tendency / AB2 / elimination, 1 = barotropic sub-cycle (all M sub-steps +
- * finish; the sub-cycle runs BT_HALO sub-steps per launch on shared-memory tiles), 2 = K3 back-substitution / correction / pressure.  (w is recomputed on the fly inside
+ * finish; the sub-cycle runs BT_HALO sub-steps per launch on shared-memory tiles), 2 = K3 back-substitution / correction / pressure,
+ * 3 = vertical mixing closure (K4 mixing coefficients + K5 per-column elimination; runs between stages 1 and 2, no
+ * launches when closure = 0).  (w is recomputed on the fly inside
  * K1 and written out only when ocn_get_fields asks for it.)
  * While enabled, ocn_time_step launches the kernels of a step directly (no CUDA graph) and
  * records a CUDA event on the model's stream between stages.  ocn_profile_read synchronises
  * the stream and returns the milliseconds and kernel launches accumulated per stage since the
  * last reset (HOST arrays of OCN_NSTAGES entries; NULL = skip). */
-#define OCN_NSTAGES 3
+#define OCN_NSTAGES 4
 ocn_status ocn_profile_enable(ocn_model* model, int on);
 ocn_status ocn_profile_read(ocn_model* model, double* ms, long long* launches, int reset);
 const char* ocn_stage_name(int stage);
@@ -117,6 +128,10 @@ const char* ocn_stage_name(int stage);
  * prognostic field (nz*ny*nx each) and the barotropic transports U, V (ny*nx). */
 ocn_status ocn_get_debug(ocn_model* model, double* Gu, double* Gv, double* GT, double* GS,
                          double* U, double* V);
+
+/* closure = 1 only (OCN_ESTATE otherwise): the mixing coefficients of the CURRENT state (K4 is run on it), HOST double
+ * buffers nz*ny*nx, value at the bottom face of tracer cell (k, j, i), 0 on closed faces and at k = 0; NULL = skip. */
+ocn_status ocn_get_mixing(ocn_model* model, double* nu, double* kappa);
 
 const char* ocn_last_error(void);
 const char* ocn_version(void);

@@ -64,6 +64,13 @@ struct DevP {
     double g_d, alpha_d, beta_d, dT0_d, dS0_d, hz_top_d;   // fp64 copies for the pressure integral
     const double* dzc_d;
     T dtau;
+    // Ri-based vertical mixing closure, closure = 1 only: (nu, kappa) at the bottom face of
+    // tracer cell (k, j, i) as a pair array, and the modified super-diagonals of the per-column Thomas solves
+    int closure;
+    T2* nk;
+    T2* cpuv;
+    T* cpt;
+    double ri_nu0, ri_c, ri_kconv, ri_n2c, ri_s2min, nu_z_d, kappa_z_d;
 };
 
 template <class T>

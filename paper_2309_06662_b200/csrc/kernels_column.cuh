@@ -237,7 +237,8 @@ __global__ void __launch_bounds__(256) k_barotropic_finish(const DevP<T> P) {
 // The implicit operator conserves the column integral, so sum_k dz u** = sum_k dz u* (SU from
 // K1) and the correction (Ubar - SU) / Hu is known before the sweep.
 // ---------------------------------------------------------------------------------------------
-template <class T>
+// RI = true (closure 1): the modified super-diagonals come from the arrays K5 wrote instead of the tables.
+template <class T, bool RI>
 __global__ void __launch_bounds__(128, sizeof(T) == 8 ? 4 : 8) k_backsub_correct(const DevP<T> P) {
     typedef Ex<T> E;
     typedef typename Pair<T>::type T2;
@@ -273,14 +274,16 @@ __global__ void __launch_bounds__(128, sizeof(T) == 8 ? 4 : 8) k_backsub_correct
     };
     constexpr int NB = 3;                                  // levels whose loads are in flight together (measured best with 8 CTAs / SM)
     for (int k0 = nz - 1; k0 >= kg; k0 -= NB) {
-        T2 d_ts[NB], d_uv[NB];
+        T2 d_ts[NB], d_uv[NB], c_uv[NB];
+        T c_t[NB];
 #pragma unroll
         for (int q = 0; q < NB; ++q) {
             const int k = k0 - q;
-            d_ts[q] = mk2(T(0), T(0)); d_uv[q] = mk2(T(0), T(0));
+            d_ts[q] = mk2(T(0), T(0)); d_uv[q] = mk2(T(0), T(0)); c_uv[q] = mk2(T(0), T(0)); c_t[q] = T(0);
             if (k >= kb) {
                 d_ts[q] = P.dts[k * sz + c];
-                if (k >= kuv) d_uv[q] = P.duv[k * sz + c];
+                if (RI) c_t[q] = P.cpt[k * sz + c];
+                if (k >= kuv) { d_uv[q] = P.duv[k * sz + c]; if (RI) c_uv[q] = P.cpuv[k * sz + c]; }
             }
         }
 #pragma unroll
@@ -290,7 +293,7 @@ __global__ void __launch_bounds__(128, sizeof(T) == 8 ? 4 : 8) k_backsub_correct
             T2 ots = mk2(T(0), T(0));
             double op = 0.0;
             if (k >= kb) {
-                const T ck = cpt[k * nz];
+                const T ck = RI ? c_t[q] : cpt[k * nz];
                 xt = E::sub(d_ts[q].x, E::mul(ck, xt));                      // cp[nz-1] = 0
                 xs = E::sub(d_ts[q].y, E::mul(ck, xs));
                 const double b0 = buoyancy(P, xt, xs);
@@ -304,8 +307,8 @@ __global__ void __launch_bounds__(128, sizeof(T) == 8 ? 4 : 8) k_backsub_correct
             if (k >= kguv) {
                 const bool mu = k >= tx1, mv = k >= ty1;
                 T un = 0, vn = 0;
-                if (mu) { xu = E::sub(d_uv[q].x, E::mul(cpu[k * nz], xu)); un = xu + cu; }
-                if (mv) { xv = E::sub(d_uv[q].y, E::mul(cpv[k * nz], xv)); vn = xv + cv; }
+                if (mu) { xu = E::sub(d_uv[q].x, E::mul(RI ? c_uv[q].x : cpu[k * nz], xu)); un = xu + cu; }
+                if (mv) { xv = E::sub(d_uv[q].y, E::mul(RI ? c_uv[q].y : cpv[k * nz], xv)); vn = xv + cv; }
                 if (sizeof(T) == 8) { if (mu | mv) P.uv[o] = mk2(xu * T(mu), xv * T(mv)); }    // u**, corrected below
                 else put(P.uv, o, mk2(un, vn));
             }

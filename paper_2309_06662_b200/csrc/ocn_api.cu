@@ -13,6 +13,7 @@
 #include "grid_host.h"
 #include "kernels_column.cuh"
 #include "kernels_tile.cuh"
+#include "kernels_mixing.cuh"
 
 namespace {
 
@@ -55,8 +56,8 @@ struct ocn_model {
     bool profiling = false;
     std::vector<cudaEvent_t> ev_pool;   // OCN_NSTAGES + 1 events per profiled step
     size_t ev_used = 0;
-    double prof_ms[OCN_NSTAGES] = {0, 0, 0};
-    long long prof_launches[OCN_NSTAGES] = {0, 0, 0};
+    double prof_ms[OCN_NSTAGES] = {0, 0, 0, 0};
+    long long prof_launches[OCN_NSTAGES] = {0, 0, 0, 0};
 };
 
 namespace {
@@ -147,6 +148,13 @@ ocn_status build_model(ocn_model* M) {
     for (T2** f : f3) if ((s = dev_alloc(M, n3, f, true)) != OCN_OK) return s;
     if ((s = dev_alloc(M, n3, &P.p, true)) != OCN_OK) return s;
     if ((s = plane(n3 + n2, &P.w)) != OCN_OK) return s;
+    P.closure = M->d.closure; P.nk = nullptr; P.cpuv = nullptr; P.cpt = nullptr;
+    if (M->d.closure == 1) {                       // (nu, kappa) pairs and the per-column super-diagonals
+        if ((s = dev_alloc(M, n3, &P.nk, true)) != OCN_OK || (s = dev_alloc(M, n3, &P.cpuv, true)) != OCN_OK ||
+            (s = dev_alloc(M, n3, &P.cpt, true)) != OCN_OK) return s;
+    }
+    P.ri_nu0 = M->d.ri_nu0; P.ri_c = M->d.ri_c; P.ri_kconv = M->d.ri_kconv; P.ri_n2c = M->d.ri_n2c; P.ri_s2min = M->d.ri_s2min;
+    P.nu_z_d = M->d.nu_z; P.kappa_z_d = M->d.kappa_z;
     T** f2[] = {&P.eta[0], &P.eta[1], &P.U[0], &P.U[1], &P.V[0], &P.V[1], &P.etab, &P.Ub, &P.Vb, &P.GU, &P.GV,
                 &P.SU, &P.SV, &P.Hu, &P.Hv, &P.rHu, &P.rHv, &P.taux, &P.tauy};
     for (T** f : f2) if ((s = plane(n2, f)) != OCN_OK) return s;
@@ -179,7 +187,8 @@ ocn_status build_model(ocn_model* M) {
     // level kf; sub-diagonal sm[k], and per (k, kf) the pivot m, its reciprocal and the modified
     // super-diagonal cp, computed in fp64 exactly as the equations of DESIGN.md §3.8 step 4 are written
     for (int pass = 0; pass < 2; ++pass) {
-        const double dtk = M->d.dt * (pass == 0 ? M->d.nu_z : M->d.kappa_z);
+        // closure 1: identity tables (K1 then leaves the predictor phi* in the d arrays; K5 eliminates per column)
+        const double dtk = M->d.closure == 1 ? 0.0 : M->d.dt * (pass == 0 ? M->d.nu_z : M->d.kappa_z);
         std::vector<double> sm(nz, 0.0), cp((size_t)nz * nz, 0.0), mm((size_t)nz * nz, 1.0), rm((size_t)nz * nz, 1.0);
         for (int k = 1; k < nz; ++k) sm[k] = dtk / (g->dz[k] * g->dzc[k]);
         for (int kf = 0; kf < nz; ++kf) {
@@ -230,7 +239,7 @@ ocn_status build_model(ocn_model* M) {
     }
     CK(cudaMalloc(&M->stage, (size_t)(nz + 1) * g->ny * g->nx * sizeof(double)));
     M->bytes += (size_t)(nz + 1) * g->ny * g->nx * sizeof(double);
-    M->launches_per_step = (M->d.substeps + BT_HALO - 1) / BT_HALO + 3;
+    M->launches_per_step = (M->d.substeps + BT_HALO - 1) / BT_HALO + 3 + (M->d.closure == 1 ? 2 : 0);
     // TMA descriptors: box origin (i0 - 4, j0 - 3), so the map starts 4 elements before (row -3, i = 0)
     {
         typedef ocn::Tile<T, TILE_X, TILE_Y, 0> C;
@@ -261,9 +270,10 @@ ocn_status prof_flush(ocn_model* M) {           // fold recorded events into the
     CK(cudaStreamSynchronize(M->stream));
     for (size_t q = 0; q + OCN_NSTAGES < M->ev_used + 1 && q < M->ev_used; q += OCN_NSTAGES + 1)
         for (int s = 0; s < OCN_NSTAGES; ++s) {
+            static const int in_time_order[OCN_NSTAGES] = {0, 1, 3, 2};   // the closure stage runs before K3
             float ms = 0.f;
             CK(cudaEventElapsedTime(&ms, M->ev_pool[q + s], M->ev_pool[q + s + 1]));
-            M->prof_ms[s] += ms;
+            M->prof_ms[in_time_order[s]] += ms;
         }
     M->ev_used = 0;
     return OCN_OK;
@@ -323,7 +333,15 @@ ocn_status launch_step(ocn_model* M, bool euler) {
     }
     ocn::k_barotropic_finish<T><<<grid2(g, b2), b2, 0, M->stream>>>(P);
     MARK(1, (M->d.substeps + BT_HALO - 1) / BT_HALO + 1);
-    ocn::k_backsub_correct<T><<<grid2(g, bc), bc, 0, M->stream>>>(P);
+    if (M->d.closure == 1) {                       // K4 on state n (still intact), K5 on K1's predictor
+        ocn::k_ri_mixing<T><<<grid2(g, bc), bc, 0, M->stream>>>(P);
+        ocn::k_ri_eliminate<T><<<grid2(g, bc), bc, 0, M->stream>>>(P);
+        MARK(3, 2);
+        ocn::k_backsub_correct<T, true><<<grid2(g, bc), bc, 0, M->stream>>>(P);
+    } else {
+        MARK(3, 0);
+        ocn::k_backsub_correct<T, false><<<grid2(g, bc), bc, 0, M->stream>>>(P);
+    }
     MARK(2, 1);
 #undef MARK
     CK(cudaGetLastError());
@@ -447,6 +465,19 @@ ocn_status get_debug_t(ocn_model* M, double* Gu, double* Gv, double* GT, double*
     return OCN_OK;
 }
 
+template <class T>
+ocn_status get_mixing_t(ocn_model* M, double* nu, double* kappa) {
+    ocn::DevP<T>& P = params<T>(M);
+    const int nz = M->g->nz;
+    const dim3 bc(32, 4);
+    ocn::k_ri_mixing<T><<<grid2(M->g, bc), bc, 0, M->stream>>>(P);
+    CK(cudaGetLastError());
+    ocn_status s;
+    if (nu && (s = get_one<T, double>(M, nu, (T*)P.nk, nz, 5, false, 2)) != OCN_OK) return s;
+    if (kappa && (s = get_one<T, double>(M, kappa, (T*)P.nk + 1, nz, 5, false, 2)) != OCN_OK) return s;
+    return OCN_OK;
+}
+
 }  // namespace
 
 // =================================================================================================
@@ -504,6 +535,9 @@ ocn_status ocn_model_create(const ocn_grid* g, const ocn_model_desc* d, ocn_mode
     if (d->precision != 32 && d->precision != 64) return fail(OCN_EINVAL, "precision must be 32 or 64");
     if (!(d->dt > 0) || d->substeps < 1) return fail(OCN_EINVAL, "dt must be > 0 and substeps >= 1");
     if (!(d->rho0 > 0)) return fail(OCN_EINVAL, "rho0 must be > 0");
+    if (d->closure != 0 && d->closure != 1) return fail(OCN_EINVAL, "closure must be 0 (constant) or 1 (Ri-based)");
+    if (d->closure == 1 && !(d->ri_n2c > 0 && d->ri_s2min > 0 && d->ri_c >= 0 && d->ri_nu0 >= 0 && d->ri_kconv >= 0))
+        return fail(OCN_EINVAL, "Ri closure: ri_n2c, ri_s2min must be > 0 and ri_c, ri_nu0, ri_kconv >= 0");
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
         return fail(OCN_ECUDA, "no CUDA device: libocn has no CPU fallback");
@@ -619,7 +653,7 @@ ocn_status ocn_profile_read(ocn_model* M, double* ms, long long* launches, int r
 }
 
 const char* ocn_stage_name(int stage) {
-    static const char* names[OCN_NSTAGES] = {"tendency", "barotropic", "backsub_correct_pressure"};
+    static const char* names[OCN_NSTAGES] = {"tendency", "barotropic", "backsub_correct_pressure", "vertical_mixing"};
     return (stage >= 0 && stage < OCN_NSTAGES) ? names[stage] : "";
 }
 
@@ -627,6 +661,13 @@ ocn_status ocn_get_debug(ocn_model* M, double* Gu, double* Gv, double* GT, doubl
     if (!M) return fail(OCN_EINVAL, "null model");
     CK(cudaSetDevice(M->d.device));
     return M->prec == 32 ? get_debug_t<float>(M, Gu, Gv, GT, GS, U, V) : get_debug_t<double>(M, Gu, Gv, GT, GS, U, V);
+}
+
+ocn_status ocn_get_mixing(ocn_model* M, double* nu, double* kappa) {
+    if (!M) return fail(OCN_EINVAL, "null model");
+    if (M->d.closure != 1) return fail(OCN_ESTATE, "model was created with closure = 0");
+    CK(cudaSetDevice(M->d.device));
+    return M->prec == 32 ? get_mixing_t<float>(M, nu, kappa) : get_mixing_t<double>(M, nu, kappa);
 }
 
 }  // extern "C"

@@ -31,7 +31,9 @@ class ocn_model_desc(C.Structure):
                 ("g", C.c_double), ("alpha", C.c_double), ("beta_s", C.c_double), ("T0", C.c_double),
                 ("S0", C.c_double), ("rho0", C.c_double), ("nu_h", C.c_double), ("kappa_h", C.c_double),
                 ("nu_z", C.c_double), ("kappa_z", C.c_double), ("filter_weights", C.POINTER(C.c_double)),
-                ("device", C.c_int), ("stream", C.c_void_p)]
+                ("device", C.c_int), ("stream", C.c_void_p),
+                ("closure", C.c_int), ("ri_nu0", C.c_double), ("ri_c", C.c_double), ("ri_kconv", C.c_double),
+                ("ri_n2c", C.c_double), ("ri_s2min", C.c_double)]
 
 
 class ocn_fields(C.Structure):
@@ -41,8 +43,8 @@ class ocn_fields(C.Structure):
 EXPORTS = ["ocn_grid_create", "ocn_grid_destroy", "ocn_model_create", "ocn_model_destroy", "ocn_set_fields",
            "ocn_time_step", "ocn_get_fields", "ocn_synchronize", "ocn_get_masks", "ocn_model_info",
            "ocn_get_debug", "ocn_last_error", "ocn_version", "ocn_profile_enable", "ocn_profile_read",
-           "ocn_stage_name"]
-NSTAGES = 3
+           "ocn_stage_name", "ocn_get_mixing"]
+NSTAGES = 4
 
 
 def lib():
@@ -66,6 +68,7 @@ def lib():
         L.ocn_get_masks.argtypes = [vp] + [vp] * 6
         L.ocn_model_info.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_ulonglong)]
         L.ocn_get_debug.argtypes = [vp] + [vp] * 6
+        L.ocn_get_mixing.argtypes = [vp, vp, vp]
         L.ocn_profile_enable.argtypes = [vp, C.c_int]
         L.ocn_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong), C.c_int]
         L.ocn_stage_name.restype = C.c_char_p
@@ -178,6 +181,12 @@ class Model:
         d = {k: np.zeros((nz, ny, nx)) for k in ("Gu", "Gv", "GT", "GS")}
         d["U"] = np.zeros((ny, nx)); d["V"] = np.zeros((ny, nx))
         _check(lib().ocn_get_debug(self.h, *[_ptr(d[k]) for k in ("Gu", "Gv", "GT", "GS", "U", "V")]))
+        return d
+
+    def mixing(self):
+        nz, ny, nx = self.nz, self.ny, self.nx
+        d = dict(nu=np.zeros((nz, ny, nx)), kappa=np.zeros((nz, ny, nx)))
+        _check(lib().ocn_get_mixing(self.h, _ptr(d["nu"]), _ptr(d["kappa"])))
         return d
 
     def close(self):

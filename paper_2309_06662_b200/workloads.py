@@ -40,7 +40,7 @@ def _params(precision, dt, substeps, nu_h, kappa_h, beta_s=8e-4):
                 nu_h=float(nu_h), kappa_h=float(kappa_h), nu_z=1e-4, kappa_z=1e-5)
 
 
-def with_ri_closure(wl, nu0=5e-3, c=5.0, kconv=0.1, n2c=1e-6, s2min=1e-10):
+def with_ri_closure(wl, nu0=5e-3, c=5.0, kconv=0.1, n2c=1e-5, s2min=1e-10):
     """Switches a workload to the Richardson-number-based vertical mixing closure (the one used in
     all of the paper's runs; parameters of the reading in DESIGN.md §3.12): only the
     parameter dict changes, nu_z / kappa_z become the background values."""

@@ -1,0 +1,117 @@
+"""Parity of the CUDA path with the Ri-based vertical mixing closure (closure = 1: K4 mixing coefficients, K5
+per-column elimination, K3 reading the stored super-diagonals) against the oracle."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2309_06662_b200 import build as ocn_build
+from paper_2309_06662_b200 import ocn
+from paper_2309_06662_b200 import workloads as W
+from util import box, clone, rel_linf
+
+pytestmark = pytest.mark.gpu
+TOL = {64: 1e-11, 32: 2e-4}
+FIELDS = ("u", "v", "w", "eta", "T", "S")
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    ocn_build.build()
+
+
+def _stir(wl, seed=3, unstable_top=0):
+    """a sheared flow so that Ri spans its range, and optionally cold water on top (convective ramp active)"""
+    rng = np.random.default_rng(seed)
+    nz = wl["grid"]["nz"]
+    prof = np.linspace(0.0, 1.0, nz)[:, None, None] ** 2
+    prec = wl["params"]["precision"]
+    wl["fields"]["u"] = W._round_to(prec, wl["fields"]["u"] + 0.3 * prof * (1 + 0.2 * rng.standard_normal(wl["fields"]["u"].shape)))
+    wl["fields"]["v"] = W._round_to(prec, wl["fields"]["v"] - 0.2 * prof * (1 + 0.2 * rng.standard_normal(wl["fields"]["v"].shape)))
+    if unstable_top:
+        wl["fields"]["T"][-unstable_top:] = W._round_to(prec, wl["fields"]["T"][-unstable_top:] - 1.5)
+    return wl
+
+
+def _run_both(wl, stops):
+    ref, gpu = oracle.RefModel(wl), ocn.Model(wl)
+    done, errs = 0, {}
+    for stop in stops:
+        ref.step(stop - done); gpu.time_step(stop - done); done = stop
+        a, b = gpu.get_fields(), ref.get_fields()
+        errs = {n: rel_linf(a[n], b[n]) for n in FIELDS}
+        bad = {n: e for n, e in errs.items() if not e <= TOL[wl["params"]["precision"]]}
+        assert not bad, (wl["name"], stop, errs)
+        assert all(np.isfinite(a[n]).all() for n in FIELDS)
+    gpu.close()
+    return errs
+
+
+def test_mixing_coefficients_match_the_oracle_fp64_bitwise_and_fp32_rounded():
+    for prec in (64, 32):
+        wl = _stir(W.with_ri_closure(W.config2(nx=96, ny=40, nz=12, steps=1, precision=prec)), unstable_top=2)
+        ref, gpu = oracle.RefModel(wl), ocn.Model(wl)
+        a, b = gpu.mixing(), ref.mixing()
+        assert b["nu"].max() > 10 * b["nu"][b["nu"] > 0].min()          # the closure is active, not just the background
+        for n in ("nu", "kappa"):
+            if prec == 64:
+                assert np.array_equal(a[n], b[n]), n
+            else:
+                assert np.array_equal(a[n] == 0.0, b[n] == 0.0), n      # closed faces: exact zeros at the same places
+                assert rel_linf(a[n], b[n]) < 1e-5, n
+        gpu.close()
+
+
+def test_closure_requires_closure_model():
+    gpu = ocn.Model(W.config0(nx=8, ny=8, nz=4))
+    with pytest.raises(RuntimeError):
+        gpu.mixing()
+    bad = W.with_ri_closure(W.config0(nx=8, ny=8, nz=4), n2c=0.0)
+    with pytest.raises(RuntimeError):
+        ocn.Model(bad)
+
+
+def test_closure_config0_periodic_fp64():
+    wl = _stir(W.with_ri_closure(W.config0()))
+    _run_both(wl, [1, 2, 10])
+
+
+def test_closure_ragged_basin_with_walls_fp64():
+    wl = _stir(W.with_ri_closure(W.config1(nx=45, ny=37, nz=11, steps=12)), unstable_top=2)
+    _run_both(wl, [1, 12])
+
+
+def test_closure_latlon_reduced_fp64():
+    wl = _stir(W.with_ri_closure(W.config2(nx=360, ny=150, nz=50, steps=10)), unstable_top=3)
+    _run_both(wl, [1, 10])
+
+
+def test_closure_latlon_reduced_fp32():
+    wl = _stir(W.with_ri_closure(W.config3(nx=360, ny=150, nz=50, steps=10)), unstable_top=3)
+    _run_both(wl, [1, 10])
+
+
+def test_closure_config4_window_fp32():
+    wl = W.with_ri_closure(W.config4(window=(500, 600, 1300, 1500), steps=10))
+    _run_both(wl, [1, 10])
+
+
+def test_closure_with_zero_amplitudes_equals_constant_coefficient_path_on_gpu():
+    # K4 + K5 + K3<RI> against the table-driven K1 / K3 of the default path: same numbers in fp64
+    wl = W.config2(nx=96, ny=40, nz=12, steps=3)
+    w2 = W.with_ri_closure(clone(wl), nu0=0.0, kconv=0.0)
+    a, b = ocn.Model(wl), ocn.Model(w2)
+    a.time_step(3); b.time_step(3)
+    fa, fb = a.get_fields(), b.get_fields()
+    for n in FIELDS:
+        assert np.array_equal(fa[n], fb[n]), n
+
+
+def test_closure_stage_is_timed():
+    wl = W.with_ri_closure(W.config3(nx=96, ny=40, nz=12, steps=3))
+    gpu = ocn.Model(wl)
+    gpu.time_step(1)
+    gpu.profile_enable(True)
+    gpu.time_step(3)
+    prof = gpu.profile_read()
+    assert prof["vertical_mixing"]["launches"] == 6 and prof["vertical_mixing"]["ms"] > 0
+    assert gpu.info()["launches_per_step"] == prof["tendency"]["launches"] // 3 + prof["barotropic"]["launches"] // 3 + 3

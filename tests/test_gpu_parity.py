@@ -300,9 +300,10 @@ def test_profiling_path_gives_the_same_bits_and_sane_times():
     fb = b.get_fields(); b.close()
     for n in FIELDS:
         assert np.array_equal(fa[n], fb[n]), n                    # graph replay and direct launches agree bit for bit
-    assert set(prof) == {"tendency", "barotropic", "backsub_correct_pressure"}
+    assert set(prof) == {"tendency", "barotropic", "backsub_correct_pressure", "vertical_mixing"}
+    assert prof["vertical_mixing"]["launches"] == 0                     # closure 0: the stage is empty
     assert prof["tendency"]["launches"] == 4 and prof["barotropic"]["launches"] == 4 * (30 // 6 + 1)
-    assert all(v["ms"] > 0 for v in prof.values())
+    assert all(v["ms"] > 0 for n, v in prof.items() if n != "vertical_mixing")
 
 
 def test_bad_arguments_on_the_gpu_side():
