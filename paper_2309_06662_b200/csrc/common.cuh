@@ -50,6 +50,7 @@ struct DevP {
     T dy, rdy;
     // vertical grid
     const T *dz, *rdz, *dzc;       // dzc[k] = zc[k] - zc[k-1] (k >= 1)
+    const T *rdzc;                 // 1 / dzc[k] (k >= 1; entry 0 is 1)
     T hz_top;                      // zf[nz] - zc[nz-1]
     // Thomas tables, bottom-up elimination in the oracle's order.  Momentum (nu_z)
     // and tracers (kappa_z).  sm[k]: sub-diagonal s^-_k (open face below); cp/m/rm are indexed

@@ -72,7 +72,7 @@ __global__ void __launch_bounds__(128) k_ri_mixing(const DevP<T> P) {
                     const V kap = V(P.kappa_z_d) + V(P.ri_nu0) * f * f * f + conv;
                     out = mk2((T)nu.v, (T)kap.v);
                 } else {                                    // fp32: difference the stored tracers first (exact for neighbours in
-                    const float rdzc = 1.0f / (float)P.dzc[k];   // a column), then the same formulas in single precision
+                    const float rdzc = (float)P.rdzc[k];         // a column), then the same formulas in single precision
                     const float N2 = (float)P.g * ((float)P.alpha * ((float)q[r].x - (float)t0) - (float)P.beta_s * ((float)q[r].y - (float)s0)) * rdzc;
                     const float duw = (float)uw1 - (float)uw0, due = (float)ue1 - (float)ue0, dvs = (float)vs1 - (float)vs0, dvn = (float)vn1 - (float)vn0;
                     const float S2 = 0.5f * ((duw * duw + due * due) + (dvs * dvs + dvn * dvn)) * rdzc * rdzc;
@@ -103,16 +103,28 @@ __global__ void __launch_bounds__(128) k_ri_mixing(const DevP<T> P) {
 template <class T>
 struct ThomasRow {
     T cp, d0, d1;                                // modified super-diagonal and two right-hand sides that share it
-    __device__ __forceinline__ void step(bool first, T dtk_lo, T dtk_hi, bool has_hi, T dzk, T dzc_lo, T dzc_hi, T phi0, T phi1) {
-        typedef Xv<T> V;
-        const V sp = has_hi ? V(dtk_hi) / (V(dzk) * V(dzc_hi)) : V(T(0));
-        const V sm = first ? V(T(0)) : V(dtk_lo) / (V(dzk) * V(dzc_lo));
-        const V b = V(T(1)) + sp + sm;
-        const V lo = -sm, up = -sp;
-        const V m = first ? b : b - lo * V(cp);
-        d0 = first ? (V(phi0) / m).v : ((V(phi0) - lo * V(d0)) / m).v;
-        d1 = first ? (V(phi1) / m).v : ((V(phi1) - lo * V(d1)) / m).v;
-        cp = (up / m).v;
+    // rz = 1 / dz_k, rc_lo = 1 / dzc_k, rc_hi = 1 / dzc_{k+1}: used by the fp32 form only
+    __device__ __forceinline__ void step(bool first, T dtk_lo, T dtk_hi, bool has_hi, T dzk, T dzc_lo, T dzc_hi,
+                                         T rz, T rc_lo, T rc_hi, T phi0, T phi1) {
+        if (sizeof(T) == 8) {                    // fp64: the equations as written, true divisions (bit-identical to the oracle)
+            typedef Xv<T> V;
+            const V sp = has_hi ? V(dtk_hi) / (V(dzk) * V(dzc_hi)) : V(T(0));
+            const V sm = first ? V(T(0)) : V(dtk_lo) / (V(dzk) * V(dzc_lo));
+            const V b = V(T(1)) + sp + sm;
+            const V lo = -sm, up = -sp;
+            const V m = first ? b : b - lo * V(cp);
+            d0 = first ? (V(phi0) / m).v : ((V(phi0) - lo * V(d0)) / m).v;
+            d1 = first ? (V(phi1) / m).v : ((V(phi1) - lo * V(d1)) / m).v;
+            cp = (up / m).v;
+        } else {                                 // fp32: reciprocal multiplies, one division per row
+            const T sp = has_hi ? dtk_hi * rz * rc_hi : T(0);
+            const T sm = first ? T(0) : dtk_lo * rz * rc_lo;
+            const T m = T(1) + sp + sm + sm * cp;                     // cp of the first row is 0 * sm
+            const T rm = T(1) / m;
+            d0 = (phi0 + sm * d0) * rm;
+            d1 = (phi1 + sm * d1) * rm;
+            cp = -sp * rm;
+        }
     }
 };
 
@@ -179,13 +191,14 @@ __global__ void __launch_bounds__(128) k_ri_eliminate(const DevP<T> P) {
                 if (k >= ty1) kv_hi = (V(P.dt) * (V(T(0.5)) * (V(nu_s[r]) + V(nu_hi[r])))).v;
             }
             const T dzk = P.dz[k], dzc_lo = k > 0 ? P.dzc[k] : T(1), dzc_hi = has_hi ? P.dzc[k + 1] : T(1);
-            rt.step(k == kb, kt_lo, kt_hi, has_hi, dzk, dzc_lo, dzc_hi, pt[r].x, pt[r].y);
+            const T rz = P.rdz[k], rc_lo = k > 0 ? P.rdzc[k] : T(1), rc_hi = has_hi ? P.rdzc[k + 1] : T(1);
+            rt.step(k == kb, kt_lo, kt_hi, has_hi, dzk, dzc_lo, dzc_hi, rz, rc_lo, rc_hi, pt[r].x, pt[r].y);
             P.dts[o] = mk2(rt.d0, rt.d1);
             P.cpt[o] = rt.cp;
             if (k >= kguv) {
                 T2 dout = mk2(T(0), T(0)), cout = mk2(T(0), T(0));
-                if (k >= tx1) { ru.step(k == tx1, ku_lo, ku_hi, has_hi, dzk, dzc_lo, dzc_hi, pm[r].x, T(0)); dout.x = ru.d0; cout.x = ru.cp; }
-                if (k >= ty1) { rv.step(k == ty1, kv_lo, kv_hi, has_hi, dzk, dzc_lo, dzc_hi, pm[r].y, T(0)); dout.y = rv.d0; cout.y = rv.cp; }
+                if (k >= tx1) { ru.step(k == tx1, ku_lo, ku_hi, has_hi, dzk, dzc_lo, dzc_hi, rz, rc_lo, rc_hi, pm[r].x, T(0)); dout.x = ru.d0; cout.x = ru.cp; }
+                if (k >= ty1) { rv.step(k == ty1, kv_lo, kv_hi, has_hi, dzk, dzc_lo, dzc_hi, rz, rc_lo, rc_hi, pm[r].y, T(0)); dout.y = rv.d0; cout.y = rv.cp; }
                 P.duv[o] = dout;
                 P.cpuv[o] = cout;
             }

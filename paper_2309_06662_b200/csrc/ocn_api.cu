@@ -177,6 +177,11 @@ ocn_status build_model(ocn_model* M) {
         (s = upload(M, recip(g->dz), &P.rdz)) != OCN_OK || (s = upload(M, g->dzc, &P.dzc)) != OCN_OK)
         return s;
     {
+        std::vector<double> r(g->dzc.size(), 1.0);
+        for (size_t q = 1; q < r.size(); ++q) r[q] = 1.0 / g->dzc[q];
+        if ((s = upload(M, r, &P.rdzc)) != OCN_OK) return s;
+    }
+    {
         const double* dzc_d = nullptr;
         if ((s = upload<double>(M, g->dzc, &dzc_d)) != OCN_OK) return s;
         P.dzc_d = dzc_d;
