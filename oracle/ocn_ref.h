@@ -4,7 +4,9 @@
  * bit-identical) fp64 restatement of the discrete equations in DESIGN.md §3, written from
  * the paper's problem statement (PAPER.md:84 hydrostatic Boussinesq / finite volume / C-grid
  * / IMEX AB2 / backward-Euler tridiagonal; PAPER.md:86 WENO advection
- * split-explicit barotropic sub-cycling; PAPER.md:102-104 lat-lon domain with bathymetry).
+ * split-explicit barotropic sub-cycling; PAPER.md:102-104 lat-lon domain with bathymetry;
+ * PAPER.md:78, 114 Ri-based vertical mixing).  Parity unpinned: nothing
+ * (pins: tests/test_oracle_*.py, listed in DESIGN.md §5).
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
  * load it.  It shares no code, header, table or helper with the CUDA library (libocn).
  *

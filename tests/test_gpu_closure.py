@@ -115,3 +115,15 @@ def test_closure_stage_is_timed():
     prof = gpu.profile_read()
     assert prof["vertical_mixing"]["launches"] == 6 and prof["vertical_mixing"]["ms"] > 0
     assert gpu.info()["launches_per_step"] == prof["tendency"]["launches"] // 3 + prof["barotropic"]["launches"] // 3 + 3
+
+
+def test_closure_fp64_is_bit_identical_to_the_oracle():
+    # K4 / K5 / K3<RI> keep the association of DESIGN.md §3.12 and §3.8-4 in non-contracted IEEE operations
+    for wl in (_stir(W.with_ri_closure(W.config0(nx=24, ny=20, nz=8))),
+               _stir(W.with_ri_closure(W.config2(nx=96, ny=40, nz=12, steps=6)), unstable_top=2)):
+        ref, gpu = oracle.RefModel(wl), ocn.Model(wl)
+        ref.step(6); gpu.time_step(6)
+        a, b = gpu.get_fields(), ref.get_fields()
+        for n in FIELDS:
+            assert np.array_equal(a[n], b[n]), (wl["name"], n, rel_linf(a[n], b[n]))
+        gpu.close()
