@@ -127,14 +127,19 @@ def test_tau_only_update_keeps_history():
 # ---------------------------------------------------------------------------------------------
 # full sizes, in the launch configuration bench.py times
 # ---------------------------------------------------------------------------------------------
-def test_config4_full_size_matches_oracle_inside_a_window():
+@pytest.mark.parametrize("closure", [0, 1])
+def test_config4_full_size_matches_oracle_inside_a_window(closure):
     """The full 2880x1200x100 fp32 grid is stepped twice on the GPU; the oracle steps a 300x220x100 window cut from
     the same seeded fields as a closed box.  One step has a finite domain of dependence (3 cells of stencil + one cell
     per barotropic sub-step = 43 cells), so after 2 steps every point further than 86 cells from the window's walls
-    must agree with the full-size run: those are outputs the oracle can compute, compared element by element."""
+    must agree with the full-size run: those are outputs the oracle can compute, compared element by element.
+    closure = 1: the same with the Ri-based vertical mixing closure (its stencil adds no horizontal reach beyond one
+    cell), i.e. the launch configuration `bench.py --closure ri` times."""
     j0, j1, i0, i1 = 450, 670, 1250, 1550
     steps, margin = 2, 2 * (40 + 3) + 2
     full = W.config4()
+    if closure:
+        W.with_ri_closure(full)
     gpu = ocn.Model(full)
     gpu.time_step(steps)
     a = gpu.get_fields()
@@ -143,6 +148,8 @@ def test_config4_full_size_matches_oracle_inside_a_window():
     assert dbg_ok
     del full
     win = W.config4(window=(j0, j1, i0, i1))
+    if closure:
+        W.with_ri_closure(win)
     ref = oracle.RefModel(win)
     ref.step(steps)
     b = ref.get_fields()
