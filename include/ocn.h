@@ -73,6 +73,9 @@ typedef struct {
      * evaluated from state n; ri_n2c, ri_s2min > 0, the others >= 0.  Costs three more 3-D arrays. */
     int closure;
     double ri_nu0, ri_c, ri_kconv, ri_n2c, ri_s2min;
+    /* Surface restoring of the top-cell tracers toward ocn_fields.restore_T / restore_S with piston velocities
+     * gamma_T, gamma_S [m/s]; 0 = off. */
+    double gamma_T, gamma_S;
 } ocn_model_desc;
 
 /* Allocates all device state (14 3-D arrays + 2-D arrays + tables) on `device`. */
@@ -86,12 +89,18 @@ typedef struct {
     void *w;                        /* (nz+1)*ny*nx, get only */
     void *eta;                      /* ny*nx */
     void *tau_x, *tau_y;            /* ny*nx, N/m^2, set only */
+    /* Surface tracer forcing ("forced by realistic surface momentum, heat, and salinity fluxes";
+     * DESIGN.md §3.13), ny*nx, set only: kinematic fluxes into the ocean flux_T [K m/s], flux_S [psu m/s] and the
+     * restoring targets restore_T [K], restore_S [psu].  Top-cell tendency: G += (flux + gamma (target - c)) / dz_top.
+     * All four default to 0. */
+    void *flux_T, *flux_S, *restore_T, *restore_S;
     int on_device;
 } ocn_fields;
 
 /* Copies fields in (masking closed faces / land), on the model's stream.  If any of u, v, T, S,
  * eta is given: re-derives U, V = sum(u dz), w, and resets the AB2 history (the next step is an
- * Euler step).  Setting only tau_x / tau_y keeps the history (per-step forcing update). */
+ * Euler step).  Setting only forcing fields (tau_x, tau_y, flux_*, restore_*) keeps the history (per-step forcing
+ * update). */
 ocn_status ocn_set_fields(ocn_model* model, const ocn_fields* fields);
 /* Enqueues n baroclinic steps on the stream; no host synchronisation. */
 ocn_status ocn_time_step(ocn_model* model, int n);

@@ -150,6 +150,7 @@ struct ocn_ref_model {
     A3 Gu, Gv, GT, GS;              // G^n
     A3 Gu1, Gv1, GT1, GS1;          // G^{n-1}
     A3 eta, U, V, taux, tauy, Hu, Hv;   // 2-D (nl = 1)
+    A3 qT, qS, rT, rS;              // surface tracer fluxes and restoring targets (2-D)
     A3 nuc, kapc;                   // closure = 1: nu, kappa at the bottom face of tracer cell (k, j, i)
     bool have_history = false;
 };
@@ -308,7 +309,9 @@ void compute_mixing(ocn_ref_model& M) {
 // ---------------------------------------------------------------------------------------------
 // DESIGN.md §3.6 / §3.7 — tendencies G^n of the current state into (Gu, Gv, GT, GS)
 // ---------------------------------------------------------------------------------------------
-void tracer_tendency(const ocn_ref_model& M, const A3& c, A3& G, A3& Fx, A3& Fy, A3& Fz) {
+// surf / target / gamma: the surface forcing of the top cell: G += wet (surf + gamma (target - c)) / dz
+void tracer_tendency(const ocn_ref_model& M, const A3& c, A3& G, A3& Fx, A3& Fy, A3& Fz,
+                     const A3& surf, const A3& target, double gamma) {
     const ocn_ref_grid& g = *M.g;
     const int nx = g.nx, ny = g.ny, nz = g.nz;
     const double kh = M.d.kappa_h;
@@ -355,6 +358,8 @@ void tracer_tendency(const ocn_ref_model& M, const A3& c, A3& G, A3& Fx, A3& Fy,
                 const double div = Fx(k, j, i + 1) - Fx(k, j, i) + Fy(k, j + 1, i) - Fy(k, j, i)
                                  + Fz(k + 1, j, i) - Fz(k, j, i);
                 G(k, j, i) = -(double)g.wet(k, j, i) * div / (g.AzC(j) * g.dz[k]);
+                if (k == nz - 1)
+                    G(k, j, i) += (double)g.wet(k, j, i) * (surf(0, j, i) + gamma * (target(0, j, i) - c(k, j, i))) / g.dz[k];
             }
 }
 
@@ -434,8 +439,8 @@ void compute_tendencies(ocn_ref_model& M, A3& Gu, A3& Gv, A3& GT, A3& GS) {
     A3 t1, t2, t3;
     t1.init(g.nx, g.ny, g.nz); t2.init(g.nx, g.ny, g.nz); t3.init(g.nx, g.ny, g.nz + 1);
     momentum_tendency(M, Gu, Gv, t1, t2, t3);
-    tracer_tendency(M, M.T, GT, t1, t2, t3);
-    tracer_tendency(M, M.S, GS, t1, t2, t3);
+    tracer_tendency(M, M.T, GT, t1, t2, t3, M.qT, M.rT, M.d.gamma_T);
+    tracer_tendency(M, M.S, GS, t1, t2, t3, M.qS, M.rS, M.d.gamma_S);
 }
 
 void fill_state_halos(ocn_ref_model& M) {
@@ -686,7 +691,7 @@ int ocn_ref_model_create(const ocn_ref_grid* g, const ocn_ref_model_desc* d, ocn
                   &M->Gu1, &M->Gv1, &M->GT1, &M->GS1}) f->init(nx, ny, nz);
     M->w.init(nx, ny, nz + 1);
     if (d->closure == 1) { M->nuc.init(nx, ny, nz); M->kapc.init(nx, ny, nz); }
-    for (A3* f : {&M->eta, &M->U, &M->V, &M->taux, &M->tauy, &M->Hu, &M->Hv}) f->init(nx, ny, 1);
+    for (A3* f : {&M->eta, &M->U, &M->V, &M->taux, &M->tauy, &M->Hu, &M->Hv, &M->qT, &M->qS, &M->rT, &M->rS}) f->init(nx, ny, 1);
     for (int j = 0; j < ny; ++j)
         for (int i = 0; i < nx; ++i) {
             double hu = 0.0, hv = 0.0;
@@ -711,6 +716,10 @@ int ocn_ref_set_fields(ocn_ref_model* M, const ocn_ref_fields* f) {
     if (f->eta) copy_in(M->eta, f->eta, 1);
     if (f->tau_x) copy_in(M->taux, f->tau_x, 1);
     if (f->tau_y) copy_in(M->tauy, f->tau_y, 1);
+    if (f->flux_T) copy_in(M->qT, f->flux_T, 1);
+    if (f->flux_S) copy_in(M->qS, f->flux_S, 1);
+    if (f->restore_T) copy_in(M->rT, f->restore_T, 1);
+    if (f->restore_S) copy_in(M->rS, f->restore_S, 1);
     // masks: closed faces carry no flow, land cells hold 0 (§3.3)
     for (int k = 0; k < nz; ++k)
         for (int j = 0; j < ny; ++j)

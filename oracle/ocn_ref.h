@@ -45,6 +45,8 @@ typedef struct {
      * 1 = Richardson-number based with convective adjustment, nu_z / kappa_z as background */
     int closure;
     double ri_nu0, ri_c, ri_kconv, ri_n2c, ri_s2min;
+    /* surface restoring piston velocities [m/s] of T and S (0 = off) */
+    double gamma_T, gamma_S;
 } ocn_ref_model_desc;
 
 typedef struct {
@@ -52,6 +54,9 @@ typedef struct {
     double *w;                /* (nz+1)*ny*nx, get only */
     double *eta;              /* ny*nx */
     double *tau_x, *tau_y;    /* ny*nx, N/m^2, set only */
+    /* surface tracer forcing ("surface momentum, heat, and salinity fluxes"), ny*nx, set only:
+     * kinematic fluxes into the ocean [K m/s], [psu m/s] and restoring targets [K], [psu] */
+    double *flux_T, *flux_S, *restore_T, *restore_S;
 } ocn_ref_fields;
 
 /* 0 = ok, non-zero = error (message via ocn_ref_last_error) */

@@ -391,7 +391,8 @@ __global__ void __launch_bounds__(128) k_init_transport(const DevP<T> P) {
 // ---------------------------------------------------------------------------------------------
 // scatter (contiguous interior -> halo'd plane layout, masked) and gather (back, land = 0)
 // st = element stride of the device array (2 = one member of a pair array, base already offset)
-// kind: 0 u, 1 v, 2 T (offset Toff), 3 S (offset Soff), 4 eta, 5 plain 2-D, 6 w (nz+1 levels, gather only)
+// kind: 0 u, 1 v, 2 T (offset Toff), 3 S (offset Soff), 4 eta, 5 plain 2-D, 6 w (nz+1 levels, gather only),
+//       7 / 8 a 2-D surface value of T / S (offset, zero on land columns)
 // ---------------------------------------------------------------------------------------------
 template <class T>
 __device__ __forceinline__ bool cell_open(const DevP<T>& P, long long c, int k, int kind) {
@@ -401,7 +402,7 @@ __device__ __forceinline__ bool cell_open(const DevP<T>& P, long long c, int k, 
         case 0: return k >= tx1;
         case 1: return k >= ty1;
         case 2: case 3: return k >= kb;
-        case 4: return kb < P.nz;
+        case 4: case 7: case 8: return kb < P.nz;
         default: return true;
     }
 }
@@ -413,7 +414,7 @@ __global__ void __launch_bounds__(256) k_scatter(const DevP<T> P, T* __restrict_
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
     if (i >= P.nx || j >= P.ny) return;
     const long long c = (long long)(j + OCN_HALO) * P.sx + i;
-    const T off = kind == 2 ? P.Toff : kind == 3 ? P.Soff : T(0);
+    const T off = (kind == 2 || kind == 7) ? P.Toff : (kind == 3 || kind == 8) ? P.Soff : T(0);
     for (int k = blockIdx.z; k < nl; k += gridDim.z) {
         const T v = cell_open(P, c, k, kind) ? src[((long long)k * P.ny + j) * P.nx + i] - off : T(0);
         store_halo(dst + k * P.sz * st, P.sx, P.nx, P.ny, P.px, P.py, j, i, v, st);

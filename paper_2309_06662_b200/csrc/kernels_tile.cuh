@@ -461,6 +461,10 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 if (k == nz - 1) {                 // tracers are stored as offsets from (Toff, Soff): exact source
                     const T src = w_c1 * rdzk;     // of the constant under the zero-top-flux linear free surface
                     GT += P.Toff * src; GS += P.Soff * src;
+                    // surface tracer forcing: flux into the ocean + restoring toward the target
+                    const T2 qf = P.qts[cT.c], rt = P.rts[cT.c];
+                    GT = (X(GT) + xdiv(X(qf.x) + X(P.gamma_T) * (X(rt.x) - X(tsc.x)), dzk, rdzk)).v;
+                    GS = (X(GS) + xdiv(X(qf.y) + X(P.gamma_S) * (X(rt.y) - X(tsc.y)), dzk, rdzk)).v;
                 }
                 // ---- quasi-AB2, predictor, elimination sweep (S3, S4) ----
                 const T Ght = (X(c0) * X(GT) - X(c1) * X(gm_ts.x)).v, Ghs = (X(c0) * X(GS) - X(c1) * X(gm_ts.y)).v;

@@ -158,6 +158,8 @@ ocn_status build_model(ocn_model* M) {
     T** f2[] = {&P.eta[0], &P.eta[1], &P.U[0], &P.U[1], &P.V[0], &P.V[1], &P.etab, &P.Ub, &P.Vb, &P.GU, &P.GV,
                 &P.SU, &P.SV, &P.Hu, &P.Hv, &P.rHu, &P.rHv, &P.taux, &P.tauy};
     for (T** f : f2) if ((s = plane(n2, f)) != OCN_OK) return s;
+    if ((s = dev_alloc(M, n2, &P.qts, true)) != OCN_OK || (s = dev_alloc(M, n2, &P.rts, true)) != OCN_OK) return s;
+    P.gamma_T = (T)M->d.gamma_T; P.gamma_S = (T)M->d.gamma_S;
     // masks
     {
         uint2* p8 = nullptr; uchar4* pz = nullptr;
@@ -408,6 +410,10 @@ ocn_status set_fields_t(ocn_model* M, const ocn_fields* f) {
     if (f->eta && (s = set_one<T>(M, f->eta, P.eta[0], 1, 4, dev)) != OCN_OK) return s;
     if (f->tau_x && (s = set_one<T>(M, f->tau_x, P.taux, 1, 5, dev)) != OCN_OK) return s;
     if (f->tau_y && (s = set_one<T>(M, f->tau_y, P.tauy, 1, 5, dev)) != OCN_OK) return s;
+    if (f->flux_T && (s = set_one<T>(M, f->flux_T, (T*)P.qts, 1, 4, dev, 2)) != OCN_OK) return s;
+    if (f->flux_S && (s = set_one<T>(M, f->flux_S, (T*)P.qts + 1, 1, 4, dev, 2)) != OCN_OK) return s;
+    if (f->restore_T && (s = set_one<T>(M, f->restore_T, (T*)P.rts, 1, 7, dev, 2)) != OCN_OK) return s;
+    if (f->restore_S && (s = set_one<T>(M, f->restore_S, (T*)P.rts + 1, 1, 8, dev, 2)) != OCN_OK) return s;
     if (f->u || f->v || f->T || f->S || f->eta) {
         const dim3 bc(32, 4);
         ocn::k_init_transport<T><<<grid2(M->g, bc), bc, 0, M->stream>>>(P);
@@ -540,6 +546,7 @@ ocn_status ocn_model_create(const ocn_grid* g, const ocn_model_desc* d, ocn_mode
     if (d->precision != 32 && d->precision != 64) return fail(OCN_EINVAL, "precision must be 32 or 64");
     if (!(d->dt > 0) || d->substeps < 1) return fail(OCN_EINVAL, "dt must be > 0 and substeps >= 1");
     if (!(d->rho0 > 0)) return fail(OCN_EINVAL, "rho0 must be > 0");
+    if (!(d->gamma_T >= 0) || !(d->gamma_S >= 0)) return fail(OCN_EINVAL, "gamma_T, gamma_S must be >= 0");
     if (d->closure != 0 && d->closure != 1) return fail(OCN_EINVAL, "closure must be 0 (constant) or 1 (Ri-based)");
     if (d->closure == 1 && !(d->ri_n2c > 0 && d->ri_s2min > 0 && d->ri_c >= 0 && d->ri_nu0 >= 0 && d->ri_kconv >= 0))
         return fail(OCN_EINVAL, "Ri closure: ri_n2c, ri_s2min must be > 0 and ri_c, ri_nu0, ri_kconv >= 0");

@@ -33,11 +33,12 @@ class ocn_model_desc(C.Structure):
                 ("nu_z", C.c_double), ("kappa_z", C.c_double), ("filter_weights", C.POINTER(C.c_double)),
                 ("device", C.c_int), ("stream", C.c_void_p),
                 ("closure", C.c_int), ("ri_nu0", C.c_double), ("ri_c", C.c_double), ("ri_kconv", C.c_double),
-                ("ri_n2c", C.c_double), ("ri_s2min", C.c_double)]
+                ("ri_n2c", C.c_double), ("ri_s2min", C.c_double), ("gamma_T", C.c_double), ("gamma_S", C.c_double)]
 
 
 class ocn_fields(C.Structure):
-    _fields_ = [(n, C.c_void_p) for n in ("u", "v", "T", "S", "w", "eta", "tau_x", "tau_y")] + [("on_device", C.c_int)]
+    _fields_ = [(n, C.c_void_p) for n in ("u", "v", "T", "S", "w", "eta", "tau_x", "tau_y",
+                                          "flux_T", "flux_S", "restore_T", "restore_S")] + [("on_device", C.c_int)]
 
 
 EXPORTS = ["ocn_grid_create", "ocn_grid_destroy", "ocn_model_create", "ocn_model_destroy", "ocn_set_fields",

@@ -50,6 +50,26 @@ def with_ri_closure(wl, nu0=5e-3, c=5.0, kconv=0.1, n2c=1e-5, s2min=1e-10):
     return wl
 
 
+def with_surface_forcing(wl, seed=SEED_BASE + 40, heat=2e-5, salt=2e-6, piston=1e-5):
+    """Adds seeded surface tracer forcing to a workload (the realistic runs are "forced by realistic
+    surface momentum, heat, and salinity fluxes"; ECCO2 data are not available, these stand in for their shape):
+    smooth kinematic fluxes flux_T [K m/s] (|.| <= heat, about 80 W/m^2), flux_S [psu m/s], and restoring of the top
+    cell toward the initial surface T, S shifted by a smooth anomaly, with piston velocity `piston` [m/s] (about 1 m/day).
+    Inputs only: no method arithmetic."""
+    rng = np.random.default_rng(seed)
+    g, prec = wl["grid"], wl["params"]["precision"]
+    ny, nx = g["ny"], g["nx"]
+    per = bool(g["periodic_x"])
+    f = wl["fields"]
+    f["flux_T"] = _round_to(prec, heat * _low_mode_field(rng, ny, nx, 3, periodic=per))
+    f["flux_S"] = _round_to(prec, salt * _low_mode_field(rng, ny, nx, 3, periodic=per))
+    f["restore_T"] = _round_to(prec, f["T"][-1] + 0.5 * _low_mode_field(rng, ny, nx, 2, periodic=per))
+    f["restore_S"] = _round_to(prec, f["S"][-1] + 0.05 * _low_mode_field(rng, ny, nx, 2, periodic=per))
+    wl["params"].update(gamma_T=float(piston), gamma_S=float(piston))
+    wl["name"] = wl.get("name", "") + "+sfc"
+    return wl
+
+
 def _round_to(precision, a):
     a = np.asarray(a, dtype=np.float64)
     if precision == 32:
