@@ -76,6 +76,9 @@ typedef struct {
     /* Surface restoring of the top-cell tracers toward ocn_fields.restore_T / restore_S with piston velocities
      * gamma_T, gamma_S [m/s]; 0 = off. */
     double gamma_T, gamma_S;
+    /* Bottom drag on the lowest open level of every u / v column:
+     * G_u -= (drag_r + drag_cd |u|) u / dz with |u| the speed at the point; drag_r [m/s], drag_cd [-], >= 0, 0 = off. */
+    double drag_r, drag_cd;
 } ocn_model_desc;
 
 /* Allocates all device state (14 3-D arrays + 2-D arrays + tables) on `device`. */

@@ -43,7 +43,8 @@ class ModelDesc(C.Structure):
                 ("nu_h", C.c_double), ("kappa_h", C.c_double), ("nu_z", C.c_double),
                 ("kappa_z", C.c_double), ("filter_weights", C.POINTER(C.c_double)),
                 ("closure", C.c_int), ("ri_nu0", C.c_double), ("ri_c", C.c_double), ("ri_kconv", C.c_double),
-                ("ri_n2c", C.c_double), ("ri_s2min", C.c_double), ("gamma_T", C.c_double), ("gamma_S", C.c_double)]
+                ("ri_n2c", C.c_double), ("ri_s2min", C.c_double), ("gamma_T", C.c_double), ("gamma_S", C.c_double),
+                ("drag_r", C.c_double), ("drag_cd", C.c_double)]
 
 
 class Fields(C.Structure):

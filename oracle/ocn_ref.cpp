@@ -408,7 +408,11 @@ void momentum_tendency(const ocn_ref_model& M, A3& Gu, A3& Gv, A3& zeta, A3& Ke,
                     const double Vu = nu * ((Dv(k, j, i) - Dv(k, j, i - 1)) / g.dxC(j)
                                           - (zeta(k, j + 1, i) - zeta(k, j, i)) / g.dy);
                     const double tau = (k == nz - 1) ? M.taux(0, j, i) / (M.d.rho0 * g.dz[k]) : 0.0;
-                    Gu(k, j, i) = m * (zt * vhat + Cu - dK - dP - Au + Vu + tau);
+                    // bottom drag on the lowest open level of the u column
+                    const bool bot = m && (k == 0 || !g.mu(k - 1, j, i));
+                    const double drag = bot ? (M.d.drag_r + M.d.drag_cd * std::sqrt(u(k, j, i) * u(k, j, i) + vhat * vhat))
+                                                  * u(k, j, i) / g.dz[k] : 0.0;
+                    Gu(k, j, i) = m * (zt * vhat + Cu - dK - dP - Au + Vu + tau - drag);
                 }
                 // ---------------- v point ----------------
                 {
@@ -428,7 +432,10 @@ void momentum_tendency(const ocn_ref_model& M, A3& Gu, A3& Gv, A3& zeta, A3& Ke,
                     const double Vv = nu * ((Dv(k, j, i) - Dv(k, j - 1, i)) / g.dy
                                           + (zeta(k, j, i + 1) - zeta(k, j, i)) / g.dxF(j));
                     const double tau = (k == nz - 1) ? M.tauy(0, j, i) / (M.d.rho0 * g.dz[k]) : 0.0;
-                    Gv(k, j, i) = m * (-zt * uhat - Cv - dK - dP - Av + Vv + tau);
+                    const bool bot = m && (k == 0 || !g.mv(k - 1, j, i));
+                    const double drag = bot ? (M.d.drag_r + M.d.drag_cd * std::sqrt(uhat * uhat + v(k, j, i) * v(k, j, i)))
+                                                  * v(k, j, i) / g.dz[k] : 0.0;
+                    Gv(k, j, i) = m * (-zt * uhat - Cv - dK - dP - Av + Vv + tau - drag);
                 }
             }
 }

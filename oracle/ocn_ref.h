@@ -47,6 +47,8 @@ typedef struct {
     double ri_nu0, ri_c, ri_kconv, ri_n2c, ri_s2min;
     /* surface restoring piston velocities [m/s] of T and S (0 = off) */
     double gamma_T, gamma_S;
+    /* bottom drag on the lowest open u / v level: linear coefficient [m/s], quadratic [-]; 0 = off */
+    double drag_r, drag_cd;
 } ocn_ref_model_desc;
 
 typedef struct {

@@ -44,6 +44,7 @@ struct DevP {
     T *taux, *tauy;
     T2 *qts, *rts;                 // surface tracer fluxes (flux_T, flux_S) and restoring targets (stored with the tracer offsets)
     T gamma_T, gamma_S;            // restoring piston velocities
+    T drag_r, drag_cd;             // bottom drag: linear [m/s] and quadratic [-] coefficients
     // compact masks (plane layout with halo): thresholds in level index
     const uint2* m8;               // bytes: kb, tx1, tx2, tx3 | ty1, ty2, ty3, 0
     const uchar4* mz;              // zu2, zu3, zv2, zv3

@@ -90,7 +90,9 @@ struct Tile {
 };
 
 
-template <class T, int TX, int TY, int MODE, int MINB>
+// DRAG: compiled with the bottom-drag term of DESIGN.md §3.14 (chosen by the host when drag_r or drag_cd is non-zero, so
+// that the default path does not carry its instructions: 10.17 ms against 10.37 ms with the term predicated off).
+template <class T, int TX, int TY, int MODE, int MINB, bool DRAG = false>
 __global__ void __launch_bounds__(TX * TY, MINB)
 k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__ CUtensorMap m_ts,
                 const __grid_constant__ CUtensorMap m_uv, const __grid_constant__ CUtensorMap m_p) {
@@ -508,7 +510,12 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 const Xv<T> Au = xdiv(half * (Whi * dhi + Wlo * dlo), vold, rAzCj * rdzk);
                 const Xv<T> Vu = nuh * (xdiv(X(kdc.y) - X(kdw.y), dxCj, rdxCj) - xdiv(X(z01) - X(z00), dy, rdy));
                 const Xv<T> tau((k == nz - 1) ? xdiv(X(P.taux[cU.c]), (X(P.rho0) * X(dzk)).v, P.rrho0 * rdzk).v : T(0));
-                const T Gu = (X(zt) * X(vhat) + Cu - dK - dP - Au + Vu + tau).v;
+                // bottom drag on the lowest open level of the column
+                T Gu = (X(zt) * X(vhat) + Cu - dK - dP - Au + Vu + tau).v;
+                if constexpr (DRAG) {
+                    const Xv<T> drag(k == tx1 ? xdiv((X(P.drag_r) + X(P.drag_cd) * X((T)sqrt((X(u_c) * X(u_c) + X(vhat) * X(vhat)).v))) * X(u_c), dzk, rdzk).v : T(0));
+                    Gu = (X(Gu) - drag).v;
+                }
                 // ---- quasi-AB2, predictor, elimination sweep (S3, S4, S5) ----
                 const T Ghu = (X(c0) * X(Gu) - X(c1) * X(gm_u)).v;
                 ((T*)(P.Guv + oU))[0] = Gu;
@@ -550,7 +557,11 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 const Xv<T> Av = xdiv(half * (Whi * dhi + Wlo * dlo), (X(AzFj) * X(dzk)).v, rAzFj * rdzk);
                 const Xv<T> Vv = nuh * (xdiv(X(kdc.y) - X(kds.y), dy, rdy) + xdiv(X(z10) - X(z00), dxFj, rdxFj));
                 const Xv<T> tau((k == nz - 1) ? xdiv(X(P.tauy[cV.c]), (X(P.rho0) * X(dzk)).v, P.rrho0 * rdzk).v : T(0));
-                const T Gv = (-X(zt) * X(uhat) - Cv - dK - dP - Av + Vv + tau).v;
+                T Gv = (-X(zt) * X(uhat) - Cv - dK - dP - Av + Vv + tau).v;
+                if constexpr (DRAG) {
+                    const Xv<T> drag(k == ty1 ? xdiv((X(P.drag_r) + X(P.drag_cd) * X((T)sqrt((X(uhat) * X(uhat) + X(v_c) * X(v_c)).v))) * X(v_c), dzk, rdzk).v : T(0));
+                    Gv = (X(Gv) - drag).v;
+                }
                 const T Ghv = (X(c0) * X(Gv) - X(c1) * X(gm_v)).v;
                 ((T*)(P.Guv + oV))[1] = Gv;
                 const T vs2 = E::add(v_c, E::mul(P.dt, Ghv));

@@ -123,8 +123,15 @@ ocn_status make_tmap(CUtensorMap* tm, bool f64, void* base, unsigned long long i
 // K1 variants: fused (all four fields), or the two prognostic-group kernels that run concurrently.  MINB = CTAs per SM
 // the register allocation is bounded for.
 template <class T> using k1_fn = void (*)(const ocn::DevP<T>, const T, const T, const CUtensorMap, const CUtensorMap, const CUtensorMap);
-template <class T> k1_fn<T> k1_fused() { return ocn::k_tendency_tile<T, TILE_X, TILE_Y, 0, (sizeof(T) == 4 ? 2 : 1)>; }
-template <class T> k1_fn<T> k1_momentum() { return ocn::k_tendency_tile<T, TILE_X, TILE_Y, 1, (sizeof(T) == 4 ? 3 : 1)>; }
+// drag: the instantiation that carries the bottom-drag term (drag_r or drag_cd non-zero)
+template <class T> k1_fn<T> k1_fused(bool drag = false) {
+    return drag ? ocn::k_tendency_tile<T, TILE_X, TILE_Y, 0, (sizeof(T) == 4 ? 2 : 1), true>
+                : ocn::k_tendency_tile<T, TILE_X, TILE_Y, 0, (sizeof(T) == 4 ? 2 : 1), false>;
+}
+template <class T> k1_fn<T> k1_momentum(bool drag = false) {
+    return drag ? ocn::k_tendency_tile<T, TILE_X, TILE_Y, 1, (sizeof(T) == 4 ? 3 : 1), true>
+                : ocn::k_tendency_tile<T, TILE_X, TILE_Y, 1, (sizeof(T) == 4 ? 3 : 1), false>;
+}
 template <class T> k1_fn<T> k1_tracers() { return ocn::k_tendency_tile<T, TILE_X, TILE_Y, 2, (sizeof(T) == 4 ? 3 : 1)>; }
 
 dim3 grid2(const ocn_grid* g, dim3 b, int z = 1) { return dim3((g->nx + b.x - 1) / b.x, (g->ny + b.y - 1) / b.y, z); }
@@ -160,6 +167,7 @@ ocn_status build_model(ocn_model* M) {
     for (T** f : f2) if ((s = plane(n2, f)) != OCN_OK) return s;
     if ((s = dev_alloc(M, n2, &P.qts, true)) != OCN_OK || (s = dev_alloc(M, n2, &P.rts, true)) != OCN_OK) return s;
     P.gamma_T = (T)M->d.gamma_T; P.gamma_S = (T)M->d.gamma_S;
+    P.drag_r = (T)M->d.drag_r; P.drag_cd = (T)M->d.drag_cd;
     // masks
     {
         uint2* p8 = nullptr; uchar4* pz = nullptr;
@@ -256,8 +264,10 @@ ocn_status build_model(ocn_model* M) {
             (s = make_tmap(&M->tm_uv, f64, (T*)P.uv - 2 * C::OX, 2 * sxu, syu, nz, 2 * C::BX, C::BY)) != OCN_OK ||
             (s = make_tmap(&M->tm_p, true, P.p - C::OX, sxu, syu, nz, C::PBX, TILE_Y + 1)) != OCN_OK)
             return s;
-        CK(cudaFuncSetAttribute(k1_fused<T>(), cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
-        CK(cudaFuncSetAttribute(k1_momentum<T>(), cudaFuncAttributeMaxDynamicSharedMemorySize, (ocn::Tile<T, TILE_X, TILE_Y, 1>::SMEM)));
+        for (int dr = 0; dr < 2; ++dr) {
+            CK(cudaFuncSetAttribute(k1_fused<T>(dr != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
+            CK(cudaFuncSetAttribute(k1_momentum<T>(dr != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, (ocn::Tile<T, TILE_X, TILE_Y, 1>::SMEM)));
+        }
         CK(cudaFuncSetAttribute(k1_tracers<T>(), cudaFuncAttributeMaxDynamicSharedMemorySize, (ocn::Tile<T, TILE_X, TILE_Y, 2>::SMEM)));
         CK(cudaFuncSetAttribute(ocn::k_barotropic_tile<T, BT_X, BT_Y>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 ocn::BtTile<T, BT_X, BT_Y>::SMEM));
@@ -313,12 +323,13 @@ ocn_status launch_step(ocn_model* M, bool euler) {
     MARK(-1, 0);
     {
         const dim3 bt(TILE_X, TILE_Y), gt = grid2(g, bt);
+        const bool drag = M->d.drag_r != 0.0 || M->d.drag_cd != 0.0;
         if (!M->split_k1) {
-            k1_fused<T>()<<<gt, bt, ocn::Tile<T, TILE_X, TILE_Y, 0>::SMEM, M->stream>>>(P, c0, c1, M->tm_ts, M->tm_uv, M->tm_p);
+            k1_fused<T>(drag)<<<gt, bt, ocn::Tile<T, TILE_X, TILE_Y, 0>::SMEM, M->stream>>>(P, c0, c1, M->tm_ts, M->tm_uv, M->tm_p);
         } else {                                   // the two group kernels side by side (fork / join on a second stream)
             CK(cudaEventRecord(M->ev_fork, M->stream));
             CK(cudaStreamWaitEvent(M->stream2, M->ev_fork, 0));
-            k1_momentum<T>()<<<gt, bt, ocn::Tile<T, TILE_X, TILE_Y, 1>::SMEM, M->stream2>>>(P, c0, c1, M->tm_ts, M->tm_uv, M->tm_p);
+            k1_momentum<T>(drag)<<<gt, bt, ocn::Tile<T, TILE_X, TILE_Y, 1>::SMEM, M->stream2>>>(P, c0, c1, M->tm_ts, M->tm_uv, M->tm_p);
             CK(cudaEventRecord(M->ev_join, M->stream2));
             k1_tracers<T>()<<<gt, bt, ocn::Tile<T, TILE_X, TILE_Y, 2>::SMEM, M->stream>>>(P, c0, c1, M->tm_ts, M->tm_uv, M->tm_p);
             CK(cudaStreamWaitEvent(M->stream, M->ev_join, 0));
@@ -547,6 +558,7 @@ ocn_status ocn_model_create(const ocn_grid* g, const ocn_model_desc* d, ocn_mode
     if (!(d->dt > 0) || d->substeps < 1) return fail(OCN_EINVAL, "dt must be > 0 and substeps >= 1");
     if (!(d->rho0 > 0)) return fail(OCN_EINVAL, "rho0 must be > 0");
     if (!(d->gamma_T >= 0) || !(d->gamma_S >= 0)) return fail(OCN_EINVAL, "gamma_T, gamma_S must be >= 0");
+    if (!(d->drag_r >= 0) || !(d->drag_cd >= 0)) return fail(OCN_EINVAL, "drag_r, drag_cd must be >= 0");
     if (d->closure != 0 && d->closure != 1) return fail(OCN_EINVAL, "closure must be 0 (constant) or 1 (Ri-based)");
     if (d->closure == 1 && !(d->ri_n2c > 0 && d->ri_s2min > 0 && d->ri_c >= 0 && d->ri_nu0 >= 0 && d->ri_kconv >= 0))
         return fail(OCN_EINVAL, "Ri closure: ri_n2c, ri_s2min must be > 0 and ri_c, ri_nu0, ri_kconv >= 0");

@@ -55,3 +55,35 @@ def test_forcing_only_update_keeps_the_ab2_history():
     fa, fb = a.get_fields(), b.get_fields()
     for n in FIELDS:
         assert np.array_equal(fa[n], fb[n]), n
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+def test_bottom_drag_latlon_reduced(prec):
+    wl = W.config2(nx=180, ny=75, nz=25, steps=10, precision=prec)
+    rng = np.random.default_rng(12)
+    wl["fields"]["u"] = W._round_to(prec, 0.2 * rng.standard_normal(wl["fields"]["u"].shape))   # flow at the bottom too
+    wl["fields"]["v"] = W._round_to(prec, 0.2 * rng.standard_normal(wl["fields"]["v"].shape))
+    wl["params"].update(drag_r=5e-4, drag_cd=2.5e-3)
+    ref, gpu = oracle.RefModel(wl), ocn.Model(wl)
+    ref.step(10); gpu.time_step(10)
+    a, b = gpu.get_fields(), ref.get_fields()
+    for n in FIELDS:
+        if prec == 64:
+            assert np.array_equal(a[n], b[n]), (n, rel_linf(a[n], b[n]))
+        else:
+            assert rel_linf(a[n], b[n]) <= TOL[32], (n, rel_linf(a[n], b[n]))
+    gpu.close()
+
+
+def test_bottom_drag_first_step_tendency_matches_on_ragged_basin():
+    wl = W.config1(nx=45, ny=37, nz=11, steps=2)
+    rng = np.random.default_rng(13)
+    wl["fields"]["u"] = 0.1 * rng.standard_normal(wl["fields"]["u"].shape)
+    wl["fields"]["v"] = 0.1 * rng.standard_normal(wl["fields"]["v"].shape)
+    wl["params"].update(drag_r=1e-3, drag_cd=3e-3)
+    ref, gpu = oracle.RefModel(wl), ocn.Model(wl)
+    G = ref.tendencies()
+    gpu.time_step(1)
+    d = gpu.debug()
+    for n in ("Gu", "Gv"):
+        assert np.array_equal(d[n], G[n]), (n, rel_linf(d[n], G[n]))

@@ -67,3 +67,69 @@ def test_uniform_heating_warms_the_top_cell_by_flux_dt_over_dz_and_zero_forcing_
     ma.step(3); mb.step(3)
     fa, fb = ma.get_fields(), mb.get_fields()
     assert all(np.array_equal(fa[k], fb[k]) for k in fa)
+
+
+# ------------------------------------------------------------------ bottom drag ----
+def test_linear_bottom_drag_obeys_the_ab2_recurrence_on_the_lowest_level_only():
+    nz, dz, dt, r, chi = 4, 25.0, 600.0, 2e-3, 0.1
+    wl = box(nx=6, ny=5, nz=nz, depth=nz * dz, f0=0.0, dt=dt, substeps=10, kappa_z=0.0, nu_z=0.0, drag_r=r)
+    wl["fields"]["u"][:] = 0.3
+    wl["fields"]["v"][:] = -0.2
+    m = oracle.RefModel(wl)
+    z = -dt * r / dz
+    q, p = np.array([0.3, -0.2]), None
+    for n in range(15):
+        m.step(1)
+        if p is None:
+            p, q = q, q + z * q
+        else:
+            p, q = q, q + z * ((1.5 + chi) * q - (0.5 + chi) * p)
+    f = m.get_fields()
+    assert np.max(np.abs(f["u"][0] - q[0])) < 1e-13 and np.max(np.abs(f["v"][0] - q[1])) < 1e-13
+    assert np.max(np.abs(f["u"][1:] - 0.3)) < 1e-13 and np.max(np.abs(f["v"][1:] + 0.2)) < 1e-13   # nu_z = 0: the rest coasts
+    assert np.abs(f["eta"]).max() < 1e-12                         # uniform transport: the free surface stays flat
+
+
+def test_quadratic_bottom_drag_first_step_closed_form_uses_the_speed_at_the_point():
+    dz, dt, cd = 20.0, 300.0, 3e-3
+    wl = box(nx=6, ny=5, nz=3, depth=3 * dz, f0=0.0, dt=dt, substeps=10, kappa_z=0.0, nu_z=0.0, drag_cd=cd)
+    wl["fields"]["u"][:] = 0.4
+    wl["fields"]["v"][:] = 0.3                                     # speed 0.5 at every u and v point
+    m = oracle.RefModel(wl)
+    m.step(1)                                                      # Euler start
+    f = m.get_fields()
+    assert np.max(np.abs(f["u"][0] - (0.4 - dt * cd * 0.5 * 0.4 / dz))) < 1e-14
+    assert np.max(np.abs(f["v"][0] - (0.3 - dt * cd * 0.5 * 0.3 / dz))) < 1e-14
+
+
+def test_drag_acts_exactly_on_the_lowest_open_u_and_v_levels_of_a_bathymetry():
+    wl = W.config2(nx=32, ny=20, nz=10, steps=1)
+    rng = np.random.default_rng(9)
+    wl["fields"]["u"] = 0.1 * rng.standard_normal(wl["fields"]["u"].shape)
+    wl["fields"]["v"] = 0.1 * rng.standard_normal(wl["fields"]["v"].shape)
+    r = 1e-3
+    a = oracle.RefModel(wl)
+    w2 = clone(wl); w2["params"].update(drag_r=r)
+    b = oracle.RefModel(w2)
+    Ga, Gb, f = a.tendencies(), b.tendencies(), a.get_fields()
+    masks = a.grid.masks()
+    dz = np.diff(wl["z_faces"])
+    for name, vel, mk in (("Gu", "u", "order_zeta_u"), ("Gv", "v", "order_zeta_v")):
+        open_ = masks[mk] > 0                                      # open faces carry a vorticity order >= 1
+        want = np.zeros_like(Ga[name])
+        for j in range(20):                                        # brute force: first open level of each column
+            for i in range(32):
+                ks = np.nonzero(open_[:, j, i])[0]
+                if ks.size:
+                    want[ks[0], j, i] = -r * f[vel][ks[0], j, i] / dz[ks[0]]
+        assert np.max(np.abs((Gb[name] - Ga[name]) - want)) < 1e-18 + 1e-12 * np.abs(want).max(), name
+        assert np.abs(want).max() > 0
+
+
+def test_zero_drag_coefficients_are_the_plain_step_bitwise():
+    a = W.config0(nx=12, ny=10, nz=6, steps=3)
+    b = clone(a); b["params"].update(drag_r=0.0, drag_cd=0.0)
+    ma, mb = oracle.RefModel(a), oracle.RefModel(b)
+    ma.step(3); mb.step(3)
+    fa, fb = ma.get_fields(), mb.get_fields()
+    assert all(np.array_equal(fa[k], fb[k]) for k in fa)
