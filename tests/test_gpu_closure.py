@@ -127,3 +127,57 @@ def test_closure_fp64_is_bit_identical_to_the_oracle():
         for n in FIELDS:
             assert np.array_equal(a[n], b[n]), (wl["name"], n, rel_linf(a[n], b[n]))
         gpu.close()
+
+
+def _all_options(wl):
+    """closure + surface forcing + bottom drag together"""
+    W.with_surface_forcing(W.with_ri_closure(wl))
+    wl["params"].update(drag_r=5e-4, drag_cd=2.5e-3)
+    return wl
+
+
+def test_degenerate_shapes_with_closure_forcing_and_drag():
+    # the smallest grids (stencil wraps onto itself, two levels = one interior face), walls, one warp-straddling width
+    for nx, ny, nz, per in ((3, 3, 2, (1, 1)), (4, 4, 2, (1, 1)), (5, 4, 3, (0, 0)), (33, 9, 2, (1, 0))):
+        wl = W.config0(nx=nx, ny=ny, nz=nz)
+        wl["grid"]["periodic_x"], wl["grid"]["periodic_y"] = per
+        _run_both(_all_options(wl), [1, 4])
+
+
+def test_all_land_and_isolated_columns_with_closure_forcing_and_drag():
+    wl = _all_options(W.config1(nx=40, ny=20, nz=6, steps=3))
+    wl["depth"][:] = 0.0
+    gpu = ocn.Model(wl)
+    gpu.time_step(3)
+    f = gpu.get_fields()
+    for n in FIELDS:
+        assert np.all(f[n] == 0.0), n
+    gpu.close()
+    rng = np.random.default_rng(11)
+    wl = W.config1(nx=70, ny=21, nz=9, steps=6)
+    d = wl["depth"]
+    d[::2, ::2] = 0.0                                   # isolated wet columns (no open faces), ragged depths
+    d[10, :] = 3500.0                                   # a one-cell-wide zonal channel
+    d[:, 35] = rng.uniform(200.0, 4000.0, size=d.shape[0])
+    d[0, :] = d[-1, :] = 0.0; d[:, 0] = d[:, -1] = 0.0
+    wl["fields"]["u"] = 0.05 * rng.standard_normal(wl["fields"]["u"].shape)
+    wl["fields"]["v"] = 0.05 * rng.standard_normal(wl["fields"]["v"].shape)
+    _run_both(_all_options(wl), [1, 6])
+
+
+def test_many_levels_with_closure_nz_150_fp64():
+    wl = W.config4(window=(600, 640, 2000, 2070), steps=3, precision=64)
+    nz = 150
+    zf = W.geometric_z_faces(nz, 5.0, 6000.0)
+    zc_old = 0.5 * (wl["z_faces"][:-1] + wl["z_faces"][1:]); zc = 0.5 * (zf[:-1] + zf[1:])
+    f = wl["fields"]
+    for n in ("u", "v", "T", "S"):
+        a = f[n]
+        out = np.empty((nz,) + a.shape[1:])
+        for j in range(a.shape[1]):
+            for i in range(a.shape[2]):
+                out[:, j, i] = np.interp(zc, zc_old, a[:, j, i])
+        f[n] = out
+    wl["z_faces"] = zf
+    wl["grid"]["nz"] = nz
+    _run_both(_all_options(wl), [1, 3])
