@@ -81,7 +81,7 @@ typedef struct {
     double drag_r, drag_cd;
 } ocn_model_desc;
 
-/* Allocates all device state (14 3-D arrays + 2-D arrays + tables) on `device`. */
+/* Allocates all device state (14 3-D arrays, 17 with closure = 1, + 2-D arrays + tables) on `device`. */
 ocn_status ocn_model_create(const ocn_grid* grid, const ocn_model_desc* desc, ocn_model** out);
 ocn_status ocn_model_destroy(ocn_model* model);
 
