@@ -20,6 +20,15 @@
 
 #include "common.cuh"
 
+// First thread of the compacted work lists of a 256-thread CTA: v cells from 0 up, tracer cells from 64
+// up, faces from 160 up (wrapping), u cells from N-1 down.  On sparse levels the four lists land on different warps; on
+// half-full levels no thread carries all four.  Measured on config 4 (profiles/r1_ncu_summary.md §6).
+#ifndef K1_TOFF
+#define K1_TOFF 64
+#define K1_VOFF 0
+#define K1_FOFF 160
+#endif
+
 namespace ocn {
 
 // ---- mbarrier / TMA (PTX; SASS: SYNCS.*, UTMALDG) ------------------------------------------------
@@ -225,7 +234,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
         };
         auto cell_emit = [&](int q, int rank) { s_cell[rank] = (unsigned short)q; };
         csort(NC, [&](int q) { return cell_key(q, 0); }, cell_emit, s_nc);
-        constexpr int TOFF = NC / 2, VOFF = 3 * NC / 4;                   // faces run from thread 0 up, tracers from N/2, v from 3N/4, u from N-1 down
+        constexpr int TOFF = K1_TOFF, VOFF = K1_VOFF;                     // first thread of the tracer and v lists (u runs from N-1 down, faces from K1_FOFF up)
         gT = s_cell[(tid + NC - TOFF) % NC];
         if constexpr (DO_M) {
             csort(NC, [&](int q) { return cell_key(q, 1); }, cell_emit, s_nc);
@@ -288,8 +297,8 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
         if (m < nz) tma_load_plane(sm + C::O_UV + (m % C::R_UV) * C::PL2, &m_uv, bar, 2 * i0, j0, m);
         if (DO_M && m - 1 >= kmin) tma_load_plane(sm + C::O_P + ((m - 1) % C::R_P) * C::PLP, &m_p, bar, i0, j0 + 2, m - 1);
     };
-    // the TMA producer is a thread of the warp with the least part-A / part-B work on sparse levels (faces run from
-    // thread 0, tracers from N/2, v from 3N/4, u from N-1 down): its issue latency stays off the critical path
+    // the TMA producer is a thread of a warp without part-A / part-B work on sparse levels (v cells run from thread 0,
+    // tracer cells from 64, faces from 160, u cells from N-1 down): its issue latency stays off the critical path
     constexpr int PROD = (3 * NT / 8) & ~31;
     if (tid == PROD) {
         issue_group(kmin, true);
@@ -298,10 +307,10 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     }
 
     // ---- per-thread column state ------------------------------------------------------------
-    // A thread owns the TRACERS of the cell of rank t in the order by first wet level, the U of the cell of rank
-    // N-1-t in the order by first open west face and the V of the cell of rank t - N/3 (mod N) in the order by first
-    // open south face: every block of part B runs on a dense run of threads, and on sparse levels the three runs
-    // (from thread 0 up, from N/3 up, from N-1 down) land on different warps instead of one after the other.
+    // A thread owns the TRACERS of the cell of rank t - K1_TOFF (mod N) in the order by first wet level, the U of the
+    // cell of rank N-1-t in the order by first open west face and the V of the cell of rank t - K1_VOFF (mod N) in the
+    // order by first open south face: every block of part B runs on a dense run of threads, and on sparse levels the
+    // runs land on different warps instead of one after the other.
     struct Cell { int cx, cy, t1, bo, by; long long c; bool incol; unsigned char z2, z3; };
     auto make_cell = [&](int g, int which) {
         Cell X;
@@ -397,7 +406,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             if constexpr (DO_T) {
                 const T2* __restrict__ s_ts = (const T2*)(sm + C::O_TS + (k & (C::R_TS - 1)) * C::PL2);
                 const int nface = s_nf[k];
-                for (int f = tid; f < nface; f += NT) {
+                for (int f = (tid + NT - K1_FOFF) % NT; f < nface; f += NT) {
                     const uint2 d = s_fs[f];
                     const int b = d.x & 1023u, row = (d.x >> 10) & 15u, fid = d.x >> 16;
                     const bool isy = (d.x >> 14) & 1u;
