@@ -299,7 +299,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     };
     // the TMA producer is a thread of a warp without part-A / part-B work on sparse levels (v cells run from thread 0,
     // tracer cells from 64, faces from 160, u cells from N-1 down): its issue latency stays off the critical path
-    constexpr int PROD = (3 * NT / 8) & ~31;
+    constexpr int PROD = 32;                 // warp 1: measured best of 32 / 96 / 128 (9.98 / 10.06 / 10.04 ms)
     if (tid == PROD) {
         issue_group(kmin, true);
 #pragma unroll
