@@ -727,6 +727,9 @@ int ocn_ref_set_fields(ocn_ref_model* M, const ocn_ref_fields* f) {
     if (f->flux_S) copy_in(M->qS, f->flux_S, 1);
     if (f->restore_T) copy_in(M->rT, f->restore_T, 1);
     if (f->restore_S) copy_in(M->rS, f->restore_S, 1);
+    // forcing-only update (tau, fluxes, restoring targets): the state and the AB2 history stay (per-step forcing, as
+    // include/ocn.h states for ocn_set_fields)
+    if (!(f->u || f->v || f->T || f->S || f->eta)) return 0;
     // masks: closed faces carry no flow, land cells hold 0 (§3.3)
     for (int k = 0; k < nz; ++k)
         for (int j = 0; j < ny; ++j)

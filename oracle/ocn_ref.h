@@ -67,6 +67,8 @@ int ocn_ref_grid_create(const ocn_ref_grid_desc*, const double* z_faces, const d
 int ocn_ref_grid_destroy(ocn_ref_grid*);
 int ocn_ref_model_create(const ocn_ref_grid*, const ocn_ref_model_desc*, ocn_ref_model** out);
 int ocn_ref_model_destroy(ocn_ref_model*);
+/* copies in; if any of u, v, T, S, eta is given: masks, re-derives U, V, w, p and resets the AB2 history (the next
+ * step is an Euler step); a forcing-only call (tau, flux, restore) keeps state and history */
 int ocn_ref_set_fields(ocn_ref_model*, const ocn_ref_fields*);
 int ocn_ref_time_step(ocn_ref_model*, int n);
 int ocn_ref_get_fields(ocn_ref_model*, ocn_ref_fields*);

@@ -87,3 +87,23 @@ def test_bottom_drag_first_step_tendency_matches_on_ragged_basin():
     d = gpu.debug()
     for n in ("Gu", "Gv"):
         assert np.array_equal(d[n], G[n]), (n, rel_linf(d[n], G[n]))
+
+
+def test_time_varying_forcing_updated_every_step():
+    # the realistic use (forcing fields change in time): wind stress and heat flux re-sent before every
+    # step on both sides; the AB2 history is kept, so this is NOT a sequence of Euler restarts
+    wl = W.with_surface_forcing(W.config2(nx=96, ny=40, nz=12, steps=6))
+    ref, gpu = oracle.RefModel(wl), ocn.Model(wl)
+    for n in range(6):
+        s = np.cos(0.7 * n)
+        upd = dict(tau_x=s * wl["fields"]["tau_x"], flux_T=(1.0 - 0.3 * n) * wl["fields"]["flux_T"])
+        ref.set_fields(**upd); gpu.set_fields(**upd)
+        ref.step(1); gpu.time_step(1)
+    a, b = gpu.get_fields(), ref.get_fields()
+    for n in FIELDS:
+        assert np.array_equal(a[n], b[n]), (n, rel_linf(a[n], b[n]))
+    euler = oracle.RefModel(wl)                                  # what Euler restarts would have given: different
+    for n in range(6):
+        euler.set_fields(tau_x=np.cos(0.7 * n) * wl["fields"]["tau_x"], u=euler.get_fields()["u"])
+        euler.step(1)
+    assert rel_linf(euler.get_fields()["u"], b["u"]) > 1e-6

@@ -133,3 +133,15 @@ def test_zero_drag_coefficients_are_the_plain_step_bitwise():
     ma.step(3); mb.step(3)
     fa, fb = ma.get_fields(), mb.get_fields()
     assert all(np.array_equal(fa[k], fb[k]) for k in fa)
+
+
+def test_forcing_only_set_fields_keeps_state_and_history_in_the_oracle():
+    # re-sending the same forcing between steps must not change anything (no Euler restart, no re-derivation)
+    wl = W.with_surface_forcing(W.config2(nx=24, ny=16, nz=8, steps=4))
+    a, b = oracle.RefModel(wl), oracle.RefModel(wl)
+    a.step(4)
+    b.step(2)
+    b.set_fields(**{k: wl["fields"][k] for k in ("tau_x", "tau_y", "flux_T", "flux_S", "restore_T", "restore_S")})
+    b.step(2)
+    fa, fb = a.get_fields(), b.get_fields()
+    assert all(np.array_equal(fa[k], fb[k]) for k in fa)
