@@ -76,9 +76,9 @@ __global__ void __launch_bounds__(128) k_ri_mixing(const DevP<T> P) {
                     const float N2 = (float)P.g * ((float)P.alpha * ((float)q[r].x - (float)t0) - (float)P.beta_s * ((float)q[r].y - (float)s0)) * rdzc;
                     const float duw = (float)uw1 - (float)uw0, due = (float)ue1 - (float)ue0, dvs = (float)vs1 - (float)vs0, dvn = (float)vn1 - (float)vn0;
                     const float S2 = 0.5f * ((duw * duw + due * due) + (dvs * dvs + dvn * dvn)) * rdzc * rdzc;
-                    const float Ri = fmaxf(N2, 0.f) / (S2 + (float)P.ri_s2min);
-                    const float f = 1.0f / (1.0f + (float)P.ri_c * Ri);
-                    const float conv = (float)P.ri_kconv * fminf(1.0f, fmaxf(-N2, 0.f) / (float)P.ri_n2c);
+                    const float Ri = __fdividef(fmaxf(N2, 0.f), S2 + (float)P.ri_s2min);     // hardware reciprocal: 2 ulp
+                    const float f = __fdividef(1.0f, 1.0f + (float)P.ri_c * Ri);
+                    const float conv = (float)P.ri_kconv * fminf(1.0f, fmaxf(-N2, 0.f) * (float)(1.0 / P.ri_n2c));
                     const float g2 = (float)P.ri_nu0 * f * f;
                     out = mk2((T)((float)P.nu_z_d + g2 + conv), (T)((float)P.kappa_z_d + g2 * f + conv));
                 }
@@ -120,7 +120,7 @@ struct ThomasRow {
             const T sp = has_hi ? dtk_hi * rz * rc_hi : T(0);
             const T sm = first ? T(0) : dtk_lo * rz * rc_lo;
             const T m = T(1) + sp + sm + sm * cp;                     // cp of the first row is 0 * sm
-            const T rm = T(1) / m;
+            const T rm = __fdividef(1.0f, (float)m);
             d0 = (phi0 + sm * d0) * rm;
             d1 = (phi1 + sm * d1) * rm;
             cp = -sp * rm;
