@@ -15,6 +15,11 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "libocn_ref.so")
 _SRC = [os.path.join(_HERE, "ocn_ref.cpp"), os.path.join(_HERE, "ocn_ref.h")]
+# tests/test_oracle_mutations.py points this at a deliberately broken copy of ocn_ref.cpp (built into its own .so next
+# to that copy) to prove that the pins of tests/ notice the mistake; unset everywhere else
+if os.environ.get("OCN_REF_MUTANT_SRC"):
+    _SRC = [os.environ["OCN_REF_MUTANT_SRC"], _SRC[1]]
+    _SO = os.environ["OCN_REF_MUTANT_SRC"] + ".so"
 _lib = None
 
 
@@ -22,7 +27,7 @@ def build(force=False):
     """Compile the oracle with g++ (plain -O2, OpenMP over rows; no fast-math)."""
     if not force and os.path.exists(_SO) and all(os.path.getmtime(_SO) >= os.path.getmtime(s) for s in _SRC):
         return _SO
-    cmd = ["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off",
+    cmd = ["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off", "-I", _HERE,
            "-o", _SO, _SRC[0]]
     subprocess.check_call(cmd)
     return _SO
@@ -195,6 +200,12 @@ class RefModel:
         nz, ny, nx = self.nz, self.ny, self.nx
         d = dict(p=np.zeros((nz, ny, nx)), U=np.zeros((ny, nx)), V=np.zeros((ny, nx)))
         _check(lib().ocn_ref_get_diagnostics(self.h, _dp(d["p"]), _dp(d["U"]), _dp(d["V"])))
+        return d
+
+    def momentum_diagnostics(self):
+        nz, ny, nx = self.nz, self.ny, self.nx
+        d = dict(zeta=np.zeros((nz, ny, nx)), K=np.zeros((nz, ny, nx)), D=np.zeros((nz, ny, nx)))
+        _check(lib().ocn_ref_get_momentum_diagnostics(self.h, _dp(d["zeta"]), _dp(d["K"]), _dp(d["D"])))
         return d
 
     def mixing(self):

@@ -862,6 +862,18 @@ int ocn_ref_get_diagnostics(ocn_ref_model* M, double* p, double* U, double* V) {
     return 0;
 }
 
+int ocn_ref_get_momentum_diagnostics(ocn_ref_model* M, double* zeta, double* K, double* D) {
+    if (!M) return fail("null argument");
+    const ocn_ref_grid& g = *M->g;
+    A3 gu, gv, z, ke, dv;
+    gu.init(g.nx, g.ny, g.nz); gv.init(g.nx, g.ny, g.nz); z.init(g.nx, g.ny, g.nz); ke.init(g.nx, g.ny, g.nz); dv.init(g.nx, g.ny, g.nz);
+    momentum_tendency(*M, gu, gv, z, ke, dv);
+    if (zeta) copy_out(z, zeta, g.nz);
+    if (K) copy_out(ke, K, g.nz);
+    if (D) copy_out(dv, D, g.nz);
+    return 0;
+}
+
 int ocn_ref_barotropic_raw(ocn_ref_model* M, int m, double dtau) {
     if (!M || m < 0) return fail("bad argument");
     const ocn_ref_grid& g = *M->g;

@@ -106,6 +106,9 @@ int ocn_ref_filter_weights(int M, double* a, double* dtau_over_dt);
 int ocn_ref_get_tendencies(ocn_ref_model*, double* Gu, double* Gv, double* GT, double* GS);
 /* stored diagnostics of the current state: p (nz*ny*nx), U, V (ny*nx); NULL = skip */
 int ocn_ref_get_diagnostics(ocn_ref_model*, double* p, double* U, double* V);
+/* the intermediates of the momentum tendency of the CURRENT state: relative vorticity zeta at the
+ * south-west corner of cell (k, j, i), kinetic energy K and horizontal divergence D at its centre; nz*ny*nx each, NULL = skip */
+int ocn_ref_get_momentum_diagnostics(ocn_ref_model*, double* zeta, double* K, double* D);
 /* m raw barotropic sub-steps of (eta, U, V) with time step dtau and forcing G^U = G^V = 0,
  * no averaging (for the gravity-wave closed form); 3-D state untouched. */
 int ocn_ref_barotropic_raw(ocn_ref_model*, int m, double dtau);

@@ -1,7 +1,7 @@
 // common.cuh — device-side parameter block, memory layout and small device helpers of libocn.
 //
 // Layout: every 3-D field is [k][j][i] with i fastest, a physical halo of 3
-// cells in i and j, row pitch sx = roundup(nx + 6, 32) elements, and the base pointer shifted so
+// cells in i and j, row pitch sx = roundup(nx + 8, 32) elements, and the base pointer shifted so
 // that element (k, j, i = 0) of every row starts a 128-byte line.  The prognostic groups are
 // stored interleaved, one element = a pair: uv = (u, v), ts = (T, S), and likewise their AB2
 // history G and eliminated right-hand sides d, so that one 8/16-byte access moves both members

@@ -39,7 +39,9 @@ inline int roundup(int a, int b) { return (a + b - 1) / b * b; }
 inline std::string build_grid(ocn_grid& g, const ocn_grid_desc& d, const double* z_faces, const double* depth) {
     g.d = d; g.nx = d.nx; g.ny = d.ny; g.nz = d.nz;
     const int nx = g.nx, ny = g.ny, nz = g.nz;
-    g.sx = roundup(nx + 2 * OCN_HALO, 32);
+    // + 2: the TMA maps of K1 start 4 columns before i = 0, so the east halo column i = nx + 2 sits at x = nx + 6 and must
+    // lie inside the row (x < sx) or the hardware zero-fills it instead of delivering the periodic image
+    g.sx = roundup(nx + 2 * OCN_HALO + 2, 32);
     g.sy = ny + 2 * OCN_HALO;
     g.zf.assign(z_faces, z_faces + nz + 1);
     for (int k = 0; k < nz; ++k) if (!(g.zf[k + 1] > g.zf[k])) return "z_faces must be strictly increasing";

@@ -24,3 +24,15 @@ def pytest_collection_modifyitems(config, items):
     for item in items:
         if "gpu" in item.keywords:
             item.add_marker(skip)
+
+
+def pytest_terminal_summary(terminalreporter):
+    try:
+        import util
+    except Exception:
+        return
+    if util.PARITY_REPORT:
+        terminalreporter.write_line("")
+        terminalreporter.write_line("parity margins (relative L-inf, normalised by max |oracle|; 0 = bit-identical):")
+        for ln in util.PARITY_REPORT:
+            terminalreporter.write_line("  " + ln)

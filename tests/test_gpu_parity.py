@@ -274,6 +274,28 @@ def test_fp64_is_bit_identical_to_the_oracle():
         gpu.close()
 
 
+@pytest.mark.parametrize("nx", [26, 58, 90])
+@pytest.mark.parametrize("closure", [0, 1])
+def test_periodic_seam_when_nx_plus_6_is_a_multiple_of_32(nx, closure):
+    """nx + 6 = 32 n: the east halo column i = nx + 2 is the last element a TMA box of the last tile can reach; with a row
+    pitch of exactly nx + 6 it fell outside the tensor map and was zero-filled (round-1 advisor finding).  fp64, periodic in
+    x, flow and tracer gradients across the seam: bit-identical to the oracle."""
+    wl = W.config2(nx=nx, ny=20, nz=8, steps=4)
+    rng = np.random.default_rng(nx)
+    wl["depth"][:, -4:] = 3000.0                        # open ocean on both sides of the seam
+    wl["depth"][:, :4] = 3000.0
+    wl["fields"]["u"] = 0.2 * rng.standard_normal(wl["fields"]["u"].shape)
+    wl["fields"]["v"] = 0.2 * rng.standard_normal(wl["fields"]["v"].shape)
+    if closure:
+        W.with_ri_closure(wl)
+    ref, gpu = oracle.RefModel(wl), ocn.Model(wl)
+    ref.step(4); gpu.time_step(4)
+    a, b = gpu.get_fields(), ref.get_fields()
+    for n in FIELDS:
+        assert np.array_equal(a[n], b[n]), (n, rel_linf(a[n], b[n]))
+    gpu.close()
+
+
 # ---------------------------------------------------------------------------------------------
 # the rest of the boundary: device buffers, caller's stream, per-step forcing, errors, profiling
 # ---------------------------------------------------------------------------------------------

@@ -1,0 +1,141 @@
+"""Mutation check of the oracle's pins: every one-token mistake below — a metric factor of the wrong row or kind, a dropped
+mask, a wrong sign — is applied to a scratch copy of oracle/ocn_ref.cpp, built on its own, and the pin tests are run
+against it in a subprocess (oracle/__init__.py loads the copy when OCN_REF_MUTANT_SRC is set).  Each mutant must make
+at least one pin FAIL; the unmodified source must pass.  This is what "pinned" means in DESIGN.md §5: a plausible mistake
+anywhere in the lat-lon metric factors or bathymetry masks of momentum_tendency, tracer_tendency, compute_w and
+barotropic_substep does not survive `-m "not gpu"`.  (The list is the one the round-1 review injected, plus a few more.
+Not listed because they are EQUIVALENT mutants: dropping the open-face masks of U, V in barotropic_substep — a closed
+face has H = 0, G^U = 0 and starts from U = 0, so it stays 0 with or without the mask.)
+"""
+import os
+import shutil
+import subprocess
+import sys
+import tempfile
+from concurrent.futures import ThreadPoolExecutor
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+SRC = os.path.join(ROOT, "oracle", "ocn_ref.cpp")
+# pins that the mutants are run against (fast ones first; -x stops at the first failure)
+PINS = ["tests/test_oracle_latlon.py", "tests/test_oracle_handcalc.py"]
+
+# (name, exact text in ocn_ref.cpp (must occur once), replacement)
+MUTANTS = [
+    ("M1 zeta: dxC(j-1) u[j-1] -> dxC(j) u[j-1]",
+     "- (g.dxC(j) * u(k, j, i) - g.dxC(j - 1) * u(k, j - 1, i))) / g.AzF(j);",
+     "- (g.dxC(j) * u(k, j, i) - g.dxC(j) * u(k, j - 1, i))) / g.AzF(j);"),
+    ("M2 F_y: v dxF(j) -> v dxC(j)",
+     "Fy(k, j, i) = vv * g.dxF(j) * g.dz[k] * cf",
+     "Fy(k, j, i) = vv * g.dxC(j) * g.dz[k] * cf"),
+    ("M3 W_v: AzC(j-1) w[j-1] -> AzC(j) w[j-1]",
+     "const double Wlo = 0.5 * (g.AzC(j - 1) * w(k, j - 1, i) + g.AzC(j) * w(k, j, i));",
+     "const double Wlo = 0.5 * (g.AzC(j) * w(k, j - 1, i) + g.AzC(j) * w(k, j, i));"),
+    ("M4 C_u: fF(j+1) -> fF(j) in the northern half",
+     "+ g.fF(j + 1) * 0.5 * g.dxF(j + 1) * (v(k, j + 1, i - 1) + v(k, j + 1, i))) / g.dxC(j);",
+     "+ g.fF(j) * 0.5 * g.dxF(j + 1) * (v(k, j + 1, i - 1) + v(k, j + 1, i))) / g.dxC(j);"),
+    ("M5 vhat: dxF(j+1) -> dxF(j)",
+     "+ g.dxF(j + 1) * (v(k, j + 1, i - 1) + v(k, j + 1, i))) / g.dxC(j);\n                    const double zs[6] = {zeta(k, j - 2, i)",
+     "+ g.dxF(j) * (v(k, j + 1, i - 1) + v(k, j + 1, i))) / g.dxC(j);\n                    const double zs[6] = {zeta(k, j - 2, i)"),
+    ("M6 compute_w: dxF(j+1) v[j+1] -> dxF(j) v[j+1]",
+     "+ g.dxF(j + 1) * M.v(k, j + 1, i) - g.dxF(j) * M.v(k, j, i)) / g.AzC(j);\n                M.w(k + 1, j, i)",
+     "+ g.dxF(j) * M.v(k, j + 1, i) - g.dxF(j) * M.v(k, j, i)) / g.AzC(j);\n                M.w(k + 1, j, i)"),
+    ("M7 V_v: (zeta[i+1]-zeta[i]) / dxF(j) -> / dxC(j)",
+     "+ (zeta(k, j, i + 1) - zeta(k, j, i)) / g.dxF(j));",
+     "+ (zeta(k, j, i + 1) - zeta(k, j, i)) / g.dxC(j));"),
+    ("M8 A_v: / (AzF(j) dz) -> / (AzC(j) dz)",
+     "const double Av = 0.5 * (Whi * dhi + Wlo * dlo) / (g.AzF(j) * g.dz[k]);",
+     "const double Av = 0.5 * (Whi * dhi + Wlo * dlo) / (g.AzC(j) * g.dz[k]);"),
+    ("M9 vertical advection of u: mask mu[k-1] dropped below",
+     "const double dlo = (k >= 1) ? (u(k, j, i) - u(k - 1, j, i)) * g.mu(k, j, i) * g.mu(k - 1, j, i) : 0.0;",
+     "const double dlo = (k >= 1) ? (u(k, j, i) - u(k - 1, j, i)) * g.mu(k, j, i) : 0.0;"),
+    ("M10 vertical advection of v: mask mv[k-1] dropped below",
+     "const double dlo = (k >= 1) ? (v(k, j, i) - v(k - 1, j, i)) * g.mv(k, j, i) * g.mv(k - 1, j, i) : 0.0;",
+     "const double dlo = (k >= 1) ? (v(k, j, i) - v(k - 1, j, i)) * g.mv(k, j, i) : 0.0;"),
+    ("M13 barotropic eta: dxF(j+1) V[j+1] -> dxF(j) V[j+1]",
+     "+ g.dxF(j + 1) * M.V(0, j + 1, i) - g.dxF(j) * M.V(0, j, i)) / g.AzC(j);",
+     "+ g.dxF(j) * M.V(0, j + 1, i) - g.dxF(j) * M.V(0, j, i)) / g.AzC(j);"),
+    ("M14 barotropic U: d(eta) / dxC(j) -> / dxF(j)",
+     "(M.eta(0, j, i) - M.eta(0, j, i - 1)) / g.dxC(j) + gu))",
+     "(M.eta(0, j, i) - M.eta(0, j, i - 1)) / g.dxF(j) + gu))"),
+    ("M15 grad p in G_u: / dxC(j) -> / dxF(j)",
+     "const double dP = (p(k, j, i) - p(k, j, i - 1)) / g.dxC(j);",
+     "const double dP = (p(k, j, i) - p(k, j, i - 1)) / g.dxF(j);"),
+    ("M16 tracer G: / (AzC(j) dz) -> / (AzF(j) dz)",
+     "G(k, j, i) = -(double)g.wet(k, j, i) * div / (g.AzC(j) * g.dz[k]);",
+     "G(k, j, i) = -(double)g.wet(k, j, i) * div / (g.AzF(j) * g.dz[k]);"),
+    ("M17 zeta: / AzF(j) -> / AzC(j)",
+     "g.dxC(j - 1) * u(k, j - 1, i))) / g.AzF(j);",
+     "g.dxC(j - 1) * u(k, j - 1, i))) / g.AzC(j);"),
+    ("M18 D in the momentum tendency: dxF(j) v[j] -> dxF(j+1) v[j]",
+     "+ g.dxF(j + 1) * v(k, j + 1, i) - g.dxF(j) * v(k, j, i)) / g.AzC(j);",
+     "+ g.dxF(j + 1) * v(k, j + 1, i) - g.dxF(j + 1) * v(k, j, i)) / g.AzC(j);"),
+    ("M19 dK/dx in G_u: / dxC(j) -> / dxF(j)",
+     "const double dK = (Ke(k, j, i) - Ke(k, j, i - 1)) / g.dxC(j);",
+     "const double dK = (Ke(k, j, i) - Ke(k, j, i - 1)) / g.dxF(j);"),
+    ("M20 C_v: fF(j) -> fF(j+1)",
+     "const double Cv = g.fF(j) * uhat;",
+     "const double Cv = g.fF(j + 1) * uhat;"),
+    ("M21 F_x diffusion: / dxC(j) -> / dxF(j)",
+     "(c(k, j, i) - c(k, j, i - 1)) / g.dxC(j) * g.mu(k, j, i);",
+     "(c(k, j, i) - c(k, j, i - 1)) / g.dxF(j) * g.mu(k, j, i);"),
+    ("M22 F_z: AzC(j) -> AzF(j)",
+     "Fz(k, j, i) = ww * g.AzC(j) * cf * g.mw(k, j, i);",
+     "Fz(k, j, i) = ww * g.AzF(j) * cf * g.mw(k, j, i);"),
+    ("M23 V_u: (D[i]-D[i-1]) / dxC(j) -> / dxF(j)",
+     "const double Vu = nu * ((Dv(k, j, i) - Dv(k, j, i - 1)) / g.dxC(j)",
+     "const double Vu = nu * ((Dv(k, j, i) - Dv(k, j, i - 1)) / g.dxF(j)"),
+    ("M25 metric: AzF from phi_c +- wrong row",
+     "g->AzF_[r] = a * a * dlam * (std::sin(pc) - std::sin(pc - dphi));",
+     "g->AzF_[r] = a * a * dlam * (std::sin(pc + dphi) - std::sin(pc));"),
+    ("M26 metric: fF at the cell centre instead of the corner",
+     "g->fF_[r] = 2.0 * d->rotation_rate * std::sin(pf);",
+     "g->fF_[r] = 2.0 * d->rotation_rate * std::sin(pc);"),
+    ("control: 1/4 -> 1/2 in K",
+     "Ke(k, j, i) = 0.25 * (u(k, j, i) * u(k, j, i) + u(k, j, i + 1) * u(k, j, i + 1))",
+     "Ke(k, j, i) = 0.5 * (u(k, j, i) * u(k, j, i) + u(k, j, i + 1) * u(k, j, i + 1))"),
+]
+
+
+def _run_pins(src_path):
+    env = dict(os.environ, OCN_REF_MUTANT_SRC=src_path, OMP_NUM_THREADS="2")
+    r = subprocess.run([sys.executable, "-m", "pytest", "-x", "-q", "-p", "no:cacheprovider"] + PINS, cwd=ROOT, env=env,
+                       stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
+    return r.returncode, r.stdout[-3000:]
+
+
+def test_every_mutant_of_the_latlon_metrics_and_masks_is_caught():
+    text = open(SRC).read()
+    tmp = tempfile.mkdtemp(prefix="ocn_mut_")
+    try:
+        jobs = []
+        for n, (name, old, new) in enumerate(MUTANTS):
+            assert text.count(old) == 1, "mutation target not found exactly once (oracle source changed?): " + name
+            path = os.path.join(tmp, "mutant_%02d.cpp" % n)
+            with open(path, "w") as f:
+                f.write(text.replace(old, new))
+            jobs.append((name, path))
+        clean = os.path.join(tmp, "clean.cpp")
+        shutil.copy(SRC, clean)
+        with ThreadPoolExecutor(max_workers=max(2, (os.cpu_count() or 4) // 2)) as ex:
+            res = list(ex.map(lambda j: _run_pins(j[1]), jobs + [("clean", clean)]))
+        rc, out = res[-1]
+        assert rc == 0, "the unmodified oracle fails its pins through the mutant loader:\n" + out
+        survivors = [name for (name, _), (rc, _) in zip(jobs, res[:-1]) if rc == 0]
+        assert not survivors, "mutants that survive every pin: %s" % survivors
+        # the harness must have run the pins and seen an assertion fail (pytest exit code 1), not crashed on build / import
+        for (name, _), (rc, out) in zip(jobs, res[:-1]):
+            assert rc == 1 and "AssertionError" in out, (name, rc, out)
+    finally:
+        shutil.rmtree(tmp, ignore_errors=True)
+
+
+if __name__ == "__main__":          # python tests/test_oracle_mutations.py: prints which pin catches which mutant
+    text = open(SRC).read()
+    tmp = tempfile.mkdtemp(prefix="ocn_mut_")
+    for n, (name, old, new) in enumerate(MUTANTS):
+        path = os.path.join(tmp, "m%02d.cpp" % n)
+        open(path, "w").write(text.replace(old, new))
+        rc, out = _run_pins(path)
+        first = [ln for ln in out.splitlines() if ln.startswith("FAILED")]
+        print("%-70s %s" % (name, first[0] if first else ("SURVIVES" if rc == 0 else "rc=%d" % rc)))
+    shutil.rmtree(tmp, ignore_errors=True)

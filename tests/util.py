@@ -36,3 +36,12 @@ def rel_linf(a, ref, mask=None):
 
 def clone(wl):
     return copy.deepcopy(wl)
+
+
+# per-field parity margins of the full-size GPU tests; tests/conftest.py prints them in the terminal summary so that the
+# driver's log of `pytest -m gpu` shows how far inside the tolerance each case is
+PARITY_REPORT = []
+
+
+def report_parity(case, steps, errs):
+    PARITY_REPORT.append("%-58s steps %3d  " % (case, steps) + "  ".join("%s %.2e" % (n, e) for n, e in errs.items()))
