@@ -32,7 +32,9 @@ typedef enum {
     OCN_OK = 0, OCN_EINVAL = 1, OCN_ENOMEM = 2, OCN_ECUDA = 3, OCN_ESTATE = 4, OCN_EUNSUPPORTED = 5
 } ocn_status;
 
-/* Horizontal grid (lat-lon domain of PAPER.md:102). */
+/* Horizontal grid.  PAPER.md:102-104 (§6): the realistic domains "span the entire longitudinal extent of the sphere and
+ * cover the latitudinal range from 75 S to 75 N", periodic in longitude, with bathymetry; PAPER.md:84 (§5.2): finite volume
+ * on a staggered C-grid.  Metrics of the curvilinear cells: DESIGN.md §3.1-3.2. */
 typedef struct {
     int kind;                       /* 0 cartesian (f/beta-plane), 1 latitude-longitude */
     int nx, ny, nz;                 /* nx, ny >= 3; 2 <= nz <= 250 */
@@ -43,10 +45,14 @@ typedef struct {
     double f0, beta;                /* cartesian: f = f0 + beta (y - y_mid) */
 } ocn_grid_desc;
 
-/* z_faces: HOST, nz+1 doubles, increasing, z_faces[nz] = 0 (surface).
+/* ocn_grid_create — the grid and the immersed-boundary bathymetry of PAPER.md:102-104; builds the metrics and the compact
+ * 2-D level-threshold masks the kernels read.
+ * z_faces: HOST, nz+1 finite doubles, strictly increasing, z_faces[nz] = 0 (the resting surface).
  * bottom_depth: HOST, ny*nx doubles, metres >= 0, 0 = land.  Immersed boundary = full cells,
  * cell wet iff its centre lies above the bottom; columns with < 2 wet cells are land
- * (DESIGN.md §3.3).  Host-only: allocates nothing on the device. */
+ * (DESIGN.md §3.3).  Host-only: allocates nothing on the device.
+ * Errors: OCN_EINVAL (null pointer, sizes, non-monotonic or non-finite z_faces, z_faces[nz] != 0, negative depth, a
+ * latitude range that reaches a pole), OCN_EUNSUPPORTED (nz > 250), OCN_ENOMEM. */
 ocn_status ocn_grid_create(const ocn_grid_desc* desc, const double* z_faces, const double* bottom_depth,
                            ocn_grid** out);
 ocn_status ocn_grid_destroy(ocn_grid* grid);
@@ -54,7 +60,8 @@ ocn_status ocn_grid_destroy(ocn_grid* grid);
 /* Model parameters. */
 typedef struct {
     int precision;                  /* 32 or 64: dtype of every field buffer crossing the ABI and
-                                       of all device fields, tendencies and metrics */
+                                       of all device fields, tendencies and metrics (PAPER.md:26, 143:
+                                       the paper runs and reports both FP32 and FP64) */
     double dt;                      /* baroclinic time step [s] */
     int substeps;                   /* barotropic sub-steps M per baroclinic step */
     double chi;                     /* quasi-AB2 offset (0.1) */
@@ -63,7 +70,10 @@ typedef struct {
     const double* filter_weights;   /* HOST, `substeps` doubles a_1..a_M, or NULL = power-law
                                        default of DESIGN.md §3.9; copied at creation */
     int device;                     /* CUDA device ordinal */
-    void* stream;                   /* cudaStream_t of the caller (e.g. torch's), NULL = default */
+    void* stream;                   /* cudaStream_t of the caller (e.g. torch's): all work of the model is enqueued on it.
+                                       NULL = the library creates a PRIVATE non-blocking stream (it does not synchronise
+                                       with the legacy default stream): device buffers passed with on_device = 1 must
+                                       then be complete before the call (caller synchronises its producer) */
     /* Vertical mixing closure ("Richardson-number-based parameterization for vertical
      * mixing due to unresolved shear and convective turbulence"; its coefficient is the second stored
      * diagnostic of PAPER.md:78; formulas: DESIGN.md §3.12).  closure = 0: constant nu_z / kappa_z.
@@ -81,7 +91,12 @@ typedef struct {
     double drag_r, drag_cd;
 } ocn_model_desc;
 
-/* Allocates all device state (14 3-D arrays, 17 with closure = 1, + 2-D arrays + tables) on `device`. */
+/* ocn_model_create — the model of PAPER.md:84 (§5.2: hydrostatic Boussinesq, IMEX quasi-AB2, backward-Euler vertical
+ * diffusion) with the split-explicit free surface of PAPER.md:94-98 (§5.3) on `grid`.  Allocates all device state
+ * (14 3-D arrays + 2-D arrays + tables) on `device`; the calling thread's current device is restored on return (as it is
+ * by every call below).  Parameters must be finite; chi, g, the viscosities / diffusivities, gamma_*, drag_* >= 0; user
+ * filter_weights must sum to 1 (1e-9) and have a positive first moment (dtau = dt / sum_m m a_m).
+ * Errors: OCN_EINVAL, OCN_ENOMEM (device allocation), OCN_ECUDA (no device: there is no CPU fallback). */
 ocn_status ocn_model_create(const ocn_grid* grid, const ocn_model_desc* desc, ocn_model** out);
 ocn_status ocn_model_destroy(ocn_model* model);
 
@@ -100,14 +115,22 @@ typedef struct {
     int on_device;
 } ocn_fields;
 
-/* Copies fields in (masking closed faces / land), on the model's stream.  If any of u, v, T, S,
- * eta is given: re-derives U, V = sum(u dz), w, and resets the AB2 history (the next step is an
- * Euler step).  Setting only forcing fields (tau_x, tau_y, flux_*, restore_*) keeps the history (per-step forcing
- * update). */
+/* ocn_set_fields — initial / boundary data of the problem of PAPER.md:102-104 (state, and the "surface momentum, heat, and
+ * salinity fluxes" that force it).  Copies fields in (masking closed faces / land), on the model's stream.  If any of u, v,
+ * T, S, eta is given: re-derives U, V = sum(u dz), w, p and resets the AB2 history (the next step is an Euler step).
+ * DEPARTURE from SURVEY.md §8(b)'s proposed contract ("resets AB2 history" on every call): a call that carries ONLY forcing
+ * fields (tau_x, tau_y, flux_*, restore_*) keeps the state and the AB2 history, so that time-varying forcing can be re-sent
+ * before each step without an Euler restart (reading 19); the oracle's ocn_ref_set_fields does the same.
+ * Host buffers may be reused as soon as the call returns.  Errors: OCN_EINVAL (null, w given), OCN_ECUDA. */
 ocn_status ocn_set_fields(ocn_model* model, const ocn_fields* fields);
-/* Enqueues n baroclinic steps on the stream; no host synchronisation. */
+/* ocn_time_step — n baroclinic steps of the algorithm of PAPER.md:84 (§5.2) and PAPER.md:94-98 (§5.3): fused tendency
+ * kernel, quasi-AB2, implicit vertical diffusion, split-explicit barotropic sub-cycle with filter
+ * weights, barotropic correction, diagnostics.  Enqueues on the stream; no host synchronisation.
+ * Errors: OCN_EINVAL (n < 0), OCN_ECUDA (launch failure; asynchronous faults surface at the next synchronising call). */
 ocn_status ocn_time_step(ocn_model* model, int n);
-/* Copies fields out (land / closed faces = 0) and synchronises the stream. */
+/* ocn_get_fields — the prognostic state (u, v, T, S, eta) and the diagnosed w.  Copies fields out (land /
+ * closed faces = 0); returns after the copies have completed (host buffers are valid on return).
+ * Errors: OCN_EINVAL, OCN_ECUDA (including asynchronous faults of earlier steps). */
 ocn_status ocn_get_fields(ocn_model* model, ocn_fields* fields);
 ocn_status ocn_synchronize(ocn_model* model);
 

@@ -49,7 +49,8 @@ class ModelDesc(C.Structure):
                 ("kappa_z", C.c_double), ("filter_weights", C.POINTER(C.c_double)),
                 ("closure", C.c_int), ("ri_nu0", C.c_double), ("ri_c", C.c_double), ("ri_kconv", C.c_double),
                 ("ri_n2c", C.c_double), ("ri_s2min", C.c_double), ("gamma_T", C.c_double), ("gamma_S", C.c_double),
-                ("drag_r", C.c_double), ("drag_cd", C.c_double)]
+                ("drag_r", C.c_double), ("drag_cd", C.c_double),
+                ("eos", C.c_int), ("eos_alpha2", C.c_double), ("eos_gamma", C.c_double), ("advection", C.c_int)]
 
 
 class Fields(C.Structure):
@@ -65,6 +66,8 @@ def lib():
         _lib.ocn_ref_last_error.restype = C.c_char_p
         _lib.ocn_ref_weno.restype = C.c_double
         _lib.ocn_ref_weno.argtypes = [C.POINTER(C.c_double), C.c_int, C.c_double]
+        _lib.ocn_ref_weno_scheme.restype = C.c_double
+        _lib.ocn_ref_weno_scheme.argtypes = [C.POINTER(C.c_double), C.c_int, C.c_double, C.c_int]
         _lib.ocn_ref_barotropic_raw.argtypes = [C.c_void_p, C.c_int, C.c_double]
         _lib.ocn_ref_implicit_column.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_ubyte),
                                                  C.c_double, C.POINTER(C.c_double)]
@@ -94,10 +97,12 @@ def set_num_threads(n):
     lib().ocn_ref_set_num_threads(int(n))
 
 
-def weno(c6, order, vel):
+def weno(c6, order, vel, scheme=0):
     c = np.ascontiguousarray(c6, dtype=np.float64)
     assert c.size == 6
-    return float(lib().ocn_ref_weno(_dp(c), int(order), float(vel)))
+    if scheme == 0:
+        return float(lib().ocn_ref_weno(_dp(c), int(order), float(vel)))
+    return float(lib().ocn_ref_weno_scheme(_dp(c), int(order), float(vel), int(scheme)))
 
 
 def implicit_column(z_faces, open_faces, dt_kappa, phi):

@@ -161,7 +161,11 @@ namespace {
 // WENO reconstruction (Jiang-Shu weights, uniform-grid coefficients)
 // c[0..5] = cells n-3 .. n+2, interface between c[2] (n-1) and c[3] (n).
 // ---------------------------------------------------------------------------------------------
-double weno(const double c[6], int order, double vel) {
+// scheme 0: the classical Jiang-Shu weights alpha_s = d_s / (eps + beta_s)^2.
+// scheme 1 (Borges et al. 2008 for r = 3, the same construction for r = 2): WENO-Z weights
+//   alpha_s = d_s (1 + (tau / (eps + beta_s))^2),  tau = |beta_0 - beta_{r-1}|
+// with the same candidate polynomials, smoothness indicators, linear weights and eps.
+double weno(const double c[6], int order, double vel, int scheme = 0) {
     double qm2, qm1, q0, q1, q2;
     if (vel > 0.0) { qm2 = c[0]; qm1 = c[1]; q0 = c[2]; q1 = c[3]; q2 = c[4]; }
     else           { qm2 = c[5]; qm1 = c[4]; q0 = c[3]; q1 = c[2]; q2 = c[1]; }
@@ -176,6 +180,12 @@ double weno(const double c[6], int order, double vel) {
                         + 0.25 * (qm1 - q1) * (qm1 - q1);
         const double b2 = 13.0 / 12.0 * (q0 - 2.0 * q1 + q2) * (q0 - 2.0 * q1 + q2)
                         + 0.25 * (3.0 * q0 - 4.0 * q1 + q2) * (3.0 * q0 - 4.0 * q1 + q2);
+        if (scheme == 1) {
+            const double tau = std::fabs(b0 - b2);
+            const double r0 = tau / (eps + b0), r1 = tau / (eps + b1), r2 = tau / (eps + b2);
+            const double a0 = 0.1 * (1.0 + r0 * r0), a1 = 0.6 * (1.0 + r1 * r1), a2 = 0.3 * (1.0 + r2 * r2);
+            return (a0 * p0 + a1 * p1 + a2 * p2) / (a0 + a1 + a2);
+        }
         const double a0 = 0.1 / ((eps + b0) * (eps + b0));
         const double a1 = 0.6 / ((eps + b1) * (eps + b1));
         const double a2 = 0.3 / ((eps + b2) * (eps + b2));
@@ -186,6 +196,12 @@ double weno(const double c[6], int order, double vel) {
         const double p1 = (q0 + q1) / 2.0;
         const double b0 = (q0 - qm1) * (q0 - qm1);
         const double b1 = (q1 - q0) * (q1 - q0);
+        if (scheme == 1) {
+            const double tau = std::fabs(b0 - b1);
+            const double r0 = tau / (eps + b0), r1 = tau / (eps + b1);
+            const double a0 = (1.0 / 3.0) * (1.0 + r0 * r0), a1 = (2.0 / 3.0) * (1.0 + r1 * r1);
+            return (a0 * p0 + a1 * p1) / (a0 + a1);
+        }
         const double a0 = (1.0 / 3.0) / ((eps + b0) * (eps + b0));
         const double a1 = (2.0 / 3.0) / ((eps + b1) * (eps + b1));
         return (a0 * p0 + a1 * p1) / (a0 + a1);
@@ -254,8 +270,14 @@ void compute_w(ocn_ref_model& M) {
     fill_halo(M.w, g.px, g.py);
 }
 
+// eos 0, the linear equation of state b = g [alpha (T - T0) - beta_S (S - S0)].
+// eos 1, a nonlinear equation of state with thermobaricity and cabbeling,
+//   b = g [alpha (1 - gamma z_c) (T - T0) + (alpha2 / 2) (T - T0)^2 - beta_S (S - S0)],   z_c <= 0 the depth of the cell centre
 inline double buoyancy(const ocn_ref_model& M, int k, int j, int i) {
-    return M.d.g * (M.d.alpha * (M.T(k, j, i) - M.d.T0) - M.d.beta_s * (M.S(k, j, i) - M.d.S0));
+    const double dT = M.T(k, j, i) - M.d.T0, dS = M.S(k, j, i) - M.d.S0;
+    if (M.d.eos == 1)
+        return M.d.g * (M.d.alpha * (1.0 - M.d.eos_gamma * M.g->zc[k]) * dT + 0.5 * M.d.eos_alpha2 * dT * dT - M.d.beta_s * dS);
+    return M.d.g * (M.d.alpha * dT - M.d.beta_s * dS);
 }
 
 void compute_p(ocn_ref_model& M) {
@@ -324,7 +346,7 @@ void tracer_tendency(const ocn_ref_model& M, const A3& c, A3& G, A3& Fx, A3& Fy,
                     const double cs[6] = {c(k, j, i - 3), c(k, j, i - 2), c(k, j, i - 1),
                                           c(k, j, i), c(k, j, i + 1), c(k, j, i + 2)};
                     const double uu = M.u(k, j, i);
-                    const double cf = weno(cs, g.order_x(k, j, i), uu);
+                    const double cf = weno(cs, g.order_x(k, j, i), uu, M.d.advection);
                     Fx(k, j, i) = uu * g.dy * g.dz[k] * cf
                                 - kh * g.dy * g.dz[k] * (c(k, j, i) - c(k, j, i - 1)) / g.dxC(j) * g.mu(k, j, i);
                 }
@@ -332,7 +354,7 @@ void tracer_tendency(const ocn_ref_model& M, const A3& c, A3& G, A3& Fx, A3& Fy,
                     const double cs[6] = {c(k, j - 3, i), c(k, j - 2, i), c(k, j - 1, i),
                                           c(k, j, i), c(k, j + 1, i), c(k, j + 2, i)};
                     const double vv = M.v(k, j, i);
-                    const double cf = weno(cs, g.order_y(k, j, i), vv);
+                    const double cf = weno(cs, g.order_y(k, j, i), vv, M.d.advection);
                     Fy(k, j, i) = vv * g.dxF(j) * g.dz[k] * cf
                                 - kh * g.dxF(j) * g.dz[k] * (c(k, j, i) - c(k, j - 1, i)) / g.dy * g.mv(k, j, i);
                 }
@@ -348,7 +370,7 @@ void tracer_tendency(const ocn_ref_model& M, const A3& c, A3& G, A3& Fx, A3& Fy,
                     cs[m] = (kk >= 0 && kk < nz) ? c(kk, j, i) : 0.0;
                 }
                 const double ww = M.w(k, j, i);
-                const double cf = weno(cs, g.order_z(k, j, i), ww);
+                const double cf = weno(cs, g.order_z(k, j, i), ww, M.d.advection);
                 Fz(k, j, i) = ww * g.AzC(j) * cf * g.mw(k, j, i);
             }
 #pragma omp parallel for schedule(static)
@@ -394,7 +416,7 @@ void momentum_tendency(const ocn_ref_model& M, A3& Gu, A3& Gv, A3& zeta, A3& Ke,
                                               + g.dxF(j + 1) * (v(k, j + 1, i - 1) + v(k, j + 1, i))) / g.dxC(j);
                     const double zs[6] = {zeta(k, j - 2, i), zeta(k, j - 1, i), zeta(k, j, i),
                                           zeta(k, j + 1, i), zeta(k, j + 2, i), zeta(k, j + 3, i)};
-                    const double zt = weno(zs, g.order_zeta_u(k, j, i), vhat);
+                    const double zt = weno(zs, g.order_zeta_u(k, j, i), vhat, M.d.advection);
                     const double Cu = 0.5 * (g.fF(j) * 0.5 * g.dxF(j) * (v(k, j, i - 1) + v(k, j, i))
                                            + g.fF(j + 1) * 0.5 * g.dxF(j + 1) * (v(k, j + 1, i - 1) + v(k, j + 1, i))) / g.dxC(j);
                     const double dK = (Ke(k, j, i) - Ke(k, j, i - 1)) / g.dxC(j);
@@ -420,7 +442,7 @@ void momentum_tendency(const ocn_ref_model& M, A3& Gu, A3& Gv, A3& zeta, A3& Ke,
                     const double uhat = 0.25 * (u(k, j - 1, i) + u(k, j, i) + u(k, j - 1, i + 1) + u(k, j, i + 1));
                     const double zs[6] = {zeta(k, j, i - 2), zeta(k, j, i - 1), zeta(k, j, i),
                                           zeta(k, j, i + 1), zeta(k, j, i + 2), zeta(k, j, i + 3)};
-                    const double zt = weno(zs, g.order_zeta_v(k, j, i), uhat);
+                    const double zt = weno(zs, g.order_zeta_v(k, j, i), uhat, M.d.advection);
                     const double Cv = g.fF(j) * uhat;
                     const double dK = (Ke(k, j, i) - Ke(k, j - 1, i)) / g.dy;
                     const double dP = (p(k, j, i) - p(k, j - 1, i)) / g.dy;
@@ -679,6 +701,8 @@ int ocn_ref_model_create(const ocn_ref_grid* g, const ocn_ref_model_desc* d, ocn
     if (!g || !d || !out) return fail("null argument");
     if (d->substeps < 1 || !(d->dt > 0)) return fail("bad dt / substeps");
     if (d->closure != 0 && d->closure != 1) return fail("closure must be 0 or 1");
+    if (d->eos != 0 && d->eos != 1) return fail("eos must be 0 (linear) or 1 (nonlinear)");
+    if (d->advection != 0 && d->advection != 1) return fail("advection must be 0 (WENO-JS) or 1 (WENO-Z)");
     if (d->closure == 1 && !(d->ri_n2c > 0 && d->ri_s2min > 0 && d->ri_c >= 0 && d->ri_nu0 >= 0 && d->ri_kconv >= 0))
         return fail("bad Ri closure parameters");
     ocn_ref_model* M = new ocn_ref_model();
@@ -804,6 +828,7 @@ int ocn_ref_get_metrics(const ocn_ref_grid* g, double* dxC, double* dxF, double*
 }
 
 double ocn_ref_weno(const double c[6], int order, double vel) { return weno(c, order, vel); }
+double ocn_ref_weno_scheme(const double c[6], int order, double vel, int scheme) { return weno(c, order, vel, scheme); }
 
 int ocn_ref_implicit_column(int nz, const double* z_faces, const unsigned char* open, double dtk, double* phi) {
     if (nz < 2 || !z_faces || !open || !phi) return fail("bad argument");

@@ -49,6 +49,12 @@ typedef struct {
     double gamma_T, gamma_S;
     /* bottom drag on the lowest open u / v level: linear coefficient [m/s], quadratic [-]; 0 = off */
     double drag_r, drag_cd;
+    /* equation of state: 0 = linear, 1 = b = g [alpha (1 - eos_gamma z) (T - T0) + eos_alpha2 / 2 (T - T0)^2
+     * - beta_s (S - S0)] (thermobaricity eos_gamma [1/m], cabbeling eos_alpha2 [1/K^2]) */
+    int eos;
+    double eos_alpha2, eos_gamma;
+    /* nonlinear WENO weights: 0 = Jiang-Shu, 1 = WENO-Z */
+    int advection;
 } ocn_ref_model_desc;
 
 typedef struct {
@@ -88,6 +94,8 @@ int ocn_ref_get_metrics(const ocn_ref_grid*, double* dxC, double* dxF, double* A
 /* WENO face value at the interface between c[2] and c[3] of the six cells c[0..5]
  * (= cells n-3..n+2), order 1..3, upwinded by the sign of vel. */
 double ocn_ref_weno(const double c[6], int order, double vel);
+/* the same with the weight family chosen: scheme 0 = Jiang-Shu, 1 = WENO-Z */
+double ocn_ref_weno_scheme(const double c[6], int order, double vel, int scheme);
 /* backward-Euler vertical diffusion of one column, in place (DESIGN.md §3.8 step 4).
  * open[k], k = 0..nz: 1 if the face below cell k is open (open[0], open[nz] ignored = closed). */
 int ocn_ref_implicit_column(int nz, const double* z_faces, const unsigned char* open,

@@ -4,9 +4,11 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -29,6 +31,20 @@ ocn_status fail(ocn_status s, const std::string& m) { g_err = m; return s; }
     } while (0)
 
 constexpr int LEAD = 32;   // elements before the first row so that i = 0 starts a 128-byte line
+
+// Every entry point that touches the device switches to the model's device and restores the caller's on return.
+struct DeviceGuard {
+    int prev = -1;
+    cudaError_t err;
+    explicit DeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+        err = cudaSetDevice(dev);
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+#define ON_DEVICE(dev)                 \
+    DeviceGuard guard_(dev);           \
+    CK(guard_.err)
 
 }  // namespace
 
@@ -101,13 +117,15 @@ ocn_status make_tmap(CUtensorMap* tm, bool f64, void* base, unsigned long long i
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
     static encode_fn encode = nullptr;
-    if (!encode) {
+    static std::once_flag once;
+    std::call_once(once, [] {
         void* fn = nullptr;
         cudaDriverEntryPointQueryResult qr;
-        CK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr));
-        if (!fn || qr != cudaDriverEntryPointSuccess) return fail(OCN_ECUDA, "cuTensorMapEncodeTiled not available");
-        encode = reinterpret_cast<encode_fn>(fn);
-    }
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) == cudaSuccess && fn &&
+            qr == cudaDriverEntryPointSuccess)
+            encode = reinterpret_cast<encode_fn>(fn);
+    });
+    if (!encode) return fail(OCN_ECUDA, "cuTensorMapEncodeTiled not available");
     const unsigned long long es = f64 ? 8 : 4;
     const cuuint64_t dims[3] = {inner, rows, levels};
     const cuuint64_t strides[2] = {inner * es, inner * rows * es};
@@ -283,9 +301,10 @@ ocn_status build_model(ocn_model* M) {
 namespace {
 
 ocn_status prof_flush(ocn_model* M) {           // fold recorded events into the per-stage totals
+    M->ev_used -= M->ev_used % (OCN_NSTAGES + 1);   // a step that failed between two marks left an incomplete group: drop it
     if (M->ev_used == 0) return OCN_OK;
     CK(cudaStreamSynchronize(M->stream));
-    for (size_t q = 0; q + OCN_NSTAGES < M->ev_used + 1 && q < M->ev_used; q += OCN_NSTAGES + 1)
+    for (size_t q = 0; q + OCN_NSTAGES < M->ev_used; q += OCN_NSTAGES + 1)
         for (int s = 0; s < OCN_NSTAGES; ++s) {
             static const int in_time_order[OCN_NSTAGES] = {0, 1, 3, 2};   // the closure stage runs before K3
             float ms = 0.f;
@@ -311,6 +330,7 @@ template <class T>
 ocn_status launch_step(ocn_model* M, bool euler) {
     const ocn_grid* g = M->g;
     ocn_status ps;
+    M->ev_used -= M->ev_used % (OCN_NSTAGES + 1);   // groups start on a step boundary (see prof_flush)
     if (M->profiling && M->ev_used + OCN_NSTAGES + 1 > 4096 && (ps = prof_flush(M)) != OCN_OK) return ps;
 #define MARK(stage, n)                                                   \
     do {                                                                 \
@@ -517,6 +537,8 @@ ocn_status ocn_grid_create(const ocn_grid_desc* d, const double* z_faces, const 
     if (d->kind != 0 && d->kind != 1) return fail(OCN_EINVAL, "kind must be 0 (cartesian) or 1 (lat-lon)");
     if (d->kind == 1 && d->periodic_y) return fail(OCN_EINVAL, "a lat-lon grid cannot be periodic in latitude");
     if (!(d->dx > 0) || !(d->dy > 0)) return fail(OCN_EINVAL, "dx, dy must be positive");
+    if (z_faces[d->nz] != 0.0) return fail(OCN_EINVAL, "z_faces[nz] must be 0 (the resting surface)");
+    for (int k = 0; k <= d->nz; ++k) if (!std::isfinite(z_faces[k])) return fail(OCN_EINVAL, "z_faces must be finite");
     ocn_grid* g = new (std::nothrow) ocn_grid();
     if (!g) return fail(OCN_ENOMEM, "host allocation failed");
     try {
@@ -557,6 +579,12 @@ ocn_status ocn_model_create(const ocn_grid* g, const ocn_model_desc* d, ocn_mode
     if (d->precision != 32 && d->precision != 64) return fail(OCN_EINVAL, "precision must be 32 or 64");
     if (!(d->dt > 0) || d->substeps < 1) return fail(OCN_EINVAL, "dt must be > 0 and substeps >= 1");
     if (!(d->rho0 > 0)) return fail(OCN_EINVAL, "rho0 must be > 0");
+    {
+        const double nonneg[] = {d->chi, d->g, d->nu_h, d->kappa_h, d->nu_z, d->kappa_z};
+        for (double x : nonneg) if (!(x >= 0) || !std::isfinite(x)) return fail(OCN_EINVAL, "chi, g, nu_h, kappa_h, nu_z, kappa_z must be finite and >= 0");
+        const double fin[] = {d->dt, d->alpha, d->beta_s, d->T0, d->S0, d->rho0, d->gamma_T, d->gamma_S, d->drag_r, d->drag_cd};
+        for (double x : fin) if (!std::isfinite(x)) return fail(OCN_EINVAL, "model parameters must be finite");
+    }
     if (!(d->gamma_T >= 0) || !(d->gamma_S >= 0)) return fail(OCN_EINVAL, "gamma_T, gamma_S must be >= 0");
     if (!(d->drag_r >= 0) || !(d->drag_cd >= 0)) return fail(OCN_EINVAL, "drag_r, drag_cd must be >= 0");
     if (d->closure != 0 && d->closure != 1) return fail(OCN_EINVAL, "closure must be 0 (constant) or 1 (Ri-based)");
@@ -566,7 +594,7 @@ ocn_status ocn_model_create(const ocn_grid* g, const ocn_model_desc* d, ocn_mode
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
         return fail(OCN_ECUDA, "no CUDA device: libocn has no CPU fallback");
     if (d->device < 0 || d->device >= ndev) return fail(OCN_EINVAL, "bad device ordinal");
-    CK(cudaSetDevice(d->device));
+    ON_DEVICE(d->device);
     ocn_model* M = new (std::nothrow) ocn_model();
     if (!M) return fail(OCN_ENOMEM, "host allocation failed");
     M->g = g; M->d = *d; M->prec = d->precision;
@@ -574,7 +602,12 @@ ocn_status ocn_model_create(const ocn_grid* g, const ocn_model_desc* d, ocn_mode
     const int Ms = d->substeps;
     M->a_w.resize(Ms);
     if (d->filter_weights) {
-        for (int m = 0; m < Ms; ++m) M->a_w[m] = d->filter_weights[m];
+        double sum = 0;
+        for (int m = 0; m < Ms; ++m) { M->a_w[m] = d->filter_weights[m]; sum += M->a_w[m]; }
+        if (!std::isfinite(sum) || std::fabs(sum - 1.0) > 1e-9) {
+            delete M;
+            return fail(OCN_EINVAL, "filter_weights must be finite and sum to 1 (they average eta, U, V over the sub-cycle)");
+        }
     } else {
         double sum = 0;
         for (int m = 1; m <= Ms; ++m) { const double s = (double)m / (double)(Ms + 1); M->a_w[m - 1] = s * s * (1.0 - s * s * s * s); sum += M->a_w[m - 1]; }
@@ -609,7 +642,7 @@ ocn_status ocn_model_create(const ocn_grid* g, const ocn_model_desc* d, ocn_mode
 
 ocn_status ocn_model_destroy(ocn_model* M) {
     if (!M) return OCN_OK;
-    cudaSetDevice(M->d.device);
+    DeviceGuard guard_(M->d.device);
     if (M->stream) cudaStreamSynchronize(M->stream);
     if (M->graph) cudaGraphExecDestroy(M->graph);
     for (cudaEvent_t e : M->ev_pool) cudaEventDestroy(e);
@@ -626,19 +659,19 @@ ocn_status ocn_model_destroy(ocn_model* M) {
 ocn_status ocn_set_fields(ocn_model* M, const ocn_fields* f) {
     if (!M || !f) return fail(OCN_EINVAL, "null argument");
     if (f->w) return fail(OCN_EINVAL, "w is diagnostic (get only)");
-    CK(cudaSetDevice(M->d.device));
+    ON_DEVICE(M->d.device);
     return M->prec == 32 ? set_fields_t<float>(M, f) : set_fields_t<double>(M, f);
 }
 
 ocn_status ocn_time_step(ocn_model* M, int n) {
     if (!M || n < 0) return fail(OCN_EINVAL, "bad argument");
-    CK(cudaSetDevice(M->d.device));
+    ON_DEVICE(M->d.device);
     return M->prec == 32 ? run_steps<float>(M, n) : run_steps<double>(M, n);
 }
 
 ocn_status ocn_get_fields(ocn_model* M, ocn_fields* f) {
     if (!M || !f) return fail(OCN_EINVAL, "null argument");
-    CK(cudaSetDevice(M->d.device));
+    ON_DEVICE(M->d.device);
     return M->prec == 32 ? get_fields_t<float>(M, f) : get_fields_t<double>(M, f);
 }
 
@@ -657,7 +690,7 @@ ocn_status ocn_model_info(const ocn_model* M, int* launches, unsigned long long*
 
 ocn_status ocn_profile_enable(ocn_model* M, int on) {
     if (!M) return fail(OCN_EINVAL, "null model");
-    CK(cudaSetDevice(M->d.device));
+    ON_DEVICE(M->d.device);
     if (!on) { const ocn_status s = prof_flush(M); if (s != OCN_OK) return s; }
     M->profiling = on != 0;
     return OCN_OK;
@@ -665,7 +698,7 @@ ocn_status ocn_profile_enable(ocn_model* M, int on) {
 
 ocn_status ocn_profile_read(ocn_model* M, double* ms, long long* launches, int reset) {
     if (!M) return fail(OCN_EINVAL, "null model");
-    CK(cudaSetDevice(M->d.device));
+    ON_DEVICE(M->d.device);
     const ocn_status s = prof_flush(M);
     if (s != OCN_OK) return s;
     for (int q = 0; q < OCN_NSTAGES; ++q) {
@@ -683,14 +716,14 @@ const char* ocn_stage_name(int stage) {
 
 ocn_status ocn_get_debug(ocn_model* M, double* Gu, double* Gv, double* GT, double* GS, double* U, double* V) {
     if (!M) return fail(OCN_EINVAL, "null model");
-    CK(cudaSetDevice(M->d.device));
+    ON_DEVICE(M->d.device);
     return M->prec == 32 ? get_debug_t<float>(M, Gu, Gv, GT, GS, U, V) : get_debug_t<double>(M, Gu, Gv, GT, GS, U, V);
 }
 
 ocn_status ocn_get_mixing(ocn_model* M, double* nu, double* kappa) {
     if (!M) return fail(OCN_EINVAL, "null model");
     if (M->d.closure != 1) return fail(OCN_ESTATE, "model was created with closure = 0");
-    CK(cudaSetDevice(M->d.device));
+    ON_DEVICE(M->d.device);
     return M->prec == 32 ? get_mixing_t<float>(M, nu, kappa) : get_mixing_t<double>(M, nu, kappa);
 }
 

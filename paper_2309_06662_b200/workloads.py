@@ -50,6 +50,21 @@ def with_ri_closure(wl, nu0=5e-3, c=5.0, kconv=0.1, n2c=1e-5, s2min=1e-10):
     return wl
 
 
+def with_nonlinear_eos(wl, alpha2=1e-5, gamma=2e-4):
+    """Switches a workload to the nonlinear equation of state of DESIGN.md §3.16: thermobaric
+    (alpha grows with depth at rate gamma [1/m]) and cabbeling (alpha2 [1/K^2]) terms; parameters only."""
+    wl["params"].update(eos=1, eos_alpha2=float(alpha2), eos_gamma=float(gamma))
+    wl["name"] = wl.get("name", "") + "+eos"
+    return wl
+
+
+def with_weno_z(wl):
+    """Switches a workload to WENO-Z nonlinear weights; parameters only."""
+    wl["params"].update(advection=1)
+    wl["name"] = wl.get("name", "") + "+wenoz"
+    return wl
+
+
 def with_surface_forcing(wl, seed=SEED_BASE + 40, heat=2e-5, salt=2e-6, piston=1e-5):
     """Adds seeded surface tracer forcing to a workload (the realistic runs are "forced by realistic
     surface momentum, heat, and salinity fluxes"; ECCO2 data are not available, these stand in for their shape):

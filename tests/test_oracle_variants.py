@@ -1,0 +1,146 @@
+"""Pins of the scheme variants the oracle offers beyond the north_star path:
+WENO-Z nonlinear weights (`advection = 1`) and the nonlinear equation of state with thermobaricity and
+cabbeling (`eos = 1`).  Each is pinned by an exact hand calculation or a closed form, by the mathematical
+properties of the family, and by the limit in which it reproduces the default scheme bit for bit."""
+import json
+import os
+from fractions import Fraction
+
+import numpy as np
+
+import oracle
+from paper_2309_06662_b200 import workloads as W
+from util import box
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+# =============================================================================================
+# WENO-Z
+# =============================================================================================
+def test_wenoz_matches_exact_rational_hand_calculation():
+    """golden/wenoz_worked.json, written by tests/golden/make_wenoz_worked.py with python Fractions (imports no
+    implementation): Borges et al. (2008) weights on the Jiang-Shu candidates, eps = 1e-6 exactly."""
+    with open(os.path.join(GOLD, "wenoz_worked.json")) as fh:
+        cases = json.load(fh)["cases"]
+    assert len(cases) >= 8
+    for c in cases:
+        exact = Fraction(int(c["num"]), int(c["den"]))
+        got = oracle.weno(c["cells"], c["order"], c["vel"], scheme=1)
+        assert abs(got - float(exact)) <= 4e-15 * max(1.0, abs(float(exact))), c
+    # and it is a different scheme from Jiang-Shu on non-smooth data
+    assert abs(oracle.weno([1, 2, 4, 8, 16, 32], 3, 1, scheme=1) - oracle.weno([1, 2, 4, 8, 16, 32], 3, 1, scheme=0)) > 1e-3
+
+
+def test_wenoz_is_exact_on_quadratics_and_linears_and_mirror_symmetric():
+    rng = np.random.default_rng(3)
+    for _ in range(50):
+        a, b, c = rng.standard_normal(3) * (1.0, 3.0, 2.0)
+        F = lambda x: a * x + b * x * x / 2 + c * x ** 3 / 3          # noqa: E731  antiderivative of the quadratic
+        avg = np.array([F(m + 1.0) - F(m + 0.0) for m in range(-3, 3)])   # unit cells -3..2, face at x = 0
+        for vel in (1.0, -1.0):
+            assert abs(oracle.weno(avg, 3, vel, 1) - a) < 1e-12 * (1 + abs(a) + abs(b) + abs(c))
+        lin = np.array([a * (m + 0.5) + b for m in range(-3, 3)])
+        for vel in (1.0, -1.0):
+            assert abs(oracle.weno(lin, 2, vel, 1) - b) < 1e-13 * (1 + abs(a) + abs(b))
+        cells = rng.standard_normal(6)
+        for order in (1, 2, 3):
+            assert oracle.weno(cells, order, 1.0, 1) == oracle.weno(cells[::-1].copy(), order, -1.0, 1)
+        assert oracle.weno(np.full(6, 4.25), 3, 1.0, 1) == 4.25
+
+
+def test_wenoz_is_closer_to_the_linear_scheme_on_smooth_data_and_fifth_order():
+    """The point of the Z weights: on smooth data they stay closer to the linear fifth-order weights than Jiang-Shu's, so the
+    error against the exact face value is smaller at every resolution; at a step both fall back to the smooth side."""
+    A = 1000.0                              # beta >> eps at every resolution used
+
+    def errs(N, scheme):
+        h = 2 * np.pi / N
+        xs = np.arange(-4, N + 4) * h
+        avg = A * (np.cos(xs[:-1]) - np.cos(xs[1:])) / h
+        return max(abs(oracle.weno(avg[n - 3:n + 3], 3, 1.0, scheme) - A * np.sin(xs[n])) for n in range(4, N + 3))
+    prev = None
+    for N in (32, 64, 128):
+        ejs, ez = errs(N, 0), errs(N, 1)
+        assert ez < 0.5 * ejs, (N, ejs, ez)
+        if prev is not None:
+            assert np.log2(prev / ez) > 4.8, (N, prev, ez)
+        prev = ez
+    # essentially non-oscillatory at a step, from both sides
+    assert abs(oracle.weno([0, 0, 0, 1, 1, 1], 3, 1.0, 1)) < 1e-10 and abs(oracle.weno([0, 0, 0, 1, 1, 1], 3, -1.0, 1) - 1) < 1e-10
+
+
+def test_wenoz_model_conserves_tracers_and_differs_from_js():
+    wl = W.with_weno_z(W.config2(nx=72, ny=30, nz=12, steps=10))
+    rng = np.random.default_rng(1)
+    wl["fields"]["u"] = 0.2 * rng.standard_normal(wl["fields"]["u"].shape)
+    wl["fields"]["v"] = 0.2 * rng.standard_normal(wl["fields"]["v"].shape)
+    m = oracle.RefModel(wl)
+    vol = m.grid.masks()["wet"] * np.diff(wl["z_faces"])[:, None, None] * m.grid.metrics()["AzC"][None, :, None]
+    f0 = m.get_fields()
+    m.step(10)
+    f1 = m.get_fields()
+    for n in "TS":
+        assert abs(np.sum(vol * f1[n]) / np.sum(vol * f0[n]) - 1.0) < 2e-14
+    wl0 = dict(wl, params=dict(wl["params"], advection=0))
+    m0 = oracle.RefModel(wl0)
+    m0.step(10)
+    assert np.abs(m0.get_fields()["T"] - f1["T"]).max() > 1e-6
+
+
+# =============================================================================================
+# nonlinear equation of state
+# =============================================================================================
+def test_nonlinear_eos_with_zero_coefficients_is_the_linear_one_bit_for_bit():
+    wl = W.config2(nx=48, ny=20, nz=10, steps=4)
+    a = oracle.RefModel(wl)
+    b = oracle.RefModel(W.with_nonlinear_eos(dict(wl, params=dict(wl["params"])), alpha2=0.0, gamma=0.0))
+    a.step(4); b.step(4)
+    fa, fb = a.get_fields(), b.get_fields()
+    for n in ("u", "v", "w", "eta", "T", "S"):
+        assert np.array_equal(fa[n], fb[n]), n
+
+
+def test_nonlinear_eos_pressure_closed_form_thermobaric_and_cabbeling():
+    """A column with a depth-independent anomaly dT: b(z) = g [alpha (1 - gamma z) dT + alpha2/2 dT^2] is linear in z, the
+    trapezoid rule between centres is exact for it, and the top half cell uses b at the top centre:
+        p(z_k) = b(z_t) z_t - [B(z_t) - B(z_k)],   B'(z) = b(z),  z_t = centre of the top cell."""
+    nz = 7
+    zf = W.geometric_z_faces(nz, 20.0, 1500.0)
+    wl = W.with_nonlinear_eos(box(nx=6, ny=5, nz=nz, depth=1500.0, z_faces=zf), alpha2=1.3e-5, gamma=2.5e-4)
+    dT = 3.5
+    wl["fields"]["T"][:] = 10.0 + dT
+    P = wl["params"]
+    m = oracle.RefModel(wl)
+    p = m.diagnostics()["p"][:, 2, 3]
+    zc = 0.5 * (zf[1:] + zf[:-1])
+    g, al, a2, ga = P["g"], P["alpha"], P["eos_alpha2"], P["eos_gamma"]
+    b = lambda z: g * (al * (1 - ga * z) * dT + 0.5 * a2 * dT * dT)                    # noqa: E731
+    B = lambda z: g * (al * dT * (z - ga * z * z / 2) + 0.5 * a2 * dT * dT * z)       # noqa: E731
+    zt = zc[-1]
+    want = b(zt) * zt - (B(zt) - B(zc))
+    assert np.max(np.abs(p - want)) < 1e-13 * np.max(np.abs(want))
+    # thermobaricity: the same temperature contrast pushes harder at depth.  T = T0 + s i: at rest
+    # G_u = -(p[i] - p[i-1]) / dx = -(s / dT) want(z_k) / dx for the linear part, the cabbeling part grows with i
+    wl2 = W.with_nonlinear_eos(box(nx=6, ny=5, nz=nz, depth=1500.0, z_faces=zf, periodic=(0, 0)), alpha2=0.0, gamma=2.5e-4)
+    s = 0.25
+    wl2["fields"]["T"][:] = 10.0 + s * np.arange(6)[None, None, :]
+    Gu = oracle.RefModel(wl2).tendencies()["Gu"]
+    lin = g * al * s * (zt * (1 - ga * zt) - ((zt - ga * zt * zt / 2) - (zc - ga * zc * zc / 2)))      # d p / d i
+    assert np.max(np.abs(Gu[:, 2, 1:] + lin[:, None] / 1000.0)) < 1e-12 * np.max(np.abs(lin)) / 1000.0
+    assert abs(Gu[0, 2, 3]) > 1.12 * abs(g * al * s * zc[0] / 1000.0)                 # stronger than the linear EOS at depth
+
+
+def test_cabbeling_mixing_two_parcels_makes_denser_water():
+    """alpha2 > 0 makes b convex in T: the mixture of two parcels is less buoyant than the mean of their buoyancies.  Seen
+    through the hydrostatic pressure of three one-column states (the top-cell rule p = -b (0 - z_t))."""
+    nz = 4
+    zf = np.array([-400.0, -300.0, -200.0, -100.0, 0.0])
+
+    def top_b(T):
+        wl = W.with_nonlinear_eos(box(nx=4, ny=4, nz=nz, depth=400.0, z_faces=zf), alpha2=1e-5, gamma=0.0)
+        wl["fields"]["T"][:] = T
+        return oracle.RefModel(wl).diagnostics()["p"][-1, 0, 0] / (-50.0)              # p_top = b z_t, z_t = -50
+    b1, b2, bm = top_b(2.0), top_b(22.0), top_b(12.0)
+    P = W._params(64, 1, 1, 0, 0)
+    assert abs((0.5 * (b1 + b2) - bm) - P["g"] * 0.5 * 1e-5 * 100.0) < 1e-12          # g alpha2/2 ((dT1^2 + dT2^2)/2 - dTm^2) = g alpha2/2 * 100
