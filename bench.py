@@ -35,12 +35,10 @@ METRIC = "cell_updates_per_s"
 UNIT = "cell-updates/s"
 # algorithmic HBM bytes per wet cell-update of each stage: compulsory reads + writes; every array is
 # `word` bytes per value except the hydrostatic pressure, which is stored in fp64 in both precisions
-# With the Ri closure (--closure ri): K4 reads uv, ts and writes (nu, kappa) = 6 words; K5 reads phi* (4) and
-# (nu, kappa) (2), writes d (4) and the super-diagonals (3) = 13 words; K3 reads the 3 super-diagonals on top.
+# With the Ri closure (--closure ri) K1 evaluates (nu, kappa) on chip and writes the 3 modified
+# super-diagonals of the per-column solves, which K3 reads: + 3 words each.
 def stage_bytes(stage, word, closure=0):
-    b = {"tendency": 16 * word + 8, "backsub_correct_pressure": (8 + (3 if closure else 0)) * word + 8}
-    if closure:
-        b["vertical_mixing"] = 19 * word
+    b = {"tendency": (16 + (3 if closure else 0)) * word + 8, "backsub_correct_pressure": (8 + (3 if closure else 0)) * word + 8}
     return b.get(stage)
 # window of config 4 the oracle is timed on: (j0, j1, i0, i1)
 CPU_WINDOW = (500, 700, 1300, 1700)

@@ -80,7 +80,8 @@ typedef struct {
      * closure = 1: at every open vertical face of a tracer column
      *   nu = nu_z + ri_nu0 f^2 + conv,  kappa = kappa_z + ri_nu0 f^3 + conv,  f = 1 / (1 + ri_c Ri),
      *   Ri = max(N2, 0) / (S2 + ri_s2min),  conv = ri_kconv min(1, max(-N2, 0) / ri_n2c),
-     * evaluated from state n; ri_n2c, ri_s2min > 0, the others >= 0.  Costs three more 3-D arrays. */
+     * evaluated from state n inside the fused tendency kernel; ri_n2c, ri_s2min > 0, the others >= 0.  Costs three more
+     * 3-D words per cell (the modified super-diagonals of the per-column solves). */
     int closure;
     double ri_nu0, ri_c, ri_kconv, ri_n2c, ri_s2min;
     /* Surface restoring of the top-cell tracers toward ocn_fields.restore_T / restore_S with piston velocities
@@ -89,6 +90,14 @@ typedef struct {
     /* Bottom drag on the lowest open level of every u / v column:
      * G_u -= (drag_r + drag_cd |u|) u / dz with |u| the speed at the point; drag_r [m/s], drag_cd [-], >= 0, 0 = off. */
     double drag_r, drag_cd;
+    /* Equation of state.  0 = linear (north_star).  1 = nonlinear:
+     * b = g [alpha (1 - eos_gamma z) (T - T0) + eos_alpha2 / 2 (T - T0)^2 - beta_s (S - S0)], z <= 0 the cell-centre depth:
+     * thermobaricity eos_gamma [1/m] and cabbeling eos_alpha2 [1/K^2]; both 0 reproduces eos = 0 bit for bit. */
+    int eos;
+    double eos_alpha2, eos_gamma;
+    /* Nonlinear weights of the WENO reconstructions ("based on WENO reconstructions", the family of refs
+     * PAPER.md:244-245): 0 = Jiang-Shu (north_star reading), 1 = WENO-Z. */
+    int advection;
 } ocn_model_desc;
 
 /* ocn_model_create — the model of PAPER.md:84 (§5.2: hydrostatic Boussinesq, IMEX quasi-AB2, backward-Euler vertical
@@ -132,6 +141,14 @@ ocn_status ocn_time_step(ocn_model* model, int n);
  * closed faces = 0); returns after the copies have completed (host buffers are valid on return).
  * Errors: OCN_EINVAL, OCN_ECUDA (including asynchronous faults of earlier steps). */
 ocn_status ocn_get_fields(ocn_model* model, ocn_fields* fields);
+/* The same read-back left in flight: returns as soon as the gathers and copies are enqueued (they run on a copy stream of
+ * the library beside later steps) and writes a ticket; the buffers are valid after ocn_wait(model, ticket) — or after any
+ * later blocking ocn_get_fields / ocn_synchronize.  Lets a caller enqueue step n+1 while the result of step n travels
+ * (one exchange per step, overlapped as the paper overlaps its communication). */
+ocn_status ocn_get_fields_async(ocn_model* model, ocn_fields* fields, unsigned long long* ticket);
+/* Blocks until the read-back named by `ticket` (and every earlier one) has landed.  OCN_EINVAL for a ticket never issued. */
+ocn_status ocn_wait(ocn_model* model, unsigned long long ticket);
+/* Blocks until everything enqueued by earlier calls (steps and copies) has completed. */
 ocn_status ocn_synchronize(ocn_model* model);
 
 /* Expanded 3-D integer masks for the bit-exact test (HOST buffers, NULL = skip): wet, order_x,
@@ -147,8 +164,8 @@ ocn_status ocn_model_info(const ocn_model* model, int* launches_per_step, unsign
 /* Per-stage device timing (used by bench.py for the roofline of the dominant kernel).
  * Stages: 0 = K1 fused tendency / AB2 / elimination, 1 = barotropic sub-cycle (all M sub-steps +
  * finish; the sub-cycle runs BT_HALO sub-steps per launch on shared-memory tiles), 2 = K3 back-substitution / correction / pressure,
- * 3 = vertical mixing closure (K4 mixing coefficients + K5 per-column elimination; runs between stages 1 and 2, no
- * launches when closure = 0).  (w is recomputed on the fly inside
+ * 3 = unused since the vertical mixing closure is evaluated inside stage 0 (always 0 launches; kept so that the stage
+ * indices are stable).  (w is recomputed on the fly inside
  * K1 and written out only when ocn_get_fields asks for it.)
  * While enabled, ocn_time_step launches the kernels of a step directly (no CUDA graph) and
  * records a CUDA event on the model's stream between stages.  ocn_profile_read synchronises

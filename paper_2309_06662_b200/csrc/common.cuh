@@ -75,6 +75,11 @@ struct DevP {
     T2* cpuv;
     T* cpt;
     double ri_nu0, ri_c, ri_kconv, ri_n2c, ri_s2min, nu_z_d, kappa_z_d;
+    // equation of state: eos = 1 adds thermobaricity and cabbeling,
+    //   b = g [ath[k] dT + ha2 dT dT - beta dS],  ath[k] = alpha (1 - gamma zc[k]),  ha2 = alpha2 / 2   (built on the host in fp64)
+    int eos;
+    const double* ath_d;
+    double ha2_d;
 };
 
 template <class T>
@@ -146,7 +151,9 @@ __device__ __forceinline__ Xv<double> xdiv(Xv<double> a, double b, double) { ret
 __device__ __forceinline__ Xv<float> xdiv(Xv<float> a, float, float rb) { return Xv<float>(a.v * rb); }
 template <class T> __device__ __forceinline__ Xv<T> X(T v) { return Xv<T>(v); }
 
-// fp64 face value with the weights evaluated as written in DESIGN.md §3.4 (alpha_s = d_s / (eps + beta_s)^2)
+// fp64 face value with the weights evaluated as written in DESIGN.md §3.4 (alpha_s = d_s / (eps + beta_s)^2) or, WZ, as
+// written in DESIGN.md §3.15 (WENO-Z: alpha_s = d_s (1 + (tau / (eps + beta_s))^2), tau = |beta_0 - beta_{r-1}|)
+template <bool WZ>
 __device__ __forceinline__ double weno_face_exact(double a, double b, double c, double d, double e, double f, double vel, int order) {
     typedef Xv<double> V;
     const bool pos = vel > 0.0;
@@ -160,12 +167,24 @@ __device__ __forceinline__ double weno_face_exact(double a, double b, double c, 
         const V b0 = c13 * (qm2 - two * qm1 + q0) * (qm2 - two * qm1 + q0) + c4 * (qm2 - V(4.0) * qm1 + V(3.0) * q0) * (qm2 - V(4.0) * qm1 + V(3.0) * q0);
         const V b1 = c13 * (qm1 - two * q0 + q1) * (qm1 - two * q0 + q1) + c4 * (qm1 - q1) * (qm1 - q1);
         const V b2 = c13 * (q0 - two * q1 + q2) * (q0 - two * q1 + q2) + c4 * (V(3.0) * q0 - V(4.0) * q1 + q2) * (V(3.0) * q0 - V(4.0) * q1 + q2);
+        if (WZ) {
+            const V tau(fabs((b0 - b2).v)), one(1.0);
+            const V r0 = tau / (eps + b0), r1 = tau / (eps + b1), r2 = tau / (eps + b2);
+            const V a0 = V(0.1) * (one + r0 * r0), a1 = V(0.6) * (one + r1 * r1), a2 = V(0.3) * (one + r2 * r2);
+            return ((a0 * p0 + a1 * p1 + a2 * p2) / (a0 + a1 + a2)).v;
+        }
         const V a0 = V(0.1) / ((eps + b0) * (eps + b0)), a1 = V(0.6) / ((eps + b1) * (eps + b1)), a2 = V(0.3) / ((eps + b2) * (eps + b2));
         return ((a0 * p0 + a1 * p1 + a2 * p2) / (a0 + a1 + a2)).v;
     }
     if (order == 2) {
         const V p0 = (-qm1 + V(3.0) * q0) / two, p1 = (q0 + q1) / two;
         const V b0 = (q0 - qm1) * (q0 - qm1), b1 = (q1 - q0) * (q1 - q0);
+        if (WZ) {
+            const V tau(fabs((b0 - b1).v)), one(1.0);
+            const V r0 = tau / (eps + b0), r1 = tau / (eps + b1);
+            const V a0 = V(1.0 / 3.0) * (one + r0 * r0), a1 = V(2.0 / 3.0) * (one + r1 * r1);
+            return ((a0 * p0 + a1 * p1) / (a0 + a1)).v;
+        }
         const V a0 = V(1.0 / 3.0) / ((eps + b0) * (eps + b0)), a1 = V(2.0 / 3.0) / ((eps + b1) * (eps + b1));
         return ((a0 * p0 + a1 * p1) / (a0 + a1)).v;
     }
@@ -177,14 +196,18 @@ __device__ __forceinline__ double weno_face_exact(double a, double b, double c, 
 // (a, b, c, d, e, f); the face lies between c and d; q0 is the upwind cell.
 // Division-free nonlinear weights: alpha_s ~ d_s * prod_{t != s} (eps + beta_t)^2, one division.
 // ---------------------------------------------------------------------------------------------
+template <bool WZ>
 __device__ __forceinline__ double weno_face(double a, double b, double c, double d, double e, double f, double vel, int order) {
-    return weno_face_exact(a, b, c, d, e, f, vel, order);
+    return weno_face_exact<WZ>(a, b, c, d, e, f, vel, order);
 }
 // quotient of the weighted sum: reciprocal-based in fp32 (2 ulp), exact in fp64
 __device__ __forceinline__ float fquot(float a, float b) { return __fdividef(a, b); }
 __device__ __forceinline__ double fquot(double a, double b) { return a / b; }
-template <class T>
-__device__ __forceinline__ T weno_face(T a, T b, T c, T d, T e, T f, T vel, int order) {
+// WZ (fp32): the WENO-Z weights in the same division-free form, alpha_s ~ d_s (B_s^2 + tau^2) prod_{t != s} B_t^2 with
+// B = eps + beta (>= 1e-6, so the triple products stay normal numbers)
+template <bool WZ>
+__device__ __forceinline__ float weno_face(float a, float b, float c, float d, float e, float f, float vel, int order) {
+    typedef float T;
     const bool pos = vel > T(0);
     const T qm2 = pos ? a : f, qm1 = pos ? b : e, q0 = pos ? c : d, q1 = pos ? d : c, q2 = pos ? e : b;
     const T eps = T(1e-6);
@@ -198,6 +221,11 @@ __device__ __forceinline__ T weno_face(T a, T b, T c, T d, T e, T f, T vel, int 
         const T b0 = eps + T(13.0 / 12.0) * s0 * s0 + T(0.25) * t0 * t0;
         const T b1 = eps + T(13.0 / 12.0) * s1 * s1 + T(0.25) * t1 * t1;
         const T b2 = eps + T(13.0 / 12.0) * s2 * s2 + T(0.25) * t2 * t2;
+        if (WZ) {
+            const T tau = b0 - b2, t2 = tau * tau, q0_ = b0 * b0, q1_ = b1 * b1, q2_ = b2 * b2;
+            const T a0 = T(0.1) * (q0_ + t2) * (q1_ * q2_), a1 = T(0.6) * (q1_ + t2) * (q0_ * q2_), a2 = T(0.3) * (q2_ + t2) * (q0_ * q1_);
+            return fquot(a0 * p0 + a1 * p1 + a2 * p2, a0 + a1 + a2);
+        }
         const T b01 = b0 * b1, b02 = b0 * b2, b12 = b1 * b2;
         const T a0 = T(0.1) * b12 * b12, a1 = T(0.6) * b02 * b02, a2 = T(0.3) * b01 * b01;
         return fquot(a0 * p0 + a1 * p1 + a2 * p2, a0 + a1 + a2);
@@ -205,6 +233,11 @@ __device__ __forceinline__ T weno_face(T a, T b, T c, T d, T e, T f, T vel, int 
     if (order == 2) {
         const T p0 = T(0.5) * (T(3) * q0 - qm1), p1 = T(0.5) * (q0 + q1);
         const T b0 = eps + (q0 - qm1) * (q0 - qm1), b1 = eps + (q1 - q0) * (q1 - q0);
+        if (WZ) {
+            const T tau = b0 - b1, t2 = tau * tau, q0_ = b0 * b0, q1_ = b1 * b1;
+            const T a0 = T(1.0 / 3.0) * (q0_ + t2) * q1_, a1 = T(2.0 / 3.0) * (q1_ + t2) * q0_;
+            return fquot(a0 * p0 + a1 * p1, a0 + a1);
+        }
         const T a0 = T(1.0 / 3.0) * b1 * b1, a1 = T(2.0 / 3.0) * b0 * b0;
         return fquot(a0 * p0 + a1 * p1, a0 + a1);
     }
@@ -224,6 +257,7 @@ __device__ __forceinline__ float2 mul2(float2 a, float2 b) { return __fmul2_rn(a
 __device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
 
 // fifth-order face value from the upwind-ordered stencil (q0 = upwind cell)
+template <bool WZ>
 __device__ __forceinline__ float2 weno5_pair(float2 qm2, float2 qm1, float2 q0, float2 q1, float2 q2) {
     const float2 p0 = fma2(f2(11.f / 6.f), q0, fma2(f2(-7.f / 6.f), qm1, mul2(f2(2.f / 6.f), qm2)));
     const float2 p1 = fma2(f2(2.f / 6.f), q1, fma2(f2(5.f / 6.f), q0, mul2(f2(-1.f / 6.f), qm1)));
@@ -235,34 +269,51 @@ __device__ __forceinline__ float2 weno5_pair(float2 qm2, float2 qm1, float2 q0, 
     const float2 b0 = fma2(mul2(c13, s0), s0, fma2(mul2(c4, t0), t0, eps));
     const float2 b1 = fma2(mul2(c13, s1), s1, fma2(mul2(c4, t1), t1, eps));
     const float2 b2 = fma2(mul2(c13, s2), s2, fma2(mul2(c4, t2), t2, eps));
-    const float2 b01 = mul2(b0, b1), b02 = mul2(b0, b2), b12 = mul2(b1, b2);
-    const float2 a0 = mul2(mul2(f2(0.1f), b12), b12), a1 = mul2(mul2(f2(0.6f), b02), b02), a2 = mul2(mul2(f2(0.3f), b01), b01);
+    float2 a0, a1, a2;
+    if (WZ) {
+        const float2 tau = fma2(f2(-1.f), b2, b0), t2 = mul2(tau, tau);
+        const float2 r0 = mul2(b0, b0), r1 = mul2(b1, b1), r2 = mul2(b2, b2);
+        a0 = mul2(mul2(f2(0.1f), add2(r0, t2)), mul2(r1, r2));
+        a1 = mul2(mul2(f2(0.6f), add2(r1, t2)), mul2(r0, r2));
+        a2 = mul2(mul2(f2(0.3f), add2(r2, t2)), mul2(r0, r1));
+    } else {
+        const float2 b01 = mul2(b0, b1), b02 = mul2(b0, b2), b12 = mul2(b1, b2);
+        a0 = mul2(mul2(f2(0.1f), b12), b12); a1 = mul2(mul2(f2(0.6f), b02), b02); a2 = mul2(mul2(f2(0.3f), b01), b01);
+    }
     const float2 num = fma2(a2, p2, fma2(a1, p1, mul2(a0, p0))), den = add2(add2(a0, a1), a2);
     return make_float2(__fdividef(num.x, den.x), __fdividef(num.y, den.y));
 }
+template <bool WZ>
 __device__ __forceinline__ float2 weno3_pair(float2 qm1, float2 q0, float2 q1) {
     const float2 p0 = fma2(f2(1.5f), q0, mul2(f2(-0.5f), qm1)), p1 = mul2(f2(0.5f), add2(q0, q1));
     const float2 d0 = fma2(f2(-1.f), qm1, q0), d1 = fma2(f2(-1.f), q0, q1);
     const float2 eps = f2(1e-6f);
     const float2 b0 = fma2(d0, d0, eps), b1 = fma2(d1, d1, eps);
-    const float2 a0 = mul2(mul2(f2(1.f / 3.f), b1), b1), a1 = mul2(mul2(f2(2.f / 3.f), b0), b0);
+    float2 a0, a1;
+    if (WZ) {
+        const float2 tau = fma2(f2(-1.f), b1, b0), t2 = mul2(tau, tau), r0 = mul2(b0, b0), r1 = mul2(b1, b1);
+        a0 = mul2(mul2(f2(1.f / 3.f), add2(r0, t2)), r1); a1 = mul2(mul2(f2(2.f / 3.f), add2(r1, t2)), r0);
+    } else {
+        a0 = mul2(mul2(f2(1.f / 3.f), b1), b1); a1 = mul2(mul2(f2(2.f / 3.f), b0), b0);
+    }
     const float2 num = fma2(a1, p1, mul2(a0, p0)), den = add2(a0, a1);
     return make_float2(__fdividef(num.x, den.x), __fdividef(num.y, den.y));
 }
 
 // face value of a pair with one advecting velocity and one order code
-template <class T2, class T>
-__device__ __forceinline__ T2 weno_face2(T2 a, T2 b, T2 c, T2 d, T2 e, T2 f, T vel, int order) {
-    T2 r;
-    r.x = weno_face(a.x, b.x, c.x, d.x, e.x, f.x, vel, order);
-    r.y = weno_face(a.y, b.y, c.y, d.y, e.y, f.y, vel, order);
+template <bool WZ>
+__device__ __forceinline__ double2 weno_face2(double2 a, double2 b, double2 c, double2 d, double2 e, double2 f, double vel, int order) {
+    double2 r;
+    r.x = weno_face<WZ>(a.x, b.x, c.x, d.x, e.x, f.x, vel, order);
+    r.y = weno_face<WZ>(a.y, b.y, c.y, d.y, e.y, f.y, vel, order);
     return r;
 }
+template <bool WZ>
 __device__ __forceinline__ float2 weno_face2(float2 a, float2 b, float2 c, float2 d, float2 e, float2 f, float vel, int order) {
     const bool pos = vel > 0.f;
     const float2 qm1 = pos ? b : e, q0 = pos ? c : d, q1 = pos ? d : c;
-    if (order >= 3) return weno5_pair(pos ? a : f, qm1, q0, q1, pos ? e : b);
-    if (order == 2) return weno3_pair(qm1, q0, q1);
+    if (order >= 3) return weno5_pair<WZ>(pos ? a : f, qm1, q0, q1, pos ? e : b);
+    if (order == 2) return weno3_pair<WZ>(qm1, q0, q1);
     return order == 1 ? q0 : make_float2(0.f, 0.f);
 }
 

@@ -44,7 +44,9 @@ inline std::string build_grid(ocn_grid& g, const ocn_grid_desc& d, const double*
     g.sx = roundup(nx + 2 * OCN_HALO + 2, 32);
     g.sy = ny + 2 * OCN_HALO;
     g.zf.assign(z_faces, z_faces + nz + 1);
+    for (int k = 0; k <= nz; ++k) if (!std::isfinite(g.zf[k])) return "z_faces must be finite";
     for (int k = 0; k < nz; ++k) if (!(g.zf[k + 1] > g.zf[k])) return "z_faces must be strictly increasing";
+    if (g.zf[nz] != 0.0) return "z_faces[nz] must be 0 (the resting surface)";
     g.dz.resize(nz); g.zc.resize(nz); g.dzc.assign(nz, 0.0);
     for (int k = 0; k < nz; ++k) { g.dz[k] = g.zf[k + 1] - g.zf[k]; g.zc[k] = 0.5 * (g.zf[k] + g.zf[k + 1]); }
     for (int k = 1; k < nz; ++k) g.dzc[k] = g.zc[k] - g.zc[k - 1];

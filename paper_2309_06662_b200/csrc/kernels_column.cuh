@@ -9,10 +9,15 @@ namespace ocn {
 // linear equation of state and one level of the downward pressure integral, in fp64 with the
 // rounding order of the equations as written; t, s are the stored (offset) tracers.  In fp32 runs this keeps
 // the rounding of p ~ 1e2 m^2/s^2 (whose horizontal differences drive the flow) out of the momentum equation.
+// eos = 1: b = g [ath[k] dT + ha2 dT dT - beta dS] with ath[k] = alpha (1 - gamma zc[k]) and ha2 = alpha2 / 2
+// built on the host with the same fp64 operations the equation is written in.
 template <class T>
-__device__ __forceinline__ double buoyancy(const DevP<T>& P, T t, T s) {
+__device__ __forceinline__ double buoyancy(const DevP<T>& P, int k, T t, T s) {
     typedef Ex<double> E;
-    return E::mul(P.g_d, E::sub(E::mul(P.alpha_d, E::sub((double)t, P.dT0_d)), E::mul(P.beta_d, E::sub((double)s, P.dS0_d))));
+    const double dT = E::sub((double)t, P.dT0_d), dS = E::sub((double)s, P.dS0_d);
+    if (P.eos == 1)
+        return E::mul(P.g_d, E::sub(E::add(E::mul(P.ath_d[k], dT), E::mul(E::mul(P.ha2_d, dT), dT)), E::mul(P.beta_d, dS)));
+    return E::mul(P.g_d, E::sub(E::mul(P.alpha_d, dT), E::mul(P.beta_d, dS)));
 }
 template <class T>
 __device__ __forceinline__ double pressure_level(const DevP<T>& P, int k, double b0, double b1, double p_above) {
@@ -296,7 +301,7 @@ __global__ void __launch_bounds__(128, sizeof(T) == 8 ? 4 : 8) k_backsub_correct
                 const T ck = RI ? c_t[q] : cpt[k * nz];
                 xt = E::sub(d_ts[q].x, E::mul(ck, xt));                      // cp[nz-1] = 0
                 xs = E::sub(d_ts[q].y, E::mul(ck, xs));
-                const double b0 = buoyancy(P, xt, xs);
+                const double b0 = buoyancy(P, k, xt, xs);
                 pk = pressure_level(P, k, b0, b1, pk);
                 b1 = b0;
                 ots = mk2(xt, xs); op = pk;
@@ -348,7 +353,7 @@ __global__ void __launch_bounds__(128) k_pressure(const DevP<T> P) {
     double b1 = 0, pk = 0;
     for (int k = nz - 1; k >= kb; --k) {
         const typename Pair<T>::type q = P.ts[k * sz + c];
-        const double b0 = buoyancy(P, q.x, q.y);
+        const double b0 = buoyancy(P, k, q.x, q.y);
         pk = pressure_level(P, k, b0, b1, pk);
         b1 = b0;
         store_halo(P.p + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, pk);

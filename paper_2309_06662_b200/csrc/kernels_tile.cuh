@@ -19,6 +19,7 @@
 #include <cuda.h>
 
 #include "common.cuh"
+#include "kernels_mixing.cuh"
 
 // First thread of the compacted work lists of a 256-thread CTA: v cells from 0 up, tracer cells from 64
 // up, faces from 160 up (wrapping), u cells from N-1 down.  On sparse levels the four lists land on different warps; on
@@ -57,13 +58,11 @@ __device__ __forceinline__ void tma_load_plane(void* dst, const CUtensorMap* map
 
 __host__ __device__ constexpr int rup128(int b) { return (b + 127) / 128 * 128; }
 
-// MODE 0: all four prognostic fields in one kernel; 1: the momentum group (u, v) only; 2: the tracer group (T, S) only.
-// The two group kernels read the same state, write disjoint outputs and run concurrently (ocn_api.cu); each has a
-// smaller register / shared-memory footprint than the fused one, so more CTAs are resident per SM.
-template <class T, int TX_, int TY_, int MODE_ = 0>
+// RI: the instantiation that evaluates the Ri-based vertical mixing closure inside the pass: two
+// more ring buffers hold (nu, kappa) at the upper face of the tile's columns (+ west / south ring).
+template <class T, int TX_, int TY_, bool RI_ = false>
 struct Tile {
-    static constexpr int MODE = MODE_;
-    static constexpr bool DO_T = MODE_ != 1, DO_M = MODE_ != 2;
+    static constexpr bool RI = RI_;
     typedef typename Pair<T>::type T2;
     static constexpr int TX = TX_, TY = TY_, NC = TX * TY, NT = NC;   // cells = threads; a thread owns the tracers of one cell and the momentum of another
     static constexpr int BX = TX + 8, BY = TY + 6;       // TMA box: origin (i0 - 4, j0 - 3)
@@ -71,27 +70,28 @@ struct Tile {
     static constexpr int DP = 2;                         // prefetch distance in levels
     // ring lengths are powers of two (slot of level q = q & (R - 1): no loop-carried slot state); needed: DP + 5, DP + 1, DP, 3
     static constexpr int R_TS = 8, R_UV = 4, R_P = 2, R_W = 4, NB = DP;
-    static_assert(DP + 5 <= R_TS && DP + 1 <= R_UV && DP <= R_P, "rings");
+    static_assert(DP + 5 <= R_TS && DP + 2 <= R_UV && DP <= R_P, "rings");      // RI fetches (u, v) one level earlier
     static constexpr int RX = TX + 1, RY = TY + 1;       // tile + west/south ring (K, D, w) or + east/north edge (faces, masks)
     static constexpr int PL2 = rup128(BX * BY * (int)sizeof(T2)), PL1 = rup128(BX * BY * (int)sizeof(T)),
                          PLP = rup128((TX + 4) * (TY + 1) * 8);   // pressure planes: fp64, box (TX + 4) x (TY + 1), origin (i0 - 4, j0 - 1)
     static constexpr int BYTES2 = BX * BY * (int)sizeof(T2), BYTESP = (TX + 4) * (TY + 1) * 8, PBX = TX + 4;
     // shared-memory map (byte offsets from a 128-byte aligned base)
     static constexpr int O_TS = 0;
-    static constexpr int O_UV = O_TS + (DO_T ? R_TS : 0) * PL2;
+    static constexpr int O_UV = O_TS + R_TS * PL2;
     static constexpr int O_P = O_UV + R_UV * PL2;
-    static constexpr int O_ZETA = O_P + (DO_M ? R_P : 0) * PLP;
-    static constexpr int O_KD = O_ZETA + (DO_M ? 2 : 0) * PL1;                               // 2 x T2 (K, D) on RX x RY
+    static constexpr int O_ZETA = O_P + R_P * PLP;
+    static constexpr int O_KD = O_ZETA + 2 * PL1;                               // 2 x T2 (K, D) on RX x RY
     static constexpr int KDB = rup128(RX * RY * (int)sizeof(T2)), WB = rup128(RX * RY * (int)sizeof(T));
     static constexpr int O_W = O_KD + 2 * KDB;                                  // R_W buffers of T on RX x RY (w at face f in slot f & 3)
     static constexpr int NFX = RX * TY, NFY = TX * RY, NF = NFX + NFY;        // west faces, then south faces
     static constexpr int FLB = rup128(NF * (int)sizeof(T2));
     static constexpr int O_FLUX = O_W + R_W * WB;                                 // 2 x T2 per face
-    static constexpr int O_M8 = O_FLUX + (DO_T ? 2 : 0) * FLB;                               // uint2 on RX x RY (not zero-filled from here on)
+    static constexpr int O_NK = O_FLUX + 2 * FLB;                                // RI: 2 x T2 (nu, kappa) on RX x RY, face f in slot f & 1
+    static constexpr int O_M8 = O_NK + (RI ? 2 : 0) * KDB;                       // uint2 on RX x RY (not zero-filled from here on)
     static constexpr int O_MET = O_M8 + rup128(RX * RY * 8);                    // 9 row-metric arrays of BY + 1
     static constexpr int O_CELL = O_MET + rup128(9 * (BY + 1) * (int)sizeof(T)); // uint16: cells sorted by first wet level
     static constexpr int O_FS = O_CELL + rup128(NC * 2);                        // uint2: face descriptors sorted by first open level
-    static constexpr int O_NC = O_FS + (DO_T ? rup128(NF * 8) : 0);                          // uint16[256]: active cells at level k
+    static constexpr int O_NC = O_FS + rup128(NF * 8);                          // uint16[256]: active cells at level k
     static constexpr int O_NF = O_NC + 512;                                     // uint16[256]: active faces at level k
     static constexpr int O_DZ = O_NF + 512;                                     // T[256] dz, T[256] 1 / dz
     static constexpr int O_BAR = O_DZ + 2 * 256 * (int)sizeof(T);
@@ -101,14 +101,15 @@ struct Tile {
 
 // DRAG: compiled with the bottom-drag term of DESIGN.md §3.14 (chosen by the host when drag_r or drag_cd is non-zero, so
 // that the default path does not carry its instructions: 10.17 ms against 10.37 ms with the term predicated off).
-template <class T, int TX, int TY, int MODE, int MINB, bool DRAG = false>
+// RI: the Ri-based closure evaluated in the pass (per-face diffusivities, per-column elimination in registers, the modified
+// super-diagonals stored for K3).  WZ: WENO-Z nonlinear weights instead of Jiang-Shu's.
+template <class T, int TX, int TY, int MINB, bool DRAG = false, bool RI = false, bool WZ = false>
 __global__ void __launch_bounds__(TX * TY, MINB)
 k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__ CUtensorMap m_ts,
                 const __grid_constant__ CUtensorMap m_uv, const __grid_constant__ CUtensorMap m_p) {
-    typedef Tile<T, TX, TY, MODE> C;
+    typedef Tile<T, TX, TY, RI> C;
     typedef typename C::T2 T2;
     typedef Ex<T> E;
-    constexpr bool DO_T = C::DO_T, DO_M = C::DO_M;
     constexpr int BX = C::BX, BY = C::BY, RX = C::RX, RY = C::RY, NT = C::NT, NC = C::NC, OX = C::OX, OY = C::OY;
     extern __shared__ __align__(1024) unsigned char sm[];     // dynamic only: starts the CTA's window, 1 KB aligned
     unsigned short* const s_cell = (unsigned short*)(sm + C::O_CELL);
@@ -169,7 +170,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     // first open level (stable counting sort on the 8-bit level), so that at level k the active work
     // is a dense prefix of each list and keeps the geometric order (coalescing) within a level ------
     {
-        constexpr int MAXR = DO_T ? (C::NF + NT - 1) / NT : 1;           // rounds of NT items
+        constexpr int MAXR = (C::NF + NT - 1) / NT;           // rounds of NT items
         unsigned short* const cnt = (unsigned short*)sm;                  // [virtual warp][key], scratch in the unused ts ring
         int* const base = (int*)(sm + MAXR * (NT / 32) * 256 * 2);        // [key] exclusive prefix, then [256 + w] warp sums
         static_assert(MAXR * (NT / 32) * 512 + 2048 <= C::O_M8, "sort scratch");
@@ -236,13 +237,13 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
         csort(NC, [&](int q) { return cell_key(q, 0); }, cell_emit, s_nc);
         constexpr int TOFF = K1_TOFF, VOFF = K1_VOFF;                     // first thread of the tracer and v lists (u runs from N-1 down, faces from K1_FOFF up)
         gT = s_cell[(tid + NC - TOFF) % NC];
-        if constexpr (DO_M) {
+        {
             csort(NC, [&](int q) { return cell_key(q, 1); }, cell_emit, s_nc);
             gU = s_cell[NC - 1 - tid];
             csort(NC, [&](int q) { return cell_key(q, 2); }, cell_emit, s_nc);
             gV = s_cell[(tid + NC - VOFF) % NC];
         }
-        if constexpr (DO_T) {
+        {
             // faces: fid < NFX = west face of cell (fid % RX, fid / RX); else south face of cell (g % TX, g / TX), g = fid - NFX
             auto face_cell = [&](int fid, bool& isy, int& fx, int& fy) {
                 isy = fid >= C::NFX;
@@ -287,15 +288,17 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     auto issue_group = [&](int m, bool first) {
         uint64_t* bar = &bars[(m - kmin) % C::NB];
         uint32_t bytes = 0;
-        const int tlo = first ? max(m - 3, 0) : m + 2, thi = DO_T ? min(m + 2, nz - 1) : -1;
+        const int tlo = first ? max(m - 3, 0) : m + 2, thi = min(m + 2, nz - 1);
+        // (u, v): plane m; RI needs plane m + 1 in iteration m (shear across the face above level m), so it runs one ahead
+        const int ulo = RI ? (first ? m : m + 1) : m, uhi = min(RI ? m + 1 : m, nz - 1);
         if (thi >= tlo) bytes += (uint32_t)(thi - tlo + 1) * C::BYTES2;
-        if (m < nz) bytes += C::BYTES2;
-        if (DO_M && m - 1 >= kmin) bytes += C::BYTESP;
-        if (bytes == 0) { mbar_arrive_plain(bar); return; }          // nothing to load for this iteration (tracer mode, m = nz)
+        if (uhi >= ulo) bytes += (uint32_t)(uhi - ulo + 1) * C::BYTES2;
+        if (m - 1 >= kmin) bytes += C::BYTESP;
+        if (bytes == 0) { mbar_arrive_plain(bar); return; }          // nothing to load for this iteration
         mbar_expect_tx(bar, bytes);
         for (int q = tlo; q <= thi; ++q) tma_load_plane(sm + C::O_TS + (q % C::R_TS) * C::PL2, &m_ts, bar, 2 * i0, j0, q);
-        if (m < nz) tma_load_plane(sm + C::O_UV + (m % C::R_UV) * C::PL2, &m_uv, bar, 2 * i0, j0, m);
-        if (DO_M && m - 1 >= kmin) tma_load_plane(sm + C::O_P + ((m - 1) % C::R_P) * C::PLP, &m_p, bar, i0, j0 + 2, m - 1);
+        for (int q = ulo; q <= uhi; ++q) tma_load_plane(sm + C::O_UV + (q % C::R_UV) * C::PL2, &m_uv, bar, 2 * i0, j0, q);
+        if (m - 1 >= kmin) tma_load_plane(sm + C::O_P + ((m - 1) % C::R_P) * C::PLP, &m_p, bar, i0, j0 + 2, m - 1);
     };
     // the TMA producer is a thread of a warp without part-A / part-B work on sparse levels (v cells run from thread 0,
     // tracer cells from 64, faces from 160, u cells from N-1 down): its issue latency stays off the critical path
@@ -335,10 +338,13 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     T ddu = 0, ddv = 0;
     T2 ddts = mk2(T(0), T(0));                           // eliminated right-hand sides of the level below
     double aGU = 0, aGV = 0, aSU = 0, aSV = 0;
+    // RI: the Thomas rows of this thread's columns and dt * diffusivity at the face below the current level
+    ThomasRow<T> rt{T(0), T(0), T(0)}, ru{T(0), T(0), T(0)}, rv{T(0), T(0), T(0)};
+    T kt_lo = 0, ku_lo = 0, kv_lo = 0;
 
     for (int m = kmin; m <= nz; ++m) {
         const int kB = m - 1;                                 // level of part B (phase 3) in this iteration
-        const bool doB = kB >= kmin, wetT = DO_T && doB && kB >= cT.t1, wetU = DO_M && doB && kB >= cU.t1, wetV = DO_M && doB && kB >= cV.t1;
+        const bool doB = kB >= kmin, wetT = doB && kB >= cT.t1, wetU = doB && kB >= cU.t1, wetV = doB && kB >= cV.t1;
         // AB2 history and pivots of level kB: issued now, consumed after part A.  A warp without an active cell or
         // face at this level (most warps on sparsely wet levels) skips this and all of part B.
         const bool anyB = __any_sync(0xffffffffu, wetT | wetU | wetV);
@@ -351,17 +357,17 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             if (wetT) {
                 oT = okB + cT.c;
                 gm_ts = P.Gts[oT];
-                piv_t = sizeof(T) == 8 ? P.m_t[kB * nz + cT.t1] : P.rm_t[kB * nz + cT.t1];
+                if (!RI) piv_t = sizeof(T) == 8 ? P.m_t[kB * nz + cT.t1] : P.rm_t[kB * nz + cT.t1];
             }
             if (wetU) {
                 oU = okB + cU.c;
                 gm_u = ((const T*)(P.Guv + oU))[0];
-                piv_u = sizeof(T) == 8 ? P.m_m[kB * nz + cU.t1] : P.rm_m[kB * nz + cU.t1];
+                if (!RI) piv_u = sizeof(T) == 8 ? P.m_m[kB * nz + cU.t1] : P.rm_m[kB * nz + cU.t1];
             }
             if (wetV) {
                 oV = okB + cV.c;
                 gm_v = ((const T*)(P.Guv + oV))[1];
-                piv_v = sizeof(T) == 8 ? P.m_m[kB * nz + cV.t1] : P.rm_m[kB * nz + cV.t1];
+                if (!RI) piv_v = sizeof(T) == 8 ? P.m_m[kB * nz + cV.t1] : P.rm_m[kB * nz + cV.t1];
             }
         }
         mbar_wait(&bars[(m - kmin) % C::NB], (uint32_t)(((m - kmin) / C::NB) & 1));
@@ -375,7 +381,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             T* __restrict__ s_w1 = (T*)(sm + C::O_W + ((k + 1) & (C::R_W - 1)) * C::WB);
             T2* __restrict__ s_flux = (T2*)(sm + C::O_FLUX + (k & 1) * C::FLB);
             // ================= phase 1: zeta, K, D, w[k+1] =================
-            if constexpr (DO_M) {
+            {
         #pragma unroll
                 for (int h = 0; h < (BX - 1) * (BY - 1); h += NT) {
                     const int q = h + (NT - 1 - tid);
@@ -400,10 +406,19 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                     double& wa = n == 0 ? wacc0 : wacc1;
                     wa = (X(wa) - X((double)dzk) * X((double)Dc)).v;
                     s_w1[q] = (T)wa;
+                    if constexpr (RI) if (k + 1 < nz) {     // (nu, kappa) at the face above level k of this column
+                        const T2* __restrict__ s_uvh = (const T2*)(sm + C::O_UV + ((k + 1) & (C::R_UV - 1)) * C::PL2);
+                        const T2 b = s_uvh[py * BX + px], be = s_uvh[py * BX + px + 1], bn = s_uvh[(py + 1) * BX + px];
+                        const T2 t0 = ((const T2*)(sm + C::O_TS + (k & (C::R_TS - 1)) * C::PL2))[py * BX + px];
+                        const T2 t1 = ((const T2*)(sm + C::O_TS + ((k + 1) & (C::R_TS - 1)) * C::PL2))[py * BX + px];
+                        ((T2*)(sm + C::O_NK + ((k + 1) & 1) * C::KDB))[q] =
+                            ri_face(P, k + 1, t1.x, t1.y, t0.x, t0.y, (X(b.x) - X(a.x)).v, (X(be.x) - X(ae.x)).v,
+                                    (X(b.y) - X(a.y)).v, (X(bn.y) - X(an.y)).v);
+                    }
                 }
             }
             // ================= phase 2: tracer face fluxes, each open face once =================
-            if constexpr (DO_T) {
+            {
                 const T2* __restrict__ s_ts = (const T2*)(sm + C::O_TS + (k & (C::R_TS - 1)) * C::PL2);
                 const int nface = s_nf[k];
                 for (int f = (tid + NT - K1_FOFF) % NT; f < nface; f += NT) {
@@ -417,7 +432,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                     const T len = isy ? s_dxF[row] : dy;                       // face length; the face area is len * dz
                     const T dd = isy ? dy : s_dxC[row], rdd = isy ? rdy : s_rdxC[row];   // centre-to-centre distance
                     const T2 cm = s_ts[b - st], cc = s_ts[b];
-                    const T2 fv = weno_face2(s_ts[b - 3 * st], s_ts[b - 2 * st], cm, cc, s_ts[b + st], s_ts[b + 2 * st], vel, ord);
+                    const T2 fv = weno_face2<WZ>(s_ts[b - 3 * st], s_ts[b - 2 * st], cm, cc, s_ts[b + st], s_ts[b + 2 * st], vel, ord);
                     const Xv<T> adv = X(vel) * X(len) * X(dzk), dif = X(P.kappa_h) * X(len) * X(dzk);
                     T2 flux;
                     flux.x = (adv * X(fv.x) - xdiv(dif * (X(cc.x) - X(cm.x)), dd, rdd)).v;
@@ -439,7 +454,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             const T2* __restrict__ s_flux = (const T2*)(sm + C::O_FLUX + (k & 1) * C::FLB);
             // ---------- tracer half: the cell of rank tid ----------
             T2 fz_top = mk2(T(0), T(0));
-            if constexpr (DO_T) if (wetT) {
+            if (wetT) {
                 const int cx = cT.cx, cy = cT.cy, kb = cT.t1, bo = cT.bo, by = cT.by;
                 const long long o = oT;
                 const T AzCj = s_AzC[by], rAzCj = s_rAzC[by];
@@ -451,7 +466,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                     auto tsz = [&](int dk) -> T2 {           // plane of level k + dk, dk = -2 .. 3
                         return ((const T2*)(sm + C::O_TS + ((k + dk) & (C::R_TS - 1)) * C::PL2))[bo];
                     };
-                    const T2 fv = weno_face2(tsz(-2), tsz(-1), tsz(0), tsz(1), tsz(2), tsz(3), w_c1, ozt);
+                    const T2 fv = weno_face2<WZ>(tsz(-2), tsz(-1), tsz(0), tsz(1), tsz(2), tsz(3), w_c1, ozt);
                     fz_top.x = (X(w_c1) * X(AzCj) * X(fv.x)).v;
                     fz_top.y = (X(w_c1) * X(AzCj) * X(fv.y)).v;
                 }
@@ -480,13 +495,23 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 // ---- quasi-AB2, predictor, elimination sweep (S3, S4) ----
                 const T Ght = (X(c0) * X(GT) - X(c1) * X(gm_ts.x)).v, Ghs = (X(c0) * X(GS) - X(c1) * X(gm_ts.y)).v;
                 P.Gts[o] = mk2(GT, GS);
+                if constexpr (RI) {               // per-face diffusivity: kappa of the own column at the face above
+                    const bool has_hi = k + 1 < nz;
+                    const T kt_hi = has_hi ? (X(P.dt) * X(((const T2*)(sm + C::O_NK + ((k + 1) & 1) * C::KDB))[(cy + 1) * RX + cx + 1].y)).v : T(0);
+                    rt.step(k == kb, kt_lo, kt_hi, has_hi, dzk, k > 0 ? P.dzc[k] : T(1), has_hi ? P.dzc[k + 1] : T(1), rdzk,
+                            k > 0 ? P.rdzc[k] : T(1), has_hi ? P.rdzc[k + 1] : T(1), E::add(tsc.x, E::mul(P.dt, Ght)), E::add(tsc.y, E::mul(P.dt, Ghs)));
+                    P.dts[o] = mk2(rt.d0, rt.d1);
+                    P.cpt[o] = rt.cp;
+                    kt_lo = kt_hi;
+                } else {
                 const T smk = k > kb ? P.sm_t[k] : T(0);
                 ddts.x = E::div(E::add(E::add(tsc.x, E::mul(P.dt, Ght)), E::mul(smk, ddts.x)), piv_t, piv_t);
                 ddts.y = E::div(E::add(E::add(tsc.y, E::mul(P.dt, Ghs)), E::mul(smk, ddts.y)), piv_t, piv_t);
                 P.dts[o] = ddts;
+                }
             }
             // ---------- momentum: the u face and the v face this thread owns ----------
-            if constexpr (DO_M) if (wetU) {
+            if (wetU) {
                 const int cx = cU.cx, cy = cU.cy, tx1 = cU.t1, bo = cU.bo, by = cU.by;
                 const int qo = (cy + 1) * RX + cx + 1;                       // this column in the ring arrays
                 const T w_c1 = s_w1[qo], w_c0 = s_w0[qo];
@@ -507,8 +532,8 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 const int ozu = 1 + (k >= cU.z2) + (k >= cU.z3);
                 const T z01 = s_zeta[bo + BX];
                 const T zt = ozu == 1 ? (vhat > T(0) ? z00 : z01)
-                                      : weno_face(s_zeta[bo - 2 * BX], s_zeta[bo - BX], z00, z01, s_zeta[bo + 2 * BX],
-                                                  s_zeta[bo + 3 * BX], vhat, ozu);
+                                      : weno_face<WZ>(s_zeta[bo - 2 * BX], s_zeta[bo - BX], z00, z01, s_zeta[bo + 2 * BX],
+                                                      s_zeta[bo + 3 * BX], vhat, ozu);
                 const Xv<T> Cu = xdiv(half * (X(fFj) * half * X(dxFj) * vsum_s + X(fFn) * half * X(dxFn) * vsum_n), dxCj, rdxCj);
                 const T2 kdw = s_kd[qo - 1];
                 const Xv<T> dK = xdiv(X(kdc.x) - X(kdw.x), dxCj, rdxCj);
@@ -530,12 +555,23 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 ((T*)(P.Guv + oU))[0] = Gu;
                 const T us = E::add(u_c, E::mul(P.dt, Ghu));
                 aGU = (X(aGU) + X((double)dzk) * X((double)Ghu)).v; aSU = (X(aSU) + X((double)dzk) * X((double)us)).v;
+                if constexpr (RI) {               // nu at the u face = mean of the two tracer columns that share it
+                    const bool has_hi = k + 1 < nz;
+                    const T2* __restrict__ s_nk1 = (const T2*)(sm + C::O_NK + ((k + 1) & 1) * C::KDB);
+                    const T ku_hi = has_hi ? (X(P.dt) * (X(T(0.5)) * (X(s_nk1[qo - 1].x) + X(s_nk1[qo].x)))).v : T(0);
+                    ru.step(k == tx1, ku_lo, ku_hi, has_hi, dzk, k > 0 ? P.dzc[k] : T(1), has_hi ? P.dzc[k + 1] : T(1), rdzk,
+                            k > 0 ? P.rdzc[k] : T(1), has_hi ? P.rdzc[k + 1] : T(1), us, T(0));
+                    ((T*)(P.duv + oU))[0] = ru.d0;
+                    ((T*)(P.cpuv + oU))[0] = ru.cp;
+                    ku_lo = ku_hi;
+                } else {
                 const T smk = k > tx1 ? P.sm_m[k] : T(0);
                 ddu = E::div(E::add(us, E::mul(smk, ddu)), piv_u, piv_u);
                 ((T*)(P.duv + oU))[0] = ddu;
+                }
                 u_dn = u_c;
             }
-            if constexpr (DO_M) if (wetV) {
+            if (wetV) {
                 const int cx = cV.cx, cy = cV.cy, ty1 = cV.t1, bo = cV.bo, by = cV.by;
                 const int qo = (cy + 1) * RX + cx + 1;
                 const T w_c1 = s_w1[qo], w_c0 = s_w0[qo];
@@ -554,7 +590,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 const int ozv = 1 + (k >= cV.z2) + (k >= cV.z3);
                 const T z10 = s_zeta[bo + 1];
                 const T zt = ozv == 1 ? (uhat > T(0) ? z00 : z10)
-                                      : weno_face(s_zeta[bo - 2], s_zeta[bo - 1], z00, z10, s_zeta[bo + 2], s_zeta[bo + 3], uhat, ozv);
+                                      : weno_face<WZ>(s_zeta[bo - 2], s_zeta[bo - 1], z00, z10, s_zeta[bo + 2], s_zeta[bo + 3], uhat, ozv);
                 const Xv<T> Cv = X(fFj) * X(uhat);
                 const T2 kds = s_kd[qo - RX];
                 const Xv<T> dK = xdiv(X(kdc.x) - X(kds.x), dy, rdy);
@@ -575,9 +611,20 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 ((T*)(P.Guv + oV))[1] = Gv;
                 const T vs2 = E::add(v_c, E::mul(P.dt, Ghv));
                 aGV = (X(aGV) + X((double)dzk) * X((double)Ghv)).v; aSV = (X(aSV) + X((double)dzk) * X((double)vs2)).v;
+                if constexpr (RI) {
+                    const bool has_hi = k + 1 < nz;
+                    const T2* __restrict__ s_nk1 = (const T2*)(sm + C::O_NK + ((k + 1) & 1) * C::KDB);
+                    const T kv_hi = has_hi ? (X(P.dt) * (X(T(0.5)) * (X(s_nk1[qo - RX].x) + X(s_nk1[qo].x)))).v : T(0);
+                    rv.step(k == ty1, kv_lo, kv_hi, has_hi, dzk, k > 0 ? P.dzc[k] : T(1), has_hi ? P.dzc[k + 1] : T(1), rdzk,
+                            k > 0 ? P.rdzc[k] : T(1), has_hi ? P.rdzc[k + 1] : T(1), vs2, T(0));
+                    ((T*)(P.duv + oV))[1] = rv.d0;
+                    ((T*)(P.cpuv + oV))[1] = rv.cp;
+                    kv_lo = kv_hi;
+                } else {
                 const T smk = k > ty1 ? P.sm_m[k] : T(0);
                 ddv = E::div(E::add(vs2, E::mul(smk, ddv)), piv_v, piv_v);
                 ((T*)(P.duv + oV))[1] = ddv;
+                }
                 v_dn = v_c;
             }
             fz_bot = fz_top;
@@ -585,7 +632,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
         __syncthreads();                       // planes of level m - 1 are dead: refill the ring
         if (tid == PROD && m + C::DP <= nz) issue_group(m + C::DP, false);
     }
-    if (DO_M && cU.incol && cU.t1 < nz) { P.GU[cU.c] = (T)aGU; P.SU[cU.c] = (T)aSU; }     // never-open faces keep their zeros
-    if (DO_M && cV.incol && cV.t1 < nz) { P.GV[cV.c] = (T)aGV; P.SV[cV.c] = (T)aSV; }
+    if (cU.incol && cU.t1 < nz) { P.GU[cU.c] = (T)aGU; P.SU[cU.c] = (T)aSU; }     // never-open faces keep their zeros
+    if (cV.incol && cV.t1 < nz) { P.GV[cV.c] = (T)aGV; P.SV[cV.c] = (T)aSV; }
 }
 }  // namespace ocn

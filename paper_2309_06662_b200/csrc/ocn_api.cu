@@ -61,12 +61,22 @@ struct ocn_model {
     unsigned long long bytes = 0;
     ocn::DevP<float> pf{};
     ocn::DevP<double> pd{};
-    void* stage = nullptr;              // contiguous staging buffer, (nz+1)*ny*nx doubles
+    // host <-> device staging: copies run on a stream of their own beside the steps; one big region for
+    // 3-D fields and a ring of small ones for 2-D fields (per-step forcing in, eta out), each guarded by two events
+    struct Stage {
+        void* buf = nullptr;
+        size_t bytes = 0;
+        cudaEvent_t filled = nullptr;   // H2D copy done (copy stream) / gather done (main stream)
+        cudaEvent_t freed = nullptr;    // last consumer done: scatter (main stream) / D2H copy (copy stream)
+    };
+    static constexpr int NSMALL = 8, NTICKET = 64;
+    Stage big, small_[NSMALL];
+    int next_small = 0;
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ticket_ev[NTICKET] = {};
+    unsigned long long tickets = 0;     // async read-backs issued so far (ticket t lives in ticket_ev[t % NTICKET])
     cudaGraphExec_t graph = nullptr;    // one steady-state (AB2) step
     CUtensorMap tm_ts{}, tm_uv{}, tm_p{};   // TMA descriptors of the halo'd (T,S), (u,v) and p arrays
-    bool split_k1 = false;              // K1 as two concurrent prognostic-group kernels (OCN_K1_SPLIT=1) or fused
-    cudaStream_t stream2 = nullptr;
-    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     int launches_per_step = 0;
     // per-stage timing (ocn_profile_*)
     bool profiling = false;
@@ -138,19 +148,26 @@ ocn_status make_tmap(CUtensorMap* tm, bool f64, void* base, unsigned long long i
     return OCN_OK;
 }
 
-// K1 variants: fused (all four fields), or the two prognostic-group kernels that run concurrently.  MINB = CTAs per SM
-// the register allocation is bounded for.
+// K1 instantiations.  MINB = CTAs per SM the register allocation is bounded for.  drag: carries the bottom-drag term
+// (drag_r or drag_cd non-zero); ri: evaluates the Ri-based closure in the pass (closure = 1); wz: WENO-Z weights (advection = 1).
 template <class T> using k1_fn = void (*)(const ocn::DevP<T>, const T, const T, const CUtensorMap, const CUtensorMap, const CUtensorMap);
-// drag: the instantiation that carries the bottom-drag term (drag_r or drag_cd non-zero)
-template <class T> k1_fn<T> k1_fused(bool drag = false) {
-    return drag ? ocn::k_tendency_tile<T, TILE_X, TILE_Y, 0, (sizeof(T) == 4 ? 2 : 1), true>
-                : ocn::k_tendency_tile<T, TILE_X, TILE_Y, 0, (sizeof(T) == 4 ? 2 : 1), false>;
+template <class T, bool DRAG, bool RI, bool WZ> k1_fn<T> k1_inst() {
+    return ocn::k_tendency_tile<T, TILE_X, TILE_Y, (sizeof(T) == 4 ? 2 : 1), DRAG, RI, WZ>;
 }
-template <class T> k1_fn<T> k1_momentum(bool drag = false) {
-    return drag ? ocn::k_tendency_tile<T, TILE_X, TILE_Y, 1, (sizeof(T) == 4 ? 3 : 1), true>
-                : ocn::k_tendency_tile<T, TILE_X, TILE_Y, 1, (sizeof(T) == 4 ? 3 : 1), false>;
+template <class T> k1_fn<T> k1_fused(bool drag, bool ri, bool wz) {
+    const int id = (drag ? 4 : 0) | (ri ? 2 : 0) | (wz ? 1 : 0);
+    switch (id) {
+        case 0: return k1_inst<T, false, false, false>();
+        case 1: return k1_inst<T, false, false, true>();
+        case 2: return k1_inst<T, false, true, false>();
+        case 3: return k1_inst<T, false, true, true>();
+        case 4: return k1_inst<T, true, false, false>();
+        case 5: return k1_inst<T, true, false, true>();
+        case 6: return k1_inst<T, true, true, false>();
+        default: return k1_inst<T, true, true, true>();
+    }
 }
-template <class T> k1_fn<T> k1_tracers() { return ocn::k_tendency_tile<T, TILE_X, TILE_Y, 2, (sizeof(T) == 4 ? 3 : 1)>; }
+template <class T> int k1_smem(bool ri) { return ri ? ocn::Tile<T, TILE_X, TILE_Y, true>::SMEM : ocn::Tile<T, TILE_X, TILE_Y, false>::SMEM; }
 
 dim3 grid2(const ocn_grid* g, dim3 b, int z = 1) { return dim3((g->nx + b.x - 1) / b.x, (g->ny + b.y - 1) / b.y, z); }
 
@@ -174,10 +191,9 @@ ocn_status build_model(ocn_model* M) {
     if ((s = dev_alloc(M, n3, &P.p, true)) != OCN_OK) return s;
     if ((s = plane(n3 + n2, &P.w)) != OCN_OK) return s;
     P.closure = M->d.closure; P.nk = nullptr; P.cpuv = nullptr; P.cpt = nullptr;
-    if (M->d.closure == 1) {                       // (nu, kappa) pairs and the per-column super-diagonals
-        if ((s = dev_alloc(M, n3, &P.nk, true)) != OCN_OK || (s = dev_alloc(M, n3, &P.cpuv, true)) != OCN_OK ||
-            (s = dev_alloc(M, n3, &P.cpt, true)) != OCN_OK) return s;
-    }
+    if (M->d.closure == 1) {                       // the per-column super-diagonals K1 leaves for K3
+        if ((s = dev_alloc(M, n3, &P.cpuv, true)) != OCN_OK || (s = dev_alloc(M, n3, &P.cpt, true)) != OCN_OK) return s;
+    }                                              // (nu, kappa) as an output array: allocated by the first ocn_get_mixing
     P.ri_nu0 = M->d.ri_nu0; P.ri_c = M->d.ri_c; P.ri_kconv = M->d.ri_kconv; P.ri_n2c = M->d.ri_n2c; P.ri_s2min = M->d.ri_s2min;
     P.nu_z_d = M->d.nu_z; P.kappa_z_d = M->d.kappa_z;
     T** f2[] = {&P.eta[0], &P.eta[1], &P.U[0], &P.U[1], &P.V[0], &P.V[1], &P.etab, &P.Ub, &P.Vb, &P.GU, &P.GV,
@@ -220,8 +236,8 @@ ocn_status build_model(ocn_model* M) {
     // level kf; sub-diagonal sm[k], and per (k, kf) the pivot m, its reciprocal and the modified
     // super-diagonal cp, computed in fp64 exactly as the equations of DESIGN.md §3.8 step 4 are written
     for (int pass = 0; pass < 2; ++pass) {
-        // closure 1: identity tables (K1 then leaves the predictor phi* in the d arrays; K5 eliminates per column)
-        const double dtk = M->d.closure == 1 ? 0.0 : M->d.dt * (pass == 0 ? M->d.nu_z : M->d.kappa_z);
+        // (closure 1 eliminates with per-face coefficients inside K1 and does not read these tables)
+        const double dtk = M->d.dt * (pass == 0 ? M->d.nu_z : M->d.kappa_z);
         std::vector<double> sm(nz, 0.0), cp((size_t)nz * nz, 0.0), mm((size_t)nz * nz, 1.0), rm((size_t)nz * nz, 1.0);
         for (int k = 1; k < nz; ++k) sm[k] = dtk / (g->dz[k] * g->dzc[k]);
         for (int kf = 0; kf < nz; ++kf) {
@@ -251,6 +267,16 @@ ocn_status build_model(ocn_model* M) {
     P.g_d = M->d.g; P.alpha_d = M->d.alpha; P.beta_d = M->d.beta_s; P.hz_top_d = g->zf[nz] - g->zc[nz - 1];
     P.dT0_d = M->d.T0 - (double)P.Toff; P.dS0_d = M->d.S0 - (double)P.Soff;
     P.nu_h = (T)M->d.nu_h; P.kappa_h = (T)M->d.kappa_h; P.dtau = (T)M->dtau;
+    // equation of state: per-level thermal expansion alpha (1 - gamma zc[k]) and alpha2 / 2, in the fp64
+    // operations the equation is written in
+    P.eos = M->d.eos; P.ha2_d = 0.5 * M->d.eos_alpha2;
+    {
+        std::vector<double> ath(nz);
+        for (int k = 0; k < nz; ++k) ath[k] = M->d.alpha * (1.0 - M->d.eos_gamma * g->zc[k]);
+        const double* a = nullptr;
+        if ((s = upload<double>(M, ath, &a)) != OCN_OK) return s;
+        P.ath_d = a;
+    }
     // Hu, Hv = sum_k dz over open faces, and reciprocals
     {
         std::vector<T> hu(n2 + 2 * LEAD, T(0)), hv(hu), rhu(hu), rhv(hu);
@@ -270,23 +296,31 @@ ocn_status build_model(ocn_model* M) {
         CK(cudaMemcpyAsync(P.rHv - LEAD, rhv.data(), nb, cudaMemcpyHostToDevice, M->stream));
         CK(cudaStreamSynchronize(M->stream));
     }
-    CK(cudaMalloc(&M->stage, (size_t)(nz + 1) * g->ny * g->nx * sizeof(double)));
-    M->bytes += (size_t)(nz + 1) * g->ny * g->nx * sizeof(double);
-    M->launches_per_step = (M->d.substeps + BT_HALO - 1) / BT_HALO + 3 + (M->d.closure == 1 ? 2 : 0);
+    {
+        auto mk = [&](ocn_model::Stage& st, size_t bytes) -> ocn_status {
+            CK(cudaMalloc(&st.buf, bytes));
+            st.bytes = bytes; M->bytes += bytes;
+            CK(cudaEventCreateWithFlags(&st.filled, cudaEventDisableTiming));
+            CK(cudaEventCreateWithFlags(&st.freed, cudaEventDisableTiming));
+            return OCN_OK;
+        };
+        if ((s = mk(M->big, (size_t)(nz + 1) * g->ny * g->nx * sizeof(double))) != OCN_OK) return s;
+        for (auto& st : M->small_) if ((s = mk(st, (size_t)g->ny * g->nx * sizeof(double))) != OCN_OK) return s;
+        CK(cudaStreamCreateWithFlags(&M->copy_stream, cudaStreamNonBlocking));
+        for (auto& e : M->ticket_ev) CK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    }
+    M->launches_per_step = (M->d.substeps + BT_HALO - 1) / BT_HALO + 3;
     // TMA descriptors: box origin (i0 - 4, j0 - 3), so the map starts 4 elements before (row -3, i = 0)
     {
-        typedef ocn::Tile<T, TILE_X, TILE_Y, 0> C;
+        typedef ocn::Tile<T, TILE_X, TILE_Y> C;
         const bool f64 = sizeof(T) == 8;
         const unsigned long long sxu = (unsigned long long)g->sx, syu = (unsigned long long)g->sy;
         if ((s = make_tmap(&M->tm_ts, f64, (T*)P.ts - 2 * C::OX, 2 * sxu, syu, nz, 2 * C::BX, C::BY)) != OCN_OK ||
             (s = make_tmap(&M->tm_uv, f64, (T*)P.uv - 2 * C::OX, 2 * sxu, syu, nz, 2 * C::BX, C::BY)) != OCN_OK ||
             (s = make_tmap(&M->tm_p, true, P.p - C::OX, sxu, syu, nz, C::PBX, TILE_Y + 1)) != OCN_OK)
             return s;
-        for (int dr = 0; dr < 2; ++dr) {
-            CK(cudaFuncSetAttribute(k1_fused<T>(dr != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
-            CK(cudaFuncSetAttribute(k1_momentum<T>(dr != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, (ocn::Tile<T, TILE_X, TILE_Y, 1>::SMEM)));
-        }
-        CK(cudaFuncSetAttribute(k1_tracers<T>(), cudaFuncAttributeMaxDynamicSharedMemorySize, (ocn::Tile<T, TILE_X, TILE_Y, 2>::SMEM)));
+        for (int id = 0; id < 8; ++id)
+            CK(cudaFuncSetAttribute(k1_fused<T>(id & 4, id & 2, id & 1), cudaFuncAttributeMaxDynamicSharedMemorySize, k1_smem<T>(id & 2)));
         CK(cudaFuncSetAttribute(ocn::k_barotropic_tile<T, BT_X, BT_Y>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 ocn::BtTile<T, BT_X, BT_Y>::SMEM));
     }
@@ -343,17 +377,8 @@ ocn_status launch_step(ocn_model* M, bool euler) {
     MARK(-1, 0);
     {
         const dim3 bt(TILE_X, TILE_Y), gt = grid2(g, bt);
-        const bool drag = M->d.drag_r != 0.0 || M->d.drag_cd != 0.0;
-        if (!M->split_k1) {
-            k1_fused<T>(drag)<<<gt, bt, ocn::Tile<T, TILE_X, TILE_Y, 0>::SMEM, M->stream>>>(P, c0, c1, M->tm_ts, M->tm_uv, M->tm_p);
-        } else {                                   // the two group kernels side by side (fork / join on a second stream)
-            CK(cudaEventRecord(M->ev_fork, M->stream));
-            CK(cudaStreamWaitEvent(M->stream2, M->ev_fork, 0));
-            k1_momentum<T>(drag)<<<gt, bt, ocn::Tile<T, TILE_X, TILE_Y, 1>::SMEM, M->stream2>>>(P, c0, c1, M->tm_ts, M->tm_uv, M->tm_p);
-            CK(cudaEventRecord(M->ev_join, M->stream2));
-            k1_tracers<T>()<<<gt, bt, ocn::Tile<T, TILE_X, TILE_Y, 2>::SMEM, M->stream>>>(P, c0, c1, M->tm_ts, M->tm_uv, M->tm_p);
-            CK(cudaStreamWaitEvent(M->stream, M->ev_join, 0));
-        }
+        const bool drag = M->d.drag_r != 0.0 || M->d.drag_cd != 0.0, ri = M->d.closure == 1, wz = M->d.advection == 1;
+        k1_fused<T>(drag, ri, wz)<<<gt, bt, k1_smem<T>(ri), M->stream>>>(P, c0, c1, M->tm_ts, M->tm_uv, M->tm_p);
     }
     MARK(0, 1);
     {
@@ -371,15 +396,9 @@ ocn_status launch_step(ocn_model* M, bool euler) {
     }
     ocn::k_barotropic_finish<T><<<grid2(g, b2), b2, 0, M->stream>>>(P);
     MARK(1, (M->d.substeps + BT_HALO - 1) / BT_HALO + 1);
-    if (M->d.closure == 1) {                       // K4 on state n (still intact), K5 on K1's predictor
-        ocn::k_ri_mixing<T><<<grid2(g, bc), bc, 0, M->stream>>>(P);
-        ocn::k_ri_eliminate<T><<<grid2(g, bc), bc, 0, M->stream>>>(P);
-        MARK(3, 2);
-        ocn::k_backsub_correct<T, true><<<grid2(g, bc), bc, 0, M->stream>>>(P);
-    } else {
-        MARK(3, 0);
-        ocn::k_backsub_correct<T, false><<<grid2(g, bc), bc, 0, M->stream>>>(P);
-    }
+    MARK(3, 0);                                    // (the closure is evaluated inside K1: stage 3 is empty)
+    if (M->d.closure == 1) ocn::k_backsub_correct<T, true><<<grid2(g, bc), bc, 0, M->stream>>>(P);
+    else ocn::k_backsub_correct<T, false><<<grid2(g, bc), bc, 0, M->stream>>>(P);
     MARK(2, 1);
 #undef MARK
     CK(cudaGetLastError());
@@ -412,19 +431,37 @@ ocn_status run_steps(ocn_model* M, int n) {
     return OCN_OK;
 }
 
+// a staging region for `bytes`: 2-D fields take the next small region of the ring, 3-D fields the big one
+ocn_model::Stage& stage_for(ocn_model* M, size_t bytes) {
+    if (bytes > M->small_[0].bytes) return M->big;
+    ocn_model::Stage& st = M->small_[M->next_small];
+    M->next_small = (M->next_small + 1) % ocn_model::NSMALL;
+    return st;
+}
+
+// host -> device: the copy runs on the copy stream (beside whatever the main stream is doing), the masked scatter into the
+// halo'd layout on the main stream after it; the host waits for the DMA only, so its buffer is reusable on return
 template <class T>
 ocn_status set_one(ocn_model* M, const void* src, T* dst, int nl, int kind, bool on_device, int st = 1) {
     const ocn_grid* g = M->g;
     const size_t n = (size_t)nl * g->ny * g->nx;
     const T* dsrc = static_cast<const T*>(src);
+    ocn_model::Stage* sg = nullptr;
     if (!on_device) {
-        CK(cudaMemcpyAsync(M->stage, src, n * sizeof(T), cudaMemcpyHostToDevice, M->stream));
-        dsrc = static_cast<const T*>(M->stage);
+        sg = &stage_for(M, n * sizeof(T));
+        CK(cudaStreamWaitEvent(M->copy_stream, sg->freed, 0));          // its last consumer (an event never recorded is complete)
+        CK(cudaMemcpyAsync(sg->buf, src, n * sizeof(T), cudaMemcpyHostToDevice, M->copy_stream));
+        CK(cudaEventRecord(sg->filled, M->copy_stream));
+        CK(cudaStreamWaitEvent(M->stream, sg->filled, 0));
+        dsrc = static_cast<const T*>(sg->buf);
     }
     const dim3 b(32, 8);
     ocn::k_scatter<T><<<grid2(g, b, nl < 64 ? nl : 64), b, 0, M->stream>>>(params<T>(M), dst, dsrc, nl, kind, st);
     CK(cudaGetLastError());
-    if (!on_device) CK(cudaStreamSynchronize(M->stream));   // staging buffer is reused by the next field
+    if (sg) {
+        CK(cudaEventRecord(sg->freed, M->stream));
+        CK(cudaEventSynchronize(sg->filled));
+    }
     return OCN_OK;
 }
 
@@ -455,41 +492,63 @@ ocn_status set_fields_t(ocn_model* M, const ocn_fields* f) {
     return OCN_OK;
 }
 
+// device -> host: gather into a staging region on the main stream, copy out on the copy stream; `last` receives the event
+// that marks the completion of the copy (the caller waits for it, or hands it out as a ticket)
 template <class T, class O>
-ocn_status get_one(ocn_model* M, void* dst, const T* src, int nl, int kind, bool on_device, int st = 1) {
+ocn_status get_one(ocn_model* M, void* dst, const T* src, int nl, int kind, bool on_device, int st = 1, cudaEvent_t* last = nullptr) {
     const ocn_grid* g = M->g;
     const size_t n = (size_t)nl * g->ny * g->nx;
-    O* ddst = on_device ? static_cast<O*>(dst) : static_cast<O*>(M->stage);
+    ocn_model::Stage* sg = nullptr;
+    O* ddst = static_cast<O*>(dst);
+    if (!on_device) {
+        sg = &stage_for(M, n * sizeof(O));
+        CK(cudaStreamWaitEvent(M->stream, sg->freed, 0));
+        ddst = static_cast<O*>(sg->buf);
+    }
     const dim3 b(32, 8);
     ocn::k_gather<T, O><<<grid2(g, b, nl < 64 ? nl : 64), b, 0, M->stream>>>(params<T>(M), ddst, src, nl, kind, st);
     CK(cudaGetLastError());
-    if (!on_device) {
-        CK(cudaMemcpyAsync(dst, M->stage, n * sizeof(O), cudaMemcpyDeviceToHost, M->stream));
-        CK(cudaStreamSynchronize(M->stream));
+    if (sg) {
+        CK(cudaEventRecord(sg->filled, M->stream));
+        CK(cudaStreamWaitEvent(M->copy_stream, sg->filled, 0));
+        CK(cudaMemcpyAsync(dst, sg->buf, n * sizeof(O), cudaMemcpyDeviceToHost, M->copy_stream));
+        CK(cudaEventRecord(sg->freed, M->copy_stream));
+        if (last) *last = sg->freed;
+        else CK(cudaEventSynchronize(sg->freed));
     }
     return OCN_OK;
 }
 
+// ticket: NULL = blocking (returns when every copy has landed); else the copies are left in flight and *ticket names them
 template <class T>
-ocn_status get_fields_t(ocn_model* M, ocn_fields* f) {
+ocn_status get_fields_t(ocn_model* M, ocn_fields* f, unsigned long long* ticket) {
     ocn::DevP<T>& P = params<T>(M);
     const int nz = M->g->nz;
     const bool dev = f->on_device != 0;
     ocn_status s;
-    if (f->u && (s = get_one<T, T>(M, f->u, (T*)P.uv, nz, 0, dev, 2)) != OCN_OK) return s;
-    if (f->v && (s = get_one<T, T>(M, f->v, (T*)P.uv + 1, nz, 1, dev, 2)) != OCN_OK) return s;
-    if (f->T && (s = get_one<T, T>(M, f->T, (T*)P.ts, nz, 2, dev, 2)) != OCN_OK) return s;
-    if (f->S && (s = get_one<T, T>(M, f->S, (T*)P.ts + 1, nz, 3, dev, 2)) != OCN_OK) return s;
+    cudaEvent_t last = nullptr;
+    if (f->u && (s = get_one<T, T>(M, f->u, (T*)P.uv, nz, 0, dev, 2, &last)) != OCN_OK) return s;
+    if (f->v && (s = get_one<T, T>(M, f->v, (T*)P.uv + 1, nz, 1, dev, 2, &last)) != OCN_OK) return s;
+    if (f->T && (s = get_one<T, T>(M, f->T, (T*)P.ts, nz, 2, dev, 2, &last)) != OCN_OK) return s;
+    if (f->S && (s = get_one<T, T>(M, f->S, (T*)P.ts + 1, nz, 3, dev, 2, &last)) != OCN_OK) return s;
     if (f->w) {                                   // w is diagnosed on demand (K1 recomputes it on the fly)
         const dim3 bc(32, 4);
         ocn::k_vertical_velocity<T><<<grid2(M->g, bc), bc, 0, M->stream>>>(P);
         CK(cudaGetLastError());
     }
-    if (f->w && (s = get_one<T, T>(M, f->w, P.w, nz + 1, 6, dev)) != OCN_OK) return s;
-    if (f->eta && (s = get_one<T, T>(M, f->eta, P.eta[0], 1, 4, dev)) != OCN_OK) return s;
-    if (f->tau_x && (s = get_one<T, T>(M, f->tau_x, P.taux, 1, 5, dev)) != OCN_OK) return s;
-    if (f->tau_y && (s = get_one<T, T>(M, f->tau_y, P.tauy, 1, 5, dev)) != OCN_OK) return s;
-    CK(cudaStreamSynchronize(M->stream));
+    if (f->w && (s = get_one<T, T>(M, f->w, P.w, nz + 1, 6, dev, 1, &last)) != OCN_OK) return s;
+    if (f->eta && (s = get_one<T, T>(M, f->eta, P.eta[0], 1, 4, dev, 1, &last)) != OCN_OK) return s;
+    if (f->tau_x && (s = get_one<T, T>(M, f->tau_x, P.taux, 1, 5, dev, 1, &last)) != OCN_OK) return s;
+    if (f->tau_y && (s = get_one<T, T>(M, f->tau_y, P.tauy, 1, 5, dev, 1, &last)) != OCN_OK) return s;
+    if (ticket) {                                 // the copy stream is in order: its position after the last copy covers them all
+        cudaEvent_t e = M->ticket_ev[M->tickets % ocn_model::NTICKET];
+        if (dev) CK(cudaEventRecord(e, M->stream)); else CK(cudaEventRecord(e, M->copy_stream));
+        *ticket = M->tickets++;
+        return OCN_OK;
+    }
+    if (dev || !last) CK(cudaStreamSynchronize(M->stream));
+    else CK(cudaEventSynchronize(last));          // implies everything the main stream did before the last gather
+    CK(cudaGetLastError());
     return OCN_OK;
 }
 
@@ -512,6 +571,10 @@ ocn_status get_mixing_t(ocn_model* M, double* nu, double* kappa) {
     ocn::DevP<T>& P = params<T>(M);
     const int nz = M->g->nz;
     const dim3 bc(32, 4);
+    if (!P.nk) {                                   // the output array of the diagnostic (the step itself keeps (nu, kappa) on chip)
+        const ocn_status sa = dev_alloc(M, (size_t)P.sz * nz, &P.nk, true);
+        if (sa != OCN_OK) return sa;
+    }
     ocn::k_ri_mixing<T><<<grid2(M->g, bc), bc, 0, M->stream>>>(P);
     CK(cudaGetLastError());
     ocn_status s;
@@ -537,8 +600,7 @@ ocn_status ocn_grid_create(const ocn_grid_desc* d, const double* z_faces, const 
     if (d->kind != 0 && d->kind != 1) return fail(OCN_EINVAL, "kind must be 0 (cartesian) or 1 (lat-lon)");
     if (d->kind == 1 && d->periodic_y) return fail(OCN_EINVAL, "a lat-lon grid cannot be periodic in latitude");
     if (!(d->dx > 0) || !(d->dy > 0)) return fail(OCN_EINVAL, "dx, dy must be positive");
-    if (z_faces[d->nz] != 0.0) return fail(OCN_EINVAL, "z_faces[nz] must be 0 (the resting surface)");
-    for (int k = 0; k <= d->nz; ++k) if (!std::isfinite(z_faces[k])) return fail(OCN_EINVAL, "z_faces must be finite");
+
     ocn_grid* g = new (std::nothrow) ocn_grid();
     if (!g) return fail(OCN_ENOMEM, "host allocation failed");
     try {
@@ -588,6 +650,9 @@ ocn_status ocn_model_create(const ocn_grid* g, const ocn_model_desc* d, ocn_mode
     if (!(d->gamma_T >= 0) || !(d->gamma_S >= 0)) return fail(OCN_EINVAL, "gamma_T, gamma_S must be >= 0");
     if (!(d->drag_r >= 0) || !(d->drag_cd >= 0)) return fail(OCN_EINVAL, "drag_r, drag_cd must be >= 0");
     if (d->closure != 0 && d->closure != 1) return fail(OCN_EINVAL, "closure must be 0 (constant) or 1 (Ri-based)");
+    if (d->eos != 0 && d->eos != 1) return fail(OCN_EINVAL, "eos must be 0 (linear) or 1 (nonlinear)");
+    if (d->eos == 1 && !(std::isfinite(d->eos_alpha2) && std::isfinite(d->eos_gamma))) return fail(OCN_EINVAL, "eos_alpha2, eos_gamma must be finite");
+    if (d->advection != 0 && d->advection != 1) return fail(OCN_EINVAL, "advection must be 0 (WENO-JS) or 1 (WENO-Z)");
     if (d->closure == 1 && !(d->ri_n2c > 0 && d->ri_s2min > 0 && d->ri_c >= 0 && d->ri_nu0 >= 0 && d->ri_kconv >= 0))
         return fail(OCN_EINVAL, "Ri closure: ri_n2c, ri_s2min must be > 0 and ri_c, ri_nu0, ri_kconv >= 0");
     int ndev = 0;
@@ -624,16 +689,6 @@ ocn_status ocn_model_create(const ocn_grid* g, const ocn_model_desc* d, ocn_mode
         if (e != cudaSuccess) { delete M; return fail(OCN_ECUDA, cudaGetErrorString(e)); }
         M->own_stream = true;
     }
-    {
-        const char* e = getenv("OCN_K1_SPLIT");
-        M->split_k1 = e && e[0] == '1';
-        if (cudaStreamCreateWithFlags(&M->stream2, cudaStreamNonBlocking) != cudaSuccess ||
-            cudaEventCreateWithFlags(&M->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
-            cudaEventCreateWithFlags(&M->ev_join, cudaEventDisableTiming) != cudaSuccess) {
-            ocn_model_destroy(M);
-            return fail(OCN_ECUDA, "stream / event creation failed");
-        }
-    }
     const ocn_status s = d->precision == 32 ? build_model<float>(M) : build_model<double>(M);
     if (s != OCN_OK) { const std::string keep = g_err; ocn_model_destroy(M); g_err = keep; return s; }
     *out = M;
@@ -646,11 +701,15 @@ ocn_status ocn_model_destroy(ocn_model* M) {
     if (M->stream) cudaStreamSynchronize(M->stream);
     if (M->graph) cudaGraphExecDestroy(M->graph);
     for (cudaEvent_t e : M->ev_pool) cudaEventDestroy(e);
-    if (M->ev_fork) cudaEventDestroy(M->ev_fork);
-    if (M->ev_join) cudaEventDestroy(M->ev_join);
-    if (M->stream2) cudaStreamDestroy(M->stream2);
     for (void* p : M->allocs) cudaFree(p);
-    if (M->stage) cudaFree(M->stage);
+    if (M->copy_stream) { cudaStreamSynchronize(M->copy_stream); cudaStreamDestroy(M->copy_stream); }
+    for (ocn_model::Stage* st : {&M->big, &M->small_[0], &M->small_[1], &M->small_[2], &M->small_[3], &M->small_[4], &M->small_[5],
+                                 &M->small_[6], &M->small_[7]}) {
+        if (st->buf) cudaFree(st->buf);
+        if (st->filled) cudaEventDestroy(st->filled);
+        if (st->freed) cudaEventDestroy(st->freed);
+    }
+    for (cudaEvent_t e : M->ticket_ev) if (e) cudaEventDestroy(e);
     if (M->own_stream && M->stream) cudaStreamDestroy(M->stream);
     delete M;
     return OCN_OK;
@@ -672,12 +731,32 @@ ocn_status ocn_time_step(ocn_model* M, int n) {
 ocn_status ocn_get_fields(ocn_model* M, ocn_fields* f) {
     if (!M || !f) return fail(OCN_EINVAL, "null argument");
     ON_DEVICE(M->d.device);
-    return M->prec == 32 ? get_fields_t<float>(M, f) : get_fields_t<double>(M, f);
+    return M->prec == 32 ? get_fields_t<float>(M, f, nullptr) : get_fields_t<double>(M, f, nullptr);
+}
+
+ocn_status ocn_get_fields_async(ocn_model* M, ocn_fields* f, unsigned long long* ticket) {
+    if (!M || !f || !ticket) return fail(OCN_EINVAL, "null argument");
+    ON_DEVICE(M->d.device);
+    return M->prec == 32 ? get_fields_t<float>(M, f, ticket) : get_fields_t<double>(M, f, ticket);
+}
+
+ocn_status ocn_wait(ocn_model* M, unsigned long long ticket) {
+    if (!M) return fail(OCN_EINVAL, "null model");
+    if (ticket >= M->tickets) return fail(OCN_EINVAL, "ticket was never issued");
+    ON_DEVICE(M->d.device);
+    // a ticket whose event slot has been reused is older than NTICKET later read-backs on the same in-order stream: wait for
+    // the oldest event still held, which was recorded after it
+    const unsigned long long held = M->tickets > ocn_model::NTICKET ? M->tickets - ocn_model::NTICKET : 0;
+    CK(cudaEventSynchronize(M->ticket_ev[(ticket < held ? held : ticket) % ocn_model::NTICKET]));
+    CK(cudaGetLastError());
+    return OCN_OK;
 }
 
 ocn_status ocn_synchronize(ocn_model* M) {
     if (!M) return fail(OCN_EINVAL, "null model");
+    ON_DEVICE(M->d.device);
     CK(cudaStreamSynchronize(M->stream));
+    CK(cudaStreamSynchronize(M->copy_stream));
     return OCN_OK;
 }
 

@@ -34,7 +34,8 @@ class ocn_model_desc(C.Structure):
                 ("device", C.c_int), ("stream", C.c_void_p),
                 ("closure", C.c_int), ("ri_nu0", C.c_double), ("ri_c", C.c_double), ("ri_kconv", C.c_double),
                 ("ri_n2c", C.c_double), ("ri_s2min", C.c_double), ("gamma_T", C.c_double), ("gamma_S", C.c_double),
-                ("drag_r", C.c_double), ("drag_cd", C.c_double)]
+                ("drag_r", C.c_double), ("drag_cd", C.c_double),
+                ("eos", C.c_int), ("eos_alpha2", C.c_double), ("eos_gamma", C.c_double), ("advection", C.c_int)]
 
 
 class ocn_fields(C.Structure):
@@ -45,7 +46,7 @@ class ocn_fields(C.Structure):
 EXPORTS = ["ocn_grid_create", "ocn_grid_destroy", "ocn_model_create", "ocn_model_destroy", "ocn_set_fields",
            "ocn_time_step", "ocn_get_fields", "ocn_synchronize", "ocn_get_masks", "ocn_model_info",
            "ocn_get_debug", "ocn_last_error", "ocn_version", "ocn_profile_enable", "ocn_profile_read",
-           "ocn_stage_name", "ocn_get_mixing"]
+           "ocn_stage_name", "ocn_get_mixing", "ocn_get_fields_async", "ocn_wait"]
 NSTAGES = 4
 
 
@@ -67,6 +68,8 @@ def lib():
         L.ocn_time_step.argtypes = [vp, C.c_int]
         L.ocn_get_fields.argtypes = [vp, C.POINTER(ocn_fields)]
         L.ocn_synchronize.argtypes = [vp]
+        L.ocn_get_fields_async.argtypes = [vp, C.POINTER(ocn_fields), C.POINTER(C.c_ulonglong)]
+        L.ocn_wait.argtypes = [vp, C.c_ulonglong]
         L.ocn_get_masks.argtypes = [vp] + [vp] * 6
         L.ocn_model_info.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_ulonglong)]
         L.ocn_get_debug.argtypes = [vp] + [vp] * 6
@@ -157,6 +160,16 @@ class Model:
     def get_fields_ptr(self, on_device=False, **ptrs):
         f = ocn_fields(on_device=int(on_device), **{k: int(v) for k, v in ptrs.items()})
         _check(lib().ocn_get_fields(self.h, C.byref(f)))
+
+    def get_fields_async_ptr(self, on_device=False, **ptrs):
+        """ocn_get_fields_async: returns a ticket; the buffers are valid after wait(ticket)."""
+        f = ocn_fields(on_device=int(on_device), **{k: int(v) for k, v in ptrs.items()})
+        t = C.c_ulonglong()
+        _check(lib().ocn_get_fields_async(self.h, C.byref(f), C.byref(t)))
+        return t.value
+
+    def wait(self, ticket):
+        _check(lib().ocn_wait(self.h, int(ticket)))
 
     def time_step(self, n=1):
         _check(lib().ocn_time_step(self.h, int(n)))

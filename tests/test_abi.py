@@ -37,6 +37,11 @@ def test_bad_arguments_return_status_not_crash():
         ocn.Grid(g, np.linspace(-300, 0, 301), np.ones((8, 8)))
     with pytest.raises(RuntimeError, match="increasing"):
         ocn.Grid(wl["grid"], wl["z_faces"][::-1].copy(), wl["depth"])
+    with pytest.raises(RuntimeError, match="resting surface"):
+        ocn.Grid(wl["grid"], wl["z_faces"] - 1.0, wl["depth"])
+    zf = wl["z_faces"].copy(); zf[1] = np.nan
+    with pytest.raises(RuntimeError, match="finite"):
+        ocn.Grid(wl["grid"], zf, wl["depth"])
     g = dict(wl["grid"], kind=1, periodic_y=1)
     with pytest.raises(RuntimeError, match="periodic in latitude"):
         ocn.Grid(g, wl["z_faces"], wl["depth"])

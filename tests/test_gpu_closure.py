@@ -106,15 +106,21 @@ def test_closure_with_zero_amplitudes_equals_constant_coefficient_path_on_gpu():
         assert np.array_equal(fa[n], fb[n]), n
 
 
-def test_closure_stage_is_timed():
+def test_closure_runs_inside_the_tendency_kernel():
+    """The closure is evaluated inside K1: no extra launches, and the step allocates no (nu, kappa) array."""
     wl = W.with_ri_closure(W.config3(nx=96, ny=40, nz=12, steps=3))
     gpu = ocn.Model(wl)
+    plain = ocn.Model(W.config3(nx=96, ny=40, nz=12, steps=3))
     gpu.time_step(1)
     gpu.profile_enable(True)
     gpu.time_step(3)
     prof = gpu.profile_read()
-    assert prof["vertical_mixing"]["launches"] == 6 and prof["vertical_mixing"]["ms"] > 0
-    assert gpu.info()["launches_per_step"] == prof["tendency"]["launches"] // 3 + prof["barotropic"]["launches"] // 3 + 3
+    assert prof["vertical_mixing"]["launches"] == 0
+    assert gpu.info()["launches_per_step"] == prof["tendency"]["launches"] // 3 + prof["barotropic"]["launches"] // 3 + 1
+    assert gpu.info()["launches_per_step"] == plain.info()["launches_per_step"]
+    n3 = gpu.info()["device_bytes"] - plain.info()["device_bytes"]
+    cells_padded = (40 + 6) * 128 * 12                      # plane layout: sy x sx x nz
+    assert 3 * 4 * cells_padded <= n3 < 3.2 * 4 * cells_padded      # three more words per cell: cp of (u, v) and of (T, S)
 
 
 def test_closure_fp64_is_bit_identical_to_the_oracle():

@@ -280,7 +280,7 @@ def test_periodic_seam_when_nx_plus_6_is_a_multiple_of_32(nx, closure):
     """nx + 6 = 32 n: the east halo column i = nx + 2 is the last element a TMA box of the last tile can reach; with a row
     pitch of exactly nx + 6 it fell outside the tensor map and was zero-filled (round-1 advisor finding).  fp64, periodic in
     x, flow and tracer gradients across the seam: bit-identical to the oracle."""
-    wl = W.config2(nx=nx, ny=20, nz=8, steps=4)
+    wl = W.config2(nx=nx, ny=40, nz=8, steps=4)
     rng = np.random.default_rng(nx)
     wl["depth"][:, -4:] = 3000.0                        # open ocean on both sides of the seam
     wl["depth"][:, :4] = 3000.0

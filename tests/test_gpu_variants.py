@@ -1,0 +1,95 @@
+"""GPU parity of the scheme variants: WENO-Z weights and the nonlinear equation of
+state, alone, together, and with the Ri closure; fp64 bit-identical to the oracle, fp32 within 2e-4."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2309_06662_b200 import build as ocn_build
+from paper_2309_06662_b200 import ocn
+from paper_2309_06662_b200 import workloads as W
+from util import rel_linf, report_parity
+
+pytestmark = pytest.mark.gpu
+FIELDS = ("u", "v", "w", "eta", "T", "S")
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    ocn_build.build()
+
+
+def _stirred(wl, seed=21):
+    rng = np.random.default_rng(seed)
+    f, prec = wl["fields"], wl["params"]["precision"]
+    f["u"] = W._round_to(prec, 0.3 * rng.standard_normal(f["u"].shape))
+    f["v"] = W._round_to(prec, 0.3 * rng.standard_normal(f["v"].shape))
+    f["T"] = W._round_to(prec, f["T"] + 0.5 * rng.standard_normal(f["T"].shape))       # non-smooth: the weights matter
+    return wl
+
+
+def _variant(kind, prec, closure):
+    wl = _stirred(W.config2(nx=180, ny=75, nz=25, steps=8, precision=prec))
+    if "z" in kind:
+        W.with_weno_z(wl)
+    if "e" in kind:
+        W.with_nonlinear_eos(wl)
+    if closure:
+        W.with_ri_closure(wl)
+    return wl
+
+
+@pytest.mark.parametrize("kind", ["z", "e", "ze"])
+@pytest.mark.parametrize("closure", [0, 1])
+def test_variants_fp64_bit_identical(kind, closure):
+    wl = _variant(kind, 64, closure)
+    ref, gpu = oracle.RefModel(wl), ocn.Model(wl)
+    ref.step(8); gpu.time_step(8)
+    a, b = gpu.get_fields(), ref.get_fields()
+    for n in FIELDS:
+        assert np.array_equal(a[n], b[n]), (kind, closure, n, rel_linf(a[n], b[n]))
+    gpu.close()
+
+
+@pytest.mark.parametrize("kind", ["z", "e", "ze"])
+@pytest.mark.parametrize("closure", [0, 1])
+def test_variants_fp32_within_tolerance(kind, closure):
+    wl = _variant(kind, 32, closure)
+    ref, gpu = oracle.RefModel(wl), ocn.Model(wl)
+    ref.step(8); gpu.time_step(8)
+    a, b = gpu.get_fields(), ref.get_fields()
+    errs = {n: rel_linf(a[n], b[n]) for n in FIELDS}
+    report_parity("variants %s%s 180x75x25 fp32" % (kind, "+ri" if closure else ""), 8, errs)
+    assert all(e <= 2e-4 for e in errs.values()), errs
+    gpu.close()
+
+
+def test_variants_change_the_answer_and_defaults_do_not():
+    base = _variant("", 64, 0)
+    g0 = ocn.Model(base); g0.time_step(4); f0 = g0.get_fields(); g0.close()
+    for kind in ("z", "e"):
+        g = ocn.Model(_variant(kind, 64, 0)); g.time_step(4); f = g.get_fields(); g.close()
+        assert np.abs(f["T"] - f0["T"]).max() > 1e-7 or np.abs(f["u"] - f0["u"]).max() > 1e-7, kind
+    # nonlinear EOS with zero coefficients = linear EOS, bit for bit, on the GPU too
+    wl = W.with_nonlinear_eos(_variant("", 64, 0), alpha2=0.0, gamma=0.0)
+    g = ocn.Model(wl); g.time_step(4); f = g.get_fields(); g.close()
+    for n in FIELDS:
+        assert np.array_equal(f[n], f0[n]), n
+
+
+def test_wenoz_first_step_tendencies_match_on_aquaplanet_shape():
+    wl = W.with_weno_z(_stirred(W.aquaplanet(nx=96, ny=40, nz=12, steps=1, precision=64)))
+    ref, gpu = oracle.RefModel(wl), ocn.Model(wl)
+    G = ref.tendencies()
+    gpu.time_step(1)
+    d = gpu.debug()
+    for n in ("Gu", "Gv", "GT", "GS"):
+        assert np.array_equal(d[n], G[n]), (n, rel_linf(d[n], G[n]))
+    gpu.close()
+
+
+def test_bad_variant_switches_are_rejected():
+    wl = W.config0()
+    for key, val in (("eos", 2), ("advection", 3)):
+        bad = dict(wl, params=dict(wl["params"], **{key: val}))
+        with pytest.raises(RuntimeError, match=key):
+            ocn.Model(bad)
