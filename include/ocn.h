@@ -176,6 +176,11 @@ ocn_status ocn_profile_enable(ocn_model* model, int on);
 ocn_status ocn_profile_read(ocn_model* model, double* ms, long long* launches, int reset);
 const char* ocn_stage_name(int stage);
 
+/* Performance knobs that do not change results (bit for bit).  "k1_geo_threshold": number of wet cells of a 32 x 8 tile-level
+ * from which on the tendency kernel marches the tile with geometric (thread = cell) instead of compacted ownership
+ * (default K1_GEO_THR of kernels_tile.cuh; 0 = always geometric, > 256 = never).  OCN_EINVAL for an unknown key. */
+ocn_status ocn_tune(ocn_model* model, const char* key, double value);
+
 /* Debug / parity hooks (HOST double buffers, NULL = skip): the AB2 history G^{n-1} of each
  * prognostic field (nz*ny*nx each) and the barotropic transports U, V (ny*nx). */
 ocn_status ocn_get_debug(ocn_model* model, double* Gu, double* Gv, double* GT, double* GS,

@@ -80,6 +80,8 @@ struct DevP {
     int eos;
     const double* ath_d;
     double ha2_d;
+    // K1: wet cells of a tile-level from which on the tile is marched with geometric ownership
+    int geo_thr;
 };
 
 template <class T>

@@ -18,12 +18,18 @@
 #pragma once
 #include <cuda.h>
 
+#include <type_traits>
+
 #include "common.cuh"
 #include "kernels_mixing.cuh"
 
 // First thread of the compacted work lists of a 256-thread CTA: v cells from 0 up, tracer cells from 64
 // up, faces from 160 up (wrapping), u cells from N-1 down.  On sparse levels the four lists land on different warps; on
 // half-full levels no thread carries all four.  Measured on config 4 (profiles/r1_ncu_summary.md §6).
+// Wet cells of a tile-level from which on the tile is marched with GEOMETRIC ownership (thread = cell).
+#ifndef K1_GEO_THR
+#define K1_GEO_THR 224
+#endif
 #ifndef K1_TOFF
 #define K1_TOFF 64
 #define K1_VOFF 0
@@ -94,7 +100,8 @@ struct Tile {
     static constexpr int O_NC = O_FS + rup128(NF * 8);                          // uint16[256]: active cells at level k
     static constexpr int O_NF = O_NC + 512;                                     // uint16[256]: active faces at level k
     static constexpr int O_DZ = O_NF + 512;                                     // T[256] dz, T[256] 1 / dz
-    static constexpr int O_BAR = O_DZ + 2 * 256 * (int)sizeof(T);
+    static constexpr int O_XP = O_DZ + 2 * 256 * (int)sizeof(T);                 // double[256][4]: column state in transit at the switch of ownership
+    static constexpr int O_BAR = O_XP + 256 * 4 * 8;
     static constexpr int SMEM = O_BAR + 128 + 128;                              // + alignment slack
 };
 
@@ -130,6 +137,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     T* const s_rdz = s_dz + 256;
     uint64_t* const bars = (uint64_t*)(sm + C::O_BAR);
     int& s_kmin = *(int*)(sm + C::O_BAR + 64);
+    int& s_ks = *(int*)(sm + C::O_BAR + 68);
 
     const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * TX + tx;
     // rasterisation: tiles are taken in bands of RB tile-rows, y fastest inside a band, so that the
@@ -143,7 +151,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     const long long sz = P.sz;
 
     // ---- masks of the tile (+ east / north edge) and the first level with any open cell -----
-    if (tid == 0) s_kmin = nz;
+    if (tid == 0) { s_kmin = nz; s_ks = nz; }
     __syncthreads();
     {
         const uint32_t nzb = (uint32_t)nz;
@@ -235,6 +243,8 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
         };
         auto cell_emit = [&](int q, int rank) { s_cell[rank] = (unsigned short)q; };
         csort(NC, [&](int q) { return cell_key(q, 0); }, cell_emit, s_nc);
+        // first level at which the tile is dense enough for geometric ownership (the fill never decreases with k)
+        for (int k = tid; k < nz; k += NT) if (s_nc[k] >= P.geo_thr) atomicMin(&s_ks, k);
         constexpr int TOFF = K1_TOFF, VOFF = K1_VOFF;                     // first thread of the tracer and v lists (u runs from N-1 down, faces from K1_FOFF up)
         gT = s_cell[(tid + NC - TOFF) % NC];
         {
@@ -310,17 +320,22 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     }
 
     // ---- per-thread column state ------------------------------------------------------------
-    // A thread owns the TRACERS of the cell of rank t - K1_TOFF (mod N) in the order by first wet level, the U of the
-    // cell of rank N-1-t in the order by first open west face and the V of the cell of rank t - K1_VOFF (mod N) in the
-    // order by first open south face: every block of part B runs on a dense run of threads, and on sparse levels the
-    // runs land on different warps instead of one after the other.
-    struct Cell { int cx, cy, t1, bo, by; long long c; bool incol; unsigned char z2, z3; };
+    // COMPACT ownership (sparse levels of the tile): a thread owns the TRACERS of the cell of rank
+    // t - K1_TOFF (mod N) in the order by first wet level, the U of the cell of rank N-1-t in the order by first open west
+    // face and the V of the cell of rank t - K1_VOFF (mod N) in the order by first open south face: every block of part B
+    // runs on a dense run of threads, and on sparse levels the runs land on different warps instead of one after the other.
+    // GEOMETRIC ownership (from the first level with >= K1_GEO_THR wet cells on): thread (tx, ty) owns tracers, u and v of
+    // cell (tx, ty) and the west / south face fluxes of that cell: shared-memory accesses of a warp fall into one row of
+    // the box (no bank conflicts), global accesses are contiguous, and no list is decoded.
+    // t1 = first level of the role the descriptor serves (which = 0: tracers, first wet level; 1: u, first open west face;
+    // 2: v, first open south face); z2, z3: thresholds of the vorticity reconstruction orders
+    struct Cell { int cx, cy, t1, bo, by; unsigned c; bool incol; unsigned char z2, z3; };
     auto make_cell = [&](int g, int which) {
         Cell X;
         X.cx = g % TX; X.cy = g / TX;
         const int i = i0 + X.cx, j = j0 + X.cy;
         X.incol = i < P.nx && j < P.ny;
-        X.c = (long long)(j + OCN_HALO) * sx + i;
+        X.c = (unsigned)((j + OCN_HALO) * sx + i);
         const uint2 mo = s_m8[X.cy * RX + X.cx];
         const int kb = X.incol ? (int)(mo.x & 255u) : nz;
         X.t1 = !X.incol ? nz : which == 0 ? kb : which == 1 ? (int)((mo.x >> 8) & 255u) : (int)(mo.y & 255u);
@@ -329,45 +344,66 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
         X.by = X.cy + OY; X.bo = X.by * BX + X.cx + OX;
         return X;
     };
-    const Cell cT = make_cell(gT, 0), cU = make_cell(gU, 1), cV = make_cell(gV, 2);
+    Cell cT = make_cell(gT, 0), cU = make_cell(gU, 1), cV = make_cell(gV, 2);
     const T dy = P.dy, rdy = P.rdy;
+    const int ks = s_ks;                                 // iterations m <= ks run compact, m > ks geometric
 
     double wacc0 = 0.0, wacc1 = 0.0;                     // w accumulators of this thread's ring points
     T2 fz_bot = mk2(T(0), T(0));                         // vertical tracer flux through the face below
     T u_dn = 0, v_dn = 0;
-    T ddu = 0, ddv = 0;
-    T2 ddts = mk2(T(0), T(0));                           // eliminated right-hand sides of the level below
     double aGU = 0, aGV = 0, aSU = 0, aSV = 0;
-    // RI: the Thomas rows of this thread's columns and dt * diffusivity at the face below the current level
+    // Thomas rows of this thread's columns: d0 (, d1) = eliminated right-hand sides of the level below; RI also carries the
+    // modified super-diagonal cp and dt * diffusivity at the face below the current level
     ThomasRow<T> rt{T(0), T(0), T(0)}, ru{T(0), T(0), T(0)}, rv{T(0), T(0), T(0)};
     T kt_lo = 0, ku_lo = 0, kv_lo = 0;
 
-    for (int m = kmin; m <= nz; ++m) {
+    // advective + diffusive flux of the (T, S) pair through one face: b = box index of the cell east / north
+    // of the face, st = box stride across it, row = box row (metrics)
+    auto face_flux = [&](const T2* __restrict__ s_ts, const T2* __restrict__ s_uv, const int b, const bool isy, const int st,
+                         const int row, const int ord, const T dzk) -> T2 {
+        const T2 uvf = s_uv[b];
+        const T vel = isy ? uvf.y : uvf.x;
+        const T len = isy ? s_dxF[row] : dy;                       // face length; the face area is len * dz
+        const T dd = isy ? dy : s_dxC[row], rdd = isy ? rdy : s_rdxC[row];   // centre-to-centre distance
+        const T2 cm = s_ts[b - st], cc = s_ts[b];
+        const T2 fv = weno_face2<WZ>(s_ts[b - 3 * st], s_ts[b - 2 * st], cm, cc, s_ts[b + st], s_ts[b + 2 * st], vel, ord);
+        const Xv<T> adv = X(vel) * X(len) * X(dzk), dif = X(P.kappa_h) * X(len) * X(dzk);
+        T2 flux;
+        flux.x = (adv * X(fv.x) - xdiv(dif * (X(cc.x) - X(cm.x)), dd, rdd)).v;
+        flux.y = (adv * X(fv.y) - xdiv(dif * (X(cc.y) - X(cm.y)), dd, rdd)).v;
+        return flux;
+    };
+
+    // one iteration of the march: parts A(m) and B(m - 1), then ONE block barrier.  GEO selects the ownership (a compile-time
+    // tag: the geometric body has one cell descriptor, constant strides and no lists)
+    auto iteration = [&](auto geo_tag, const int m, const Cell& XT, const Cell& XU, const Cell& XV) {
+        constexpr bool GEO = decltype(geo_tag)::value;
         const int kB = m - 1;                                 // level of part B (phase 3) in this iteration
-        const bool doB = kB >= kmin, wetT = doB && kB >= cT.t1, wetU = doB && kB >= cU.t1, wetV = doB && kB >= cV.t1;
+        const bool doB = kB >= kmin, wetT = doB && kB >= XT.t1, wetU = doB && kB >= XU.t1, wetV = doB && kB >= XV.t1;
         // AB2 history and pivots of level kB: issued now, consumed after part A.  A warp without an active cell or
         // face at this level (most warps on sparsely wet levels) skips this and all of part B.
         const bool anyB = __any_sync(0xffffffffu, wetT | wetU | wetV);
-        long long oT = 0, oU = 0, oV = 0;
         T2 gm_ts = mk2(T(0), T(0));
         T gm_u = 0, gm_v = 0;
         T piv_t = 1, piv_u = 1, piv_v = 1;
+        const long long okB = (long long)kB * sz;             // warp-uniform level base; the column offsets are 32-bit
         if (anyB) {
-            const long long okB = (long long)kB * sz;
             if (wetT) {
-                oT = okB + cT.c;
-                gm_ts = P.Gts[oT];
-                if (!RI) piv_t = sizeof(T) == 8 ? P.m_t[kB * nz + cT.t1] : P.rm_t[kB * nz + cT.t1];
+                gm_ts = (P.Gts + okB)[XT.c];
+                if (!RI) piv_t = sizeof(T) == 8 ? P.m_t[kB * nz + XT.t1] : P.rm_t[kB * nz + XT.t1];
             }
-            if (wetU) {
-                oU = okB + cU.c;
-                gm_u = ((const T*)(P.Guv + oU))[0];
-                if (!RI) piv_u = sizeof(T) == 8 ? P.m_m[kB * nz + cU.t1] : P.rm_m[kB * nz + cU.t1];
+            if (GEO) {
+                if (wetU | wetV) {
+                    const T2 g2 = (P.Guv + okB)[XU.c];
+                    gm_u = g2.x; gm_v = g2.y;
+                }
+            } else {
+                if (wetU) gm_u = ((const T*)(P.Guv + okB + XU.c))[0];
+                if (wetV) gm_v = ((const T*)(P.Guv + okB + XV.c))[1];
             }
-            if (wetV) {
-                oV = okB + cV.c;
-                gm_v = ((const T*)(P.Guv + oV))[1];
-                if (!RI) piv_v = sizeof(T) == 8 ? P.m_m[kB * nz + cV.t1] : P.rm_m[kB * nz + cV.t1];
+            if (!RI) {
+                if (wetU) piv_u = sizeof(T) == 8 ? P.m_m[kB * nz + XU.t1] : P.rm_m[kB * nz + XU.t1];
+                if (wetV) piv_v = sizeof(T) == 8 ? P.m_m[kB * nz + XV.t1] : P.rm_m[kB * nz + XV.t1];
             }
         }
         mbar_wait(&bars[(m - kmin) % C::NB], (uint32_t)(((m - kmin) / C::NB) & 1));
@@ -418,26 +454,33 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 }
             }
             // ================= phase 2: tracer face fluxes, each open face once =================
-            {
-                const T2* __restrict__ s_ts = (const T2*)(sm + C::O_TS + (k & (C::R_TS - 1)) * C::PL2);
+            const T2* __restrict__ s_ts = (const T2*)(sm + C::O_TS + (k & (C::R_TS - 1)) * C::PL2);
+            if constexpr (GEO) {
+                // the west and the south face of the own cell (thresholds of the cell's own mask word), then the east edge of
+                // the tile by lanes 0 .. TY-1 of warp 0 and the north edge by warp 1
+                const uint2 mo = s_m8[XT.cy * RX + XT.cx];
+                const int ox = order3(k, (mo.x >> 8) & 255u, (mo.x >> 16) & 255u, mo.x >> 24);
+                const int oy = order3(k, mo.y & 255u, (mo.y >> 8) & 255u, (mo.y >> 16) & 255u);
+                if (ox > 0) s_flux[XT.cy * RX + XT.cx] = face_flux(s_ts, s_uv, XT.bo, false, 1, XT.by, ox, dzk);
+                if (oy > 0) s_flux[C::NFX + XT.cy * TX + XT.cx] = face_flux(s_ts, s_uv, XT.bo, true, BX, XT.by, oy, dzk);
+                if (tid < TY) {
+                    const uint2 me = s_m8[tid * RX + TX];
+                    const int oe = order3(k, (me.x >> 8) & 255u, (me.x >> 16) & 255u, me.x >> 24);
+                    if (oe > 0) s_flux[tid * RX + TX] = face_flux(s_ts, s_uv, (tid + OY) * BX + TX + OX, false, 1, tid + OY, oe, dzk);
+                } else if (tid >= 32 && tid < 32 + TX) {
+                    const int fx = tid - 32;
+                    const uint2 mn = s_m8[TY * RX + fx];
+                    const int on = order3(k, mn.y & 255u, (mn.y >> 8) & 255u, (mn.y >> 16) & 255u);
+                    if (on > 0) s_flux[C::NFX + TY * TX + fx] = face_flux(s_ts, s_uv, (TY + OY) * BX + fx + OX, true, BX, TY + OY, on, dzk);
+                }
+            } else {
                 const int nface = s_nf[k];
                 for (int f = (tid + NT - K1_FOFF) % NT; f < nface; f += NT) {
                     const uint2 d = s_fs[f];
                     const int b = d.x & 1023u, row = (d.x >> 10) & 15u, fid = d.x >> 16;
                     const bool isy = (d.x >> 14) & 1u;
-                    const int st = isy ? BX : 1;
                     const int ord = order3(k, d.y & 255u, (d.y >> 8) & 255u, (d.y >> 16) & 255u);   // >= 1 here
-                    const T2 uvf = s_uv[b];
-                    const T vel = isy ? uvf.y : uvf.x;
-                    const T len = isy ? s_dxF[row] : dy;                       // face length; the face area is len * dz
-                    const T dd = isy ? dy : s_dxC[row], rdd = isy ? rdy : s_rdxC[row];   // centre-to-centre distance
-                    const T2 cm = s_ts[b - st], cc = s_ts[b];
-                    const T2 fv = weno_face2<WZ>(s_ts[b - 3 * st], s_ts[b - 2 * st], cm, cc, s_ts[b + st], s_ts[b + 2 * st], vel, ord);
-                    const Xv<T> adv = X(vel) * X(len) * X(dzk), dif = X(P.kappa_h) * X(len) * X(dzk);
-                    T2 flux;
-                    flux.x = (adv * X(fv.x) - xdiv(dif * (X(cc.x) - X(cm.x)), dd, rdd)).v;
-                    flux.y = (adv * X(fv.y) - xdiv(dif * (X(cc.y) - X(cm.y)), dd, rdd)).v;
-                    s_flux[fid] = flux;
+                    s_flux[fid] = face_flux(s_ts, s_uv, b, isy, isy ? BX : 1, row, ord, dzk);
                 }
             }
         }
@@ -452,25 +495,33 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             const T* __restrict__ s_zeta = (const T*)(sm + C::O_ZETA + (k & 1) * C::PL1);
             const T2* __restrict__ s_kd = (const T2*)(sm + C::O_KD + (k & 1) * C::KDB);
             const T2* __restrict__ s_flux = (const T2*)(sm + C::O_FLUX + (k & 1) * C::FLB);
-            // ---------- tracer half: the cell of rank tid ----------
+            const bool has_hi = k + 1 < nz;
+            // RI: vertical spacings around level k for the per-column elimination
+            T dzc_lo = T(1), dzc_hi = T(1), rc_lo = T(1), rc_hi = T(1);
+            const T2* __restrict__ s_nk1 = nullptr;
+            if constexpr (RI) {
+                if (k > 0) { dzc_lo = P.dzc[k]; rc_lo = P.rdzc[k]; }
+                if (has_hi) { dzc_hi = P.dzc[k + 1]; rc_hi = P.rdzc[k + 1]; }
+                s_nk1 = (const T2*)(sm + C::O_NK + ((k + 1) & 1) * C::KDB);
+            }
+            // ---------- tracer half ----------
             T2 fz_top = mk2(T(0), T(0));
             if (wetT) {
-                const int cx = cT.cx, cy = cT.cy, kb = cT.t1, bo = cT.bo, by = cT.by;
-                const long long o = oT;
+                const int cx = XT.cx, cy = XT.cy, kb = XT.t1, bo = XT.bo, by = XT.by;
                 const T AzCj = s_AzC[by], rAzCj = s_rAzC[by];
                 const T w_c1 = s_w1[(cy + 1) * RX + cx + 1];
                 // vertical face above cell k (own column)
                 {
-                const int ozt = (k + 1 < nz) ? min(3, min(k + 1 - kb, nz - k - 1)) : 0;
-                if (ozt > 0) {
-                    auto tsz = [&](int dk) -> T2 {           // plane of level k + dk, dk = -2 .. 3
-                        return ((const T2*)(sm + C::O_TS + ((k + dk) & (C::R_TS - 1)) * C::PL2))[bo];
-                    };
-                    const T2 fv = weno_face2<WZ>(tsz(-2), tsz(-1), tsz(0), tsz(1), tsz(2), tsz(3), w_c1, ozt);
-                    fz_top.x = (X(w_c1) * X(AzCj) * X(fv.x)).v;
-                    fz_top.y = (X(w_c1) * X(AzCj) * X(fv.y)).v;
+                    const int ozt = has_hi ? min(3, min(k + 1 - kb, nz - k - 1)) : 0;
+                    if (ozt > 0) {
+                        auto tsz = [&](int dk) -> T2 {           // plane of level k + dk, dk = -2 .. 3
+                            return ((const T2*)(sm + C::O_TS + ((k + dk) & (C::R_TS - 1)) * C::PL2))[bo];
+                        };
+                        const T2 fv = weno_face2<WZ>(tsz(-2), tsz(-1), tsz(0), tsz(1), tsz(2), tsz(3), w_c1, ozt);
+                        fz_top.x = (X(w_c1) * X(AzCj) * X(fv.x)).v;
+                        fz_top.y = (X(w_c1) * X(AzCj) * X(fv.y)).v;
+                    }
                 }
-            }
                 // ---- tracers ----
                 const T2 fw = s_flux[cy * RX + cx], fe = s_flux[cy * RX + cx + 1];
                 const T2 fs = s_flux[C::NFX + cy * TX + cx], fn = s_flux[C::NFX + (cy + 1) * TX + cx];
@@ -488,31 +539,30 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                     const T src = w_c1 * rdzk;     // of the constant under the zero-top-flux linear free surface
                     GT += P.Toff * src; GS += P.Soff * src;
                     // surface tracer forcing: flux into the ocean + restoring toward the target
-                    const T2 qf = P.qts[cT.c], rt = P.rts[cT.c];
-                    GT = (X(GT) + xdiv(X(qf.x) + X(P.gamma_T) * (X(rt.x) - X(tsc.x)), dzk, rdzk)).v;
-                    GS = (X(GS) + xdiv(X(qf.y) + X(P.gamma_S) * (X(rt.y) - X(tsc.y)), dzk, rdzk)).v;
+                    const T2 qf = P.qts[XT.c], rtg = P.rts[XT.c];
+                    GT = (X(GT) + xdiv(X(qf.x) + X(P.gamma_T) * (X(rtg.x) - X(tsc.x)), dzk, rdzk)).v;
+                    GS = (X(GS) + xdiv(X(qf.y) + X(P.gamma_S) * (X(rtg.y) - X(tsc.y)), dzk, rdzk)).v;
                 }
                 // ---- quasi-AB2, predictor, elimination sweep (S3, S4) ----
                 const T Ght = (X(c0) * X(GT) - X(c1) * X(gm_ts.x)).v, Ghs = (X(c0) * X(GS) - X(c1) * X(gm_ts.y)).v;
-                P.Gts[o] = mk2(GT, GS);
+                (P.Gts + okB)[XT.c] = mk2(GT, GS);
                 if constexpr (RI) {               // per-face diffusivity: kappa of the own column at the face above
-                    const bool has_hi = k + 1 < nz;
-                    const T kt_hi = has_hi ? (X(P.dt) * X(((const T2*)(sm + C::O_NK + ((k + 1) & 1) * C::KDB))[(cy + 1) * RX + cx + 1].y)).v : T(0);
-                    rt.step(k == kb, kt_lo, kt_hi, has_hi, dzk, k > 0 ? P.dzc[k] : T(1), has_hi ? P.dzc[k + 1] : T(1), rdzk,
-                            k > 0 ? P.rdzc[k] : T(1), has_hi ? P.rdzc[k + 1] : T(1), E::add(tsc.x, E::mul(P.dt, Ght)), E::add(tsc.y, E::mul(P.dt, Ghs)));
-                    P.dts[o] = mk2(rt.d0, rt.d1);
-                    P.cpt[o] = rt.cp;
+                    const T kt_hi = has_hi ? (X(P.dt) * X(s_nk1[(cy + 1) * RX + cx + 1].y)).v : T(0);
+                    rt.step(k == kb, kt_lo, kt_hi, has_hi, dzk, dzc_lo, dzc_hi, rdzk, rc_lo, rc_hi,
+                            E::add(tsc.x, E::mul(P.dt, Ght)), E::add(tsc.y, E::mul(P.dt, Ghs)));
+                    (P.cpt + okB)[XT.c] = rt.cp;
                     kt_lo = kt_hi;
                 } else {
-                const T smk = k > kb ? P.sm_t[k] : T(0);
-                ddts.x = E::div(E::add(E::add(tsc.x, E::mul(P.dt, Ght)), E::mul(smk, ddts.x)), piv_t, piv_t);
-                ddts.y = E::div(E::add(E::add(tsc.y, E::mul(P.dt, Ghs)), E::mul(smk, ddts.y)), piv_t, piv_t);
-                P.dts[o] = ddts;
+                    const T smk = k > kb ? P.sm_t[k] : T(0);
+                    rt.d0 = E::div(E::add(E::add(tsc.x, E::mul(P.dt, Ght)), E::mul(smk, rt.d0)), piv_t, piv_t);
+                    rt.d1 = E::div(E::add(E::add(tsc.y, E::mul(P.dt, Ghs)), E::mul(smk, rt.d1)), piv_t, piv_t);
                 }
+                (P.dts + okB)[XT.c] = mk2(rt.d0, rt.d1);
             }
             // ---------- momentum: the u face and the v face this thread owns ----------
+            T Gu_out = 0, du_out = 0, cpu_out = 0;
             if (wetU) {
-                const int cx = cU.cx, cy = cU.cy, tx1 = cU.t1, bo = cU.bo, by = cU.by;
+                const int cx = XU.cx, cy = XU.cy, tx1 = XU.t1, bo = XU.bo, by = XU.by;
                 const int qo = (cy + 1) * RX + cx + 1;                       // this column in the ring arrays
                 const T w_c1 = s_w1[qo], w_c0 = s_w0[qo];
                 const T dxFj = s_dxF[by], dxFn = s_dxF[by + 1], dxCj = s_dxC[by], rdxCj = s_rdxC[by];
@@ -521,7 +571,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 const T2 uvc = s_uv[bo];
                 const T u_c = uvc.x, v_c = uvc.y;
                 const T2 uv_w = s_uv[bo - 1], uv_n = s_uv[bo + BX], uv_nw = s_uv[bo + BX - 1];
-                const T u_up = (k + 1 < nz) ? s_uv1[bo].x : T(0);
+                const T u_up = has_hi ? s_uv1[bo].x : T(0);
                 const T z00 = s_zeta[bo];
                 const T2 kdc = s_kd[qo];
                 const int pbo = (cy + 1) * C::PBX + cx + 4;
@@ -529,7 +579,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 const T vold = (X(AzCj) * X(dzk)).v;
                 const Xv<T> vsum_s = X(uv_w.y) + X(v_c), vsum_n = X(uv_nw.y) + X(uv_n.y);
                 const T vhat = xdiv(quart * (X(dxFj) * vsum_s + X(dxFn) * vsum_n), dxCj, rdxCj).v;
-                const int ozu = 1 + (k >= cU.z2) + (k >= cU.z3);
+                const int ozu = 1 + (k >= XU.z2) + (k >= XU.z3);
                 const T z01 = s_zeta[bo + BX];
                 const T zt = ozu == 1 ? (vhat > T(0) ? z00 : z01)
                                       : weno_face<WZ>(s_zeta[bo - 2 * BX], s_zeta[bo - BX], z00, z01, s_zeta[bo + 2 * BX],
@@ -539,40 +589,38 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 const Xv<T> dK = xdiv(X(kdc.x) - X(kdw.x), dxCj, rdxCj);
                 const Xv<T> dP = xdiv(X((T)(s_p[pbo] - s_p[pbo - 1])), dxCj, rdxCj);
                 const Xv<T> dlo((k >= 1 && k - 1 >= tx1) ? (X(u_c) - X(u_dn)).v : T(0));
-                const Xv<T> dhi((k + 1 <= nz - 1) ? (X(u_up) - X(u_c)).v : T(0));
+                const Xv<T> dhi(has_hi ? (X(u_up) - X(u_c)).v : T(0));
                 const Xv<T> Whi = half * X(AzCj) * (X(s_w1[qo - 1]) + X(w_c1)), Wlo = half * X(AzCj) * (X(s_w0[qo - 1]) + X(w_c0));
                 const Xv<T> Au = xdiv(half * (Whi * dhi + Wlo * dlo), vold, rAzCj * rdzk);
                 const Xv<T> Vu = nuh * (xdiv(X(kdc.y) - X(kdw.y), dxCj, rdxCj) - xdiv(X(z01) - X(z00), dy, rdy));
-                const Xv<T> tau((k == nz - 1) ? xdiv(X(P.taux[cU.c]), (X(P.rho0) * X(dzk)).v, P.rrho0 * rdzk).v : T(0));
-                // bottom drag on the lowest open level of the column
+                const Xv<T> tau((k == nz - 1) ? xdiv(X(P.taux[XU.c]), (X(P.rho0) * X(dzk)).v, P.rrho0 * rdzk).v : T(0));
                 T Gu = (X(zt) * X(vhat) + Cu - dK - dP - Au + Vu + tau).v;
-                if constexpr (DRAG) {
+                if constexpr (DRAG) {             // bottom drag on the lowest open level of the column
                     const Xv<T> drag(k == tx1 ? xdiv((X(P.drag_r) + X(P.drag_cd) * X((T)sqrt((X(u_c) * X(u_c) + X(vhat) * X(vhat)).v))) * X(u_c), dzk, rdzk).v : T(0));
                     Gu = (X(Gu) - drag).v;
                 }
                 // ---- quasi-AB2, predictor, elimination sweep (S3, S4, S5) ----
                 const T Ghu = (X(c0) * X(Gu) - X(c1) * X(gm_u)).v;
-                ((T*)(P.Guv + oU))[0] = Gu;
                 const T us = E::add(u_c, E::mul(P.dt, Ghu));
                 aGU = (X(aGU) + X((double)dzk) * X((double)Ghu)).v; aSU = (X(aSU) + X((double)dzk) * X((double)us)).v;
                 if constexpr (RI) {               // nu at the u face = mean of the two tracer columns that share it
-                    const bool has_hi = k + 1 < nz;
-                    const T2* __restrict__ s_nk1 = (const T2*)(sm + C::O_NK + ((k + 1) & 1) * C::KDB);
                     const T ku_hi = has_hi ? (X(P.dt) * (X(T(0.5)) * (X(s_nk1[qo - 1].x) + X(s_nk1[qo].x)))).v : T(0);
-                    ru.step(k == tx1, ku_lo, ku_hi, has_hi, dzk, k > 0 ? P.dzc[k] : T(1), has_hi ? P.dzc[k + 1] : T(1), rdzk,
-                            k > 0 ? P.rdzc[k] : T(1), has_hi ? P.rdzc[k + 1] : T(1), us, T(0));
-                    ((T*)(P.duv + oU))[0] = ru.d0;
-                    ((T*)(P.cpuv + oU))[0] = ru.cp;
+                    ru.step(k == tx1, ku_lo, ku_hi, has_hi, dzk, dzc_lo, dzc_hi, rdzk, rc_lo, rc_hi, us, T(0));
                     ku_lo = ku_hi;
                 } else {
-                const T smk = k > tx1 ? P.sm_m[k] : T(0);
-                ddu = E::div(E::add(us, E::mul(smk, ddu)), piv_u, piv_u);
-                ((T*)(P.duv + oU))[0] = ddu;
+                    const T smk = k > tx1 ? P.sm_m[k] : T(0);
+                    ru.d0 = E::div(E::add(us, E::mul(smk, ru.d0)), piv_u, piv_u);
+                }
+                if constexpr (GEO) { Gu_out = Gu; du_out = ru.d0; cpu_out = ru.cp; }
+                else {
+                    ((T*)(P.Guv + okB + XU.c))[0] = Gu; ((T*)(P.duv + okB + XU.c))[0] = ru.d0;
+                    if constexpr (RI) ((T*)(P.cpuv + okB + XU.c))[0] = ru.cp;
                 }
                 u_dn = u_c;
             }
+            T Gv_out = 0, dv_out = 0, cpv_out = 0;
             if (wetV) {
-                const int cx = cV.cx, cy = cV.cy, ty1 = cV.t1, bo = cV.bo, by = cV.by;
+                const int cx = XV.cx, cy = XV.cy, ty1 = XV.t1, bo = XV.bo, by = XV.by;
                 const int qo = (cy + 1) * RX + cx + 1;
                 const T w_c1 = s_w1[qo], w_c0 = s_w0[qo];
                 const T dxFj = s_dxF[by], rdxFj = s_rdxF[by];
@@ -581,13 +629,13 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 const T2 uvc = s_uv[bo];
                 const T u_c = uvc.x, v_c = uvc.y;
                 const T2 uv_s = s_uv[bo - BX], uv_e = s_uv[bo + 1], uv_se = s_uv[bo - BX + 1];
-                const T v_up = (k + 1 < nz) ? s_uv1[bo].y : T(0);
+                const T v_up = has_hi ? s_uv1[bo].y : T(0);
                 const T z00 = s_zeta[bo];
                 const T2 kdc = s_kd[qo];
                 const int pbo = (cy + 1) * C::PBX + cx + 4;
                 const Xv<T> half(T(0.5)), quart(T(0.25)), nuh(P.nu_h);
                 const T uhat = (quart * (X(uv_s.x) + X(u_c) + X(uv_se.x) + X(uv_e.x))).v;
-                const int ozv = 1 + (k >= cV.z2) + (k >= cV.z3);
+                const int ozv = 1 + (k >= XV.z2) + (k >= XV.z3);
                 const T z10 = s_zeta[bo + 1];
                 const T zt = ozv == 1 ? (uhat > T(0) ? z00 : z10)
                                       : weno_face<WZ>(s_zeta[bo - 2], s_zeta[bo - 1], z00, z10, s_zeta[bo + 2], s_zeta[bo + 3], uhat, ozv);
@@ -596,41 +644,90 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 const Xv<T> dK = xdiv(X(kdc.x) - X(kds.x), dy, rdy);
                 const Xv<T> dP = xdiv(X((T)(s_p[pbo] - s_p[pbo - C::PBX])), dy, rdy);
                 const Xv<T> dlo((k >= 1 && k - 1 >= ty1) ? (X(v_c) - X(v_dn)).v : T(0));
-                const Xv<T> dhi((k + 1 <= nz - 1) ? (X(v_up) - X(v_c)).v : T(0));
+                const Xv<T> dhi(has_hi ? (X(v_up) - X(v_c)).v : T(0));
                 const Xv<T> Whi = half * (X(AzCs) * X(s_w1[qo - RX]) + X(AzCj) * X(w_c1));
                 const Xv<T> Wlo = half * (X(AzCs) * X(s_w0[qo - RX]) + X(AzCj) * X(w_c0));
                 const Xv<T> Av = xdiv(half * (Whi * dhi + Wlo * dlo), (X(AzFj) * X(dzk)).v, rAzFj * rdzk);
                 const Xv<T> Vv = nuh * (xdiv(X(kdc.y) - X(kds.y), dy, rdy) + xdiv(X(z10) - X(z00), dxFj, rdxFj));
-                const Xv<T> tau((k == nz - 1) ? xdiv(X(P.tauy[cV.c]), (X(P.rho0) * X(dzk)).v, P.rrho0 * rdzk).v : T(0));
+                const Xv<T> tau((k == nz - 1) ? xdiv(X(P.tauy[XV.c]), (X(P.rho0) * X(dzk)).v, P.rrho0 * rdzk).v : T(0));
                 T Gv = (-X(zt) * X(uhat) - Cv - dK - dP - Av + Vv + tau).v;
                 if constexpr (DRAG) {
                     const Xv<T> drag(k == ty1 ? xdiv((X(P.drag_r) + X(P.drag_cd) * X((T)sqrt((X(uhat) * X(uhat) + X(v_c) * X(v_c)).v))) * X(v_c), dzk, rdzk).v : T(0));
                     Gv = (X(Gv) - drag).v;
                 }
                 const T Ghv = (X(c0) * X(Gv) - X(c1) * X(gm_v)).v;
-                ((T*)(P.Guv + oV))[1] = Gv;
                 const T vs2 = E::add(v_c, E::mul(P.dt, Ghv));
                 aGV = (X(aGV) + X((double)dzk) * X((double)Ghv)).v; aSV = (X(aSV) + X((double)dzk) * X((double)vs2)).v;
                 if constexpr (RI) {
-                    const bool has_hi = k + 1 < nz;
-                    const T2* __restrict__ s_nk1 = (const T2*)(sm + C::O_NK + ((k + 1) & 1) * C::KDB);
                     const T kv_hi = has_hi ? (X(P.dt) * (X(T(0.5)) * (X(s_nk1[qo - RX].x) + X(s_nk1[qo].x)))).v : T(0);
-                    rv.step(k == ty1, kv_lo, kv_hi, has_hi, dzk, k > 0 ? P.dzc[k] : T(1), has_hi ? P.dzc[k + 1] : T(1), rdzk,
-                            k > 0 ? P.rdzc[k] : T(1), has_hi ? P.rdzc[k + 1] : T(1), vs2, T(0));
-                    ((T*)(P.duv + oV))[1] = rv.d0;
-                    ((T*)(P.cpuv + oV))[1] = rv.cp;
+                    rv.step(k == ty1, kv_lo, kv_hi, has_hi, dzk, dzc_lo, dzc_hi, rdzk, rc_lo, rc_hi, vs2, T(0));
                     kv_lo = kv_hi;
                 } else {
-                const T smk = k > ty1 ? P.sm_m[k] : T(0);
-                ddv = E::div(E::add(vs2, E::mul(smk, ddv)), piv_v, piv_v);
-                ((T*)(P.duv + oV))[1] = ddv;
+                    const T smk = k > ty1 ? P.sm_m[k] : T(0);
+                    rv.d0 = E::div(E::add(vs2, E::mul(smk, rv.d0)), piv_v, piv_v);
+                }
+                if constexpr (GEO) { Gv_out = Gv; dv_out = rv.d0; cpv_out = rv.cp; }
+                else {
+                    ((T*)(P.Guv + okB + XV.c))[1] = Gv; ((T*)(P.duv + okB + XV.c))[1] = rv.d0;
+                    if constexpr (RI) ((T*)(P.cpuv + okB + XV.c))[1] = rv.cp;
                 }
                 v_dn = v_c;
+            }
+            // stores of the momentum group: one pair store per array in geometric ownership (the same cell), member stores else
+            if constexpr (GEO) {
+                if (wetU | wetV) {
+                    (P.Guv + okB)[XU.c] = mk2(Gu_out, Gv_out);       // closed members hold 0, as they always have
+                    (P.duv + okB)[XU.c] = mk2(du_out, dv_out);
+                    if constexpr (RI) (P.cpuv + okB)[XU.c] = mk2(cpu_out, cpv_out);
+                }
             }
             fz_bot = fz_top;
         }
         __syncthreads();                       // planes of level m - 1 are dead: refill the ring
-        if (tid == PROD && m + C::DP <= nz) issue_group(m + C::DP, false);
+        if (tid == PROD && m + C::DP <= nz) {
+            const int g = m + C::DP;
+            if (g + 2 < nz) {                  // steady state: one plane of each array (the general form handles the ends)
+                uint64_t* bar = &bars[(g - kmin) % C::NB];
+                mbar_expect_tx(bar, 2 * C::BYTES2 + C::BYTESP);
+                tma_load_plane(sm + C::O_TS + ((g + 2) % C::R_TS) * C::PL2, &m_ts, bar, 2 * i0, j0, g + 2);
+                tma_load_plane(sm + C::O_UV + ((g + (RI ? 1 : 0)) % C::R_UV) * C::PL2, &m_uv, bar, 2 * i0, j0, g + (RI ? 1 : 0));
+                tma_load_plane(sm + C::O_P + ((g - 1) % C::R_P) * C::PLP, &m_p, bar, i0, j0 + 2, g - 1);
+            } else {
+                issue_group(g, false);
+            }
+        }
+    };
+
+    typedef std::true_type GeoTag;
+    typedef std::false_type CmpTag;
+    int m = kmin;
+    for (; m <= nz && m <= ks; ++m) iteration(CmpTag{}, m, cT, cU, cV);
+    if (m <= nz) {
+        // ---- switch of ownership: the column state travels through shared memory to the thread of the cell's own position.
+        // Every cell is owned by exactly one thread in each of the three compact orders, so every slot is written once.
+        double* const xp = (double*)(sm + C::O_XP);
+        auto travel = [&](const int gold, double a, double b, double c, double d, double (&out)[4]) {
+            xp[gold * 4 + 0] = a; xp[gold * 4 + 1] = b; xp[gold * 4 + 2] = c; xp[gold * 4 + 3] = d;
+            __syncthreads();
+#pragma unroll
+            for (int q = 0; q < 4; ++q) out[q] = xp[tid * 4 + q];
+            __syncthreads();
+        };
+        double r[4];
+        travel(gT, (double)rt.cp, (double)rt.d0, (double)rt.d1, (double)kt_lo, r);
+        rt.cp = (T)r[0]; rt.d0 = (T)r[1]; rt.d1 = (T)r[2]; kt_lo = (T)r[3];
+        travel(gT, (double)fz_bot.x, (double)fz_bot.y, 0.0, 0.0, r);
+        fz_bot = mk2((T)r[0], (T)r[1]);
+        travel(gU, (double)ru.cp, (double)ru.d0, (double)ku_lo, (double)u_dn, r);
+        ru.cp = (T)r[0]; ru.d0 = (T)r[1]; ku_lo = (T)r[2]; u_dn = (T)r[3];
+        travel(gU, aGU, aSU, 0.0, 0.0, r);
+        aGU = r[0]; aSU = r[1];
+        travel(gV, (double)rv.cp, (double)rv.d0, (double)kv_lo, (double)v_dn, r);
+        rv.cp = (T)r[0]; rv.d0 = (T)r[1]; kv_lo = (T)r[2]; v_dn = (T)r[3];
+        travel(gV, aGV, aSV, 0.0, 0.0, r);
+        aGV = r[0]; aSV = r[1];
+        cT = make_cell(tid, 0); cU = make_cell(tid, 1); cV = make_cell(tid, 2);
+        for (; m <= nz; ++m) iteration(GeoTag{}, m, cT, cU, cV);
     }
     if (cU.incol && cU.t1 < nz) { P.GU[cU.c] = (T)aGU; P.SU[cU.c] = (T)aSU; }     // never-open faces keep their zeros
     if (cV.incol && cV.t1 < nz) { P.GV[cV.c] = (T)aGV; P.SV[cV.c] = (T)aSV; }

@@ -269,6 +269,7 @@ ocn_status build_model(ocn_model* M) {
     P.nu_h = (T)M->d.nu_h; P.kappa_h = (T)M->d.kappa_h; P.dtau = (T)M->dtau;
     // equation of state: per-level thermal expansion alpha (1 - gamma zc[k]) and alpha2 / 2, in the fp64
     // operations the equation is written in
+    P.geo_thr = K1_GEO_THR;
     P.eos = M->d.eos; P.ha2_d = 0.5 * M->d.eos_alpha2;
     {
         std::vector<double> ath(nz);
@@ -785,6 +786,19 @@ ocn_status ocn_profile_read(ocn_model* M, double* ms, long long* launches, int r
         if (launches) launches[q] = M->prof_launches[q];
         if (reset) { M->prof_ms[q] = 0; M->prof_launches[q] = 0; }
     }
+    return OCN_OK;
+}
+
+ocn_status ocn_tune(ocn_model* M, const char* key, double value) {
+    if (!M || !key) return fail(OCN_EINVAL, "null argument");
+    ON_DEVICE(M->d.device);
+    if (std::string(key) == "k1_geo_threshold") {
+        if (!(value >= 0 && value <= 1e6)) return fail(OCN_EINVAL, "k1_geo_threshold out of range");
+        M->pf.geo_thr = (int)value; M->pd.geo_thr = (int)value;
+    } else {
+        return fail(OCN_EINVAL, std::string("unknown tuning key: ") + key);
+    }
+    if (M->graph) { CK(cudaStreamSynchronize(M->stream)); cudaGraphExecDestroy(M->graph); M->graph = nullptr; }   // re-capture with the new arguments
     return OCN_OK;
 }
 

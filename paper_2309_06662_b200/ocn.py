@@ -46,7 +46,7 @@ class ocn_fields(C.Structure):
 EXPORTS = ["ocn_grid_create", "ocn_grid_destroy", "ocn_model_create", "ocn_model_destroy", "ocn_set_fields",
            "ocn_time_step", "ocn_get_fields", "ocn_synchronize", "ocn_get_masks", "ocn_model_info",
            "ocn_get_debug", "ocn_last_error", "ocn_version", "ocn_profile_enable", "ocn_profile_read",
-           "ocn_stage_name", "ocn_get_mixing", "ocn_get_fields_async", "ocn_wait"]
+           "ocn_stage_name", "ocn_get_mixing", "ocn_get_fields_async", "ocn_wait", "ocn_tune"]
 NSTAGES = 4
 
 
@@ -70,6 +70,7 @@ def lib():
         L.ocn_synchronize.argtypes = [vp]
         L.ocn_get_fields_async.argtypes = [vp, C.POINTER(ocn_fields), C.POINTER(C.c_ulonglong)]
         L.ocn_wait.argtypes = [vp, C.c_ulonglong]
+        L.ocn_tune.argtypes = [vp, C.c_char_p, C.c_double]
         L.ocn_get_masks.argtypes = [vp] + [vp] * 6
         L.ocn_model_info.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_ulonglong)]
         L.ocn_get_debug.argtypes = [vp] + [vp] * 6
@@ -170,6 +171,9 @@ class Model:
 
     def wait(self, ticket):
         _check(lib().ocn_wait(self.h, int(ticket)))
+
+    def tune(self, key, value):
+        _check(lib().ocn_tune(self.h, key.encode(), float(value)))
 
     def time_step(self, n=1):
         _check(lib().ocn_time_step(self.h, int(n)))
