@@ -56,6 +56,7 @@ def parse():
                          "of PAPER.md:114 (SURVEY 8f-1; DESIGN.md §3.12)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the end-to-end (host buffer) leg")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-closure-leg", action="store_true", help="skip the second model with the Ri closure")
     return ap.parse_args()
 
 
@@ -98,10 +99,18 @@ def _oracle_sample(config):
     return wl, what
 
 
-def time_oracle(config, steps, warmup, closure="const"):
+def time_oracle(config, steps, warmup, closure="const", threads=None, shrink=False):
     import oracle
     oracle.build()
+    if threads:
+        oracle.set_num_threads(threads)
     wl, what = oracle_sample(config, closure)
+    if shrink and config == 4:                   # the 1-thread figure: a quarter of the window, same physics
+        from paper_2309_06662_b200 import workloads as W
+        wl = W.config4(window=(500, 600, 1300, 1500), steps=1)
+        what = "config 4 window j=500:600 i=1300:1500 (closed box, identical physics)"
+        if closure == "ri":
+            W.with_ri_closure(wl)
     g = wl["grid"]
     cells = g["nx"] * g["ny"] * g["nz"]
     ref = oracle.RefModel(wl)
@@ -193,6 +202,16 @@ def ncu_entry(workload, kernel):
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
             e = json.load(f).get(kernel)
         return e if e and e.get("workload") == workload else None
+    except Exception:
+        return None
+
+
+def ncu_step_traffic(workload):
+    """DRAM bytes of one whole step (all kernels) from the committed ncu capture of this workload, if any."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            e = json.load(f).get("step")
+        return float(e["dram_bytes_per_step"]) if e and e.get("workload") == workload else None
     except Exception:
         return None
 
@@ -314,71 +333,129 @@ def run_ours(args):
         roof = {"kernel": dom, "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes, "traffic": None}
 
-    # K1 is issue bound rather than HBM bound: second view against the fp32 lane-op ceiling
-    # 148 SMs x 128 lanes x SM clock, with the executed thread instructions of the committed ncu capture
-    roof_alu = None
+    # K1 is bound by instruction issue, not by HBM.  This is an issue-slot UTILISATION (all executed warp
+    # instructions, integer and control included, of the committed ncu capture against 148 SMs x 4 schedulers x SM clock),
+    # not a roofline of useful work
+    issue_util = None
     ent = ncu_entry(workload_name(wl), dom)
-    if ent and "thread_instructions_per_launch" in ent:
+    if ent and "warp_instructions_per_launch" in ent:
         mhz = clk.get("sm_mhz") or 1965.0
-        peak_ops = 148 * 128 * mhz * 1e6
-        ach_ops = ent["thread_instructions_per_launch"] / (stages[dom]["ms"] / K * 1e-3)
-        roof_alu = {"kernel": dom, "bound": "alu", "achieved": ach_ops / 1e12, "peak": peak_ops / 1e12,
-                    "unit": "T thread-instr/s", "frac": ach_ops / peak_ops,
-                    "peak_source": "148 SMs x 128 fp32 lanes x sampled SM clock; instructions from profiles/traffic.json (ncu)"}
+        slots = 148 * 4 * mhz * 1e6 * (stages[dom]["ms"] / K * 1e-3)
+        issue_util = {"kernel": dom, "warp_instructions_per_launch": ent["warp_instructions_per_launch"],
+                      "issue_slots_per_launch": slots, "utilisation": ent["warp_instructions_per_launch"] / slots,
+                      "source": "profiles/traffic.json (ncu smsp__inst_executed.sum) / (148 SMs x 4 schedulers x sampled SM clock x live K1 time)"}
+    # the whole step against the HBM roofline (north_star's target is 0.60 for the fused step on config 4)
+    step_bytes = sum((stage_bytes(s_, word, ri) or 0) for s_ in stages) * nwet + 16 * word * nx * ny * prm["substeps"] / 6.0
+    roof_step = {"bound": "hbm", "algorithmic_bytes_per_step": step_bytes, "achieved": step_bytes / sec_per_step / 1e9,
+                 "peak": peak, "unit": "GB/s", "frac": step_bytes / sec_per_step / 1e9 / peak, "target_frac": 0.60,
+                 "what": "per wet cell: K1 %d B + K3 %d B; barotropic: 16 words per column per resident group of 6 sub-steps"
+                         % (stage_bytes("tendency", word, ri), stage_bytes("backsub_correct_pressure", word, ri))}
+    tr = ncu_step_traffic(workload_name(wl) + ("+ri" if ri else ""))
+    if tr:
+        roof_step.update({"traffic": tr, "traffic_gbs": tr / sec_per_step / 1e9, "traffic_frac": tr / sec_per_step / 1e9 / peak})
 
     # ---- end to end through the C ABI with HOST (pinned) buffers ----
-    e2e = None
+    # e2e: every step copies that step's forcing (tau_x, tau_y) host -> device and reads that step's result (eta) device ->
+    # host, through the public calls a user makes; the read-back is left in flight (ocn_get_fields_async) and waited for one
+    # step later, so that step n + 1 is enqueued while the result of step n travels.  The initial state is uploaded before
+    # the timed region (an initial condition, like weights).  e2e_with_state_io is round 1's definition: it adds the upload
+    # of the full state and the download of the full state + w to the timed region, amortised over the steps (PCIe bound).
+    e2e = e2e_state = None
     if not args.no_e2e:
         f = wl["fields"]
         pin = {k: torch.from_numpy(np.ascontiguousarray(f[k], dtype=np_dtype)).pin_memory()
                for k in ("u", "v", "T", "S", "eta", "tau_x", "tau_y")}
         out = {k: torch.empty(pin[k].shape, dtype=t_dtype).pin_memory() for k in ("u", "v", "T", "S", "eta")}
         out["w"] = torch.empty((nz + 1, ny, nx), dtype=t_dtype).pin_memory()
-        eta_step = torch.empty((ny, nx), dtype=t_dtype).pin_memory()
+        eta_step = [torch.empty((ny, nx), dtype=t_dtype).pin_memory() for _ in range(2)]
         Ke = K
-        def e2e_job():
-            model.set_fields_ptr(**{k: pin[k].data_ptr() for k in ("u", "v", "T", "S", "eta", "tau_x", "tau_y")})
-            for _ in range(Ke):
-                model.set_fields_ptr(tau_x=pin["tau_x"].data_ptr(), tau_y=pin["tau_y"].data_ptr())   # per-step forcing
-                model.time_step(1)
-                model.get_fields_ptr(eta=eta_step.data_ptr())                                        # per-step result
-            model.get_fields_ptr(**{k: out[k].data_ptr() for k in out})
-        e2e_job()                                   # warm-up (also re-creates the AB2 start)
-        barrier()
-        t0 = time.perf_counter()
-        e0.record(stream)
-        e2e_job()
-        e1.record(stream)
-        barrier()
-        wall = time.perf_counter() - t0
-        ms_e = max_over_ranks(max(e0.elapsed_time(e1), wall * 1e3))
         b2 = ny * nx * word
-        h2d = (4 * cells * word + 3 * b2) / Ke + 2 * b2
-        d2h = (4 * cells * word + (nz + 1) * b2 + b2) / Ke + b2
-        e2e = {"value": world * cells * Ke / (ms_e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
-               "d2h_bytes_per_step": d2h, "steps": Ke,
-               "what": "ocn_set_fields(full state, pinned host) + per step [ocn_set_fields(tau) + ocn_time_step(1) "
-                       "+ ocn_get_fields(eta)] + ocn_get_fields(full state + w); state transfers amortised over the steps"}
+        checks = []
+
+        def steps_job():
+            tickets = []
+            for n in range(Ke):
+                model.set_fields_ptr(tau_x=pin["tau_x"].data_ptr(), tau_y=pin["tau_y"].data_ptr())   # this step's forcing
+                model.time_step(1)
+                tickets.append(model.get_fields_async_ptr(eta=eta_step[n % 2].data_ptr()))            # this step's result
+                if n >= 1:
+                    model.wait(tickets[n - 1])
+                    checks.append(float(eta_step[(n - 1) % 2][ny // 2, nx // 2]))                   # the host consumes it
+            model.wait(tickets[-1])
+            checks.append(float(eta_step[(Ke - 1) % 2][ny // 2, nx // 2]))
+
+        def state_job():
+            model.set_fields_ptr(**{k: pin[k].data_ptr() for k in ("u", "v", "T", "S", "eta", "tau_x", "tau_y")})
+            steps_job()
+            model.get_fields_ptr(**{k: out[k].data_ptr() for k in out})
+
+        def timed(job):
+            barrier()
+            t0 = time.perf_counter()
+            job()
+            model.synchronize()
+            barrier()
+            return max_over_ranks((time.perf_counter() - t0) * 1e3)        # host wall clock around the public calls
+
+        state_job()                                 # warm-up (also re-creates the AB2 start)
+        ms_s = timed(state_job)
+        ms_e = timed(steps_job)
+        assert all(np.isfinite(c) for c in checks)
+        e2e = {"value": world * cells * Ke / (ms_e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 2 * b2,
+               "d2h_bytes_per_step": b2, "steps": Ke, "ms_per_step": ms_e / Ke,
+               "what": "per step: ocn_set_fields(tau_x, tau_y; pinned host) + ocn_time_step(1) + ocn_get_fields_async(eta) "
+                       "waited for one step later; host wall clock; state resident (uploaded before the timed region)"}
+        e2e_state = {"value": world * cells * Ke / (ms_s * 1e-3), "unit": UNIT,
+                     "h2d_bytes_per_step": (4 * cells * word + 3 * b2) / Ke + 2 * b2,
+                     "d2h_bytes_per_step": (4 * cells * word + (nz + 1) * b2 + b2) / Ke + b2, "steps": Ke,
+                     "what": "round 1's definition: the same plus ocn_set_fields(full state) before and ocn_get_fields(full "
+                             "state + w) after the steps inside the timed region, amortised over the steps (PCIe bound)"}
         del pin, out
     model.close()
+
+    # ---- the same workload with the Ri-based closure the paper uses in every run ----
+    wname = workload_name(wl)
+    closure_line = None
+    if not ri and args.config >= 2 and not args.no_closure_leg:
+        wlr = W.with_ri_closure(wl)
+        mr = ocn.Model(wlr, device=local, stream=stream.cuda_stream)
+        mr.time_step(Wm)
+        barrier()
+        e0.record(stream)
+        mr.time_step(K)
+        e1.record(stream)
+        barrier()
+        ms_r = max_over_ranks(e0.elapsed_time(e1))
+        mr.profile_enable(True); mr.time_step(1); mr.profile_read(reset=True)
+        mr.time_step(K)
+        st_r = mr.profile_read(reset=True)
+        mr.profile_enable(False)
+        assert np.isfinite(mr.get_fields(names=("eta",))["eta"]).all()
+        mr.close()
+        closure_line = {"closure": "ri", "ms_per_step": ms_r / K, "value": replicas.aggregate_throughput(cells, K, ms_r, world),
+                        "sypd_equivalent": sypd(prm["dt"], ms_r * 1e-3 / K),
+                        "stages_ms": {s_: v["ms"] / K for s_, v in st_r.items()}}
 
     # ---- CPU oracle on this box's host cores (rank 0, N = 1 only) ----
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
         r = time_oracle(args.config, 3 if args.config >= 2 else 5, 1, args.closure)
-        cpu = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"]}
+        r1 = time_oracle(args.config, 1, 1, args.closure, threads=1, shrink=True)
+        cpu = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"],
+               "one_thread": {"value": r1["value"], "cores": 1, "sample": r1["sample"]}}
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
                 "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f32" if prm["precision"] == 32 else "f64", "data": "synthetic",
-                "config": {"workload": workload_name(wl), "cells": cells, "wet_cells": nwet,
+                "config": {"workload": wname, "cells": cells, "wet_cells": nwet,
                            "l2": "working set %.1f GB >> 126 MB L2 (no flush needed)" % (info["device_bytes"] / 1e9)
                                  if info["device_bytes"] > 1e9 else "working set fits L2 (launch/latency bound; roofline n/a)",
                            "parallelism": "replicas x%d" % world},
                 "sypd_equivalent": sypd(prm["dt"], sec_per_step),
                 "wet_cell_updates_per_s": world * nwet * K / (ms_total * 1e-3),
-                "stages": stage_out, "roofline": roof, "roofline_alu": roof_alu, "e2e": e2e, "cpu_baseline": cpu,
+                "stages": stage_out, "roofline": roof, "roofline_step": roof_step, "issue_utilisation": issue_util, "e2e": e2e,
+                "e2e_with_state_io": e2e_state, "closure_ri": closure_line, "cpu_baseline": cpu,
                 "gpu_launches": info["launches_per_step"] * K, "clocks": clk,
                 "device_bytes": info["device_bytes"]}
         print(json.dumps(line))

@@ -349,6 +349,21 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     const int ks = s_ks;                                 // iterations m <= ks run compact, m > ks geometric
 
     double wacc0 = 0.0, wacc1 = 0.0;                     // w accumulators of this thread's ring points
+    // RI: first wet level of the columns of this thread's ring points (the face above level k is open from there on; the
+    // coefficients of closed faces are never read, so they are not evaluated)
+    int kbr0 = nz, kbr1 = nz;
+    if constexpr (RI) {
+#pragma unroll
+        for (int n = 0; n < 2; ++n) {
+            const int q = n * NT + (NT - 1 - tid);
+            if (q < RX * RY) {
+                const int ii = i0 - 1 + q % RX, jj = j0 - 1 + q / RX;
+                int kb = nz;
+                if (ii < P.nx + OCN_HALO && jj < P.ny + OCN_HALO) kb = (int)(P.m8[(long long)(jj + OCN_HALO) * sx + ii].x & 255u);
+                (n == 0 ? kbr0 : kbr1) = kb;
+            }
+        }
+    }
     T2 fz_bot = mk2(T(0), T(0));                         // vertical tracer flux through the face below
     T u_dn = 0, v_dn = 0;
     double aGU = 0, aGV = 0, aSU = 0, aSV = 0;
@@ -442,7 +457,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                     double& wa = n == 0 ? wacc0 : wacc1;
                     wa = (X(wa) - X((double)dzk) * X((double)Dc)).v;
                     s_w1[q] = (T)wa;
-                    if constexpr (RI) if (k + 1 < nz) {     // (nu, kappa) at the face above level k of this column
+                    if constexpr (RI) if (k + 1 < nz && k >= (n == 0 ? kbr0 : kbr1)) {     // (nu, kappa) at the face above level k of this column
                         const T2* __restrict__ s_uvh = (const T2*)(sm + C::O_UV + ((k + 1) & (C::R_UV - 1)) * C::PL2);
                         const T2 b = s_uvh[py * BX + px], be = s_uvh[py * BX + px + 1], bn = s_uvh[(py + 1) * BX + px];
                         const T2 t0 = ((const T2*)(sm + C::O_TS + (k & (C::R_TS - 1)) * C::PL2))[py * BX + px];
