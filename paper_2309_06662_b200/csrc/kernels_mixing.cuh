@@ -52,6 +52,37 @@ __device__ __forceinline__ typename Pair<T>::type ri_face(const DevP<T>& P, int 
     }
 }
 
+// The fp32 form with its constants converted once (K1 evaluates it on every ring point of every level): same arithmetic as
+// the fp32 branch of ri_face; rdzc = 1 / dzc_k from the caller's table.
+struct RiConst {
+    float g, alpha, beta, c, nu0, kconv, rn2c, s2min, nuz, kapz, ha2;
+    int eos;
+    template <class T>
+    __device__ __forceinline__ void init(const DevP<T>& P) {
+        g = (float)P.g; alpha = (float)P.alpha; beta = (float)P.beta_s; c = (float)P.ri_c; nu0 = (float)P.ri_nu0;
+        kconv = (float)P.ri_kconv; rn2c = (float)(1.0 / P.ri_n2c); s2min = (float)P.ri_s2min; nuz = (float)P.nu_z_d;
+        kapz = (float)P.kappa_z_d; ha2 = (float)P.ha2_d; eos = P.eos;
+    }
+};
+__device__ __forceinline__ float2 ri_face_f32(const RiConst& R, const double* __restrict__ ath, int k, float rdzc, float t1, float s1,
+                                              float t0, float s0, float duw, float due, float dvs, float dvn) {
+    const float dT = t1 - t0, dS = s1 - s0;
+    float db;
+    if (R.eos == 1) {
+        const float a1 = (float)ath[k], a0 = (float)ath[k - 1];
+        db = a1 * dT + (a1 - a0) * t0 + R.ha2 * dT * (t1 + t0) - R.beta * dS;
+    } else {
+        db = R.alpha * dT - R.beta * dS;
+    }
+    const float N2 = R.g * db * rdzc;
+    const float S2 = 0.5f * ((duw * duw + due * due) + (dvs * dvs + dvn * dvn)) * rdzc * rdzc;
+    const float Ri = __fdividef(fmaxf(N2, 0.f), S2 + R.s2min);
+    const float f = __fdividef(1.0f, 1.0f + R.c * Ri);
+    const float conv = R.kconv * fminf(1.0f, fmaxf(-N2, 0.f) * R.rn2c);
+    const float g2 = R.nu0 * f * f;
+    return make_float2(R.nuz + g2 + conv, R.kapz + g2 * f + conv);
+}
+
 // ---------------------------------------------------------------------------------------------
 // One row of the Thomas elimination with per-face diffusivities (DESIGN.md §3.8 step 4 with dt*kappa per face, §3.12),
 // bottom-up in the order the equations are written:

@@ -100,7 +100,8 @@ struct Tile {
     static constexpr int O_NC = O_FS + rup128(NF * 8);                          // uint16[256]: active cells at level k
     static constexpr int O_NF = O_NC + 512;                                     // uint16[256]: active faces at level k
     static constexpr int O_DZ = O_NF + 512;                                     // T[256] dz, T[256] 1 / dz
-    static constexpr int O_XP = O_DZ + 2 * 256 * (int)sizeof(T);                 // double[256][4]: column state in transit at the switch of ownership
+    static constexpr int O_DZC = O_DZ + 2 * 256 * (int)sizeof(T);               // RI: T[256] dzc, T[256] 1 / dzc
+    static constexpr int O_XP = O_DZC + (RI ? 2 * 256 * (int)sizeof(T) : 0);                 // double[256][4]: column state in transit at the switch of ownership
     static constexpr int O_BAR = O_XP + 256 * 4 * 8;
     static constexpr int SMEM = O_BAR + 128 + 128;                              // + alignment slack
 };
@@ -135,6 +136,10 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
     T* const s_AzF = s_rdxF + (BY + 1);
     T* const s_dz = (T*)(sm + C::O_DZ);
     T* const s_rdz = s_dz + 256;
+    T* const s_dzc = (T*)(sm + C::O_DZC);                // RI only
+    T* const s_rdzc = s_dzc + 256;
+    RiConst RC;
+    if constexpr (RI) RC.init(P);
     uint64_t* const bars = (uint64_t*)(sm + C::O_BAR);
     int& s_kmin = *(int*)(sm + C::O_BAR + 64);
     int& s_ks = *(int*)(sm + C::O_BAR + 68);
@@ -283,7 +288,10 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             s_AzC[q] = P.AzC[r]; s_fF[q] = P.fF[r]; s_rdxF[q] = P.rdxF[r]; s_AzF[q] = P.AzF[r];
         }
     }
-    for (int q = tid; q < nz; q += NT) { s_dz[q] = P.dz[q]; s_rdz[q] = P.rdz[q]; }
+    for (int q = tid; q < nz; q += NT) {
+        s_dz[q] = P.dz[q]; s_rdz[q] = P.rdz[q];
+        if constexpr (RI) { s_dzc[q] = q > 0 ? P.dzc[q] : T(1); s_rdzc[q] = q > 0 ? P.rdzc[q] : T(1); }
+    }
     if (tid == 0) {
 #pragma unroll
         for (int b = 0; b < C::NB; ++b) mbar_init(&bars[b], 1);
@@ -462,9 +470,12 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                         const T2 b = s_uvh[py * BX + px], be = s_uvh[py * BX + px + 1], bn = s_uvh[(py + 1) * BX + px];
                         const T2 t0 = ((const T2*)(sm + C::O_TS + (k & (C::R_TS - 1)) * C::PL2))[py * BX + px];
                         const T2 t1 = ((const T2*)(sm + C::O_TS + ((k + 1) & (C::R_TS - 1)) * C::PL2))[py * BX + px];
-                        ((T2*)(sm + C::O_NK + ((k + 1) & 1) * C::KDB))[q] =
-                            ri_face(P, k + 1, t1.x, t1.y, t0.x, t0.y, (X(b.x) - X(a.x)).v, (X(be.x) - X(ae.x)).v,
-                                    (X(b.y) - X(a.y)).v, (X(bn.y) - X(an.y)).v);
+                        T2* const s_nkw = (T2*)(sm + C::O_NK + ((k + 1) & 1) * C::KDB);
+                        if constexpr (sizeof(T) == 4)
+                            s_nkw[q] = ri_face_f32(RC, P.ath_d, k + 1, s_rdzc[k + 1], t1.x, t1.y, t0.x, t0.y, b.x - a.x, be.x - ae.x, b.y - a.y, bn.y - an.y);
+                        else
+                            s_nkw[q] = ri_face(P, k + 1, t1.x, t1.y, t0.x, t0.y, (X(b.x) - X(a.x)).v, (X(be.x) - X(ae.x)).v,
+                                               (X(b.y) - X(a.y)).v, (X(bn.y) - X(an.y)).v);
                     }
                 }
             }
@@ -515,8 +526,8 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             T dzc_lo = T(1), dzc_hi = T(1), rc_lo = T(1), rc_hi = T(1);
             const T2* __restrict__ s_nk1 = nullptr;
             if constexpr (RI) {
-                if (k > 0) { dzc_lo = P.dzc[k]; rc_lo = P.rdzc[k]; }
-                if (has_hi) { dzc_hi = P.dzc[k + 1]; rc_hi = P.rdzc[k + 1]; }
+                dzc_lo = s_dzc[k]; rc_lo = s_rdzc[k];
+                if (has_hi) { dzc_hi = s_dzc[k + 1]; rc_hi = s_rdzc[k + 1]; }
                 s_nk1 = (const T2*)(sm + C::O_NK + ((k + 1) & 1) * C::KDB);
             }
             // ---------- tracer half ----------
