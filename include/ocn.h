@@ -181,6 +181,11 @@ const char* ocn_stage_name(int stage);
  * (default K1_GEO_THR of kernels_tile.cuh; 0 = always geometric, > 256 = never).  OCN_EINVAL for an unknown key. */
 ocn_status ocn_tune(ocn_model* model, const char* key, double value);
 
+/* Self-test of the fp64 path's three-instruction division (reciprocal + Markstein correction, csrc/common.cuh) against the
+ * correctly rounded __ddiv_rn on n pseudo-random operand pairs (a quarter of them within a few ulps of a power of two, an
+ * eighth with the divisor 6): *mismatches must come back 0.  Runs on `device`, synchronous. */
+ocn_status ocn_selftest_division(int device, unsigned long long n, unsigned long long seed, unsigned long long* mismatches);
+
 /* Debug / parity hooks (HOST double buffers, NULL = skip): the AB2 history G^{n-1} of each
  * prognostic field (nz*ny*nx each) and the barotropic transports U, V (ny*nx). */
 ocn_status ocn_get_debug(ocn_model* model, double* Gu, double* Gv, double* GT, double* GS,

@@ -90,12 +90,23 @@ __device__ __forceinline__ T ldg(const T* p) { return __ldg(p); }
 // Arithmetic whose rounding order is fixed (no FMA contraction) in fp64, so that the tracer /
 // pressure column passes reproduce the rounding sequence of the discrete equations as written
 // (DESIGN.md §6.5); fp32 lets the compiler contract and divides by multiplying with rm.
+// Correctly rounded fp64 quotient from a correctly rounded reciprocal rb = RN(1 / b) (Markstein's correction: q = RN(a rb),
+// r = a - q b exactly by FMA, RN(q + r rb) = RN(a / b) when nothing under- or overflows): three instructions where
+// __ddiv_rn needs about twenty-five.  The reciprocals are the host's fp64 tables (1.0 / x), compile-time constants, or
+// __drcp_rn.  ocn_selftest_division compares it with __ddiv_rn on random and adversarial operands (tests/test_gpu_parity.py).
+__device__ __forceinline__ double ddiv_m(double a, double b, double rb) {
+    const double q = __dmul_rn(a, rb);
+    return __fma_rn(__fma_rn(-q, b, a), rb, q);
+}
+__device__ __forceinline__ double xrcp(double b, double) { return __drcp_rn(b); }
+__device__ __forceinline__ float xrcp(float, float approx) { return approx; }
+
 template <class T> struct Ex;
 template <> struct Ex<double> {
     static __device__ __forceinline__ double mul(double a, double b) { return __dmul_rn(a, b); }
     static __device__ __forceinline__ double add(double a, double b) { return __dadd_rn(a, b); }
     static __device__ __forceinline__ double sub(double a, double b) { return __dsub_rn(a, b); }
-    static __device__ __forceinline__ double div(double a, double m, double) { return __ddiv_rn(a, m); }
+    static __device__ __forceinline__ double div(double a, double m, double) { return ddiv_m(a, m, __drcp_rn(m)); }
 };
 template <> struct Ex<float> {
     static __device__ __forceinline__ float mul(float a, float b) { return a * b; }
@@ -142,14 +153,15 @@ template <class T> struct Xv { T v; __device__ __forceinline__ explicit Xv(T x) 
 __device__ __forceinline__ Xv<double> operator*(Xv<double> a, Xv<double> b) { return Xv<double>(__dmul_rn(a.v, b.v)); }
 __device__ __forceinline__ Xv<double> operator+(Xv<double> a, Xv<double> b) { return Xv<double>(__dadd_rn(a.v, b.v)); }
 __device__ __forceinline__ Xv<double> operator-(Xv<double> a, Xv<double> b) { return Xv<double>(__dsub_rn(a.v, b.v)); }
-__device__ __forceinline__ Xv<double> operator/(Xv<double> a, Xv<double> b) { return Xv<double>(__ddiv_rn(a.v, b.v)); }
+__device__ __forceinline__ Xv<double> operator/(Xv<double> a, Xv<double> b) { return Xv<double>(ddiv_m(a.v, b.v, __drcp_rn(b.v))); }
 __device__ __forceinline__ Xv<double> operator-(Xv<double> a) { return Xv<double>(-a.v); }
 __device__ __forceinline__ Xv<float> operator*(Xv<float> a, Xv<float> b) { return Xv<float>(a.v * b.v); }
 __device__ __forceinline__ Xv<float> operator+(Xv<float> a, Xv<float> b) { return Xv<float>(a.v + b.v); }
 __device__ __forceinline__ Xv<float> operator-(Xv<float> a, Xv<float> b) { return Xv<float>(a.v - b.v); }
 __device__ __forceinline__ Xv<float> operator/(Xv<float> a, Xv<float> b) { return Xv<float>(a.v / b.v); }
 __device__ __forceinline__ Xv<float> operator-(Xv<float> a) { return Xv<float>(-a.v); }
-__device__ __forceinline__ Xv<double> xdiv(Xv<double> a, double b, double) { return Xv<double>(__ddiv_rn(a.v, b)); }
+// rb MUST be RN(1 / b): a host table entry or xrcp(b, .)
+__device__ __forceinline__ Xv<double> xdiv(Xv<double> a, double b, double rb) { return Xv<double>(ddiv_m(a.v, b, rb)); }
 __device__ __forceinline__ Xv<float> xdiv(Xv<float> a, float, float rb) { return Xv<float>(a.v * rb); }
 template <class T> __device__ __forceinline__ Xv<T> X(T v) { return Xv<T>(v); }
 
@@ -162,9 +174,10 @@ __device__ __forceinline__ double weno_face_exact(double a, double b, double c, 
     const V qm2(pos ? a : f), qm1(pos ? b : e), q0(pos ? c : d), q1(pos ? d : c), q2(pos ? e : b);
     const V eps(1e-6), two(2.0);
     if (order >= 3) {
-        const V p0 = (two * qm2 - V(7.0) * qm1 + V(11.0) * q0) / V(6.0);
-        const V p1 = (-qm1 + V(5.0) * q0 + two * q1) / V(6.0);
-        const V p2 = (two * q0 + V(5.0) * q1 - q2) / V(6.0);
+        // x / 6.0 with the compile-time reciprocal (correctly rounded, see ddiv_m)
+        const V p0(ddiv_m((two * qm2 - V(7.0) * qm1 + V(11.0) * q0).v, 6.0, 1.0 / 6.0));
+        const V p1(ddiv_m((-qm1 + V(5.0) * q0 + two * q1).v, 6.0, 1.0 / 6.0));
+        const V p2(ddiv_m((two * q0 + V(5.0) * q1 - q2).v, 6.0, 1.0 / 6.0));
         const V c13(13.0 / 12.0), c4(0.25);
         const V b0 = c13 * (qm2 - two * qm1 + q0) * (qm2 - two * qm1 + q0) + c4 * (qm2 - V(4.0) * qm1 + V(3.0) * q0) * (qm2 - V(4.0) * qm1 + V(3.0) * q0);
         const V b1 = c13 * (qm1 - two * q0 + q1) * (qm1 - two * q0 + q1) + c4 * (qm1 - q1) * (qm1 - q1);
@@ -179,7 +192,7 @@ __device__ __forceinline__ double weno_face_exact(double a, double b, double c, 
         return ((a0 * p0 + a1 * p1 + a2 * p2) / (a0 + a1 + a2)).v;
     }
     if (order == 2) {
-        const V p0 = (-qm1 + V(3.0) * q0) / two, p1 = (q0 + q1) / two;
+        const V p0 = (-qm1 + V(3.0) * q0) * V(0.5), p1 = (q0 + q1) * V(0.5);      // x / 2 is exact
         const V b0 = (q0 - qm1) * (q0 - qm1), b1 = (q1 - q0) * (q1 - q0);
         if (WZ) {
             const V tau(fabs((b0 - b1).v)), one(1.0);

@@ -394,6 +394,34 @@ __global__ void __launch_bounds__(128) k_init_transport(const DevP<T> P) {
 }
 
 // ---------------------------------------------------------------------------------------------
+// Self-test of ddiv_m (common.cuh): counts operand pairs for which the three-instruction quotient differs from __ddiv_rn.
+// Operands: counter-based pseudo-random mantissas and exponents in the range the model's quantities live in, every fourth
+// pair with mantissas within a few ulps of 1 or 2 (the hard cases of reciprocal-based division), every eighth with b = 6.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned long long mix64(unsigned long long z) {
+    z += 0x9e3779b97f4a7c15ull; z = (z ^ (z >> 30)) * 0xbf58476d1ce4e5b9ull; z = (z ^ (z >> 27)) * 0x94d049bb133111ebull;
+    return z ^ (z >> 31);
+}
+__global__ void k_selftest_division(unsigned long long n, unsigned long long seed, unsigned long long* bad) {
+    unsigned long long local = 0;
+    for (unsigned long long q = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; q < n; q += (unsigned long long)gridDim.x * blockDim.x) {
+        const unsigned long long ra = mix64(seed + 2 * q), rb = mix64(seed + 2 * q + 1);
+        unsigned long long ma = ra & 0xfffffffffffffull, mb = rb & 0xfffffffffffffull;
+        if ((q & 3) == 1) { ma = (ra >> 52 & 1) ? (ma & 7) : (0xfffffffffffffull - (ma & 7)); }
+        if ((q & 3) == 2) { mb = (rb >> 52 & 1) ? (mb & 7) : (0xfffffffffffffull - (mb & 7)); }
+        const int ea = 1023 + (int)((ra >> 53) % 121) - 60, eb = 1023 + (int)((rb >> 53) % 121) - 60;     // 2^-60 .. 2^60
+        double a = __longlong_as_double((long long)(((unsigned long long)ea << 52) | ma | ((ra >> 63) << 63)));
+        double b = __longlong_as_double((long long)(((unsigned long long)eb << 52) | mb));
+        if ((q & 7) == 7) b = 6.0;
+        if ((q & 1023) == 0) a = 0.0;
+        const double want = __ddiv_rn(a, b);
+        const double got = (q & 7) == 7 ? ddiv_m(a, 6.0, 1.0 / 6.0) : ddiv_m(a, b, __drcp_rn(b));
+        local += (want != got);
+    }
+    if (local) atomicAdd(bad, local);
+}
+
+// ---------------------------------------------------------------------------------------------
 // scatter (contiguous interior -> halo'd plane layout, masked) and gather (back, land = 0)
 // st = element stride of the device array (2 = one member of a pair array, base already offset)
 // kind: 0 u, 1 v, 2 T (offset Toff), 3 S (offset Soff), 4 eta, 5 plain 2-D, 6 w (nz+1 levels, gather only),

@@ -552,7 +552,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 const T2 fw = s_flux[cy * RX + cx], fe = s_flux[cy * RX + cx + 1];
                 const T2 fs = s_flux[C::NFX + cy * TX + cx], fn = s_flux[C::NFX + (cy + 1) * TX + cx];
                 const T2 tsc = ((const T2*)(sm + C::O_TS + (k & (C::R_TS - 1)) * C::PL2))[bo];
-                const T vol = (X(AzCj) * X(dzk)).v, rvol = rAzCj * rdzk;
+                const T vol = (X(AzCj) * X(dzk)).v, rvol = xrcp(vol, rAzCj * rdzk);
                 T GT, GS;
                 if constexpr (sizeof(T) == 8) {    // the flux divergence summed in the order of DESIGN.md §3.7
                     GT = xdiv(-(X(fe.x) - X(fw.x) + X(fn.x) - X(fs.x) + X(fz_top.x) - X(fz_bot.x)), vol, rvol).v;
@@ -617,9 +617,10 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 const Xv<T> dlo((k >= 1 && k - 1 >= tx1) ? (X(u_c) - X(u_dn)).v : T(0));
                 const Xv<T> dhi(has_hi ? (X(u_up) - X(u_c)).v : T(0));
                 const Xv<T> Whi = half * X(AzCj) * (X(s_w1[qo - 1]) + X(w_c1)), Wlo = half * X(AzCj) * (X(s_w0[qo - 1]) + X(w_c0));
-                const Xv<T> Au = xdiv(half * (Whi * dhi + Wlo * dlo), vold, rAzCj * rdzk);
+                const Xv<T> Au = xdiv(half * (Whi * dhi + Wlo * dlo), vold, xrcp(vold, rAzCj * rdzk));
                 const Xv<T> Vu = nuh * (xdiv(X(kdc.y) - X(kdw.y), dxCj, rdxCj) - xdiv(X(z01) - X(z00), dy, rdy));
-                const Xv<T> tau((k == nz - 1) ? xdiv(X(P.taux[XU.c]), (X(P.rho0) * X(dzk)).v, P.rrho0 * rdzk).v : T(0));
+                const T rhodz = (X(P.rho0) * X(dzk)).v;
+                const Xv<T> tau((k == nz - 1) ? xdiv(X(P.taux[XU.c]), rhodz, xrcp(rhodz, P.rrho0 * rdzk)).v : T(0));
                 T Gu = (X(zt) * X(vhat) + Cu - dK - dP - Au + Vu + tau).v;
                 if constexpr (DRAG) {             // bottom drag on the lowest open level of the column
                     const Xv<T> drag(k == tx1 ? xdiv((X(P.drag_r) + X(P.drag_cd) * X((T)sqrt((X(u_c) * X(u_c) + X(vhat) * X(vhat)).v))) * X(u_c), dzk, rdzk).v : T(0));
@@ -673,9 +674,11 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 const Xv<T> dhi(has_hi ? (X(v_up) - X(v_c)).v : T(0));
                 const Xv<T> Whi = half * (X(AzCs) * X(s_w1[qo - RX]) + X(AzCj) * X(w_c1));
                 const Xv<T> Wlo = half * (X(AzCs) * X(s_w0[qo - RX]) + X(AzCj) * X(w_c0));
-                const Xv<T> Av = xdiv(half * (Whi * dhi + Wlo * dlo), (X(AzFj) * X(dzk)).v, rAzFj * rdzk);
+                const T volf = (X(AzFj) * X(dzk)).v;
+                const Xv<T> Av = xdiv(half * (Whi * dhi + Wlo * dlo), volf, xrcp(volf, rAzFj * rdzk));
                 const Xv<T> Vv = nuh * (xdiv(X(kdc.y) - X(kds.y), dy, rdy) + xdiv(X(z10) - X(z00), dxFj, rdxFj));
-                const Xv<T> tau((k == nz - 1) ? xdiv(X(P.tauy[XV.c]), (X(P.rho0) * X(dzk)).v, P.rrho0 * rdzk).v : T(0));
+                const T rhodz = (X(P.rho0) * X(dzk)).v;
+                const Xv<T> tau((k == nz - 1) ? xdiv(X(P.tauy[XV.c]), rhodz, xrcp(rhodz, P.rrho0 * rdzk)).v : T(0));
                 T Gv = (-X(zt) * X(uhat) - Cv - dK - dP - Av + Vv + tau).v;
                 if constexpr (DRAG) {
                     const Xv<T> drag(k == ty1 ? xdiv((X(P.drag_r) + X(P.drag_cd) * X((T)sqrt((X(uhat) * X(uhat) + X(v_c) * X(v_c)).v))) * X(v_c), dzk, rdzk).v : T(0));

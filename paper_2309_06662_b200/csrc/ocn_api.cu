@@ -269,7 +269,7 @@ ocn_status build_model(ocn_model* M) {
     P.nu_h = (T)M->d.nu_h; P.kappa_h = (T)M->d.kappa_h; P.dtau = (T)M->dtau;
     // equation of state: per-level thermal expansion alpha (1 - gamma zc[k]) and alpha2 / 2, in the fp64
     // operations the equation is written in
-    P.geo_thr = K1_GEO_THR;
+    P.geo_thr = sizeof(T) == 4 ? K1_GEO_THR : 1 << 20;   // fp64: lane efficiency decides (measured on config 2: 9.0 ms compact, 11.6 geometric)
     P.eos = M->d.eos; P.ha2_d = 0.5 * M->d.eos_alpha2;
     {
         std::vector<double> ath(nz);
@@ -799,6 +799,21 @@ ocn_status ocn_tune(ocn_model* M, const char* key, double value) {
         return fail(OCN_EINVAL, std::string("unknown tuning key: ") + key);
     }
     if (M->graph) { CK(cudaStreamSynchronize(M->stream)); cudaGraphExecDestroy(M->graph); M->graph = nullptr; }   // re-capture with the new arguments
+    return OCN_OK;
+}
+
+ocn_status ocn_selftest_division(int device, unsigned long long n, unsigned long long seed, unsigned long long* mismatches) {
+    if (!mismatches) return fail(OCN_EINVAL, "null argument");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return fail(OCN_ECUDA, "no such CUDA device");
+    ON_DEVICE(device);
+    unsigned long long* d = nullptr;
+    CK(cudaMalloc(&d, 8));
+    CK(cudaMemset(d, 0, 8));
+    ocn::k_selftest_division<<<148 * 8, 256>>>(n, seed, d);
+    CK(cudaGetLastError());
+    CK(cudaMemcpy(mismatches, d, 8, cudaMemcpyDeviceToHost));
+    CK(cudaFree(d));
     return OCN_OK;
 }
 

@@ -46,7 +46,7 @@ class ocn_fields(C.Structure):
 EXPORTS = ["ocn_grid_create", "ocn_grid_destroy", "ocn_model_create", "ocn_model_destroy", "ocn_set_fields",
            "ocn_time_step", "ocn_get_fields", "ocn_synchronize", "ocn_get_masks", "ocn_model_info",
            "ocn_get_debug", "ocn_last_error", "ocn_version", "ocn_profile_enable", "ocn_profile_read",
-           "ocn_stage_name", "ocn_get_mixing", "ocn_get_fields_async", "ocn_wait", "ocn_tune"]
+           "ocn_stage_name", "ocn_get_mixing", "ocn_get_fields_async", "ocn_wait", "ocn_tune", "ocn_selftest_division"]
 NSTAGES = 4
 
 
@@ -71,6 +71,7 @@ def lib():
         L.ocn_get_fields_async.argtypes = [vp, C.POINTER(ocn_fields), C.POINTER(C.c_ulonglong)]
         L.ocn_wait.argtypes = [vp, C.c_ulonglong]
         L.ocn_tune.argtypes = [vp, C.c_char_p, C.c_double]
+        L.ocn_selftest_division.argtypes = [C.c_int, C.c_ulonglong, C.c_ulonglong, C.POINTER(C.c_ulonglong)]
         L.ocn_get_masks.argtypes = [vp] + [vp] * 6
         L.ocn_model_info.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_ulonglong)]
         L.ocn_get_debug.argtypes = [vp] + [vp] * 6
@@ -81,6 +82,13 @@ def lib():
         L.ocn_stage_name.argtypes = [C.c_int]
         _lib = L
     return _lib
+
+
+def selftest_division(n, seed=1, device=0):
+    """ocn_selftest_division: number of operand pairs (of n) on which the fast fp64 quotient differs from __ddiv_rn."""
+    bad = C.c_ulonglong()
+    _check(lib().ocn_selftest_division(int(device), int(n), int(seed), C.byref(bad)))
+    return bad.value
 
 
 def _check(rc):
