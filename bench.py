@@ -345,11 +345,11 @@ def run_ours(args):
                       "issue_slots_per_launch": slots, "utilisation": ent["warp_instructions_per_launch"] / slots,
                       "source": "profiles/traffic.json (ncu smsp__inst_executed.sum) / (148 SMs x 4 schedulers x sampled SM clock x live K1 time)"}
     # the whole step against the HBM roofline (north_star's target is 0.60 for the fused step on config 4)
-    step_bytes = sum((stage_bytes(s_, word, ri) or 0) for s_ in stages) * nwet + 16 * word * nx * ny * prm["substeps"] / 6.0
+    step_bytes = sum((stage_bytes(s_, word, ri) or 0) for s_ in stages) * nwet + 16 * word * nx * ny * (info["launches_per_step"] - 3)
     roof_step = {"bound": "hbm", "algorithmic_bytes_per_step": step_bytes, "achieved": step_bytes / sec_per_step / 1e9,
                  "peak": peak, "unit": "GB/s", "frac": step_bytes / sec_per_step / 1e9 / peak, "target_frac": 0.60,
-                 "what": "per wet cell: K1 %d B + K3 %d B; barotropic: 16 words per column per resident group of 6 sub-steps"
-                         % (stage_bytes("tendency", word, ri), stage_bytes("backsub_correct_pressure", word, ri))}
+                 "what": "per wet cell: K1 %d B + K3 %d B; barotropic: 16 words per column per resident group of sub-steps (%d groups)"
+                         % (stage_bytes("tendency", word, ri), stage_bytes("backsub_correct_pressure", word, ri), info["launches_per_step"] - 3)}
     tr = ncu_step_traffic(workload_name(wl) + ("+ri" if ri else ""))
     if tr:
         roof_step.update({"traffic": tr, "traffic_gbs": tr / sec_per_step / 1e9, "traffic_frac": tr / sec_per_step / 1e9 / peak})

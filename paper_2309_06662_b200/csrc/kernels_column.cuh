@@ -224,6 +224,134 @@ __global__ void __launch_bounds__((BtTile<T, BTX, BTY>::NT)) k_barotropic_tile(c
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// S6, resident form for fp32 models, register strips: as k_barotropic_tile, but a thread owns a strip of
+// four consecutive points of a row of the extended tile and keeps their eta, U, V, the five folded coefficients and the
+// filter sums in REGISTERS for the whole launch.  Shared memory only carries what neighbours need: per sub-step a strip
+// publishes its eta / U / V with three 128-bit stores and reads the U east of it, the eta west of it (32-bit) and the V
+// row north / eta row south of it (128-bit) - 7 shared-memory instructions per four points where the point-wise kernel
+// needs about fifty, which is what bounded it (LSU pipe 74 % busy, profiles/r1_ncu_summary.md).  NS <= H sub-steps per
+// launch on a halo of H that is recomputed redundantly and shrinks one ring per sub-step (PAPER.md:98 on chip).
+// ---------------------------------------------------------------------------------------------
+#define BT_MAXW 12
+template <class T> struct BtWeights { T a[BT_MAXW]; };
+
+template <int BTX, int BTY, int H>
+struct BtStrip {
+    static constexpr int EX = BTX + 2 * H, EY = BTY + 2 * H, SPR = EX / 4, NS = SPR * EY;   // strips per row, strips
+    static_assert(EX % 4 == 0, "extended row must be a whole number of strips");
+    static constexpr int NT = (NS + 31) / 32 * 32;
+    static_assert(NT <= 1024, "one strip per thread");
+    static constexpr int SMEM = 3 * EX * EY * 4 + 2 * (EY + 1) * 4 + 16;
+};
+
+template <int BTX, int BTY, int H>
+__global__ void __launch_bounds__((BtStrip<BTX, BTY, H>::NT), 1)
+k_barotropic_strip(const DevP<float> P, const int cur, const int ns, const int first, const BtWeights<float> W) {
+    typedef BtStrip<BTX, BTY, H> C;
+    constexpr int EX = C::EX, EY = C::EY, SPR = C::SPR;
+    extern __shared__ __align__(16) unsigned char smb[];
+    float* const se = (float*)smb;
+    float* const sU = se + EX * EY;
+    float* const sV = sU + EX * EY;
+    float* const dF = sV + EX * EY;                 // dxF per extended row, EY + 1 entries
+    float* const rAz = dF + (EY + 1);               // 1 / AzC per extended row
+    const int tid = threadIdx.x;
+    const int i0 = blockIdx.x * BTX, j0 = blockIdx.y * BTY;
+    const int nx = P.nx, ny = P.ny, nz = P.nz, sx = P.sx;
+    for (int q = tid; q <= EY; q += C::NT) {
+        int jj = j0 - H + q;
+        if (P.py) { while (jj < 0) jj += ny; while (jj >= ny) jj -= ny; }
+        const int r = min(max(jj, -OCN_HALO), ny + OCN_HALO) + OCN_HALO;
+        dF[q] = P.dxF[r];
+        if (q < EY) rAz[q] = P.rAzC[r];
+    }
+    const bool on = tid < C::NS;
+    const int y = on ? tid / SPR : 0, x0 = on ? 4 * (tid % SPR) : 0;
+    const int qb = y * EX + x0;                     // first point of the strip in the extended tile
+    const float dy = P.dy, dtau = P.dtau, g = P.g, rdy = P.rdy;
+    float e[4], u[4], v[4], ce[4], cu[4], cv[4], gu[4], gv[4], be[4], bU[4], bV[4];
+    int cidx[4];
+    {
+        int jj = j0 - H + y;
+        bool iny = true;
+        if (P.py) { while (jj < 0) jj += ny; while (jj >= ny) jj -= ny; } else iny = jj >= 0 && jj < ny;
+        int rr = min(max(jj, -OCN_HALO), ny + OCN_HALO) + OCN_HALO;
+        const float rdxr = P.rdxC[rr], rAzr = P.rAzC[rr];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const int x = x0 + r;
+            int ii = i0 - H + x;
+            bool in = on && iny;
+            if (P.px) { while (ii < 0) ii += nx; while (ii >= nx) ii -= nx; } else in = in && ii >= 0 && ii < nx;
+            e[r] = u[r] = v[r] = ce[r] = cu[r] = cv[r] = gu[r] = gv[r] = be[r] = bU[r] = bV[r] = 0.f;
+            cidx[r] = -1;
+            if (in) {
+                const int c = (jj + OCN_HALO) * sx + ii;
+                const uint2 m = P.m8[c];
+                const bool wet = (m.x & 255u) < (unsigned)nz, ou = ((m.x >> 8) & 255u) < (unsigned)nz, ov = (m.y & 255u) < (unsigned)nz;
+                if (wet | ou | ov) { e[r] = P.eta[cur][c]; u[r] = P.U[cur][c]; v[r] = P.V[cur][c]; }
+                if (x < EX - 1 && y < EY - 1 && wet) ce[r] = dtau * rAzr;
+                if (x > 0 && ou) { cu[r] = dtau * g * P.Hu[c] * rdxr; gu[r] = dtau * P.GU[c]; }
+                if (y > 0 && ov) { cv[r] = dtau * g * P.Hv[c] * rdy; gv[r] = dtau * P.GV[c]; }
+                const int xi = x - H, yi = y - H;
+                if (xi >= 0 && xi < BTX && yi >= 0 && yi < BTY && i0 + xi < nx && j0 + yi < ny) {
+                    cidx[r] = c;                    // interior points are inside the domain: no wrap happened
+                    if (!first) { be[r] = P.etab[c]; bU[r] = P.Ub[c]; bV[r] = P.Vb[c]; }
+                }
+            }
+        }
+    }
+    if (on) {
+        *(float4*)(sU + qb) = make_float4(u[0], u[1], u[2], u[3]);
+        *(float4*)(sV + qb) = make_float4(v[0], v[1], v[2], v[3]);
+    }
+    __syncthreads();
+    const int qe = min(qb + 4, EX * EY - 1);                    // U east of the strip (rim: ce = 0)
+    const int qn = (y < EY - 1 ? qb + EX : qb);                 // V row north of the strip
+    const int qw = max(qb - 1, 0);                              // eta west of the strip (rim: cu = 0)
+    const int qs = (y > 0 ? qb - EX : qb);                      // eta row south of the strip
+    const float dFs = dF[y], dFn = dF[y + 1];
+    for (int s = 0; s < ns; ++s) {
+        if (on) {
+            const float ue = sU[qe];
+            const float4 vn = *(const float4*)(sV + qn);
+            e[0] = e[0] - ce[0] * (dy * (u[1] - u[0]) + dFn * vn.x - dFs * v[0]);
+            e[1] = e[1] - ce[1] * (dy * (u[2] - u[1]) + dFn * vn.y - dFs * v[1]);
+            e[2] = e[2] - ce[2] * (dy * (u[3] - u[2]) + dFn * vn.z - dFs * v[2]);
+            e[3] = e[3] - ce[3] * (dy * (ue - u[3]) + dFn * vn.w - dFs * v[3]);
+            *(float4*)(se + qb) = make_float4(e[0], e[1], e[2], e[3]);
+        }
+        __syncthreads();
+        if (on) {
+            const float am = W.a[s];
+            const float ew = se[qw];
+            const float4 es = *(const float4*)(se + qs);
+            u[0] = u[0] + (cu[0] * (ew - e[0]) + gu[0]);
+            u[1] = u[1] + (cu[1] * (e[0] - e[1]) + gu[1]);
+            u[2] = u[2] + (cu[2] * (e[1] - e[2]) + gu[2]);
+            u[3] = u[3] + (cu[3] * (e[2] - e[3]) + gu[3]);
+            v[0] = v[0] + (cv[0] * (es.x - e[0]) + gv[0]);
+            v[1] = v[1] + (cv[1] * (es.y - e[1]) + gv[1]);
+            v[2] = v[2] + (cv[2] * (es.z - e[2]) + gv[2]);
+            v[3] = v[3] + (cv[3] * (es.w - e[3]) + gv[3]);
+#pragma unroll
+            for (int r = 0; r < 4; ++r) { be[r] += am * e[r]; bU[r] += am * u[r]; bV[r] += am * v[r]; }
+            *(float4*)(sU + qb) = make_float4(u[0], u[1], u[2], u[3]);
+            *(float4*)(sV + qb) = make_float4(v[0], v[1], v[2], v[3]);
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        if (cidx[r] >= 0) {
+            const int c = cidx[r];
+            P.eta[cur ^ 1][c] = e[r]; P.U[cur ^ 1][c] = u[r]; P.V[cur ^ 1][c] = v[r];
+            P.etab[c] = be[r]; P.Ub[c] = bU[r]; P.Vb[c] = bV[r];
+        }
+    }
+}
+
 // step 7: the filtered values become the barotropic state (buffer 0, with halos)
 template <class T>
 __global__ void __launch_bounds__(256) k_barotropic_finish(const DevP<T> P) {

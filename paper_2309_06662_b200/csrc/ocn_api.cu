@@ -118,7 +118,14 @@ template <> ocn::DevP<float>& params<float>(ocn_model* M) { return M->pf; }
 template <> ocn::DevP<double>& params<double>(ocn_model* M) { return M->pd; }
 
 constexpr int TILE_X = 32, TILE_Y = 8;    // K1 tile (kernels_tile.cuh)
-constexpr int BT_X = 32, BT_Y = 32;       // barotropic tile (kernels_column.cuh)
+constexpr int BT_X = 32, BT_Y = 32;       // barotropic tile of the point-wise kernel (fp64 models; kernels_column.cuh)
+#ifndef BS_X
+#define BS_X 64
+#define BS_Y 28
+#define BS_H 10
+#endif                                    // tile and halo (= sub-steps per launch) of the register-strip kernel (fp32 models);
+                                          // measured on config 4 (M = 40): 64x32/6 1.13 ms, 64x32/8 0.86, 64x28/10 0.855 (4 launches)
+template <class T> constexpr int bt_substeps_per_launch() { return sizeof(T) == 4 ? BS_H : BT_HALO; }
 
 // TMA descriptor of a halo'd 3-D array seen as [levels][rows][inner] scalars
 ocn_status make_tmap(CUtensorMap* tm, bool f64, void* base, unsigned long long inner, unsigned long long rows,
@@ -310,7 +317,7 @@ ocn_status build_model(ocn_model* M) {
         CK(cudaStreamCreateWithFlags(&M->copy_stream, cudaStreamNonBlocking));
         for (auto& e : M->ticket_ev) CK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     }
-    M->launches_per_step = (M->d.substeps + BT_HALO - 1) / BT_HALO + 3;
+    M->launches_per_step = (M->d.substeps + bt_substeps_per_launch<T>() - 1) / bt_substeps_per_launch<T>() + 3;
     // TMA descriptors: box origin (i0 - 4, j0 - 3), so the map starts 4 elements before (row -3, i = 0)
     {
         typedef ocn::Tile<T, TILE_X, TILE_Y> C;
@@ -324,6 +331,8 @@ ocn_status build_model(ocn_model* M) {
             CK(cudaFuncSetAttribute(k1_fused<T>(id & 4, id & 2, id & 1), cudaFuncAttributeMaxDynamicSharedMemorySize, k1_smem<T>(id & 2)));
         CK(cudaFuncSetAttribute(ocn::k_barotropic_tile<T, BT_X, BT_Y>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 ocn::BtTile<T, BT_X, BT_Y>::SMEM));
+        CK(cudaFuncSetAttribute(ocn::k_barotropic_strip<BS_X, BS_Y, BS_H>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                ocn::BtStrip<BS_X, BS_Y, BS_H>::SMEM));
     }
     return OCN_OK;
 }
@@ -382,7 +391,18 @@ ocn_status launch_step(ocn_model* M, bool euler) {
         k1_fused<T>(drag, ri, wz)<<<gt, bt, k1_smem<T>(ri), M->stream>>>(P, c0, c1, M->tm_ts, M->tm_uv, M->tm_p);
     }
     MARK(0, 1);
-    {
+    if constexpr (sizeof(T) == 4) {                // register-strip kernel, BS_H sub-steps per launch
+        typedef ocn::BtStrip<BS_X, BS_Y, BS_H> B;
+        const dim3 gb((g->nx + BS_X - 1) / BS_X, (g->ny + BS_Y - 1) / BS_Y);
+        int cur = 0;
+        for (int m0 = 0; m0 < M->d.substeps; m0 += BS_H) {
+            const int ns = std::min(BS_H, M->d.substeps - m0);
+            ocn::BtWeights<float> W{};
+            for (int q = 0; q < ns; ++q) W.a[q] = (float)M->a_w[m0 + q];
+            ocn::k_barotropic_strip<BS_X, BS_Y, BS_H><<<gb, B::NT, B::SMEM, M->stream>>>(P, cur, ns, m0 == 0 ? 1 : 0, W);
+            cur ^= 1;
+        }
+    } else {
         typedef ocn::BtTile<T, BT_X, BT_Y> B;
         const dim3 gb((g->nx + BT_X - 1) / BT_X, (g->ny + BT_Y - 1) / BT_Y);
         int cur = 0;
@@ -396,7 +416,7 @@ ocn_status launch_step(ocn_model* M, bool euler) {
         }
     }
     ocn::k_barotropic_finish<T><<<grid2(g, b2), b2, 0, M->stream>>>(P);
-    MARK(1, (M->d.substeps + BT_HALO - 1) / BT_HALO + 1);
+    MARK(1, (M->d.substeps + bt_substeps_per_launch<T>() - 1) / bt_substeps_per_launch<T>() + 1);
     MARK(3, 0);                                    // (the closure is evaluated inside K1: stage 3 is empty)
     if (M->d.closure == 1) ocn::k_backsub_correct<T, true><<<grid2(g, bc), bc, 0, M->stream>>>(P);
     else ocn::k_backsub_correct<T, false><<<grid2(g, bc), bc, 0, M->stream>>>(P);

@@ -333,13 +333,15 @@ def test_profiling_path_gives_the_same_bits_and_sane_times():
     a = ocn.Model(wl); a.time_step(4); fa = a.get_fields(); a.close()
     b = ocn.Model(wl); b.profile_enable(True); b.time_step(4)
     prof = b.profile_read()
-    fb = b.get_fields(); b.close()
+    fb = b.get_fields()
     for n in FIELDS:
         assert np.array_equal(fa[n], fb[n]), n                    # graph replay and direct launches agree bit for bit
     assert set(prof) == {"tendency", "barotropic", "backsub_correct_pressure", "vertical_mixing"}
     assert prof["vertical_mixing"]["launches"] == 0                     # closure 0: the stage is empty
-    assert prof["tendency"]["launches"] == 4 and prof["barotropic"]["launches"] == 4 * (30 // 6 + 1)
+    per_step = b.info()["launches_per_step"]                     # K1 + the resident sub-cycle groups + finish + K3
+    assert prof["tendency"]["launches"] == 4 and prof["barotropic"]["launches"] == 4 * (per_step - 2) and per_step - 3 <= 4
     assert all(v["ms"] > 0 for n, v in prof.items() if n != "vertical_mixing")
+    b.close()
 
 
 def test_bad_arguments_on_the_gpu_side():
