@@ -200,7 +200,7 @@ def measured_peak():
 def ncu_entry(workload, kernel):
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            e = json.load(f).get(kernel)
+            e = json.load(f).get(kernel + ("+ri" if "+ri" in workload else ""))
         return e if e and e.get("workload") == workload else None
     except Exception:
         return None
@@ -210,7 +210,7 @@ def ncu_step_traffic(workload):
     """DRAM bytes of one whole step (all kernels) from the committed ncu capture of this workload, if any."""
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            e = json.load(f).get("step")
+            e = json.load(f).get("step" + ("+ri" if "+ri" in workload else ""))
         return float(e["dram_bytes_per_step"]) if e and e.get("workload") == workload else None
     except Exception:
         return None
@@ -222,7 +222,7 @@ def ncu_traffic(workload, kernel):
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
             t = json.load(f)
-        e = t.get(kernel)
+        e = t.get(kernel + ("+ri" if "+ri" in workload else ""))
         if e and e.get("workload") == workload:
             return float(e["dram_bytes_per_launch"])
     except Exception:
@@ -350,7 +350,7 @@ def run_ours(args):
                  "peak": peak, "unit": "GB/s", "frac": step_bytes / sec_per_step / 1e9 / peak, "target_frac": 0.60,
                  "what": "per wet cell: K1 %d B + K3 %d B; barotropic: 16 words per column per resident group of sub-steps (%d groups)"
                          % (stage_bytes("tendency", word, ri), stage_bytes("backsub_correct_pressure", word, ri), info["launches_per_step"] - 3)}
-    tr = ncu_step_traffic(workload_name(wl) + ("+ri" if ri else ""))
+    tr = ncu_step_traffic(workload_name(wl))
     if tr:
         roof_step.update({"traffic": tr, "traffic_gbs": tr / sec_per_step / 1e9, "traffic_frac": tr / sec_per_step / 1e9 / peak})
 

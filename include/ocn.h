@@ -181,6 +181,12 @@ const char* ocn_stage_name(int stage);
  * (default K1_GEO_THR of kernels_tile.cuh; 0 = always geometric, > 256 = never).  OCN_EINVAL for an unknown key. */
 ocn_status ocn_tune(ocn_model* model, const char* key, double value);
 
+/* Diagnostic builds only (nvcc -DOCN_K1_TIMELINE; OCN_EUNSUPPORTED otherwise): SM cycles every warp of the tendency kernel
+ * has spent per phase of its march since the last reset, summed over all CTAs.  cycles: HOST, 64 doubles = [8 warps][8]:
+ * 0 prologue (history loads; includes the wait at the previous block barrier), 1 wait for the TMA planes, 2 phase 1
+ * (zeta, K, D, w), 3 face fluxes, 4 part B, 5 barrier issue, 6 iterations executed, 7 unused. */
+ocn_status ocn_get_timeline(ocn_model* model, double* cycles, int reset);
+
 /* Self-test of the fp64 path's three-instruction division (reciprocal + Markstein correction, csrc/common.cuh) against the
  * correctly rounded __ddiv_rn on n pseudo-random operand pairs (a quarter of them within a few ulps of a power of two, an
  * eighth with the divisor 6): *mismatches must come back 0.  Runs on `device`, synchronous. */

@@ -24,7 +24,8 @@ def build(force=False, verbose=False):
     if not force and os.path.exists(SO) and all(os.path.getmtime(SO) >= os.path.getmtime(s) for s in src):
         return SO
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", SO, os.path.join(CSRC, "ocn_api.cu")]
+    extra = os.environ.get("OCN_NVCC_FLAGS", "").split()        # e.g. -DOCN_K1_TIMELINE for the diagnostic build
+    cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", SO, os.path.join(CSRC, "ocn_api.cu")]
     subprocess.check_call(cmd)
     return SO
 

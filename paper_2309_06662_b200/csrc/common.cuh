@@ -82,6 +82,7 @@ struct DevP {
     double ha2_d;
     // K1: wet cells of a tile-level from which on the tile is marched with geometric ownership
     int geo_thr;
+    unsigned long long* timeline;   // [8 warps][8]: cycles per phase + iterations (filled by OCN_K1_TIMELINE builds only)
 };
 
 template <class T>

@@ -399,6 +399,15 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
 
     // one iteration of the march: parts A(m) and B(m - 1), then ONE block barrier.  GEO selects the ownership (a compile-time
     // tag: the geometric body has one cell descriptor, constant strides and no lists)
+    // OCN_K1_TIMELINE (diagnostic builds only, `OCN_NVCC_FLAGS=-DOCN_K1_TIMELINE python -m paper_2309_06662_b200.build --force`):
+    // every warp accumulates the SM cycles it spends in each phase of an iteration; read with ocn_get_timeline.  Note that
+    // BAR.SYNC does not block at issue: the time a warp waits at the block barrier shows up in the NEXT phase (the prologue).
+#ifdef OCN_K1_TIMELINE
+    long long tl_acc[6] = {0, 0, 0, 0, 0, 0}, tl_last = clock64();
+#define TLA(i) { const long long now_ = clock64(); tl_acc[i] += now_ - tl_last; tl_last = now_; }
+#else
+#define TLA(i)
+#endif
     auto iteration = [&](auto geo_tag, const int m, const Cell& XT, const Cell& XU, const Cell& XV) {
         constexpr bool GEO = decltype(geo_tag)::value;
         const int kB = m - 1;                                 // level of part B (phase 3) in this iteration
@@ -429,7 +438,9 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 if (wetV) piv_v = sizeof(T) == 8 ? P.m_m[kB * nz + XV.t1] : P.rm_m[kB * nz + XV.t1];
             }
         }
+        TLA(0)
         mbar_wait(&bars[(m - kmin) % C::NB], (uint32_t)(((m - kmin) / C::NB) & 1));
+        TLA(1)
 
         if (m < nz) {                                         // ---------------- part A: level k = m ----------------
             const int k = m;
@@ -479,6 +490,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                     }
                 }
             }
+            TLA(2)
             // ================= phase 2: tracer face fluxes, each open face once =================
             const T2* __restrict__ s_ts = (const T2*)(sm + C::O_TS + (k & (C::R_TS - 1)) * C::PL2);
             if constexpr (GEO) {
@@ -510,6 +522,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                 }
             }
         }
+        TLA(3)
         if (anyB) {                                           // ---------------- part B: level k = m - 1 ----------------
             const int k = kB;
             const T dzk = s_dz[k], rdzk = s_rdz[k];
@@ -712,7 +725,9 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             }
             fz_bot = fz_top;
         }
+        TLA(4)
         __syncthreads();                       // planes of level m - 1 are dead: refill the ring
+        TLA(5)
         if (tid == PROD && m + C::DP <= nz) {
             const int g = m + C::DP;
             if (g + 2 < nz) {                  // steady state: one plane of each array (the general form handles the ends)
@@ -758,6 +773,12 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
         cT = make_cell(tid, 0); cU = make_cell(tid, 1); cV = make_cell(tid, 2);
         for (; m <= nz; ++m) iteration(GeoTag{}, m, cT, cU, cV);
     }
+#ifdef OCN_K1_TIMELINE
+    if ((tid & 31) == 0) {
+        for (int q = 0; q < 6; ++q) atomicAdd(&P.timeline[(tid >> 5) * 8 + q], (unsigned long long)tl_acc[q]);
+        atomicAdd(&P.timeline[(tid >> 5) * 8 + 6], (unsigned long long)(nz + 1 - kmin));
+    }
+#endif
     if (cU.incol && cU.t1 < nz) { P.GU[cU.c] = (T)aGU; P.SU[cU.c] = (T)aSU; }     // never-open faces keep their zeros
     if (cV.incol && cV.t1 < nz) { P.GV[cV.c] = (T)aGV; P.SV[cV.c] = (T)aSV; }
 }

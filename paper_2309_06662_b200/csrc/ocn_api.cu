@@ -276,6 +276,7 @@ ocn_status build_model(ocn_model* M) {
     P.nu_h = (T)M->d.nu_h; P.kappa_h = (T)M->d.kappa_h; P.dtau = (T)M->dtau;
     // equation of state: per-level thermal expansion alpha (1 - gamma zc[k]) and alpha2 / 2, in the fp64
     // operations the equation is written in
+    if ((s = dev_alloc(M, 64, &P.timeline, false)) != OCN_OK) return s;
     P.geo_thr = sizeof(T) == 4 ? K1_GEO_THR : 1 << 20;   // fp64: lane efficiency decides (measured on config 2: 9.0 ms compact, 11.6 geometric)
     P.eos = M->d.eos; P.ha2_d = 0.5 * M->d.eos_alpha2;
     {
@@ -835,6 +836,23 @@ ocn_status ocn_selftest_division(int device, unsigned long long n, unsigned long
     CK(cudaMemcpy(mismatches, d, 8, cudaMemcpyDeviceToHost));
     CK(cudaFree(d));
     return OCN_OK;
+}
+
+ocn_status ocn_get_timeline(ocn_model* M, double* cycles, int reset) {
+    if (!M || !cycles) return fail(OCN_EINVAL, "null argument");
+#ifndef OCN_K1_TIMELINE
+    (void)reset;
+    return fail(OCN_EUNSUPPORTED, "libocn was built without -DOCN_K1_TIMELINE");
+#else
+    ON_DEVICE(M->d.device);
+    unsigned long long* d = M->prec == 32 ? M->pf.timeline : M->pd.timeline;
+    unsigned long long h[64];
+    CK(cudaStreamSynchronize(M->stream));
+    CK(cudaMemcpy(h, d, sizeof(h), cudaMemcpyDeviceToHost));
+    if (reset) CK(cudaMemset(d, 0, sizeof(h)));
+    for (int q = 0; q < 64; ++q) cycles[q] = (double)h[q];
+    return OCN_OK;
+#endif
 }
 
 const char* ocn_stage_name(int stage) {

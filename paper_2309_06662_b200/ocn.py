@@ -46,7 +46,7 @@ class ocn_fields(C.Structure):
 EXPORTS = ["ocn_grid_create", "ocn_grid_destroy", "ocn_model_create", "ocn_model_destroy", "ocn_set_fields",
            "ocn_time_step", "ocn_get_fields", "ocn_synchronize", "ocn_get_masks", "ocn_model_info",
            "ocn_get_debug", "ocn_last_error", "ocn_version", "ocn_profile_enable", "ocn_profile_read",
-           "ocn_stage_name", "ocn_get_mixing", "ocn_get_fields_async", "ocn_wait", "ocn_tune", "ocn_selftest_division"]
+           "ocn_stage_name", "ocn_get_mixing", "ocn_get_fields_async", "ocn_wait", "ocn_tune", "ocn_selftest_division", "ocn_get_timeline"]
 NSTAGES = 4
 
 
@@ -71,6 +71,7 @@ def lib():
         L.ocn_get_fields_async.argtypes = [vp, C.POINTER(ocn_fields), C.POINTER(C.c_ulonglong)]
         L.ocn_wait.argtypes = [vp, C.c_ulonglong]
         L.ocn_tune.argtypes = [vp, C.c_char_p, C.c_double]
+        L.ocn_get_timeline.argtypes = [vp, C.POINTER(C.c_double), C.c_int]
         L.ocn_selftest_division.argtypes = [C.c_int, C.c_ulonglong, C.c_ulonglong, C.POINTER(C.c_ulonglong)]
         L.ocn_get_masks.argtypes = [vp] + [vp] * 6
         L.ocn_model_info.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_ulonglong)]
@@ -182,6 +183,13 @@ class Model:
 
     def tune(self, key, value):
         _check(lib().ocn_tune(self.h, key.encode(), float(value)))
+
+    def timeline(self, reset=True):
+        """ocn_get_timeline (diagnostic builds): {phase: cycles per iteration, per warp}."""
+        buf = (C.c_double * 64)()
+        _check(lib().ocn_get_timeline(self.h, buf, int(bool(reset))))
+        names = ("prologue+barrier_wait", "tma_wait", "phase1", "faces", "partB", "barrier_issue")
+        return [{n: buf[w * 8 + q] / max(buf[w * 8 + 6], 1.0) for q, n in enumerate(names)} for w in range(8)]
 
     def time_step(self, n=1):
         _check(lib().ocn_time_step(self.h, int(n)))
