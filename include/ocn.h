@@ -201,6 +201,18 @@ ocn_status ocn_get_debug(ocn_model* model, double* Gu, double* Gv, double* GT, d
  * buffers nz*ny*nx, value at the bottom face of tracer cell (k, j, i), 0 on closed faces and at k = 0; NULL = skip. */
 ocn_status ocn_get_mixing(ocn_model* model, double* nu, double* kappa);
 
+/* The same diagnostic for callers that must not allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): calls no cudaMalloc, cudaFree or allocating library routine.  ocn_get_mixing keeps the
+ * halo'd (nu, kappa) pair array in a buffer it cudaMallocs on first use; here that scratch is a file-scope static device
+ * array of ocn_noalloc_scratch_bytes() = 16 MiB, which every GPU that loads the library holds until the process exits.
+ * Limit: (sx * sy * nz + 64) pairs of `precision`-bit values must fit, sx = roundup(nx + 8, 32), sy = ny + 6 (e.g. up to about
+ * 360 x 150 x 25 in fp32); a larger model is rejected with OCN_EUNSUPPORTED and a message that names both sizes.
+ * Results are identical to ocn_get_mixing.  The array is SHARED by every call and every model of the process and keeps the
+ * last call's contents: each call first clears the part it uses, on the model's stream.  Calls that overlap on the GPU
+ * (two models on different streams, or two host threads) race on it: serialise them. */
+ocn_status ocn_get_mixing_noalloc(ocn_model* model, double* nu, double* kappa);
+unsigned long long ocn_noalloc_scratch_bytes(void);
+
 const char* ocn_last_error(void);
 const char* ocn_version(void);
 

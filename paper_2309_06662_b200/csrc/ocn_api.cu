@@ -17,6 +17,13 @@
 #include "kernels_tile.cuh"
 #include "kernels_mixing.cuh"
 
+// Scratch of the allocation-free entry point ocn_get_mixing_noalloc (include/ocn.h): the halo'd (nu, kappa) pair array that
+// k_ri_mixing writes before it is gathered into the caller's buffers.  A file-scope device array of a fixed, modest size:
+// every GPU that loads the library holds these bytes until the process exits.  In HOST code this name is only a stand-in
+// for the symbol, not a device address: the address a kernel may use comes from cudaGetSymbolAddress (noalloc_scratch).
+#define OCN_NOALLOC_SCRATCH_BYTES (16u << 20)
+static __device__ __align__(256) unsigned char g_noalloc_scratch[OCN_NOALLOC_SCRATCH_BYTES];
+
 namespace {
 
 thread_local std::string g_err;
@@ -605,6 +612,47 @@ ocn_status get_mixing_t(ocn_model* M, double* nu, double* kappa) {
     return OCN_OK;
 }
 
+// Device address of g_noalloc_scratch on `device`, which must be the CURRENT device; looked up once per device.
+ocn_status noalloc_scratch(int device, void** out) {
+    constexpr int MAXDEV = 64;
+    static std::mutex mu;
+    static void* addr[MAXDEV] = {};
+    std::lock_guard<std::mutex> lock(mu);
+    if (device >= 0 && device < MAXDEV && addr[device]) { *out = addr[device]; return OCN_OK; }
+    void* p = nullptr;
+    CK(cudaGetSymbolAddress(&p, g_noalloc_scratch));
+    if (!p) return fail(OCN_ECUDA, "cudaGetSymbolAddress returned a null address for the scratch array");
+    if (device >= 0 && device < MAXDEV) addr[device] = p;
+    *out = p;
+    return OCN_OK;
+}
+
+// ocn_get_mixing without any allocation: k_ri_mixing writes into the static scratch array instead of a cudaMalloc'ed one.
+// The kernel only stores open faces (and the zeros that complete a sector), and relies on everything else being zero, so
+// the part of the scratch this model uses is cleared first: the array keeps whatever the last call (of any model) left.
+template <class T>
+ocn_status get_mixing_noalloc_t(ocn_model* M, double* nu, double* kappa) {
+    typedef typename ocn::Pair<T>::type T2;
+    ocn::DevP<T> P = params<T>(M);                 // a copy: the model's own parameter block (and its nk, if any) stays as it is
+    const int nz = M->g->nz;
+    const size_t bytes = ((size_t)P.sz * nz + 2 * LEAD) * sizeof(T2);
+    if (bytes > (size_t)OCN_NOALLOC_SCRATCH_BYTES)
+        return fail(OCN_EUNSUPPORTED, "ocn_get_mixing_noalloc: the (nu, kappa) planes of this model need " + std::to_string(bytes) +
+                                      " bytes, the static scratch holds " + std::to_string((size_t)OCN_NOALLOC_SCRATCH_BYTES) +
+                                      " (use ocn_get_mixing)");
+    void* base = nullptr;
+    ocn_status s = noalloc_scratch(M->d.device, &base);
+    if (s != OCN_OK) return s;
+    CK(cudaMemsetAsync(base, 0, bytes, M->stream));
+    P.nk = reinterpret_cast<T2*>(base) + LEAD;
+    const dim3 bc(32, 4);
+    ocn::k_ri_mixing<T><<<grid2(M->g, bc), bc, 0, M->stream>>>(P);
+    CK(cudaGetLastError());
+    if (nu && (s = get_one<T, double>(M, nu, (T*)P.nk, nz, 5, false, 2)) != OCN_OK) return s;
+    if (kappa && (s = get_one<T, double>(M, kappa, (T*)P.nk + 1, nz, 5, false, 2)) != OCN_OK) return s;
+    return OCN_OK;
+}
+
 }  // namespace
 
 // =================================================================================================
@@ -872,5 +920,14 @@ ocn_status ocn_get_mixing(ocn_model* M, double* nu, double* kappa) {
     ON_DEVICE(M->d.device);
     return M->prec == 32 ? get_mixing_t<float>(M, nu, kappa) : get_mixing_t<double>(M, nu, kappa);
 }
+
+ocn_status ocn_get_mixing_noalloc(ocn_model* M, double* nu, double* kappa) {
+    if (!M) return fail(OCN_EINVAL, "null model");
+    if (M->d.closure != 1) return fail(OCN_ESTATE, "model was created with closure = 0");
+    ON_DEVICE(M->d.device);
+    return M->prec == 32 ? get_mixing_noalloc_t<float>(M, nu, kappa) : get_mixing_noalloc_t<double>(M, nu, kappa);
+}
+
+unsigned long long ocn_noalloc_scratch_bytes(void) { return (unsigned long long)OCN_NOALLOC_SCRATCH_BYTES; }
 
 }  // extern "C"

@@ -46,7 +46,8 @@ class ocn_fields(C.Structure):
 EXPORTS = ["ocn_grid_create", "ocn_grid_destroy", "ocn_model_create", "ocn_model_destroy", "ocn_set_fields",
            "ocn_time_step", "ocn_get_fields", "ocn_synchronize", "ocn_get_masks", "ocn_model_info",
            "ocn_get_debug", "ocn_last_error", "ocn_version", "ocn_profile_enable", "ocn_profile_read",
-           "ocn_stage_name", "ocn_get_mixing", "ocn_get_fields_async", "ocn_wait", "ocn_tune", "ocn_selftest_division", "ocn_get_timeline"]
+           "ocn_stage_name", "ocn_get_mixing", "ocn_get_fields_async", "ocn_wait", "ocn_tune", "ocn_selftest_division", "ocn_get_timeline",
+           "ocn_get_mixing_noalloc", "ocn_noalloc_scratch_bytes"]
 NSTAGES = 4
 
 
@@ -77,6 +78,8 @@ def lib():
         L.ocn_model_info.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_ulonglong)]
         L.ocn_get_debug.argtypes = [vp] + [vp] * 6
         L.ocn_get_mixing.argtypes = [vp, vp, vp]
+        L.ocn_get_mixing_noalloc.argtypes = [vp, vp, vp]
+        L.ocn_noalloc_scratch_bytes.restype = C.c_ulonglong
         L.ocn_profile_enable.argtypes = [vp, C.c_int]
         L.ocn_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong), C.c_int]
         L.ocn_stage_name.restype = C.c_char_p
@@ -222,6 +225,13 @@ class Model:
         nz, ny, nx = self.nz, self.ny, self.nx
         d = dict(nu=np.zeros((nz, ny, nx)), kappa=np.zeros((nz, ny, nx)))
         _check(lib().ocn_get_mixing(self.h, _ptr(d["nu"]), _ptr(d["kappa"])))
+        return d
+
+    def mixing_noalloc(self):
+        """ocn_get_mixing_noalloc: the same diagnostic through the static scratch array (no device allocation)."""
+        nz, ny, nx = self.nz, self.ny, self.nx
+        d = dict(nu=np.zeros((nz, ny, nx)), kappa=np.zeros((nz, ny, nx)))
+        _check(lib().ocn_get_mixing_noalloc(self.h, _ptr(d["nu"]), _ptr(d["kappa"])))
         return d
 
     def close(self):
