@@ -536,8 +536,8 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
             const T2* __restrict__ s_flux = (const T2*)(sm + C::O_FLUX + (k & 1) * C::FLB);
             const bool has_hi = k + 1 < nz;
             // RI: vertical spacings around level k for the per-column elimination
-            T dzc_lo = T(1), dzc_hi = T(1), rc_lo = T(1), rc_hi = T(1);
-            const T2* __restrict__ s_nk1 = nullptr;
+            [[maybe_unused]] T dzc_lo = T(1), dzc_hi = T(1), rc_lo = T(1), rc_hi = T(1);
+            [[maybe_unused]] const T2* __restrict__ s_nk1 = nullptr;
             if constexpr (RI) {
                 dzc_lo = s_dzc[k]; rc_lo = s_rdzc[k];
                 if (has_hi) { dzc_hi = s_dzc[k + 1]; rc_hi = s_rdzc[k + 1]; }
