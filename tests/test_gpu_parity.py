@@ -328,6 +328,73 @@ def test_device_buffers_and_callers_stream_match_host_path():
     dev.close()
 
 
+def test_async_read_back_and_tickets():
+    """ocn_get_fields_async leaves the copy in flight beside later steps; ocn_wait(ticket) makes the buffer valid.  The value
+    read back is the state at the time of the call (the gather is ordered on the model's stream), not a later one."""
+    import torch
+    wl = W.config3(nx=96, ny=40, nz=12, steps=6)
+    ref = ocn.Model(wl)
+    want = []
+    for _ in range(6):
+        ref.time_step(1)
+        want.append(ref.get_fields(names=("eta",))["eta"].copy())
+    ref.close()
+    m = ocn.Model(wl)
+    bufs = [torch.empty((m.ny, m.nx), dtype=torch.float32).pin_memory() for _ in range(6)]
+    tickets = []
+    for n in range(6):
+        m.time_step(1)
+        tickets.append(m.get_fields_async_ptr(eta=bufs[n].data_ptr()))       # all six in flight, steps keep being enqueued
+    assert tickets == sorted(tickets) and len(set(tickets)) == 6
+    m.wait(tickets[-1])                                                       # waits for every earlier one too
+    for n in range(6):
+        assert np.array_equal(bufs[n].numpy(), want[n]), n
+    with pytest.raises(RuntimeError, match="never issued"):
+        m.wait(tickets[-1] + 1000)
+    # more read-backs than the library holds events for: old tickets stay waitable
+    for _ in range(80):
+        t = m.get_fields_async_ptr(eta=bufs[0].data_ptr())
+    m.wait(tickets[0]); m.wait(t)
+    assert np.array_equal(bufs[0].numpy(), want[5])
+    # 3-D fields through the big staging region, and the blocking call after async ones
+    u = torch.empty((m.nz, m.ny, m.nx), dtype=torch.float32).pin_memory()
+    tk = m.get_fields_async_ptr(u=u.data_ptr())
+    full = m.get_fields()
+    m.wait(tk)
+    assert np.array_equal(u.numpy(), full["u"])
+    m.close()
+
+
+def test_results_do_not_depend_on_the_ownership_threshold():
+    """ocn_tune("k1_geo_threshold"): compact ownership only, the default switch, and geometric ownership from the first level
+    on give identical bits (fp32 and fp64, with and without the closure); unknown keys are rejected."""
+    for prec, closure in ((32, 0), (32, 1), (64, 0)):
+        wl = W.config2(nx=180, ny=75, nz=25, steps=5, precision=prec)
+        rng = np.random.default_rng(8)
+        wl["fields"]["u"] = W._round_to(prec, 0.2 * rng.standard_normal(wl["fields"]["u"].shape))
+        wl["fields"]["v"] = W._round_to(prec, 0.2 * rng.standard_normal(wl["fields"]["v"].shape))
+        if closure:
+            W.with_ri_closure(wl)
+        res = []
+        for thr in (100000, 224, 64, 0):
+            m = ocn.Model(wl)
+            m.tune("k1_geo_threshold", thr)
+            m.time_step(5)
+            res.append(m.get_fields())
+            m.close()
+        for r in res[1:]:
+            for n in FIELDS:
+                assert np.array_equal(r[n], res[0][n]), (prec, closure, n)
+    m = ocn.Model(W.config0())
+    with pytest.raises(RuntimeError, match="unknown tuning key"):
+        m.tune("no_such_knob", 1)
+    m.time_step(2)
+    m.tune("k1_geo_threshold", 0)                     # after the graph was captured: it is re-captured
+    m.time_step(2)
+    assert np.isfinite(m.get_fields()["eta"]).all()
+    m.close()
+
+
 def test_profiling_path_gives_the_same_bits_and_sane_times():
     wl = W.config3(nx=96, ny=40, nz=12, steps=4)
     a = ocn.Model(wl); a.time_step(4); fa = a.get_fields(); a.close()
