@@ -37,6 +37,12 @@ UNIT = "cell-updates/s"
 # `word` bytes per value except the hydrostatic pressure, which is stored in fp64 in both precisions
 # With the Ri closure (--closure ri) K1 evaluates (nu, kappa) on chip and writes the 3 modified
 # super-diagonals of the per-column solves, which K3 reads: + 3 words each.
+# algorithmic floating-point operations of K1 per wet cell-update (+, -, x, / of the formulas of sections
+# 3.4-3.8 as written, every face reconstructed once, all orders 3): 8 WENO reconstructions x 68 + fluxes and divergence 56 +
+# zeta, K, D 24 + the u and v points 86 + quasi-AB2, predictor, elimination, column sums, w 42
+K1_FLOPS_PER_WET_CELL = 8 * 68 + 56 + 24 + 86 + 42
+
+
 def stage_bytes(stage, word, closure=0):
     b = {"tendency": (16 + (3 if closure else 0)) * word + 8, "backsub_correct_pressure": (8 + (3 if closure else 0)) * word + 8}
     return b.get(stage)
@@ -344,6 +350,17 @@ def run_ours(args):
         issue_util = {"kernel": dom, "warp_instructions_per_launch": ent["warp_instructions_per_launch"],
                       "issue_slots_per_launch": slots, "utilisation": ent["warp_instructions_per_launch"] / slots,
                       "source": "profiles/traffic.json (ncu smsp__inst_executed.sum) / (148 SMs x 4 schedulers x sampled SM clock x live K1 time)"}
+    # second view of K1, which is bound by arithmetic: the flops of the formulas as written (NOT executed instructions) against
+    # the plain-ALU peak of the chip, 148 SMs x 128 fp32 lanes (64 in fp64) x 2 flop per FMA x sampled SM clock
+    roof_alu = None
+    if dom == "tendency":
+        mhz = clk.get("sm_mhz") or 1965.0
+        peak_tf = 148 * (128 if word == 4 else 64) * 2 * mhz * 1e6 / 1e12
+        ach_tf = K1_FLOPS_PER_WET_CELL * nwet / (stages[dom]["ms"] / K * 1e-3) / 1e12
+        roof_alu = {"kernel": dom, "bound": "alu", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach_tf / peak_tf,
+                    "flops_per_wet_cell": K1_FLOPS_PER_WET_CELL,
+                    "peak_source": "148 SMs x %d lanes x 2 (FMA) x sampled SM clock; flop count of the formulas: DESIGN.md section 7"
+                                   % (128 if word == 4 else 64)}
     # the whole step against the HBM roofline (north_star's target is 0.60 for the fused step on config 4)
     step_bytes = sum((stage_bytes(s_, word, ri) or 0) for s_ in stages) * nwet + 16 * word * nx * ny * (info["launches_per_step"] - 3)
     roof_step = {"bound": "hbm", "algorithmic_bytes_per_step": step_bytes, "achieved": step_bytes / sec_per_step / 1e9,
@@ -454,7 +471,7 @@ def run_ours(args):
                            "parallelism": "replicas x%d" % world},
                 "sypd_equivalent": sypd(prm["dt"], sec_per_step),
                 "wet_cell_updates_per_s": world * nwet * K / (ms_total * 1e-3),
-                "stages": stage_out, "roofline": roof, "roofline_step": roof_step, "issue_utilisation": issue_util, "e2e": e2e,
+                "stages": stage_out, "roofline": roof, "roofline_step": roof_step, "roofline_alu": roof_alu, "issue_utilisation": issue_util, "e2e": e2e,
                 "e2e_with_state_io": e2e_state, "closure_ri": closure_line, "cpu_baseline": cpu,
                 "gpu_launches": info["launches_per_step"] * K, "clocks": clk,
                 "device_bytes": info["device_bytes"]}

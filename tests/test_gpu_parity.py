@@ -212,6 +212,19 @@ def test_smallest_grids_and_two_levels():
         run_both(wl, 4, check_every=[1, 4])
 
 
+def test_smallest_and_doubly_periodic_grids_fp32():
+    """The fp32 path has its own barotropic kernel (register strips, halo 10 wrapped at load time): tiny grids where the
+    extended tile wraps around the domain several times, periodic in one or both directions, ragged against the 64 x 28 tile."""
+    for nx, ny, nz, per in ((3, 3, 2, (1, 1)), (5, 4, 3, (0, 0)), (33, 9, 2, (1, 0)), (9, 33, 3, (0, 1)), (70, 31, 4, (1, 1)),
+                            (130, 57, 3, (1, 1))):
+        wl = W.config0(nx=nx, ny=ny, nz=nz)
+        wl["grid"]["periodic_x"], wl["grid"]["periodic_y"] = per
+        wl["params"]["precision"] = 32
+        wl["fields"] = {k: W._round_to(32, v) for k, v in wl["fields"].items()}
+        wl["fields"]["eta"] = W._round_to(32, 0.05 * np.cos(2 * np.pi * (np.arange(nx)[None, :] / nx + np.arange(ny)[:, None] / ny)))
+        run_both(wl, 4, check_every=[1, 4])
+
+
 def test_isolated_columns_and_one_cell_channels():
     # a checkerboard-ish bathymetry: isolated wet columns (no open faces) and one-cell-wide channels, ragged depths
     rng = np.random.default_rng(11)
