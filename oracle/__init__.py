@@ -50,7 +50,8 @@ class ModelDesc(C.Structure):
                 ("closure", C.c_int), ("ri_nu0", C.c_double), ("ri_c", C.c_double), ("ri_kconv", C.c_double),
                 ("ri_n2c", C.c_double), ("ri_s2min", C.c_double), ("gamma_T", C.c_double), ("gamma_S", C.c_double),
                 ("drag_r", C.c_double), ("drag_cd", C.c_double),
-                ("eos", C.c_int), ("eos_alpha2", C.c_double), ("eos_gamma", C.c_double), ("advection", C.c_int)]
+                ("eos", C.c_int), ("eos_alpha2", C.c_double), ("eos_gamma", C.c_double), ("advection", C.c_int),
+                ("filter_weights_uv", C.POINTER(C.c_double))]
 
 
 class Fields(C.Structure):
@@ -166,12 +167,14 @@ class RefModel:
     """Oracle model.  `workload` is a dict from paper_2309_06662_b200.workloads (passed in by the
     caller; this module does not import it)."""
 
-    def __init__(self, workload, filter_weights=None):
+    def __init__(self, workload, filter_weights=None, filter_weights_uv=None):
         self.grid = RefGrid(workload["grid"], workload["z_faces"], workload["depth"])
         p = dict(workload["params"])
         p.pop("precision", None)
         self._fw = None if filter_weights is None else np.ascontiguousarray(filter_weights, dtype=np.float64)
-        self.desc = ModelDesc(filter_weights=_dp(self._fw) if self._fw is not None else None, **p)
+        self._fwuv = None if filter_weights_uv is None else np.ascontiguousarray(filter_weights_uv, dtype=np.float64)
+        self.desc = ModelDesc(filter_weights=_dp(self._fw) if self._fw is not None else None,
+                              filter_weights_uv=_dp(self._fwuv) if self._fwuv is not None else None, **p)
         self.nx, self.ny, self.nz = self.grid.nx, self.grid.ny, self.grid.nz
         self.h = C.c_void_p()
         _check(lib().ocn_ref_model_create(self.grid.h, C.byref(self.desc), C.byref(self.h)))

@@ -145,6 +145,7 @@ struct ocn_ref_model {
     const ocn_ref_grid* g;
     ocn_ref_model_desc d;
     std::vector<double> a_w;        // filter weights a_m, m = 1..M  (index m-1)
+    std::vector<double> b_w;        // filter weights of the transports U, V; = a_w unless given
     double dtau;
     A3 u, v, T, S, w, p;            // w has nz+1 levels
     A3 Gu, Gv, GT, GS;              // G^n
@@ -572,12 +573,12 @@ void time_step(ocn_ref_model& M) {
     fill_halo(M.eta, g.px, g.py); fill_halo(M.U, g.px, g.py); fill_halo(M.V, g.px, g.py);
     for (int m = 1; m <= M.d.substeps; ++m) {
         barotropic_substep(M, M.dtau, &GU, &GV);
-        const double a = M.a_w[m - 1];
+        const double a = M.a_w[m - 1], b = M.b_w[m - 1];
         for (int j = 0; j < ny; ++j)
             for (int i = 0; i < nx; ++i) {
                 etab(0, j, i) += a * M.eta(0, j, i);
-                Ub(0, j, i) += a * M.U(0, j, i);
-                Vb(0, j, i) += a * M.V(0, j, i);
+                Ub(0, j, i) += b * M.U(0, j, i);
+                Vb(0, j, i) += b * M.V(0, j, i);
             }
     }
     // 7. the filtered values become the new barotropic state
@@ -706,7 +707,7 @@ int ocn_ref_model_create(const ocn_ref_grid* g, const ocn_ref_model_desc* d, ocn
     if (d->closure == 1 && !(d->ri_n2c > 0 && d->ri_s2min > 0 && d->ri_c >= 0 && d->ri_nu0 >= 0 && d->ri_kconv >= 0))
         return fail("bad Ri closure parameters");
     ocn_ref_model* M = new ocn_ref_model();
-    M->g = g; M->d = *d; M->d.filter_weights = nullptr;
+    M->g = g; M->d = *d; M->d.filter_weights = nullptr; M->d.filter_weights_uv = nullptr;
     double ratio;
     if (d->filter_weights) {
         M->a_w.assign(d->filter_weights, d->filter_weights + d->substeps);
@@ -717,6 +718,8 @@ int ocn_ref_model_create(const ocn_ref_grid* g, const ocn_ref_model_desc* d, ocn
         filter_weights(d->substeps, M->a_w, ratio);
     }
     M->dtau = d->dt * ratio;
+    M->b_w = M->a_w;
+    if (d->filter_weights_uv) M->b_w.assign(d->filter_weights_uv, d->filter_weights_uv + d->substeps);
     const int nx = g->nx, ny = g->ny, nz = g->nz;
     for (A3* f : {&M->u, &M->v, &M->T, &M->S, &M->p, &M->Gu, &M->Gv, &M->GT, &M->GS,
                   &M->Gu1, &M->Gv1, &M->GT1, &M->GS1}) f->init(nx, ny, nz);

@@ -55,6 +55,8 @@ typedef struct {
     double eos_alpha2, eos_gamma;
     /* nonlinear WENO weights: 0 = Jiang-Shu, 1 = WENO-Z */
     int advection;
+    /* separate filter weights b_m (m = 1..M) for the barotropic transports U, V; NULL = the weights of eta */
+    const double* filter_weights_uv;
 } ocn_ref_model_desc;
 
 typedef struct {

@@ -144,3 +144,54 @@ def test_cabbeling_mixing_two_parcels_makes_denser_water():
     b1, b2, bm = top_b(2.0), top_b(22.0), top_b(12.0)
     P = W._params(64, 1, 1, 0, 0)
     assert abs((0.5 * (b1 + b2) - bm) - P["g"] * 0.5 * 1e-5 * 100.0) < 1e-12          # g alpha2/2 ((dT1^2 + dT2^2)/2 - dTm^2) = g alpha2/2 * 100
+
+
+# =============================================================================================
+# separate filter weights for the barotropic transports
+# =============================================================================================
+def _other_weights(M, p=1, q=2):
+    s = np.arange(1, M + 1) / (M + 1.0)
+    b = s ** p * (1.0 - s ** q)
+    return b / b.sum()
+
+
+def test_transport_weights_equal_to_eta_weights_change_nothing():
+    wl = W.config2(nx=48, ny=20, nz=10, steps=4)
+    a, _ = oracle.filter_weights(wl["params"]["substeps"])
+    m0, m1 = oracle.RefModel(wl), oracle.RefModel(wl, filter_weights_uv=a)
+    m0.step(4); m1.step(4)
+    f0, f1 = m0.get_fields(), m1.get_fields()
+    for n in ("u", "v", "w", "eta", "T", "S"):
+        assert np.array_equal(f0[n], f1[n]), n
+
+
+def test_transport_weights_closed_form_uniform_wind_on_a_flat_periodic_box():
+    """Flat doubly periodic box at rest, f = 0, uniform wind stress: G^U = tau / rho0 everywhere, eta stays flat, so
+    U^m = m dtau G^U and the filtered transport is dtau G^U sum_m m b_m (Euler first step) - it tells b from a, whose first
+    moment is dt / dtau by construction; eta-bar stays exactly 0 and the corrected u has the depth mean U-bar / H."""
+    M, dt, H = 12, 100.0, 400.0
+    wl = box(nx=8, ny=6, nz=4, depth=H, f0=0.0, dt=dt, substeps=M, nu_z=0.0)
+    wl["fields"]["tau_x"][:] = 0.2
+    a, ratio = oracle.filter_weights(M)
+    b = _other_weights(M)
+    assert abs(np.dot(np.arange(1, M + 1), b) - np.dot(np.arange(1, M + 1), a)) > 0.3
+    for weights, moment in ((None, 1.0 / ratio), (b, float(np.dot(np.arange(1, M + 1), b)))):
+        m = oracle.RefModel(wl, filter_weights_uv=weights)
+        m.step(1)
+        U = m.diagnostics()["U"]
+        want = (dt * ratio) * (0.2 / wl["params"]["rho0"]) * moment
+        assert np.max(np.abs(U - want)) < 1e-14 * want, (weights is None, U[0, 0], want)
+        f = m.get_fields()
+        assert np.all(f["eta"] == 0.0) and np.all(f["v"] == 0.0)
+        dz = np.diff(wl["z_faces"])
+        assert np.max(np.abs((f["u"] * dz[:, None, None]).sum(axis=0) - want)) < 1e-13 * want
+
+
+def test_transport_weights_leave_eta_filter_and_tracers_alone_but_change_the_flow():
+    wl = W.config2(nx=48, ny=20, nz=10, steps=3)
+    b = _other_weights(wl["params"]["substeps"])
+    m0, m1 = oracle.RefModel(wl), oracle.RefModel(wl, filter_weights_uv=b)
+    m0.step(1); m1.step(1)
+    f0, f1 = m0.get_fields(), m1.get_fields()
+    assert np.array_equal(f0["eta"], f1["eta"]) and np.array_equal(f0["T"], f1["T"])     # first step: eta-bar and T do not see U-bar
+    assert np.abs(f0["u"] - f1["u"]).max() > 1e-9
