@@ -98,6 +98,10 @@ typedef struct {
     /* Nonlinear weights of the WENO reconstructions ("based on WENO reconstructions", the family of refs
      * PAPER.md:244-245): 0 = Jiang-Shu (north_star reading), 1 = WENO-Z. */
     int advection;
+    /* Separate filter weights b_1..b_M for the barotropic TRANSPORTS: HOST, `substeps`
+     * doubles that sum to 1, or NULL = the weights of eta (filter_weights).  eta-bar = sum a_m eta^m, U-bar = sum b_m U^m,
+     * V-bar likewise; dtau is still set by the first moment of a.  Copied at creation. */
+    const double* filter_weights_uv;
 } ocn_model_desc;
 
 /* ocn_model_create — the model of PAPER.md:84 (§5.2: hydrostatic Boussinesq, IMEX quasi-AB2, backward-Euler vertical

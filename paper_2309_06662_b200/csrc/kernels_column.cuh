@@ -39,6 +39,11 @@ __device__ __forceinline__ double pressure_level(const DevP<T>& P, int k, double
 #define BT_HALO 6                  // sub-steps per launch = halo rings of the resident tile (<= 6: the launch carries six weights)
 #endif
 
+// filter weights of the sub-steps of one launch: a for eta, b for the transports U, V (b = a unless
+// the model was given filter_weights_uv)
+#define BT_MAXW 12
+template <class T> struct BtWeights { T a[BT_MAXW], b[BT_MAXW]; };
+
 template <class T, int BTX, int BTY>
 struct BtTile {
     static constexpr int EX = BTX + 2 * BT_HALO, EY = BTY + 2 * BT_HALO, NE = EX * EY;
@@ -48,7 +53,7 @@ struct BtTile {
 
 template <class T, int BTX, int BTY>
 __global__ void __launch_bounds__((BtTile<T, BTX, BTY>::NT)) k_barotropic_tile(const DevP<T> P, const int cur, const int ns, const int first,
-                                                         const T a0, const T a1, const T a2, const T a3, const T a4, const T a5) {
+                                                         const BtWeights<T> W) {
     typedef BtTile<T, BTX, BTY> C;
     constexpr int EX = C::EX, EY = C::EY, NE = C::NE, NT = C::NT, H = BT_HALO;
     extern __shared__ __align__(16) unsigned char smb[];
@@ -70,9 +75,8 @@ __global__ void __launch_bounds__((BtTile<T, BTX, BTY>::NT)) k_barotropic_tile(c
     const int i0 = blockIdx.x * BTX, j0 = blockIdx.y * BTY;
     const int nx = P.nx, ny = P.ny, nz = P.nz, sx = P.sx;
     if (tid == 0) {
-        const T aw[6] = {a0, a1, a2, a3, a4, a5};
 #pragma unroll
-        for (int q = 0; q < BT_HALO; ++q) saw[q] = aw[q];
+        for (int q = 0; q < BT_HALO; ++q) saw[q] = W.a[q];
     }
 
     // ---- load the extended tile (wrap / land) ----
@@ -168,7 +172,7 @@ __global__ void __launch_bounds__((BtTile<T, BTX, BTY>::NT)) k_barotropic_tile(c
                 }
             }
             __syncthreads();
-            const T am = saw[s];
+            const T am = saw[s], bm = W.b[s];
 #pragma unroll
             for (int n = 0; n < C::PER; ++n) {
                 const int q = n * NT + tid;
@@ -177,7 +181,7 @@ __global__ void __launch_bounds__((BtTile<T, BTX, BTY>::NT)) k_barotropic_tile(c
                     const T un = sU[q] + (cu[n] * (ew - ec) + gu[n]);
                     const T vn = sV[q] + (cv[n] * (es - ec) + gv[n]);
                     sU[q] = un; sV[q] = vn;
-                    if (cidx[n] >= 0) { be[n] += am * ec; bU[n] += am * un; bV[n] += am * vn; }
+                    if (cidx[n] >= 0) { be[n] += am * ec; bU[n] += bm * un; bV[n] += bm * vn; }
                 }
             }
             __syncthreads();
@@ -192,7 +196,7 @@ __global__ void __launch_bounds__((BtTile<T, BTX, BTY>::NT)) k_barotropic_tile(c
                                          Az[y], rAz[y])).v;
         }
         __syncthreads();
-        const T am = saw[s];
+        const T am = saw[s], bm = W.b[s];
 #pragma unroll
         for (int n = 0; n < C::PER; ++n) {
             const int q = n * NT + tid;
@@ -205,7 +209,7 @@ __global__ void __launch_bounds__((BtTile<T, BTX, BTY>::NT)) k_barotropic_tile(c
                 if (y > 0) vn = (mk & 4) ? (X(vn) + X(dtau) * (xdiv(-X(g) * X(sHv[q]) * (X(ec) - X(se[q - EX])), dy, rdy) + X(sGV[q]))).v : T(0);
                 sU[q] = un; sV[q] = vn;
                 if (cidx[n] >= 0) {
-                    be[n] = (X(be[n]) + X(am) * X(ec)).v; bU[n] = (X(bU[n]) + X(am) * X(un)).v; bV[n] = (X(bV[n]) + X(am) * X(vn)).v;
+                    be[n] = (X(be[n]) + X(am) * X(ec)).v; bU[n] = (X(bU[n]) + X(bm) * X(un)).v; bV[n] = (X(bV[n]) + X(bm) * X(vn)).v;
                 }
             }
         }
@@ -233,9 +237,6 @@ __global__ void __launch_bounds__((BtTile<T, BTX, BTY>::NT)) k_barotropic_tile(c
 // needs about fifty, which is what bounded it (LSU pipe 74 % busy, profiles/r1_ncu_summary.md).  NS <= H sub-steps per
 // launch on a halo of H that is recomputed redundantly and shrinks one ring per sub-step (PAPER.md:98 on chip).
 // ---------------------------------------------------------------------------------------------
-#define BT_MAXW 12
-template <class T> struct BtWeights { T a[BT_MAXW]; };
-
 template <int BTX, int BTY, int H>
 struct BtStrip {
     static constexpr int EX = BTX + 2 * H, EY = BTY + 2 * H, SPR = EX / 4, NS = SPR * EY;   // strips per row, strips
@@ -324,7 +325,7 @@ k_barotropic_strip(const DevP<float> P, const int cur, const int ns, const int f
         }
         __syncthreads();
         if (on) {
-            const float am = W.a[s];
+            const float am = W.a[s], bm = W.b[s];
             const float ew = se[qw];
             const float4 es = *(const float4*)(se + qs);
             u[0] = u[0] + (cu[0] * (ew - e[0]) + gu[0]);
@@ -336,7 +337,7 @@ k_barotropic_strip(const DevP<float> P, const int cur, const int ns, const int f
             v[2] = v[2] + (cv[2] * (es.z - e[2]) + gv[2]);
             v[3] = v[3] + (cv[3] * (es.w - e[3]) + gv[3]);
 #pragma unroll
-            for (int r = 0; r < 4; ++r) { be[r] += am * e[r]; bU[r] += am * u[r]; bV[r] += am * v[r]; }
+            for (int r = 0; r < 4; ++r) { be[r] += am * e[r]; bU[r] += bm * u[r]; bV[r] += bm * v[r]; }
             *(float4*)(sU + qb) = make_float4(u[0], u[1], u[2], u[3]);
             *(float4*)(sV + qb) = make_float4(v[0], v[1], v[2], v[3]);
         }

@@ -61,7 +61,7 @@ struct ocn_model {
     int prec = 64;
     cudaStream_t stream = nullptr;
     bool own_stream = false;
-    std::vector<double> a_w;
+    std::vector<double> a_w, b_w;       // filter weights of eta and of the transports (b_w = a_w unless filter_weights_uv was given)
     double dtau = 0;
     bool have_history = false;
     std::vector<void*> allocs;
@@ -406,7 +406,7 @@ ocn_status launch_step(ocn_model* M, bool euler) {
         for (int m0 = 0; m0 < M->d.substeps; m0 += BS_H) {
             const int ns = std::min(BS_H, M->d.substeps - m0);
             ocn::BtWeights<float> W{};
-            for (int q = 0; q < ns; ++q) W.a[q] = (float)M->a_w[m0 + q];
+            for (int q = 0; q < ns; ++q) { W.a[q] = (float)M->a_w[m0 + q]; W.b[q] = (float)M->b_w[m0 + q]; }
             ocn::k_barotropic_strip<BS_X, BS_Y, BS_H><<<gb, B::NT, B::SMEM, M->stream>>>(P, cur, ns, m0 == 0 ? 1 : 0, W);
             cur ^= 1;
         }
@@ -416,10 +416,9 @@ ocn_status launch_step(ocn_model* M, bool euler) {
         int cur = 0;
         for (int m0 = 0; m0 < M->d.substeps; m0 += BT_HALO) {
             const int ns = std::min(BT_HALO, M->d.substeps - m0);
-            T a[6];
-            for (int q = 0; q < 6; ++q) a[q] = q < ns ? (T)M->a_w[m0 + q] : T(0);
-            ocn::k_barotropic_tile<T, BT_X, BT_Y><<<gb, B::NT, B::SMEM, M->stream>>>(P, cur, ns, m0 == 0 ? 1 : 0, a[0], a[1], a[2],
-                                                                                 a[3], a[4], a[5]);
+            ocn::BtWeights<T> W{};
+            for (int q = 0; q < ns; ++q) { W.a[q] = (T)M->a_w[m0 + q]; W.b[q] = (T)M->b_w[m0 + q]; }
+            ocn::k_barotropic_tile<T, BT_X, BT_Y><<<gb, B::NT, B::SMEM, M->stream>>>(P, cur, ns, m0 == 0 ? 1 : 0, W);
             cur ^= 1;
         }
     }
@@ -753,6 +752,16 @@ ocn_status ocn_model_create(const ocn_grid* g, const ocn_model_desc* d, ocn_mode
     if (!(first > 0)) { delete M; return fail(OCN_EINVAL, "filter weights have no positive first moment"); }
     M->dtau = d->dt * (1.0 / first);
     M->d.filter_weights = nullptr;
+    M->b_w = M->a_w;
+    if (d->filter_weights_uv) {
+        double sum = 0;
+        for (int m = 0; m < Ms; ++m) { M->b_w[m] = d->filter_weights_uv[m]; sum += M->b_w[m]; }
+        if (!std::isfinite(sum) || std::fabs(sum - 1.0) > 1e-9) {
+            delete M;
+            return fail(OCN_EINVAL, "filter_weights_uv must be finite and sum to 1");
+        }
+    }
+    M->d.filter_weights_uv = nullptr;
     if (d->stream) M->stream = static_cast<cudaStream_t>(d->stream);
     else {
         cudaError_t e = cudaStreamCreateWithFlags(&M->stream, cudaStreamNonBlocking);

@@ -35,7 +35,8 @@ class ocn_model_desc(C.Structure):
                 ("closure", C.c_int), ("ri_nu0", C.c_double), ("ri_c", C.c_double), ("ri_kconv", C.c_double),
                 ("ri_n2c", C.c_double), ("ri_s2min", C.c_double), ("gamma_T", C.c_double), ("gamma_S", C.c_double),
                 ("drag_r", C.c_double), ("drag_cd", C.c_double),
-                ("eos", C.c_int), ("eos_alpha2", C.c_double), ("eos_gamma", C.c_double), ("advection", C.c_int)]
+                ("eos", C.c_int), ("eos_alpha2", C.c_double), ("eos_gamma", C.c_double), ("advection", C.c_int),
+                ("filter_weights_uv", C.POINTER(C.c_double))]
 
 
 class ocn_fields(C.Structure):
@@ -137,14 +138,16 @@ class Grid:
 class Model:
     """ocn_model_create + ocn_set_fields on a workload dict (paper_2309_06662_b200.workloads)."""
 
-    def __init__(self, workload, device=0, stream=None, filter_weights=None, set_fields=True):
+    def __init__(self, workload, device=0, stream=None, filter_weights=None, set_fields=True, filter_weights_uv=None):
         self.grid = Grid(workload["grid"], workload["z_faces"], workload["depth"])
         p = dict(workload["params"])
         self.precision = int(p["precision"])
         self.dtype = np.float32 if self.precision == 32 else np.float64
         self._fw = None if filter_weights is None else np.ascontiguousarray(filter_weights, dtype=np.float64)
         fw = self._fw.ctypes.data_as(C.POINTER(C.c_double)) if self._fw is not None else None
-        self.desc = ocn_model_desc(filter_weights=fw, device=int(device), stream=stream, **p)
+        self._fwuv = None if filter_weights_uv is None else np.ascontiguousarray(filter_weights_uv, dtype=np.float64)
+        fwuv = self._fwuv.ctypes.data_as(C.POINTER(C.c_double)) if self._fwuv is not None else None
+        self.desc = ocn_model_desc(filter_weights=fw, filter_weights_uv=fwuv, device=int(device), stream=stream, **p)
         self.nx, self.ny, self.nz = self.grid.nx, self.grid.ny, self.grid.nz
         self.h = C.c_void_p()
         _check(lib().ocn_model_create(self.grid.h, C.byref(self.desc), C.byref(self.h)))

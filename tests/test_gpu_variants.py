@@ -93,3 +93,32 @@ def test_bad_variant_switches_are_rejected():
         bad = dict(wl, params=dict(wl["params"], **{key: val}))
         with pytest.raises(RuntimeError, match=key):
             ocn.Model(bad)
+
+
+def _other_weights(M, p=1, q=2):
+    s = np.arange(1, M + 1) / (M + 1.0)
+    b = s ** p * (1.0 - s ** q)
+    return b / b.sum()
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+def test_separate_transport_filter_weights(prec):
+    """filter_weights_uv: both barotropic kernels (fp64 point-wise tile, fp32 register strips; M = 30 is
+    not a multiple of either kernel's sub-steps per launch) against the oracle; fp64 bit-identical."""
+    wl = _stirred(W.config2(nx=180, ny=75, nz=25, steps=6, precision=prec))
+    b = _other_weights(wl["params"]["substeps"])
+    ref, gpu = oracle.RefModel(wl, filter_weights_uv=b), ocn.Model(wl, filter_weights_uv=b)
+    plain = ocn.Model(wl)
+    ref.step(6); gpu.time_step(6); plain.time_step(6)
+    a, r, p0 = gpu.get_fields(), ref.get_fields(), plain.get_fields()
+    assert np.abs(a["u"].astype(np.float64) - p0["u"]).max() > 1e-6             # the weights matter
+    errs = {n: rel_linf(a[n], r[n]) for n in FIELDS}
+    if prec == 64:
+        for n in FIELDS:
+            assert np.array_equal(a[n], r[n]), (n, errs[n])
+    else:
+        report_parity("transport weights 180x75x25 fp32", 6, errs)
+        assert all(e <= 2e-4 for e in errs.values()), errs
+    gpu.close(); plain.close()
+    with pytest.raises(RuntimeError, match="filter_weights_uv"):
+        ocn.Model(wl, filter_weights_uv=2.0 * b)
