@@ -463,6 +463,82 @@ void momentum_tendency(const ocn_ref_model& M, A3& Gu, A3& Gv, A3& zeta, A3& Ke,
             }
 }
 
+// ---------------------------------------------------------------------------------------------
+// biharmonic horizontal dissipation: the horizontal Laplacian applied twice.
+//   vector Laplacian of a C-grid vector (a at u points, b at v points), in the vector-invariant form of §3.6:
+//     Da = [dy (a[i+1] - a[i]) + dxF[j+1] b[j+1] - dxF[j] b[j]] / AzC[j]
+//     Za = [dy (b[i] - b[i-1]) - (dxC[j] a[j] - dxC[j-1] a[j-1])] / AzF[j]
+//     La = mu [(Da[i] - Da[i-1]) / dxC[j] - (Za[j+1] - Za[j]) / dy],  Lb = mv [(Da[j] - Da[j-1]) / dy + (Za[i+1] - Za[i]) / dxF[j]]
+//   scalar Laplacian of a tracer with no flux through closed faces:
+//     fx[i] = dy (c[i] - c[i-1]) / dxC[j] mu[i],  fy[j] = dxF[j] (c[j] - c[j-1]) / dy mv[j],
+//     Lc = wet [(fx[i+1] - fx[i]) + (fy[j+1] - fy[j])] / AzC[j]
+// Inputs must be halo-filled; outputs are halo-filled here.
+// ---------------------------------------------------------------------------------------------
+void vector_laplacian(const ocn_ref_grid& g, const A3& a, const A3& b, A3& La, A3& Lb) {
+    const int nx = g.nx, ny = g.ny, nz = g.nz;
+    A3 Da, Za;
+    Da.init(nx, ny, nz); Za.init(nx, ny, nz);
+#pragma omp parallel for schedule(static)
+    for (int j = -2; j < ny + HALO - 1; ++j)
+        for (int k = 0; k < nz; ++k)
+            for (int i = -2; i < nx + HALO - 1; ++i) {
+                Da(k, j, i) = (g.dy * (a(k, j, i + 1) - a(k, j, i)) + g.dxF(j + 1) * b(k, j + 1, i) - g.dxF(j) * b(k, j, i)) / g.AzC(j);
+                Za(k, j, i) = (g.dy * (b(k, j, i) - b(k, j, i - 1)) - (g.dxC(j) * a(k, j, i) - g.dxC(j - 1) * a(k, j - 1, i))) / g.AzF(j);
+            }
+#pragma omp parallel for schedule(static)
+    for (int j = 0; j < ny; ++j)
+        for (int k = 0; k < nz; ++k)
+            for (int i = 0; i < nx; ++i) {
+                La(k, j, i) = g.mu(k, j, i) * ((Da(k, j, i) - Da(k, j, i - 1)) / g.dxC(j) - (Za(k, j + 1, i) - Za(k, j, i)) / g.dy);
+                Lb(k, j, i) = g.mv(k, j, i) * ((Da(k, j, i) - Da(k, j - 1, i)) / g.dy + (Za(k, j, i + 1) - Za(k, j, i)) / g.dxF(j));
+            }
+    fill_halo(La, g.px, g.py); fill_halo(Lb, g.px, g.py);
+}
+
+void scalar_laplacian(const ocn_ref_grid& g, const A3& c, A3& Lc) {
+    const int nx = g.nx, ny = g.ny, nz = g.nz;
+#pragma omp parallel for schedule(static)
+    for (int j = 0; j < ny; ++j)
+        for (int k = 0; k < nz; ++k)
+            for (int i = 0; i < nx; ++i) {
+                const double fxw = g.dy * (c(k, j, i) - c(k, j, i - 1)) / g.dxC(j) * g.mu(k, j, i);
+                const double fxe = g.dy * (c(k, j, i + 1) - c(k, j, i)) / g.dxC(j) * g.mu(k, j, i + 1);
+                const double fys = g.dxF(j) * (c(k, j, i) - c(k, j - 1, i)) / g.dy * g.mv(k, j, i);
+                const double fyn = g.dxF(j + 1) * (c(k, j + 1, i) - c(k, j, i)) / g.dy * g.mv(k, j + 1, i);
+                Lc(k, j, i) = g.wet(k, j, i) * ((fxe - fxw) + (fyn - fys)) / g.AzC(j);
+            }
+    fill_halo(Lc, g.px, g.py);
+}
+
+// G_u += -nu4 La(La(u, v)), G_v likewise, G_c += -kappa4 Lc(Lc(c))   (each evaluated on its own and added to the tendency)
+void add_biharmonic(const ocn_ref_model& M, A3& Gu, A3& Gv, A3& GT, A3& GS) {
+    const ocn_ref_grid& g = *M.g;
+    const int nx = g.nx, ny = g.ny, nz = g.nz;
+    A3 l1, l2, m1, m2;
+    l1.init(nx, ny, nz); l2.init(nx, ny, nz); m1.init(nx, ny, nz); m2.init(nx, ny, nz);
+    if (M.d.nu4_h != 0.0) {
+        vector_laplacian(g, M.u, M.v, l1, l2);
+        vector_laplacian(g, l1, l2, m1, m2);
+        for (int k = 0; k < nz; ++k)
+            for (int j = 0; j < ny; ++j)
+                for (int i = 0; i < nx; ++i) {
+                    Gu(k, j, i) += -(M.d.nu4_h * m1(k, j, i));
+                    Gv(k, j, i) += -(M.d.nu4_h * m2(k, j, i));
+                }
+    }
+    if (M.d.kappa4_h != 0.0) {
+        const A3* c[2] = {&M.T, &M.S};
+        A3* G[2] = {&GT, &GS};
+        for (int f = 0; f < 2; ++f) {
+            scalar_laplacian(g, *c[f], l1);
+            scalar_laplacian(g, l1, m1);
+            for (int k = 0; k < nz; ++k)
+                for (int j = 0; j < ny; ++j)
+                    for (int i = 0; i < nx; ++i) (*G[f])(k, j, i) += -(M.d.kappa4_h * m1(k, j, i));
+        }
+    }
+}
+
 // state must be halo-filled and w, p consistent with it
 void compute_tendencies(ocn_ref_model& M, A3& Gu, A3& Gv, A3& GT, A3& GS) {
     const ocn_ref_grid& g = *M.g;
@@ -471,6 +547,7 @@ void compute_tendencies(ocn_ref_model& M, A3& Gu, A3& Gv, A3& GT, A3& GS) {
     momentum_tendency(M, Gu, Gv, t1, t2, t3);
     tracer_tendency(M, M.T, GT, t1, t2, t3, M.qT, M.rT, M.d.gamma_T);
     tracer_tendency(M, M.S, GS, t1, t2, t3, M.qS, M.rS, M.d.gamma_S);
+    if (M.d.nu4_h != 0.0 || M.d.kappa4_h != 0.0) add_biharmonic(M, Gu, Gv, GT, GS);
 }
 
 void fill_state_halos(ocn_ref_model& M) {
@@ -702,6 +779,7 @@ int ocn_ref_model_create(const ocn_ref_grid* g, const ocn_ref_model_desc* d, ocn
     if (!g || !d || !out) return fail("null argument");
     if (d->substeps < 1 || !(d->dt > 0)) return fail("bad dt / substeps");
     if (d->closure != 0 && d->closure != 1) return fail("closure must be 0 or 1");
+    if (!(d->nu4_h >= 0 && d->kappa4_h >= 0)) return fail("nu4_h, kappa4_h must be >= 0");
     if (d->eos != 0 && d->eos != 1) return fail("eos must be 0 (linear) or 1 (nonlinear)");
     if (d->advection != 0 && d->advection != 1) return fail("advection must be 0 (WENO-JS) or 1 (WENO-Z)");
     if (d->closure == 1 && !(d->ri_n2c > 0 && d->ri_s2min > 0 && d->ri_c >= 0 && d->ri_nu0 >= 0 && d->ri_kconv >= 0))

@@ -57,6 +57,8 @@ typedef struct {
     int advection;
     /* separate filter weights b_m (m = 1..M) for the barotropic transports U, V; NULL = the weights of eta */
     const double* filter_weights_uv;
+    /* biharmonic horizontal dissipation: viscosity nu4_h and diffusivity kappa4_h [m^4/s], 0 = off */
+    double nu4_h, kappa4_h;
 } ocn_ref_model_desc;
 
 typedef struct {

@@ -3,7 +3,7 @@ mask, a wrong sign — is applied to a scratch copy of oracle/ocn_ref.cpp, built
 against it in a subprocess (oracle/__init__.py loads the copy when OCN_REF_MUTANT_SRC is set).  Each mutant must make
 at least one pin FAIL; the unmodified source must pass.  This is what "pinned" means in DESIGN.md §5: a plausible mistake
 anywhere in the lat-lon metric factors or bathymetry masks of momentum_tendency, tracer_tendency, compute_w and
-barotropic_substep does not survive `-m "not gpu"`.  (The list is the one the round-1 review injected, plus a few more.
+barotropic_substep — and of the biharmonic operators (B1-B7) — does not survive `-m "not gpu"`.  (The list is the one the round-1 review injected, plus a few more.
 Not listed because they are EQUIVALENT mutants: dropping the open-face masks of U, V in barotropic_substep — a closed
 face has H = 0, G^U = 0 and starts from U = 0, so it stays 0 with or without the mask.)
 """
@@ -17,7 +17,7 @@ from concurrent.futures import ThreadPoolExecutor
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 SRC = os.path.join(ROOT, "oracle", "ocn_ref.cpp")
 # pins that the mutants are run against (fast ones first; -x stops at the first failure)
-PINS = ["tests/test_oracle_latlon.py", "tests/test_oracle_handcalc.py"]
+PINS = ["tests/test_oracle_latlon.py", "tests/test_oracle_handcalc.py", "tests/test_oracle_variants.py"]
 
 # (name, exact text in ocn_ref.cpp (must occur once), replacement)
 MUTANTS = [
@@ -76,8 +76,8 @@ MUTANTS = [
      "const double Cv = g.fF(j) * uhat;",
      "const double Cv = g.fF(j + 1) * uhat;"),
     ("M21 F_x diffusion: / dxC(j) -> / dxF(j)",
-     "(c(k, j, i) - c(k, j, i - 1)) / g.dxC(j) * g.mu(k, j, i);",
-     "(c(k, j, i) - c(k, j, i - 1)) / g.dxF(j) * g.mu(k, j, i);"),
+     "- kh * g.dy * g.dz[k] * (c(k, j, i) - c(k, j, i - 1)) / g.dxC(j) * g.mu(k, j, i);",
+     "- kh * g.dy * g.dz[k] * (c(k, j, i) - c(k, j, i - 1)) / g.dxF(j) * g.mu(k, j, i);"),
     ("M22 F_z: AzC(j) -> AzF(j)",
      "Fz(k, j, i) = ww * g.AzC(j) * cf * g.mw(k, j, i);",
      "Fz(k, j, i) = ww * g.AzF(j) * cf * g.mw(k, j, i);"),
@@ -90,6 +90,27 @@ MUTANTS = [
     ("M26 metric: fF at the cell centre instead of the corner",
      "g->fF_[r] = 2.0 * d->rotation_rate * std::sin(pf);",
      "g->fF_[r] = 2.0 * d->rotation_rate * std::sin(pc);"),
+    ("B1 biharmonic La: (Da[i]-Da[i-1]) / dxC(j) -> / dxF(j)",
+     "La(k, j, i) = g.mu(k, j, i) * ((Da(k, j, i) - Da(k, j, i - 1)) / g.dxC(j)",
+     "La(k, j, i) = g.mu(k, j, i) * ((Da(k, j, i) - Da(k, j, i - 1)) / g.dxF(j)"),
+    ("B2 biharmonic Za: dxC(j-1) a[j-1] -> dxC(j) a[j-1]",
+     "- (g.dxC(j) * a(k, j, i) - g.dxC(j - 1) * a(k, j - 1, i))) / g.AzF(j);",
+     "- (g.dxC(j) * a(k, j, i) - g.dxC(j) * a(k, j - 1, i))) / g.AzF(j);"),
+    ("B3 biharmonic Lb: (Za[i+1]-Za[i]) / dxF(j) -> / dxC(j)",
+     "+ (Za(k, j, i + 1) - Za(k, j, i)) / g.dxF(j));",
+     "+ (Za(k, j, i + 1) - Za(k, j, i)) / g.dxC(j));"),
+    ("B4 biharmonic Da: / AzC(j) -> / AzF(j)",
+     "g.dxF(j + 1) * b(k, j + 1, i) - g.dxF(j) * b(k, j, i)) / g.AzC(j);",
+     "g.dxF(j + 1) * b(k, j + 1, i) - g.dxF(j) * b(k, j, i)) / g.AzF(j);"),
+    ("B5 scalar Laplacian: northern flux with dxF(j) instead of dxF(j+1)",
+     "const double fyn = g.dxF(j + 1) * (c(k, j + 1, i) - c(k, j, i)) / g.dy * g.mv(k, j + 1, i);",
+     "const double fyn = g.dxF(j) * (c(k, j + 1, i) - c(k, j, i)) / g.dy * g.mv(k, j + 1, i);"),
+    ("B6 scalar Laplacian: eastern flux not masked",
+     "const double fxe = g.dy * (c(k, j, i + 1) - c(k, j, i)) / g.dxC(j) * g.mu(k, j, i + 1);",
+     "const double fxe = g.dy * (c(k, j, i + 1) - c(k, j, i)) / g.dxC(j);"),
+    ("B7 biharmonic: sign of the tracer term",
+     "(*G[f])(k, j, i) += -(M.d.kappa4_h * m1(k, j, i));",
+     "(*G[f])(k, j, i) += (M.d.kappa4_h * m1(k, j, i));"),
     ("control: 1/4 -> 1/2 in K",
      "Ke(k, j, i) = 0.25 * (u(k, j, i) * u(k, j, i) + u(k, j, i + 1) * u(k, j, i + 1))",
      "Ke(k, j, i) = 0.5 * (u(k, j, i) * u(k, j, i) + u(k, j, i + 1) * u(k, j, i + 1))"),

@@ -195,3 +195,130 @@ def test_transport_weights_leave_eta_filter_and_tracers_alone_but_change_the_flo
     f0, f1 = m0.get_fields(), m1.get_fields()
     assert np.array_equal(f0["eta"], f1["eta"]) and np.array_equal(f0["T"], f1["T"])     # first step: eta-bar and T do not see U-bar
     assert np.abs(f0["u"] - f1["u"]).max() > 1e-9
+
+
+# =============================================================================================
+# biharmonic horizontal dissipation
+# =============================================================================================
+def test_biharmonic_with_zero_coefficients_changes_nothing():
+    wl = W.config2(nx=48, ny=20, nz=10, steps=3)
+    w0 = dict(wl, params=dict(wl["params"], nu4_h=0.0, kappa4_h=0.0))
+    a, b = oracle.RefModel(wl), oracle.RefModel(w0)
+    a.step(3); b.step(3)
+    fa, fb = a.get_fields(), b.get_fields()
+    for n in ("u", "v", "w", "eta", "T", "S"):
+        assert np.array_equal(fa[n], fb[n]), n
+
+
+def test_biharmonic_plane_waves_closed_form_on_a_periodic_box():
+    """On a uniform doubly periodic box the discrete Laplacian of cos(k x) cos(l y) is lam * itself with
+    lam = -(4/dx^2) sin^2(k dx/2) - (4/dy^2) sin^2(l dy/2); applied twice: the biharmonic tendency is -coef * lam^2 * field.
+    Isolated as the difference between a model with and one without the term (everything else is identical)."""
+    nx, ny, nz, dx, dy = 16, 12, 3, 2000.0, 3000.0
+    x = (np.arange(nx) + 0.5) * dx; xf = np.arange(nx) * dx
+    y = (np.arange(ny) + 0.5) * dy; yf = np.arange(ny) * dy
+    kx, ly = 2 * np.pi * 2 / (nx * dx), 2 * np.pi * 1 / (ny * dy)
+    lam = -(4 / dx ** 2) * np.sin(kx * dx / 2) ** 2 - (4 / dy ** 2) * np.sin(ly * dy / 2) ** 2
+    nu4, k4 = 3.0e9, 1.5e9
+
+    def models(**fields):
+        out = []
+        for on in (0, 1):
+            wl = box(nx=nx, ny=ny, nz=nz, depth=300.0, dx=dx, dy=dy, f0=1e-4, nu_h=7.0, kappa_h=2.0,
+                     nu4_h=on * nu4, kappa4_h=on * k4)
+            for n, v in fields.items():
+                wl["fields"][n] = np.broadcast_to(v, (nz, ny, nx)).copy()
+            out.append(oracle.RefModel(wl).tendencies())
+        return out
+    c = 10.0 + 0.5 * np.cos(kx * x)[None, :] * np.cos(ly * y)[:, None]
+    u = 0.3 * np.cos(kx * xf)[None, :] * np.cos(ly * y)[:, None]            # u lives on west faces, v on south faces
+    v = 0.2 * np.cos(kx * x)[None, :] * np.cos(ly * yf)[:, None]
+    G0, G1 = models(T=c, S=35.0 - 0.1 * (c - 10.0), u=u, v=v)
+    for n, f, coef in (("GT", c - 10.0, k4), ("GS", -0.1 * (c - 10.0), k4), ("Gu", u, nu4), ("Gv", v, nu4)):
+        got = (G1[n] - G0[n])[1]
+        want = -coef * lam ** 2 * f
+        assert np.max(np.abs(got - want)) < 2e-9 * np.max(np.abs(want)), n      # difference of two O(1e-5..1e-3) tendencies
+    assert np.max(np.abs(-k4 * lam ** 2 * 0.5)) > 1e-8
+
+
+def _laplacians_from_the_pinned_second_order_terms(wl):
+    """L(u, v) and L(c) of a state obtained from the Laplacian viscosity / diffusion terms, which the lat-lon hand evaluator
+    of tests/test_oracle_latlon.py pins: G(coefficient 1) - G(coefficient 0) with the flow frozen."""
+    def G(nu_h, kappa_h):
+        w = dict(wl, params=dict(wl["params"], nu_h=nu_h, kappa_h=kappa_h, nu4_h=0.0, kappa4_h=0.0))
+        return oracle.RefModel(w).tendencies()
+    a, b = G(1.0, 1.0), G(0.0, 0.0)
+    return {n: a[n] - b[n] for n in a}
+
+
+def test_biharmonic_is_the_pinned_laplacian_applied_twice_on_the_sphere_with_land():
+    """<a, L b> = <L a, b> for the masked C-grid Laplacians on a lat-lon grid with land (sum by parts; areas dxC dy for u,
+    dxF dy for v, AzC for tracers), so  sum u . B(u) dA = -nu4 sum |L u|^2 dA  with L taken from the ALREADY PINNED
+    second-order term: a metric factor of the wrong row or a dropped mask in the second application breaks the identity."""
+    wl = W.config2(nx=40, ny=28, nz=5, steps=1)
+    rng = np.random.default_rng(12)
+    for n, amp in (("u", 0.3), ("v", 0.3), ("T", 2.0), ("S", 0.5)):
+        wl["fields"][n] = wl["fields"][n] + amp * rng.standard_normal(wl["fields"][n].shape)
+    wl["params"].update(nu_h=0.0, kappa_h=0.0)
+    L = _laplacians_from_the_pinned_second_order_terms(wl)
+    nu4, k4 = 2.0e12, 1.0e12
+    w1 = dict(wl, params=dict(wl["params"], nu4_h=nu4, kappa4_h=k4))
+    m0, m1 = oracle.RefModel(wl), oracle.RefModel(w1)
+    G0, G1, st = m0.tendencies(), m1.tendencies(), m0.get_fields()            # st: masked state
+    B = {n: G1[n] - G0[n] for n in G0}
+    g = wl["grid"]
+    a, dlam, dphi = g["radius"], np.deg2rad(g["dx"]), np.deg2rad(g["dy"])
+    pf = np.deg2rad(g["y0"] + np.arange(g["ny"] + 1) * g["dy"]); pc = 0.5 * (pf[1:] + pf[:-1])
+    Au = (a * np.cos(pc) * dlam * a * dphi)[None, :, None]
+    Av = (a * np.cos(pf[:-1]) * dlam * a * dphi)[None, :, None]
+    Ac = (a * a * dlam * (np.sin(pf[1:]) - np.sin(pf[:-1])))[None, :, None]
+    lhs = np.sum(st["u"] * B["Gu"] * Au + st["v"] * B["Gv"] * Av)
+    rhs = -nu4 * np.sum(L["Gu"] ** 2 * Au + L["Gv"] ** 2 * Av)
+    assert rhs < 0 and abs(lhs - rhs) < 1e-9 * abs(rhs), (lhs, rhs)
+    wet = m0.grid.masks()["wet"]
+    for n, c, c0 in (("GT", "T", 10.0), ("GS", "S", 35.0)):
+        # sum B A = 0 (flux form), so the constant part of the tracer drops out: take it out before it costs digits
+        lhs = np.sum((st[c] - c0) * wet * B[n] * Ac)
+        rhs = -k4 * np.sum(L[n] ** 2 * Ac)
+        assert abs(np.sum(B[n] * Ac)) < 1e-10 * np.sum(np.abs(B[n]) * Ac)       # B is a difference of two rounded tendencies
+        assert rhs < 0 and abs(lhs - rhs) < 1e-8 * abs(rhs), (n, lhs, rhs)
+    # and cross-wise with another field (symmetry, not only the quadratic form): <w, B(u)> = -nu4 <L w, L u>
+    wl2 = clone_fields(wl, rng)
+    L2 = _laplacians_from_the_pinned_second_order_terms(wl2)
+    st2 = oracle.RefModel(wl2).get_fields()
+    lhs = np.sum(st2["u"] * B["Gu"] * Au + st2["v"] * B["Gv"] * Av)
+    rhs = -nu4 * np.sum(L2["Gu"] * L["Gu"] * Au + L2["Gv"] * L["Gv"] * Av)
+    assert abs(lhs - rhs) < 1e-9 * abs(rhs), (lhs, rhs)
+    lhs = np.sum((st2["T"] - 10.0) * wet * B["GT"] * Ac); rhs = -k4 * np.sum(L2["GT"] * L["GT"] * Ac)
+    assert abs(lhs - rhs) < 1e-8 * abs(rhs)
+
+
+def clone_fields(wl, rng):
+    w = dict(wl, fields={k: v.copy() for k, v in wl["fields"].items()})
+    for n, amp in (("u", 0.3), ("v", 0.3), ("T", 2.0)):
+        w["fields"][n] = w["fields"][n] + amp * rng.standard_normal(w["fields"][n].shape)
+    return w
+
+
+def test_biharmonic_diffusion_conserves_tracers_and_damps_grid_noise():
+    wl = W.config2(nx=48, ny=24, nz=6, steps=8)
+    rng = np.random.default_rng(4)
+    wl["fields"]["T"] = wl["fields"]["T"] + 0.5 * rng.standard_normal(wl["fields"]["T"].shape)
+    dxmin = wl["grid"]["radius"] * np.deg2rad(wl["grid"]["dx"]) * np.cos(np.deg2rad(75.0))
+    k4 = 0.01 * dxmin ** 4 / wl["params"]["dt"]                                   # well inside the explicit stability limit
+    wl["params"].update(kappa_h=0.0, kappa4_h=k4, nu4_h=k4)
+    m = oracle.RefModel(wl)
+    vol = m.grid.masks()["wet"] * np.diff(wl["z_faces"])[:, None, None] * m.grid.metrics()["AzC"][None, :, None]
+    f0 = m.get_fields()
+    m.step(8)
+    f1 = m.get_fields()
+    for n in "TS":
+        assert abs(np.sum(vol * f1[n]) / np.sum(vol * f0[n]) - 1.0) < 2e-14, n
+    # grid-scale roughness along x in the polar rows (where dx is smallest and the coefficient bites), over wet triples only
+    wet = m.grid.masks()["wet"].astype(bool)
+    ok = (wet[:, :, 2:] & wet[:, :, 1:-1] & wet[:, :, :-2])
+    rows = np.r_[0:3, 21:24]
+    lap = lambda a: np.abs(a[:, :, 2:] - 2 * a[:, :, 1:-1] + a[:, :, :-2])[:, rows][ok[:, rows]].mean()      # noqa: E731
+    ref = dict(wl, params=dict(wl["params"], kappa4_h=0.0, nu4_h=0.0))
+    r = oracle.RefModel(ref); r.step(8)
+    assert ok[:, rows].sum() > 100 and lap(f1["T"]) < 0.9 * lap(r.get_fields()["T"])
