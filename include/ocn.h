@@ -102,6 +102,10 @@ typedef struct {
      * doubles that sum to 1, or NULL = the weights of eta (filter_weights).  eta-bar = sum a_m eta^m, U-bar = sum b_m U^m,
      * V-bar likewise; dtau is still set by the first moment of a.  Copied at creation. */
     const double* filter_weights_uv;
+    /* Biharmonic horizontal dissipation: viscosity nu4_h and tracer diffusivity kappa4_h
+     * [m^4/s], >= 0, 0 = off.  G -= coefficient x L(L(.)) with the masked C-grid Laplacians of the second-order terms.
+     * Costs two pre-pass launches per step and four more 3-D pair arrays; the default path is unchanged. */
+    double nu4_h, kappa4_h;
 } ocn_model_desc;
 
 /* ocn_model_create — the model of PAPER.md:84 (§5.2: hydrostatic Boussinesq, IMEX quasi-AB2, backward-Euler vertical

@@ -80,6 +80,9 @@ struct DevP {
     int eos;
     const double* ath_d;
     double ha2_d;
+    // biharmonic horizontal dissipation: scratch Laplacians and the finished terms K1 adds (bih = 1 only)
+    int bih;
+    T2 *Luv, *Lts, *Buv, *Bts;
     // K1: wet cells of a tile-level from which on the tile is marched with geometric ownership
     int geo_thr;
     unsigned long long* timeline;   // [8 warps][8]: cycles per phase + iterations (filled by OCN_K1_TIMELINE builds only)

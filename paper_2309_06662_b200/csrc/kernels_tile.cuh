@@ -419,6 +419,13 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
         T gm_u = 0, gm_v = 0;
         T piv_t = 1, piv_u = 1, piv_v = 1;
         const long long okB = (long long)kB * sz;             // warp-uniform level base; the column offsets are 32-bit
+        T2 bih_ts = mk2(T(0), T(0));                          // biharmonic terms of the own cell (pre-pass)
+        T bih_u = 0, bih_v = 0;
+        if (P.bih && anyB) {
+            if (wetT) bih_ts = (P.Bts + okB)[XT.c];
+            if (wetU) bih_u = ((const T*)(P.Buv + okB + XU.c))[0];
+            if (wetV) bih_v = ((const T*)(P.Buv + okB + XV.c))[1];
+        }
         if (anyB) {
             if (wetT) {
                 gm_ts = (P.Gts + okB)[XT.c];
@@ -582,6 +589,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                     GT = (X(GT) + xdiv(X(qf.x) + X(P.gamma_T) * (X(rtg.x) - X(tsc.x)), dzk, rdzk)).v;
                     GS = (X(GS) + xdiv(X(qf.y) + X(P.gamma_S) * (X(rtg.y) - X(tsc.y)), dzk, rdzk)).v;
                 }
+                if (P.bih) { GT = (X(GT) + X(bih_ts.x)).v; GS = (X(GS) + X(bih_ts.y)).v; }
                 // ---- quasi-AB2, predictor, elimination sweep (S3, S4) ----
                 const T Ght = (X(c0) * X(GT) - X(c1) * X(gm_ts.x)).v, Ghs = (X(c0) * X(GS) - X(c1) * X(gm_ts.y)).v;
                 (P.Gts + okB)[XT.c] = mk2(GT, GS);
@@ -639,6 +647,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                     const Xv<T> drag(k == tx1 ? xdiv((X(P.drag_r) + X(P.drag_cd) * X((T)sqrt((X(u_c) * X(u_c) + X(vhat) * X(vhat)).v))) * X(u_c), dzk, rdzk).v : T(0));
                     Gu = (X(Gu) - drag).v;
                 }
+                if (P.bih) Gu = (X(Gu) + X(bih_u)).v;
                 // ---- quasi-AB2, predictor, elimination sweep (S3, S4, S5) ----
                 const T Ghu = (X(c0) * X(Gu) - X(c1) * X(gm_u)).v;
                 const T us = E::add(u_c, E::mul(P.dt, Ghu));
@@ -697,6 +706,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                     const Xv<T> drag(k == ty1 ? xdiv((X(P.drag_r) + X(P.drag_cd) * X((T)sqrt((X(uhat) * X(uhat) + X(v_c) * X(v_c)).v))) * X(v_c), dzk, rdzk).v : T(0));
                     Gv = (X(Gv) - drag).v;
                 }
+                if (P.bih) Gv = (X(Gv) + X(bih_v)).v;
                 const T Ghv = (X(c0) * X(Gv) - X(c1) * X(gm_v)).v;
                 const T vs2 = E::add(v_c, E::mul(P.dt, Ghv));
                 aGV = (X(aGV) + X((double)dzk) * X((double)Ghv)).v; aSV = (X(aSV) + X((double)dzk) * X((double)vs2)).v;

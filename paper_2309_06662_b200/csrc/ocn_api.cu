@@ -16,6 +16,7 @@
 #include "kernels_column.cuh"
 #include "kernels_tile.cuh"
 #include "kernels_mixing.cuh"
+#include "kernels_biharmonic.cuh"
 
 // Scratch of the allocation-free entry point ocn_get_mixing_noalloc (include/ocn.h): the halo'd (nu, kappa) pair array that
 // k_ri_mixing writes before it is gathered into the caller's buffers.  A file-scope device array of a fixed, modest size:
@@ -208,6 +209,12 @@ ocn_status build_model(ocn_model* M) {
     if (M->d.closure == 1) {                       // the per-column super-diagonals K1 leaves for K3
         if ((s = dev_alloc(M, n3, &P.cpuv, true)) != OCN_OK || (s = dev_alloc(M, n3, &P.cpt, true)) != OCN_OK) return s;
     }                                              // (nu, kappa) as an output array: allocated by the first ocn_get_mixing
+    P.bih = (M->d.nu4_h != 0.0 || M->d.kappa4_h != 0.0) ? 1 : 0;
+    P.Luv = P.Lts = P.Buv = P.Bts = nullptr;
+    if (P.bih) {                                   // two scratch Laplacians and the two finished terms
+        T2** fb[] = {&P.Luv, &P.Lts, &P.Buv, &P.Bts};
+        for (T2** f : fb) if ((s = dev_alloc(M, n3, f, true)) != OCN_OK) return s;
+    }
     P.ri_nu0 = M->d.ri_nu0; P.ri_c = M->d.ri_c; P.ri_kconv = M->d.ri_kconv; P.ri_n2c = M->d.ri_n2c; P.ri_s2min = M->d.ri_s2min;
     P.nu_z_d = M->d.nu_z; P.kappa_z_d = M->d.kappa_z;
     T** f2[] = {&P.eta[0], &P.eta[1], &P.U[0], &P.U[1], &P.V[0], &P.V[1], &P.etab, &P.Ub, &P.Vb, &P.GU, &P.GV,
@@ -325,7 +332,7 @@ ocn_status build_model(ocn_model* M) {
         CK(cudaStreamCreateWithFlags(&M->copy_stream, cudaStreamNonBlocking));
         for (auto& e : M->ticket_ev) CK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     }
-    M->launches_per_step = (M->d.substeps + bt_substeps_per_launch<T>() - 1) / bt_substeps_per_launch<T>() + 3;
+    M->launches_per_step = (M->d.substeps + bt_substeps_per_launch<T>() - 1) / bt_substeps_per_launch<T>() + 3 + (P.bih ? 2 : 0);
     // TMA descriptors: box origin (i0 - 4, j0 - 3), so the map starts 4 elements before (row -3, i = 0)
     {
         typedef ocn::Tile<T, TILE_X, TILE_Y> C;
@@ -395,10 +402,14 @@ ocn_status launch_step(ocn_model* M, bool euler) {
     MARK(-1, 0);
     {
         const dim3 bt(TILE_X, TILE_Y), gt = grid2(g, bt);
+        if (P.bih) {                               // biharmonic pre-pass: L of the state, then -coefficient L(L)
+            ocn::k_laplacians<T><<<grid2(g, bc), bc, 0, M->stream>>>(P, P.uv, P.ts, P.Luv, P.Lts, T(1), T(1), 0);
+            ocn::k_laplacians<T><<<grid2(g, bc), bc, 0, M->stream>>>(P, P.Luv, P.Lts, P.Buv, P.Bts, (T)M->d.nu4_h, (T)M->d.kappa4_h, 1);
+        }
         const bool drag = M->d.drag_r != 0.0 || M->d.drag_cd != 0.0, ri = M->d.closure == 1, wz = M->d.advection == 1;
         k1_fused<T>(drag, ri, wz)<<<gt, bt, k1_smem<T>(ri), M->stream>>>(P, c0, c1, M->tm_ts, M->tm_uv, M->tm_p);
     }
-    MARK(0, 1);
+    MARK(0, P.bih ? 3 : 1);
     if constexpr (sizeof(T) == 4) {                // register-strip kernel, BS_H sub-steps per launch
         typedef ocn::BtStrip<BS_X, BS_Y, BS_H> B;
         const dim3 gb((g->nx + BS_X - 1) / BS_X, (g->ny + BS_Y - 1) / BS_Y);
@@ -719,6 +730,8 @@ ocn_status ocn_model_create(const ocn_grid* g, const ocn_model_desc* d, ocn_mode
     if (!(d->gamma_T >= 0) || !(d->gamma_S >= 0)) return fail(OCN_EINVAL, "gamma_T, gamma_S must be >= 0");
     if (!(d->drag_r >= 0) || !(d->drag_cd >= 0)) return fail(OCN_EINVAL, "drag_r, drag_cd must be >= 0");
     if (d->closure != 0 && d->closure != 1) return fail(OCN_EINVAL, "closure must be 0 (constant) or 1 (Ri-based)");
+    if (!(d->nu4_h >= 0 && d->kappa4_h >= 0) || !std::isfinite(d->nu4_h) || !std::isfinite(d->kappa4_h))
+        return fail(OCN_EINVAL, "nu4_h, kappa4_h must be finite and >= 0");
     if (d->eos != 0 && d->eos != 1) return fail(OCN_EINVAL, "eos must be 0 (linear) or 1 (nonlinear)");
     if (d->eos == 1 && !(std::isfinite(d->eos_alpha2) && std::isfinite(d->eos_gamma))) return fail(OCN_EINVAL, "eos_alpha2, eos_gamma must be finite");
     if (d->advection != 0 && d->advection != 1) return fail(OCN_EINVAL, "advection must be 0 (WENO-JS) or 1 (WENO-Z)");

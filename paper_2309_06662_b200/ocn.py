@@ -36,7 +36,7 @@ class ocn_model_desc(C.Structure):
                 ("ri_n2c", C.c_double), ("ri_s2min", C.c_double), ("gamma_T", C.c_double), ("gamma_S", C.c_double),
                 ("drag_r", C.c_double), ("drag_cd", C.c_double),
                 ("eos", C.c_int), ("eos_alpha2", C.c_double), ("eos_gamma", C.c_double), ("advection", C.c_int),
-                ("filter_weights_uv", C.POINTER(C.c_double))]
+                ("filter_weights_uv", C.POINTER(C.c_double)), ("nu4_h", C.c_double), ("kappa4_h", C.c_double)]
 
 
 class ocn_fields(C.Structure):

@@ -122,3 +122,55 @@ def test_separate_transport_filter_weights(prec):
     gpu.close(); plain.close()
     with pytest.raises(RuntimeError, match="filter_weights_uv"):
         ocn.Model(wl, filter_weights_uv=2.0 * b)
+
+
+def _bih(wl, frac=0.01):
+    g = wl["grid"]
+    dxmin = g["radius"] * np.deg2rad(g["dx"]) * np.cos(np.deg2rad(max(abs(g["y0"]), abs(g["y0"] + g["ny"] * g["dy"])) - 0.5 * g["dy"]))
+    k4 = frac * dxmin ** 4 / wl["params"]["dt"]
+    wl["params"].update(nu4_h=float(k4), kappa4_h=float(0.5 * k4))
+    wl["name"] = wl.get("name", "") + "+bih"
+    return wl
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+@pytest.mark.parametrize("closure", [0, 1])
+def test_biharmonic_dissipation(prec, closure):
+    """nu4_h, kappa4_h: the pre-pass kernel pair + the add in K1 against the oracle on a lat-lon grid with
+    land, periodic in x, noisy state (so that the term is large); fp64 bit-identical, fp32 within 2e-4."""
+    wl = _bih(_stirred(W.config2(nx=180, ny=75, nz=25, steps=6, precision=prec)))
+    if closure:
+        W.with_ri_closure(wl)
+    ref, gpu = oracle.RefModel(wl), ocn.Model(wl)
+    off = ocn.Model(dict(wl, params=dict(wl["params"], nu4_h=0.0, kappa4_h=0.0)))
+    assert gpu.info()["launches_per_step"] == off.info()["launches_per_step"] + 2
+    G = ref.tendencies()
+    ref.step(1); gpu.time_step(1); off.time_step(1)
+    d, d0 = gpu.debug(), off.debug()
+    for n in ("Gu", "Gv", "GT", "GS"):                          # first-step tendencies: the term is visible
+        assert np.abs(d[n] - d0[n]).max() > 0.0, n             # the term is there (its size is pinned on the oracle side)
+        if prec == 64:
+            assert np.array_equal(d[n], G[n]), (n, rel_linf(d[n], G[n]))
+    ref.step(5); gpu.time_step(5)
+    a, r = gpu.get_fields(), ref.get_fields()
+    errs = {n: rel_linf(a[n], r[n]) for n in FIELDS}
+    if prec == 64:
+        for n in FIELDS:
+            assert np.array_equal(a[n], r[n]), (n, errs[n])
+    else:
+        report_parity("biharmonic%s 180x75x25 fp32" % ("+ri" if closure else ""), 6, errs)
+        assert all(e <= 2e-4 for e in errs.values()), errs
+    gpu.close(); off.close()
+
+
+def test_biharmonic_on_small_periodic_and_walled_boxes_fp64():
+    for nx, ny, per in ((5, 4, (1, 1)), (33, 9, (1, 0)), (12, 10, (0, 0))):
+        wl = W.config0(nx=nx, ny=ny, nz=3)
+        wl["grid"]["periodic_x"], wl["grid"]["periodic_y"] = per
+        wl["params"].update(nu4_h=1.0e8, kappa4_h=5.0e7)
+        ref, gpu = oracle.RefModel(wl), ocn.Model(wl)
+        ref.step(4); gpu.time_step(4)
+        a, r = gpu.get_fields(), ref.get_fields()
+        for n in FIELDS:
+            assert np.array_equal(a[n], r[n]), (nx, ny, per, n, rel_linf(a[n], r[n]))
+        gpu.close()
