@@ -68,6 +68,7 @@ struct DevP {
     double g_d, alpha_d, beta_d, dT0_d, dS0_d, hz_top_d;   // fp64 copies for the pressure integral
     const double* dzc_d;
     T dtau;
+    const T *fw_a, *fw_b;  // filter weights a_m of eta and b_m of the transports, m = 1..M at index m - 1
     // Ri-based vertical mixing closure, closure = 1 only: (nu, kappa) at the bottom face of
     // tracer cell (k, j, i) as a pair array, and the modified super-diagonals of the per-column Thomas solves
     int closure;

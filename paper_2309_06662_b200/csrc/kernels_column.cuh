@@ -39,21 +39,19 @@ __device__ __forceinline__ double pressure_level(const DevP<T>& P, int k, double
 #define BT_HALO 6                  // sub-steps per launch = halo rings of the resident tile (<= 6: the launch carries six weights)
 #endif
 
-// filter weights of the sub-steps of one launch: a for eta, b for the transports U, V (b = a unless
-// the model was given filter_weights_uv)
+// most sub-steps one launch advances (the filter weights of the launch, a for eta and b for the transports U, V, DESIGN.md
+// §3.9, §3.17, are staged from the model's device tables into shared memory)
 #define BT_MAXW 12
-template <class T> struct BtWeights { T a[BT_MAXW], b[BT_MAXW]; };
 
 template <class T, int BTX, int BTY>
 struct BtTile {
     static constexpr int EX = BTX + 2 * BT_HALO, EY = BTY + 2 * BT_HALO, NE = EX * EY;
     static constexpr int NT = BTX * BTY >= 2048 ? 1024 : 512, PER = (NE + NT - 1) / NT;      // extended-tile points per thread
-    static constexpr int SMEM = NE * (7 * (int)sizeof(T) + 1) + 6 * (EY + 1) * (int)sizeof(T) + 64 + BT_HALO * (int)sizeof(T);
+    static constexpr int SMEM = NE * (7 * (int)sizeof(T) + 1) + 6 * (EY + 1) * (int)sizeof(T) + 64 + 2 * BT_HALO * (int)sizeof(T);
 };
 
 template <class T, int BTX, int BTY>
-__global__ void __launch_bounds__((BtTile<T, BTX, BTY>::NT)) k_barotropic_tile(const DevP<T> P, const int cur, const int ns, const int first,
-                                                         const BtWeights<T> W) {
+__global__ void __launch_bounds__((BtTile<T, BTX, BTY>::NT)) k_barotropic_tile(const DevP<T> P, const int cur, const int ns, const int first, const int m0) {
     typedef BtTile<T, BTX, BTY> C;
     constexpr int EX = C::EX, EY = C::EY, NE = C::NE, NT = C::NT, H = BT_HALO;
     extern __shared__ __align__(16) unsigned char smb[];
@@ -69,15 +67,13 @@ __global__ void __launch_bounds__((BtTile<T, BTX, BTY>::NT)) k_barotropic_tile(c
     T* const dF = rdx + (EY + 1);          // EY + 1 entries
     T* const Az = dF + (EY + 1);           // AzC, dxC per extended row (fp64 divides, fp32 multiplies by the reciprocals)
     T* const dxc = Az + (EY + 1);
-    T* const saw = dxc + (EY + 1);         // filter weights of this launch
-    unsigned char* const smk = (unsigned char*)(saw + BT_HALO);   // bit 0 wet, bit 1 open u face, bit 2 open v face
+    T* const saw = dxc + (EY + 1);         // filter weights of this launch: a (eta), then b (transports)
+    T* const sbw = saw + BT_HALO;
+    unsigned char* const smk = (unsigned char*)(sbw + BT_HALO);   // bit 0 wet, bit 1 open u face, bit 2 open v face
     const int tid = threadIdx.x;
     const int i0 = blockIdx.x * BTX, j0 = blockIdx.y * BTY;
     const int nx = P.nx, ny = P.ny, nz = P.nz, sx = P.sx;
-    if (tid == 0) {
-#pragma unroll
-        for (int q = 0; q < BT_HALO; ++q) saw[q] = W.a[q];
-    }
+    if (tid < ns) { saw[tid] = P.fw_a[m0 + tid]; sbw[tid] = P.fw_b[m0 + tid]; }
 
     // ---- load the extended tile (wrap / land) ----
     for (int q = tid; q <= EY; q += NT) {
@@ -172,7 +168,7 @@ __global__ void __launch_bounds__((BtTile<T, BTX, BTY>::NT)) k_barotropic_tile(c
                 }
             }
             __syncthreads();
-            const T am = saw[s], bm = W.b[s];
+            const T am = saw[s], bm = sbw[s];
 #pragma unroll
             for (int n = 0; n < C::PER; ++n) {
                 const int q = n * NT + tid;
@@ -196,7 +192,7 @@ __global__ void __launch_bounds__((BtTile<T, BTX, BTY>::NT)) k_barotropic_tile(c
                                          Az[y], rAz[y])).v;
         }
         __syncthreads();
-        const T am = saw[s], bm = W.b[s];
+        const T am = saw[s], bm = sbw[s];
 #pragma unroll
         for (int n = 0; n < C::PER; ++n) {
             const int q = n * NT + tid;
@@ -243,12 +239,12 @@ struct BtStrip {
     static_assert(EX % 4 == 0, "extended row must be a whole number of strips");
     static constexpr int NT = (NS + 31) / 32 * 32;
     static_assert(NT <= 1024, "one strip per thread");
-    static constexpr int SMEM = 3 * EX * EY * 4 + 2 * (EY + 1) * 4 + 16;
+    static constexpr int SMEM = 3 * EX * EY * 4 + 2 * (EY + 1) * 4 + 16 + 2 * BT_MAXW * 4;
 };
 
 template <int BTX, int BTY, int H>
 __global__ void __launch_bounds__((BtStrip<BTX, BTY, H>::NT), 1)
-k_barotropic_strip(const DevP<float> P, const int cur, const int ns, const int first, const BtWeights<float> W) {
+k_barotropic_strip(const DevP<float> P, const int cur, const int ns, const int first, const int m0) {
     typedef BtStrip<BTX, BTY, H> C;
     constexpr int EX = C::EX, EY = C::EY, SPR = C::SPR;
     extern __shared__ __align__(16) unsigned char smb[];
@@ -257,6 +253,8 @@ k_barotropic_strip(const DevP<float> P, const int cur, const int ns, const int f
     float* const sV = sU + EX * EY;
     float* const dF = sV + EX * EY;                 // dxF per extended row, EY + 1 entries
     float* const rAz = dF + (EY + 1);               // 1 / AzC per extended row
+    float* const saw = rAz + (EY + 1) + 2;          // filter weights of this launch: a (eta), then b (transports)
+    float* const sbw = saw + BT_MAXW;
     const int tid = threadIdx.x;
     const int i0 = blockIdx.x * BTX, j0 = blockIdx.y * BTY;
     const int nx = P.nx, ny = P.ny, nz = P.nz, sx = P.sx;
@@ -267,6 +265,7 @@ k_barotropic_strip(const DevP<float> P, const int cur, const int ns, const int f
         dF[q] = P.dxF[r];
         if (q < EY) rAz[q] = P.rAzC[r];
     }
+    if (tid < ns) { saw[tid] = P.fw_a[m0 + tid]; sbw[tid] = P.fw_b[m0 + tid]; }
     const bool on = tid < C::NS;
     const int y = on ? tid / SPR : 0, x0 = on ? 4 * (tid % SPR) : 0;
     const int qb = y * EX + x0;                     // first point of the strip in the extended tile
@@ -325,7 +324,7 @@ k_barotropic_strip(const DevP<float> P, const int cur, const int ns, const int f
         }
         __syncthreads();
         if (on) {
-            const float am = W.a[s], bm = W.b[s];
+            const float am = saw[s], bm = sbw[s];
             const float ew = se[qw];
             const float4 es = *(const float4*)(se + qs);
             u[0] = u[0] + (cu[0] * (ew - e[0]) + gu[0]);

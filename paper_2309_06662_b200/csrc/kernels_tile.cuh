@@ -107,8 +107,9 @@ struct Tile {
 };
 
 
-// DRAG: compiled with the bottom-drag term of DESIGN.md §3.14 (chosen by the host when drag_r or drag_cd is non-zero, so
-// that the default path does not carry its instructions: 10.17 ms against 10.37 ms with the term predicated off).
+// DRAG: the "extras" instantiation: compiled with the bottom-drag term of DESIGN.md §3.14 and the add of the biharmonic terms
+// of §3.18 (chosen by the host when drag_r, drag_cd, nu4_h or kappa4_h is non-zero, so that the default path does not carry
+// their instructions: the drag term predicated off cost 2 %, the biharmonic flag 3 % of the default kernel).
 // RI: the Ri-based closure evaluated in the pass (per-face diffusivities, per-column elimination in registers, the modified
 // super-diagonals stored for K3).  WZ: WENO-Z nonlinear weights instead of Jiang-Shu's.
 template <class T, int TX, int TY, int MINB, bool DRAG = false, bool RI = false, bool WZ = false>
@@ -421,7 +422,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
         const long long okB = (long long)kB * sz;             // warp-uniform level base; the column offsets are 32-bit
         T2 bih_ts = mk2(T(0), T(0));                          // biharmonic terms of the own cell (pre-pass)
         T bih_u = 0, bih_v = 0;
-        if (P.bih && anyB) {
+        if (DRAG && P.bih && anyB) {                          // (the extras instantiation; the default one has no trace of it)
             if (wetT) bih_ts = (P.Bts + okB)[XT.c];
             if (wetU) bih_u = ((const T*)(P.Buv + okB + XU.c))[0];
             if (wetV) bih_v = ((const T*)(P.Buv + okB + XV.c))[1];
@@ -589,7 +590,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                     GT = (X(GT) + xdiv(X(qf.x) + X(P.gamma_T) * (X(rtg.x) - X(tsc.x)), dzk, rdzk)).v;
                     GS = (X(GS) + xdiv(X(qf.y) + X(P.gamma_S) * (X(rtg.y) - X(tsc.y)), dzk, rdzk)).v;
                 }
-                if (P.bih) { GT = (X(GT) + X(bih_ts.x)).v; GS = (X(GS) + X(bih_ts.y)).v; }
+                if constexpr (DRAG) if (P.bih) { GT = (X(GT) + X(bih_ts.x)).v; GS = (X(GS) + X(bih_ts.y)).v; }
                 // ---- quasi-AB2, predictor, elimination sweep (S3, S4) ----
                 const T Ght = (X(c0) * X(GT) - X(c1) * X(gm_ts.x)).v, Ghs = (X(c0) * X(GS) - X(c1) * X(gm_ts.y)).v;
                 (P.Gts + okB)[XT.c] = mk2(GT, GS);
@@ -647,7 +648,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                     const Xv<T> drag(k == tx1 ? xdiv((X(P.drag_r) + X(P.drag_cd) * X((T)sqrt((X(u_c) * X(u_c) + X(vhat) * X(vhat)).v))) * X(u_c), dzk, rdzk).v : T(0));
                     Gu = (X(Gu) - drag).v;
                 }
-                if (P.bih) Gu = (X(Gu) + X(bih_u)).v;
+                if constexpr (DRAG) if (P.bih) Gu = (X(Gu) + X(bih_u)).v;
                 // ---- quasi-AB2, predictor, elimination sweep (S3, S4, S5) ----
                 const T Ghu = (X(c0) * X(Gu) - X(c1) * X(gm_u)).v;
                 const T us = E::add(u_c, E::mul(P.dt, Ghu));
@@ -706,7 +707,7 @@ k_tendency_tile(const DevP<T> P, const T c0, const T c1, const __grid_constant__
                     const Xv<T> drag(k == ty1 ? xdiv((X(P.drag_r) + X(P.drag_cd) * X((T)sqrt((X(uhat) * X(uhat) + X(v_c) * X(v_c)).v))) * X(v_c), dzk, rdzk).v : T(0));
                     Gv = (X(Gv) - drag).v;
                 }
-                if (P.bih) Gv = (X(Gv) + X(bih_v)).v;
+                if constexpr (DRAG) if (P.bih) Gv = (X(Gv) + X(bih_v)).v;
                 const T Ghv = (X(c0) * X(Gv) - X(c1) * X(gm_v)).v;
                 const T vs2 = E::add(v_c, E::mul(P.dt, Ghv));
                 aGV = (X(aGV) + X((double)dzk) * X((double)Ghv)).v; aSV = (X(aSV) + X((double)dzk) * X((double)vs2)).v;

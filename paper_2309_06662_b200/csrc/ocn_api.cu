@@ -288,6 +288,7 @@ ocn_status build_model(ocn_model* M) {
     P.g_d = M->d.g; P.alpha_d = M->d.alpha; P.beta_d = M->d.beta_s; P.hz_top_d = g->zf[nz] - g->zc[nz - 1];
     P.dT0_d = M->d.T0 - (double)P.Toff; P.dS0_d = M->d.S0 - (double)P.Soff;
     P.nu_h = (T)M->d.nu_h; P.kappa_h = (T)M->d.kappa_h; P.dtau = (T)M->dtau;
+    if ((s = upload(M, M->a_w, &P.fw_a)) != OCN_OK || (s = upload(M, M->b_w, &P.fw_b)) != OCN_OK) return s;
     // equation of state: per-level thermal expansion alpha (1 - gamma zc[k]) and alpha2 / 2, in the fp64
     // operations the equation is written in
     if ((s = dev_alloc(M, 64, &P.timeline, false)) != OCN_OK) return s;
@@ -406,7 +407,8 @@ ocn_status launch_step(ocn_model* M, bool euler) {
             ocn::k_laplacians<T><<<grid2(g, bc), bc, 0, M->stream>>>(P, P.uv, P.ts, P.Luv, P.Lts, T(1), T(1), 0);
             ocn::k_laplacians<T><<<grid2(g, bc), bc, 0, M->stream>>>(P, P.Luv, P.Lts, P.Buv, P.Bts, (T)M->d.nu4_h, (T)M->d.kappa4_h, 1);
         }
-        const bool drag = M->d.drag_r != 0.0 || M->d.drag_cd != 0.0, ri = M->d.closure == 1, wz = M->d.advection == 1;
+        // the extras instantiation carries bottom drag and the biharmonic add
+        const bool drag = M->d.drag_r != 0.0 || M->d.drag_cd != 0.0 || P.bih, ri = M->d.closure == 1, wz = M->d.advection == 1;
         k1_fused<T>(drag, ri, wz)<<<gt, bt, k1_smem<T>(ri), M->stream>>>(P, c0, c1, M->tm_ts, M->tm_uv, M->tm_p);
     }
     MARK(0, P.bih ? 3 : 1);
@@ -416,9 +418,7 @@ ocn_status launch_step(ocn_model* M, bool euler) {
         int cur = 0;
         for (int m0 = 0; m0 < M->d.substeps; m0 += BS_H) {
             const int ns = std::min(BS_H, M->d.substeps - m0);
-            ocn::BtWeights<float> W{};
-            for (int q = 0; q < ns; ++q) { W.a[q] = (float)M->a_w[m0 + q]; W.b[q] = (float)M->b_w[m0 + q]; }
-            ocn::k_barotropic_strip<BS_X, BS_Y, BS_H><<<gb, B::NT, B::SMEM, M->stream>>>(P, cur, ns, m0 == 0 ? 1 : 0, W);
+            ocn::k_barotropic_strip<BS_X, BS_Y, BS_H><<<gb, B::NT, B::SMEM, M->stream>>>(P, cur, ns, m0 == 0 ? 1 : 0, m0);
             cur ^= 1;
         }
     } else {
@@ -427,9 +427,7 @@ ocn_status launch_step(ocn_model* M, bool euler) {
         int cur = 0;
         for (int m0 = 0; m0 < M->d.substeps; m0 += BT_HALO) {
             const int ns = std::min(BT_HALO, M->d.substeps - m0);
-            ocn::BtWeights<T> W{};
-            for (int q = 0; q < ns; ++q) { W.a[q] = (T)M->a_w[m0 + q]; W.b[q] = (T)M->b_w[m0 + q]; }
-            ocn::k_barotropic_tile<T, BT_X, BT_Y><<<gb, B::NT, B::SMEM, M->stream>>>(P, cur, ns, m0 == 0 ? 1 : 0, W);
+            ocn::k_barotropic_tile<T, BT_X, BT_Y><<<gb, B::NT, B::SMEM, M->stream>>>(P, cur, ns, m0 == 0 ? 1 : 0, m0);
             cur ^= 1;
         }
     }
