@@ -243,7 +243,7 @@ struct BtStrip {
 };
 
 template <int BTX, int BTY, int H>
-__global__ void __launch_bounds__((BtStrip<BTX, BTY, H>::NT), 1)
+__global__ void __launch_bounds__((BtStrip<BTX, BTY, H>::NT), (1024 / BtStrip<BTX, BTY, H>::NT))
 k_barotropic_strip(const DevP<float> P, const int cur, const int ns, const int first, const int m0) {
     typedef BtStrip<BTX, BTY, H> C;
     constexpr int EX = C::EX, EY = C::EY, SPR = C::SPR;
