@@ -60,6 +60,7 @@ def parse():
     ap.add_argument("--closure", default="const", choices=["const", "ri"],
                     help="vertical mixing: constant coefficients (default, the north_star path) or the Ri-based closure "
                          "of PAPER.md:114 (SURVEY 8f-1; DESIGN.md §3.12)")
+    ap.add_argument("--patch", default="16x4", help="config 6 only (kernel analysis): WxH ocean patch of every 32x8 tile")
     ap.add_argument("--no-e2e", action="store_true", help="skip the end-to-end (host buffer) leg")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-closure-leg", action="store_true", help="skip the second model with the Ri closure")
@@ -96,6 +97,9 @@ def _oracle_sample(config):
     elif config == 5:
         wl = W.aquaplanet(window=(300, 500, 900, 1300), steps=1)
         what = "aqua-planet window j=300:500 i=900:1300 (closed box)"
+    elif config == 6:
+        wl = W.make(6, nx=320, ny=160)
+        what = "patch planet 320x160 (default patch)"
     elif config in (2, 3):
         wl = W.make(config, window=(200, 400, 500, 900), steps=1)
         what = "config %d window j=200:400 i=500:900 (closed box)" % config
@@ -120,11 +124,13 @@ def time_oracle(config, steps, warmup, closure="const", threads=None, shrink=Fal
     g = wl["grid"]
     cells = g["nx"] * g["ny"] * g["nz"]
     ref = oracle.RefModel(wl)
+    nwet = int(ref.grid.masks()["wet"].sum(dtype=np.int64))
     ref.step(max(1, warmup))                     # Euler start + AB2 warm-up
     t0 = time.perf_counter()
     ref.step(steps)
     dt = time.perf_counter() - t0
-    return dict(value=cells * steps / dt, sec_per_step=dt / steps, cores=oracle.num_threads(), cells=cells,
+    return dict(value=cells * steps / dt, wet_value=nwet * steps / dt, wet_fraction=nwet / cells,
+                sec_per_step=dt / steps, cores=oracle.num_threads(), cells=cells,
                 sample="%s: %dx%dx%d cells, %d steps after %d warm-up" % (what, g["nx"], g["ny"], g["nz"], steps,
                                                                          max(1, warmup)),
                 dt_model=wl["params"]["dt"], name=workload_name(wl))
@@ -142,7 +148,8 @@ def run_reference(args):
             "config": {"workload": r["name"], "sample": r["sample"]},
             "sypd_equivalent_of_sample": sypd(r["dt_model"], r["sec_per_step"]),
             "cpu_baseline": {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle",
-                             "sample": r["sample"]},
+                             "sample": r["sample"], "wet_cell_updates_per_s": r["wet_value"],
+                             "wet_fraction_of_sample": r["wet_fraction"]},
             "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
@@ -269,7 +276,11 @@ def run_ours(args):
         dist.barrier()
 
     K, Wm = args.steps, max(args.warmup, 3)
-    wl = W.make(args.config)
+    if args.config == 6:
+        pw, ph = (int(x) for x in args.patch.lower().split("x"))
+        wl = W.make(6, w=pw, h=ph)
+    else:
+        wl = W.make(args.config)
     if args.closure == "ri":
         W.with_ri_closure(wl)
     ri = 1 if args.closure == "ri" else 0
@@ -459,7 +470,8 @@ def run_ours(args):
         r = time_oracle(args.config, 3 if args.config >= 2 else 5, 1, args.closure)
         r1 = time_oracle(args.config, 1, 1, args.closure, threads=1, shrink=True)
         cpu = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"],
-               "one_thread": {"value": r1["value"], "cores": 1, "sample": r1["sample"]}}
+               "wet_cell_updates_per_s": r["wet_value"], "wet_fraction_of_sample": r["wet_fraction"],
+               "one_thread": {"value": r1["value"], "wet_cell_updates_per_s": r1["wet_value"], "cores": 1, "sample": r1["sample"]}}
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,

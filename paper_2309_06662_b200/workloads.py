@@ -308,7 +308,20 @@ def aquaplanet(nx=2160, ny=900, nz=100, steps=20, precision=32, seed=SEED_BASE +
                   window=window, bathymetry="aquaplanet")
 
 
-CONFIGS = {0: config0, 1: config1, 2: config2, 3: config3, 4: config4, 5: aquaplanet}
+def tile_patch_planet(w=16, h=4, nx=1440, ny=600, nz=100, tile=(32, 8), steps=10, precision=32, seed=SEED_BASE + 6):
+    """A synthetic mask for kernel analysis (profiles/: the floor / slope model of the tendency kernel): the aqua-planet
+    fields at nx x ny x nz on a flat 6 km floor where only a w x h patch of every tile[0] x tile[1] block of columns is ocean
+    (all nz levels wet there), the rest land - every tile-level of the tendency kernel then holds exactly w * h wet cells.
+    Not a BASELINE.json config; inputs only."""
+    wl = aquaplanet(nx=nx, ny=ny, nz=nz, steps=steps, precision=precision, seed=seed)
+    jj, ii = np.meshgrid(np.arange(ny), np.arange(nx), indexing="ij")
+    ocean = (ii % tile[0] < w) & (jj % tile[1] < h)
+    wl["depth"] = np.where(ocean, 6000.0, 0.0)
+    wl["name"] = "patch_%dx%d_of_%dx%d" % (w, h, tile[0], tile[1])
+    return wl
+
+
+CONFIGS = {0: config0, 1: config1, 2: config2, 3: config3, 4: config4, 5: aquaplanet, 6: tile_patch_planet}
 
 
 def make(config, **kw):
