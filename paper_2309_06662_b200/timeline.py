@@ -16,8 +16,13 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--closure", default="const", choices=["const", "ri"])
+    ap.add_argument("--patch", default="16x4", help="config 6 only: WxH ocean patch of every 32x8 tile")
     a = ap.parse_args()
-    wl = W.make(a.config)
+    if a.config == 6:
+        pw, ph = (int(x) for x in a.patch.lower().split("x"))
+        wl = W.make(6, w=pw, h=ph)
+    else:
+        wl = W.make(a.config)
     if a.closure == "ri":
         W.with_ri_closure(wl)
     m = ocn.Model(wl)
