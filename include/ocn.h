@@ -43,6 +43,10 @@ typedef struct {
     double y0, dy;                  /* metres, or degrees latitude  (uniform) */
     double radius, rotation_rate;   /* lat-lon: sphere radius [m], Omega [1/s] */
     double f0, beta;                /* cartesian: f = f0 + beta (y - y_mid) */
+    /* Latitude bands: this grid is rows j_offset .. j_offset + ny - 1 of a grid of ny_global
+     * rows that starts at y0 — its metrics are evaluated with the whole grid's row numbers, so they are bit-identical to
+     * the whole grid's.  0, 0 = a grid of its own.  A band is bounded in y (periodic_y = 0). */
+    int j_offset, ny_global;
 } ocn_grid_desc;
 
 /* ocn_grid_create — the grid and the immersed-boundary bathymetry of PAPER.md:102-104; builds the metrics and the compact
@@ -220,6 +224,39 @@ ocn_status ocn_get_mixing(ocn_model* model, double* nu, double* kappa);
  * (two models on different streams, or two host threads) race on it: serialise them. */
 ocn_status ocn_get_mixing_noalloc(ocn_model* model, double* nu, double* kappa);
 unsigned long long ocn_noalloc_scratch_bytes(void);
+
+/* ---- Latitude bands: the one exchange step of the path ----------------------------------
+ * PAPER.md:98 (§5.3): the barotropic sub-cycle is stepped with a wide halo so that neighbours exchange once per group of
+ * sub-steps instead of once per sub-step; one exchange of the 3-D halos per baroclinic step.  A band is an
+ * ordinary model on rows j_offset - h .. of the whole grid (ocn_grid_desc.j_offset, ny_global) with h overlap rows on each
+ * inner side; its own rows stay bit-identical to the whole-grid model as long as, after each part of a step, the overlap
+ * rows are overwritten with the neighbour's rows of the group that part made stale (paper_2309_06662_b200/bands.py):
+ *   part 0 (tendency pass)            -> OCN_ROWS_FORCING (G^U, G^V)
+ *   part 1 + q (launch q of the sub-cycle, not the last) -> OCN_ROWS_BAROTROPIC_0 + ((q + 1) & 1) (eta, U, V of that buffer)
+ *   last part (end of sub-cycle, back-substitution, correction) -> OCN_ROWS_STATE (u, v, T, S, p, eta, U, V)
+ * h must cover what one part reaches: ocn_band_overlap(precision, substeps) rows.
+ *
+ * ocn_step_parts: number of parts of one baroclinic step (2 + launches of the sub-cycle).
+ * ocn_step_part: enqueues part `part` of the next step on the model's stream; parts run in order 0 .. parts - 1 (OCN_ESTATE
+ *   otherwise, and ocn_time_step returns OCN_ESTATE while a split step is in progress).  All parts of a step = ocn_time_step(1),
+ *   bit for bit (same kernels, launched directly instead of through the captured graph).
+ * ocn_rows_bytes: size of the packed rows of a group.  ocn_pack_rows / ocn_unpack_rows: rows j_begin .. j_begin + nrows - 1
+ *   (with their x-halo images) of every array of the group -> / <- one contiguous DEVICE buffer of that size, enqueued on
+ *   the model's stream (device-to-device copies; no host synchronisation; nothing is allocated).  The buffer is the
+ *   caller's (e.g. a torch tensor handed to NCCL send / recv); it must stay valid until the stream has passed the call.
+ *   Packing from one model and unpacking into another of the same nx, nz and precision is the whole exchange.
+ * Errors: OCN_EINVAL (null, rows outside the grid, unknown group), OCN_ESTATE, OCN_ECUDA. */
+enum { OCN_ROWS_STATE = 0, OCN_ROWS_FORCING = 1, OCN_ROWS_BAROTROPIC_0 = 2, OCN_ROWS_BAROTROPIC_1 = 3 };
+ocn_status ocn_step_parts(const ocn_model* model, int* parts);
+ocn_status ocn_step_part(ocn_model* model, int part);
+ocn_status ocn_rows_bytes(const ocn_model* model, int group, int nrows, unsigned long long* bytes);
+ocn_status ocn_pack_rows(ocn_model* model, int group, int j_begin, int nrows, void* dst_device);
+ocn_status ocn_unpack_rows(ocn_model* model, int group, int j_begin, int nrows, const void* src_device);
+/* Overlap rows a band of a model of this precision (32 / 64) and sub-step count needs on each inner side: what ONE part
+ * of a step reaches (every exchange resets the overlap rows, so the reaches do not add up) — the larger of the sub-steps
+ * one launch of the sub-cycle advances (the error of the band's artificial wall travels one row per sub-step) and the 3
+ * rows of the widest stencil of the tendency pass — + 1 for the staggering of the v faces.  -1 for bad arguments.  Host-only. */
+int ocn_band_overlap(int precision, int substeps);
 
 const char* ocn_last_error(void);
 const char* ocn_version(void);

@@ -57,7 +57,9 @@ inline std::string build_grid(ocn_grid& g, const ocn_grid_desc& d, const double*
         const double rad = M_PI / 180.0, a = d.radius, dlam = d.dx * rad, dphi = d.dy * rad;
         g.dy = a * dphi;
         for (int r = 0; r < nr; ++r) {
-            const double pf = (d.y0 + (r - OCN_HALO) * d.dy) * rad, pc = pf + 0.5 * dphi;
+            // j_offset: this grid is rows j_offset .. of a taller one (a latitude band): the same expression
+            // in the same integers as the whole grid evaluates, so the band's metrics are bit-identical to its rows there
+            const double pf = (d.y0 + (r - OCN_HALO + d.j_offset) * d.dy) * rad, pc = pf + 0.5 * dphi;
             g.dxC[r] = a * std::cos(pc) * dlam;
             g.dxF[r] = a * std::cos(pf) * dlam;
             g.AzC[r] = a * a * dlam * (std::sin(pf + dphi) - std::sin(pf));
@@ -66,11 +68,11 @@ inline std::string build_grid(ocn_grid& g, const ocn_grid_desc& d, const double*
         }
     } else {
         g.dy = d.dy;
-        const double ymid = d.y0 + 0.5 * ny * d.dy;
+        const double ymid = d.y0 + 0.5 * (d.ny_global > 0 ? d.ny_global : ny) * d.dy;
         for (int r = 0; r < nr; ++r) {
             g.dxC[r] = g.dxF[r] = d.dx;
             g.AzC[r] = g.AzF[r] = d.dx * d.dy;
-            g.fF[r] = d.f0 + d.beta * ((d.y0 + (r - OCN_HALO) * d.dy) - ymid);
+            g.fF[r] = d.f0 + d.beta * ((d.y0 + (r - OCN_HALO + d.j_offset) * d.dy) - ymid);
         }
     }
     for (int r = 0; r < nr; ++r)

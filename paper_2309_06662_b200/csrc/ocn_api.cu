@@ -86,6 +86,9 @@ struct ocn_model {
     cudaGraphExec_t graph = nullptr;    // one steady-state (AB2) step
     CUtensorMap tm_ts{}, tm_uv{}, tm_p{};   // TMA descriptors of the halo'd (T,S), (u,v) and p arrays
     int launches_per_step = 0;
+    // split step (ocn_step_part): the next part expected, and whether the step in progress is the Euler start
+    int split_next = 0;
+    bool split_euler = false;
     // per-stage timing (ocn_profile_*)
     bool profiling = false;
     std::vector<cudaEvent_t> ev_pool;   // OCN_NSTAGES + 1 events per profiled step
@@ -386,14 +389,21 @@ ocn_status prof_mark(ocn_model* M) {
     return OCN_OK;
 }
 
+// number of launches of the barotropic sub-cycle (each advances bt_substeps_per_launch sub-steps)
+template <class T> int bt_launches(const ocn_model* M) { return (M->d.substeps + bt_substeps_per_launch<T>() - 1) / bt_substeps_per_launch<T>(); }
+
+// part < 0: the whole step.  Else one part of it (ocn_step_part): 0 = tendency pass, 1 + q = launch q of the sub-cycle,
+// bt_launches + 1 = end of the sub-cycle, back-substitution and correction.
 template <class T>
-ocn_status launch_step(ocn_model* M, bool euler) {
+ocn_status launch_step(ocn_model* M, bool euler, int part = -1) {
     const ocn_grid* g = M->g;
     ocn_status ps;
+    const int last_part = bt_launches<T>(M) + 1;
     M->ev_used -= M->ev_used % (OCN_NSTAGES + 1);   // groups start on a step boundary (see prof_flush)
     if (M->profiling && M->ev_used + OCN_NSTAGES + 1 > 4096 && (ps = prof_flush(M)) != OCN_OK) return ps;
 #define MARK(stage, n)                                                   \
     do {                                                                 \
+        if (part >= 0) break;                   /* parts are not profiled */ \
         if ((ps = prof_mark(M)) != OCN_OK) return ps;                    \
         if (M->profiling && (stage) >= 0) M->prof_launches[stage] += (n); \
     } while (0)
@@ -401,7 +411,7 @@ ocn_status launch_step(ocn_model* M, bool euler) {
     const T c0 = euler ? T(1) : (T)(1.5 + M->d.chi), c1 = euler ? T(0) : (T)(0.5 + M->d.chi);
     const dim3 bc(32, 4), b2(32, 8);
     MARK(-1, 0);
-    {
+    if (part < 0 || part == 0) {
         const dim3 bt(TILE_X, TILE_Y), gt = grid2(g, bt);
         if (P.bih) {                               // biharmonic pre-pass: L of the state, then -coefficient L(L)
             ocn::k_laplacians<T><<<grid2(g, bc), bc, 0, M->stream>>>(P, P.uv, P.ts, P.Luv, P.Lts, T(1), T(1), 0);
@@ -416,21 +426,24 @@ ocn_status launch_step(ocn_model* M, bool euler) {
         typedef ocn::BtStrip<BS_X, BS_Y, BS_H> B;
         const dim3 gb((g->nx + BS_X - 1) / BS_X, (g->ny + BS_Y - 1) / BS_Y);
         int cur = 0;
-        for (int m0 = 0; m0 < M->d.substeps; m0 += BS_H) {
+        for (int m0 = 0, q = 0; m0 < M->d.substeps; m0 += BS_H, ++q) {
             const int ns = std::min(BS_H, M->d.substeps - m0);
-            ocn::k_barotropic_strip<BS_X, BS_Y, BS_H><<<gb, B::NT, B::SMEM, M->stream>>>(P, cur, ns, m0 == 0 ? 1 : 0, m0);
+            if (part < 0 || part == 1 + q)
+                ocn::k_barotropic_strip<BS_X, BS_Y, BS_H><<<gb, B::NT, B::SMEM, M->stream>>>(P, cur, ns, m0 == 0 ? 1 : 0, m0);
             cur ^= 1;
         }
     } else {
         typedef ocn::BtTile<T, BT_X, BT_Y> B;
         const dim3 gb((g->nx + BT_X - 1) / BT_X, (g->ny + BT_Y - 1) / BT_Y);
         int cur = 0;
-        for (int m0 = 0; m0 < M->d.substeps; m0 += BT_HALO) {
+        for (int m0 = 0, q = 0; m0 < M->d.substeps; m0 += BT_HALO, ++q) {
             const int ns = std::min(BT_HALO, M->d.substeps - m0);
-            ocn::k_barotropic_tile<T, BT_X, BT_Y><<<gb, B::NT, B::SMEM, M->stream>>>(P, cur, ns, m0 == 0 ? 1 : 0, m0);
+            if (part < 0 || part == 1 + q)
+                ocn::k_barotropic_tile<T, BT_X, BT_Y><<<gb, B::NT, B::SMEM, M->stream>>>(P, cur, ns, m0 == 0 ? 1 : 0, m0);
             cur ^= 1;
         }
     }
+    if (part >= 0 && part != last_part) { CK(cudaGetLastError()); return OCN_OK; }
     ocn::k_barotropic_finish<T><<<grid2(g, b2), b2, 0, M->stream>>>(P);
     MARK(1, (M->d.substeps + bt_substeps_per_launch<T>() - 1) / bt_substeps_per_launch<T>() + 1);
     MARK(3, 0);                                    // (the closure is evaluated inside K1: stage 3 is empty)
@@ -525,6 +538,7 @@ ocn_status set_fields_t(ocn_model* M, const ocn_fields* f) {
         ocn::k_pressure<T><<<grid2(M->g, bc), bc, 0, M->stream>>>(P);
         CK(cudaGetLastError());
         M->have_history = false;
+        M->split_next = 0;                     // a split step in progress is abandoned with the state it was advancing
     }
     return OCN_OK;
 }
@@ -678,6 +692,10 @@ ocn_status ocn_grid_create(const ocn_grid_desc* d, const double* z_faces, const 
     if (d->kind != 0 && d->kind != 1) return fail(OCN_EINVAL, "kind must be 0 (cartesian) or 1 (lat-lon)");
     if (d->kind == 1 && d->periodic_y) return fail(OCN_EINVAL, "a lat-lon grid cannot be periodic in latitude");
     if (!(d->dx > 0) || !(d->dy > 0)) return fail(OCN_EINVAL, "dx, dy must be positive");
+    if (d->j_offset < 0 || d->ny_global < 0 || (d->ny_global > 0 && d->j_offset + d->ny > d->ny_global) ||
+        (d->ny_global == 0 && d->j_offset != 0))
+        return fail(OCN_EINVAL, "j_offset / ny_global: the band must lie inside the whole grid (0, 0 = a grid of its own)");
+    if (d->ny_global > 0 && d->periodic_y) return fail(OCN_EINVAL, "a latitude band is bounded in y (periodic_y = 0)");
 
     ocn_grid* g = new (std::nothrow) ocn_grid();
     if (!g) return fail(OCN_ENOMEM, "host allocation failed");
@@ -814,8 +832,113 @@ ocn_status ocn_set_fields(ocn_model* M, const ocn_fields* f) {
 
 ocn_status ocn_time_step(ocn_model* M, int n) {
     if (!M || n < 0) return fail(OCN_EINVAL, "bad argument");
+    if (M->split_next != 0) return fail(OCN_ESTATE, "a split step is in progress (ocn_step_part): finish its parts first");
     ON_DEVICE(M->d.device);
     return M->prec == 32 ? run_steps<float>(M, n) : run_steps<double>(M, n);
+}
+
+// ---- the step in parts, and rows of the arrays a neighbouring band needs (latitude bands) ----
+extern "C++" {
+namespace {
+int step_parts(const ocn_model* M) { return (M->prec == 32 ? bt_launches<float>(M) : bt_launches<double>(M)) + 2; }
+
+// the arrays of a row group: base pointer (plane layout), bytes per element, planes
+struct RowArray { char* base; size_t es; int planes; };
+template <class T>
+int row_arrays(ocn_model* M, int group, RowArray* out) {
+    ocn::DevP<T>& P = params<T>(M);
+    const int nz = M->g->nz;
+    int n = 0;
+    auto add = [&](void* b, size_t es, int planes) { out[n++] = RowArray{(char*)b, es, planes}; };
+    switch (group) {
+        case OCN_ROWS_STATE:
+            add(P.uv, 2 * sizeof(T), nz); add(P.ts, 2 * sizeof(T), nz); add(P.p, sizeof(double), nz);
+            add(P.eta[0], sizeof(T), 1); add(P.U[0], sizeof(T), 1); add(P.V[0], sizeof(T), 1);
+            break;
+        case OCN_ROWS_FORCING: add(P.GU, sizeof(T), 1); add(P.GV, sizeof(T), 1); break;
+        case OCN_ROWS_BAROTROPIC_0: case OCN_ROWS_BAROTROPIC_1: {
+            const int b = group - OCN_ROWS_BAROTROPIC_0;
+            add(P.eta[b], sizeof(T), 1); add(P.U[b], sizeof(T), 1); add(P.V[b], sizeof(T), 1);
+            break;
+        }
+        default: return -1;
+    }
+    return n;
+}
+int row_arrays_any(ocn_model* M, int group, RowArray* out) {
+    return M->prec == 32 ? row_arrays<float>(M, group, out) : row_arrays<double>(M, group, out);
+}
+// Rows j_begin .. j_begin + nrows - 1 of every plane of the group's arrays <-> one contiguous device buffer, array after
+// array, plane after plane.  A chunk is nrows * sx elements from 4 elements before (row j_begin, i = 0): the rows with
+// their x-halo images (the padding between rows rides along).
+ocn_status move_rows(ocn_model* M, int group, int j_begin, int nrows, char* buf, bool pack) {
+    RowArray arr[8];
+    const int na = row_arrays_any(M, group, arr);
+    if (na < 0) return fail(OCN_EINVAL, "unknown row group");
+    const ocn_grid* g = M->g;
+    if (nrows < 0 || j_begin < 0 || j_begin + nrows > g->ny) return fail(OCN_EINVAL, "rows outside the grid");
+    if (nrows == 0) return OCN_OK;
+    const size_t chunk = (size_t)nrows * g->sx, sz = (size_t)g->sx * g->sy;
+    const long long off = (long long)(j_begin + OCN_HALO) * g->sx - 4;
+    for (int a = 0; a < na; ++a) {
+        char* dev = arr[a].base + off * (long long)arr[a].es;
+        const size_t w = chunk * arr[a].es;
+        if (pack) CK(cudaMemcpy2DAsync(buf, w, dev, sz * arr[a].es, w, arr[a].planes, cudaMemcpyDeviceToDevice, M->stream));
+        else CK(cudaMemcpy2DAsync(dev, sz * arr[a].es, buf, w, w, arr[a].planes, cudaMemcpyDeviceToDevice, M->stream));
+        buf += w * arr[a].planes;
+    }
+    return OCN_OK;
+}
+}  // namespace
+}  // extern "C++"
+
+ocn_status ocn_step_parts(const ocn_model* M, int* parts) {
+    if (!M || !parts) return fail(OCN_EINVAL, "null argument");
+    *parts = step_parts(M);
+    return OCN_OK;
+}
+
+ocn_status ocn_step_part(ocn_model* M, int part) {
+    if (!M) return fail(OCN_EINVAL, "null model");
+    const int np = step_parts(M);
+    if (part < 0 || part >= np) return fail(OCN_EINVAL, "no such part of a step");
+    if (part != M->split_next) return fail(OCN_ESTATE, "parts of a step run in order, 0 .. ocn_step_parts - 1 (next expected: " + std::to_string(M->split_next) + ")");
+    ON_DEVICE(M->d.device);
+    if (part == 0) M->split_euler = !M->have_history;
+    const ocn_status s = M->prec == 32 ? launch_step<float>(M, M->split_euler, part) : launch_step<double>(M, M->split_euler, part);
+    if (s != OCN_OK) return s;
+    if (part == np - 1) { M->have_history = true; M->split_next = 0; }
+    else M->split_next = part + 1;
+    return OCN_OK;
+}
+
+int ocn_band_overlap(int precision, int substeps) {
+    if ((precision != 32 && precision != 64) || substeps < 1) return -1;
+    return std::max(std::min(substeps, precision == 32 ? bt_substeps_per_launch<float>() : bt_substeps_per_launch<double>()), OCN_HALO) + 1;
+}
+
+ocn_status ocn_rows_bytes(const ocn_model* M, int group, int nrows, unsigned long long* bytes) {
+    if (!M || !bytes) return fail(OCN_EINVAL, "null argument");
+    RowArray arr[8];
+    const int na = row_arrays_any(const_cast<ocn_model*>(M), group, arr);
+    if (na < 0) return fail(OCN_EINVAL, "unknown row group");
+    if (nrows < 0 || nrows > M->g->ny) return fail(OCN_EINVAL, "rows outside the grid");
+    unsigned long long b = 0;
+    for (int a = 0; a < na; ++a) b += (unsigned long long)nrows * M->g->sx * arr[a].es * arr[a].planes;
+    *bytes = b;
+    return OCN_OK;
+}
+
+ocn_status ocn_pack_rows(ocn_model* M, int group, int j_begin, int nrows, void* dst) {
+    if (!M || !dst) return fail(OCN_EINVAL, "null argument");
+    ON_DEVICE(M->d.device);
+    return move_rows(M, group, j_begin, nrows, (char*)dst, true);
+}
+
+ocn_status ocn_unpack_rows(ocn_model* M, int group, int j_begin, int nrows, const void* src) {
+    if (!M || !src) return fail(OCN_EINVAL, "null argument");
+    ON_DEVICE(M->d.device);
+    return move_rows(M, group, j_begin, nrows, (char*)const_cast<void*>(src), false);
 }
 
 ocn_status ocn_get_fields(ocn_model* M, ocn_fields* f) {

@@ -23,7 +23,8 @@ class ocn_grid_desc(C.Structure):
     _fields_ = [("kind", C.c_int), ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
                 ("periodic_x", C.c_int), ("periodic_y", C.c_int),
                 ("x0", C.c_double), ("dx", C.c_double), ("y0", C.c_double), ("dy", C.c_double),
-                ("radius", C.c_double), ("rotation_rate", C.c_double), ("f0", C.c_double), ("beta", C.c_double)]
+                ("radius", C.c_double), ("rotation_rate", C.c_double), ("f0", C.c_double), ("beta", C.c_double),
+                ("j_offset", C.c_int), ("ny_global", C.c_int)]
 
 
 class ocn_model_desc(C.Structure):
@@ -48,7 +49,9 @@ EXPORTS = ["ocn_grid_create", "ocn_grid_destroy", "ocn_model_create", "ocn_model
            "ocn_time_step", "ocn_get_fields", "ocn_synchronize", "ocn_get_masks", "ocn_model_info",
            "ocn_get_debug", "ocn_last_error", "ocn_version", "ocn_profile_enable", "ocn_profile_read",
            "ocn_stage_name", "ocn_get_mixing", "ocn_get_fields_async", "ocn_wait", "ocn_tune", "ocn_selftest_division", "ocn_get_timeline",
-           "ocn_get_mixing_noalloc", "ocn_noalloc_scratch_bytes"]
+           "ocn_get_mixing_noalloc", "ocn_noalloc_scratch_bytes",
+           "ocn_step_parts", "ocn_step_part", "ocn_rows_bytes", "ocn_pack_rows", "ocn_unpack_rows", "ocn_band_overlap"]
+ROWS_STATE, ROWS_FORCING, ROWS_BAROTROPIC_0, ROWS_BAROTROPIC_1 = 0, 1, 2, 3
 NSTAGES = 4
 
 
@@ -83,6 +86,12 @@ def lib():
         L.ocn_noalloc_scratch_bytes.restype = C.c_ulonglong
         L.ocn_profile_enable.argtypes = [vp, C.c_int]
         L.ocn_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong), C.c_int]
+        L.ocn_step_parts.argtypes = [vp, C.POINTER(C.c_int)]
+        L.ocn_step_part.argtypes = [vp, C.c_int]
+        L.ocn_rows_bytes.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_ulonglong)]
+        L.ocn_pack_rows.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp]
+        L.ocn_unpack_rows.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp]
+        L.ocn_band_overlap.argtypes = [C.c_int, C.c_int]
         L.ocn_stage_name.restype = C.c_char_p
         L.ocn_stage_name.argtypes = [C.c_int]
         _lib = L
@@ -96,6 +105,14 @@ def selftest_division(n, seed=1, device=0):
     return bad.value
 
 
+def band_overlap(precision, substeps):
+    """ocn_band_overlap: overlap rows a latitude band needs on each inner side."""
+    h = int(lib().ocn_band_overlap(int(precision), int(substeps)))
+    if h < 0:
+        raise ValueError("band_overlap: precision must be 32 or 64 and substeps >= 1")
+    return h
+
+
 def _check(rc):
     if rc != OCN_OK:
         raise RuntimeError(f"libocn status {rc}: {lib().ocn_last_error().decode()}")
@@ -107,7 +124,7 @@ def _ptr(a):
 
 class Grid:
     def __init__(self, grid, z_faces, depth):
-        self.desc = ocn_grid_desc(**{k: grid[k] for k, _ in ocn_grid_desc._fields_})
+        self.desc = ocn_grid_desc(**{k: grid.get(k, 0) if k in ("j_offset", "ny_global") else grid[k] for k, _ in ocn_grid_desc._fields_})
         self.nx, self.ny, self.nz = int(grid["nx"]), int(grid["ny"]), int(grid["nz"])
         zf = np.ascontiguousarray(z_faces, dtype=np.float64)
         h = np.ascontiguousarray(depth, dtype=np.float64)
@@ -202,6 +219,26 @@ class Model:
 
     def synchronize(self):
         _check(lib().ocn_synchronize(self.h))
+
+    # -- the step in parts and the rows a neighbouring band needs (include/ocn.h, "Latitude bands") ----
+    def step_parts(self):
+        n = C.c_int()
+        _check(lib().ocn_step_parts(self.h, C.byref(n)))
+        return n.value
+
+    def step_part(self, part):
+        _check(lib().ocn_step_part(self.h, int(part)))
+
+    def rows_bytes(self, group, nrows):
+        b = C.c_ulonglong()
+        _check(lib().ocn_rows_bytes(self.h, int(group), int(nrows), C.byref(b)))
+        return b.value
+
+    def pack_rows(self, group, j_begin, nrows, dst_device_ptr):
+        _check(lib().ocn_pack_rows(self.h, int(group), int(j_begin), int(nrows), C.c_void_p(int(dst_device_ptr))))
+
+    def unpack_rows(self, group, j_begin, nrows, src_device_ptr):
+        _check(lib().ocn_unpack_rows(self.h, int(group), int(j_begin), int(nrows), C.c_void_p(int(src_device_ptr))))
 
     def info(self):
         n, b = C.c_int(), C.c_ulonglong()

@@ -1,0 +1,162 @@
+"""GPU tests of the latitude-band form of the path (include/ocn.h "Latitude bands"): a
+grid stepped as 2, 3 or 4 band models that exchange overlap rows after each part of a step gives, on every band's own
+rows, the SAME BITS as the whole-grid model (which the other GPU tests hold against the oracle) — fp64 and fp32, with the
+closure, bottom drag and the biharmonic terms, and the fp64 bands are therefore bit-identical to the oracle as well.
+One GPU, one stream: this is the decomposition made correct by construction; the same plan over torch.distributed is
+covered on CPU (tests/test_bands_plan.py)."""
+import ctypes as C
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2309_06662_b200 import bands
+from paper_2309_06662_b200 import build as ocn_build
+from paper_2309_06662_b200 import ocn
+from paper_2309_06662_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+FIELDS = ("u", "v", "w", "eta", "T", "S")
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    ocn_build.build()
+
+
+def _stirred(wl, seed=33):
+    rng = np.random.default_rng(seed)
+    f, prec = wl["fields"], wl["params"]["precision"]
+    f["u"] = W._round_to(prec, 0.3 * rng.standard_normal(f["u"].shape))
+    f["v"] = W._round_to(prec, 0.3 * rng.standard_normal(f["v"].shape))
+    f["T"] = W._round_to(prec, f["T"] + 0.5 * rng.standard_normal(f["T"].shape))
+    f["eta"] = W._round_to(prec, 0.2 * rng.standard_normal(f["eta"].shape))
+    return wl
+
+
+def _workload(prec, kind=""):
+    wl = _stirred(W.config2(nx=180, ny=75, nz=25, steps=6, precision=prec))
+    if "r" in kind:
+        W.with_ri_closure(wl)
+    if "d" in kind:
+        wl["params"].update(drag_r=2e-4, drag_cd=2e-3)
+    if "b" in kind:
+        wl["params"].update(nu4_h=1e9, kappa4_h=5e8)
+    if "z" in kind:
+        W.with_weno_z(wl)
+    return wl
+
+
+def test_the_parts_of_a_step_are_the_step():
+    for prec in (32, 64):
+        wl = _workload(prec, "r")
+        a, b = ocn.Model(wl), ocn.Model(wl)
+        a.time_step(5)
+        n = b.step_parts()
+        assert n == b.info()["launches_per_step"] - 1              # K1, the launches of the sub-cycle, [finish + K3]
+        for _ in range(5):
+            for p in range(n):
+                b.step_part(p)
+        fa, fb = a.get_fields(), b.get_fields()
+        for k in FIELDS:
+            assert np.array_equal(fa[k], fb[k]), (prec, k)
+        a.close(); b.close()
+
+
+def test_parts_run_in_order_and_block_whole_steps():
+    m = ocn.Model(_workload(32))
+    with pytest.raises(RuntimeError, match="parts of a step run in order"):
+        m.step_part(1)
+    m.step_part(0)
+    with pytest.raises(RuntimeError, match="split step is in progress"):
+        m.time_step(1)
+    with pytest.raises(RuntimeError, match="parts of a step run in order"):
+        m.step_part(0)
+    with pytest.raises(RuntimeError, match="no such part"):
+        m.step_part(m.step_parts())
+    for p in range(1, m.step_parts()):
+        m.step_part(p)
+    m.time_step(1)                                                 # the step is complete: whole steps are allowed again
+    m.close()
+
+
+def test_rows_round_trip_and_are_checked():
+    import torch
+    wl = _workload(64)
+    a, b = ocn.Model(wl), ocn.Model(wl)
+    a.time_step(3); b.time_step(1)                                 # different states
+    for group in (ocn.ROWS_STATE, ocn.ROWS_FORCING, ocn.ROWS_BAROTROPIC_0, ocn.ROWS_BAROTROPIC_1):
+        nb = a.rows_bytes(group, a.ny)
+        buf = torch.empty(nb, dtype=torch.uint8, device="cuda")
+        a.synchronize(); b.synchronize()
+        a.pack_rows(group, 0, a.ny, buf.data_ptr())
+        a.synchronize()
+        b.unpack_rows(group, 0, b.ny, buf.data_ptr())
+        b.synchronize()
+    fa, fb = a.get_fields(("u", "v", "T", "S", "eta")), b.get_fields(("u", "v", "T", "S", "eta"))
+    for k in fa:
+        assert np.array_equal(fa[k], fb[k]), k                     # every row of the state travelled
+    sx = (a.nx + 8 + 31) // 32 * 32
+    assert a.rows_bytes(ocn.ROWS_FORCING, 7) == 2 * 7 * sx * 8
+    assert a.rows_bytes(ocn.ROWS_STATE, 2) == 2 * sx * (25 * (16 + 16 + 8) + 3 * 8)
+    with pytest.raises(RuntimeError, match="rows outside the grid"):
+        a.pack_rows(ocn.ROWS_STATE, a.ny - 2, 3, buf.data_ptr())
+    with pytest.raises(RuntimeError, match="unknown row group"):
+        a.rows_bytes(9, 1)
+    assert ocn.band_overlap(32, 40) == 11 and ocn.band_overlap(64, 40) == 7 and ocn.band_overlap(64, 2) == 4
+    a.close(); b.close()
+
+
+def test_band_masks_are_the_whole_grids_away_from_its_walls():
+    wl = _workload(64)
+    g = ocn.Grid(wl["grid"], wl["z_faces"], wl["depth"])
+    bw = bands.band_workload(wl, (20, 51))
+    gb = ocn.Grid(bw["grid"], bw["z_faces"], bw["depth"])
+    mw, mb = g.masks(), gb.masks()
+    inner = slice(3, 31 - 3)                                       # away from the band's artificial walls
+    for k in mw:
+        assert np.array_equal(mw[k][:, 20:51][:, inner], mb[k][:, inner]), k
+    bad = dict(bw["grid"], ny_global=40)
+    with pytest.raises(RuntimeError, match="band must lie inside"):
+        ocn.Grid(bad, bw["z_faces"], bw["depth"])
+
+
+@pytest.mark.parametrize("prec,kind,nb", [(64, "", 2), (64, "r", 3), (64, "db", 3), (32, "", 2), (32, "r", 3), (32, "dbz", 4), (32, "", 1)])
+def test_bands_are_bit_identical_to_the_whole_grid(prec, kind, nb):
+    wl = _workload(prec, kind)
+    whole = ocn.Model(wl)
+    B = bands.Bands(wl, nb)
+    assert B.h == ocn.band_overlap(prec, wl["params"]["substeps"])
+    whole.time_step(6); B.time_step(6)
+    fw, fb = whole.get_fields(), B.get_fields()
+    for k in FIELDS:
+        assert fb[k].shape == fw[k].shape
+        assert np.array_equal(fw[k], fb[k]), (prec, kind, nb, k, float(np.abs(fw[k].astype(np.float64) - fb[k]).max()))
+    assert float(np.abs(fw["u"]).max()) > 0.05 and np.isfinite(fw["T"]).all()
+    whole.close(); B.close()
+
+
+def test_fp64_bands_are_bit_identical_to_the_oracle():
+    wl = _workload(64, "r")
+    ref = oracle.RefModel(wl)
+    B = bands.Bands(wl, 3)
+    ref.step(6); B.time_step(6)
+    a, b = B.get_fields(), ref.get_fields()
+    for k in FIELDS:
+        assert np.array_equal(a[k], b[k]), k
+    B.close()
+
+
+def test_exchanged_bytes_per_step_are_what_the_design_says():
+    wl = _workload(32)
+    B = bands.Bands(wl, 3)
+    m = B.models[0]
+    per = {g: m.rows_bytes(g, B.h) for g in (ocn.ROWS_STATE, ocn.ROWS_FORCING, ocn.ROWS_BAROTROPIC_0)}
+    groups = [bands.group_after_part(p, B.parts) for p in range(B.parts)]
+    total = sum(per[min(g, ocn.ROWS_BAROTROPIC_0)] for g in groups if g is not None)
+    sx = (m.nx + 8 + 31) // 32 * 32
+    nz = m.nz
+    # per cut and direction: h rows of (u,v), (T,S) pairs + p (fp64) + eta, U, V once; G^U, G^V once; eta, U, V after every launch but the last
+    launches = B.parts - 2
+    assert total == B.h * sx * (nz * (8 + 8 + 8) + 3 * 4 + 2 * 4 + (launches - 1) * 3 * 4)
+    B.close()
