@@ -61,6 +61,10 @@ def parse():
                     help="vertical mixing: constant coefficients (default, the north_star path) or the Ri-based closure "
                          "of PAPER.md:114 (SURVEY 8f-1; DESIGN.md §3.12)")
     ap.add_argument("--patch", default="16x4", help="config 6 only (kernel analysis): WxH ocean patch of every 32x8 tile")
+    ap.add_argument("--bands", type=int, default=0,
+                    help="(analysis, DESIGN.md section 9) step the grid as this many latitude bands: all on this one GPU "
+                         "(no torchrun: time of the slowest-possible serial execution / N = the projected band time), "
+                         "or one band per rank under torchrun with --gpus N (strong scaling, NCCL point-to-point)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the end-to-end (host buffer) leg")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-closure-leg", action="store_true", help="skip the second model with the Ri closure")
@@ -492,10 +496,96 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_bands(args):
+    """--bands N: the grid as N latitude bands (paper_2309_06662_b200/bands.py).  Single process: all bands on this GPU, one
+    stream — their summed time / N is what one GPU of N would spend on its band (kernels + packing; the copies between
+    bands run at HBM instead of NVLink speed, so the line also gives the bytes per cut and their time at NVLink speed).
+    Under torchrun: one band per rank, exchanges over NCCL, strong scaling of the whole grid."""
+    import torch
+    from paper_2309_06662_b200 import bands, build as ocn_build
+    from paper_2309_06662_b200 import ocn, replicas, workloads as W
+
+    rank, world, local = (int(os.environ.get(k, d)) for k, d in (("RANK", "0"), ("WORLD_SIZE", "1"), ("LOCAL_RANK", "0")))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (libocn has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        ocn_build.build()
+    if dist is not None:
+        dist.barrier()
+    K, Wm = args.steps, max(args.warmup, 3)
+    wl = W.make(args.config)
+    if args.closure == "ri":
+        W.with_ri_closure(wl)
+    g, prm = wl["grid"], wl["params"]
+    cells = g["nx"] * g["ny"] * g["nz"]
+    stream = torch.cuda.Stream(device=local)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def timed(obj):
+        obj.time_step(Wm)
+        replicas.barrier(dist, torch.cuda.synchronize)
+        e0.record(stream)
+        obj.time_step(K)
+        e1.record(stream)
+        replicas.barrier(dist, torch.cuda.synchronize)
+        return replicas.max_over_ranks(e0.elapsed_time(e1), dist, device="cuda") / K
+
+    clocks = ClockSampler(local)
+    with torch.cuda.stream(stream):
+        if world > 1:
+            if args.bands != world:
+                raise SystemExit("bench.py --bands N under torchrun: N must equal the number of ranks")
+            B = bands.DistBand(wl, dist, device=local, stream=stream.cuda_stream)
+            ms = timed(B)
+            m0, nb, whole_ms = B.model, world, None
+        else:
+            whole = ocn.Model(wl, device=local, stream=stream.cuda_stream)
+            whole_ms = timed(whole)
+            whole.close()
+            B = bands.Bands(wl, args.bands, device=local, stream=stream)
+            ms = timed(B)
+            m0, nb = B.models[len(B.models) // 2], args.bands
+        groups = [bands.group_after_part(p, B.parts) for p in range(B.parts)]
+        bytes_cut = sum(m0.rows_bytes(min(gr, ocn.ROWS_BAROTROPIC_0), B.h) for gr in groups if gr is not None)
+        eta_ok = bool(np.isfinite(m0.get_fields(("eta",))["eta"]).all())
+    clk = clocks.stop()
+    assert eta_ok, "non-finite eta after the timed steps"
+    if rank == 0:
+        nvl = bytes_cut / 900e9 * 1e3                   # one direction of one cut at NVLink 5 speed (both directions run at once)
+        out = {"metric": METRIC, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm, "higher_is_better": True,
+               "dtype": "f32" if prm["precision"] == 32 else "f64", "data": "synthetic", "vs_baseline": None, "clocks": clk,
+               "config": {"workload": workload_name(wl), "cells": cells,
+                          "parallelism": ("%d latitude bands, one per GPU (NCCL send / recv)" % nb) if world > 1
+                                         else "%d latitude bands, ALL ON ONE GPU (projection of the band time)" % nb},
+               "bands": {"n": nb, "overlap_rows": B.h, "own_rows": [o[1] - o[0] for o in B.own], "parts_per_step": B.parts,
+                         "exchanges_per_step": sum(gr is not None for gr in groups),
+                         "bytes_per_step_per_cut_and_direction": bytes_cut, "ms_of_those_bytes_at_900_GB_s": nvl}}
+        if world > 1:
+            out.update(value=cells * 1e3 / ms, ms_per_step=ms, scaling="strong")
+        else:
+            per_band = ms / nb
+            out.update(value=cells * 1e3 / ms, ms_per_step=ms, scaling="n/a (one GPU)")
+            out["bands"].update(ms_per_step_whole_grid_one_model=whole_ms, ms_per_step_all_bands_on_one_gpu=ms,
+                                ms_per_step_per_band=per_band,
+                                redundant_rows_fraction=sum(e[1] - e[0] for e in B.ext) / g["ny"] - 1.0,
+                                projected_speedup_on_n_gpus=whole_ms / (per_band + nvl))
+        print(json.dumps(out))
+    B.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         run_reference(args)
+    elif args.bands > 0:
+        run_bands(args)
     else:
         run_ours(args)
 
