@@ -184,9 +184,11 @@ class DistBand:
 
     The band's model works on the stream that is current when it is built (`stream` = its handle), so that the packs,
     torch.distributed's point-to-point calls and the unpacks are ordered by torch's stream semantics with no host
-    synchronisation.  model_factory / alloc as in Bands; alloc returns (tensor, pointer) and the TENSOR is what is sent."""
+    synchronisation.  model_factory / alloc as in Bands; alloc returns (tensor, pointer) and the TENSOR is what is sent.
+    host_staging=True: the packed rows travel through pinned host tensors (device -> host, send / recv, host -> device) for
+    process groups that cannot send device memory (gloo: the 2-process test on one GPU); the default sends device tensors."""
 
-    def __init__(self, wl, dist, device=0, h=None, model_factory=None, alloc=None, stream=None):
+    def __init__(self, wl, dist, device=0, h=None, model_factory=None, alloc=None, stream=None, host_staging=False):
         self.dist = dist
         self.rank, self.world = dist.get_rank(), dist.get_world_size()
         self.ny = int(wl["grid"]["ny"])
@@ -206,11 +208,19 @@ class DistBand:
         self.parts = self.model.step_parts()
         self._alloc = alloc
         self._buf = {}
+        self._host = {}
+        self.host_staging = bool(host_staging)
 
     def _buffer(self, key, nbytes):
         if (key, nbytes) not in self._buf:
             self._buf[(key, nbytes)] = self._alloc(nbytes)
         return self._buf[(key, nbytes)]
+
+    def _host_buffer(self, key, nbytes):
+        import torch
+        if (key, nbytes) not in self._host:
+            self._host[(key, nbytes)] = torch.empty(int(nbytes), dtype=torch.uint8, pin_memory=True)
+        return self._host[(key, nbytes)]
 
     def exchange(self, group):
         """Sends this band's own edge rows to the neighbours and fills its overlap rows from theirs."""
@@ -220,17 +230,28 @@ class DistBand:
             if t.nrows == 0:
                 continue
             if t.src == self.rank:
-                buf, ptr = self._buffer(("s", n), self.model.rows_bytes(group, t.nrows))
+                nbytes = self.model.rows_bytes(group, t.nrows)
+                buf, ptr = self._buffer(("s", n), nbytes)
                 self.model.pack_rows(group, t.src_row, t.nrows, ptr)
+                if self.host_staging:                      # torch's current stream is the model's: the copy follows the pack
+                    hb = self._host_buffer(("s", n), nbytes)
+                    hb.copy_(buf, non_blocking=True)
+                    buf = hb
                 ops.append(dist.P2POp(dist.isend, buf, t.dst, tag=n))
             elif t.dst == self.rank:
-                buf, ptr = self._buffer(("r", n), self.model.rows_bytes(group, t.nrows))
-                ops.append(dist.P2POp(dist.irecv, buf, t.src, tag=n))
-                recvs.append((t, ptr))
+                nbytes = self.model.rows_bytes(group, t.nrows)
+                buf, ptr = self._buffer(("r", n), nbytes)
+                hb = self._host_buffer(("r", n), nbytes) if self.host_staging else None
+                ops.append(dist.P2POp(dist.irecv, hb if hb is not None else buf, t.src, tag=n))
+                recvs.append((t, ptr, buf, hb))
         if ops:
+            if self.host_staging:
+                self.model.synchronize()                   # the host tensors hold the packed rows before they are sent
             for w in dist.batch_isend_irecv(ops):
                 w.wait()
-        for t, ptr in recvs:
+        for t, ptr, buf, hb in recvs:
+            if hb is not None:
+                buf.copy_(hb, non_blocking=True)
             self.model.unpack_rows(group, t.dst_row, t.nrows, ptr)
 
     def time_step(self, n=1):

@@ -160,3 +160,73 @@ def test_exchanged_bytes_per_step_are_what_the_design_says():
     launches = B.parts - 2
     assert total == B.h * sx * (nz * (8 + 8 + 8) + 3 * 4 + 2 * 4 + (launches - 1) * 3 * 4)
     B.close()
+
+
+# ---- one band per PROCESS: two ranks share this one GPU, the packed rows travel through pinned host memory over gloo (NCCL
+# cannot put two ranks on one device).  No kernel of one rank waits for a kernel of the other: the ranks meet on the host.
+def _free_port():
+    import socket
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _rank_worker(rank, world, port, prec, kind, steps, out):
+    import os
+    import torch
+    import torch.distributed as dist
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        torch.cuda.set_device(0)
+        s = torch.cuda.Stream()
+        with torch.cuda.stream(s):
+            D = bands.DistBand(_workload(prec, kind), dist, device=0, stream=s.cuda_stream, host_staging=True)
+            D.time_step(steps)
+            f = D.own_fields(FIELDS)
+        out.put((rank, D.own[rank], {k: np.array(v) for k, v in f.items()}))
+        dist.barrier()
+        D.close()
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("prec,kind,world", [(32, "r", 2), (64, "", 3)])
+def test_one_band_per_process_is_bit_identical_to_the_whole_grid(prec, kind, world):
+    import torch.multiprocessing as mp
+    steps = 4
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    ps = [ctx.Process(target=_rank_worker, args=(r, world, port, prec, kind, steps, q)) for r in range(world)]
+    for p in ps:
+        p.start()
+    whole = ocn.Model(_workload(prec, kind))
+    whole.time_step(steps)
+    fw = whole.get_fields()
+    whole.close()
+    res = sorted((q.get(timeout=600) for _ in ps), key=lambda r: r[0])
+    for p in ps:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    assert res[0][1][0] == 0 and res[-1][1][1] == fw["eta"].shape[0]
+    for rank, own, f in res:
+        for k in FIELDS:
+            assert np.array_equal(f[k], fw[k][..., own[0]:own[1], :]), (rank, k)
+
+
+def test_bench_bands_line():
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--bands", "3", "--config", "3", "--steps", "2", "--warmup", "3"],
+                       capture_output=True, text=True, timeout=900, cwd=root)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    b = d["bands"]
+    assert b["n"] == 3 and b["overlap_rows"] == 11 and sum(b["own_rows"]) == 600 and b["exchanges_per_step"] == b["parts_per_step"] - 1
+    assert b["ms_per_step_per_band"] > 0 and 1.0 < b["projected_speedup_on_n_gpus"] < 3.0
