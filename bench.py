@@ -65,6 +65,9 @@ def parse():
                     help="(analysis, DESIGN.md section 9) step the grid as this many latitude bands: all on this one GPU "
                          "(no torchrun: time of the slowest-possible serial execution / N = the projected band time), "
                          "or one band per rank under torchrun with --gpus N (strong scaling, NCCL point-to-point)")
+    ap.add_argument("--ny", type=int, default=0,
+                    help="with --bands: rows of the whole grid instead of the configuration's (weak-scaling projection: "
+                         "--config 5 --ny 1800 --bands 2 gives every band the 900 rows of the aqua-planet)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the end-to-end (host buffer) leg")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-closure-leg", action="store_true", help="skip the second model with the Ri closure")
@@ -518,7 +521,7 @@ def run_bands(args):
     if dist is not None:
         dist.barrier()
     K, Wm = args.steps, max(args.warmup, 3)
-    wl = W.make(args.config)
+    wl = W.make(args.config, ny=args.ny) if args.ny > 0 else W.make(args.config)
     if args.closure == "ri":
         W.with_ri_closure(wl)
     g, prm = wl["grid"], wl["params"]
