@@ -65,6 +65,9 @@ def parse():
                     help="(analysis, DESIGN.md section 9) step the grid as this many latitude bands: all on this one GPU "
                          "(no torchrun: time of the slowest-possible serial execution / N = the projected band time), "
                          "or one band per rank under torchrun with --gpus N (strong scaling, NCCL point-to-point)")
+    ap.add_argument("--fused-put", action="store_true",
+                    help="with --bands: the back-substitution kernel stores the 3-D overlap rows into the neighbours' arrays itself "
+                         "(peer memory; CUDA IPC under torchrun) instead of packing and sending them")
     ap.add_argument("--ny", type=int, default=0,
                     help="with --bands: rows of the whole grid instead of the configuration's (weak-scaling projection: "
                          "--config 5 --ny 1800 --bands 2 gives every band the 900 rows of the aqua-planet)")
@@ -543,18 +546,22 @@ def run_bands(args):
         if world > 1:
             if args.bands != world:
                 raise SystemExit("bench.py --bands N under torchrun: N must equal the number of ranks")
-            B = bands.DistBand(wl, dist, device=local, stream=stream.cuda_stream)
+            B = bands.DistBand(wl, dist, device=local, stream=stream.cuda_stream, fused_put=args.fused_put)
             ms = timed(B)
             m0, nb, whole_ms = B.model, world, None
         else:
             whole = ocn.Model(wl, device=local, stream=stream.cuda_stream)
             whole_ms = timed(whole)
             whole.close()
-            B = bands.Bands(wl, args.bands, device=local, stream=stream)
+            B = bands.Bands(wl, args.bands, device=local, stream=stream, fused_put=args.fused_put)
             ms = timed(B)
             m0, nb = B.models[len(B.models) // 2], args.bands
         groups = [bands.group_after_part(p, B.parts) for p in range(B.parts)]
-        bytes_cut = sum(m0.rows_bytes(min(gr, ocn.ROWS_BAROTROPIC_0), B.h) for gr in groups if gr is not None)
+        if args.fused_put:                               # the 3-D rows are put by the kernel: only (eta, U, V) are packed at the end
+            groups = [ocn.ROWS_STATE_2D if gr == ocn.ROWS_STATE else gr for gr in groups]
+        sent = {gr: m0.rows_bytes(gr, B.h) for gr in set(groups) if gr is not None}
+        bytes_cut = sum(sent[gr] for gr in groups if gr is not None)
+        bytes_put = m0.rows_bytes(ocn.ROWS_STATE, B.h) - m0.rows_bytes(ocn.ROWS_STATE_2D, B.h) if args.fused_put else 0
         eta_ok = bool(np.isfinite(m0.get_fields(("eta",))["eta"]).all())
     clk = clocks.stop()
     assert eta_ok, "non-finite eta after the timed steps"
@@ -567,6 +574,7 @@ def run_bands(args):
                                          else "%d latitude bands, ALL ON ONE GPU (projection of the band time)" % nb},
                "bands": {"n": nb, "overlap_rows": B.h, "own_rows": [o[1] - o[0] for o in B.own], "parts_per_step": B.parts,
                          "exchanges_per_step": sum(gr is not None for gr in groups),
+                         "fused_put": bool(args.fused_put), "bytes_put_by_the_kernel_per_step_per_cut_and_direction": bytes_put,
                          "bytes_per_step_per_cut_and_direction": bytes_cut, "ms_of_those_bytes_at_900_GB_s": nvl}}
         if world > 1:
             out.update(value=cells * 1e3 / ms, ms_per_step=ms, scaling="strong")
@@ -576,7 +584,8 @@ def run_bands(args):
             out["bands"].update(ms_per_step_whole_grid_one_model=whole_ms, ms_per_step_all_bands_on_one_gpu=ms,
                                 ms_per_step_per_band=per_band,
                                 redundant_rows_fraction=sum(e[1] - e[0] for e in B.ext) / g["ny"] - 1.0,
-                                projected_speedup_on_n_gpus=whole_ms / (per_band + nvl))
+                                projected_speedup_on_n_gpus=whole_ms / (per_band + nvl),
+                                projected_speedup_if_the_puts_do_not_overlap=whole_ms / (per_band + nvl + bytes_put / 900e9 * 1e3))
         print(json.dumps(out))
     B.close()
     if dist is not None:

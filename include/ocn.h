@@ -246,12 +246,40 @@ unsigned long long ocn_noalloc_scratch_bytes(void);
  *   caller's (e.g. a torch tensor handed to NCCL send / recv); it must stay valid until the stream has passed the call.
  *   Packing from one model and unpacking into another of the same nx, nz and precision is the whole exchange.
  * Errors: OCN_EINVAL (null, rows outside the grid, unknown group), OCN_ESTATE, OCN_ECUDA. */
-enum { OCN_ROWS_STATE = 0, OCN_ROWS_FORCING = 1, OCN_ROWS_BAROTROPIC_0 = 2, OCN_ROWS_BAROTROPIC_1 = 3 };
+enum { OCN_ROWS_STATE = 0, OCN_ROWS_FORCING = 1, OCN_ROWS_BAROTROPIC_0 = 2, OCN_ROWS_BAROTROPIC_1 = 3,
+       OCN_ROWS_STATE_2D = 4 /* eta, U, V only: what is left to exchange after the last part with fused puts */ };
 ocn_status ocn_step_parts(const ocn_model* model, int* parts);
 ocn_status ocn_step_part(ocn_model* model, int part);
 ocn_status ocn_rows_bytes(const ocn_model* model, int group, int nrows, unsigned long long* bytes);
 ocn_status ocn_pack_rows(ocn_model* model, int group, int j_begin, int nrows, void* dst_device);
 ocn_status ocn_unpack_rows(ocn_model* model, int group, int j_begin, int nrows, const void* src_device);
+/* Fused puts ("peer memory"): instead of packing, sending and unpacking the new 3-D state after the last part of a
+ * step — 99 % of the exchanged bytes — the kernel that produces it (back-substitution + correction + pressure) stores the rows
+ * a neighbouring band overlaps straight into the neighbour's arrays, and leaves the rows it overlaps itself to the neighbour:
+ * compute and transfer in one kernel, stores over NVLink when the neighbour lives on another GPU.  Only (u, v), (T, S) and p
+ * travel this way — no other part of a step touches them, so a put can only race with the tendency pass of the NEXT step; the
+ * 2-D state (eta, U, V: scratch of the sub-cycle) still goes through OCN_ROWS_STATE_2D after the last part, and the arrival of
+ * those rows is the signal that the neighbour's puts are complete (they were enqueued before the rows were packed).
+ * ocn_peer_export: what a neighbour needs to reach this model's arrays (u,v), (T,S), p: their addresses (valid in this
+ *   process) and CUDA IPC handles + offsets (for another process on the same node).  Plain data: send it as bytes.
+ * ocn_peer_attach: from now on rows my_first_row .. + rows - 1 of this model's new state are also stored at rows
+ *   peer_first_row .. of the neighbour on `side` (0 = south, 1 = north), and this model no longer stores ITS overlap rows on
+ *   that side (everything south of my_first_row for side 0, north of my_first_row + rows for side 1: the neighbour's puts fill
+ *   them).  same_process = 1 uses the addresses, 0 opens the IPC handles (peer access is enabled lazily by the driver).
+ *   After attaching, the bands of a grid step in parts and exchange OCN_ROWS_STATE_2D instead of OCN_ROWS_STATE after the last
+ *   part (bands.py).
+ * Errors: OCN_EINVAL (null, side, mismatched nx / nz / precision, rows outside a grid), OCN_ESTATE (a split step in progress),
+ * OCN_ECUDA (IPC). */
+#define OCN_PEER_ARRAYS 3
+typedef struct {
+    int nx, ny, nz, precision, sx, sy, device;
+    void* ptr[OCN_PEER_ARRAYS];                      /* (u,v), (T,S), p */
+    unsigned char ipc[OCN_PEER_ARRAYS][64];          /* cudaIpcMemHandle_t of the allocation that holds each */
+    unsigned long long ipc_offset[OCN_PEER_ARRAYS];  /* byte offset of the array in that allocation */
+} ocn_peer;
+ocn_status ocn_peer_export(ocn_model* model, ocn_peer* out);
+ocn_status ocn_peer_attach(ocn_model* model, int side, const ocn_peer* peer, int my_first_row, int peer_first_row, int rows,
+                           int same_process);
 /* Overlap rows a band of a model of this precision (32 / 64) and sub-step count needs on each inner side: what ONE part
  * of a step reaches (every exchange resets the overlap rows, so the reaches do not add up) — the larger of the sub-steps
  * one launch of the sub-cycle advances (the error of the band's artificial wall travels one row per sub-step) and the 3

@@ -21,7 +21,7 @@ import numpy as np
 
 from . import ocn
 
-STATE, FORCING, BAROTROPIC_0 = ocn.ROWS_STATE, ocn.ROWS_FORCING, ocn.ROWS_BAROTROPIC_0
+STATE, FORCING, BAROTROPIC_0, STATE_2D = ocn.ROWS_STATE, ocn.ROWS_FORCING, ocn.ROWS_BAROTROPIC_0, ocn.ROWS_STATE_2D
 
 
 # ------------------------------------------------------------------------------------------------
@@ -115,7 +115,7 @@ class Bands:
     model_factory(workload, stream) builds a band (default: ocn.Model on `device` with that stream); alloc(nbytes) returns
     (handle, device pointer) of a transit buffer (default: a torch uint8 tensor on `device`)."""
 
-    def __init__(self, wl, nbands, device=0, h=None, model_factory=None, alloc=None, stream=None):
+    def __init__(self, wl, nbands, device=0, h=None, model_factory=None, alloc=None, stream=None, fused_put=False):
         self.ny = int(wl["grid"]["ny"])
         self.h = overlap_rows(wl) if h is None else int(h)
         self.own, self.ext, self.transfers = exchange_plan(self.ny, nbands, self.h)
@@ -134,6 +134,12 @@ class Bands:
         self.parts = self.models[0].step_parts()
         self._alloc = alloc
         self._buf = {}
+        # fused puts (include/ocn.h): the last part of a step stores the 3-D rows a neighbour overlaps into the neighbour's arrays
+        self.fused_put = bool(fused_put) and len(self.models) > 1
+        if self.fused_put:
+            peers = [m.peer_export() for m in self.models]
+            for t in self.transfers:
+                self.models[t.src].peer_attach(1 if t.dst > t.src else 0, peers[t.dst], t.src_row, t.dst_row, t.nrows, True)
 
     def _buffer(self, nbytes):
         if nbytes not in self._buf:
@@ -156,7 +162,7 @@ class Bands:
                     m.step_part(part)
                 g = group_after_part(part, self.parts)
                 if g is not None and len(self.models) > 1:
-                    self.exchange(g)
+                    self.exchange(STATE_2D if (g == STATE and self.fused_put) else g)
 
     def synchronize(self):
         for m in self.models:
@@ -188,7 +194,8 @@ class DistBand:
     host_staging=True: the packed rows travel through pinned host tensors (device -> host, send / recv, host -> device) for
     process groups that cannot send device memory (gloo: the 2-process test on one GPU); the default sends device tensors."""
 
-    def __init__(self, wl, dist, device=0, h=None, model_factory=None, alloc=None, stream=None, host_staging=False):
+    def __init__(self, wl, dist, device=0, h=None, model_factory=None, alloc=None, stream=None, host_staging=False,
+                 fused_put=False):
         self.dist = dist
         self.rank, self.world = dist.get_rank(), dist.get_world_size()
         self.ny = int(wl["grid"]["ny"])
@@ -210,6 +217,15 @@ class DistBand:
         self._buf = {}
         self._host = {}
         self.host_staging = bool(host_staging)
+        # fused puts: the neighbours' arrays are reached through CUDA IPC (one process per GPU on one node); of the new state only
+        # the 2-D part is exchanged, and its arrival says that the neighbour's puts (enqueued before its pack) are complete
+        self.fused_put = bool(fused_put) and self.world > 1
+        if self.fused_put:
+            peers = [None] * self.world
+            dist.all_gather_object(peers, self.model.peer_export())
+            for t in self.transfers:
+                if t.src == self.rank:
+                    self.model.peer_attach(1 if t.dst > t.src else 0, peers[t.dst], t.src_row, t.dst_row, t.nrows, False)
 
     def _buffer(self, key, nbytes):
         if (key, nbytes) not in self._buf:
@@ -260,7 +276,7 @@ class DistBand:
                 self.model.step_part(part)
                 g = group_after_part(part, self.parts)
                 if g is not None and self.world > 1:
-                    self.exchange(g)
+                    self.exchange(STATE_2D if (g == STATE and self.fused_put) else g)
 
     def own_fields(self, names=("u", "v", "T", "S", "w", "eta")):
         """This band's own rows (global rows self.own[rank])."""

@@ -89,6 +89,26 @@ struct DevP {
     unsigned long long* timeline;   // [8 warps][8]: cycles per phase + iterations (filled by OCN_K1_TIMELINE builds only)
 };
 
+// Latitude bands with fused puts: rows [lo, hi) of this model are ALSO stored into the neighbouring band's arrays
+// (peer memory: the same device, or another GPU's over NVLink) by the kernel that produces the new 3-D state, and rows outside
+// [own_lo, own_hi) are not stored at all (the neighbour that owns them stores them here the same way).  Only arrays that no
+// other part of a step touches are put this way: (u, v), (T, S), p.  The 2-D state is scratch of the sub-cycle until a step ends.
+template <class T>
+struct PeerSide {
+    typedef typename Pair<T>::type T2;
+    int lo, hi;            // local rows that are mirrored (hi <= lo: none)
+    int dj;                // the neighbour's row of my row j is j + dj
+    int ny;                // the neighbour's ny
+    long long sz;          // the neighbour's level stride (its sx is mine)
+    T2 *uv, *ts;
+    double* p;
+};
+template <class T>
+struct PeerPut {
+    PeerSide<T> side[2];   // 0: the band to the south, 1: the band to the north
+    int own_lo, own_hi;
+};
+
 template <class T>
 __device__ __forceinline__ T ldg(const T* p) { return __ldg(p); }
 

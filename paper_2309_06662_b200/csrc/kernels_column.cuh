@@ -371,13 +371,17 @@ __global__ void __launch_bounds__(256) k_barotropic_finish(const DevP<T> P) {
 // K1) and the correction (Ubar - SU) / Hu is known before the sweep.
 // ---------------------------------------------------------------------------------------------
 // RI = true (closure 1): the modified super-diagonals come from the arrays K5 wrote instead of the tables.
-template <class T, bool RI>
-__global__ void __launch_bounds__(128, sizeof(T) == 8 ? 4 : 8) k_backsub_correct(const DevP<T> P) {
+// PUT (latitude bands with fused puts): only own rows are processed, and what is stored in rows a neighbouring band
+// overlaps is stored into the neighbour's arrays as well (Q; peer memory), so the new state needs no exchange afterwards.
+template <class T, bool RI, bool PUT = false>
+__global__ void __launch_bounds__(128, sizeof(T) == 8 ? 4 : (PUT ? 6 : 8)) k_backsub_correct(const DevP<T> P, const PeerPut<T> Q) {
     typedef Ex<T> E;
     typedef typename Pair<T>::type T2;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
     if (j >= P.ny) return;                                  // uniform over the warp (blockDim.x is a multiple of 32)
+    if (PUT && (j < Q.own_lo || j >= Q.own_hi)) return;     // (uniform too) rows of the neighbour: it stores them here
+    const bool to0 = PUT && j >= Q.side[0].lo && j < Q.side[0].hi, to1 = PUT && j >= Q.side[1].lo && j < Q.side[1].hi;
     const bool incol = i < P.nx;
     const int sx = P.sx, nz = P.nz;
     const long long sz = P.sz, c = (long long)(j + OCN_HALO) * sx + min(i, P.nx - 1);
@@ -401,9 +405,15 @@ __global__ void __launch_bounds__(128, sizeof(T) == 8 ? 4 : 8) k_backsub_correct
     double b1 = 0, pk = 0;
     // columns next to a periodic edge also write their halo images; all others store straight
     const bool edge = (P.px && (i < OCN_HALO || i >= P.nx - OCN_HALO)) || (P.py && (j < OCN_HALO || j >= P.ny - OCN_HALO));
-    auto put = [&](auto* plane, long long o, auto val) {
+    // q0, q1: the same array of the southern / northern neighbour (PUT only)
+    auto put = [&](auto* plane, auto* q0, auto* q1, int k, auto val) {
+        const long long o = k * sz + c;
         if (edge) store_halo(plane + (o - c), sx, P.nx, P.ny, P.px, P.py, j, i, val);
         else plane[o] = val;
+        if constexpr (PUT) {
+            if (to0) store_halo(q0 + k * Q.side[0].sz, sx, P.nx, Q.side[0].ny, P.px, 0, j + Q.side[0].dj, i, val);
+            if (to1) store_halo(q1 + k * Q.side[1].sz, sx, P.nx, Q.side[1].ny, P.px, 0, j + Q.side[1].dj, i, val);
+        }
     };
     constexpr int NB = 3;                                  // levels whose loads are in flight together (measured best with 8 CTAs / SM)
     for (int k0 = nz - 1; k0 >= kg; k0 -= NB) {
@@ -435,15 +445,15 @@ __global__ void __launch_bounds__(128, sizeof(T) == 8 ? 4 : 8) k_backsub_correct
                 ots = mk2(xt, xs); op = pk;
             }
             const long long o = k * sz + c;
-            put(P.ts, o, ots);
-            put(P.p, o, op);
+            put(P.ts, Q.side[0].ts, Q.side[1].ts, k, ots);
+            put(P.p, Q.side[0].p, Q.side[1].p, k, op);
             if (k >= kguv) {
                 const bool mu = k >= tx1, mv = k >= ty1;
                 T un = 0, vn = 0;
                 if (mu) { xu = E::sub(d_uv[q].x, E::mul(RI ? c_uv[q].x : cpu[k * nz], xu)); un = xu + cu; }
                 if (mv) { xv = E::sub(d_uv[q].y, E::mul(RI ? c_uv[q].y : cpv[k * nz], xv)); vn = xv + cv; }
                 if (sizeof(T) == 8) { if (mu | mv) P.uv[o] = mk2(xu * T(mu), xv * T(mv)); }    // u**, corrected below
-                else put(P.uv, o, mk2(un, vn));
+                else put(P.uv, Q.side[0].uv, Q.side[1].uv, k, mk2(un, vn));
             }
         }
     }
@@ -464,6 +474,10 @@ __global__ void __launch_bounds__(128, sizeof(T) == 8 ? 4 : 8) k_backsub_correct
             const T un = k >= tx1 ? (T)(X((double)q.x) + X(cu2)).v : T(0);
             const T vn = k >= ty1 ? (T)(X((double)q.y) + X(cv2)).v : T(0);
             store_halo(P.uv + k * sz, sx, P.nx, P.ny, P.px, P.py, j, i, mk2(un, vn));
+            if constexpr (PUT) {
+                if (to0) store_halo(Q.side[0].uv + k * Q.side[0].sz, sx, P.nx, Q.side[0].ny, P.px, 0, j + Q.side[0].dj, i, mk2(un, vn));
+                if (to1) store_halo(Q.side[1].uv + k * Q.side[1].sz, sx, P.nx, Q.side[1].ny, P.px, 0, j + Q.side[1].dj, i, mk2(un, vn));
+            }
         }
     }
 }

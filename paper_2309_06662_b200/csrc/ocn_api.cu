@@ -89,6 +89,11 @@ struct ocn_model {
     // split step (ocn_step_part): the next part expected, and whether the step in progress is the Euler start
     int split_next = 0;
     bool split_euler = false;
+    // fused puts into neighbouring bands (ocn_peer_attach): what the last part of a step also stores into peer memory
+    bool put = false;
+    ocn::PeerPut<float> qf{};
+    ocn::PeerPut<double> qd{};
+    std::vector<void*> ipc_open;        // bases mapped with cudaIpcOpenMemHandle
     // per-stage timing (ocn_profile_*)
     bool profiling = false;
     std::vector<cudaEvent_t> ev_pool;   // OCN_NSTAGES + 1 events per profiled step
@@ -99,10 +104,13 @@ struct ocn_model {
 
 namespace {
 
+// ipc: an array a neighbouring band in another process maps through CUDA IPC (ocn_peer_export).  The driver carves small
+// allocations out of shared 2 MiB pages and an IPC handle names the whole page, so these get whole pages of their own.
 template <class T>
-ocn_status dev_alloc(ocn_model* M, size_t n, T** out, bool lead) {
+ocn_status dev_alloc(ocn_model* M, size_t n, T** out, bool lead, bool ipc = false) {
     void* p = nullptr;
-    const size_t total = (n + (lead ? 2 * LEAD : 0)) * sizeof(T);
+    size_t total = (n + (lead ? 2 * LEAD : 0)) * sizeof(T);
+    if (ipc) total = (total + ((size_t)2 << 20) - 1) / ((size_t)2 << 20) * ((size_t)2 << 20);
     CK(cudaMalloc(&p, total));
     CK(cudaMemsetAsync(p, 0, total, M->stream));
     M->allocs.push_back(p);
@@ -122,6 +130,10 @@ ocn_status upload(ocn_model* M, const std::vector<double>& src, const T** out) {
     *out = p;
     return OCN_OK;
 }
+
+template <class T> ocn::PeerPut<T>& peer_put(ocn_model* M);
+template <> ocn::PeerPut<float>& peer_put<float>(ocn_model* M) { return M->qf; }
+template <> ocn::PeerPut<double>& peer_put<double>(ocn_model* M) { return M->qd; }
 
 template <class T>
 ocn::DevP<T>& params(ocn_model* M);
@@ -205,8 +217,8 @@ ocn_status build_model(ocn_model* M) {
     };
     typedef typename ocn::Pair<T>::type T2;
     T2** f3[] = {&P.uv, &P.ts, &P.duv, &P.dts, &P.Guv, &P.Gts};
-    for (T2** f : f3) if ((s = dev_alloc(M, n3, f, true)) != OCN_OK) return s;
-    if ((s = dev_alloc(M, n3, &P.p, true)) != OCN_OK) return s;
+    for (T2** f : f3) if ((s = dev_alloc(M, n3, f, true, f == &P.uv || f == &P.ts)) != OCN_OK) return s;
+    if ((s = dev_alloc(M, n3, &P.p, true, true)) != OCN_OK) return s;
     if ((s = plane(n3 + n2, &P.w)) != OCN_OK) return s;
     P.closure = M->d.closure; P.nk = nullptr; P.cpuv = nullptr; P.cpt = nullptr;
     if (M->d.closure == 1) {                       // the per-column super-diagonals K1 leaves for K3
@@ -444,11 +456,17 @@ ocn_status launch_step(ocn_model* M, bool euler, int part = -1) {
         }
     }
     if (part >= 0 && part != last_part) { CK(cudaGetLastError()); return OCN_OK; }
+    const ocn::PeerPut<T>& Q = peer_put<T>(M);
     ocn::k_barotropic_finish<T><<<grid2(g, b2), b2, 0, M->stream>>>(P);
     MARK(1, (M->d.substeps + bt_substeps_per_launch<T>() - 1) / bt_substeps_per_launch<T>() + 1);
     MARK(3, 0);                                    // (the closure is evaluated inside K1: stage 3 is empty)
-    if (M->d.closure == 1) ocn::k_backsub_correct<T, true><<<grid2(g, bc), bc, 0, M->stream>>>(P);
-    else ocn::k_backsub_correct<T, false><<<grid2(g, bc), bc, 0, M->stream>>>(P);
+    if (M->put) {
+        if (M->d.closure == 1) ocn::k_backsub_correct<T, true, true><<<grid2(g, bc), bc, 0, M->stream>>>(P, Q);
+        else ocn::k_backsub_correct<T, false, true><<<grid2(g, bc), bc, 0, M->stream>>>(P, Q);
+    } else {
+        if (M->d.closure == 1) ocn::k_backsub_correct<T, true><<<grid2(g, bc), bc, 0, M->stream>>>(P, Q);
+        else ocn::k_backsub_correct<T, false><<<grid2(g, bc), bc, 0, M->stream>>>(P, Q);
+    }
     MARK(2, 1);
 #undef MARK
     CK(cudaGetLastError());
@@ -818,6 +836,7 @@ ocn_status ocn_model_destroy(ocn_model* M) {
         if (st->freed) cudaEventDestroy(st->freed);
     }
     for (cudaEvent_t e : M->ticket_ev) if (e) cudaEventDestroy(e);
+    for (void* b : M->ipc_open) cudaIpcCloseMemHandle(b);
     if (M->own_stream && M->stream) cudaStreamDestroy(M->stream);
     delete M;
     return OCN_OK;
@@ -855,6 +874,7 @@ int row_arrays(ocn_model* M, int group, RowArray* out) {
             add(P.uv, 2 * sizeof(T), nz); add(P.ts, 2 * sizeof(T), nz); add(P.p, sizeof(double), nz);
             add(P.eta[0], sizeof(T), 1); add(P.U[0], sizeof(T), 1); add(P.V[0], sizeof(T), 1);
             break;
+        case OCN_ROWS_STATE_2D: add(P.eta[0], sizeof(T), 1); add(P.U[0], sizeof(T), 1); add(P.V[0], sizeof(T), 1); break;
         case OCN_ROWS_FORCING: add(P.GU, sizeof(T), 1); add(P.GV, sizeof(T), 1); break;
         case OCN_ROWS_BAROTROPIC_0: case OCN_ROWS_BAROTROPIC_1: {
             const int b = group - OCN_ROWS_BAROTROPIC_0;
@@ -909,6 +929,77 @@ ocn_status ocn_step_part(ocn_model* M, int part) {
     if (s != OCN_OK) return s;
     if (part == np - 1) { M->have_history = true; M->split_next = 0; }
     else M->split_next = part + 1;
+    return OCN_OK;
+}
+
+// ---- fused puts: the arrays of the new state as seen by a neighbouring band ----
+extern "C++" {
+namespace {
+template <class T>
+void peer_arrays(ocn_model* M, void** out) {
+    ocn::DevP<T>& P = params<T>(M);
+    out[0] = P.uv; out[1] = P.ts; out[2] = P.p;
+}
+template <class T>
+void peer_fill(ocn_model* M, int side, void* const* a, int lo, int rows, int dj, int peer_ny, long long peer_sz) {
+    typedef typename ocn::Pair<T>::type T2;
+    ocn::PeerPut<T>& Q = peer_put<T>(M);
+    ocn::PeerSide<T>& S = Q.side[side];
+    S.lo = lo; S.hi = lo + rows; S.dj = dj; S.ny = peer_ny; S.sz = peer_sz;
+    S.uv = (T2*)a[0]; S.ts = (T2*)a[1]; S.p = (double*)a[2];
+    if (side == 0) Q.own_lo = lo; else Q.own_hi = lo + rows;
+}
+}  // namespace
+}  // extern "C++"
+
+ocn_status ocn_peer_export(ocn_model* M, ocn_peer* out) {
+    if (!M || !out) return fail(OCN_EINVAL, "null argument");
+    ON_DEVICE(M->d.device);
+    std::memset(out, 0, sizeof(*out));
+    out->nx = M->g->nx; out->ny = M->g->ny; out->nz = M->g->nz; out->precision = M->prec; out->sx = M->g->sx; out->sy = M->g->sy;
+    out->device = M->d.device;
+    if (M->prec == 32) peer_arrays<float>(M, out->ptr); else peer_arrays<double>(M, out->ptr);
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "ipc handle size");
+    for (int a = 0; a < OCN_PEER_ARRAYS; ++a) {
+        void* base = nullptr;                      // the allocation that holds the array (the largest base below it)
+        for (void* b : M->allocs) if (b <= out->ptr[a] && (!base || b > base)) base = b;
+        if (!base) return fail(OCN_ESTATE, "array without an allocation");
+        cudaIpcMemHandle_t h;
+        CK(cudaIpcGetMemHandle(&h, base));
+        std::memcpy(out->ipc[a], &h, 64);
+        out->ipc_offset[a] = (unsigned long long)((char*)out->ptr[a] - (char*)base);
+    }
+    return OCN_OK;
+}
+
+ocn_status ocn_peer_attach(ocn_model* M, int side, const ocn_peer* peer, int my_first_row, int peer_first_row, int rows, int same_process) {
+    if (!M || !peer) return fail(OCN_EINVAL, "null argument");
+    if (side != 0 && side != 1) return fail(OCN_EINVAL, "side must be 0 (south) or 1 (north)");
+    if (peer->nx != M->g->nx || peer->nz != M->g->nz || peer->precision != M->prec || peer->sx != M->g->sx)
+        return fail(OCN_EINVAL, "the neighbouring band must have the same nx, nz and precision");
+    if (rows < 1 || my_first_row < 0 || my_first_row + rows > M->g->ny || peer_first_row < 0 || peer_first_row + rows > peer->ny)
+        return fail(OCN_EINVAL, "rows outside a grid");
+    if (M->split_next != 0) return fail(OCN_ESTATE, "a split step is in progress");
+    ON_DEVICE(M->d.device);
+    void* arr[OCN_PEER_ARRAYS];
+    for (int a = 0; a < OCN_PEER_ARRAYS; ++a) {
+        if (same_process) { arr[a] = peer->ptr[a]; continue; }
+        cudaIpcMemHandle_t h;
+        std::memcpy(&h, peer->ipc[a], 64);
+        void* base = nullptr;
+        CK(cudaIpcOpenMemHandle(&base, h, cudaIpcMemLazyEnablePeerAccess));
+        M->ipc_open.push_back(base);
+        arr[a] = (char*)base + peer->ipc_offset[a];
+    }
+    const long long psz = (long long)peer->sx * peer->sy;
+    if (M->prec == 32) peer_fill<float>(M, side, arr, my_first_row, rows, peer_first_row - my_first_row, peer->ny, psz);
+    else peer_fill<double>(M, side, arr, my_first_row, rows, peer_first_row - my_first_row, peer->ny, psz);
+    if (!M->put) {                                 // first attachment: the other side has no neighbour yet
+        if (side == 0) { M->qf.own_hi = M->qd.own_hi = M->g->ny; M->qf.side[1].lo = M->qf.side[1].hi = M->qd.side[1].lo = M->qd.side[1].hi = 0; }
+        else { M->qf.own_lo = M->qd.own_lo = 0; M->qf.side[0].lo = M->qf.side[0].hi = M->qd.side[0].lo = M->qd.side[0].hi = 0; }
+    }
+    M->put = true;
+    if (M->graph) { cudaGraphExecDestroy(M->graph); M->graph = nullptr; }     // the captured step stored without puts
     return OCN_OK;
 }
 

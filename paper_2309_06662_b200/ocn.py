@@ -45,13 +45,19 @@ class ocn_fields(C.Structure):
                                           "flux_T", "flux_S", "restore_T", "restore_S")] + [("on_device", C.c_int)]
 
 
+class ocn_peer(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int), ("precision", C.c_int), ("sx", C.c_int), ("sy", C.c_int),
+                ("device", C.c_int), ("ptr", C.c_void_p * 3), ("ipc", (C.c_ubyte * 64) * 3), ("ipc_offset", C.c_ulonglong * 3)]
+
+
 EXPORTS = ["ocn_grid_create", "ocn_grid_destroy", "ocn_model_create", "ocn_model_destroy", "ocn_set_fields",
            "ocn_time_step", "ocn_get_fields", "ocn_synchronize", "ocn_get_masks", "ocn_model_info",
            "ocn_get_debug", "ocn_last_error", "ocn_version", "ocn_profile_enable", "ocn_profile_read",
            "ocn_stage_name", "ocn_get_mixing", "ocn_get_fields_async", "ocn_wait", "ocn_tune", "ocn_selftest_division", "ocn_get_timeline",
            "ocn_get_mixing_noalloc", "ocn_noalloc_scratch_bytes",
-           "ocn_step_parts", "ocn_step_part", "ocn_rows_bytes", "ocn_pack_rows", "ocn_unpack_rows", "ocn_band_overlap"]
-ROWS_STATE, ROWS_FORCING, ROWS_BAROTROPIC_0, ROWS_BAROTROPIC_1 = 0, 1, 2, 3
+           "ocn_step_parts", "ocn_step_part", "ocn_rows_bytes", "ocn_pack_rows", "ocn_unpack_rows", "ocn_band_overlap",
+           "ocn_peer_export", "ocn_peer_attach"]
+ROWS_STATE, ROWS_FORCING, ROWS_BAROTROPIC_0, ROWS_BAROTROPIC_1, ROWS_STATE_2D = 0, 1, 2, 3, 4
 NSTAGES = 4
 
 
@@ -92,6 +98,8 @@ def lib():
         L.ocn_pack_rows.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp]
         L.ocn_unpack_rows.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp]
         L.ocn_band_overlap.argtypes = [C.c_int, C.c_int]
+        L.ocn_peer_export.argtypes = [vp, C.POINTER(ocn_peer)]
+        L.ocn_peer_attach.argtypes = [vp, C.c_int, C.POINTER(ocn_peer), C.c_int, C.c_int, C.c_int, C.c_int]
         L.ocn_stage_name.restype = C.c_char_p
         L.ocn_stage_name.argtypes = [C.c_int]
         _lib = L
@@ -236,6 +244,17 @@ class Model:
 
     def pack_rows(self, group, j_begin, nrows, dst_device_ptr):
         _check(lib().ocn_pack_rows(self.h, int(group), int(j_begin), int(nrows), C.c_void_p(int(dst_device_ptr))))
+
+    def peer_export(self):
+        """ocn_peer_export as bytes (plain data: addresses for this process, CUDA IPC handles for another)."""
+        p = ocn_peer()
+        _check(lib().ocn_peer_export(self.h, C.byref(p)))
+        return bytes(p)
+
+    def peer_attach(self, side, peer_bytes, my_first_row, peer_first_row, rows, same_process):
+        p = ocn_peer.from_buffer_copy(peer_bytes)
+        _check(lib().ocn_peer_attach(self.h, int(side), C.byref(p), int(my_first_row), int(peer_first_row), int(rows),
+                                     int(bool(same_process))))
 
     def unpack_rows(self, group, j_begin, nrows, src_device_ptr):
         _check(lib().ocn_unpack_rows(self.h, int(group), int(j_begin), int(nrows), C.c_void_p(int(src_device_ptr))))

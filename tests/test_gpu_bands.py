@@ -85,7 +85,7 @@ def test_rows_round_trip_and_are_checked():
     wl = _workload(64)
     a, b = ocn.Model(wl), ocn.Model(wl)
     a.time_step(3); b.time_step(1)                                 # different states
-    for group in (ocn.ROWS_STATE, ocn.ROWS_FORCING, ocn.ROWS_BAROTROPIC_0, ocn.ROWS_BAROTROPIC_1):
+    for group in (ocn.ROWS_STATE, ocn.ROWS_STATE_2D, ocn.ROWS_FORCING, ocn.ROWS_BAROTROPIC_0, ocn.ROWS_BAROTROPIC_1):
         nb = a.rows_bytes(group, a.ny)
         buf = torch.empty(nb, dtype=torch.uint8, device="cuda")
         a.synchronize(); b.synchronize()
@@ -99,6 +99,7 @@ def test_rows_round_trip_and_are_checked():
     sx = (a.nx + 8 + 31) // 32 * 32
     assert a.rows_bytes(ocn.ROWS_FORCING, 7) == 2 * 7 * sx * 8
     assert a.rows_bytes(ocn.ROWS_STATE, 2) == 2 * sx * (25 * (16 + 16 + 8) + 3 * 8)
+    assert a.rows_bytes(ocn.ROWS_STATE_2D, 2) == 2 * sx * 3 * 8
     with pytest.raises(RuntimeError, match="rows outside the grid"):
         a.pack_rows(ocn.ROWS_STATE, a.ny - 2, 3, buf.data_ptr())
     with pytest.raises(RuntimeError, match="unknown row group"):
@@ -230,3 +231,74 @@ def test_bench_bands_line():
     b = d["bands"]
     assert b["n"] == 3 and b["overlap_rows"] == 11 and sum(b["own_rows"]) == 600 and b["exchanges_per_step"] == b["parts_per_step"] - 1
     assert b["ms_per_step_per_band"] > 0 and 1.0 < b["projected_speedup_on_n_gpus"] < 3.0
+
+
+# ---- fused puts: the last part of a step stores the overlap rows of the neighbours itself (no exchange of the new state) ----
+@pytest.mark.parametrize("prec,kind,nb", [(64, "r", 3), (64, "db", 2), (32, "", 2), (32, "r", 4), (32, "dbz", 3)])
+def test_bands_with_fused_puts_are_bit_identical_to_the_whole_grid(prec, kind, nb):
+    wl = _workload(prec, kind)
+    whole = ocn.Model(wl)
+    B = bands.Bands(wl, nb, fused_put=True)
+    whole.time_step(6); B.time_step(6)
+    fw, fb = whole.get_fields(), B.get_fields()
+    for k in FIELDS:
+        assert np.array_equal(fw[k], fb[k]), (prec, kind, nb, k)
+    whole.close(); B.close()
+
+
+def test_peer_attach_is_checked():
+    a, b = ocn.Model(_workload(32)), ocn.Model(_workload(64))
+    with pytest.raises(RuntimeError, match="same nx, nz and precision"):
+        a.peer_attach(0, b.peer_export(), 0, 0, 4, True)
+    c = ocn.Model(_workload(32))
+    with pytest.raises(RuntimeError, match="rows outside a grid"):
+        a.peer_attach(1, c.peer_export(), a.ny - 2, 0, 4, True)
+    with pytest.raises(RuntimeError, match="side must be"):
+        a.peer_attach(2, c.peer_export(), 0, 0, 4, True)
+    for m in (a, b, c):
+        m.close()
+
+
+def _rank_worker_put(rank, world, port, prec, kind, steps, out):
+    import os
+    import torch
+    import torch.distributed as dist
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        torch.cuda.set_device(0)
+        s = torch.cuda.Stream()
+        with torch.cuda.stream(s):
+            D = bands.DistBand(_workload(prec, kind), dist, device=0, stream=s.cuda_stream, host_staging=True, fused_put=True)
+            D.time_step(steps)
+            f = D.own_fields(FIELDS)
+        out.put((rank, D.own[rank], {k: np.array(v) for k, v in f.items()}))
+        dist.barrier()
+        D.close()
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("prec,kind,world", [(32, "r", 2), (64, "", 3)])
+def test_fused_puts_across_processes_through_cuda_ipc(prec, kind, world):
+    """One band per process, all on this one GPU: the new state reaches the neighbour through CUDA IPC mappings written by the
+    producing kernels; the small 2-D groups and the per-step tokens travel over gloo."""
+    import torch.multiprocessing as mp
+    steps = 4
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    ps = [ctx.Process(target=_rank_worker_put, args=(r, world, port, prec, kind, steps, q)) for r in range(world)]
+    for p in ps:
+        p.start()
+    whole = ocn.Model(_workload(prec, kind))
+    whole.time_step(steps)
+    fw = whole.get_fields()
+    whole.close()
+    res = sorted((q.get(timeout=600) for _ in ps), key=lambda r: r[0])
+    for p in ps:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    for rank, own, f in res:
+        for k in FIELDS:
+            assert np.array_equal(f[k], fw[k][..., own[0]:own[1], :]), (rank, k)
