@@ -242,7 +242,7 @@ unsigned long long ocn_noalloc_scratch_bytes(void);
  *   bit for bit (same kernels, launched directly instead of through the captured graph).
  * ocn_rows_bytes: size of the packed rows of a group.  ocn_pack_rows / ocn_unpack_rows: rows j_begin .. j_begin + nrows - 1
  *   (with their x-halo images) of every array of the group -> / <- one contiguous DEVICE buffer of that size, enqueued on
- *   the model's stream (device-to-device copies; no host synchronisation; nothing is allocated).  The buffer is the
+ *   the model's stream (one copy kernel per call; no host synchronisation; nothing is allocated).  The 16-byte aligned buffer is the
  *   caller's (e.g. a torch tensor handed to NCCL send / recv); it must stay valid until the stream has passed the call.
  *   Packing from one model and unpacking into another of the same nx, nz and precision is the whole exchange.
  * Errors: OCN_EINVAL (null, rows outside the grid, unknown group), OCN_ESTATE, OCN_ECUDA. */

@@ -365,22 +365,39 @@ __global__ void __launch_bounds__(256) k_barotropic_finish(const DevP<T> P) {
 }
 
 // ---------------------------------------------------------------------------------------------
+// Rows of up to 8 plane-layout arrays <-> one contiguous buffer in ONE launch (ocn_pack_rows / ocn_unpack_rows: the overlap
+// rows of a latitude band).  Every chunk is a whole number of 16-byte words (sx is a multiple of 32 elements
+// and a chunk starts 4 elements before a row): plain uint4 copies, x = words of a plane's chunk, y = plane, z = array.
+// ---------------------------------------------------------------------------------------------
+struct RowMoves {
+    struct One { const uint4* src; uint4* dst; long long src_pitch, dst_pitch; int planes; } a[8];   // pitches in 16-byte words
+    unsigned w[8];                                                                                     // words of one plane's chunk
+};
+__global__ void __launch_bounds__(256) k_move_rows(const RowMoves R) {
+    const RowMoves::One& A = R.a[blockIdx.z];
+    const unsigned x = blockIdx.x * blockDim.x + threadIdx.x;
+    if (x >= R.w[blockIdx.z]) return;
+    for (int pl = blockIdx.y; pl < A.planes; pl += gridDim.y) A.dst[pl * A.dst_pitch + x] = A.src[pl * A.src_pitch + x];
+}
+
+// ---------------------------------------------------------------------------------------------
 // S4 (back-substitution, top-down) + S7 (barotropic correction) + S9 (hydrostatic pressure of
 // the new T, S, integrated downward from the surface in the same sweep).
 // The implicit operator conserves the column integral, so sum_k dz u** = sum_k dz u* (SU from
 // K1) and the correction (Ubar - SU) / Hu is known before the sweep.
 // ---------------------------------------------------------------------------------------------
 // RI = true (closure 1): the modified super-diagonals come from the arrays K5 wrote instead of the tables.
-// PUT (latitude bands with fused puts): only own rows are processed, and what is stored in rows a neighbouring band
-// overlaps is stored into the neighbour's arrays as well (Q; peer memory), so the new state needs no exchange afterwards.
+// The launch covers rows Q.own_lo .. Q.own_hi - 1 (all rows of a model on its own).
+// PUT (latitude bands with fused puts): what is stored in rows a neighbouring band overlaps is stored into the
+// neighbour's arrays as well (Q.side; peer memory), so the new 3-D state needs no exchange afterwards.  The host launches this
+// variant on the mirrored rows only and the plain one on the rows in between; the band's own overlap rows are not processed at all.
 template <class T, bool RI, bool PUT = false>
 __global__ void __launch_bounds__(128, sizeof(T) == 8 ? 4 : (PUT ? 6 : 8)) k_backsub_correct(const DevP<T> P, const PeerPut<T> Q) {
     typedef Ex<T> E;
     typedef typename Pair<T>::type T2;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const int j = blockIdx.y * blockDim.y + threadIdx.y;
-    if (j >= P.ny) return;                                  // uniform over the warp (blockDim.x is a multiple of 32)
-    if (PUT && (j < Q.own_lo || j >= Q.own_hi)) return;     // (uniform too) rows of the neighbour: it stores them here
+    const int j = Q.own_lo + blockIdx.y * blockDim.y + threadIdx.y;
+    if (j >= Q.own_hi) return;                              // uniform over the warp (blockDim.x is a multiple of 32)
     const bool to0 = PUT && j >= Q.side[0].lo && j < Q.side[0].hi, to1 = PUT && j >= Q.side[1].lo && j < Q.side[1].hi;
     const bool incol = i < P.nx;
     const int sx = P.sx, nz = P.nz;

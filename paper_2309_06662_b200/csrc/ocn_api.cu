@@ -460,12 +460,30 @@ ocn_status launch_step(ocn_model* M, bool euler, int part = -1) {
     ocn::k_barotropic_finish<T><<<grid2(g, b2), b2, 0, M->stream>>>(P);
     MARK(1, (M->d.substeps + bt_substeps_per_launch<T>() - 1) / bt_substeps_per_launch<T>() + 1);
     MARK(3, 0);                                    // (the closure is evaluated inside K1: stage 3 is empty)
-    if (M->put) {
-        if (M->d.closure == 1) ocn::k_backsub_correct<T, true, true><<<grid2(g, bc), bc, 0, M->stream>>>(P, Q);
-        else ocn::k_backsub_correct<T, false, true><<<grid2(g, bc), bc, 0, M->stream>>>(P, Q);
-    } else {
-        if (M->d.closure == 1) ocn::k_backsub_correct<T, true><<<grid2(g, bc), bc, 0, M->stream>>>(P, Q);
-        else ocn::k_backsub_correct<T, false><<<grid2(g, bc), bc, 0, M->stream>>>(P, Q);
+    {
+        // rows lo .. hi - 1 with the plain kernel or with the one that also stores into the neighbours' arrays
+        auto k3 = [&](int lo, int hi, bool put) {
+            if (hi <= lo) return;
+            ocn::PeerPut<T> R = Q;
+            R.own_lo = lo; R.own_hi = hi;
+            const dim3 gk((g->nx + bc.x - 1) / bc.x, (hi - lo + bc.y - 1) / bc.y);
+            const bool ri = M->d.closure == 1;
+            if (put) {
+                if (ri) ocn::k_backsub_correct<T, true, true><<<gk, bc, 0, M->stream>>>(P, R);
+                else ocn::k_backsub_correct<T, false, true><<<gk, bc, 0, M->stream>>>(P, R);
+            } else {
+                if (ri) ocn::k_backsub_correct<T, true><<<gk, bc, 0, M->stream>>>(P, R);
+                else ocn::k_backsub_correct<T, false><<<gk, bc, 0, M->stream>>>(P, R);
+            }
+        };
+        if (!M->put) k3(0, g->ny, false);
+        else {                                     // own rows only: the mirrored rows at either end with puts, the rest plain
+            const int s_hi = std::max(Q.own_lo, std::min(Q.side[0].hi, Q.own_hi)), n_lo = std::min(Q.own_hi, std::max(Q.side[1].lo, s_hi));
+            k3(Q.own_lo, Q.side[0].hi > Q.side[0].lo ? s_hi : Q.own_lo, true);
+            const int mid_lo = Q.side[0].hi > Q.side[0].lo ? s_hi : Q.own_lo, mid_hi = Q.side[1].hi > Q.side[1].lo ? n_lo : Q.own_hi;
+            k3(mid_lo, mid_hi, false);
+            k3(mid_hi, Q.own_hi, true);
+        }
     }
     MARK(2, 1);
 #undef MARK
@@ -900,13 +918,24 @@ ocn_status move_rows(ocn_model* M, int group, int j_begin, int nrows, char* buf,
     if (nrows == 0) return OCN_OK;
     const size_t chunk = (size_t)nrows * g->sx, sz = (size_t)g->sx * g->sy;
     const long long off = (long long)(j_begin + OCN_HALO) * g->sx - 4;
+    if (((uintptr_t)buf & 15u) != 0) return fail(OCN_EINVAL, "the row buffer must be 16-byte aligned");
+    ocn::RowMoves R{};
+    unsigned wmax = 0;
+    int pmax = 1;
     for (int a = 0; a < na; ++a) {
         char* dev = arr[a].base + off * (long long)arr[a].es;
-        const size_t w = chunk * arr[a].es;
-        if (pack) CK(cudaMemcpy2DAsync(buf, w, dev, sz * arr[a].es, w, arr[a].planes, cudaMemcpyDeviceToDevice, M->stream));
-        else CK(cudaMemcpy2DAsync(dev, sz * arr[a].es, buf, w, w, arr[a].planes, cudaMemcpyDeviceToDevice, M->stream));
+        const size_t w = chunk * arr[a].es;                 // bytes of one plane's chunk: a multiple of 128
+        ocn::RowMoves::One& A = R.a[a];
+        A.planes = arr[a].planes;
+        if (pack) { A.src = (const uint4*)dev; A.dst = (uint4*)buf; A.src_pitch = (long long)(sz * arr[a].es / 16); A.dst_pitch = (long long)(w / 16); }
+        else { A.src = (const uint4*)buf; A.dst = (uint4*)dev; A.src_pitch = (long long)(w / 16); A.dst_pitch = (long long)(sz * arr[a].es / 16); }
+        R.w[a] = (unsigned)(w / 16);
+        wmax = std::max(wmax, R.w[a]);
+        pmax = std::max(pmax, arr[a].planes);
         buf += w * arr[a].planes;
     }
+    ocn::k_move_rows<<<dim3((wmax + 255) / 256, std::min(pmax, 32), na), 256, 0, M->stream>>>(R);
+    CK(cudaGetLastError());
     return OCN_OK;
 }
 }  // namespace
