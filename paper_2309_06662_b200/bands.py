@@ -102,6 +102,15 @@ def band_workload(wl, ext, name=None):
     return out
 
 
+FORCING_FIELDS = ("tau_x", "tau_y", "flux_T", "flux_S", "restore_T", "restore_S")
+
+
+def _forcing_only(fields):
+    bad = [k for k in fields if k not in FORCING_FIELDS]
+    if bad:
+        raise ValueError("set_forcing takes %s, not %s" % (", ".join(FORCING_FIELDS), ", ".join(bad)))
+
+
 def overlap_rows(wl):
     return ocn.band_overlap(wl["params"]["precision"], wl["params"]["substeps"])
 
@@ -163,6 +172,13 @@ class Bands:
                 g = group_after_part(part, self.parts)
                 if g is not None and len(self.models) > 1:
                     self.exchange(STATE_2D if (g == STATE and self.fused_put) else g)
+
+    def set_forcing(self, **fields):
+        """Whole-grid forcing fields (tau_x, tau_y, flux_T, flux_S, restore_T, restore_S; host arrays of ny x nx) to every band:
+        each gets the rows it covers.  State fields are set through the workload (they restart the time stepping)."""
+        _forcing_only(fields)
+        for m, e in zip(self.models, self.ext):
+            m.set_fields(**{k: np.ascontiguousarray(v[e[0]:e[1]]) for k, v in fields.items()})
 
     def synchronize(self):
         for m in self.models:
@@ -277,6 +293,12 @@ class DistBand:
                 g = group_after_part(part, self.parts)
                 if g is not None and self.world > 1:
                     self.exchange(STATE_2D if (g == STATE and self.fused_put) else g)
+
+    def set_forcing(self, **fields):
+        """Whole-grid forcing fields (host arrays of ny x nx): this band takes the rows it covers."""
+        _forcing_only(fields)
+        e = self.ext[self.rank]
+        self.model.set_fields(**{k: np.ascontiguousarray(v[e[0]:e[1]]) for k, v in fields.items()})
 
     def own_fields(self, names=("u", "v", "T", "S", "w", "eta")):
         """This band's own rows (global rows self.own[rank])."""

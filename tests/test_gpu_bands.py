@@ -302,3 +302,22 @@ def test_fused_puts_across_processes_through_cuda_ipc(prec, kind, world):
     for rank, own, f in res:
         for k in FIELDS:
             assert np.array_equal(f[k], fw[k][..., own[0]:own[1], :]), (rank, k)
+
+
+def test_forcing_that_changes_between_steps_reaches_every_band():
+    wl = _workload(32, "r")
+    whole = ocn.Model(wl)
+    B = bands.Bands(wl, 3)
+    rng = np.random.default_rng(8)
+    for n in range(3):
+        tx = (0.1 * rng.standard_normal(wl["fields"]["tau_x"].shape)).astype(np.float32)
+        qT = (1e-5 * rng.standard_normal(tx.shape)).astype(np.float32)
+        whole.set_fields(tau_x=tx, flux_T=qT)
+        B.set_forcing(tau_x=tx, flux_T=qT)
+        whole.time_step(2); B.time_step(2)
+    fw, fb = whole.get_fields(), B.get_fields()
+    for k in FIELDS:
+        assert np.array_equal(fw[k], fb[k]), k
+    with pytest.raises(ValueError, match="set_forcing takes"):
+        B.set_forcing(u=wl["fields"]["u"])
+    whole.close(); B.close()
