@@ -225,6 +225,21 @@ ocn_status ocn_get_mixing(ocn_model* model, double* nu, double* kappa);
 ocn_status ocn_get_mixing_noalloc(ocn_model* model, double* nu, double* kappa);
 unsigned long long ocn_noalloc_scratch_bytes(void);
 
+/* ---- Checkpoint / resume and the finite check ("a restart re-starts AB2 with an Euler step unless G- is added") ----
+ * ocn_set_fields / ocn_get_fields move the prognostic state only, and a model restarted from them takes an Euler step.  A
+ * checkpoint holds everything a step reads that an earlier step or the caller wrote — (u, v), (T, S), p, the quasi-AB2 history
+ * G^- (DESIGN.md §3.8), the barotropic state (eta, U, V) and the forcing fields — as raw device words, so a model of
+ * the same grid and parameters that loads it continues BIT FOR BIT where the saved one stood (tests/test_gpu_checkpoint.py).
+ * ocn_checkpoint_bytes: size of the blob.  ocn_checkpoint_save: blob -> HOST buffer of that size (blocks until it is there).
+ * ocn_checkpoint_load: HOST blob of `bytes` bytes -> model (blocks); the blob must come from a model of the same nx, ny, nz
+ * and precision (OCN_EINVAL otherwise: bad magic, size, shape).  The format is the library version's own (not portable).
+ * ocn_check_finite: number of NaN / infinite words in u, v, T, S, eta (0 = healthy); blocks.  Cheap enough to call every few
+ * hundred steps (three small reductions). */
+ocn_status ocn_checkpoint_bytes(const ocn_model* model, unsigned long long* bytes);
+ocn_status ocn_checkpoint_save(ocn_model* model, void* host_buffer);
+ocn_status ocn_checkpoint_load(ocn_model* model, const void* host_buffer, unsigned long long bytes);
+ocn_status ocn_check_finite(ocn_model* model, unsigned long long* nonfinite);
+
 /* ---- Latitude bands: the one exchange step of the path ----------------------------------
  * PAPER.md:98 (§5.3): the barotropic sub-cycle is stepped with a wide halo so that neighbours exchange once per group of
  * sub-steps instead of once per sub-step; one exchange of the 3-D halos per baroclinic step.  A band is an

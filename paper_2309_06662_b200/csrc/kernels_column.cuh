@@ -581,6 +581,17 @@ __global__ void k_selftest_division(unsigned long long n, unsigned long long see
 }
 
 // ---------------------------------------------------------------------------------------------
+// ocn_check_finite: counts the words of an array (any layout: halo and land hold finite zeros) that are NaN or infinite
+// ---------------------------------------------------------------------------------------------
+template <class T>
+__global__ void __launch_bounds__(256) k_count_nonfinite(const T* __restrict__ a, unsigned long long n, unsigned long long* bad) {
+    unsigned long long local = 0;
+    for (unsigned long long q = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; q < n; q += (unsigned long long)gridDim.x * blockDim.x)
+        local += !isfinite(a[q]);
+    if (local) atomicAdd(bad, local);
+}
+
+// ---------------------------------------------------------------------------------------------
 // scatter (contiguous interior -> halo'd plane layout, masked) and gather (back, land = 0)
 // st = element stride of the device array (2 = one member of a pair array, base already offset)
 // kind: 0 u, 1 v, 2 T (offset Toff), 3 S (offset Soff), 4 eta, 5 plain 2-D, 6 w (nz+1 levels, gather only),

@@ -961,6 +961,109 @@ ocn_status ocn_step_part(ocn_model* M, int part) {
     return OCN_OK;
 }
 
+// ---- checkpoint / resume and the finite check ----
+extern "C++" {
+namespace {
+struct CkptHeader {
+    char magic[8];
+    int nx, ny, nz, precision, sx, sy, have_history, reserved;
+    unsigned long long payload;
+};
+struct CkptArray { char* base; size_t bytes; };
+// everything a step reads that an earlier step or the caller wrote: state, pressure, AB2 history, the barotropic state a
+// step starts from, and the forcing fields; each as its whole plane-layout allocation (halo images included)
+template <class T>
+int ckpt_arrays(ocn_model* M, CkptArray* out) {
+    ocn::DevP<T>& P = params<T>(M);
+    const size_t n3 = (size_t)P.sz * P.nz, n2 = (size_t)P.sz;
+    int n = 0;
+    auto add = [&](void* p, size_t es, size_t cnt) { out[n++] = CkptArray{(char*)p - LEAD * es, (cnt + 2 * LEAD) * es}; };
+    add(P.uv, 2 * sizeof(T), n3); add(P.ts, 2 * sizeof(T), n3); add(P.p, sizeof(double), n3);
+    add(P.Guv, 2 * sizeof(T), n3); add(P.Gts, 2 * sizeof(T), n3);
+    add(P.eta[0], sizeof(T), n2); add(P.U[0], sizeof(T), n2); add(P.V[0], sizeof(T), n2);
+    add(P.taux, sizeof(T), n2); add(P.tauy, sizeof(T), n2); add(P.qts, 2 * sizeof(T), n2); add(P.rts, 2 * sizeof(T), n2);
+    return n;
+}
+int ckpt_arrays_any(ocn_model* M, CkptArray* out) { return M->prec == 32 ? ckpt_arrays<float>(M, out) : ckpt_arrays<double>(M, out); }
+template <class T>
+ocn_status count_nonfinite(ocn_model* M, unsigned long long* bad) {
+    ocn::DevP<T>& P = params<T>(M);
+    const unsigned long long n3 = (unsigned long long)P.sz * P.nz * 2, n2 = (unsigned long long)P.sz;
+    unsigned long long* d = P.timeline + 63;               // a spare device word of the model (the timeline uses 8 x 7)
+    CK(cudaMemsetAsync(d, 0, sizeof(*d), M->stream));
+    ocn::k_count_nonfinite<T><<<592, 256, 0, M->stream>>>((const T*)P.uv, n3, d);
+    ocn::k_count_nonfinite<T><<<592, 256, 0, M->stream>>>((const T*)P.ts, n3, d);
+    ocn::k_count_nonfinite<T><<<64, 256, 0, M->stream>>>((const T*)P.eta[0], n2, d);
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(bad, d, sizeof(*d), cudaMemcpyDeviceToHost, M->stream));
+    CK(cudaStreamSynchronize(M->stream));
+    return OCN_OK;
+}
+}  // namespace
+}  // extern "C++"
+
+ocn_status ocn_check_finite(ocn_model* M, unsigned long long* nonfinite) {
+    if (!M || !nonfinite) return fail(OCN_EINVAL, "null argument");
+    ON_DEVICE(M->d.device);
+    return M->prec == 32 ? count_nonfinite<float>(M, nonfinite) : count_nonfinite<double>(M, nonfinite);
+}
+
+ocn_status ocn_checkpoint_bytes(const ocn_model* M, unsigned long long* bytes) {
+    if (!M || !bytes) return fail(OCN_EINVAL, "null argument");
+    CkptArray arr[16];
+    const int n = ckpt_arrays_any(const_cast<ocn_model*>(M), arr);
+    unsigned long long b = sizeof(CkptHeader);
+    for (int a = 0; a < n; ++a) b += arr[a].bytes;
+    *bytes = b;
+    return OCN_OK;
+}
+
+ocn_status ocn_checkpoint_save(ocn_model* M, void* host) {
+    if (!M || !host) return fail(OCN_EINVAL, "null argument");
+    if (M->split_next != 0) return fail(OCN_ESTATE, "a split step is in progress");
+    ON_DEVICE(M->d.device);
+    CkptArray arr[16];
+    const int n = ckpt_arrays_any(M, arr);
+    CkptHeader h{};
+    std::memcpy(h.magic, "OCNCKPT1", 8);
+    h.nx = M->g->nx; h.ny = M->g->ny; h.nz = M->g->nz; h.precision = M->prec; h.sx = M->g->sx; h.sy = M->g->sy;
+    h.have_history = M->have_history ? 1 : 0;
+    char* dst = (char*)host + sizeof(h);
+    for (int a = 0; a < n; ++a) {
+        CK(cudaMemcpyAsync(dst, arr[a].base, arr[a].bytes, cudaMemcpyDeviceToHost, M->stream));
+        dst += arr[a].bytes;
+    }
+    h.payload = (unsigned long long)(dst - (char*)host) - sizeof(h);
+    CK(cudaStreamSynchronize(M->stream));
+    std::memcpy(host, &h, sizeof(h));
+    return OCN_OK;
+}
+
+ocn_status ocn_checkpoint_load(ocn_model* M, const void* host, unsigned long long bytes) {
+    if (!M || !host) return fail(OCN_EINVAL, "null argument");
+    CkptHeader h;
+    if (bytes < sizeof(h)) return fail(OCN_EINVAL, "not a checkpoint (too short)");
+    std::memcpy(&h, host, sizeof(h));
+    if (std::memcmp(h.magic, "OCNCKPT1", 8) != 0) return fail(OCN_EINVAL, "not a checkpoint (bad magic)");
+    if (h.nx != M->g->nx || h.ny != M->g->ny || h.nz != M->g->nz || h.precision != M->prec || h.sx != M->g->sx || h.sy != M->g->sy)
+        return fail(OCN_EINVAL, "the checkpoint was written by a model of another size or precision");
+    ON_DEVICE(M->d.device);
+    CkptArray arr[16];
+    const int n = ckpt_arrays_any(M, arr);
+    unsigned long long need = 0;
+    for (int a = 0; a < n; ++a) need += arr[a].bytes;
+    if (h.payload != need || bytes != need + sizeof(h)) return fail(OCN_EINVAL, "checkpoint size mismatch");
+    const char* src = (const char*)host + sizeof(h);
+    for (int a = 0; a < n; ++a) {
+        CK(cudaMemcpyAsync(arr[a].base, src, arr[a].bytes, cudaMemcpyHostToDevice, M->stream));
+        src += arr[a].bytes;
+    }
+    CK(cudaStreamSynchronize(M->stream));
+    M->have_history = h.have_history != 0;
+    M->split_next = 0;
+    return OCN_OK;
+}
+
 // ---- fused puts: the arrays of the new state as seen by a neighbouring band ----
 extern "C++" {
 namespace {

@@ -56,7 +56,8 @@ EXPORTS = ["ocn_grid_create", "ocn_grid_destroy", "ocn_model_create", "ocn_model
            "ocn_stage_name", "ocn_get_mixing", "ocn_get_fields_async", "ocn_wait", "ocn_tune", "ocn_selftest_division", "ocn_get_timeline",
            "ocn_get_mixing_noalloc", "ocn_noalloc_scratch_bytes",
            "ocn_step_parts", "ocn_step_part", "ocn_rows_bytes", "ocn_pack_rows", "ocn_unpack_rows", "ocn_band_overlap",
-           "ocn_peer_export", "ocn_peer_attach"]
+           "ocn_peer_export", "ocn_peer_attach",
+           "ocn_checkpoint_bytes", "ocn_checkpoint_save", "ocn_checkpoint_load", "ocn_check_finite"]
 ROWS_STATE, ROWS_FORCING, ROWS_BAROTROPIC_0, ROWS_BAROTROPIC_1, ROWS_STATE_2D = 0, 1, 2, 3, 4
 NSTAGES = 4
 
@@ -98,6 +99,10 @@ def lib():
         L.ocn_pack_rows.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp]
         L.ocn_unpack_rows.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp]
         L.ocn_band_overlap.argtypes = [C.c_int, C.c_int]
+        L.ocn_checkpoint_bytes.argtypes = [vp, C.POINTER(C.c_ulonglong)]
+        L.ocn_checkpoint_save.argtypes = [vp, vp]
+        L.ocn_checkpoint_load.argtypes = [vp, vp, C.c_ulonglong]
+        L.ocn_check_finite.argtypes = [vp, C.POINTER(C.c_ulonglong)]
         L.ocn_peer_export.argtypes = [vp, C.POINTER(ocn_peer)]
         L.ocn_peer_attach.argtypes = [vp, C.c_int, C.POINTER(ocn_peer), C.c_int, C.c_int, C.c_int, C.c_int]
         L.ocn_stage_name.restype = C.c_char_p
@@ -244,6 +249,25 @@ class Model:
 
     def pack_rows(self, group, j_begin, nrows, dst_device_ptr):
         _check(lib().ocn_pack_rows(self.h, int(group), int(j_begin), int(nrows), C.c_void_p(int(dst_device_ptr))))
+
+    # -- checkpoint / resume, finite check ----
+    def checkpoint(self):
+        """ocn_checkpoint_save into a new numpy uint8 array (everything a bit-exact resume needs)."""
+        n = C.c_ulonglong()
+        _check(lib().ocn_checkpoint_bytes(self.h, C.byref(n)))
+        buf = np.empty(n.value, np.uint8)
+        _check(lib().ocn_checkpoint_save(self.h, _ptr(buf)))
+        return buf
+
+    def restore(self, blob):
+        buf = np.ascontiguousarray(blob, dtype=np.uint8)
+        _check(lib().ocn_checkpoint_load(self.h, _ptr(buf), buf.size))
+
+    def nonfinite(self):
+        """ocn_check_finite: number of NaN / infinite words in u, v, T, S, eta."""
+        n = C.c_ulonglong()
+        _check(lib().ocn_check_finite(self.h, C.byref(n)))
+        return n.value
 
     def peer_export(self):
         """ocn_peer_export as bytes (plain data: addresses for this process, CUDA IPC handles for another)."""
