@@ -389,10 +389,11 @@ __global__ void __launch_bounds__(256) k_move_rows(const RowMoves R) {
 // RI = true (closure 1): the modified super-diagonals come from the arrays K5 wrote instead of the tables.
 // The launch covers rows Q.own_lo .. Q.own_hi - 1 (all rows of a model on its own).
 // PUT (latitude bands with fused puts): what is stored in rows a neighbouring band overlaps is stored into the
-// neighbour's arrays as well (Q.side; peer memory), so the new 3-D state needs no exchange afterwards.  The host launches this
-// variant on the mirrored rows only and the plain one on the rows in between; the band's own overlap rows are not processed at all.
+// neighbour's arrays as well (Q.side; peer memory), so the new 3-D state needs no exchange afterwards.  The host launches it on
+// the band's own rows; its overlap rows are not processed at all (the neighbours' puts fill them).  (Launched on the mirrored
+// rows alone, with the plain kernel on the rest, it was slower: a launch of 11 rows is one latency-bound column sweep, 118 us.)
 template <class T, bool RI, bool PUT = false>
-__global__ void __launch_bounds__(128, sizeof(T) == 8 ? 4 : (PUT ? 6 : 8)) k_backsub_correct(const DevP<T> P, const PeerPut<T> Q) {
+__global__ void __launch_bounds__(128, sizeof(T) == 8 ? 4 : 8) k_backsub_correct(const DevP<T> P, const PeerPut<T> Q) {
     typedef Ex<T> E;
     typedef typename Pair<T>::type T2;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;

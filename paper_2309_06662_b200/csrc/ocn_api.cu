@@ -477,13 +477,7 @@ ocn_status launch_step(ocn_model* M, bool euler, int part = -1) {
             }
         };
         if (!M->put) k3(0, g->ny, false);
-        else {                                     // own rows only: the mirrored rows at either end with puts, the rest plain
-            const int s_hi = std::max(Q.own_lo, std::min(Q.side[0].hi, Q.own_hi)), n_lo = std::min(Q.own_hi, std::max(Q.side[1].lo, s_hi));
-            k3(Q.own_lo, Q.side[0].hi > Q.side[0].lo ? s_hi : Q.own_lo, true);
-            const int mid_lo = Q.side[0].hi > Q.side[0].lo ? s_hi : Q.own_lo, mid_hi = Q.side[1].hi > Q.side[1].lo ? n_lo : Q.own_hi;
-            k3(mid_lo, mid_hi, false);
-            k3(mid_hi, Q.own_hi, true);
-        }
+        else k3(Q.own_lo, Q.own_hi, true);         // own rows only; the mirrored rows among them also go to the neighbours
     }
     MARK(2, 1);
 #undef MARK
