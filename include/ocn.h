@@ -110,6 +110,13 @@ typedef struct {
      * [m^4/s], >= 0, 0 = off.  G -= coefficient x L(L(.)) with the masked C-grid Laplacians of the second-order terms.
      * Costs two pre-pass launches per step and four more 3-D pair arrays; the default path is unchanged. */
     double nu4_h, kappa4_h;
+    /* Caller-supplied device memory ("optionally a caller-supplied torch workspace"): 256-byte aligned DEVICE
+     * memory of at least ocn_model_workspace_bytes bytes on `device`, e.g. a torch tensor; the model lives in it (no cudaMalloc
+     * at creation or while stepping) and the caller frees it after ocn_model_destroy.  NULL = the library allocates.  Not in it:
+     * the output array of ocn_get_mixing (allocated by the library on first use).  A model in a workspace cannot be reached
+     * from another process (ocn_peer_export leaves the IPC handles empty). */
+    void* workspace;
+    unsigned long long workspace_bytes;
 } ocn_model_desc;
 
 /* ocn_model_create — the model of PAPER.md:84 (§5.2: hydrostatic Boussinesq, IMEX quasi-AB2, backward-Euler vertical
@@ -120,6 +127,10 @@ typedef struct {
  * Errors: OCN_EINVAL, OCN_ENOMEM (device allocation), OCN_ECUDA (no device: there is no CPU fallback). */
 ocn_status ocn_model_create(const ocn_grid* grid, const ocn_model_desc* desc, ocn_model** out);
 ocn_status ocn_model_destroy(ocn_model* model);
+/* Bytes of device memory a model of this grid and these parameters takes (all its arrays, tables and staging regions): the size
+ * of ocn_model_desc.workspace, and what ocn_model_create will allocate itself otherwise (2 MiB page rounding of the arrays a
+ * neighbouring band may map aside).  Host-only dry run of the construction; validates the parameters like ocn_model_create. */
+ocn_status ocn_model_workspace_bytes(const ocn_grid* grid, const ocn_model_desc* desc, unsigned long long* bytes);
 
 /* Field set.  NULL member = skip.  on_device = 0: HOST pointers; 1: DEVICE pointers on the
  * model's device (contiguous, same layout). */

@@ -38,6 +38,9 @@ ocn_status fail(ocn_status s, const std::string& m) { g_err = m; return s; }
                         std::string(#call) + ": " + cudaGetErrorString(e_));                       \
     } while (0)
 
+// a device call of model construction: skipped in the dry run that sizes a workspace (M->measure)
+#define DEV(call) do { if (!M->measure) CK(call); } while (0)
+
 constexpr int LEAD = 32;   // elements before the first row so that i = 0 starts a 128-byte line
 
 // Every entry point that touches the device switches to the model's device and restores the caller's on return.
@@ -45,6 +48,7 @@ struct DeviceGuard {
     int prev = -1;
     cudaError_t err;
     explicit DeviceGuard(int dev) {
+        if (dev < 0) { err = cudaSuccess; return; }        // (host-only call: nothing to switch)
         if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
         err = cudaSetDevice(dev);
     }
@@ -67,6 +71,11 @@ struct ocn_model {
     bool have_history = false;
     std::vector<void*> allocs;
     unsigned long long bytes = 0;
+    // caller-supplied device memory (ocn_model_desc.workspace): allocations are carved from it in order; `measure` is the
+    // dry run of ocn_model_workspace_bytes (same code path, no device call, addresses from a made-up base)
+    char* ws = nullptr;
+    size_t ws_cap = 0, ws_used = 0;
+    bool measure = false;
     ocn::DevP<float> pf{};
     ocn::DevP<double> pd{};
     // host <-> device staging: copies run on a stream of their own beside the steps; one big region for
@@ -106,15 +115,30 @@ namespace {
 
 // ipc: an array a neighbouring band in another process maps through CUDA IPC (ocn_peer_export).  The driver carves small
 // allocations out of shared 2 MiB pages and an IPC handle names the whole page, so these get whole pages of their own.
+// bytes from the library (cudaMalloc) or, 256-byte aligned and in call order, from the caller's workspace
+inline ocn_status raw_alloc(ocn_model* M, size_t total, void** out, bool ipc) {
+    if (M->ws || M->measure) {
+        const size_t off = (M->ws_used + 255) / 256 * 256;
+        if (!M->measure && off + total > M->ws_cap)
+            return fail(OCN_ENOMEM, "workspace too small: ocn_model_workspace_bytes gives the size for this grid and these parameters");
+        *out = (M->measure ? (char*)(uintptr_t)0x100000000ull : M->ws) + off;
+        M->ws_used = off + total;
+    } else {
+        if (ipc) total = (total + ((size_t)2 << 20) - 1) / ((size_t)2 << 20) * ((size_t)2 << 20);
+        CK(cudaMalloc(out, total));
+        M->allocs.push_back(*out);
+    }
+    M->bytes += total;
+    return OCN_OK;
+}
+
 template <class T>
 ocn_status dev_alloc(ocn_model* M, size_t n, T** out, bool lead, bool ipc = false) {
     void* p = nullptr;
-    size_t total = (n + (lead ? 2 * LEAD : 0)) * sizeof(T);
-    if (ipc) total = (total + ((size_t)2 << 20) - 1) / ((size_t)2 << 20) * ((size_t)2 << 20);
-    CK(cudaMalloc(&p, total));
-    CK(cudaMemsetAsync(p, 0, total, M->stream));
-    M->allocs.push_back(p);
-    M->bytes += total;
+    const size_t total = (n + (lead ? 2 * LEAD : 0)) * sizeof(T);
+    const ocn_status sa = raw_alloc(M, total, &p, ipc);
+    if (sa != OCN_OK) return sa;
+    DEV(cudaMemsetAsync(p, 0, total, M->stream));
     *out = reinterpret_cast<T*>(p) + (lead ? LEAD : 0);
     return OCN_OK;
 }
@@ -125,8 +149,8 @@ ocn_status upload(ocn_model* M, const std::vector<double>& src, const T** out) {
     T* p = nullptr;
     ocn_status s = dev_alloc(M, tmp.size(), &p, false);
     if (s != OCN_OK) return s;
-    CK(cudaMemcpyAsync(p, tmp.data(), tmp.size() * sizeof(T), cudaMemcpyHostToDevice, M->stream));
-    CK(cudaStreamSynchronize(M->stream));
+    DEV(cudaMemcpyAsync(p, tmp.data(), tmp.size() * sizeof(T), cudaMemcpyHostToDevice, M->stream));
+    DEV(cudaStreamSynchronize(M->stream));
     *out = p;
     return OCN_OK;
 }
@@ -243,8 +267,8 @@ ocn_status build_model(ocn_model* M) {
         uint2* p8 = nullptr; uchar4* pz = nullptr;
         if ((s = dev_alloc(M, g->m8.size(), &p8, false)) != OCN_OK) return s;
         if ((s = dev_alloc(M, g->mz.size(), &pz, false)) != OCN_OK) return s;
-        CK(cudaMemcpyAsync(p8, g->m8.data(), g->m8.size() * 8, cudaMemcpyHostToDevice, M->stream));
-        CK(cudaMemcpyAsync(pz, g->mz.data(), g->mz.size() * 4, cudaMemcpyHostToDevice, M->stream));
+        DEV(cudaMemcpyAsync(p8, g->m8.data(), g->m8.size() * 8, cudaMemcpyHostToDevice, M->stream));
+        DEV(cudaMemcpyAsync(pz, g->mz.data(), g->mz.size() * 4, cudaMemcpyHostToDevice, M->stream));
         P.m8 = p8 + LEAD; P.mz = pz + LEAD;          // host planes were built with the same lead
     }
     // metrics (+ reciprocals), vertical grid
@@ -329,25 +353,27 @@ ocn_status build_model(ocn_model* M) {
                 hu[q] = (T)a; hv[q] = (T)b; rhu[q] = a > 0 ? (T)(1.0 / a) : T(0); rhv[q] = b > 0 ? (T)(1.0 / b) : T(0);
             }
         const size_t nb = hu.size() * sizeof(T);
-        CK(cudaMemcpyAsync(P.Hu - LEAD, hu.data(), nb, cudaMemcpyHostToDevice, M->stream));
-        CK(cudaMemcpyAsync(P.Hv - LEAD, hv.data(), nb, cudaMemcpyHostToDevice, M->stream));
-        CK(cudaMemcpyAsync(P.rHu - LEAD, rhu.data(), nb, cudaMemcpyHostToDevice, M->stream));
-        CK(cudaMemcpyAsync(P.rHv - LEAD, rhv.data(), nb, cudaMemcpyHostToDevice, M->stream));
-        CK(cudaStreamSynchronize(M->stream));
+        DEV(cudaMemcpyAsync(P.Hu - LEAD, hu.data(), nb, cudaMemcpyHostToDevice, M->stream));
+        DEV(cudaMemcpyAsync(P.Hv - LEAD, hv.data(), nb, cudaMemcpyHostToDevice, M->stream));
+        DEV(cudaMemcpyAsync(P.rHu - LEAD, rhu.data(), nb, cudaMemcpyHostToDevice, M->stream));
+        DEV(cudaMemcpyAsync(P.rHv - LEAD, rhv.data(), nb, cudaMemcpyHostToDevice, M->stream));
+        DEV(cudaStreamSynchronize(M->stream));
     }
     {
         auto mk = [&](ocn_model::Stage& st, size_t bytes) -> ocn_status {
-            CK(cudaMalloc(&st.buf, bytes));
-            st.bytes = bytes; M->bytes += bytes;
-            CK(cudaEventCreateWithFlags(&st.filled, cudaEventDisableTiming));
-            CK(cudaEventCreateWithFlags(&st.freed, cudaEventDisableTiming));
+            const ocn_status sa = raw_alloc(M, bytes, &st.buf, false);
+            if (sa != OCN_OK) return sa;
+            st.bytes = bytes;
+            DEV(cudaEventCreateWithFlags(&st.filled, cudaEventDisableTiming));
+            DEV(cudaEventCreateWithFlags(&st.freed, cudaEventDisableTiming));
             return OCN_OK;
         };
         if ((s = mk(M->big, (size_t)(nz + 1) * g->ny * g->nx * sizeof(double))) != OCN_OK) return s;
         for (auto& st : M->small_) if ((s = mk(st, (size_t)g->ny * g->nx * sizeof(double))) != OCN_OK) return s;
-        CK(cudaStreamCreateWithFlags(&M->copy_stream, cudaStreamNonBlocking));
-        for (auto& e : M->ticket_ev) CK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        DEV(cudaStreamCreateWithFlags(&M->copy_stream, cudaStreamNonBlocking));
+        for (auto& e : M->ticket_ev) DEV(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     }
+    if (M->measure) return OCN_OK;                 // everything below allocates nothing
     M->launches_per_step = (M->d.substeps + bt_substeps_per_launch<T>() - 1) / bt_substeps_per_launch<T>() + 3 + (P.bih ? 2 : 0);
     // TMA descriptors: box origin (i0 - 4, j0 - 3), so the map starts 4 elements before (row -3, i = 0)
     {
@@ -653,7 +679,10 @@ ocn_status get_mixing_t(ocn_model* M, double* nu, double* kappa) {
     const int nz = M->g->nz;
     const dim3 bc(32, 4);
     if (!P.nk) {                                   // the output array of the diagnostic (the step itself keeps (nu, kappa) on chip)
+        char* const ws = M->ws;                    // allocated by the library on first use, also for a model in a workspace
+        M->ws = nullptr;
         const ocn_status sa = dev_alloc(M, (size_t)P.sz * nz, &P.nk, true);
+        M->ws = ws;
         if (sa != OCN_OK) return sa;
     }
     ocn::k_ri_mixing<T><<<grid2(M->g, bc), bc, 0, M->stream>>>(P);
@@ -762,8 +791,10 @@ ocn_status ocn_get_masks(const ocn_grid* g, unsigned char* wet, unsigned char* o
     return OCN_OK;
 }
 
-ocn_status ocn_model_create(const ocn_grid* g, const ocn_model_desc* d, ocn_model** out) {
-    if (!g || !d || !out) return fail(OCN_EINVAL, "null argument");
+// measure_bytes != nullptr: the dry run of ocn_model_workspace_bytes (no device call, no model returned)
+static ocn_status create_impl(const ocn_grid* g, const ocn_model_desc* d, ocn_model** out, unsigned long long* measure_bytes) {
+    const bool measure = measure_bytes != nullptr;
+    if (!g || !d || (!out && !measure)) return fail(OCN_EINVAL, "null argument");
     if (d->precision != 32 && d->precision != 64) return fail(OCN_EINVAL, "precision must be 32 or 64");
     if (!(d->dt > 0) || d->substeps < 1) return fail(OCN_EINVAL, "dt must be > 0 and substeps >= 1");
     if (!(d->rho0 > 0)) return fail(OCN_EINVAL, "rho0 must be > 0");
@@ -783,14 +814,22 @@ ocn_status ocn_model_create(const ocn_grid* g, const ocn_model_desc* d, ocn_mode
     if (d->advection != 0 && d->advection != 1) return fail(OCN_EINVAL, "advection must be 0 (WENO-JS) or 1 (WENO-Z)");
     if (d->closure == 1 && !(d->ri_n2c > 0 && d->ri_s2min > 0 && d->ri_c >= 0 && d->ri_nu0 >= 0 && d->ri_kconv >= 0))
         return fail(OCN_EINVAL, "Ri closure: ri_n2c, ri_s2min must be > 0 and ri_c, ri_nu0, ri_kconv >= 0");
+    if (!measure && d->workspace && ((uintptr_t)d->workspace & 255u))
+        return fail(OCN_EINVAL, "workspace must be 256-byte aligned device memory");
     int ndev = 0;
-    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
-        return fail(OCN_ECUDA, "no CUDA device: libocn has no CPU fallback");
-    if (d->device < 0 || d->device >= ndev) return fail(OCN_EINVAL, "bad device ordinal");
-    ON_DEVICE(d->device);
+    if (!measure) {
+        if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+            return fail(OCN_ECUDA, "no CUDA device: libocn has no CPU fallback");
+        if (d->device < 0 || d->device >= ndev) return fail(OCN_EINVAL, "bad device ordinal");
+    }
+    DeviceGuard guard_(measure ? -1 : d->device);
+    if (!measure) CK(guard_.err);
     ocn_model* M = new (std::nothrow) ocn_model();
     if (!M) return fail(OCN_ENOMEM, "host allocation failed");
     M->g = g; M->d = *d; M->prec = d->precision;
+    M->measure = measure;
+    if (!measure && d->workspace) { M->ws = static_cast<char*>(d->workspace); M->ws_cap = (size_t)d->workspace_bytes; }
+    M->d.workspace = nullptr;
     // filter weights: power law p = 2, q = 4 unless given; dtau centres the average on t^{n+1}
     const int Ms = d->substeps;
     M->a_w.resize(Ms);
@@ -821,6 +860,12 @@ ocn_status ocn_model_create(const ocn_grid* g, const ocn_model_desc* d, ocn_mode
         }
     }
     M->d.filter_weights_uv = nullptr;
+    if (measure) {
+        const ocn_status s = d->precision == 32 ? build_model<float>(M) : build_model<double>(M);
+        *measure_bytes = (unsigned long long)((M->ws_used + 255) / 256 * 256);
+        delete M;
+        return s;
+    }
     if (d->stream) M->stream = static_cast<cudaStream_t>(d->stream);
     else {
         cudaError_t e = cudaStreamCreateWithFlags(&M->stream, cudaStreamNonBlocking);
@@ -833,6 +878,16 @@ ocn_status ocn_model_create(const ocn_grid* g, const ocn_model_desc* d, ocn_mode
     return OCN_OK;
 }
 
+ocn_status ocn_model_create(const ocn_grid* g, const ocn_model_desc* d, ocn_model** out) {
+    if (!out) return fail(OCN_EINVAL, "null argument");
+    return create_impl(g, d, out, nullptr);
+}
+
+ocn_status ocn_model_workspace_bytes(const ocn_grid* g, const ocn_model_desc* d, unsigned long long* bytes) {
+    if (!bytes) return fail(OCN_EINVAL, "null argument");
+    return create_impl(g, d, nullptr, bytes);
+}
+
 ocn_status ocn_model_destroy(ocn_model* M) {
     if (!M) return OCN_OK;
     DeviceGuard guard_(M->d.device);
@@ -843,8 +898,7 @@ ocn_status ocn_model_destroy(ocn_model* M) {
     if (M->copy_stream) { cudaStreamSynchronize(M->copy_stream); cudaStreamDestroy(M->copy_stream); }
     for (ocn_model::Stage* st : {&M->big, &M->small_[0], &M->small_[1], &M->small_[2], &M->small_[3], &M->small_[4], &M->small_[5],
                                  &M->small_[6], &M->small_[7]}) {
-        if (st->buf) cudaFree(st->buf);
-        if (st->filled) cudaEventDestroy(st->filled);
+        if (st->filled) cudaEventDestroy(st->filled);      // (the buffer is in `allocs` or in the caller's workspace)
         if (st->freed) cudaEventDestroy(st->freed);
     }
     for (cudaEvent_t e : M->ticket_ev) if (e) cudaEventDestroy(e);
@@ -1087,6 +1141,7 @@ ocn_status ocn_peer_export(ocn_model* M, ocn_peer* out) {
     if (M->prec == 32) peer_arrays<float>(M, out->ptr); else peer_arrays<double>(M, out->ptr);
     static_assert(sizeof(cudaIpcMemHandle_t) == 64, "ipc handle size");
     for (int a = 0; a < OCN_PEER_ARRAYS; ++a) {
+        if (M->ws) continue;                       // in the caller's workspace: reachable in this process only (no IPC handle)
         void* base = nullptr;                      // the allocation that holds the array (the largest base below it)
         for (void* b : M->allocs) if (b <= out->ptr[a] && (!base || b > base)) base = b;
         if (!base) return fail(OCN_ESTATE, "array without an allocation");

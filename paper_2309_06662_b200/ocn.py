@@ -37,7 +37,8 @@ class ocn_model_desc(C.Structure):
                 ("ri_n2c", C.c_double), ("ri_s2min", C.c_double), ("gamma_T", C.c_double), ("gamma_S", C.c_double),
                 ("drag_r", C.c_double), ("drag_cd", C.c_double),
                 ("eos", C.c_int), ("eos_alpha2", C.c_double), ("eos_gamma", C.c_double), ("advection", C.c_int),
-                ("filter_weights_uv", C.POINTER(C.c_double)), ("nu4_h", C.c_double), ("kappa4_h", C.c_double)]
+                ("filter_weights_uv", C.POINTER(C.c_double)), ("nu4_h", C.c_double), ("kappa4_h", C.c_double),
+                ("workspace", C.c_void_p), ("workspace_bytes", C.c_ulonglong)]
 
 
 class ocn_fields(C.Structure):
@@ -57,7 +58,7 @@ EXPORTS = ["ocn_grid_create", "ocn_grid_destroy", "ocn_model_create", "ocn_model
            "ocn_get_mixing_noalloc", "ocn_noalloc_scratch_bytes",
            "ocn_step_parts", "ocn_step_part", "ocn_rows_bytes", "ocn_pack_rows", "ocn_unpack_rows", "ocn_band_overlap",
            "ocn_peer_export", "ocn_peer_attach",
-           "ocn_checkpoint_bytes", "ocn_checkpoint_save", "ocn_checkpoint_load", "ocn_check_finite"]
+           "ocn_checkpoint_bytes", "ocn_checkpoint_save", "ocn_checkpoint_load", "ocn_check_finite", "ocn_model_workspace_bytes"]
 ROWS_STATE, ROWS_FORCING, ROWS_BAROTROPIC_0, ROWS_BAROTROPIC_1, ROWS_STATE_2D = 0, 1, 2, 3, 4
 NSTAGES = 4
 
@@ -76,6 +77,7 @@ def lib():
         L.ocn_grid_destroy.argtypes = [vp]
         L.ocn_model_create.argtypes = [vp, C.POINTER(ocn_model_desc), C.POINTER(vp)]
         L.ocn_model_destroy.argtypes = [vp]
+        L.ocn_model_workspace_bytes.argtypes = [vp, C.POINTER(ocn_model_desc), C.POINTER(C.c_ulonglong)]
         L.ocn_set_fields.argtypes = [vp, C.POINTER(ocn_fields)]
         L.ocn_time_step.argtypes = [vp, C.c_int]
         L.ocn_get_fields.argtypes = [vp, C.POINTER(ocn_fields)]
@@ -168,7 +170,10 @@ class Grid:
 class Model:
     """ocn_model_create + ocn_set_fields on a workload dict (paper_2309_06662_b200.workloads)."""
 
-    def __init__(self, workload, device=0, stream=None, filter_weights=None, set_fields=True, filter_weights_uv=None):
+    def __init__(self, workload, device=0, stream=None, filter_weights=None, set_fields=True, filter_weights_uv=None,
+                 workspace=None):
+        """workspace: None (the library allocates), or a callable nbytes -> (handle, device pointer) that provides the model's
+        device memory (e.g. a torch uint8 tensor and its data_ptr()); the handle is kept alive with the model."""
         self.grid = Grid(workload["grid"], workload["z_faces"], workload["depth"])
         p = dict(workload["params"])
         self.precision = int(p["precision"])
@@ -179,10 +184,22 @@ class Model:
         fwuv = self._fwuv.ctypes.data_as(C.POINTER(C.c_double)) if self._fwuv is not None else None
         self.desc = ocn_model_desc(filter_weights=fw, filter_weights_uv=fwuv, device=int(device), stream=stream, **p)
         self.nx, self.ny, self.nz = self.grid.nx, self.grid.ny, self.grid.nz
+        self._workspace = None
+        if workspace is not None:
+            need = self.workspace_bytes()
+            got = workspace(need)                          # (handle, pointer) or (handle, pointer, bytes actually provided)
+            self._workspace, ptr = got[0], got[1]
+            self.desc.workspace, self.desc.workspace_bytes = int(ptr), int(got[2]) if len(got) > 2 else need
         self.h = C.c_void_p()
         _check(lib().ocn_model_create(self.grid.h, C.byref(self.desc), C.byref(self.h)))
         if set_fields and "fields" in workload:
             self.set_fields(**workload["fields"])
+
+    def workspace_bytes(self):
+        """ocn_model_workspace_bytes for this grid and these parameters (host-only)."""
+        n = C.c_ulonglong()
+        _check(lib().ocn_model_workspace_bytes(self.grid.h, C.byref(self.desc), C.byref(n)))
+        return n.value
 
     # -- host numpy arrays ---------------------------------------------------------------
     def set_fields(self, **kw):

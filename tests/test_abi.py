@@ -68,3 +68,32 @@ def test_masks_bit_exact_against_oracle(wl):
     want = oracle.RefGrid(wl["grid"], wl["z_faces"], wl["depth"]).masks()
     for n in want:
         assert np.array_equal(got[n], want[n]), n
+
+
+def test_workspace_bytes_is_a_host_only_dry_run():
+    """ocn_model_workspace_bytes sizes a model without touching a device (this test runs on the CPU box)."""
+    import ctypes as C
+    from paper_2309_06662_b200 import workloads as W
+    wl = W.make(3, nx=96, ny=48, nz=12)
+    g = ocn.Grid(wl["grid"], wl["z_faces"], wl["depth"])
+
+    def size(**over):
+        p = dict(wl["params"]); p.update(over)
+        d = ocn.ocn_model_desc(device=0, **p)
+        n = C.c_ulonglong()
+        rc = ocn.lib().ocn_model_workspace_bytes(g.h, C.byref(d), C.byref(n))
+        return rc, n.value
+
+    rc, base = size()
+    assert rc == 0
+    sx, sy, nz = 128, 48 + 6, 12
+    assert base > 7 * 8 * sx * sy * nz                     # at least the seven 3-D pair / fp64 arrays
+    rc, ri = size(closure=1, ri_nu0=5e-3, ri_c=5.0, ri_kconv=0.1, ri_n2c=1e-7, ri_s2min=1e-10)
+    assert rc == 0 and ri >= base + (8 + 4) * sx * sy * nz  # + the two super-diagonal arrays
+    rc, bih = size(nu4_h=1e9)
+    assert rc == 0 and bih >= base + 4 * 8 * sx * sy * nz
+    rc, f64 = size(precision=64)
+    assert rc == 0 and f64 > 1.5 * base
+    rc, _ = size(dt=-1.0)
+    assert rc != 0 and b"dt must be > 0" in ocn.lib().ocn_last_error()
+    g.close()
