@@ -199,7 +199,9 @@ ocn_status ocn_profile_enable(ocn_model* model, int on);
 ocn_status ocn_profile_read(ocn_model* model, double* ms, long long* launches, int reset);
 const char* ocn_stage_name(int stage);
 
-/* Performance knobs that do not change results (bit for bit).  "k1_geo_threshold": number of wet cells of a 32 x 8 tile-level
+/* Knobs that do not change results (bit for bit).  "nvtx" (0 / 1): NVTX host ranges around ocn_time_step and the parts of
+ * ocn_step_part for timeline tools (PAPER.md:116 profiles with Nsight Systems + NVTX ranges; header-only NVTX 3, a no-op
+ * without a tool attached).  "k1_geo_threshold": number of wet cells of a 32 x 8 tile-level
  * from which on the tendency kernel marches the tile with geometric (thread = cell) instead of compacted ownership
  * (default K1_GEO_THR of kernels_tile.cuh; 0 = always geometric, > 256 = never).  OCN_EINVAL for an unknown key. */
 ocn_status ocn_tune(ocn_model* model, const char* key, double value);

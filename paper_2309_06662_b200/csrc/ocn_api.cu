@@ -2,6 +2,7 @@
 // hot path runs in the kernels of kernels_tend.cuh / kernels_column.cuh.
 #include <cuda.h>
 #include <cuda_runtime.h>
+#include <nvtx3/nvToolsExt.h>
 
 #include <algorithm>
 #include <cmath>
@@ -98,6 +99,7 @@ struct ocn_model {
     // split step (ocn_step_part): the next part expected, and whether the step in progress is the Euler start
     int split_next = 0;
     bool split_euler = false;
+    bool nvtx = false;                  // ocn_tune("nvtx", 1): host ranges around steps, parts and profiled stages
     // fused puts into neighbouring bands (ocn_peer_attach): what the last part of a step also stores into peer memory
     bool put = false;
     ocn::PeerPut<float> qf{};
@@ -919,7 +921,10 @@ ocn_status ocn_time_step(ocn_model* M, int n) {
     if (!M || n < 0) return fail(OCN_EINVAL, "bad argument");
     if (M->split_next != 0) return fail(OCN_ESTATE, "a split step is in progress (ocn_step_part): finish its parts first");
     ON_DEVICE(M->d.device);
-    return M->prec == 32 ? run_steps<float>(M, n) : run_steps<double>(M, n);
+    if (M->nvtx) nvtxRangePushA("ocn_time_step");
+    const ocn_status s = M->prec == 32 ? run_steps<float>(M, n) : run_steps<double>(M, n);
+    if (M->nvtx) nvtxRangePop();
+    return s;
 }
 
 // ---- the step in parts, and rows of the arrays a neighbouring band needs (latitude bands) ----
@@ -1002,7 +1007,9 @@ ocn_status ocn_step_part(ocn_model* M, int part) {
     if (part != M->split_next) return fail(OCN_ESTATE, "parts of a step run in order, 0 .. ocn_step_parts - 1 (next expected: " + std::to_string(M->split_next) + ")");
     ON_DEVICE(M->d.device);
     if (part == 0) M->split_euler = !M->have_history;
+    if (M->nvtx) nvtxRangePushA(part == 0 ? "ocn_step_part tendency" : part == np - 1 ? "ocn_step_part backsub_correct" : "ocn_step_part barotropic");
     const ocn_status s = M->prec == 32 ? launch_step<float>(M, M->split_euler, part) : launch_step<double>(M, M->split_euler, part);
+    if (M->nvtx) nvtxRangePop();
     if (s != OCN_OK) return s;
     if (part == np - 1) { M->have_history = true; M->split_next = 0; }
     else M->split_next = part + 1;
@@ -1276,6 +1283,7 @@ ocn_status ocn_profile_read(ocn_model* M, double* ms, long long* launches, int r
 ocn_status ocn_tune(ocn_model* M, const char* key, double value) {
     if (!M || !key) return fail(OCN_EINVAL, "null argument");
     ON_DEVICE(M->d.device);
+    if (std::string(key) == "nvtx") { M->nvtx = value != 0; return OCN_OK; }
     if (std::string(key) == "k1_geo_threshold") {
         if (!(value >= 0 && value <= 1e6)) return fail(OCN_EINVAL, "k1_geo_threshold out of range");
         M->pf.geo_thr = (int)value; M->pd.geo_thr = (int)value;

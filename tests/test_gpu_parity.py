@@ -450,3 +450,19 @@ def test_aquaplanet_reduced_fp32_and_fp64():
     for n in FIELDS:
         assert np.array_equal(a[n], b[n]), n
     gpu.close()
+
+
+def test_nvtx_ranges_are_a_no_op_for_the_results():
+    wl = W.config2(nx=96, ny=48, nz=12, steps=3, precision=32)
+    a, b = ocn.Model(wl), ocn.Model(wl)
+    b.tune("nvtx", 1)
+    a.time_step(3)
+    b.time_step(1)
+    for p in range(b.step_parts()):
+        b.step_part(p)
+    b.tune("nvtx", 0)
+    b.time_step(1)
+    fa, fb = a.get_fields(), b.get_fields()
+    for k in fa:
+        assert np.array_equal(fa[k], fb[k]), k
+    a.close(); b.close()
