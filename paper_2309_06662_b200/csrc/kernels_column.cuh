@@ -433,10 +433,30 @@ __global__ void __launch_bounds__(128, sizeof(T) == 8 ? 4 : 8) k_backsub_correct
             if (to1) store_halo(q1 + k * Q.side[1].sz, sx, P.nx, Q.side[1].ny, P.px, 0, j + Q.side[1].dj, i, val);
         }
     };
-    constexpr int NB = 3;                                  // levels whose loads are in flight together (measured best with 8 CTAs / SM)
+#ifndef K3_NB
+#define K3_NB 3
+#endif
+#ifndef K3_PF_DIST
+#define K3_PF_DIST (RI ? 0 : (sizeof(T) == 8 ? 2 : 1))
+#endif
+    constexpr int NB = K3_NB;                              // levels whose loads are in flight together (measured best with 8 CTAs / SM)
     for (int k0 = nz - 1; k0 >= kg; k0 -= NB) {
         T2 d_ts[NB], d_uv[NB], c_uv[NB];
         T c_t[NB];
+        // The lines of a later group into L2 (no registers held): the loads below then find them there.  K3 1.94 -> 1.75 ms on
+        // config 4 one group ahead, 0.82 -> 0.73 ms in fp64 (config 2) two groups ahead; with the closure's two extra arrays in
+        // flight it gains nothing (2.03 against 2.04 ms) and two groups ahead cost 4 %: off there (profiles/r2_ncu_summary.md §10).
+        constexpr int PF = K3_PF_DIST;
+        if (PF > 0) {
+#pragma unroll
+            for (int q = 0; q < NB; ++q) {
+                const int k = k0 - PF * NB - q;
+                if (k >= kb) {
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(P.dts + k * sz + c));
+                    if (k >= kuv) asm volatile("prefetch.global.L2 [%0];" ::"l"(P.duv + k * sz + c));
+                }
+            }
+        }
 #pragma unroll
         for (int q = 0; q < NB; ++q) {
             const int k = k0 - q;
