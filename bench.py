@@ -490,7 +490,8 @@ def run_ours(args):
                 "config": {"workload": wname, "cells": cells, "wet_cells": nwet,
                            "l2": "working set %.1f GB >> 126 MB L2 (no flush needed)" % (info["device_bytes"] / 1e9)
                                  if info["device_bytes"] > 1e9 else "working set fits L2 (launch/latency bound; roofline n/a)",
-                           "parallelism": "replicas x%d" % world},
+                           "parallelism": "replicas x%d (independent ensemble members, no exchange; the sharded form of the "
+                                          "path, latitude bands with one exchange step, runs with --bands N: DESIGN.md section 9)" % world},
                 "sypd_equivalent": sypd(prm["dt"], sec_per_step),
                 "wet_cell_updates_per_s": world * nwet * K / (ms_total * 1e-3),
                 "stages": stage_out, "roofline": roof, "roofline_step": roof_step, "roofline_alu": roof_alu, "issue_utilisation": issue_util, "e2e": e2e,
