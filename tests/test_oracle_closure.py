@@ -89,6 +89,27 @@ def test_mixing_v_shear_counts_like_u_shear():
     assert np.allclose(ma["nu"], mb["nu"], rtol=1e-12) and np.allclose(ma["kappa"], mb["kappa"], rtol=1e-12)
 
 
+def test_mixing_takes_the_shear_from_the_four_faces_of_the_column():
+    """Horizontally varying u, v (random, periodic box): S2 at tracer column (j, i) averages the squared shear of ITS west and
+    east u faces (i, i + 1) and ITS south and north v faces (j, j + 1) — a face of a neighbouring column must not enter.
+    Expected values from array shifts in numpy."""
+    rng = np.random.default_rng(31)
+    wl = _sheared_box(2e-3, 0.0)
+    f = wl["fields"]
+    f["u"] = 0.05 * rng.standard_normal(f["u"].shape)
+    f["v"] = 0.05 * rng.standard_normal(f["v"].shape)
+    mix = oracle.RefModel(wl).mixing()
+    zc = 0.5 * (wl["z_faces"][:-1] + wl["z_faces"][1:])
+    dzc = np.diff(zc)[:, None, None]
+    du, dv = np.diff(f["u"], axis=0), np.diff(f["v"], axis=0)          # level k minus level k - 1, k = 1 .. nz - 1
+    S2 = (0.5 * (du ** 2 + np.roll(du, -1, axis=2) ** 2) + 0.5 * (dv ** 2 + np.roll(dv, -1, axis=1) ** 2)) / dzc ** 2
+    N2 = G * ALPHA * np.diff(f["T"], axis=0) / dzc
+    ff = 1.0 / (1.0 + RI["ri_c"] * np.maximum(N2, 0.0) / (S2 + RI["ri_s2min"]))
+    assert np.allclose(mix["nu"][1:], 1e-4 + RI["ri_nu0"] * ff ** 2, rtol=1e-12, atol=0)
+    assert np.allclose(mix["kappa"][1:], 1e-5 + RI["ri_nu0"] * ff ** 3, rtol=1e-12, atol=0)
+    assert ff.min() < 0.5 and ff.max() > 0.9                             # the case spans weak and strong mixing
+
+
 def test_mixing_neutral_and_convective_limits():
     # neutral column: Ri = 0 whatever the shear -> nu_z + nu0, kappa_z + nu0
     mix = oracle.RefModel(_sheared_box(0.0, 4e-3)).mixing()

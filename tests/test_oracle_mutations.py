@@ -117,11 +117,79 @@ MUTANTS = [
 ]
 
 
-def _run_pins(src_path):
+# the same check for the options beyond the north_star path: vertical mixing closure, nonlinear equation of
+# state (§3.16), bottom drag (§3.14), surface tracer forcing (§3.13), the implicit vertical solve (§3.8 step 4)
+PINS_OPTIONS = ["tests/test_oracle_closure.py", "tests/test_oracle_forcing.py", "tests/test_oracle_variants.py",
+                "tests/test_oracle_handcalc.py", "tests/test_oracle_physics.py"]
+MUTANTS_OPTIONS = [
+    ("C1 closure: nu with f^3 instead of f^2",
+     "M.nuc(k, j, i) = d.nu_z + d.ri_nu0 * f * f + conv;",
+     "M.nuc(k, j, i) = d.nu_z + d.ri_nu0 * f * f * f + conv;"),
+    ("C2 closure: Ri from N2 without the clip at 0",
+     "const double Ri = std::max(N2, 0.0) / (S2 + d.ri_s2min);",
+     "const double Ri = N2 / (S2 + d.ri_s2min);"),
+    ("C3 closure: convective ramp on +N2",
+     "const double conv = d.ri_kconv * std::min(1.0, std::max(-N2, 0.0) / d.ri_n2c);",
+     "const double conv = d.ri_kconv * std::min(1.0, std::max(N2, 0.0) / d.ri_n2c);"),
+    ("C4 closure: kappa without the convective term",
+     "M.kapc(k, j, i) = d.kappa_z + d.ri_nu0 * f * f * f + conv;",
+     "M.kapc(k, j, i) = d.kappa_z + d.ri_nu0 * f * f * f;"),
+    ("C5 closure: shear of the east face taken at i instead of i + 1",
+     "due = M.u(k, j, i + 1) - M.u(k - 1, j, i + 1);",
+     "due = M.u(k, j, i) - M.u(k - 1, j, i + 1);"),
+    ("C6 closure: S2 divided by dzc once",
+     "+ 0.5 * (dvs * dvs + dvn * dvn)) / (g.dzc[k] * g.dzc[k]);",
+     "+ 0.5 * (dvs * dvs + dvn * dvn)) / (g.dzc[k]);"),
+    ("E1 equation of state: thermobaric factor 1 + gamma z",
+     "(1.0 - M.d.eos_gamma * M.g->zc[k]) * dT",
+     "(1.0 + M.d.eos_gamma * M.g->zc[k]) * dT"),
+    ("E2 equation of state: cabbeling without the 1/2",
+     "+ 0.5 * M.d.eos_alpha2 * dT * dT",
+     "+ M.d.eos_alpha2 * dT * dT"),
+    ("D1 bottom drag on u: speed without the transverse velocity",
+     "std::sqrt(u(k, j, i) * u(k, j, i) + vhat * vhat))",
+     "std::sqrt(u(k, j, i) * u(k, j, i)))"),
+    ("D2 bottom drag on u: every level instead of the lowest open one",
+     "const bool bot = m && (k == 0 || !g.mu(k - 1, j, i));",
+     "const bool bot = m;"),
+    ("F1 surface forcing: restoring with the wrong sign",
+     "(surf(0, j, i) + gamma * (target(0, j, i) - c(k, j, i))) / g.dz[k];",
+     "(surf(0, j, i) - gamma * (target(0, j, i) - c(k, j, i))) / g.dz[k];"),
+    ("T1 implicit solve: upper coefficient with dzc[k] instead of dzc[k + 1]",
+     "const double sp = (k + 1 <= nz - 1 && open[k + 1]) ? dtk[k + 1] / (dz[k] * dzc[k + 1]) : 0.0;",
+     "const double sp = (k + 1 <= nz - 1 && open[k + 1]) ? dtk[k + 1] / (dz[k] * dzc[k]) : 0.0;"),
+    ("T2 implicit solve: back-substitution with the wrong sign",
+     "phi[k] = dp[k] - cp[k] * phi[k + 1];",
+     "phi[k] = dp[k] + cp[k] * phi[k + 1];"),
+]
+
+
+def _run_pins(src_path, pins=None):
     env = dict(os.environ, OCN_REF_MUTANT_SRC=src_path, OMP_NUM_THREADS="2")
-    r = subprocess.run([sys.executable, "-m", "pytest", "-x", "-q", "-p", "no:cacheprovider"] + PINS, cwd=ROOT, env=env,
+    r = subprocess.run([sys.executable, "-m", "pytest", "-x", "-q", "-p", "no:cacheprovider"] + (pins or PINS), cwd=ROOT, env=env,
                        stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
     return r.returncode, r.stdout[-3000:]
+
+
+def test_every_mutant_of_the_options_is_caught():
+    text = open(SRC).read()
+    tmp = tempfile.mkdtemp(prefix="ocn_mut_")
+    try:
+        jobs = []
+        for n, (name, old, new) in enumerate(MUTANTS_OPTIONS):
+            assert text.count(old) == 1, "mutation target not found exactly once (oracle source changed?): " + name
+            path = os.path.join(tmp, "option_%02d.cpp" % n)
+            with open(path, "w") as f:
+                f.write(text.replace(old, new))
+            jobs.append((name, path))
+        with ThreadPoolExecutor(max_workers=max(2, (os.cpu_count() or 4) // 2)) as ex:
+            res = list(ex.map(lambda j: _run_pins(j[1], PINS_OPTIONS), jobs))
+        survivors = [name for (name, _), (rc, _) in zip(jobs, res) if rc == 0]
+        assert not survivors, "mutants that survive every pin: %s" % survivors
+        for (name, _), (rc, out) in zip(jobs, res):
+            assert rc == 1 and "AssertionError" in out, (name, rc, out)
+    finally:
+        shutil.rmtree(tmp, ignore_errors=True)
 
 
 def test_every_mutant_of_the_latlon_metrics_and_masks_is_caught():
@@ -153,10 +221,10 @@ def test_every_mutant_of_the_latlon_metrics_and_masks_is_caught():
 if __name__ == "__main__":          # python tests/test_oracle_mutations.py: prints which pin catches which mutant
     text = open(SRC).read()
     tmp = tempfile.mkdtemp(prefix="ocn_mut_")
-    for n, (name, old, new) in enumerate(MUTANTS):
+    for n, (name, old, new) in enumerate(MUTANTS + MUTANTS_OPTIONS):
         path = os.path.join(tmp, "m%02d.cpp" % n)
         open(path, "w").write(text.replace(old, new))
-        rc, out = _run_pins(path)
+        rc, out = _run_pins(path, PINS if n < len(MUTANTS) else PINS_OPTIONS)
         first = [ln for ln in out.splitlines() if ln.startswith("FAILED")]
         print("%-70s %s" % (name, first[0] if first else ("SURVIVES" if rc == 0 else "rc=%d" % rc)))
     shutil.rmtree(tmp, ignore_errors=True)
