@@ -110,6 +110,43 @@ def test_mixing_takes_the_shear_from_the_four_faces_of_the_column():
     assert ff.min() < 0.5 and ff.max() > 0.9                             # the case spans weak and strong mixing
 
 
+def test_viscosity_at_a_velocity_face_is_the_mean_of_the_two_columns_that_share_it():
+    """Stronger stratification in ONE tracer column (j0, i0) changes nu there and the pressure there, nothing else of state n.
+    After one step the vertical structure of u (u minus its depth mean: the barotropic correction is depth independent)
+    may therefore change only at the two u faces of that column, (j0, i0) and (j0, i0 + 1), and that of v only at
+    (j0, i0) and (j0 + 1, i0) — the faces whose nu is the mean over the column and its west / south neighbour
+    (DESIGN.md §3.12).  An average taken over the wrong pair of columns moves other faces."""
+    gamma = 2e-3
+    wl = _sheared_box(gamma, 2e-3)
+    zc = 0.5 * (wl["z_faces"][:-1] + wl["z_faces"][1:])
+    dz = np.diff(wl["z_faces"])[:, None, None]
+    wl["fields"]["v"] = 1e-3 * zc[:, None, None] + np.zeros_like(wl["fields"]["v"])
+    j0, i0 = 2, 3
+    pert = clone(wl)
+    pert["fields"]["T"][:, j0, i0] = 10.0 + 4.0 * gamma * zc
+
+    def structure(wl_):
+        m = oracle.RefModel(wl_)
+        m.step(1)
+        f = m.get_fields()
+        return [f[n] - (dz * f[n]).sum(axis=0) / dz.sum() for n in ("u", "v")]
+
+    (ua, va), (ub, vb) = structure(wl), structure(pert)
+    du, dv = np.abs(ub - ua).max(axis=0), np.abs(vb - va).max(axis=0)
+    moved_u = {(j0, i0), (j0, (i0 + 1) % du.shape[1])}
+    moved_v = {(j0, i0), ((j0 + 1) % dv.shape[0], i0)}
+    for j in range(du.shape[0]):
+        for i in range(du.shape[1]):
+            if (j, i) in moved_u:
+                assert du[j, i] > 1e-9, (j, i, du[j, i])
+            else:
+                assert du[j, i] < 1e-15, (j, i, du[j, i])
+            if (j, i) in moved_v:
+                assert dv[j, i] > 1e-9, (j, i, dv[j, i])
+            else:
+                assert dv[j, i] < 1e-15, (j, i, dv[j, i])
+
+
 def test_mixing_neutral_and_convective_limits():
     # neutral column: Ri = 0 whatever the shear -> nu_z + nu0, kappa_z + nu0
     mix = oracle.RefModel(_sheared_box(0.0, 4e-3)).mixing()

@@ -8,6 +8,8 @@ Not listed because they are EQUIVALENT mutants: dropping the open-face masks of 
 face has H = 0, G^U = 0 and starts from U = 0, so it stays 0 with or without the mask.)
 """
 import os
+
+import pytest
 import shutil
 import subprocess
 import sys
@@ -164,6 +166,67 @@ MUTANTS_OPTIONS = [
 ]
 
 
+# and for the time stepping itself: quasi-AB2, predictor, barotropic forcing and filter, correction, history
+PINS_STEP = ["tests/test_oracle_handcalc.py", "tests/test_oracle_physics.py", "tests/test_oracle_units.py",
+             "tests/test_oracle_variants.py", "tests/test_oracle_closure.py", "tests/test_oracle_forcing.py"]
+MUTANTS_STEP = [
+    ("S1 quasi-AB2: c0 = 3/2 - chi",
+     "const double c0 = M.have_history ? 1.5 + M.d.chi : 1.0;",
+     "const double c0 = M.have_history ? 1.5 - M.d.chi : 1.0;"),
+    ("S2 quasi-AB2: c1 without chi",
+     "const double c1 = M.have_history ? 0.5 + M.d.chi : 0.0;",
+     "const double c1 = M.have_history ? 0.5 : 0.0;"),
+    ("S3 Euler start with c0 = 3/2",
+     "const double c0 = M.have_history ? 1.5 + M.d.chi : 1.0;",
+     "const double c0 = M.have_history ? 1.5 + M.d.chi : 1.5;"),
+    ("S4 predictor from G^n instead of the AB2 combination",
+     "col[k] = ((*fld[f])(k, j, i) + dt * Gh) * m;",
+     "col[k] = ((*fld[f])(k, j, i) + dt * (*Gn[f])(k, j, i)) * m;"),
+    ("S5 barotropic forcing: sum of G without the layer thickness",
+     "su += g.dz[k] * g.mu(k, j, i) * Ghu(k, j, i);",
+     "su += g.mu(k, j, i) * Ghu(k, j, i);"),
+    ("S6 filter: transports averaged with the eta weights",
+     "Ub(0, j, i) += b * M.U(0, j, i);",
+     "Ub(0, j, i) += a * M.U(0, j, i);"),
+    ("S7 filter: eta averaged with the transport weights",
+     "etab(0, j, i) += a * M.eta(0, j, i);",
+     "etab(0, j, i) += b * M.eta(0, j, i);"),
+    ("S8 correction of u divided by Hv",
+     "const double cu = M.Hu(0, j, i) > 0.0 ? (M.U(0, j, i) - su) / M.Hu(0, j, i) : 0.0;",
+     "const double cu = M.Hu(0, j, i) > 0.0 ? (M.U(0, j, i) - su) / M.Hv(0, j, i) : 0.0;"),
+    ("S9 closure: nu at the u face from columns i, i + 1",
+     "dtk[k] = f == 0 ? dt * (0.5 * (M.nuc(k, j, i - 1) + M.nuc(k, j, i)))",
+     "dtk[k] = f == 0 ? dt * (0.5 * (M.nuc(k, j, i) + M.nuc(k, j, i + 1)))"),
+    ("S10 closure: nu at the v face from the column to the west",
+     ": f == 1 ? dt * (0.5 * (M.nuc(k, j - 1, i) + M.nuc(k, j, i)))",
+     ": f == 1 ? dt * (0.5 * (M.nuc(k, j, i - 1) + M.nuc(k, j, i)))"),
+    ("S11 closure: tracers diffused with nu",
+     ": dt * M.kapc(k, j, i);",
+     ": dt * M.nuc(k, j, i);"),
+    ("S12 history of S takes the tendency of T",
+     "M.GS1.a = M.GS.a;",
+     "M.GS1.a = M.GT.a;"),
+    ("S13 barotropic eta with the wrong sign",
+     "M.eta(0, j, i) -= dtau * (g.dy * (M.U(0, j, i + 1) - M.U(0, j, i))",
+     "M.eta(0, j, i) += dtau * (g.dy * (M.U(0, j, i + 1) - M.U(0, j, i))"),
+    ("S14 implicit solve of u: face open if the upper cell is",
+     "open[k] = f == 0 ? (g.mu(k, j, i) && g.mu(k - 1, j, i))",
+     "open[k] = f == 0 ? (g.mu(k, j, i))"),
+    ("S15 sub-step length from the zeroth instead of the first moment of the weights",
+     "for (int m = 1; m <= d->substeps; ++m) first += m * M->a_w[m - 1];",
+     "for (int m = 1; m <= d->substeps; ++m) first += M->a_w[m - 1];"),
+    ("S16 pressure: top half cell with the full thickness",
+     "M.p(nz - 1, j, i) = -buoyancy(M, nz - 1, j, i) * (g.zf[nz] - g.zc[nz - 1]);",
+     "M.p(nz - 1, j, i) = -buoyancy(M, nz - 1, j, i) * (g.zf[nz] - g.zf[nz - 1]);"),
+    ("S17 pressure: trapezoid with the spacing of the wrong face",
+     "- 0.5 * (buoyancy(M, k + 1, j, i) + buoyancy(M, k, j, i)) * g.dzc[k + 1];",
+     "- 0.5 * (buoyancy(M, k + 1, j, i) + buoyancy(M, k, j, i)) * g.dzc[k];"),
+    ("S18 vertical velocity integrated with the wrong sign",
+     "M.w(k + 1, j, i) = M.w(k, j, i) - g.dz[k] * D;",
+     "M.w(k + 1, j, i) = M.w(k, j, i) + g.dz[k] * D;"),
+]
+
+
 def _run_pins(src_path, pins=None):
     env = dict(os.environ, OCN_REF_MUTANT_SRC=src_path, OMP_NUM_THREADS="2")
     r = subprocess.run([sys.executable, "-m", "pytest", "-x", "-q", "-p", "no:cacheprovider"] + (pins or PINS), cwd=ROOT, env=env,
@@ -171,19 +234,21 @@ def _run_pins(src_path, pins=None):
     return r.returncode, r.stdout[-3000:]
 
 
-def test_every_mutant_of_the_options_is_caught():
+@pytest.mark.parametrize("group", ["options", "step"])
+def test_every_mutant_of_the_options_and_of_the_time_stepping_is_caught(group):
+    mutants, pins = (MUTANTS_OPTIONS, PINS_OPTIONS) if group == "options" else (MUTANTS_STEP, PINS_STEP)
     text = open(SRC).read()
     tmp = tempfile.mkdtemp(prefix="ocn_mut_")
     try:
         jobs = []
-        for n, (name, old, new) in enumerate(MUTANTS_OPTIONS):
+        for n, (name, old, new) in enumerate(mutants):
             assert text.count(old) == 1, "mutation target not found exactly once (oracle source changed?): " + name
             path = os.path.join(tmp, "option_%02d.cpp" % n)
             with open(path, "w") as f:
                 f.write(text.replace(old, new))
             jobs.append((name, path))
         with ThreadPoolExecutor(max_workers=max(2, (os.cpu_count() or 4) // 2)) as ex:
-            res = list(ex.map(lambda j: _run_pins(j[1], PINS_OPTIONS), jobs))
+            res = list(ex.map(lambda j: _run_pins(j[1], pins), jobs))
         survivors = [name for (name, _), (rc, _) in zip(jobs, res) if rc == 0]
         assert not survivors, "mutants that survive every pin: %s" % survivors
         for (name, _), (rc, out) in zip(jobs, res):
@@ -221,10 +286,10 @@ def test_every_mutant_of_the_latlon_metrics_and_masks_is_caught():
 if __name__ == "__main__":          # python tests/test_oracle_mutations.py: prints which pin catches which mutant
     text = open(SRC).read()
     tmp = tempfile.mkdtemp(prefix="ocn_mut_")
-    for n, (name, old, new) in enumerate(MUTANTS + MUTANTS_OPTIONS):
+    for n, (name, old, new) in enumerate(MUTANTS + MUTANTS_OPTIONS + MUTANTS_STEP):
         path = os.path.join(tmp, "m%02d.cpp" % n)
         open(path, "w").write(text.replace(old, new))
-        rc, out = _run_pins(path, PINS if n < len(MUTANTS) else PINS_OPTIONS)
+        rc, out = _run_pins(path, PINS if n < len(MUTANTS) else PINS_OPTIONS if n < len(MUTANTS) + len(MUTANTS_OPTIONS) else PINS_STEP)
         first = [ln for ln in out.splitlines() if ln.startswith("FAILED")]
         print("%-70s %s" % (name, first[0] if first else ("SURVIVES" if rc == 0 else "rc=%d" % rc)))
     shutil.rmtree(tmp, ignore_errors=True)

@@ -187,6 +187,22 @@ def test_transport_weights_closed_form_uniform_wind_on_a_flat_periodic_box():
         assert np.max(np.abs((f["u"] * dz[:, None, None]).sum(axis=0) - want)) < 1e-13 * want
 
 
+def test_user_filter_weights_set_the_sub_step_so_that_the_average_lands_on_the_new_time_level():
+    """The same box with the caller's own weights a_m for everything (filter_weights): the sub-step is dt / sum_m m a_m
+    (the weighted mean of the sub-step times is t^{n+1}), so the filtered transport of the uniformly forced
+    ocean is exactly dt G^U whatever the weights are — with dtau = dt / sum_m a_m it would be dt G^U times their first moment."""
+    M, dt, H = 12, 100.0, 400.0
+    wl = box(nx=8, ny=6, nz=4, depth=H, f0=0.0, dt=dt, substeps=M, nu_z=0.0)
+    wl["fields"]["tau_x"][:] = 0.2
+    want = dt * 0.2 / wl["params"]["rho0"]
+    for a in (_other_weights(M), np.eye(M)[M - 1], np.eye(M)[2]):       # spread out, all on the last sub-step, all on the third
+        assert abs(np.dot(np.arange(1, M + 1), a) - 1.0) > 0.5
+        m = oracle.RefModel(wl, filter_weights=a)
+        m.step(1)
+        U = m.diagnostics()["U"]
+        assert np.max(np.abs(U - want)) < 1e-13 * want, (a, U[0, 0], want)
+
+
 def test_transport_weights_leave_eta_filter_and_tracers_alone_but_change_the_flow():
     wl = W.config2(nx=48, ny=20, nz=10, steps=3)
     b = _other_weights(wl["params"]["substeps"])
