@@ -227,6 +227,64 @@ MUTANTS_STEP = [
 ]
 
 
+# signs, factors and stencil directions of the tendencies that are not metric rows (those are in MUTANTS)
+PINS_TERMS = ["tests/test_oracle_handcalc.py", "tests/test_oracle_latlon.py", "tests/test_oracle_physics.py",
+              "tests/test_oracle_units.py", "tests/test_oracle_forcing.py"]
+MUTANTS_TERMS = [
+    ("G1 u: vorticity flux with the wrong sign",
+     "Gu(k, j, i) = m * (zt * vhat + Cu - dK - dP - Au + Vu + tau - drag);",
+     "Gu(k, j, i) = m * (-zt * vhat + Cu - dK - dP - Au + Vu + tau - drag);"),
+    ("G2 v: Coriolis with the wrong sign",
+     "Gv(k, j, i) = m * (-zt * uhat - Cv - dK - dP - Av + Vv + tau - drag);",
+     "Gv(k, j, i) = m * (-zt * uhat + Cv - dK - dP - Av + Vv + tau - drag);"),
+    ("G3 u: viscous term with the wrong sign",
+     "Gu(k, j, i) = m * (zt * vhat + Cu - dK - dP - Au + Vu + tau - drag);",
+     "Gu(k, j, i) = m * (zt * vhat + Cu - dK - dP - Au - Vu + tau - drag);"),
+    ("G4 v: vertical advection with the wrong sign",
+     "Gv(k, j, i) = m * (-zt * uhat - Cv - dK - dP - Av + Vv + tau - drag);",
+     "Gv(k, j, i) = m * (-zt * uhat - Cv - dK - dP + Av + Vv + tau - drag);"),
+    ("G5 u: vorticity upwinded against the flow",
+     "const double zt = weno(zs, g.order_zeta_u(k, j, i), vhat, M.d.advection);",
+     "const double zt = weno(zs, g.order_zeta_u(k, j, i), -vhat, M.d.advection);"),
+    ("G6 v: vorticity stencil shifted by one column",
+     "const double zs[6] = {zeta(k, j, i - 2), zeta(k, j, i - 1), zeta(k, j, i),\n                                          zeta(k, j, i + 1), zeta(k, j, i + 2), zeta(k, j, i + 3)};",
+     "const double zs[6] = {zeta(k, j, i - 3), zeta(k, j, i - 2), zeta(k, j, i - 1),\n                                          zeta(k, j, i), zeta(k, j, i + 1), zeta(k, j, i + 2)};"),
+    ("G7 u: viscous vorticity term with the wrong sign inside V_u",
+     "- (zeta(k, j + 1, i) - zeta(k, j, i)) / g.dy);\n                    const double tau = (k == nz - 1) ? M.taux",
+     "+ (zeta(k, j + 1, i) - zeta(k, j, i)) / g.dy);\n                    const double tau = (k == nz - 1) ? M.taux"),
+    ("G8 wind stress without the reference density",
+     "const double tau = (k == nz - 1) ? M.taux(0, j, i) / (M.d.rho0 * g.dz[k]) : 0.0;",
+     "const double tau = (k == nz - 1) ? M.taux(0, j, i) / (g.dz[k]) : 0.0;"),
+    ("G9 u: upper half of the vertical advection uses the lower velocity difference",
+     "const double Au = 0.5 * (Whi * dhi + Wlo * dlo) / (g.AzC(j) * g.dz[k]);",
+     "const double Au = 0.5 * (Whi * dlo + Wlo * dlo) / (g.AzC(j) * g.dz[k]);"),
+    ("G10 uhat from three of its four neighbours twice",
+     "const double uhat = 0.25 * (u(k, j - 1, i) + u(k, j, i) + u(k, j - 1, i + 1) + u(k, j, i + 1));",
+     "const double uhat = 0.25 * (u(k, j - 1, i) + u(k, j, i) + u(k, j, i + 1) + u(k, j, i + 1));"),
+    ("R1 tracers: zonal flux upwinded against the flow",
+     "const double cf = weno(cs, g.order_x(k, j, i), uu, M.d.advection);",
+     "const double cf = weno(cs, g.order_x(k, j, i), -uu, M.d.advection);"),
+    ("R2 tracers: horizontal diffusion with the wrong sign",
+     "- kh * g.dxF(j) * g.dz[k] * (c(k, j, i) - c(k, j - 1, i)) / g.dy * g.mv(k, j, i);",
+     "+ kh * g.dxF(j) * g.dz[k] * (c(k, j, i) - c(k, j - 1, i)) / g.dy * g.mv(k, j, i);"),
+    ("R3 tracers: vertical stencil shifted by one level",
+     "const int kk = k - 3 + m;",
+     "const int kk = k - 2 + m;"),
+    ("R4 tracers: divergence without the vertical flux below",
+     "+ Fz(k + 1, j, i) - Fz(k, j, i);",
+     "+ Fz(k + 1, j, i);"),
+    ("R5 surface flux spread over the wrong thickness",
+     "(surf(0, j, i) + gamma * (target(0, j, i) - c(k, j, i))) / g.dz[k];",
+     "(surf(0, j, i) + gamma * (target(0, j, i) - c(k, j, i))) / g.dz[0];"),
+    ("K1 divergence: zonal difference taken one cell to the west",
+     "Dv(k, j, i) = (g.dy * (u(k, j, i + 1) - u(k, j, i))",
+     "Dv(k, j, i) = (g.dy * (u(k, j, i) - u(k, j, i - 1))"),
+    ("K2 kinetic energy without the meridional half",
+     "+ 0.25 * (v(k, j, i) * v(k, j, i) + v(k, j + 1, i) * v(k, j + 1, i));",
+     "+ 0.25 * (v(k, j, i) * v(k, j, i) + v(k, j, i) * v(k, j, i));"),
+]
+
+
 def _run_pins(src_path, pins=None):
     env = dict(os.environ, OCN_REF_MUTANT_SRC=src_path, OMP_NUM_THREADS="2")
     r = subprocess.run([sys.executable, "-m", "pytest", "-x", "-q", "-p", "no:cacheprovider"] + (pins or PINS), cwd=ROOT, env=env,
@@ -234,9 +292,9 @@ def _run_pins(src_path, pins=None):
     return r.returncode, r.stdout[-3000:]
 
 
-@pytest.mark.parametrize("group", ["options", "step"])
+@pytest.mark.parametrize("group", ["options", "step", "terms"])
 def test_every_mutant_of_the_options_and_of_the_time_stepping_is_caught(group):
-    mutants, pins = (MUTANTS_OPTIONS, PINS_OPTIONS) if group == "options" else (MUTANTS_STEP, PINS_STEP)
+    mutants, pins = {"options": (MUTANTS_OPTIONS, PINS_OPTIONS), "step": (MUTANTS_STEP, PINS_STEP), "terms": (MUTANTS_TERMS, PINS_TERMS)}[group]
     text = open(SRC).read()
     tmp = tempfile.mkdtemp(prefix="ocn_mut_")
     try:
