@@ -285,6 +285,51 @@ MUTANTS_TERMS = [
 ]
 
 
+# the reconstruction itself, the default filter and the initial transports
+PINS_WENO = ["tests/test_oracle_units.py", "tests/test_oracle_variants.py", "tests/test_oracle_handcalc.py", "tests/test_oracle_physics.py"]
+MUTANTS_WENO = [
+    ("W1 WENO5: first candidate with -5 instead of -7",
+     "const double p0 = (2.0 * qm2 - 7.0 * qm1 + 11.0 * q0) / 6.0;",
+     "const double p0 = (2.0 * qm2 - 5.0 * qm1 + 11.0 * q0) / 6.0;"),
+    ("W2 WENO5: smoothness indicator with 13/10",
+     "const double b1 = 13.0 / 12.0 * (qm1 - 2.0 * q0 + q1) * (qm1 - 2.0 * q0 + q1)",
+     "const double b1 = 13.0 / 10.0 * (qm1 - 2.0 * q0 + q1) * (qm1 - 2.0 * q0 + q1)"),
+    ("W3 WENO5: first-difference part of beta_2 with the wrong stencil",
+     "+ 0.25 * (3.0 * q0 - 4.0 * q1 + q2) * (3.0 * q0 - 4.0 * q1 + q2);",
+     "+ 0.25 * (q0 - 4.0 * q1 + 3.0 * q2) * (q0 - 4.0 * q1 + 3.0 * q2);"),
+    ("W4 WENO5: linear weights 0.1 and 0.3 swapped",
+     "const double a0 = 0.1 / ((eps + b0) * (eps + b0));",
+     "const double a0 = 0.3 / ((eps + b0) * (eps + b0));"),
+    ("W5 WENO5: weights with the first power of the indicator",
+     "const double a1 = 0.6 / ((eps + b1) * (eps + b1));",
+     "const double a1 = 0.6 / ((eps + b1));"),
+    ("W6 WENO3: linear weights 1/3 and 2/3 swapped",
+     "const double a1 = (2.0 / 3.0) / ((eps + b1) * (eps + b1));",
+     "const double a1 = (1.0 / 3.0) / ((eps + b1) * (eps + b1));"),
+    ("W7 WENO3: extrapolating candidate with 2 instead of 3",
+     "const double p0 = (-qm1 + 3.0 * q0) / 2.0;",
+     "const double p0 = (-qm1 + 2.0 * q0) / 2.0;"),
+    ("W8 downwind stencil not mirrored",
+     "else           { qm2 = c[5]; qm1 = c[4]; q0 = c[3]; q1 = c[2]; q2 = c[1]; }",
+     "else           { qm2 = c[5]; qm1 = c[4]; q0 = c[3]; q1 = c[2]; q2 = c[0]; }"),
+    ("W9 WENO-Z: tau from beta_0 and beta_1",
+     "const double tau = std::fabs(b0 - b2);",
+     "const double tau = std::fabs(b0 - b1);"),
+    ("W10 eps of the weights",
+     "const double eps = 1e-6;",
+     "const double eps = 1e-2;"),
+    ("P1 default filter: exponent q = 2",
+     "a[m - 1] = s * s * (1.0 - s * s * s * s);",
+     "a[m - 1] = s * s * (1.0 - s * s);"),
+    ("P2 default filter: s = m / M",
+     "const double s = (double)m / (double)(M + 1);",
+     "const double s = (double)m / (double)(M);"),
+    ("I1 initial transports without the layer thickness",
+     "su += g.dz[k] * M->u(k, j, i); sv += g.dz[k] * M->v(k, j, i);",
+     "su += M->u(k, j, i); sv += g.dz[k] * M->v(k, j, i);"),
+]
+
+
 def _run_pins(src_path, pins=None):
     env = dict(os.environ, OCN_REF_MUTANT_SRC=src_path, OMP_NUM_THREADS="2")
     r = subprocess.run([sys.executable, "-m", "pytest", "-x", "-q", "-p", "no:cacheprovider"] + (pins or PINS), cwd=ROOT, env=env,
@@ -292,9 +337,10 @@ def _run_pins(src_path, pins=None):
     return r.returncode, r.stdout[-3000:]
 
 
-@pytest.mark.parametrize("group", ["options", "step", "terms"])
+@pytest.mark.parametrize("group", ["options", "step", "terms", "weno"])
 def test_every_mutant_of_the_options_and_of_the_time_stepping_is_caught(group):
-    mutants, pins = {"options": (MUTANTS_OPTIONS, PINS_OPTIONS), "step": (MUTANTS_STEP, PINS_STEP), "terms": (MUTANTS_TERMS, PINS_TERMS)}[group]
+    mutants, pins = {"options": (MUTANTS_OPTIONS, PINS_OPTIONS), "step": (MUTANTS_STEP, PINS_STEP), "terms": (MUTANTS_TERMS, PINS_TERMS),
+                     "weno": (MUTANTS_WENO, PINS_WENO)}[group]
     text = open(SRC).read()
     tmp = tempfile.mkdtemp(prefix="ocn_mut_")
     try:
