@@ -321,3 +321,21 @@ def test_forcing_that_changes_between_steps_reaches_every_band():
     with pytest.raises(ValueError, match="set_forcing takes"):
         B.set_forcing(u=wl["fields"]["u"])
     whole.close(); B.close()
+
+
+def test_the_overlap_is_the_smallest_that_keeps_the_bits_in_fp64():
+    """ocn_band_overlap is the reach of one part + 1: with one row less the error of the band's artificial wall arrives on own
+    rows within a launch of the sub-cycle (1e-16 relative after six sub-steps, but not the same bits).  (In fp32 the same
+    intrusion falls below the rounding of the fields for a few rows more; the overlap there is the bound, not the observation.)"""
+    wl = _workload(64, "")
+    whole = ocn.Model(wl)
+    whole.time_step(6)
+    fw = whole.get_fields()
+    whole.close()
+    h = ocn.band_overlap(64, wl["params"]["substeps"])
+    B = bands.Bands(wl, 3, h=h - 1)
+    B.time_step(6)
+    fb = B.get_fields()
+    B.close()
+    assert not np.array_equal(fw["eta"], fb["eta"])
+    assert np.abs(fw["eta"] - fb["eta"]).max() < 1e-12
