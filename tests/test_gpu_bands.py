@@ -339,3 +339,22 @@ def test_the_overlap_is_the_smallest_that_keeps_the_bits_in_fp64():
     B.close()
     assert not np.array_equal(fw["eta"], fb["eta"])
     assert np.abs(fw["eta"] - fb["eta"]).max() < 1e-12
+
+
+@pytest.mark.parametrize("nb,fused", [(2, False), (8, True)])
+def test_bands_at_the_full_size_of_config_4_are_bit_identical(nb, fused):
+    """The grid bench.py times (2880 x 1200 x 100, fp32, M = 40), cut into 2 bands with packed-row exchange and into 8 bands with
+    fused puts: the same bits as one model after an Euler step and three quasi-AB2 steps."""
+    wl = W.make(4)
+    names = ("u", "v", "T", "eta")
+    whole = ocn.Model(wl)
+    whole.time_step(4)
+    fw = whole.get_fields(names)
+    whole.close()
+    B = bands.Bands(wl, nb, fused_put=fused)
+    B.time_step(4)
+    fb = B.get_fields(names)
+    B.close()
+    for k in names:
+        assert np.array_equal(fw[k], fb[k]), (nb, fused, k)
+    assert float(np.abs(fw["u"]).max()) > 1e-3
