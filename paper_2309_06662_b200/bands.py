@@ -204,9 +204,11 @@ class Bands:
 class DistBand:
     """This rank's band of the whole grid; the neighbours are ranks rank - 1 (south) and rank + 1 (north).
 
-    The band's model works on the stream that is current when it is built (`stream` = its handle), so that the packs,
-    torch.distributed's point-to-point calls and the unpacks are ordered by torch's stream semantics with no host
-    synchronisation.  model_factory / alloc as in Bands; alloc returns (tensor, pointer) and the TENSOR is what is sent.
+    The band's model and torch.distributed's point-to-point calls work on ONE stream, so that the packs, the sends / receives and
+    the unpacks are ordered by torch's stream semantics with no host synchronisation: by default a torch stream this object
+    creates and makes current around every exchange (torch's legacy default stream has handle 0, which the library would take
+    for "give me a private stream"); with `stream` = the handle of a stream of the caller's, that stream must be torch's current
+    stream whenever time_step is called.  model_factory / alloc as in Bands; alloc returns (tensor, pointer) and the TENSOR is what is sent.
     host_staging=True: the packed rows travel through pinned host tensors (device -> host, send / recv, host -> device) for
     process groups that cannot send device memory (gloo: the 2-process test on one GPU); the default sends device tensors."""
 
@@ -219,13 +221,15 @@ class DistBand:
         self.own, self.ext, self.transfers = exchange_plan(self.ny, self.world, self.h)
         if model_factory is None:
             import torch
-            handle = torch.cuda.current_stream(device).cuda_stream if stream is None else stream
+            self._tstream = torch.cuda.Stream(device=device) if stream is None else None
+            handle = self._tstream.cuda_stream if stream is None else stream
             model_factory = lambda w, s: ocn.Model(w, device=device, stream=s)
             if alloc is None:
                 def alloc(nbytes):
                     t = torch.empty(int(nbytes), dtype=torch.uint8, device="cuda:%d" % device)
                     return t, t.data_ptr()
         else:
+            self._tstream = None
             handle = stream
         self.model = model_factory(band_workload(wl, self.ext[self.rank]), handle)
         self.parts = self.model.step_parts()
@@ -256,6 +260,13 @@ class DistBand:
 
     def exchange(self, group):
         """Sends this band's own edge rows to the neighbours and fills its overlap rows from theirs."""
+        if self._tstream is not None:
+            import torch
+            with torch.cuda.stream(self._tstream):
+                return self._exchange(group)
+        return self._exchange(group)
+
+    def _exchange(self, group):
         dist = self.dist
         ops, recvs = [], []
         for n, t in enumerate(self.transfers):

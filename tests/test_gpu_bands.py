@@ -267,11 +267,9 @@ def _rank_worker_put(rank, world, port, prec, kind, steps, out):
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
         torch.cuda.set_device(0)
-        s = torch.cuda.Stream()
-        with torch.cuda.stream(s):
-            D = bands.DistBand(_workload(prec, kind), dist, device=0, stream=s.cuda_stream, host_staging=True, fused_put=True)
-            D.time_step(steps)
-            f = D.own_fields(FIELDS)
+        D = bands.DistBand(_workload(prec, kind), dist, device=0, host_staging=True, fused_put=True)   # on a stream of its own
+        D.time_step(steps)
+        f = D.own_fields(FIELDS)
         out.put((rank, D.own[rank], {k: np.array(v) for k, v in f.items()}))
         dist.barrier()
         D.close()
