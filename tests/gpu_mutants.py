@@ -17,7 +17,7 @@ from concurrent.futures import ThreadPoolExecutor
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 CSRC = os.path.join(ROOT, "paper_2309_06662_b200", "csrc")
 SO = os.path.join(ROOT, "paper_2309_06662_b200", "libocn.so")
-TESTS = ["tests/test_gpu_parity.py", "tests/test_gpu_closure.py", "tests/test_gpu_variants.py"]
+TESTS = ["tests/test_gpu_parity.py", "tests/test_gpu_closure.py", "tests/test_gpu_variants.py", "tests/test_gpu_forcing.py"]
 
 # (name, file in csrc, exact text (once), replacement)
 MUTANTS = [
@@ -45,6 +45,19 @@ MUTANTS = [
      "const float g2 = R.nu0 * f;\n    return make_float2(R.nuz + g2 + conv, R.kapz + g2 * f + conv);"),
     ("weno5_pair_linear_weight", "common.cuh",
      "a1 = mul2(mul2(f2(0.6f), b02), b02);", "a1 = mul2(mul2(f2(0.5f), b02), b02);"),
+    ("strip_transport_filter_weight", "kernels_column.cuh",
+     "for (int r = 0; r < 4; ++r) { be[r] += am * e[r]; bU[r] += bm * u[r]; bV[r] += bm * v[r]; }",
+     "for (int r = 0; r < 4; ++r) { be[r] += am * e[r]; bU[r] += am * u[r]; bV[r] += bm * v[r]; }"),
+    ("k1_restoring_sign", "kernels_tile.cuh",
+     "X(P.gamma_T) * (X(rtg.x) - X(tsc.x))", "X(P.gamma_T) * (X(tsc.x) - X(rtg.x))"),
+    ("k1_drag_speed_u", "kernels_tile.cuh",
+     "X(P.drag_cd) * X((T)sqrt((X(u_c) * X(u_c) + X(vhat) * X(vhat)).v))) * X(u_c), dzk, rdzk)",
+     "X(P.drag_cd) * X((T)sqrt((X(u_c) * X(u_c)).v))) * X(u_c), dzk, rdzk)"),
+    ("eos_cabbeling_power", "kernels_column.cuh",
+     "E::add(E::mul(P.ath_d[k], dT), E::mul(E::mul(P.ha2_d, dT), dT))", "E::add(E::mul(P.ath_d[k], dT), E::mul(P.ha2_d, dT))"),
+    ("biharmonic_divergence_row", "kernels_biharmonic.cuh",
+     "const Xv<T> Ds = xdiv(X(dy) * (X(vse.x) - X(vs.x)) + X(dxFj) * X(v00.y) - X(dxFs) * X(vs.y), AzCs, rAzCs);",
+     "const Xv<T> Ds = xdiv(X(dy) * (X(vse.x) - X(vs.x)) + X(dxFj) * X(v00.y) - X(dxFs) * X(vs.y), AzCj, rAzCj);"),
 ]
 
 
@@ -99,7 +112,10 @@ if __name__ == "__main__":
     ap = argparse.ArgumentParser()
     ap.add_argument("--build")
     ap.add_argument("--run")
+    ap.add_argument("--only", default="", help="comma-separated mutant names (default: all)")
     a = ap.parse_args()
+    if a.only:
+        MUTANTS[:] = [m for m in MUTANTS if m[0] in a.only.split(",")]
     if a.build:
         build(a.build)
     if a.run:
